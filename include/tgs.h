@@ -1,0 +1,142 @@
+/* include/tgs.h -- C-ABI boundary of the B200-native TemporalGS hot path (libtgs.so).
+ *
+ * Method: TemporalGS, arxiv/paper_2607_03390.  Citations are PAPER.md:L<line>; "R<n>" are the
+ * readings of silent / ambiguous passages listed in DESIGN.md §2.  Every step of the path runs in
+ * hand-written CUDA kernels for sm_100a (paper_2607_03390_b200/csrc); there is no CPU fallback --
+ * a call fails with TGS_E_CUDA when no device is usable.
+ *
+ * General rules
+ *  - Every function returns 0 (TGS_OK) on success or a negative tgs_status; no exceptions cross.
+ *  - A context is bound to one CUDA device and one stream; it is not thread-safe.
+ *  - `mem` says where a caller buffer lives: TGS_HOST or TGS_DEVICE (same device as the context).
+ *    Input buffers are copied during the call; the caller keeps ownership of everything it passes.
+ *  - tgs_render only enqueues work; tgs_read_* / tgs_get_stats / tgs_debug_get with TGS_HOST block until
+ *    the data is on the host.  With TGS_DEVICE they enqueue a device copy on the context's stream.
+ *  - Conventions (R6): `view` is a rigid world->camera matrix, row-major 4x4, camera looks along +z,
+ *    x right, y down; pixel (i,j) is sampled at (u,v)=(i,j); 16x16 tiles, tile id =
+ *    ty*TX+tx.  Depth of a pixel without geometry is TGS_DEPTH_INVALID ("z_far + eps", L97, R12).
+ */
+#ifndef TGS_H
+#define TGS_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TGS_DEPTH_INVALID 3.0e38f
+
+typedef enum { TGS_HOST = 0, TGS_DEVICE = 1 } tgs_mem;
+
+/* render modes (argument of tgs_render) */
+typedef enum {
+  TGS_FULL = 0,       /* reference frame R: vanilla 3DGS + construction of the priors (L65, L73-84, L103, L109) */
+  TGS_PSEUDO_REF = 1, /* pseudo reference frame P: reference frame with AFC (L128) */
+  TGS_TEMPORAL = 2,   /* TemporalGS frame S: AFC + TOC + selective rendering (L105-128) */
+  TGS_AUTO = 3        /* scheduler A0 decides: lambda_TDC, lambda_SR, eta (L67, L107, L128, L142) */
+} tgs_mode;
+
+/* frame types (tgs_stats.frame_type) */
+enum { TGS_FRAME_R = 0, TGS_FRAME_P = 1, TGS_FRAME_S = 2 };
+
+typedef enum {
+  TGS_OK = 0,
+  TGS_E_INVALID_ARG = -1, /* null pointer, bad size, non-finite input, unknown name */
+  TGS_E_NO_SCENE = -2,    /* tgs_render before tgs_load_gaussians */
+  TGS_E_NO_CAMERA = -3,   /* tgs_render before tgs_set_camera */
+  TGS_E_NO_PRIORS = -4,   /* TGS_TEMPORAL / TGS_PSEUDO_REF without valid priors */
+  TGS_E_CAPACITY = -5,    /* the (Gaussian, tile) pair buffer overflowed; the frame is invalid */
+  TGS_E_CUDA = -6         /* CUDA runtime error; see tgs_last_error */
+} tgs_status;
+
+/* per-Gaussian flags in the "rec_flags" debug buffer */
+enum {
+  TGS_CULL_NEAR = 1,       /* d <= z_near (L61, R4) */
+  TGS_CULL_AFC = 2,        /* outside the adaptive frustum (L109-111) */
+  TGS_CULL_TOC = 4,        /* behind the warped TGB (L113) */
+  TGS_CULL_DEGENERATE = 8, /* det(Sigma') <= 0 */
+  TGS_CULL_EMPTY = 16,     /* intersects no tile (L61) */
+  TGS_VISIBLE = 32,
+  TGS_NEWLY_VISIBLE = 64   /* L119 */
+};
+
+typedef struct {
+  float lambda1, lambda2; /* surface range [D - l1 s, D + l2 s]; 3, 0 (L99) */
+  int lambda_tdc;         /* a reference frame every lambda_tdc frames; 50 (L142) */
+  int lambda_sr;          /* a (pseudo) reference frame every lambda_sr frames; 5 (L142) */
+  float eta;              /* S frame with more than eta*T selected tiles forces a P frame next; 0.40 (L128) */
+  float bg[3];            /* background colour, part of the TAB (R27); 0 */
+  int enable_afc, enable_toc, enable_sr; /* module toggles of Table IV (L221-231); 1 */
+  uint32_t max_pairs;     /* capacity of the (Gaussian, tile) pair buffers; 0 = automatic */
+} tgs_params;
+
+typedef struct {
+  int frame_type; /* TGS_FRAME_R / P / S */
+  uint32_t n_total, n_near, n_afc, n_toc, n_degenerate, n_empty, n_visible, n_newly_visible;
+  uint64_t n_pairs; /* P: sort length */
+  uint32_t n_tiles, n_sel_oc, n_sel_um, n_sel;
+  uint32_t n_rendered; /* |G_rendered| (R / P frames) */
+  uint32_t overflow;   /* 1: n_pairs exceeded the capacity, frame invalid */
+  float ms_stage[8];   /* per-stage device time when timing is on (tgs_debug_run_stage("timing_on")):
+                          0 warp, 1 fill+corr, 2 preprocess, 3 select+count+scan+keys, 4 sort, 5 ranges,
+                          6 blend+stitch, 7 post (F reduction, stats) */
+  float ms_total;
+  uint64_t device_bytes; /* device memory held by the context */
+} tgs_stats;
+
+typedef struct tgs_ctx tgs_ctx;
+
+/* Create a context on `cuda_device`; all work is enqueued on `cuda_stream` (a cudaStream_t; NULL = the
+ * legacy default stream).  *out is owned by the caller until tgs_destroy. */
+int tgs_create(tgs_ctx** out, int cuda_device, void* cuda_stream);
+void tgs_destroy(tgs_ctx*);
+
+/* Load the scene (mean, covariance = R S S^T R^T, opacity, SH).  means [n][3]; scales
+ * [n][3] linear (post-exp); quats [n][4] (w,x,y,z), normalised here; opacity [n] post-sigmoid; sh
+ * [n][K][3], K=(sh_degree+1)^2, sh_degree 0..3.  Data are copied and repacked on the device (cull
+ * record {mean, opacity}, 3-D covariance, tau = 2 ln(255 o)); invalidates the priors.  Host inputs with
+ * a non-finite value are rejected (TGS_E_INVALID_ARG). */
+int tgs_load_gaussians(tgs_ctx*, uint32_t n, int sh_degree, const float* means, const float* scales,
+                       const float* quats, const float* opacity, const float* sh, int mem);
+
+/* Camera of the NEXT frame (W, K).  Changing W, H or the intrinsics invalidates the priors. */
+int tgs_set_camera(tgs_ctx*, const float view[16], float fx, float fy, float cx, float cy, int W, int H,
+                   float znear, float zfar);
+
+void tgs_default_params(tgs_params*);
+int tgs_set_params(tgs_ctx*, const tgs_params*);
+
+/* Render one frame of the stream.  Enqueues the whole path A1-A10 of DESIGN.md §1. */
+int tgs_render(tgs_ctx*, int mode);
+
+/* Current frame.  rgb [H][W][3] in [0,1] (+bg); depth [H][W] (Eq.1; stitched on S frames, R31);
+ * sigma [H][W] (Eq.2), nullable; sel [TY][TX]: bit0 = T^oc (L119), bit1 = T^um (L121), bit2 = selected. */
+int tgs_read_image(tgs_ctx*, float* rgb, int mem);
+int tgs_read_depth(tgs_ctx*, float* depth, float* sigma, int mem);
+int tgs_read_tile_mask(tgs_ctx*, uint8_t* sel, int mem);
+int tgs_get_stats(tgs_ctx*, tgs_stats* out);
+
+/* Drop the temporal priors: the next TGS_AUTO frame is a reference frame. */
+int tgs_reset_priors(tgs_ctx*);
+
+const char* tgs_strerror(int code);
+const char* tgs_last_error(tgs_ctx*);
+
+/* ---- test-only: named intermediate buffers, so that a stage can be fed the oracle's inputs ----
+ * tgs_debug_get copies min(bytes, size) bytes and returns the buffer's size in bytes (>= 0) or an error.
+ * Readable: rec_uvdo rec_conic (float4 [N]) rec_rect (uint16x4 [N]) rec_flags (uint32 [N]) rec_rgb
+ *   (float4 [N]) tiles_touched (uint32 [N]) keys (uint64 [P]) vals (uint32 [P]) ranges (uint32 [T][2])
+ *   warp_depth warp_sigma fill_depth (float [H][W]) rendered (uint8 [N]) F (float[4]) prior_depth
+ *   prior_sigma (float [H][W]) prior_image (float [H][W][3]) cov3d (float [N][6]) tau (float [N]).
+ * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):
+ *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
+ * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off". */
+long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int mem);
+int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);
+int tgs_debug_run_stage(tgs_ctx*, const char* stage);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TGS_H */

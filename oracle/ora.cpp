@@ -29,8 +29,13 @@ constexpr int TILE = 16;                       // 16x16 tiles
 constexpr double ALPHA_MIN = 1.0 / 255.0;      // PAPER.md:L119 (and R2)
 constexpr double ALPHA_MAX = 0.99;             // R2
 constexpr double T_STOP = 1.0e-4;              // R2
-constexpr double MARGIN_ALPHA = 1.0e-4;        // relative margins of "borderline" decisions (R29)
+// Relative margins of "borderline" decisions (R29).  The wide pair bounds which Gaussians an fp32
+// implementation MAY mark as rendered; the tight pair marks the pixels where an fp32 implementation
+// (alpha accurate to ~1e-6, T to ~1e-5 relative) may legitimately take the other branch.
+constexpr double MARGIN_ALPHA = 1.0e-4;
 constexpr double MARGIN_T = 1.0e-2;
+constexpr double PIX_MARGIN_ALPHA = 2.0e-5;
+constexpr double PIX_MARGIN_T = 1.0e-3;
 
 struct Cam {
   float V[16];
@@ -433,18 +438,21 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
               continue;
             }
             if (alpha < ALPHA_MIN) {                                 // skip alpha < 1/255 (R2)
-              if (alpha >= ALPHA_MIN * (1.0 - MARGIN_ALPHA)) { c->borderline[pix] = 1; c->rendered_maybe[g] = 1; }
+              if (alpha >= ALPHA_MIN * (1.0 - MARGIN_ALPHA)) c->rendered_maybe[g] = 1;
+              if (alpha >= ALPHA_MIN * (1.0 - PIX_MARGIN_ALPHA)) c->borderline[pix] = 1;
               continue;
             }
             const double Tn = T * (1.0 - alpha);
             if (Tn < T_STOP) {                                       // stop; this record is not blended (R2)
               if (Tn < T_STOP * (1.0 - MARGIN_T)) break;
-              c->borderline[pix] = 1; c->rendered_maybe[g] = 1; stopped = true; Tv = Tn;
+              if (Tn >= T_STOP * (1.0 - PIX_MARGIN_T)) c->borderline[pix] = 1;
+              c->rendered_maybe[g] = 1; stopped = true; Tv = Tn;
               continue;
             }
             const bool a_border = alpha < ALPHA_MIN * (1.0 + MARGIN_ALPHA);
-            if (a_border) c->borderline[pix] = 1;
-            if (Tn < T_STOP * (1.0 + MARGIN_T)) { c->borderline[pix] = 1; sure_alive = false; }
+            if (alpha < ALPHA_MIN * (1.0 + PIX_MARGIN_ALPHA)) c->borderline[pix] = 1;
+            if (Tn < T_STOP * (1.0 + PIX_MARGIN_T)) c->borderline[pix] = 1;
+            if (Tn < T_STOP * (1.0 + MARGIN_T)) sure_alive = false;
             const double w = alpha * T;                              // w_i = alpha_i T_i (R1)
             C[0] += w * r.r; C[1] += w * r.g; C[2] += w * r.b;
             Sw += w; Sd += w * (double)r.d; Sdd += w * (double)r.d * (double)r.d;   // Eq.1-2 sums

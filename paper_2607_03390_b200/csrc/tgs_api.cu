@@ -1,0 +1,544 @@
+// tgs_api.cu -- C-ABI of libtgs.so (include/tgs.h): context, host-side frame scheduler A0, buffer
+// management, the per-frame launch sequence A1-A10 and the read-back / debug calls.
+// No CPU fallback: every step of the path is a kernel launch; the host only computes the relative pose
+// (12 floats) and the frame type.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "tgs_internal.cuh"
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      snprintf(c->err, sizeof(c->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+      return TGS_E_CUDA;                                                                           \
+    }                                                                                              \
+  } while (0)
+
+struct Sched { int since_R = 0, since_ref = 0, force_P = 0; };
+
+struct tgs_ctx {
+  int device = 0;
+  int num_sms = 148;
+  cudaStream_t stream = nullptr;
+  char err[512] = {0};
+  // scene
+  uint32_t n = 0; int deg = 0, K = 1;
+  // camera
+  bool cam_set = false;
+  float view[16]; float fx, fy, cx, cy, znear, zfar; int W = 0, H = 0, TX = 0, TY = 0;
+  tgs_params prm;
+  // priors
+  bool priors_valid = false, F_valid = false;
+  float prior_view[16];
+  int prior_idx = 0;           // image/depth/sigma[prior_idx] hold TAB / TGB
+  int cur_idx = 0;             // buffers of the last rendered frame
+  int sorted_idx = 0;          // keys/vals[sorted_idx] hold the sorted pairs of the last frame
+  bool have_frame = false;
+  bool put_depth = false, put_sigma = false, put_image = false;
+  Sched sched;
+  int force_all = 0;
+  // capacities
+  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint64_t device_bytes = 0;
+  DevBuffers b;
+  std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
+  // stats
+  Counters* h_counters = nullptr;      // pinned
+  uint32_t* h_sel = nullptr;           // pinned: n_sel of the last S frame (for the eta rule)
+  cudaEvent_t ev_sel = nullptr, ev_done = nullptr;
+  bool sel_pending = false;
+  int last_ftype = -1; uint32_t last_n_tiles = 0;
+  bool timing = false;
+  cudaEvent_t ev_stage[10];
+  FrameConst fc;
+};
+
+namespace {
+
+template <typename T>
+int dev_alloc(tgs_ctx* c, T** p, size_t count, std::vector<void*>& list) {
+  *p = nullptr;
+  if (!count) count = 1;
+  CK(cudaMalloc((void**)p, count * sizeof(T)));
+  list.push_back(*p);
+  c->device_bytes += count * sizeof(T);
+  return TGS_OK;
+}
+
+void free_list(tgs_ctx* c, std::vector<void*>& list) {
+  for (void* p : list) cudaFree(p);
+  list.clear();
+  (void)c;
+}
+
+bool finite_all(const float* p, size_t n) {
+  for (size_t i = 0; i < n; ++i) if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+// rigid relative pose M = W_b W_a^{-1}, double arithmetic, rounded once to float (Eq.3)
+void relative_pose(const float* Wa, const float* Wb, float* M) {
+  double Ra[9], ta[3], Rb[9], tb[3];
+  for (int i = 0; i < 3; ++i) {
+    for (int j = 0; j < 3; ++j) { Ra[i * 3 + j] = Wa[i * 4 + j]; Rb[i * 3 + j] = Wb[i * 4 + j]; }
+    ta[i] = Wa[i * 4 + 3]; tb[i] = Wb[i * 4 + 3];
+  }
+  for (int i = 0; i < 3; ++i) {
+    double row[3];
+    for (int j = 0; j < 3; ++j) row[j] = (Rb[i * 3] * Ra[j * 3] + Rb[i * 3 + 1] * Ra[j * 3 + 1]) + Rb[i * 3 + 2] * Ra[j * 3 + 2];
+    const double mt = tb[i] - ((row[0] * ta[0] + row[1] * ta[1]) + row[2] * ta[2]);
+    M[i * 4] = (float)row[0]; M[i * 4 + 1] = (float)row[1]; M[i * 4 + 2] = (float)row[2]; M[i * 4 + 3] = (float)mt;
+  }
+}
+
+int alloc_frame_buffers(tgs_ctx* c) {
+  const size_t px = (size_t)c->W * c->H;
+  const int T = c->TX * c->TY;
+  if (px <= c->px_cap && T <= c->tiles_cap) return TGS_OK;
+  cudaStreamSynchronize(c->stream);
+  for (void* p : c->allocs_frame) cudaFree(p);
+  c->allocs_frame.clear();
+  DevBuffers& b = c->b;
+  for (int i = 0; i < 2; ++i) {
+    if (int r = dev_alloc(c, &b.image[i], px * 3, c->allocs_frame)) return r;
+    if (int r = dev_alloc(c, &b.depth[i], px, c->allocs_frame)) return r;
+    if (int r = dev_alloc(c, &b.sigma[i], px, c->allocs_frame)) return r;
+  }
+  if (int r = dev_alloc(c, &b.warp_depth, px, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.warp_sigma, px, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.fill_depth, px, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.tile_flags, (size_t)T, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.tile_mask, (size_t)T, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.sel_bits, (size_t)(T + 31) / 32 + 1, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.tile_order, (size_t)T, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.ranges, (size_t)T, c->allocs_frame)) return r;
+  c->px_cap = px; c->tiles_cap = T;
+  return TGS_OK;
+}
+
+int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs) {
+  if (max_pairs <= c->max_pairs) return TGS_OK;
+  cudaStreamSynchronize(c->stream);
+  for (void* p : c->allocs_pairs) cudaFree(p);
+  c->allocs_pairs.clear();
+  DevBuffers& b = c->b;
+  for (int i = 0; i < 2; ++i) {
+    if (int r = dev_alloc(c, &b.keys[i], (size_t)max_pairs, c->allocs_pairs)) return r;
+    if (int r = dev_alloc(c, &b.vals[i], (size_t)max_pairs, c->allocs_pairs)) return r;
+  }
+  const uint32_t tiles = (max_pairs + sort_tile_items() - 1) / sort_tile_items() + 1;
+  if (int r = dev_alloc(c, &b.sort_desc, (size_t)8 * tiles * 256, c->allocs_pairs)) return r;
+  c->sort_tiles_cap = tiles;
+  c->max_pairs = max_pairs;
+  return TGS_OK;
+}
+
+uint32_t auto_max_pairs(const tgs_ctx* c) {
+  // heuristic capacity: 24 pairs per Gaussian, at least 4 M, at most 2^30 - 1 (look-back value field)
+  unsigned long long want = (unsigned long long)c->n * 24ull;
+  if (want < (4ull << 20)) want = 4ull << 20;
+  if (want > (1ull << 30) - 1) want = (1ull << 30) - 1;
+  return (uint32_t)want;
+}
+
+void invalidate_priors(tgs_ctx* c) {
+  c->priors_valid = false; c->F_valid = false; c->sched = Sched();
+  c->put_depth = c->put_sigma = c->put_image = false;
+}
+
+int copy_out(tgs_ctx* c, void* dst, const void* src, size_t bytes, int mem) {
+  if (mem == TGS_DEVICE) { CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, c->stream)); return TGS_OK; }
+  CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return TGS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tgs_strerror(int code) {
+  switch (code) {
+    case TGS_OK: return "ok";
+    case TGS_E_INVALID_ARG: return "invalid argument";
+    case TGS_E_NO_SCENE: return "no Gaussians loaded";
+    case TGS_E_NO_CAMERA: return "no camera set";
+    case TGS_E_NO_PRIORS: return "no valid temporal priors (render a reference frame first)";
+    case TGS_E_CAPACITY: return "pair buffer capacity exceeded";
+    case TGS_E_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+const char* tgs_last_error(tgs_ctx* c) { return c ? c->err : "null context"; }
+
+void tgs_default_params(tgs_params* p) {
+  if (!p) return;
+  p->lambda1 = 3.0f; p->lambda2 = 0.0f; p->lambda_tdc = 50; p->lambda_sr = 5; p->eta = 0.40f;
+  p->bg[0] = p->bg[1] = p->bg[2] = 0.0f;
+  p->enable_afc = p->enable_toc = p->enable_sr = 1;
+  p->max_pairs = 0;
+}
+
+int tgs_create(tgs_ctx** out, int device, void* stream) {
+  if (!out) return TGS_E_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return TGS_E_CUDA;
+  tgs_ctx* c = new tgs_ctx();
+  c->device = device; c->stream = (cudaStream_t)stream;
+  tgs_default_params(&c->prm);
+  auto fail = [&](int code) { delete c; return code; };
+  if (cudaSetDevice(device) != cudaSuccess) return fail(TGS_E_CUDA);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(TGS_E_CUDA);
+  c->num_sms = prop.multiProcessorCount;
+  if (cudaMallocHost((void**)&c->h_counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
+  if (cudaMallocHost((void**)&c->h_sel, 2 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
+  memset(c->h_counters, 0, sizeof(Counters));
+  if (cudaMalloc((void**)&c->b.counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
+  if (cudaMalloc((void**)&c->b.F_key, 4 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
+  if (cudaMalloc((void**)&c->b.sort_hist, 8 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
+  cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
+  for (auto& e : c->ev_stage) cudaEventCreate(&e);
+  *out = c;
+  return TGS_OK;
+}
+
+void tgs_destroy(tgs_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  free_list(c, c->allocs_scene); free_list(c, c->allocs_frame); free_list(c, c->allocs_pairs);
+  cudaFree(c->b.counters); cudaFree(c->b.F_key); cudaFree(c->b.sort_hist);
+  cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
+  cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
+  for (auto& e : c->ev_stage) cudaEventDestroy(e);
+  delete c;
+}
+
+int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, const float* scales, const float* quats,
+                       const float* opacity, const float* sh, int mem) {
+  if (!c) return TGS_E_INVALID_ARG;
+  if (deg < 0 || deg > 3 || n == 0 || !means || !scales || !quats || !opacity || !sh || (mem != TGS_HOST && mem != TGS_DEVICE)) return TGS_E_INVALID_ARG;
+  const int K = (deg + 1) * (deg + 1);
+  CK(cudaSetDevice(c->device));
+  if (mem == TGS_HOST && (!finite_all(means, 3 * (size_t)n) || !finite_all(scales, 3 * (size_t)n) || !finite_all(quats, 4 * (size_t)n) ||
+                          !finite_all(opacity, n) || !finite_all(sh, (size_t)n * K * 3))) return TGS_E_INVALID_ARG;
+  CK(cudaStreamSynchronize(c->stream));
+  for (void* p : c->allocs_scene) cudaFree(p);
+  c->allocs_scene.clear();
+  DevBuffers& b = c->b;
+  c->n = 0;
+#define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
+  A(b.cull4, n) A(b.cov3d, 6 * (size_t)n) A(b.tau, n) A(b.sh, (size_t)n * K * 3)
+  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, n) A(b.rec_rgb, n)
+  A(b.tiles_touched, (size_t)n + 4) A(b.offsets, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
+  A(b.scan_desc, (size_t)n / scan_tile_items() + 2)
+#undef A
+  const float *d_means = means, *d_scales = scales, *d_quats = quats, *d_opacity = opacity, *d_sh = sh;
+  std::vector<void*> tmp;
+  if (mem == TGS_HOST) {
+    auto up = [&](const float* h, size_t cnt, const float** d) -> int {
+      float* p = nullptr;
+      CK(cudaMalloc((void**)&p, cnt * sizeof(float)));
+      tmp.push_back(p);
+      CK(cudaMemcpyAsync(p, h, cnt * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+      *d = p;
+      return TGS_OK;
+    };
+    int r = up(means, 3 * (size_t)n, &d_means);
+    if (!r) r = up(scales, 3 * (size_t)n, &d_scales);
+    if (!r) r = up(quats, 4 * (size_t)n, &d_quats);
+    if (!r) r = up(opacity, n, &d_opacity);
+    if (!r) r = up(sh, (size_t)n * K * 3, &d_sh);
+    if (r) { for (void* p : tmp) cudaFree(p); return r; }
+  }
+  launch_repack(c->stream, n, K, d_means, d_scales, d_quats, d_opacity, d_sh, b);
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  for (void* p : tmp) cudaFree(p);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) { snprintf(c->err, sizeof(c->err), "load: %s", cudaGetErrorString(e)); return TGS_E_CUDA; }
+  c->n = n; c->deg = deg; c->K = K;
+  invalidate_priors(c);
+  c->have_frame = false;
+  return TGS_OK;
+}
+
+int tgs_set_camera(tgs_ctx* c, const float view[16], float fx, float fy, float cx, float cy, int W, int H, float znear, float zfar) {
+  if (!c || !view || W <= 0 || H <= 0 || W > 65535 * 16 || H > 65535 * 16 || !(fx > 0) || !(fy > 0) || !(znear > 0)) return TGS_E_INVALID_ARG;
+  const float intr[6] = {fx, fy, cx, cy, znear, zfar};
+  if (!finite_all(view, 16) || !finite_all(intr, 6)) return TGS_E_INVALID_ARG;
+  if (c->cam_set && (c->W != W || c->H != H || c->fx != fx || c->fy != fy || c->cx != cx || c->cy != cy)) { invalidate_priors(c); c->have_frame = false; }
+  memcpy(c->view, view, sizeof(c->view));
+  c->fx = fx; c->fy = fy; c->cx = cx; c->cy = cy; c->W = W; c->H = H; c->znear = znear; c->zfar = zfar;
+  c->TX = (W + TGS_TILE - 1) / TGS_TILE; c->TY = (H + TGS_TILE - 1) / TGS_TILE;
+  c->cam_set = true;
+  return TGS_OK;
+}
+
+int tgs_set_params(tgs_ctx* c, const tgs_params* p) {
+  if (!c || !p || p->lambda_tdc < 1 || p->lambda_sr < 1 || !std::isfinite(p->lambda1) || !std::isfinite(p->lambda2) ||
+      !std::isfinite(p->eta) || !finite_all(p->bg, 3)) return TGS_E_INVALID_ARG;
+  c->prm = *p;
+  return TGS_OK;
+}
+
+int tgs_reset_priors(tgs_ctx* c) {
+  if (!c) return TGS_E_INVALID_ARG;
+  invalidate_priors(c);
+  return TGS_OK;
+}
+
+int tgs_render(tgs_ctx* c, int mode) {
+  if (!c) return TGS_E_INVALID_ARG;
+  if (!c->n) return TGS_E_NO_SCENE;
+  if (!c->cam_set) return TGS_E_NO_CAMERA;
+  CK(cudaSetDevice(c->device));
+  // ---- A0: frame type (R9, R23)
+  if (c->sel_pending) {   // eta rule needs the selected-tile count of the previous S frame
+    CK(cudaEventSynchronize(c->ev_sel));
+    c->sched.force_P = ((float)c->h_sel[0] > c->prm.eta * (float)c->last_n_tiles) ? 1 : 0;
+    c->sel_pending = false;
+  }
+  int ftype;
+  if (mode == TGS_AUTO) {
+    if (!c->priors_valid || c->sched.since_R >= c->prm.lambda_tdc) ftype = TGS_FRAME_R;
+    else if (c->sched.since_ref >= c->prm.lambda_sr || c->sched.force_P) ftype = TGS_FRAME_P;
+    else ftype = TGS_FRAME_S;
+  } else if (mode == TGS_FULL) ftype = TGS_FRAME_R;
+  else if (mode == TGS_PSEUDO_REF) ftype = TGS_FRAME_P;
+  else if (mode == TGS_TEMPORAL) ftype = TGS_FRAME_S;
+  else return TGS_E_INVALID_ARG;
+  if (ftype != TGS_FRAME_R && !c->priors_valid) return TGS_E_NO_PRIORS;
+
+  if (int r = alloc_frame_buffers(c)) return r;
+  if (int r = alloc_pair_buffers(c, c->prm.max_pairs ? c->prm.max_pairs : auto_max_pairs(c))) return r;
+  // grow the pair buffers when the previous frame came close to (or over) the capacity
+  if (!c->prm.max_pairs && c->have_frame) {
+    if (cudaEventQuery(c->ev_done) == cudaSuccess && (c->h_counters->overflow || c->h_counters->n_pairs > c->max_pairs / 2)) {
+      unsigned long long want = (unsigned long long)c->max_pairs * 2ull;
+      if (want > (1ull << 30) - 1) want = (1ull << 30) - 1;
+      if (int r = alloc_pair_buffers(c, (uint32_t)want)) return r;
+    }
+  }
+
+  FrameConst& fc = c->fc;
+  CamConst& k = fc.cam;
+  for (int i = 0; i < 12; ++i) k.V[i] = c->view[i];
+  k.fx = c->fx; k.fy = c->fy; k.cx = c->cx; k.cy = c->cy; k.Wf = (float)c->W; k.Hf = (float)c->H;
+  const float tanx = (0.5f * (float)c->W) / c->fx, tany = (0.5f * (float)c->H) / c->fy;
+  k.limx = 1.3f * tanx; k.limy = 1.3f * tany;
+  k.znear = c->znear;
+  for (int j = 0; j < 3; ++j)
+    k.campos[j] = (float)-(((double)c->view[0 * 4 + j] * c->view[3] + (double)c->view[1 * 4 + j] * c->view[7]) + (double)c->view[2 * 4 + j] * c->view[11]);
+  k.W = c->W; k.H = c->H; k.TX = c->TX; k.TY = c->TY;
+  if (ftype == TGS_FRAME_S) { relative_pose(c->prior_view, c->view, fc.M); relative_pose(c->view, c->prior_view, fc.Minv); }
+  else { memset(fc.M, 0, sizeof(fc.M)); memset(fc.Minv, 0, sizeof(fc.Minv)); }
+  fc.lambda1 = c->prm.lambda1; fc.lambda2 = c->prm.lambda2;
+  for (int j = 0; j < 3; ++j) fc.bg[j] = c->prm.bg[j];
+  fc.n = c->n; fc.max_pairs = c->max_pairs; fc.sh_degree = c->deg; fc.ftype = ftype;
+  fc.do_afc = (ftype != TGS_FRAME_R) && c->prm.enable_afc && c->F_valid;
+  fc.do_tgb = (ftype == TGS_FRAME_S);
+  fc.do_toc = fc.do_tgb && c->prm.enable_toc;
+  fc.all_tiles = !(ftype == TGS_FRAME_S && c->prm.enable_sr && !c->force_all);
+  fc.n_tiles = c->TX * c->TY;
+
+  DevBuffers& b = c->b;
+  cudaStream_t s = c->stream;
+  const bool builds_priors = ftype != TGS_FRAME_S;
+  const int out_idx = c->prior_idx ^ 1;   // never overwrite the priors while they are being read
+  const float* prior_image = c->priors_valid ? b.image[c->prior_idx] : nullptr;
+  uint8_t* rendered_next = builds_priors ? b.rendered_next : nullptr;
+  int ev = 0;
+  auto mark = [&]() { if (c->timing) cudaEventRecord(c->ev_stage[ev], s); ++ev; };
+  mark();                                                                      // 0
+  launch_frame_init(s, fc, b, ftype == TGS_FRAME_R, rendered_next);
+  if (ftype == TGS_FRAME_S) launch_warp(s, fc, b, b.depth[c->prior_idx], b.sigma[c->prior_idx]);          // A1
+  mark();                                                                      // 1
+  if (ftype == TGS_FRAME_S) launch_fill_corr(s, fc, b);                                                    // A2
+  mark();                                                                      // 2
+  launch_preprocess(s, fc, b);                                                                             // A3 (+ T^oc of A4)
+  mark();                                                                      // 3
+  launch_select(s, fc, b);                                                                                 // A4
+  if (ftype == TGS_FRAME_S) {
+    CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    CK(cudaEventRecord(c->ev_sel, s));
+    c->sel_pending = true;
+  }
+  launch_count_color(s, fc, b);                                                                            // A5
+  launch_scan_emit(s, fc, b, c->num_sms);
+  mark();                                                                      // 4
+  const int sorted = launch_sort(s, fc, b, c->num_sms, c->sort_tiles_cap);                                 // A6
+  mark();                                                                      // 5
+  launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
+  mark();                                                                      // 6
+  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms);                         // A8 + A9
+  mark();                                                                      // 7
+  if (builds_priors) launch_frustum(s, fc, b, rendered_next, ftype == TGS_FRAME_R);                        // F_min/F_max (L109)
+  CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
+  mark();                                                                      // 8
+  CK(cudaEventRecord(c->ev_done, s));
+  CK(cudaGetLastError());
+  // ---- A10: prior commit (pointer swap) and scheduler counters
+  c->cur_idx = out_idx; c->sorted_idx = sorted;
+  if (builds_priors) {
+    c->prior_idx = out_idx;
+    std::swap(b.rendered, b.rendered_next);
+    memcpy(c->prior_view, c->view, sizeof(c->prior_view));
+    c->priors_valid = true;
+    if (ftype == TGS_FRAME_R) c->F_valid = true;
+  }
+  if (ftype == TGS_FRAME_R) { c->sched.since_R = 0; c->sched.since_ref = 0; c->sched.force_P = 0; }
+  else if (ftype == TGS_FRAME_P) { c->sched.since_ref = 0; c->sched.force_P = 0; }
+  ++c->sched.since_R; ++c->sched.since_ref;
+  c->last_ftype = ftype; c->last_n_tiles = (uint32_t)fc.n_tiles;
+  c->have_frame = true;
+  return TGS_OK;
+}
+
+int tgs_read_image(tgs_ctx* c, float* rgb, int mem) {
+  if (!c || !rgb || !c->have_frame) return TGS_E_INVALID_ARG;
+  return copy_out(c, rgb, c->b.image[c->cur_idx], (size_t)c->W * c->H * 3 * sizeof(float), mem);
+}
+
+int tgs_read_depth(tgs_ctx* c, float* depth, float* sigma, int mem) {
+  if (!c || !depth || !c->have_frame) return TGS_E_INVALID_ARG;
+  if (sigma) { if (int r = copy_out(c, sigma, c->b.sigma[c->cur_idx], (size_t)c->W * c->H * sizeof(float), mem)) return r; }
+  return copy_out(c, depth, c->b.depth[c->cur_idx], (size_t)c->W * c->H * sizeof(float), mem);
+}
+
+int tgs_read_tile_mask(tgs_ctx* c, uint8_t* sel, int mem) {
+  if (!c || !sel || !c->have_frame) return TGS_E_INVALID_ARG;
+  return copy_out(c, sel, c->b.tile_mask, (size_t)c->TX * c->TY, mem);
+}
+
+int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
+  if (!c || !out || !c->have_frame) return TGS_E_INVALID_ARG;
+  CK(cudaEventSynchronize(c->ev_done));
+  const Counters& h = *c->h_counters;
+  memset(out, 0, sizeof(*out));
+  out->frame_type = c->last_ftype;
+  out->n_total = c->n; out->n_near = h.n_near; out->n_afc = h.n_afc; out->n_toc = h.n_toc; out->n_degenerate = h.n_degenerate;
+  out->n_empty = h.n_empty; out->n_visible = h.n_visible; out->n_newly_visible = h.n_newly_visible;
+  out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
+  out->n_rendered = h.n_rendered; out->overflow = h.overflow;
+  out->device_bytes = c->device_bytes;
+  if (c->timing) {
+    for (int i = 0; i < 8; ++i) cudaEventElapsedTime(&out->ms_stage[i], c->ev_stage[i], c->ev_stage[i + 1]);
+    cudaEventElapsedTime(&out->ms_total, c->ev_stage[0], c->ev_stage[8]);
+  }
+  if (h.error) { snprintf(c->err, sizeof(c->err), "device watchdog: look-back stalled (code %u)", h.error); return TGS_E_CUDA; }
+  if (h.overflow) return TGS_E_CAPACITY;
+  return TGS_OK;
+}
+
+
+// ------------------------------------------------------------------ test-only access to intermediates
+static uint32_t f2key_host(float f) { uint32_t b; memcpy(&b, &f, 4); return (b & 0x80000000u) ? ~b : (b | 0x80000000u); }
+static float key2f_host(uint32_t k) { const uint32_t b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k; float f; memcpy(&f, &b, 4); return f; }
+
+long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int mem) {
+  if (!c || !nm || (mem != TGS_HOST && mem != TGS_DEVICE)) return TGS_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  const std::string name(nm);
+  const DevBuffers& b = c->b;
+  const size_t N = c->n, px = (size_t)c->W * c->H, T = (size_t)c->TX * c->TY;
+  const void* src = nullptr; size_t have = 0;
+  if (name == "keys" || name == "vals") {
+    if (!c->have_frame) return TGS_E_INVALID_ARG;
+    CK(cudaEventSynchronize(c->ev_done));
+    const size_t P = c->h_counters->n_pairs;
+    if (name == "keys") { src = b.keys[c->sorted_idx]; have = P * 8; } else { src = b.vals[c->sorted_idx]; have = P * 4; }
+  } else if (name == "F") {
+    uint32_t keys[4]; float F[4];
+    CK(cudaMemcpyAsync(keys, b.F_key, sizeof(keys), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < 4; ++i) F[i] = key2f_host(keys[i]);
+    if (dst && bytes) {
+      if (mem == TGS_HOST) memcpy(dst, F, bytes < 16 ? bytes : 16);
+      else { CK(cudaMemcpy(dst, F, bytes < 16 ? bytes : 16, cudaMemcpyHostToDevice)); }
+    }
+    return 16;
+  }
+  else if (name == "rec_uvdo") { src = b.rec_uvdo; have = N * 16; }
+  else if (name == "rec_conic") { src = b.rec_conic; have = N * 16; }
+  else if (name == "rec_rect") { src = b.rec_rect; have = N * 8; }
+  else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
+  else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }
+  else if (name == "tiles_touched") { src = b.tiles_touched; have = N * 4; }
+  else if (name == "offsets") { src = b.offsets; have = N * 4; }
+  else if (name == "ranges") { src = b.ranges; have = T * 8; }
+  else if (name == "tile_order") { src = b.tile_order; have = T * 4; }
+  else if (name == "warp_depth") { src = b.warp_depth; have = px * 4; }
+  else if (name == "warp_sigma") { src = b.warp_sigma; have = px * 4; }
+  else if (name == "fill_depth") { src = b.fill_depth; have = px * 4; }
+  else if (name == "rendered") { src = b.rendered; have = N; }
+  else if (name == "prior_depth") { src = b.depth[c->prior_idx]; have = px * 4; }
+  else if (name == "prior_sigma") { src = b.sigma[c->prior_idx]; have = px * 4; }
+  else if (name == "prior_image") { src = b.image[c->prior_idx]; have = px * 12; }
+  else if (name == "cov3d") { src = b.cov3d; have = N * 24; }
+  else if (name == "tau") { src = b.tau; have = N * 4; }
+  else return TGS_E_INVALID_ARG;
+  if (!src) return TGS_E_INVALID_ARG;
+  if (dst && bytes && have) { if (int r = copy_out(c, dst, src, bytes < have ? bytes : have, mem)) return r; }
+  return (long long)have;
+}
+
+int tgs_debug_put(tgs_ctx* c, const char* nm, const void* src, size_t bytes, int mem) {
+  if (!c || !nm || !src || (mem != TGS_HOST && mem != TGS_DEVICE) || !c->cam_set || !c->n) return TGS_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  if (int r = alloc_frame_buffers(c)) return r;
+  const std::string name(nm);
+  DevBuffers& b = c->b;
+  const size_t N = c->n, px = (size_t)c->W * c->H;
+  const cudaMemcpyKind kind = mem == TGS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  auto put = [&](void* dstp, size_t want) -> int {
+    if (bytes != want) return TGS_E_INVALID_ARG;
+    CK(cudaMemcpyAsync(dstp, src, bytes, kind, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return TGS_OK;
+  };
+  if (name == "prior_depth") { int r = put(b.depth[c->prior_idx], px * 4); if (!r) c->put_depth = true; return r; }
+  if (name == "prior_sigma") { int r = put(b.sigma[c->prior_idx], px * 4); if (!r) c->put_sigma = true; return r; }
+  if (name == "prior_image") { int r = put(b.image[c->prior_idx], px * 12); if (!r) c->put_image = true; return r; }
+  if (name == "rendered") return put(b.rendered, N);
+  if (name == "F") {
+    if (bytes != 16) return TGS_E_INVALID_ARG;
+    float F[4]; uint32_t keys[4];
+    if (mem == TGS_HOST) memcpy(F, src, 16); else { CK(cudaMemcpy(F, src, 16, cudaMemcpyDeviceToHost)); }
+    for (int i = 0; i < 4; ++i) keys[i] = f2key_host(F[i]);
+    CK(cudaMemcpyAsync(b.F_key, keys, 16, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->F_valid = true;
+    return TGS_OK;
+  }
+  if (name == "prior_view") {
+    if (bytes != 64) return TGS_E_INVALID_ARG;
+    if (mem == TGS_HOST) memcpy(c->prior_view, src, 64); else { CK(cudaMemcpy(c->prior_view, src, 64, cudaMemcpyDeviceToHost)); }
+    if (!c->priors_valid) {
+      if (!(c->put_depth && c->put_sigma && c->put_image)) return TGS_E_NO_PRIORS;
+      c->priors_valid = true;
+    }
+    return TGS_OK;
+  }
+  return TGS_E_INVALID_ARG;
+}
+
+int tgs_debug_run_stage(tgs_ctx* c, const char* st) {
+  if (!c || !st) return TGS_E_INVALID_ARG;
+  const std::string s(st);
+  if (s == "timing_on") { c->timing = true; return TGS_OK; }
+  if (s == "timing_off") { c->timing = false; return TGS_OK; }
+  if (s == "force_all_tiles_on") { c->force_all = 1; return TGS_OK; }
+  if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
+  return TGS_E_INVALID_ARG;
+}
+
+}  // extern "C"

@@ -1,0 +1,111 @@
+// tgs_internal.cuh -- shared declarations of the CUDA path (NOT shared with oracle/).
+// Paper: TemporalGS, arxiv/paper_2607_03390; citations are PAPER.md:L<line>; steps A0-A10 and data
+// layout are described in DESIGN.md §1 / §6.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tgs.h"
+
+#define TGS_TILE 16
+#define TGS_INVALID_BITS 0x7f61b1e6u /* bits of 3.0e38f */
+
+// ------------------------------------------------------------------ per-frame constants (kernel argument)
+struct CamConst {
+  float V[12];              // world->camera, rows 0..2 of the 4x4
+  float fx, fy, cx, cy;
+  float Wf, Hf;             // (float)W, (float)H
+  float limx, limy;         // 1.3 tan(fov/2) (R3)
+  float znear;
+  float campos[3];          // camera centre, for the SH view direction
+  int W, H, TX, TY;
+};
+
+struct FrameConst {
+  CamConst cam;
+  float M[12];              // reference -> current (Eq.3)
+  float Minv[12];           // current -> reference (backward query, L121)
+  float lambda1, lambda2;   // L99
+  float bg[3];
+  uint32_t n;
+  uint32_t max_pairs;
+  int sh_degree;
+  int ftype;                // TGS_FRAME_R / P / S
+  int do_afc, do_toc, do_tgb, all_tiles;
+  int n_tiles;
+};
+
+// ------------------------------------------------------------------ device counters (one block, zeroed per frame)
+struct Counters {
+  uint32_t n_near, n_afc, n_toc, n_degenerate, n_empty, n_visible, n_newly_visible;
+  uint32_t n_pairs;
+  uint32_t n_sel_oc, n_sel_um, n_sel;
+  uint32_t n_rendered;
+  uint32_t overflow;
+  uint32_t error;           // look-back watchdog etc.
+  // work tickets of the persistent kernels
+  uint32_t ticket_scan;
+  uint32_t ticket_blend;
+  uint32_t ticket_sort[8];
+  uint32_t pad[10];
+};
+
+// ------------------------------------------------------------------ device buffers of a context
+struct DevBuffers {
+  // scene (repacked at load)
+  float4* cull4 = nullptr;       // [N] {x,y,z,opacity}
+  float* cov3d = nullptr;        // [N][6] xx,xy,xz,yy,yz,zz
+  float* tau = nullptr;          // [N] 2 ln(255 o)
+  float* sh = nullptr;           // [N][K][3]
+  // per-Gaussian records of the current frame
+  float4* rec_uvdo = nullptr;    // [N] {u,v,d,o}
+  float4* rec_conic = nullptr;   // [N] {A,B,C,tau}
+  uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16
+  uint32_t* rec_flags = nullptr; // [N]
+  float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
+  uint32_t* tiles_touched = nullptr;  // [N]
+  uint32_t* offsets = nullptr;        // [N] exclusive scan
+  uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
+  uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
+  // pairs
+  uint64_t* keys[2] = {nullptr, nullptr};
+  uint32_t* vals[2] = {nullptr, nullptr};
+  uint32_t* sort_hist = nullptr;      // [8][256]
+  uint32_t* sort_desc = nullptr;      // [passes][tiles][256] look-back descriptors
+  uint64_t* scan_desc = nullptr;      // look-back descriptors of the offsets scan
+  // tiles
+  uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
+  uint8_t* tile_mask = nullptr;       // [T] bit0 oc, bit1 um, bit2 selected
+  uint32_t* sel_bits = nullptr;       // [ceil(T/32)]
+  uint32_t* tile_order = nullptr;     // [T] selected tiles first, then the others
+  uint2* ranges = nullptr;            // [T] {start,end}
+  // images
+  float* image[2] = {nullptr, nullptr};   // [H][W][3]
+  float* depth[2] = {nullptr, nullptr};   // [H][W]
+  float* sigma[2] = {nullptr, nullptr};   // [H][W]
+  float* warp_depth = nullptr;  // D^min (uint bits during the splat)
+  float* warp_sigma = nullptr;  // sigma^max
+  float* fill_depth = nullptr;  // D'
+  uint32_t* F_key = nullptr;    // [4] ordered-uint keys of F_min.x, F_min.y, F_max.x, F_max.y
+  Counters* counters = nullptr;
+};
+
+// ------------------------------------------------------------------ launchers (definitions in k_*.cu)
+void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const float* scales, const float* quats,
+                   const float* opacity, const float* sh, DevBuffers& b);
+void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next);
+void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma);
+void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_count_color(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint8_t* rendered_now, bool update_F);
+void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
+// returns the index (0/1) of the key/val buffer that holds the sorted result
+int launch_sort(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms, uint32_t sort_tiles_cap);
+void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
+void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
+                  const float* prior_image, uint8_t* rendered_next, int num_sms);
+uint32_t sort_tile_items();
+uint32_t scan_tile_items();
+int sort_num_passes(int n_tiles);

@@ -1,0 +1,151 @@
+"""Helpers of the GPU parity tests: drive the CUDA path (through the C-ABI binding) and the oracle on the
+same seeded inputs and compare them element by element.
+
+Tolerances (BASELINE.json north_star; derivation in DESIGN.md §5):
+  integers (flags, rects, pair counts, sorted keys and values, ranges, tile masks, warped-pixel hits): bit-exact;
+  decision floats (u, v, d, conic, warped depth/sigma, repaired depth): bit-exact (same fp32 operation order);
+  RGB: max abs error <= 2e-3; depth: <= 1e-4 relative; sigma: <= 2e-3 * depth (sqrt of an fp32 cancellation);
+  pixels the oracle marks `borderline` (an alpha or transmittance test within its rounding margin) may take
+  the other branch: there RGB <= 1.2e-2 and they must be rare.
+"""
+import numpy as np
+
+from oracle import ora
+from oracle.ora import Oracle
+from paper_2607_03390_b200 import tgs
+
+RGB_TOL = 2e-3
+DEPTH_RTOL = 1e-4
+SIGMA_TOL_REL_DEPTH = 2e-3
+BORDERLINE_RGB_TOL = 1.2e-2
+
+MODE_G = {"full": tgs.FULL, "pseudo": tgs.PSEUDO_REF, "temporal": tgs.TEMPORAL, "auto": tgs.AUTO}
+MODE_O = {"full": ora.FULL, "pseudo": ora.PSEUDO_REF, "temporal": ora.TEMPORAL, "auto": ora.AUTO}
+
+
+def make_pair(sc, params=None):
+    g = tgs.Context(0)
+    o = Oracle()
+    g.load_scene(sc)
+    o.load_scene(sc)
+    if params:
+        pg, po = g.default_params(), o.default_params()
+        for k, v in params.items():
+            if k == "bg":
+                for i in range(3):
+                    pg.bg[i] = v[i]
+                    po.bg[i] = v[i]
+            else:
+                setattr(pg, k, v)
+                if k != "max_pairs":
+                    setattr(po, k, v)
+        g.set_params(pg)
+        o.set_params(po)
+    return g, o
+
+
+def inject_priors(g, o):
+    """Feed the oracle's priors to the CUDA context so that an S / P frame starts from identical inputs."""
+    g.debug_put("prior_depth", o.get("prior_depth"))
+    g.debug_put("prior_sigma", o.get("prior_sigma"))
+    g.debug_put("prior_image", o.get("prior_image"))
+    g.debug_put("rendered", o.get("rendered"))
+    g.debug_put("F", o.get("F"))
+    g.debug_put("prior_view", o.get("prior_view"))
+
+
+def bits(a):
+    return np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+
+
+def compare_records(g, o, n):
+    rec = o.get("records")
+    fl_g = g.debug_get("rec_flags")
+    assert np.array_equal(fl_g, rec["flags"]), f"flags differ at {np.nonzero(fl_g != rec['flags'])[0][:10]}"
+    vis = (rec["flags"] & ora.VISIBLE) != 0
+    uvdo = g.debug_get("rec_uvdo").reshape(n, 4)
+    conic = g.debug_get("rec_conic").reshape(n, 4)
+    rect = g.debug_get("rec_rect").reshape(n, 4)
+    for j, name in enumerate(("u", "v", "d", "o")):
+        assert np.array_equal(bits(uvdo[vis, j]), bits(rec[name][vis])), name
+    for j, name in enumerate(("A", "B", "C", "tau")):
+        assert np.array_equal(bits(conic[vis, j]), bits(rec[name][vis])), name
+    for j, name in enumerate(("x_lo", "x_hi", "y_lo", "y_hi")):
+        assert np.array_equal(rect[vis, j], rec[name][vis]), name
+    tt = g.debug_get("tiles_touched")
+    assert np.array_equal(tt, rec["tiles_touched"])
+    col = tt > 0
+    rgb = g.debug_get("rec_rgb").reshape(n, 4)[:, :3]
+    ref = np.stack([rec["r"], rec["g"], rec["b"]], 1)
+    np.testing.assert_allclose(rgb[col], ref[col], atol=2e-5)
+    return rec
+
+
+def compare_binning(g, o):
+    keys_o, vals_o, ranges_o = o.get("keys"), o.get("vals"), o.get("ranges")
+    keys_g, vals_g, ranges_g = g.debug_get("keys"), g.debug_get("vals"), g.debug_get("ranges")
+    assert len(keys_g) == len(keys_o)
+    assert np.array_equal(keys_g, keys_o)
+    assert np.array_equal(vals_g, vals_o)
+    assert np.array_equal(ranges_g, ranges_o)
+
+
+def compare_temporal_buffers(g, o):
+    wd_o, ws_o, fd_o = o.get("warp_depth"), o.get("warp_sigma"), o.get("fill_depth")
+    assert np.array_equal(bits(g.debug_get("warp_depth")), bits(wd_o))
+    assert np.array_equal(bits(g.debug_get("warp_sigma")), bits(ws_o))
+    assert np.array_equal(bits(g.debug_get("fill_depth")), bits(fd_o))
+
+
+def compare_outputs(g, o, ftype):
+    img_g, img_o = g.read_image(), o.read_image()
+    d_g, s_g = g.read_depth()
+    d_o, s_o = o.read_depth()
+    border = o.get("borderline").reshape(d_o.shape).astype(bool)
+    err = np.abs(img_g - img_o).max(-1)
+    assert border.mean() < 5e-3, border.mean()
+    assert err[~border].max() <= RGB_TOL, err[~border].max()
+    assert err.max() <= BORDERLINE_RGB_TOL, err.max()
+    ok = ~border
+    vg, vo = d_g < 1e38, d_o < 1e38
+    assert np.array_equal(vg[ok], vo[ok])
+    both = vg & vo & ok
+    rel = np.abs(d_g[both] - d_o[both]) / d_o[both]
+    assert rel.max() <= DEPTH_RTOL, rel.max()
+    serr = np.abs(s_g[both] - s_o[both]) / d_o[both]
+    assert serr.max() <= SIGMA_TOL_REL_DEPTH, serr.max()
+    return float(err.max()), float(rel.max()) if rel.size else 0.0
+
+
+def compare_rendered(g, o):
+    """G_rendered: must contain every Gaussian the oracle surely blended and none it surely did not."""
+    r_g = g.debug_get("rendered").astype(bool)
+    sure, maybe = o.get("rendered_sure").astype(bool), o.get("rendered_maybe").astype(bool)
+    assert not np.any(sure & ~r_g), np.nonzero(sure & ~r_g)[0][:10]
+    assert not np.any(r_g & ~maybe), np.nonzero(r_g & ~maybe)[0][:10]
+    return int((r_g != o.get("rendered").astype(bool)).sum())
+
+
+STAT_KEYS = ("frame_type", "n_total", "n_near", "n_afc", "n_toc", "n_degenerate", "n_empty", "n_visible", "n_newly_visible",
+             "n_pairs", "n_tiles", "n_sel_oc", "n_sel_um", "n_sel")
+
+
+def compare_stats(g, o):
+    sg, so = g.get_stats(), o.stats()
+    for k in STAT_KEYS:
+        assert sg[k] == so[k], (k, sg[k], so[k])
+    return sg, so
+
+
+def compare_frame(g, o, n, ftype, check_rendered=True):
+    """Everything of one frame, both sides already rendered."""
+    sg, so = compare_stats(g, o)
+    if ftype == ora.FRAME_S:
+        compare_temporal_buffers(g, o)
+    assert np.array_equal(g.read_tile_mask(), o.read_tile_mask())
+    compare_records(g, o, n)
+    compare_binning(g, o)
+    out = compare_outputs(g, o, ftype)
+    if ftype != ora.FRAME_S and check_rendered:
+        compare_rendered(g, o)
+    return sg, so, out

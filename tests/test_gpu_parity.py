@@ -1,0 +1,278 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle on the same seeded inputs.
+
+Sizes: small cases the oracle finishes in seconds (several tiles, ragged tails, several sort tiles) and
+one case at BASELINE.json's full size (config 3: 3 M Gaussians, 1080p) in the launch configuration
+bench.py times.  Edge cases: empty frames, one Gaussian, whole-screen splats, ragged image sizes,
+every SH degree, capacity overflow, missing priors.
+"""
+import numpy as np
+import pytest
+
+from oracle import ora
+from synth import Camera, make_config, look_at
+
+pytestmark = pytest.mark.gpu
+
+
+def _p():
+    import parity as P          # tests/parity.py (loads the CUDA library: only inside gpu tests)
+    return P
+
+
+def _tgs():
+    from paper_2607_03390_b200 import tgs
+    return tgs
+
+
+# ------------------------------------------------------------------------------------------------ config 1
+def test_config1_full_then_temporal_injected():
+    """Config 1 as stated: frame 0 full, frames 1-7 temporal.  The CUDA context is fed the oracle's priors, so
+    every integer output of the S frames must be bit-exact."""
+    P = _p()
+    sc = make_config(1)
+    g, o = P.make_pair(sc)
+    n = sc.n
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); assert o.render(ora.FULL) == ora.FRAME_R
+    P.compare_frame(g, o, n, ora.FRAME_R)
+    F_g, F_o = g.debug_get("F"), o.get("F")
+    P.inject_priors(g, o)
+    sel_fracs = []
+    for f in range(1, len(sc.poses)):
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G["temporal"]); assert o.render(ora.TEMPORAL) == ora.FRAME_S
+        sg, so, _ = P.compare_frame(g, o, n, ora.FRAME_S)
+        sel_fracs.append(sg["n_sel"] / sg["n_tiles"])
+    assert min(sel_fracs) < 1.0            # selective rendering really skipped tiles
+    # F of the GPU's own reference frame: equal unless a borderline Gaussian sits on the hull
+    assert np.allclose(F_g, F_o, atol=1e-3)
+
+
+def test_config1_end_to_end_own_priors():
+    """Same stream without injection: the CUDA path builds and consumes its own priors."""
+    P = _p()
+    sc = make_config(1)
+    g, o = P.make_pair(sc)
+    for f in range(len(sc.poses)):
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        mode = "full" if f == 0 else "temporal"
+        g.render(P.MODE_G[mode]); o.render(P.MODE_O[mode])
+        sg, so = g.get_stats(), o.stats()
+        mg, mo = g.read_tile_mask(), o.read_tile_mask()
+        # the GPU's TGB differs from the oracle's by rounding, so a few decisions may flip
+        assert (mg != mo).mean() < 0.05
+        same = np.kron((mg & 4) == (mo & 4), np.ones((16, 16), bool))[: sc.camera.H, : sc.camera.W]
+        err = np.abs(g.read_image() - o.read_image()).max(-1)
+        assert np.quantile(err[same], 0.999) < 2e-3
+        assert abs(int(sg["n_visible"]) - int(so["n_visible"])) <= 0.01 * so["n_visible"] + 5
+
+
+def test_pseudo_reference_frame_with_afc():
+    P = _p()
+    sc = make_config(1, n=8000)
+    g, o = P.make_pair(sc, {"bg": (0.1, 0.3, 0.2)})
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[3], sc.camera); o.set_camera(sc.poses[3], sc.camera)
+    g.render(P.MODE_G["pseudo"]); assert o.render(ora.PSEUDO_REF) == ora.FRAME_P
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_P)
+    assert sg["n_sel"] == sg["n_tiles"] and sg["n_toc"] == 0
+    # the P frame rebuilt the priors: a following S frame uses them
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[4], sc.camera); o.set_camera(sc.poses[4], sc.camera)
+    g.render(P.MODE_G["temporal"]); o.render(ora.TEMPORAL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_S)
+
+
+# ------------------------------------------------------------------------------------------------ denser scenes, sort at scale
+def _dense_scene(n, W, H, seed_cfg=2, frames=4):
+    sc = make_config(seed_cfg, n=n, frames=frames, width=W, height=H)
+    return sc
+
+
+def test_medium_scene_sh3_many_sort_tiles_ragged():
+    """200 k Gaussians, SH degree 3, 500x281 (ragged in x and y): P spans dozens of 4096-pair sort tiles with a
+    ragged tail; whole sorted key / value lists are compared."""
+    P = _p()
+    sc = _dense_scene(200_000, 500, 281)
+    sc.scales *= 2.0
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    assert sg["n_pairs"] > 20 * 4096 and sg["n_pairs"] % 4096 != 0
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[2], sc.camera); o.set_camera(sc.poses[2], sc.camera)
+    g.render(P.MODE_G["temporal"]); o.render(ora.TEMPORAL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+    assert 0 < sg["n_sel"] < sg["n_tiles"] and sg["n_toc"] > 0
+
+
+@pytest.mark.parametrize("deg", [0, 1, 2, 3])
+def test_sh_degrees(deg):
+    P = _p()
+    rng = np.random.default_rng(40 + deg)
+    sc = make_config(1, n=3000, frames=1, width=96, height=80)
+    K = (deg + 1) ** 2
+    sc.sh = rng.normal(0, 0.3, size=(sc.n, K, 3)).astype(np.float32)
+    sc.sh_degree = deg
+    sc.scales *= 3
+    g, o = P.make_pair(sc)
+    V = look_at((1.0, 0.5, -3.0), (0, 0, 0), (0, 1, 0))
+    g.set_camera(V, sc.camera); o.set_camera(V, sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_R)
+
+
+def test_layered_scene_config5_reduced():
+    """Config 5 recipe (stacked semi-opaque sheets, SH degree 1) reduced: heavy occlusion, TOC culls a lot."""
+    P = _p()
+    sc = make_config(5, n=60_000, frames=12, width=320, height=180)
+    sc.scales[:, :2] *= 6.0                       # keep the sheets closed at the reduced density
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    P.inject_priors(g, o)
+    for f in (1, 2):
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G["temporal"]); o.render(ora.TEMPORAL)
+        sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+    assert sg["n_toc"] > 0.2 * sc.n
+
+
+# ------------------------------------------------------------------------------------------------ scheduler through the ABI
+def test_auto_schedule_matches_oracle():
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=6000, frames=8)
+    sc.scales *= 2
+    poses = [look_at((6.0 * np.sin(np.radians(a)), 0.0, -6.0 * np.cos(np.radians(a))), (0, 0, 0), (0, 1, 0))
+             for a in np.concatenate([np.arange(0, 6) * 0.3, 1.5 + np.arange(1, 8) * 4.0])]
+    g, o = P.make_pair(sc, {"lambda_tdc": 9, "lambda_sr": 4, "eta": 0.5})
+    types_g, types_o = [], []
+    for V in poses:
+        g.set_camera(V, sc.camera); o.set_camera(V, sc.camera)
+        g.render(tgs.AUTO); t = o.render(ora.AUTO)
+        sg, so = g.get_stats(), o.stats()
+        types_g.append(sg["frame_type"]); types_o.append(t)
+        if sg["frame_type"] == t == ora.FRAME_S:
+            assert abs(int(sg["n_sel"]) - int(so["n_sel"])) <= 0.05 * so["n_tiles"]
+    assert types_g == types_o
+    assert ora.FRAME_P in types_g and ora.FRAME_S in types_g and types_g[0] == ora.FRAME_R and types_g[9] == ora.FRAME_R
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def test_edge_empty_frame_and_single_gaussian():
+    P = _p()
+    tgs = _tgs()
+    cam = Camera(W=70, H=37, fx=60.0, fy=60.0, cx=34.5, cy=18.0)
+    sc = make_config(1, n=500, frames=1, width=70, height=37)
+    sc.camera = cam
+    sc.means[:, 2] = -5.0 - np.abs(sc.means[:, 2])            # everything behind the camera
+    g, o = P.make_pair(sc, {"bg": (0.25, 0.5, 0.75)})
+    g.set_camera(np.eye(4), cam); o.set_camera(np.eye(4), cam)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    assert sg["n_pairs"] == 0 and sg["n_near"] == sc.n
+    assert np.allclose(g.read_image(), np.array([0.25, 0.5, 0.75], np.float32))
+    assert np.all(g.read_depth()[0] == tgs.DEPTH_INVALID)
+    # S frame on empty priors: nothing warps, every tile is unmatched -> all selected, still empty
+    P.inject_priors(g, o)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+    assert sg["n_sel_um"] == sg["n_tiles"]
+    # a single Gaussian
+    one = make_config(1, n=1, frames=1, width=70, height=37)
+    one.camera = cam
+    one.means[:] = [[0.1, -0.05, 2.0]]; one.scales[:] = 0.2; one.opacity[:] = 0.9
+    g, o = P.make_pair(one)
+    g.set_camera(np.eye(4), cam); o.set_camera(np.eye(4), cam)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    P.compare_frame(g, o, 1, ora.FRAME_R)
+
+
+def test_edge_whole_screen_splats():
+    """Gaussians right in front of the camera cover every tile: exercises the warp-cooperative key emission."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=4000, frames=2, width=400, height=300)
+    sc.means[:40, 2] = -5.9 + 0.002 * np.arange(40)           # ~0.1 m in front of the camera at z = -6
+    sc.means[:40, :2] *= 0.01
+    sc.scales[:40] = 0.5
+    sc.opacity[:40] = 0.02
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    T = sg["n_tiles"]
+    assert (o.get("records")["tiles_touched"][:40] == T).all()
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[1], sc.camera); o.set_camera(sc.poses[1], sc.camera)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_S)
+
+
+def test_edge_capacity_overflow_and_errors():
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=5000, frames=1)
+    g, o = P.make_pair(sc, {"max_pairs": 1000})
+    assert g.render_rc(tgs.FULL) == tgs.E_NO_CAMERA
+    g.set_camera(sc.poses[0], sc.camera)
+    assert g.render_rc(tgs.TEMPORAL) == tgs.E_NO_PRIORS and g.render_rc(tgs.PSEUDO_REF) == tgs.E_NO_PRIORS
+    g.render(tgs.FULL)
+    with pytest.raises(tgs.TgsError) as ei:
+        g.get_stats()
+    assert ei.value.code == tgs.E_CAPACITY
+    empty = tgs.Context(0)
+    assert empty.render_rc(tgs.FULL) == tgs.E_NO_SCENE
+    bad = sc.means.copy(); bad[7, 1] = np.nan
+    with pytest.raises(tgs.TgsError) as ei:
+        empty.load_gaussians(bad, sc.scales, sc.quats, sc.opacity, sc.sh, 0)
+    assert ei.value.code == tgs.E_INVALID_ARG
+
+
+def test_device_pointers_and_torch_stream():
+    """Inputs / outputs as device pointers of torch tensors on a non-default torch stream (north_star: PyTorch is
+    used only for device memory and streams)."""
+    import torch
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=5000, frames=2)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (sc.means, sc.scales, sc.quats, sc.opacity, sc.sh)]
+    stream.synchronize()
+    g = tgs.Context(0, stream.cuda_stream)
+    g.load_gaussians(*dev, sc.sh_degree)
+    g.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL)
+    img = torch.empty((sc.camera.H, sc.camera.W, 3), dtype=torch.float32, device="cuda")
+    g.read_image(img)
+    stream.synchronize()
+    h, o = P.make_pair(sc)
+    h.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    h.render(tgs.FULL); o.render(ora.FULL)
+    assert np.array_equal(img.cpu().numpy(), h.read_image())
+    assert np.abs(img.cpu().numpy() - o.read_image()).max() < 1.2e-2
+
+
+# ------------------------------------------------------------------------------------------------ full size
+def test_full_size_config3_reference_and_temporal():
+    """BASELINE.json config 3 (3 M Gaussians, SH 3, 1920x1080) in the launch configuration bench.py times: one
+    reference frame and one TemporalGS frame, every output compared with the oracle."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(3, frames=4)
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, out = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    assert sg["n_pairs"] > 1_000_000
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[2], sc.camera); o.set_camera(sc.poses[2], sc.camera)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    sg, so, out = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+    assert sg["n_sel"] < sg["n_tiles"]
