@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- rendered FPS over the config-3 trajectory (3 M Gaussians, 1080p): TemporalGS (AUTO schedule)
+and full render every frame, on the CUDA path through the C-ABI (BASELINE.json: metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A step = one frame of the trajectory = one pass of the whole hot path (A0-A10 of DESIGN.md §1).  With N > 1
+(torchrun) every rank renders the same trajectory on its own GPU: the path does not shard ("replicas only",
+DESIGN.md §9), so `value` is the sum of the ranks' frames over the slowest rank's time ("weak").
+`--impl reference` times the CPU oracle as it stands on the host cores (rank 0 only).
+Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full render"
+# FP32-pipe cost of one (pixel, Gaussian) interaction of the blend inner loop, in warp-lane instructions on
+# the FMA pipe, counted from the SASS of k_blend: 2 FADD (dx, dy) + 5 FMUL/FFMA (exponent)
+# + 1 FADD (log2 o) = 8 up to the alpha test, which most interactions do not pass.
+BLEND_FMA_LANE_INSTR = 8.0
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc:
+            time.sleep(0.12)
+            self.proc.terminate()
+        sm, mx, reasons = [], 0.0, set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx = max(mx, float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def trajectory_pose(sc, f):
+    """Frame f of an endless smooth trajectory: the config's poses played forward, then backward, ..."""
+    F = len(sc.poses)
+    k = f % (2 * F - 2) if F > 1 else 0
+    return sc.poses[k if k < F else 2 * F - 2 - k]
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_03390_b200 import build as tgs_build
+    from synth import make_config
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    tgs_build.build()
+    from paper_2607_03390_b200 import tgs           # raises if libtgs.so is missing: no fallback
+
+    sc = make_config(args.config, n=args.n, frames=None)
+    stream = torch.cuda.Stream()
+    ctx = tgs.Context(local, stream.cuda_stream)
+    ctx.load_scene(sc)                              # scene resident in HBM before any timed region
+    cam = sc.camera
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(mode, steps, readback=None):
+        """Device time (CUDA events on the context's stream) of `steps` frames; returns ms."""
+        ctx.reset_priors()
+        for f in range(W):                          # warm-up frames (untimed) -- same path, same mode
+            ctx.set_camera(trajectory_pose(sc, f), cam)
+            ctx.render(mode)
+        ctx.reset_priors()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for f in range(steps):
+                ctx.set_camera(trajectory_pose(sc, f), cam)
+                ctx.render(mode)
+                if readback is not None:
+                    ctx.read_image(readback)        # device -> pinned host, blocks until the frame is there
+            e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ms_tgs = timed(tgs.AUTO, K)
+    clocks = sampler.stop() if rank == 0 else None
+    ms_full = timed(tgs.FULL, K)
+    pinned = torch.empty((cam.H, cam.W, 3), dtype=torch.float32).pin_memory().numpy()
+    ms_e2e = timed(tgs.AUTO, K, readback=pinned)
+
+    # ---- per-stage pass (untimed for `value`): stage events + interaction counter, one sync per frame
+    ctx.debug_run_stage("timing_on")
+    ctx.debug_run_stage("count_interactions_on")
+    ctx.reset_priors()
+    per_type = {0: [], 1: [], 2: []}
+    prof_frames = min(K, 60)
+    for f in range(prof_frames):
+        ctx.set_camera(trajectory_pose(sc, f), cam)
+        ctx.render(tgs.AUTO)
+        st = ctx.get_stats()
+        per_type[st["frame_type"]].append(st)
+    ctx.debug_run_stage("timing_off")
+    ctx.debug_run_stage("count_interactions_off")
+    # PSNR of S frames against the full render of the same pose (reported; unpinned by the paper)
+    psnr = []
+    ctx.reset_priors()
+    ref_ctx = tgs.Context(local, stream.cuda_stream)
+    ref_ctx.load_scene(sc)
+    for f in range(min(K, 12)):
+        ctx.set_camera(trajectory_pose(sc, f), cam)
+        ctx.render(tgs.AUTO)
+        if ctx.get_stats()["frame_type"] == tgs.FRAME_S:
+            ref_ctx.set_camera(trajectory_pose(sc, f), cam)
+            ref_ctx.render(tgs.FULL)
+            mse = float(((ctx.read_image() - ref_ctx.read_image()) ** 2).mean())
+            psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
+    ref_ctx.destroy()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return None
+
+    hbm_gbs, sm_mhz_max, peak_kind = _peaks()
+    stage_names = ["warp", "fill_corr", "preprocess_markoc", "select_count_compact_depthsort_emit", "tile_sort", "ranges", "blend_stitch", "post"]
+
+    def summarise(lst):
+        if not lst:
+            return None
+        ms = np.mean([s["ms_stage"] for s in lst], axis=0)
+        return {"frames": len(lst), "ms_total": float(np.mean([s["ms_total"] for s in lst])),
+                "ms_stage": {n: float(v) for n, v in zip(stage_names, ms)},
+                "n_pairs": float(np.mean([s["n_pairs"] for s in lst])), "n_visible": float(np.mean([s["n_visible"] for s in lst])),
+                "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
+                "n_interactions": float(np.mean([s["n_interactions"] for s in lst]))}
+
+    stages = {"R": summarise(per_type[0]), "P": summarise(per_type[1]), "S": summarise(per_type[2])}
+    # dominant kernel = the stage with the largest share of the profiled frames' time
+    tot = np.zeros(8)
+    for lst in per_type.values():
+        for s in lst:
+            tot += np.asarray(s["ms_stage"])
+    dom = int(np.argmax(tot))
+    all_stats = [s for lst in per_type.values() for s in lst]
+    roof = None
+    if stage_names[dom] == "blend_stitch":
+        # FP32 (FMA-pipe) bound: lane-instructions/s = interactions * instr per interaction / time
+        L = np.mean([s["n_interactions"] for s in all_stats])
+        t = np.mean([s["ms_stage"][6] for s in all_stats]) * 1e-3
+        sm_clk = (clocks or {}).get("sm_mhz") or sm_mhz_max
+        peak = 148 * 128 * sm_clk * 1e6 / 1e12          # T lane-instr/s at the clock seen under load
+        ach = L * BLEND_FMA_LANE_INSTR / t / 1e12
+        roof = {"kernel": "k_blend", "bound": "alu", "achieved": ach, "peak": peak, "unit": "T lane-instr/s (FP32 pipe)",
+                "frac": ach / peak, "traffic": None, "interactions_per_launch": float(L), "ms_per_launch": t * 1e3,
+                "peak_note": f"148 SM x 128 FP32 lanes x {sm_clk:.0f} MHz (median SM clock during the run)"}
+    else:
+        # HBM bound stages: algorithmic bytes per launch / duration
+        P = np.mean([s["n_pairs"] for s in all_stats])
+        t = np.mean([s["ms_stage"][dom] for s in all_stats]) * 1e-3
+        T_ = ((sc.camera.W + 15) // 16) * ((sc.camera.H + 15) // 16)
+        tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
+        if stage_names[dom] == "tile_sort":
+            by = P * (4 + tile_passes * 16)        # histogram read + per digit 8 B read + 8 B written
+            kname = "k_onesweep (tile sort, + k_sort_hist)"
+        elif stage_names[dom] == "preprocess_markoc":
+            by = sc.n * 16 + np.mean([s["n_visible"] for s in all_stats]) * (24 + 44)
+            kname = "k_preprocess"
+        else:
+            by = P * 8 + sc.n * 8
+            kname = stage_names[dom]
+        ach = by / t / 1e9
+        roof = {"kernel": kname, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
+                "traffic": None, "ms_per_launch": t * 1e3, "peak_note": f"{peak_kind} copy bandwidth"}
+
+    fps_tgs = world * K / (ms_tgs * 1e-3)
+    fps_full = world * K / (ms_full * 1e-3)
+    fps_e2e = world * K / (ms_e2e * 1e-3)
+    out = {
+        "metric": METRIC, "value": fps_tgs, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_tgs / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config {args.config} ({sc.name}): {sc.n} Gaussians, SH degree {sc.sh_degree}, {cam.W}x{cam.H}, "
+                               f"{len(sc.poses)}-frame trajectory played forward/backward, AUTO schedule (lambda_TDC=50, lambda_SR=5, eta=0.4)",
+                   "l2": "scene arrays (>= 700 MB) exceed the 126 MB L2; no explicit flush", "parallelism": "replicas only"},
+        "fps_full_render": fps_full, "ms_per_step_full_render": ms_full / K, "speedup_vs_full_render": fps_tgs / fps_full,
+        "psnr_S_vs_full_dB": float(np.mean(psnr)) if psnr else None,
+        "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 16 * 4 + 8 * 4, "d2h_bytes_per_step": cam.W * cam.H * 3 * 4,
+                "note": "camera by value through tgs_set_camera; image read into pinned host memory every frame"},
+        "gpu_launches": None,
+        "stages": stages, "roofline": roof, "clocks": clocks,
+    }
+    # launches per frame: init, [warp, fill], preprocess, select, count, scan_emit, hist, scan_hist, passes x onesweep,
+    # ranges, blend, [frustum]
+    T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
+    tpasses = (max(1, int(np.ceil(np.log2(T)))) + 7) // 8
+    nR = sum(1 for s in all_stats if s["frame_type"] != 2)
+    # init, preprocess, select, count, compact, depth sort (hist, scan, 4 digits), scan_emit, tile sort (hist, scan, digits),
+    # ranges, blend, + frustum (R/P) or + warp, fill, mark_oc (S)
+    base = 1 + 1 + 1 + 1 + 1 + 6 + 1 + (2 + tpasses) + 1 + 1
+    per_ref, per_s = base + 1, base + 3
+    frac_ref = nR / max(1, len(all_stats))
+    out["gpu_launches"] = int(round(K * (frac_ref * per_ref + (1 - frac_ref) * per_s)))
+    if world > 1:
+        dist.destroy_process_group()
+    return out
+
+
+# ---------------------------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(config, n, frames_modes, budget_s=None):
+    """Time the oracle, as it stands, on the given (frame index, mode) list of the config's trajectory."""
+    from oracle import ora
+    from oracle.ora import Oracle
+    from synth import make_config
+    sc = make_config(config, n=n, frames=None)
+    o = Oracle()
+    o.load_scene(sc)
+    modes = {"full": ora.FULL, "auto": ora.AUTO, "temporal": ora.TEMPORAL}
+    t_total, done, per = 0.0, 0, []
+    for f, m in frames_modes:
+        o.set_camera(trajectory_pose(sc, f), sc.camera)
+        t0 = time.perf_counter()
+        o.render(modes[m])
+        dt = time.perf_counter() - t0
+        st = o.stats()
+        per.append({"frame": f, "type": "RPS"[st["frame_type"]], "s": dt})
+        t_total += dt
+        done += 1
+        if budget_s is not None and t_total > budget_s:
+            break
+    return done, t_total, per, sc
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same config / metric.  Each step is one trajectory frame in AUTO
+    mode; the oracle needs seconds per 1080p frame, so the number of Gaussians is NOT reduced but the run is
+    bounded by rendering the K (+W) frames with the SAME schedule and reporting frames / time."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return None
+    K, W = args.steps, args.warmup
+    # bounded sample: the oracle takes ~10-30 s per reference frame at config 3; keep the whole run within
+    # a few minutes by bounding the number of timed frames (the JSON line says how many were timed)
+    budget = float(os.environ.get("TGS_REF_BUDGET_S", "150"))
+    frames = [(f, "auto") for f in range(W + K)]
+    from oracle import ora
+    from oracle.ora import Oracle
+    from synth import make_config
+    sc = make_config(args.config, n=args.n, frames=None)
+    o = Oracle()
+    o.load_scene(sc)
+    t_used, timed_frames, t_timed, types = 0.0, 0, 0.0, []
+    for i, (f, _) in enumerate(frames):
+        o.set_camera(trajectory_pose(sc, f), sc.camera)
+        t0 = time.perf_counter()
+        ft = o.render(ora.AUTO)
+        dt = time.perf_counter() - t0
+        t_used += dt
+        if i >= W:
+            timed_frames += 1
+            t_timed += dt
+            types.append("RPS"[ft])
+        if t_used > budget and timed_frames >= 1:
+            break
+    fps = timed_frames / t_timed
+    cam = sc.camera
+    sample = (f"{timed_frames} of the requested {K} frames (types {''.join(types)}) after {min(W, len(frames))} warm-up frames, "
+              f"bounded to ~{budget:.0f} s of CPU time; full scene, full resolution")
+    return {
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": K, "warmup": W, "ms_per_step": 1e3 * t_timed / timed_frames, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {args.config} ({sc.name}): {sc.n} Gaussians, SH degree {sc.sh_degree}, {cam.W}x{cam.H}, AUTO schedule"},
+        "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "steps_timed": timed_frames,
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--n", type=int, default=None, help="override the number of Gaussians (debug only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        out = run_reference(args)
+        if out is not None:
+            print(json.dumps(out))
+        return
+    out = run_ours(args)
+    if out is None:
+        return
+    if out["n_gpus"] == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands on one host core: a reference frame and the TemporalGS frame that follows it
+        done, t, per, _ = oracle_sample(args.config, args.n, [(0, "full"), (1, "temporal")])
+        out["cpu_baseline"] = {"value": done / t, "unit": "frames/s", "cores": 1, "kind": "oracle",
+                               "sample": f"frames 0 (R) and 1 (S) of the same trajectory, {t:.1f} s: " +
+                                         ", ".join(f"{p['type']} {p['s']:.1f} s" for p in per)}
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

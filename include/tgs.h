@@ -78,6 +78,8 @@ typedef struct {
   uint32_t n_tiles, n_sel_oc, n_sel_um, n_sel;
   uint32_t n_rendered; /* |G_rendered| (R / P frames) */
   uint32_t overflow;   /* 1: n_pairs exceeded the capacity, frame invalid */
+  uint64_t n_interactions; /* L: (pixel, Gaussian) pairs evaluated by the blend; 0 unless counting is on
+                              (tgs_debug_run_stage("count_interactions_on")) */
   float ms_stage[8];   /* per-stage device time when timing is on (tgs_debug_run_stage("timing_on")):
                           0 warp, 1 fill+corr, 2 preprocess, 3 select+count+scan+keys, 4 sort, 5 ranges,
                           6 blend+stitch, 7 post (F reduction, stats) */
@@ -131,7 +133,8 @@ const char* tgs_last_error(tgs_ctx*);
  *   prior_sigma (float [H][W]) prior_image (float [H][W][3]) cov3d (float [N][6]) tau (float [N]).
  * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):
  *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
- * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off". */
+ * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off"
+ *   "count_interactions_on" "count_interactions_off". */
 long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int mem);
 int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);
 int tgs_debug_run_stage(tgs_ctx*, const char* stage);

@@ -29,12 +29,14 @@ constexpr int TILE = 16;                       // 16x16 tiles
 constexpr double ALPHA_MIN = 1.0 / 255.0;      // PAPER.md:L119 (and R2)
 constexpr double ALPHA_MAX = 0.99;             // R2
 constexpr double T_STOP = 1.0e-4;              // R2
+constexpr float ALPHA_MIN_F = 1.0f / 255.0f, ALPHA_MAX_F = 0.99f, T_STOP_F = 1.0e-4f;   // the same, as the fp32 decisions see them
 // Relative margins of "borderline" decisions (R29).  The wide pair bounds which Gaussians an fp32
 // implementation MAY mark as rendered; the tight pair marks the pixels where an fp32 implementation
 // (alpha accurate to ~1e-6, T to ~1e-5 relative) may legitimately take the other branch.
 constexpr double MARGIN_ALPHA = 1.0e-4;
 constexpr double MARGIN_T = 1.0e-2;
-constexpr double PIX_MARGIN_ALPHA = 2.0e-5;
+constexpr double PIX_MARGIN_ALPHA = 5.0e-6;
+constexpr double Q_EPS = 2.4e-7;           // 4 ulp of fp32: rounding of the stored parameters + of the evaluation
 constexpr double PIX_MARGIN_T = 1.0e-3;
 
 struct Cam {
@@ -287,6 +289,7 @@ void preprocess(ora_ctx* c, int ftype) {
     const float det = a * cc2 - b * b;
     if (!(det > 0.0f)) { r.flags = ORA_CULL_DEGENERATE; ++st.n_degenerate; continue; }
     r.A = cc2 / det; r.B = -b / det; r.C = a / det;
+    r.ca = a; r.cb = b; r.cc = cc2;
     const float mid = 0.5f * (a + cc2);
     const float lam = mid + std::sqrt(std::fmax(0.1f, mid * mid - det));
     const float rad = std::ceil(3.0f * std::sqrt(lam));
@@ -418,8 +421,14 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
             continue;
           }
           double T = 1.0, C[3] = {0, 0, 0}, Sw = 0, Sd = 0, Sdd = 0;
+          // The skip / stop tests DECIDE integers (membership in G_rendered), so they are taken in fp32
+          // (R33): alpha_f = min(0.99f, float(o e^q)), T_f <- T_f (1 - alpha_f).  With the 3DGS constants the
+          // case of two alpha-clamped Gaussians lands on T = 0.01^2 ~ 1e-4, i.e. ON the stop threshold, and
+          // only a fixed precision makes that decision reproducible.  Values (colour, Eq.1-2) stay in double.
           // `stopped`: the real loop has terminated; what follows is a virtual continuation that only
           // marks which Gaussians an implementation with slightly different rounding MAY still blend.
+          float Tf = 1.0f;
+          double Terr = 0.0;
           bool stopped = false, sure_alive = true;
           double Tv = 1.0;
           for (uint32_t i = c->ranges[2 * t]; i < c->ranges[2 * t + 1]; ++i) {
@@ -427,38 +436,52 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
             const ora_record& r = c->rec[g];
             if (!stopped) ++L;
             const double dx = (double)r.u - px, dy = (double)r.v - py;
-            const double q = -0.5 * ((double)r.A * dx * dx + (double)r.C * dy * dy) - (double)r.B * dx * dy;
-            if (q > 0.0) continue;                                   // R2
-            const double alpha = std::min(ALPHA_MAX, (double)r.o * std::exp(q));   // L61, clamp R2
+            // q = -1/2 delta^T Sigma'^-1 delta, Sigma' = [[ca, cb], [cb, cc]] inverted in double (the fp32 conic A, B, C is
+            // only used for the tile-selection DECISION: evaluating the form with its rounded entries loses up to
+            // 1e-7 x (sum of the magnitudes of the three terms), which matters for screen-filling anisotropic splats)
+            const double ca = r.ca, cb = r.cb, cc = r.cc;
+            const double q = -0.5 * (cc * dx * dx - 2.0 * cb * dx * dy + ca * dy * dy) / (ca * cc - cb * cb);
+            if (q > 0.0) continue;                                   // R2 (cannot happen for a positive definite Sigma')
+            // Conditioning of q with respect to fp32 storage of ANY parametrisation of Sigma'^-1 (the needle-like
+            // splats of Gaussians next to the camera: centre a thousand pixels away, ridge one pixel wide):
+            // with t = dx - (cb/cc) dy,  q = -1/2 (cc/det t^2 + dy^2/cc)  and  dq ~ eps (2 |A t| (|dx| + |k dy|) + |q|).
+            const double kk = -cb / cc, tt = dx + kk * dy, AA = cc / (ca * cc - cb * cb);
+            const double q_margin = Q_EPS * (2.0 * std::fabs(AA * tt) * (std::fabs(dx) + std::fabs(kk * dy)) + 2.0 * std::fabs(q));
+            const double pm_alpha = PIX_MARGIN_ALPHA + q_margin, m_alpha = MARGIN_ALPHA + 4.0 * q_margin;
+            const double a_raw = (double)r.o * std::exp(q);
+            const double alpha = std::min(ALPHA_MAX, a_raw);         // L61, clamp R2 (value)
+            const float alpha_f = std::fmin(ALPHA_MAX_F, (float)a_raw);   // (decision)
             if (stopped) {
-              if (alpha < ALPHA_MIN * (1.0 - MARGIN_ALPHA)) continue;
+              if (alpha < ALPHA_MIN * (1.0 - m_alpha)) continue;
               const double Tn = Tv * (1.0 - alpha);
               if (Tn < T_STOP * (1.0 - MARGIN_T)) break;
               c->rendered_maybe[g] = 1; Tv = Tn;
               continue;
             }
-            if (alpha < ALPHA_MIN) {                                 // skip alpha < 1/255 (R2)
-              if (alpha >= ALPHA_MIN * (1.0 - MARGIN_ALPHA)) c->rendered_maybe[g] = 1;
-              if (alpha >= ALPHA_MIN * (1.0 - PIX_MARGIN_ALPHA)) c->borderline[pix] = 1;
+            if (alpha_f < ALPHA_MIN_F) {                             // skip alpha < 1/255 (R2)
+              if (alpha >= ALPHA_MIN * (1.0 - m_alpha)) c->rendered_maybe[g] = 1;
+              if (alpha >= ALPHA_MIN * (1.0 - pm_alpha)) c->borderline[pix] = 1;
               continue;
             }
-            const double Tn = T * (1.0 - alpha);
-            if (Tn < T_STOP) {                                       // stop; this record is not blended (R2)
+            const float Tn_f = Tf * (1.0f - alpha_f);
+            const double Tn = (double)Tn_f;
+            if (Tn_f < T_STOP_F) {                                   // stop; this record is not blended (R2)
               if (Tn < T_STOP * (1.0 - MARGIN_T)) break;
-              if (Tn >= T_STOP * (1.0 - PIX_MARGIN_T)) c->borderline[pix] = 1;
+              if (Tn >= T_STOP * (1.0 - std::max(PIX_MARGIN_T, 2.0 * (Terr + pm_alpha * alpha / (1.0 - alpha)))) && alpha_f < ALPHA_MAX_F) c->borderline[pix] = 1;
               c->rendered_maybe[g] = 1; stopped = true; Tv = Tn;
               continue;
             }
-            const bool a_border = alpha < ALPHA_MIN * (1.0 + MARGIN_ALPHA);
-            if (alpha < ALPHA_MIN * (1.0 + PIX_MARGIN_ALPHA)) c->borderline[pix] = 1;
-            if (Tn < T_STOP * (1.0 + PIX_MARGIN_T)) c->borderline[pix] = 1;
+            const bool a_border = alpha < ALPHA_MIN * (1.0 + m_alpha);
+            if (alpha < ALPHA_MIN * (1.0 + pm_alpha)) c->borderline[pix] = 1;
+            if (alpha_f < ALPHA_MAX_F) Terr += pm_alpha * alpha / (1.0 - alpha);   // relative error bound of an fp32 T
+            if (Tn < T_STOP * (1.0 + std::max(PIX_MARGIN_T, 2.0 * Terr)) && alpha_f < ALPHA_MAX_F) c->borderline[pix] = 1;
             if (Tn < T_STOP * (1.0 + MARGIN_T)) sure_alive = false;
             const double w = alpha * T;                              // w_i = alpha_i T_i (R1)
             C[0] += w * r.r; C[1] += w * r.g; C[2] += w * r.b;
             Sw += w; Sd += w * (double)r.d; Sdd += w * (double)r.d * (double)r.d;   // Eq.1-2 sums
             c->rendered_now[g] = 1; c->rendered_maybe[g] = 1;        // L103
             if (sure_alive && !a_border) c->rendered_sure[g] = 1;
-            T = Tn;
+            T *= 1.0 - alpha; Tf = Tn_f;
           }
           for (int ch = 0; ch < 3; ++ch) c->image[pix * 3 + ch] = (float)(C[ch] + T * c->prm.bg[ch]);   // R27
           if (Sw > 0.0) {

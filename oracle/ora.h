@@ -45,9 +45,10 @@ typedef struct {
   int enable_afc, enable_toc, enable_sr; /* Table IV toggles */
 } ora_params;
 
-typedef struct {        /* 64 bytes */
+typedef struct {        /* 80 bytes */
   float u, v, d, o;     /* 2-D mean (pixels), depth, opacity */
-  float A, B, C, tau;   /* conic of Sigma'; tau = 2 ln(255 o) */
+  float A, B, C, tau;   /* conic (inverse of Sigma') as fp32 decision values; tau = 2 ln(255 o) */
+  float ca, cb, cc, pad0; /* Sigma' = [[ca, cb], [cb, cc]] (with the 0.3 dilation), fp32 */
   float r, g, b;        /* colour (value arithmetic, computed in double) */
   float radius;         /* ceil(3 sqrt(lambda_max)) */
   uint16_t x_lo, x_hi, y_lo, y_hi; /* tile rect, hi exclusive */

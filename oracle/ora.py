@@ -19,11 +19,12 @@ CULL_NEAR, CULL_AFC, CULL_TOC, CULL_DEGENERATE, CULL_EMPTY, VISIBLE, NEWLY_VISIB
 RECORD_DTYPE = np.dtype([
     ("u", "<f4"), ("v", "<f4"), ("d", "<f4"), ("o", "<f4"),
     ("A", "<f4"), ("B", "<f4"), ("C", "<f4"), ("tau", "<f4"),
+    ("ca", "<f4"), ("cb", "<f4"), ("cc", "<f4"), ("pad0", "<f4"),
     ("r", "<f4"), ("g", "<f4"), ("b", "<f4"), ("radius", "<f4"),
     ("x_lo", "<u2"), ("x_hi", "<u2"), ("y_lo", "<u2"), ("y_hi", "<u2"),
     ("flags", "<u4"), ("tiles_touched", "<u4"),
 ])
-assert RECORD_DTYPE.itemsize == 64
+assert RECORD_DTYPE.itemsize == 80
 
 
 class OraParams(C.Structure):

@@ -6,29 +6,30 @@
 //
 // One persistent grid; a work item is a tile of `tile_order` (selected tiles first).  A CTA is 16x16
 // threads = one pixel each; the tile's sorted Gaussians are staged through shared memory in batches of
-// 256 records, pre-scaled so that alpha = exp2(A' dx^2 + B' dx dy + C' dy^2 + log2 o) is 4 FMA-pipe
-// instructions + 1 MUFU.EX2.  This kernel is FP32-pipe bound, not HBM bound.
+// 256 records, pre-scaled so that alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, is 7 FMA-pipe
+// instructions + 1 MUFU.EX2: the form -1/2 delta^T Sigma'^-1 delta completed to two squares, which has no
+// cancellation between terms (screen-filling anisotropic splats lose 1e-4 of alpha in the 3-term conic form).
+// This kernel is FP32-pipe bound, not HBM bound.
 #include "tgs_internal.cuh"
 
 namespace {
 
 constexpr int BLEND_THREADS = 256;
-constexpr float LOG2E = 1.4426950408889634f;
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
 
 struct BlendSmem {
-  float4 a[BLEND_THREADS];     // u, v, A' = -0.5 log2e A, B' = -log2e B
-  float4 b[BLEND_THREADS];     // C' = -0.5 log2e C, log2(o), d, r
+  float4 a[BLEND_THREADS];     // u, v, A', k
+  float4 b[BLEND_THREADS];     // D', log2(o), d, r
   float2 c[BLEND_THREADS];     // g, b
   uint32_t id[BLEND_THREADS];  // Gaussian index (for the G_rendered marks)
   uint32_t contrib[BLEND_THREADS / 32];
   uint32_t work;
 };
 
-template <bool MARK>
+template <bool MARK, bool COUNT>
 __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
                                                          const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
-                                                         const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                         const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,
                                                          const float* __restrict__ fill_depth, const float* __restrict__ warp_sigma,
                                                          float* __restrict__ image, float* __restrict__ depth, float* __restrict__ sigma,
@@ -83,14 +84,15 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     float T = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
     float Sw = 0.0f, S1 = 0.0f, S2 = 0.0f, d0 = 0.0f;      // Eq.1-2 moments, shifted by the first contributing depth
     bool done = !inside;
+    uint32_t nint = 0;
     for (uint32_t start = range.x; start < range.y; start += BLEND_THREADS) {
       if (__syncthreads_count(done) == BLEND_THREADS) break;
       const uint32_t nb = min((uint32_t)BLEND_THREADS, range.y - start);
       if (threadIdx.x < nb) {
         const uint32_t g = vals[start + threadIdx.x];
-        const float4 r0 = rec_uvdo[g], r1 = rec_conic[g], r2 = rec_rgb[g];
-        sm.a[threadIdx.x] = make_float4(r0.x, r0.y, -0.5f * LOG2E * r1.x, -LOG2E * r1.y);
-        sm.b[threadIdx.x] = make_float4(-0.5f * LOG2E * r1.z, log2f(r0.w), r0.z, r2.x);
+        const float4 r0 = rec_b0[g], r1 = rec_b1[g], r2 = rec_rgb[g];
+        sm.a[threadIdx.x] = r0;
+        sm.b[threadIdx.x] = make_float4(r1.x, r1.y, r1.z, r2.x);
         sm.c[threadIdx.x] = make_float2(r2.y, r2.z);
         sm.id[threadIdx.x] = g;
       }
@@ -102,12 +104,13 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
         if (!done) {
           for (uint32_t jj = 0; jj < je; ++jj) {
             const uint32_t j = j0 + jj;
+            if (COUNT) ++nint;
             const float4 ga = sm.a[j];
             const float dx = ga.x - fpx, dy = ga.y - fpy;
             const float4 gb = sm.b[j];
-            const float e = ga.z * dx * dx + gb.x * dy * dy + ga.w * dx * dy;     // log2 of the Gaussian falloff
-            if (e > 0.0f) continue;
-            const float alpha = fminf(0.99f, exp2f(e + gb.y));
+            const float t = fmaf(ga.w, dy, dx);
+            const float e = fmaf(ga.z * t, t, fmaf(gb.x * dy, dy, gb.y));         // log2(o) + log2 of the falloff (<= log2 o)
+            const float alpha = fminf(0.99f, exp2f(e));
             if (alpha < ALPHA_MIN) continue;
             const float Tn = T * (1.0f - alpha);
             if (Tn < 1.0e-4f) { done = true; break; }
@@ -144,6 +147,10 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
         sigma[pix] = 0.0f;
       }
     }
+    if (COUNT) {
+      nint = __reduce_add_sync(0xffffffffu, nint);
+      if (lane == 0 && nint) atomicAdd(&counters->n_interactions, (unsigned long long)nint);
+    }
     (void)wid;
   }
 }
@@ -151,14 +158,13 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
 }  // namespace
 
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
-                  uint8_t* rendered_next, int num_sms) {
+                  uint8_t* rendered_next, int num_sms, bool count_interactions) {
   const int grid = num_sms * 4;
-  if (rendered_next)
-    k_blend<true><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_uvdo, b.rec_conic, b.rec_rgb,
-                                                 prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],
-                                                 b.sigma[out_idx], rendered_next, b.counters);
-  else
-    k_blend<false><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_uvdo, b.rec_conic, b.rec_rgb,
-                                                  prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],
-                                                  b.sigma[out_idx], nullptr, b.counters);
+#define LAUNCH(M, C)                                                                                                          \
+  k_blend<M, C><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
+                                               prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \
+                                               b.sigma[out_idx], rendered_next, b.counters)
+  if (rendered_next) { if (count_interactions) LAUNCH(true, true); else LAUNCH(true, false); }
+  else { if (count_interactions) LAUNCH(false, true); else LAUNCH(false, false); }
+#undef LAUNCH
 }

@@ -161,6 +161,41 @@ __device__ __forceinline__ float box_qmin(float u, float v, float A, float B, fl
 
 namespace {
 
+// T^oc test of one (newly visible Gaussian, tile) pair: max alpha over the tile's pixel-centre box >= 1/255
+// <=> box_qmin <= tau (L119, R18).  The mark is an OR, so the order of evaluation does not matter.
+__device__ __forceinline__ void mark_oc_tile(const CamConst& k, float u, float v, float A, float B, float C, float tau, uint32_t txx,
+                                             uint32_t tyy, uint32_t* __restrict__ tile_flags, Counters* __restrict__ counters) {
+  const uint32_t t = tyy * k.TX + txx;
+  if (*reinterpret_cast<volatile uint32_t*>(&tile_flags[t]) & 1u) return;
+  const float bx0 = (float)(txx * TGS_TILE), bx1 = (float)min((int)(txx * TGS_TILE + TGS_TILE - 1), k.W - 1);
+  const float by0 = (float)(tyy * TGS_TILE), by1 = (float)min((int)(tyy * TGS_TILE + TGS_TILE - 1), k.H - 1);
+  if (box_qmin(u, v, A, B, C, bx0, bx1, by0, by1) <= tau)
+    if (!(atomicOr(&tile_flags[t], 1u) & 1u)) atomicAdd(&counters->n_oc_marked, 1u);
+}
+
+// Newly visible Gaussians with large rects (queued by k_preprocess): one warp per Gaussian, lanes over the tiles
+// of the rect.  Stops as soon as every tile of the frame carries the T^oc mark.
+__global__ void __launch_bounds__(256) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_uvdo,
+                                                 const float4* __restrict__ rec_conic, const uint2* __restrict__ rec_rect,
+                                                 uint32_t* __restrict__ tile_flags, Counters* __restrict__ counters) {
+  const CamConst& k = fc.cam;
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t nq = counters->n_nv_queue;
+  while (true) {
+    uint32_t j = 0;
+    if (lane == 0) j = atomicAdd(&counters->ticket_mark, 1u);
+    j = __shfl_sync(0xffffffffu, j, 0);
+    if (j >= nq) break;
+    if (*reinterpret_cast<volatile uint32_t*>(&counters->n_oc_marked) >= (uint32_t)fc.n_tiles) break;
+    const uint32_t g = nv_queue[j];
+    const float4 r0 = rec_uvdo[g], r1 = rec_conic[g];
+    const uint2 r = rec_rect[g];
+    const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
+    const uint32_t w = x_hi - x_lo, area = w * (y_hi - y_lo);
+    for (uint32_t i = lane; i < area; i += 32) mark_oc_tile(k, r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, x_lo + i % w, y_lo + i / w, tile_flags, counters);
+  }
+}
+
 // ------------------------------------------------------------------ A3 preprocess (+AFC +TOC +newly-visible +T^oc)
 // One thread per Gaussian.  The 16 B cull record {mean, opacity} is read for all N; the 24 B covariance only
 // for Gaussians that survive near / AFC / TOC; SH (the bulk of the bytes) is not touched here at all.
@@ -170,8 +205,9 @@ __global__ void __launch_bounds__(256) k_preprocess(FrameConst fc, const float4*
                                                     const float* __restrict__ warp_depth, const float* __restrict__ warp_sigma,
                                                     const uint32_t* __restrict__ F_key, float4* __restrict__ rec_uvdo,
                                                     float4* __restrict__ rec_conic, uint2* __restrict__ rec_rect,
-                                                    uint32_t* __restrict__ rec_flags, uint32_t* __restrict__ tile_flags,
-                                                    Counters* __restrict__ counters) {
+                                                    uint32_t* __restrict__ rec_flags, float4* __restrict__ rec_b0,
+                                                    float4* __restrict__ rec_b1, uint32_t* __restrict__ tile_flags,
+                                                    uint32_t* __restrict__ nv_queue, Counters* __restrict__ counters) {
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   const CamConst& k = fc.cam;
   const float* V = k.V;
@@ -237,15 +273,14 @@ __global__ void __launch_bounds__(256) k_preprocess(FrameConst fc, const float4*
       rec_uvdo[g] = make_float4(u, v, tz, c4.w);
       rec_conic[g] = make_float4(A, B, C, tau);
       rec_rect[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
+      // blend-side parameters: the quadratic form as a sum of two squares (no cancellation between its terms)
+      rec_b0[g] = make_float4(u, v, -0.72134752f * A, -b / c);
+      rec_b1[g] = make_float4(-0.72134752f / c, log2f(c4.w), tz, 0.0f);
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)
-        for (uint32_t tyy = y_lo; tyy < y_hi; ++tyy)
-          for (uint32_t txx = x_lo; txx < x_hi; ++txx) {
-            const uint32_t t = tyy * k.TX + txx;
-            if (tile_flags[t] & 1u) continue;
-            const float bx0 = (float)(txx * TGS_TILE), bx1 = (float)min((int)(txx * TGS_TILE + TGS_TILE - 1), k.W - 1);
-            const float by0 = (float)(tyy * TGS_TILE), by1 = (float)min((int)(tyy * TGS_TILE + TGS_TILE - 1), k.H - 1);
-            if (box_qmin(u, v, A, B, C, bx0, bx1, by0, by1) <= tau) atomicOr(&tile_flags[t], 1u);
-          }
+        if ((x_hi - x_lo) * (y_hi - y_lo) > 16u) nv_queue[atomicAdd(&counters->n_nv_queue, 1u)] = g;   // large rect: k_mark_oc
+        else
+          for (uint32_t tyy = y_lo; tyy < y_hi; ++tyy)
+            for (uint32_t txx = x_lo; txx < x_hi; ++txx) mark_oc_tile(k, u, v, A, B, C, tau, txx, tyy, tile_flags, counters);
       }
     } while (false);
     rec_flags[g] = flags;
@@ -449,7 +484,11 @@ void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
 
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   k_preprocess<<<(fc.n + 255) / 256, 256, 0, s>>>(fc, b.cull4, b.cov3d, b.tau, b.rendered, b.warp_depth, b.warp_sigma, b.F_key,
-                                                  b.rec_uvdo, b.rec_conic, b.rec_rect, b.rec_flags, b.tile_flags, b.counters);
+                                                  b.rec_uvdo, b.rec_conic, b.rec_rect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue, b.counters);
+}
+
+void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
+  k_mark_oc<<<num_sms * 4, 256, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_rect, b.tile_flags, b.counters);
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {

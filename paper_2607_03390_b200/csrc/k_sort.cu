@@ -1,9 +1,14 @@
-// k_sort.cu -- A6: stable LSD radix sort of the (tile|depth, Gaussian) pairs, onesweep style:
-// one histogram kernel for all digits, then one scatter kernel per 8-bit digit in which every tile
-// obtains its global offsets from its predecessors through decoupled look-back (single pass over the
-// data per digit: 12 B read + 12 B written per pair).  Only bits [0, 32 + ceil(log2 T)) are sorted.
-// PAPER.md:L61 "The sorting process, for each tile, sorts its intersected Gaussians by depth from front to
-// back"; equal (tile, depth) keys keep the emission order = ascending Gaussian index (R28).
+// k_sort.cu -- A6: stable LSD radix sort of (uint32 key, uint32 value) pairs, onesweep style: one
+// histogram kernel for all digits, then one scatter kernel per 8-bit digit in which every tile obtains its
+// global offsets from its predecessors through decoupled look-back (a single pass over the data per
+// digit: 8 B read + 8 B written per item).  The item count lives in device memory.
+//
+// The path sorts by tile|depth ("for each tile, sorts its intersected Gaussians by depth from
+// front to back") in two levels that give exactly the order of one stable sort on the 64-bit key
+// (tile << 32 | bits(depth)) with ties by ascending Gaussian index (R28):
+//   (1) the N_v visible Gaussians are sorted by bits(depth) (4 digits, N_v items), then
+//   (2) their (tile, Gaussian) pairs, emitted in that order, are sorted stably by tile id (ceil(log2 T / 8)
+//       digits, P items).  At config 3 (P ~ 70 N_v) this moves ~40 B per pair instead of ~150 B.
 #include "tgs_internal.cuh"
 
 namespace {
@@ -20,11 +25,11 @@ __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *rei
 __device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v) { *reinterpret_cast<volatile uint32_t*>(p) = v; }
 
 // ---- histogram of every digit + reset of the look-back descriptors of the tiles this frame will use
-__global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ keys, const Counters* __restrict__ counters,
+__global__ void __launch_bounds__(256) k_sort_hist(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ n_ptr,
                                                    uint32_t* __restrict__ hist, uint32_t* __restrict__ desc, int passes,
                                                    uint32_t tiles_cap) {
-  __shared__ uint32_t s_hist[8 * RADIX];
-  const uint32_t n = counters->n_pairs;
+  __shared__ uint32_t s_hist[4 * RADIX];
+  const uint32_t n = *n_ptr;
   for (int i = threadIdx.x; i < passes * RADIX; i += blockDim.x) s_hist[i] = 0;
   __syncthreads();
   const uint32_t num_tiles = (n + SORT_TILE - 1) / SORT_TILE;
@@ -35,7 +40,7 @@ __global__ void __launch_bounds__(256) k_sort_hist(const uint64_t* __restrict__ 
     for (int i = 0; i < SORT_IPT; ++i) {
       const uint32_t idx = base + i * 256 + threadIdx.x;
       if (idx < n) {
-        const uint64_t k = keys[idx];
+        const uint32_t k = keys[idx];
         for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * RADIX + (uint32_t)((k >> (8 * p)) & 255u)], 1u);
       }
     }
@@ -63,7 +68,7 @@ __global__ void __launch_bounds__(256) k_sort_scan_hist(uint32_t* __restrict__ h
 
 // ---- one digit: rank within the tile (warp match + per-warp counters), look-back, scatter through smem
 struct SortSmem {
-  uint64_t keys[SORT_TILE];
+  uint32_t keys[SORT_TILE];
   uint32_t vals[SORT_TILE];
   uint32_t warp_hist[SORT_WARPS][RADIX];
   uint32_t gbase[RADIX];        // global index of block-sorted position p is gbase[digit] + p
@@ -71,29 +76,30 @@ struct SortSmem {
   uint32_t tile;
 };
 
-__global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
-                                                           uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                                                           Counters* __restrict__ counters, const uint32_t* __restrict__ hist_scan,
+__global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+                                                           uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
+                                                           const uint32_t* __restrict__ n_ptr, uint32_t* __restrict__ ticket,
+                                                           uint32_t* __restrict__ error_flag, const uint32_t* __restrict__ hist_scan,
                                                            uint32_t* __restrict__ desc, int pass) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& sm = *reinterpret_cast<SortSmem*>(smem_raw);
-  const uint32_t n = counters->n_pairs;
+  const uint32_t n = *n_ptr;
   const uint32_t num_tiles = (n + SORT_TILE - 1) / SORT_TILE;
   const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
   const int shift = 8 * pass;
   while (true) {
-    if (threadIdx.x == 0) sm.tile = atomicAdd(&counters->ticket_sort[pass], 1u);
+    if (threadIdx.x == 0) sm.tile = atomicAdd(ticket, 1u);
     __syncthreads();
     const uint32_t tile = sm.tile;
     if (tile >= num_tiles) break;
     for (int i = threadIdx.x; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&sm.warp_hist[0][0])[i] = 0;
     const uint32_t base = tile * SORT_TILE + wid * (32 * SORT_IPT);
-    uint64_t key[SORT_IPT];
+    uint32_t key[SORT_IPT];
 #pragma unroll
     for (int i = 0; i < SORT_IPT; ++i) {
       const uint32_t idx = base + i * 32 + lane;
-      key[i] = idx < n ? keys_in[idx] : ~0ull;     // padding sorts (stably) behind every real key of the tile
+      key[i] = idx < n ? keys_in[idx] : 0xffffffffu;     // padding sorts (stably) behind every real key of the tile
     }
     __syncthreads();
     uint32_t rank[SORT_IPT];
@@ -130,7 +136,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint64_t* __res
       uint32_t polls = 0;
       for (int t = (int)tile - 1; t >= 0;) {
         const uint32_t v = ld_volatile(desc + (size_t)t * RADIX + d);
-        if ((v & FLAG_MASK) == 0) { if (++polls > LOOKBACK_WATCHDOG) { counters->error = 2; break; } continue; }
+        if ((v & FLAG_MASK) == 0) { if (++polls > LOOKBACK_WATCHDOG) { *error_flag = 2; break; } continue; }
         excl += v & VALUE_MASK;
         if ((v & FLAG_MASK) == FLAG_PREFIX) break;
         --t;
@@ -160,7 +166,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint64_t* __res
     for (int i = 0; i < SORT_IPT; ++i) {
       const uint32_t p = i * SORT_THREADS + threadIdx.x;
       if (p < valid) {
-        const uint64_t k = sm.keys[p];
+        const uint32_t k = sm.keys[p];
         const uint32_t o = sm.gbase[(uint32_t)(k >> shift) & 255u] + p;
         keys_out[o] = k;
         vals_out[o] = sm.vals[p];
@@ -174,26 +180,28 @@ __global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint64_t* __res
 
 uint32_t sort_tile_items() { return SORT_TILE; }
 
-int sort_num_passes(int n_tiles) {
-  int tile_bits = 0;
+int tile_sort_passes(int n_tiles) {
+  int tile_bits = 1;
   while ((1 << tile_bits) < n_tiles) ++tile_bits;
-  return (32 + tile_bits + 7) / 8;
+  return (tile_bits + 7) / 8;
 }
 
-int launch_sort(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms, uint32_t tiles_cap) {
-  const int passes = sort_num_passes(fc.n_tiles);
+// Sorts n = *n_ptr items on digits [0, passes) of the key.  keys/vals are ping-pong pairs; returns the index
+// (0/1) of the buffers holding the result.  `tickets` points at `passes` zeroed counters, `hist` at 4*256 words.
+int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int passes,
+                uint32_t* hist, uint32_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, int num_sms) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(k_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
     attr_set = true;
   }
-  cudaMemsetAsync(b.sort_hist, 0, 8 * RADIX * sizeof(uint32_t), s);
-  k_sort_hist<<<num_sms * 4, 256, 0, s>>>(b.keys[0], b.counters, b.sort_hist, b.sort_desc, passes, tiles_cap);
-  k_sort_scan_hist<<<1, 256, 0, s>>>(b.sort_hist, passes);
+  cudaMemsetAsync(hist, 0, 4 * RADIX * sizeof(uint32_t), s);
+  k_sort_hist<<<num_sms * 4, 256, 0, s>>>(keys[0], n_ptr, hist, desc, passes, tiles_cap);
+  k_sort_scan_hist<<<1, 256, 0, s>>>(hist, passes);
   int cur = 0;
   for (int p = 0; p < passes; ++p) {
-    k_onesweep<<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(b.keys[cur], b.vals[cur], b.keys[cur ^ 1], b.vals[cur ^ 1], b.counters,
-                                                                   b.sort_hist + p * RADIX, b.sort_desc + (size_t)p * tiles_cap * RADIX, p);
+    k_onesweep<<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
+                                                                   error_flag, hist + p * RADIX, desc + (size_t)p * tiles_cap * RADIX, p);
     cur ^= 1;
   }
   return cur;

@@ -43,7 +43,8 @@ struct tgs_ctx {
   Sched sched;
   int force_all = 0;
   // capacities
-  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint64_t* keys64 = nullptr;  // test-only scratch of tgs_debug_get("keys")
   uint64_t device_bytes = 0;
   DevBuffers b;
   std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
@@ -54,6 +55,7 @@ struct tgs_ctx {
   bool sel_pending = false;
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
+  bool count_interactions = false;
   cudaEvent_t ev_stage[10];
   FrameConst fc;
 };
@@ -126,13 +128,14 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs) {
   cudaStreamSynchronize(c->stream);
   for (void* p : c->allocs_pairs) cudaFree(p);
   c->allocs_pairs.clear();
+  c->keys64 = nullptr;
   DevBuffers& b = c->b;
   for (int i = 0; i < 2; ++i) {
     if (int r = dev_alloc(c, &b.keys[i], (size_t)max_pairs, c->allocs_pairs)) return r;
     if (int r = dev_alloc(c, &b.vals[i], (size_t)max_pairs, c->allocs_pairs)) return r;
   }
   const uint32_t tiles = (max_pairs + sort_tile_items() - 1) / sort_tile_items() + 1;
-  if (int r = dev_alloc(c, &b.sort_desc, (size_t)8 * tiles * 256, c->allocs_pairs)) return r;
+  if (int r = dev_alloc(c, &b.sort_desc, (size_t)4 * tiles * 256, c->allocs_pairs)) return r;
   c->sort_tiles_cap = tiles;
   c->max_pairs = max_pairs;
   return TGS_OK;
@@ -203,7 +206,7 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   memset(c->h_counters, 0, sizeof(Counters));
   if (cudaMalloc((void**)&c->b.counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
   if (cudaMalloc((void**)&c->b.F_key, 4 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
-  if (cudaMalloc((void**)&c->b.sort_hist, 8 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
+  if (cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
   for (auto& e : c->ev_stage) cudaEventCreate(&e);
@@ -238,9 +241,12 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   c->n = 0;
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
   A(b.cull4, n) A(b.cov3d, 6 * (size_t)n) A(b.tau, n) A(b.sh, (size_t)n * K * 3)
-  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, n) A(b.rec_rgb, n)
+  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, n) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.offsets, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
-  A(b.scan_desc, (size_t)n / scan_tile_items() + 2)
+  A(b.scan_desc, (size_t)n / scan_tile_items() + 3)
+  A(b.ckeys[0], n) A(b.ckeys[1], n) A(b.cvals[0], n) A(b.cvals[1], n) A(b.nv_queue, n)
+  c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
+  A(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
 #undef A
   const float *d_means = means, *d_scales = scales, *d_quats = quats, *d_opacity = opacity, *d_sh = sh;
   std::vector<void*> tmp;
@@ -364,22 +370,27 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 1
   if (ftype == TGS_FRAME_S) launch_fill_corr(s, fc, b);                                                    // A2
   mark();                                                                      // 2
-  launch_preprocess(s, fc, b);                                                                             // A3 (+ T^oc of A4)
+  launch_preprocess(s, fc, b);                                                                             // A3 (+ small-rect T^oc)
+  if (ftype == TGS_FRAME_S) launch_mark_oc(s, fc, b, c->num_sms);                                          // A4: T^oc of large rects
   mark();                                                                      // 3
-  launch_select(s, fc, b);                                                                                 // A4
+  launch_select(s, fc, b);                                                                                 // A4: T_sel
   if (ftype == TGS_FRAME_S) {
     CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     CK(cudaEventRecord(c->ev_sel, s));
     c->sel_pending = true;
   }
-  launch_count_color(s, fc, b);                                                                            // A5
-  launch_scan_emit(s, fc, b, c->num_sms);
+  launch_count_color(s, fc, b);                                                                            // A5: counts, colour
+  launch_compact(s, fc, b, c->num_sms);
+  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_emit, 4, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
+                                  &b.counters->ticket_sort[0], &b.counters->error, c->num_sms);            // A6 level 1: by depth
+  launch_scan_emit(s, fc, b, dsorted, c->num_sms);                                                         // A5: offsets + pairs
   mark();                                                                      // 4
-  const int sorted = launch_sort(s, fc, b, c->num_sms, c->sort_tiles_cap);                                 // A6
+  const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_sort_passes(fc.n_tiles), b.sort_hist + 4 * 256,
+                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, c->num_sms);   // A6 level 2: by tile
   mark();                                                                      // 5
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
   mark();                                                                      // 6
-  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms);                         // A8 + A9
+  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);                         // A8 + A9
   mark();                                                                      // 7
   if (builds_priors) launch_frustum(s, fc, b, rendered_next, ftype == TGS_FRAME_R);                        // F_min/F_max (L109)
   CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
@@ -428,7 +439,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_total = c->n; out->n_near = h.n_near; out->n_afc = h.n_afc; out->n_toc = h.n_toc; out->n_degenerate = h.n_degenerate;
   out->n_empty = h.n_empty; out->n_visible = h.n_visible; out->n_newly_visible = h.n_newly_visible;
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
-  out->n_rendered = h.n_rendered; out->overflow = h.overflow;
+  out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions;
   out->device_bytes = c->device_bytes;
   if (c->timing) {
     for (int i = 0; i < 8; ++i) cudaEventElapsedTime(&out->ms_stage[i], c->ev_stage[i], c->ev_stage[i + 1]);
@@ -455,7 +466,12 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
     if (!c->have_frame) return TGS_E_INVALID_ARG;
     CK(cudaEventSynchronize(c->ev_done));
     const size_t P = c->h_counters->n_pairs;
-    if (name == "keys") { src = b.keys[c->sorted_idx]; have = P * 8; } else { src = b.vals[c->sorted_idx]; have = P * 4; }
+    if (name == "keys") {
+      if (!c->keys64 && P) { if (int r = dev_alloc(c, &c->keys64, (size_t)c->max_pairs, c->allocs_pairs)) return r; }
+      launch_keys64(c->stream, c->b, c->sorted_idx, (uint32_t)P, c->keys64);
+      src = c->keys64; have = P * 8;
+      if (!P) return 0;
+    } else { src = b.vals[c->sorted_idx]; have = P * 4; if (!P) return 0; }
   } else if (name == "F") {
     uint32_t keys[4]; float F[4];
     CK(cudaMemcpyAsync(keys, b.F_key, sizeof(keys), cudaMemcpyDeviceToHost, c->stream));
@@ -536,6 +552,8 @@ int tgs_debug_run_stage(tgs_ctx* c, const char* st) {
   const std::string s(st);
   if (s == "timing_on") { c->timing = true; return TGS_OK; }
   if (s == "timing_off") { c->timing = false; return TGS_OK; }
+  if (s == "count_interactions_on") { c->count_interactions = true; return TGS_OK; }
+  if (s == "count_interactions_off") { c->count_interactions = false; return TGS_OK; }
   if (s == "force_all_tiles_on") { c->force_all = 1; return TGS_OK; }
   if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
   return TGS_E_INVALID_ARG;

@@ -38,17 +38,21 @@ struct FrameConst {
 // ------------------------------------------------------------------ device counters (one block, zeroed per frame)
 struct Counters {
   uint32_t n_near, n_afc, n_toc, n_degenerate, n_empty, n_visible, n_newly_visible;
-  uint32_t n_pairs;
+  uint32_t n_pairs;         // P
   uint32_t n_sel_oc, n_sel_um, n_sel;
   uint32_t n_rendered;
   uint32_t overflow;
   uint32_t error;           // look-back watchdog etc.
+  uint32_t n_emit;          // Gaussians that emit at least one pair
+  uint32_t n_nv_queue;      // newly visible Gaussians queued for the cooperative T^oc marking
+  uint32_t n_oc_marked;     // tiles whose T^oc bit is set
   // work tickets of the persistent kernels
-  uint32_t ticket_scan;
-  uint32_t ticket_blend;
-  uint32_t ticket_sort[8];
-  uint32_t pad[10];
+  uint32_t ticket_scan, ticket_blend, ticket_compact, ticket_mark;
+  uint32_t ticket_sort[8];  // [0..3] depth sort, [4..7] tile sort
+  uint32_t pad[3];
+  unsigned long long n_interactions;   // L (only when interaction counting is on)
 };
+static_assert(sizeof(Counters) == 136, "Counters layout");
 
 // ------------------------------------------------------------------ device buffers of a context
 struct DevBuffers {
@@ -63,15 +67,23 @@ struct DevBuffers {
   uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16
   uint32_t* rec_flags = nullptr; // [N]
   float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
+  // blend-side parameters (values, not decisions): alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, which is
+  // -1/2 delta^T Sigma'^-1 delta completed to a sum of two squares: A' = -log2e/2 * c/det, k = -b/c, D' = -log2e/2 / c
+  float4* rec_b0 = nullptr;      // [N] {u, v, A', k}
+  float4* rec_b1 = nullptr;      // [N] {D', log2 o, d, -}
   uint32_t* tiles_touched = nullptr;  // [N]
   uint32_t* offsets = nullptr;        // [N] exclusive scan
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
   // pairs
-  uint64_t* keys[2] = {nullptr, nullptr};
-  uint32_t* vals[2] = {nullptr, nullptr};
-  uint32_t* sort_hist = nullptr;      // [8][256]
-  uint32_t* sort_desc = nullptr;      // [passes][tiles][256] look-back descriptors
+  uint32_t* keys[2] = {nullptr, nullptr};    // [max_pairs] tile id of a pair
+  uint32_t* vals[2] = {nullptr, nullptr};    // [max_pairs] Gaussian index of a pair
+  uint32_t* ckeys[2] = {nullptr, nullptr};   // [N] bits(depth) of the emitting Gaussians
+  uint32_t* cvals[2] = {nullptr, nullptr};   // [N] their indices
+  uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with large rects
+  uint32_t* sort_hist = nullptr;      // [2][4][256]: depth sort, tile sort
+  uint32_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors
+  uint32_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
   uint64_t* scan_desc = nullptr;      // look-back descriptors of the offsets scan
   // tiles
   uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
@@ -100,12 +112,16 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_count_color(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint8_t* rendered_now, bool update_F);
-void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
-// returns the index (0/1) of the key/val buffer that holds the sorted result
-int launch_sort(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms, uint32_t sort_tiles_cap);
+void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
+void launch_compact(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
+void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms);
+// Sorts *n_ptr items on digits [0, passes) of the uint32 key; returns the index (0/1) of the result buffers.
+int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int passes,
+                uint32_t* hist, uint32_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, int num_sms);
+void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
-                  const float* prior_image, uint8_t* rendered_next, int num_sms);
+                  const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions);
 uint32_t sort_tile_items();
 uint32_t scan_tile_items();
-int sort_num_passes(int n_tiles);
+int tile_sort_passes(int n_tiles);

@@ -121,13 +121,15 @@ def test_p3_termination_marks_not_rendered():
     K = 20
     z = 2.0 + 0.01 * np.arange(K)
     means = np.stack([np.zeros(K), np.zeros(K), z], 1)
-    # opacity 0.99 everywhere within the footprint: T after k = 0.01^k -> 2 blended, third stops (1e-6 < 1e-4)
-    _one(o, means, np.full((K, 3), 5.0), np.tile([1, 0, 0, 0], (K, 1)), np.full(K, 1.0), np.full((K, 3), 1.0), cam)
+    # alpha ~ 0.8 everywhere within the (huge) footprint: T after k = 0.2^k -> 3.2e-4 after 5, 6.4e-5 after 6:
+    # five are blended, the sixth stops the loop, the rest is never reached.  (alpha = 0.99 would put 0.01^2 ON
+    # the 1e-4 threshold, where only the fp32 rounding decides -- see R33.)
+    _one(o, means, np.full((K, 3), 5.0), np.tile([1, 0, 0, 0], (K, 1)), np.full(K, 0.8), np.full((K, 3), 1.0), cam)
     o.render(ora.FULL)
     rendered = o.get("rendered")
-    assert rendered[:2].all() and not rendered[2:].any()
+    assert rendered[:5].all() and not rendered[5:].any()
     st = o.stats()
-    assert st["n_rendered"] == 2
+    assert st["n_rendered"] == 5
 
 
 # ----------------------------------------------------------------------------------------- P4
@@ -228,7 +230,10 @@ def _brute_force_image(rec, cam, bg):
     bits = rec["d"].view(np.uint32)
     order = vis[np.lexsort((vis, bits[vis]))]
     R = rec[order]
-    u, v, A, B, Cc, op, d = (R[k].astype(np.float64) for k in ("u", "v", "A", "B", "C", "o", "d"))
+    u, v, op, d = (R[k].astype(np.float64) for k in ("u", "v", "o", "d"))
+    # conic = inverse of Sigma' = [[ca, cb], [cb, cc]] by numpy, in double
+    inv = np.linalg.inv(np.stack([np.stack([R["ca"], R["cb"]], -1), np.stack([R["cb"], R["cc"]], -1)], -2).astype(np.float64))
+    A, B, Cc = inv[:, 0, 0], inv[:, 0, 1], inv[:, 1, 1]
     col = np.stack([R["r"], R["g"], R["b"]], 1).astype(np.float64)
     img = np.zeros((H, W, 3))
     dep = np.full((H, W), float(ora.DEPTH_INVALID))
