@@ -16,13 +16,22 @@ namespace {
 
 constexpr int BLEND_THREADS = 256;
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
+// log2(1/255) = -7.99435...; anything below this bound (with a safety gap far above the rounding of e and of
+// ex2.approx) has alpha < 1/255 for sure, so the exact test on alpha is only evaluated near or above the threshold
+constexpr float LOG2_ALPHA_MIN_LO = -7.9950f;
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 
 struct BlendSmem {
   float4 a[BLEND_THREADS];     // u, v, A', k
   float4 b[BLEND_THREADS];     // D', log2(o), d, r
   float2 c[BLEND_THREADS];     // g, b
   uint32_t id[BLEND_THREADS];  // Gaussian index (for the G_rendered marks)
-  uint32_t contrib[BLEND_THREADS / 32];
+  uint8_t contrib[BLEND_THREADS];   // G_rendered marks of the batch (benign same-value races)
   uint32_t work;
 };
 
@@ -96,42 +105,35 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
         sm.c[threadIdx.x] = make_float2(r2.y, r2.z);
         sm.id[threadIdx.x] = g;
       }
-      if (MARK && threadIdx.x < BLEND_THREADS / 32) sm.contrib[threadIdx.x] = 0;
+      if (MARK) sm.contrib[threadIdx.x] = 0;
       __syncthreads();
-      for (uint32_t j0 = 0; j0 < nb; j0 += 32) {
-        uint32_t mask = 0;
-        const uint32_t je = min(32u, nb - j0);
-        if (!done) {
-          for (uint32_t jj = 0; jj < je; ++jj) {
-            const uint32_t j = j0 + jj;
-            if (COUNT) ++nint;
-            const float4 ga = sm.a[j];
-            const float dx = ga.x - fpx, dy = ga.y - fpy;
-            const float4 gb = sm.b[j];
-            const float t = fmaf(ga.w, dy, dx);
-            const float e = fmaf(ga.z * t, t, fmaf(gb.x * dy, dy, gb.y));         // log2(o) + log2 of the falloff (<= log2 o)
-            const float alpha = fminf(0.99f, exp2f(e));
-            if (alpha < ALPHA_MIN) continue;
-            const float Tn = T * (1.0f - alpha);
-            if (Tn < 1.0e-4f) { done = true; break; }
-            const float wgt = alpha * T;
-            const float2 gc = sm.c[j];
-            Cr += wgt * gb.w; Cg += wgt * gc.x; Cb += wgt * gc.y;
-            if (Sw == 0.0f) d0 = gb.z;
-            const float dd = gb.z - d0;
-            Sw += wgt; S1 += wgt * dd; S2 += wgt * dd * dd;
-            T = Tn;
-            if (MARK) mask |= 1u << jj;
-          }
-        }
-        if (MARK) {
-          mask = __reduce_or_sync(0xffffffffu, mask);
-          if (lane == 0 && mask) atomicOr(&sm.contrib[j0 >> 5], mask);
+      if (!done) {
+#pragma unroll 4
+        for (uint32_t j = 0; j < nb; ++j) {
+          if (COUNT) ++nint;
+          const float4 ga = sm.a[j];
+          const float4 gb = sm.b[j];
+          const float dx = ga.x - fpx, dy = ga.y - fpy;
+          const float t = fmaf(ga.w, dy, dx);
+          const float e = fmaf(ga.z * t, t, fmaf(gb.x * dy, dy, gb.y));         // log2(o) + log2 of the falloff (<= log2 o)
+          if (e < LOG2_ALPHA_MIN_LO) continue;                                  // surely alpha < 1/255: no MUFU
+          const float alpha = fminf(0.99f, ex2_approx(e));
+          if (alpha < ALPHA_MIN) continue;
+          const float Tn = T * (1.0f - alpha);
+          if (Tn < 1.0e-4f) { done = true; break; }
+          const float wgt = alpha * T;
+          const float2 gc = sm.c[j];
+          Cr = fmaf(wgt, gb.w, Cr); Cg = fmaf(wgt, gc.x, Cg); Cb = fmaf(wgt, gc.y, Cb);
+          if (Sw == 0.0f) d0 = gb.z;
+          const float dd = gb.z - d0;
+          Sw += wgt; S1 = fmaf(wgt, dd, S1); S2 = fmaf(wgt * dd, dd, S2);
+          T = Tn;
+          if (MARK) sm.contrib[j] = 1;
         }
       }
       if (MARK) {
         __syncthreads();
-        if (threadIdx.x < nb && ((sm.contrib[threadIdx.x >> 5] >> (threadIdx.x & 31)) & 1u)) rendered_next[sm.id[threadIdx.x]] = 1;
+        if (threadIdx.x < nb && sm.contrib[threadIdx.x]) rendered_next[sm.id[threadIdx.x]] = 1;
       }
     }
     if (inside) {
