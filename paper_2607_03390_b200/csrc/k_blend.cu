@@ -4,17 +4,21 @@
 // L101 + L125-128 (bilinear TAB, Eq.4).  Constants of R2: alpha <= 0.99, skip alpha < 1/255, stop when
 // T(1-alpha) < 1e-4.
 //
-// One persistent grid; a work item is a tile of `tile_order` (selected tiles first).  A CTA is 16x16
-// threads = one pixel each; the tile's sorted Gaussians are staged through shared memory in batches of
-// 256 records, pre-scaled so that alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, is 7 FMA-pipe
-// instructions + 1 MUFU.EX2: the form -1/2 delta^T Sigma'^-1 delta completed to two squares, which has no
-// cancellation between terms (screen-filling anisotropic splats lose 1e-4 of alpha in the 3-term conic form).
-// This kernel is FP32-pipe bound, not HBM bound.
+// One persistent grid; a work item is a tile of `tile_order` (selected tiles first).  A CTA is 64 threads
+// = one 16x16 tile, each thread owning a run of 4 horizontally adjacent pixels, so that everything that depends
+// only on the Gaussian and the row (two shared-memory loads, dy, D' dy^2 + log2 o, t at the first pixel) is paid once
+// per 4 interactions: alpha_i = exp2(A' t_i^2 + D' dy^2 + log2 o), t_i = t_0 - i, is 3 FMA-pipe instructions per
+// pixel + 5 per run.  The form is -1/2 delta^T Sigma'^-1 delta completed to two squares, which has no cancellation
+// between terms (screen-filling anisotropic splats lose 1e-4 of alpha in the 3-term conic form).  The tile's
+// sorted Gaussians are staged through shared memory in batches of 128 records.
+// This kernel is FP32-pipe / issue bound, not HBM bound.
 #include "tgs_internal.cuh"
 
 namespace {
 
-constexpr int BLEND_THREADS = 256;
+constexpr int BLEND_THREADS = 64;      // 16 rows x 4 runs of 4 pixels
+constexpr int BLEND_BATCH = 128;
+constexpr int PPT = 4;                 // pixels per thread
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
 // log2(1/255) = -7.99435...; anything below this bound (with a safety gap far above the rounding of e and of
 // ex2.approx) has alpha < 1/255 for sure, so the exact test on alpha is only evaluated near or above the threshold
@@ -27,12 +31,16 @@ __device__ __forceinline__ float ex2_approx(float x) {
 }
 
 struct BlendSmem {
-  float4 a[BLEND_THREADS];     // u, v, A', k
-  float4 b[BLEND_THREADS];     // D', log2(o), d, r
-  float2 c[BLEND_THREADS];     // g, b
-  uint32_t id[BLEND_THREADS];  // Gaussian index (for the G_rendered marks)
-  uint8_t contrib[BLEND_THREADS];   // G_rendered marks of the batch (benign same-value races)
+  float4 a[BLEND_BATCH];     // u, v, A', k
+  float4 b[BLEND_BATCH];     // D', log2(o), d, r
+  float2 c[BLEND_BATCH];     // g, b
+  uint32_t id[BLEND_BATCH];  // Gaussian index (for the G_rendered marks)
+  uint8_t contrib[BLEND_BATCH];   // G_rendered marks of the batch (benign same-value races)
   uint32_t work;
+};
+
+struct Pixel {               // per-pixel state of the front-to-back loop
+  float T, Cr, Cg, Cb, Sw, S1, S2, d0;
 };
 
 template <bool MARK, bool COUNT>
@@ -45,9 +53,9 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
                                                          uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters) {
   __shared__ BlendSmem sm;
   const CamConst& k = fc.cam;
-  const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  // a warp covers a 16x2 pixel strip of the tile
-  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
+  const uint32_t lane = threadIdx.x & 31;
+  const int lx = (threadIdx.x & 3) * PPT, ly = threadIdx.x >> 2;
+  const uint32_t n_sel = counters->n_sel;
   while (true) {
     __syncthreads();
     if (threadIdx.x == 0) sm.work = atomicAdd(&counters->ticket_blend, 1u);
@@ -55,12 +63,15 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     const uint32_t w = sm.work;
     if (w >= (uint32_t)fc.n_tiles) break;
     const uint32_t tile = tile_order[w];
-    const int px = (int)(tile % k.TX) * TGS_TILE + lx, py = (int)(tile / k.TX) * TGS_TILE + ly;
-    const bool inside = px < k.W && py < k.H;
-    const size_t pix = (size_t)py * k.W + px;
-    if (w >= counters->n_sel) {
+    const int px0 = (int)(tile % k.TX) * TGS_TILE + lx, py = (int)(tile / k.TX) * TGS_TILE + ly;
+    const bool row_in = py < k.H;
+    if (w >= n_sel) {
       // ------------------------------------------------ A9 stitch (Eq.4, second case)
-      if (inside) {
+#pragma unroll
+      for (int i = 0; i < PPT; ++i) {
+        const int px = px0 + i;
+        if (!row_in || px >= k.W) continue;
+        const size_t pix = (size_t)py * k.W + px;
         const float D = fill_depth[pix];
         const float* M = fc.Minv;
         const float rx = ((float)px - k.cx) / k.fx, ry = ((float)py - k.cy) / k.fy;
@@ -89,61 +100,86 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     }
     // -------------------------------------------------- A8 blend
     const uint2 range = ranges[tile];
-    const float fpx = (float)px, fpy = (float)py;
-    float T = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
-    float Sw = 0.0f, S1 = 0.0f, S2 = 0.0f, d0 = 0.0f;      // Eq.1-2 moments, shifted by the first contributing depth
-    bool done = !inside;
+    const float fpx = (float)px0, fpy = (float)py;
+    Pixel p[PPT];
+    bool alive[PPT];
+#pragma unroll
+    for (int i = 0; i < PPT; ++i) {
+      p[i].T = 1.0f; p[i].Cr = p[i].Cg = p[i].Cb = 0.0f; p[i].Sw = p[i].S1 = p[i].S2 = p[i].d0 = 0.0f;
+      alive[i] = row_in && px0 + i < k.W;
+    }
     uint32_t nint = 0;
-    for (uint32_t start = range.x; start < range.y; start += BLEND_THREADS) {
-      if (__syncthreads_count(done) == BLEND_THREADS) break;
-      const uint32_t nb = min((uint32_t)BLEND_THREADS, range.y - start);
-      if (threadIdx.x < nb) {
-        const uint32_t g = vals[start + threadIdx.x];
+    for (uint32_t start = range.x; start < range.y; start += BLEND_BATCH) {
+      const bool any_alive = alive[0] || alive[1] || alive[2] || alive[3];
+      if (__syncthreads_count(any_alive) == 0) break;
+      const uint32_t nb = min((uint32_t)BLEND_BATCH, range.y - start);
+      for (uint32_t j = threadIdx.x; j < nb; j += BLEND_THREADS) {
+        const uint32_t g = vals[start + j];
         const float4 r0 = rec_b0[g], r1 = rec_b1[g], r2 = rec_rgb[g];
-        sm.a[threadIdx.x] = r0;
-        sm.b[threadIdx.x] = make_float4(r1.x, r1.y, r1.z, r2.x);
-        sm.c[threadIdx.x] = make_float2(r2.y, r2.z);
-        sm.id[threadIdx.x] = g;
+        sm.a[j] = r0;
+        sm.b[j] = make_float4(r1.x, r1.y, r1.z, r2.x);
+        sm.c[j] = make_float2(r2.y, r2.z);
+        sm.id[j] = g;
+        if (MARK) sm.contrib[j] = 0;
       }
-      if (MARK) sm.contrib[threadIdx.x] = 0;
       __syncthreads();
-      if (!done) {
-#pragma unroll 4
+      if (any_alive) {
+#pragma unroll 2
         for (uint32_t j = 0; j < nb; ++j) {
-          if (COUNT) ++nint;
           const float4 ga = sm.a[j];
           const float4 gb = sm.b[j];
-          const float dx = ga.x - fpx, dy = ga.y - fpy;
-          const float t = fmaf(ga.w, dy, dx);
-          const float e = fmaf(ga.z * t, t, fmaf(gb.x * dy, dy, gb.y));         // log2(o) + log2 of the falloff (<= log2 o)
-          if (e < LOG2_ALPHA_MIN_LO) continue;                                  // surely alpha < 1/255: no MUFU
-          const float alpha = fminf(0.99f, ex2_approx(e));
-          if (alpha < ALPHA_MIN) continue;
-          const float Tn = T * (1.0f - alpha);
-          if (Tn < 1.0e-4f) { done = true; break; }
-          const float wgt = alpha * T;
+          const float dy = ga.y - fpy;
+          const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
+          float t = fmaf(ga.w, dy, ga.x - fpx);                       // t at the first pixel of the run
+          if (COUNT) nint += (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3];
+          bool hit[PPT];
+          float e[PPT];
+#pragma unroll
+          for (int i = 0; i < PPT; ++i) {
+            e[i] = fmaf(ga.z * t, t, e1);                             // log2(o) + log2 of the falloff
+            hit[i] = alive[i] && e[i] >= LOG2_ALPHA_MIN_LO;           // else surely alpha < 1/255: no MUFU
+            t -= 1.0f;
+          }
+          if (!(hit[0] || hit[1] || hit[2] || hit[3])) continue;
           const float2 gc = sm.c[j];
-          Cr = fmaf(wgt, gb.w, Cr); Cg = fmaf(wgt, gc.x, Cg); Cb = fmaf(wgt, gc.y, Cb);
-          if (Sw == 0.0f) d0 = gb.z;
-          const float dd = gb.z - d0;
-          Sw += wgt; S1 = fmaf(wgt, dd, S1); S2 = fmaf(wgt * dd, dd, S2);
-          T = Tn;
-          if (MARK) sm.contrib[j] = 1;
+          bool marked = false;
+#pragma unroll
+          for (int i = 0; i < PPT; ++i) {
+            if (!hit[i]) continue;
+            const float alpha = fminf(0.99f, ex2_approx(e[i]));
+            if (alpha < ALPHA_MIN) continue;
+            const float Tn = p[i].T * (1.0f - alpha);
+            if (Tn < 1.0e-4f) { alive[i] = false; continue; }
+            const float wgt = alpha * p[i].T;
+            p[i].Cr = fmaf(wgt, gb.w, p[i].Cr); p[i].Cg = fmaf(wgt, gc.x, p[i].Cg); p[i].Cb = fmaf(wgt, gc.y, p[i].Cb);
+            if (p[i].Sw == 0.0f) p[i].d0 = gb.z;
+            const float dd = gb.z - p[i].d0;
+            p[i].Sw += wgt; p[i].S1 = fmaf(wgt, dd, p[i].S1); p[i].S2 = fmaf(wgt * dd, dd, p[i].S2);
+            p[i].T = Tn;
+            marked = true;
+          }
+          if (MARK && marked) sm.contrib[j] = 1;
+          if (!(alive[0] || alive[1] || alive[2] || alive[3])) break;
         }
       }
       if (MARK) {
         __syncthreads();
-        if (threadIdx.x < nb && sm.contrib[threadIdx.x]) rendered_next[sm.id[threadIdx.x]] = 1;
+        for (uint32_t j = threadIdx.x; j < nb; j += BLEND_THREADS)
+          if (sm.contrib[j]) rendered_next[sm.id[j]] = 1;
       }
     }
-    if (inside) {
-      image[pix * 3 + 0] = Cr + T * fc.bg[0];
-      image[pix * 3 + 1] = Cg + T * fc.bg[1];
-      image[pix * 3 + 2] = Cb + T * fc.bg[2];
-      if (Sw > 0.0f) {
-        const float m1 = S1 / Sw;
-        depth[pix] = d0 + m1;
-        sigma[pix] = sqrtf(fmaxf(0.0f, S2 / Sw - m1 * m1));
+#pragma unroll
+    for (int i = 0; i < PPT; ++i) {
+      const int px = px0 + i;
+      if (!row_in || px >= k.W) continue;
+      const size_t pix = (size_t)py * k.W + px;
+      image[pix * 3 + 0] = p[i].Cr + p[i].T * fc.bg[0];
+      image[pix * 3 + 1] = p[i].Cg + p[i].T * fc.bg[1];
+      image[pix * 3 + 2] = p[i].Cb + p[i].T * fc.bg[2];
+      if (p[i].Sw > 0.0f) {
+        const float m1 = p[i].S1 / p[i].Sw;
+        depth[pix] = p[i].d0 + m1;
+        sigma[pix] = sqrtf(fmaxf(0.0f, p[i].S2 / p[i].Sw - m1 * m1));
       } else {
         depth[pix] = TGS_DEPTH_INVALID;
         sigma[pix] = 0.0f;
@@ -153,7 +189,6 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
       nint = __reduce_add_sync(0xffffffffu, nint);
       if (lane == 0 && nint) atomicAdd(&counters->n_interactions, (unsigned long long)nint);
     }
-    (void)wid;
   }
 }
 
@@ -161,7 +196,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
 
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
                   uint8_t* rendered_next, int num_sms, bool count_interactions) {
-  const int grid = num_sms * 4;
+  const int grid = num_sms * 16;
 #define LAUNCH(M, C)                                                                                                          \
   k_blend<M, C><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \
