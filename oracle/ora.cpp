@@ -357,8 +357,13 @@ void select_tiles(ora_ctx* c, int ftype) {
 // ---------------------------------------------------------------- O5-O7 pairs, sort, ranges (A5-A7)
 // PAPER.md:L61 "Gaussians that intersect with multiple tiles are duplicated ... sorts its intersected
 // Gaussians by depth from front to back"; L123 only the Gaussians intersecting T_selected are sorted.
+// "Intersect" is not defined by the paper.  exact_tiles = 0: every tile of the 3-sigma rect (vanilla 3DGS, R3).
+// exact_tiles = 1 (default, R39): additionally max alpha over the tile's pixel-centre box >= 1/255, the test the
+// paper itself uses for tile contributions (L119).  A pair dropped by it is skipped at every pixel of the tile
+// (alpha < 1/255, R2) and can never stop a loop, so the image, the TGB and G_rendered do not depend on it
+// (up to alpha within rounding of 1/255); only the lists get shorter.
 void bin_and_sort(ora_ctx* c) {
-  const int TX = c->TX;
+  const int TX = c->TX, W = c->cam.W, H = c->cam.H;
   std::vector<std::pair<uint64_t, uint32_t>> pairs;
   for (uint32_t g = 0; g < c->n; ++g) {
     ora_record& r = c->rec[g];
@@ -368,6 +373,11 @@ void bin_and_sort(ora_ctx* c) {
       for (int tx = r.x_lo; tx < r.x_hi; ++tx) {
         const uint32_t t = (uint32_t)(ty * TX + tx);
         if (!(c->tile_mask[t] & 4)) continue;
+        if (c->prm.exact_tiles) {   // R39: "intersect" = some point of the tile's pixel box has alpha >= 1/255
+          const float x0 = (float)(tx * TILE), x1 = (float)std::min(tx * TILE + TILE - 1, W - 1);
+          const float y0 = (float)(ty * TILE), y1 = (float)std::min(ty * TILE + TILE - 1, H - 1);
+          if (!(r.tau >= 0.0f && box_qmin(r.u, r.v, r.A, r.B, r.C, x0, x1, y0, y1) <= r.tau)) continue;
+        }
         pairs.emplace_back(((uint64_t)t << 32) | f2u(r.d), g);
         ++cnt;
       }
@@ -523,7 +533,7 @@ extern "C" {
 
 void ora_default_params(ora_params* p) {
   p->lambda1 = 3.0f; p->lambda2 = 0.0f; p->lambda_tdc = 50; p->lambda_sr = 5; p->eta = 0.40f;
-  p->bg[0] = p->bg[1] = p->bg[2] = 0.0f; p->enable_afc = p->enable_toc = p->enable_sr = 1;
+  p->bg[0] = p->bg[1] = p->bg[2] = 0.0f; p->enable_afc = p->enable_toc = p->enable_sr = 1; p->exact_tiles = 1;
 }
 
 ora_ctx* ora_create(void) { ora_ctx* c = new ora_ctx(); ora_default_params(&c->prm); return c; }

@@ -43,6 +43,8 @@ typedef struct {
   float eta;              /* 0.40 */
   float bg[3];            /* background colour (R27) */
   int enable_afc, enable_toc, enable_sr; /* Table IV toggles */
+  int exact_tiles;        /* 1: a Gaussian "intersects" a tile iff max alpha over the tile's pixel box >= 1/255
+                             (R39, same box test as L119); 0: every tile of the 3-sigma rect (vanilla 3DGS) */
 } ora_params;
 
 typedef struct {        /* 80 bytes */

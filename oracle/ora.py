@@ -30,7 +30,7 @@ assert RECORD_DTYPE.itemsize == 80
 class OraParams(C.Structure):
     _fields_ = [("lambda1", C.c_float), ("lambda2", C.c_float), ("lambda_tdc", C.c_int), ("lambda_sr", C.c_int),
                 ("eta", C.c_float), ("bg", C.c_float * 3),
-                ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int)]
+                ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int), ("exact_tiles", C.c_int)]
 
 
 class OraStats(C.Structure):

@@ -293,6 +293,43 @@ def test_p5_tile_binned_equals_per_pixel_brute_force():
         assert np.all((keys[s:e] >> np.uint64(32)) == t)
 
 
+def test_exact_tile_intersection_drops_only_dead_pairs():
+    """R39: with exact_tiles the pair list is a subset of the 3-sigma-rect list, every dropped pair has alpha < 1/255
+    at all 256 pixel centres of its tile (brute force through Sigma'^-1, not through the box test), and image, depth
+    and G_rendered are bit-identical to the rect-binned render."""
+    sc = make_config(1, n=3000, frames=1, width=80, height=64)
+    sc.scales *= 3
+    V = look_at((0.4, 0.2, -4.0), (0, 0, 0), (0, 1, 0))
+    out = {}
+    for ex in (0, 1):
+        o = Oracle()
+        o.load_scene(sc)
+        p = o.default_params(); p.exact_tiles = ex
+        o.set_params(p)
+        o.set_camera(V, sc.camera)
+        o.render(ora.FULL)
+        out[ex] = dict(img=o.read_image(), dep=o.read_depth(), ren=o.get("rendered"), keys=o.get("keys"), vals=o.get("vals"),
+                       rec=o.get("records"))
+    a, b = out[0], out[1]
+    assert np.array_equal(a["img"].view(np.uint32), b["img"].view(np.uint32))
+    assert np.array_equal(a["dep"][0].view(np.uint32), b["dep"][0].view(np.uint32)) and np.array_equal(a["ren"], b["ren"])
+    pa = set(zip((a["keys"] >> np.uint64(32)).tolist(), a["vals"].tolist()))
+    pb = set(zip((b["keys"] >> np.uint64(32)).tolist(), b["vals"].tolist()))
+    assert pb < pa and len(pb) < 0.9 * len(pa)
+    rec, TX = a["rec"], (sc.camera.W + 15) // 16
+    for (t, g) in list(pa - pb)[:3000]:
+        r = rec[g]
+        inv = np.linalg.inv(np.array([[r["ca"], r["cb"]], [r["cb"], r["cc"]]], dtype=np.float64))
+        xs = np.arange((t % TX) * 16, min((t % TX) * 16 + 16, sc.camera.W)) - float(r["u"])
+        ys = np.arange((t // TX) * 16, min((t // TX) * 16 + 16, sc.camera.H)) - float(r["v"])
+        dx, dy = np.meshgrid(xs, ys)
+        q = -0.5 * (inv[0, 0] * dx * dx + 2 * inv[0, 1] * dx * dy + inv[1, 1] * dy * dy)
+        assert (float(r["o"]) * np.exp(q)).max() < (1 / 255) * (1 + 1e-4)
+    # the sorted order of the surviving pairs is the order they had in the rect-binned list
+    keep = np.array([(int(k) >> 32, int(v)) in pb for k, v in zip(a["keys"], a["vals"])])
+    assert np.array_equal(a["keys"][keep], b["keys"]) and np.array_equal(a["vals"][keep], b["vals"])
+
+
 # ----------------------------------------------------------------------------------------- P6
 def test_p6_sh_orthonormal_and_hand_values():
     xs, ws = np.polynomial.legendre.leggauss(24)
