@@ -69,6 +69,9 @@ typedef struct {
   float bg[3];            /* background colour, part of the TAB (R27); 0 */
   int enable_afc, enable_toc, enable_sr; /* module toggles of Table IV (L221-231); 1 */
   uint32_t max_pairs;     /* capacity of the (Gaussian, tile) pair buffers; 0 = automatic */
+  int exact_tiles;        /* 1 (default, R39): a Gaussian "intersects" a tile (L61) iff its max alpha over the tile's pixel
+                             box is >= 1/255 -- the test L119 uses for tile contributions; 0: every tile of the 3-sigma
+                             rect.  Images, TGB and G_rendered do not depend on it, only the pair lists get shorter. */
 } tgs_params;
 
 typedef struct {

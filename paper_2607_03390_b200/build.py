@@ -2,7 +2,7 @@
 
     python -m paper_2607_03390_b200.build [--force]
 
-k_decide.cu is compiled with -fmad=false: its fp32 arithmetic decides integers and must round exactly
+k_decide.cu and k_bin.cu are compiled with -fmad=false: their fp32 arithmetic decides integers and must round exactly
 as written (DESIGN.md §2 R33).  Nothing here uses --use_fast_math.
 """
 from __future__ import annotations
@@ -23,7 +23,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE
 SOURCES = {
     "tgs_api.cu": [],
     "k_decide.cu": ["-fmad=false"],
-    "k_bin.cu": [],
+    "k_bin.cu": ["-fmad=false"],       # k_emit repeats the tile test of k_count_color (decide_math.cuh)
     "k_sort.cu": [],
     "k_blend.cu": [],
 }

@@ -8,6 +8,7 @@
 // from device memory; the kernels run as persistent grids pulling work tickets, so a frame needs no host
 // round trip.
 #include "tgs_internal.cuh"
+#include "decide_math.cuh"   // this file is compiled with -fmad=false: k_emit repeats k_count_color's tile test
 
 namespace {
 
@@ -136,7 +137,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_offsets(FrameConst fc, co
 // Gaussians -- the ones covering hundreds or thousands of tiles -- are neighbours, and this spreads them over all SMs.
 // Pairs are written in the oracle's order (ty ascending, then tx) at offsets[i].
 __global__ void __launch_bounds__(256) k_emit(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ offsets,
-                                              const uint2* __restrict__ rec_rect, const uint32_t* __restrict__ sel_bits,
+                                              const uint2* __restrict__ rec_rect, const float4* __restrict__ rec_uvdo,
+                                              const float4* __restrict__ rec_conic, const uint32_t* __restrict__ sel_bits,
                                               uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
                                               const Counters* __restrict__ counters) {
   if (counters->overflow) return;
@@ -149,10 +151,14 @@ __global__ void __launch_bounds__(256) k_emit(FrameConst fc, const uint32_t* __r
     const uint2 r = rec_rect[g];
     const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
     const uint32_t w = x_hi - x_lo, area = w * (y_hi - y_lo);
+    float4 uv, cn;
+    if (fc.exact_tiles) { uv = rec_uvdo[g]; cn = rec_conic[g]; }
     for (uint32_t base = 0; base < area; base += 32) {
       const uint32_t idx = base + lane;
-      const uint32_t t = (y_lo + idx / w) * fc.cam.TX + x_lo + idx % w;
-      const bool sel = idx < area && (fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u));
+      const uint32_t ry = idx / w, ty = y_lo + ry, tx = x_lo + (idx - ry * w);
+      const uint32_t t = ty * fc.cam.TX + tx;
+      bool sel = idx < area && (fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u));
+      if (sel && fc.exact_tiles) sel = tile_alpha_reach(uv.x, uv.y, cn.x, cn.y, cn.z, cn.w, tx, ty, fc.cam.W, fc.cam.H);   // R39
       const uint32_t bal = __ballot_sync(0xffffffffu, sel);
       if (sel) {
         const uint32_t p = off + __popc(bal & ((1u << lane) - 1u));
@@ -205,7 +211,7 @@ void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int s
   const uint32_t grid = num_tiles < (uint32_t)(num_sms * 4) ? num_tiles : (uint32_t)(num_sms * 4);
   k_scan_offsets<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, b.cvals[sorted_g_idx], b.tiles_touched, (unsigned long long*)b.scan_desc,
                                                          b.offsets, b.counters);
-  k_emit<<<num_sms * 8, 256, 0, s>>>(fc, b.cvals[sorted_g_idx], b.offsets, b.rec_rect, b.sel_bits, b.keys[0], b.vals[0], b.counters);
+  k_emit<<<num_sms * 8, 256, 0, s>>>(fc, b.cvals[sorted_g_idx], b.offsets, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, b.keys[0], b.vals[0], b.counters);
 }
 
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms) {

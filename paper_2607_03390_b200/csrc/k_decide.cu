@@ -7,6 +7,7 @@
 // A3 preprocess + AFC + TOC + newly-visible + T^oc (L61, L109-113, L119), A4 tile selection (L117-123),
 // A5a count + SH colour, F reduction (L109).
 #include "tgs_internal.cuh"
+#include "decide_math.cuh"
 
 namespace {
 
@@ -133,28 +134,6 @@ __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* _
   }
   const int any = __syncthreads_or(unmatched ? 1 : 0);
   if (threadIdx.x == 0 && any) tile_flags[blockIdx.y * k.TX + blockIdx.x] = 2u;   // bit1 = T^um (first writer of this word)
-}
-
-// min over the tile's pixel-centre box of A dx^2 + 2B dx dy + C dy^2 (L119, R18); same operation order as
-// stated in DESIGN.md §2 R18.
-__device__ __forceinline__ float box_qmin(float u, float v, float A, float B, float C, float x0, float x1, float y0, float y1) {
-  if (u >= x0 && u <= x1 && v >= y0 && v <= y1) return 0.0f;
-  const float xl = x0 - u, xh = x1 - u, yl = y0 - v, yh = y1 - v;
-  const float B2 = 2.0f * B;
-  float best;
-  {
-    float t = -(B * xl) / C; t = fminf(fmaxf(t, yl), yh);
-    best = ((A * xl) * xl + (B2 * xl) * t) + (C * t) * t;
-    t = -(B * xh) / C; t = fminf(fmaxf(t, yl), yh);
-    best = fminf(best, ((A * xh) * xh + (B2 * xh) * t) + (C * t) * t);
-  }
-  {
-    float t = -(B * yl) / A; t = fminf(fmaxf(t, xl), xh);
-    best = fminf(best, ((A * t) * t + (B2 * t) * yl) + (C * yl) * yl);
-    t = -(B * yh) / A; t = fminf(fmaxf(t, xl), xh);
-    best = fminf(best, ((A * t) * t + (B2 * t) * yh) + (C * yh) * yh);
-  }
-  return best;
 }
 
 }  // namespace
@@ -385,24 +364,64 @@ __device__ __forceinline__ void sh_basis(int deg, float x, float y, float z, flo
 }
 
 // ------------------------------------------------------------------ A5a pair count + SH colour
-// tiles_touched[g] = number of SELECTED tiles in the rect (= pairs this Gaussian emits; 0 if invisible).
+// tiles_touched[g] = number of pairs this Gaussian emits (0 if invisible): the SELECTED tiles of its rect (L123)
+// that it intersects (L61) -- with exact_tiles (R39) those where max alpha over the tile's pixel box >= 1/255,
+// else every tile of the 3-sigma rect.  Rects of more than 4 tiles are counted by the whole warp (lanes over
+// tiles): near Gaussians cover hundreds of tiles and would otherwise serialise one thread.
 // SH -> RGB (L61 "color c_i"; R5) only for Gaussians that emit at least one pair: on S frames the 12K bytes
 // of SH are read only for Gaussians that reach a selected tile.
 template <int DEG>
 __global__ void __launch_bounds__(256) k_count_color(FrameConst fc, const float4* __restrict__ cull4, const float* __restrict__ sh,
                                                      const uint32_t* __restrict__ rec_flags, const uint2* __restrict__ rec_rect,
+                                                     const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
                                                      const uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tiles_touched,
                                                      float4* __restrict__ rec_rgb) {
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
-  if (g >= fc.n) return;
+  const uint32_t lane = threadIdx.x & 31;
+  const int TX = fc.cam.TX;
   uint32_t cnt = 0;
-  if (rec_flags[g] & TGS_VISIBLE) {
+  const bool vis = g < fc.n && (rec_flags[g] & TGS_VISIBLE);
+  uint32_t x_lo = 0, y_lo = 0, w = 0, area = 0;
+  if (vis) {
     const uint2 r = rec_rect[g];
-    const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
-    if (fc.all_tiles) cnt = (x_hi - x_lo) * (y_hi - y_lo);
-    else
-      for (uint32_t ty = y_lo; ty < y_hi; ++ty) cnt += popc_range(sel_bits, ty * fc.cam.TX + x_lo, ty * fc.cam.TX + x_hi);
+    x_lo = r.x & 0xffffu; y_lo = r.y & 0xffffu;
+    w = (r.x >> 16) - x_lo; area = w * ((r.y >> 16) - y_lo);
   }
+  if (!fc.exact_tiles) {
+    if (vis) {
+      if (fc.all_tiles) cnt = area;
+      else
+        for (uint32_t ty = y_lo; ty < y_lo + area / w; ++ty) cnt += popc_range(sel_bits, ty * TX + x_lo, ty * TX + x_lo + w);
+    }
+  } else {
+    float4 uv = make_float4(0.f, 0.f, 0.f, 0.f), cn = make_float4(0.f, 0.f, 0.f, -1.f);
+    if (vis) { uv = rec_uvdo[g]; cn = rec_conic[g]; }
+    const bool big = area > 4u;
+    if (vis && !big)
+      for (uint32_t i = 0; i < area; ++i) {
+        const uint32_t ty = y_lo + i / w, tx = x_lo + i % w, t = ty * TX + tx;
+        if ((fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u)) && tile_alpha_reach(uv.x, uv.y, cn.x, cn.y, cn.z, cn.w, tx, ty, fc.cam.W, fc.cam.H)) ++cnt;
+      }
+    uint32_t m = __ballot_sync(0xffffffffu, vis && big);
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      const float su = __shfl_sync(0xffffffffu, uv.x, src), sv = __shfl_sync(0xffffffffu, uv.y, src);
+      const float sA = __shfl_sync(0xffffffffu, cn.x, src), sB = __shfl_sync(0xffffffffu, cn.y, src);
+      const float sC = __shfl_sync(0xffffffffu, cn.z, src), st = __shfl_sync(0xffffffffu, cn.w, src);
+      const uint32_t sx = __shfl_sync(0xffffffffu, x_lo, src), sy = __shfl_sync(0xffffffffu, y_lo, src);
+      const uint32_t sw = __shfl_sync(0xffffffffu, w, src), sa = __shfl_sync(0xffffffffu, area, src);
+      uint32_t c = 0;
+      if (st >= 0.0f)
+        for (uint32_t i = lane; i < sa; i += 32) {
+          const uint32_t ry = i / sw, ty = sy + ry, tx = sx + (i - ry * sw), t = ty * TX + tx;
+          if ((fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u)) && tile_alpha_reach(su, sv, sA, sB, sC, st, tx, ty, fc.cam.W, fc.cam.H)) ++c;
+        }
+      c = warp_sum(c);
+      if ((int)lane == src) cnt = c;
+    }
+  }
+  if (g >= fc.n) return;
   tiles_touched[g] = cnt;
   if (!cnt) return;
   constexpr int K = (DEG + 1) * (DEG + 1);
@@ -497,7 +516,7 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
 
 void launch_count_color(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   const dim3 grid((fc.n + 255) / 256);
-#define LAUNCH(D) k_count_color<D><<<grid, 256, 0, s>>>(fc, b.cull4, b.sh, b.rec_flags, b.rec_rect, b.sel_bits, b.tiles_touched, b.rec_rgb)
+#define LAUNCH(D) k_count_color<D><<<grid, 256, 0, s>>>(fc, b.cull4, b.sh, b.rec_flags, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, b.tiles_touched, b.rec_rgb)
   switch (fc.sh_degree) {
     case 0: LAUNCH(0); break;
     case 1: LAUNCH(1); break;

@@ -186,6 +186,7 @@ void tgs_default_params(tgs_params* p) {
   p->bg[0] = p->bg[1] = p->bg[2] = 0.0f;
   p->enable_afc = p->enable_toc = p->enable_sr = 1;
   p->max_pairs = 0;
+  p->exact_tiles = 1;
 }
 
 int tgs_create(tgs_ctx** out, int device, void* stream) {
@@ -354,6 +355,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   fc.do_tgb = (ftype == TGS_FRAME_S);
   fc.do_toc = fc.do_tgb && c->prm.enable_toc;
   fc.all_tiles = !(ftype == TGS_FRAME_S && c->prm.enable_sr && !c->force_all);
+  fc.exact_tiles = c->prm.exact_tiles ? 1 : 0;
   fc.n_tiles = c->TX * c->TY;
 
   DevBuffers& b = c->b;

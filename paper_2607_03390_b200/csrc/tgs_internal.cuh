@@ -32,6 +32,7 @@ struct FrameConst {
   int sh_degree;
   int ftype;                // TGS_FRAME_R / P / S
   int do_afc, do_toc, do_tgb, all_tiles;
+  int exact_tiles;          // R39
   int n_tiles;
 };
 
