@@ -133,7 +133,7 @@ const char* tgs_last_error(tgs_ctx*);
  * Readable: rec_uvdo rec_conic (float4 [N]) rec_rect (uint16x4 [N]) rec_flags (uint32 [N]) rec_rgb
  *   (float4 [N]) tiles_touched (uint32 [N]) keys (uint64 [P]) vals (uint32 [P]) ranges (uint32 [T][2])
  *   warp_depth warp_sigma fill_depth (float [H][W]) rendered (uint8 [N]) F (float[4]) prior_depth
- *   prior_sigma (float [H][W]) prior_image (float [H][W][3]) cov3d (float [N][6]) tau (float [N]).
+ *   prior_sigma (float [H][W]) prior_image (float [H][W][3]) g2 (float [N][8]: Sigma xx xy xz yy yz zz, opacity, tau).
  * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):
  *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
  * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off"

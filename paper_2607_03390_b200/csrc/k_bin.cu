@@ -1,116 +1,49 @@
-// k_bin.cu -- integer work around the sort (A5, A7): compaction of the Gaussians that emit pairs,
-// pair offsets (single-pass scan with decoupled look-back) fused with the (tile, Gaussian) pair emission
-// in depth order, per-tile ranges, and the reconstruction of the 64-bit tile|depth keys for the tests.
+// k_bin.cu -- A5 + A7: which (Gaussian, tile) pairs exist, in which order, and where each tile's list starts.
 // PAPER.md:L61 ("Gaussians that intersect with multiple tiles are duplicated ... sorts its intersected
 // Gaussians by depth from front to back"), L123 (only Gaussians intersecting T_selected are sorted).
 //
-// Problem sizes that are not known on the host (number of emitting Gaussians, number of pairs P) are read
-// from device memory; the kernels run as persistent grids pulling work tickets, so a frame needs no host
-// round trip.
+// The visible Gaussians arrive sorted by (depth, index).  Every (Gaussian, tile of its 3-sigma rect) combination
+// is one TEST; the tests of all Gaussians, in that order and row-major inside a rect, form one flat index space
+// (k_scan_area: prefix sums of the rect areas).  k_bin cuts that space into equal chunks -- so a screen-filling
+// Gaussian is spread over many CTAs instead of stalling one warp -- evaluates each test once (tile selected, L123,
+// and reached with alpha >= 1/255, R39), ranks the passing tests with a single-pass scan (decoupled look-back) and
+// writes the pairs (tile id, Gaussian) in exactly the oracle's emission order; the stable sort by tile id that
+// follows (k_sort.cu) then leaves every tile's list in (depth, index) order.  The same kernel counts the pairs per
+// Gaussian and evaluates SH -> RGB (L61 "color c_i"; R5) for the Gaussians that emitted at least one pair, so on S
+// frames the SH bytes are read only for Gaussians that reach a selected tile.
+//
+// Compiled with -fmad=false: the tile test is decision arithmetic (decide_math.cuh).
+// Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory; the
+// kernels are persistent grids pulling work tickets, so a frame needs no host round trip.
 #include "tgs_internal.cuh"
-#include "decide_math.cuh"   // this file is compiled with -fmad=false: k_emit repeats k_count_color's tile test
+#include "decide_math.cuh"
+#include "scan.cuh"
 
 namespace {
 
-constexpr uint32_t LOOKBACK_WATCHDOG = 1u << 26;   // polls before a look-back gives up and flags an error
-
-__device__ __forceinline__ unsigned long long ld_volatile64(const unsigned long long* p) {
-  return *reinterpret_cast<const volatile unsigned long long*>(p);
-}
-__device__ __forceinline__ void st_volatile64(unsigned long long* p, unsigned long long v) {
-  *reinterpret_cast<volatile unsigned long long*>(p) = v;
-}
-
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_IPT = 4;
-constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // items per tile
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 
-// Block-wide exclusive scan of per-thread sums + decoupled look-back across tiles.
-// Returns the exclusive prefix of this thread's first item; *incl_total = inclusive prefix of the tile.
-__device__ __forceinline__ uint32_t tile_scan(uint32_t tsum, uint32_t tile, unsigned long long* __restrict__ desc,
-                                              uint32_t* s_warp, uint32_t* s_excl, uint32_t* error_flag, uint32_t* incl_total) {
-  const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  uint32_t incl = tsum;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
-  if (lane == 31) s_warp[wid] = incl;
-  __syncthreads();
-  uint32_t wbase = 0, total = 0;
-#pragma unroll
-  for (int w = 0; w < SCAN_THREADS / 32; ++w) { const uint32_t t = s_warp[w]; if ((uint32_t)w < wid) wbase += t; total += t; }
-  if (wid == 0) {   // warp-parallel decoupled look-back: 32 predecessor descriptors per step
-    uint32_t excl = 0;
-    if (tile > 0) {
-      if (lane == 0) st_volatile64(&desc[tile], (1ull << 32) | total);   // aggregate available
-      int base = (int)tile - 1;
-      uint32_t polls = 0;
-      while (true) {
-        const int t = base - (int)lane;
-        const unsigned long long d = t >= 0 ? ld_volatile64(&desc[t]) : (2ull << 32);   // "prefix 0" before tile 0
-        const uint32_t st = (uint32_t)(d >> 32);
-        const uint32_t ready = __ballot_sync(0xffffffffu, st != 0), pref = __ballot_sync(0xffffffffu, st == 2);
-        const int first = pref ? __ffs(pref) - 1 : 31;
-        const uint32_t span = first == 31 ? 0xffffffffu : ((2u << first) - 1u);         // lanes 0..first
-        if ((ready & span) != span) { if (++polls > LOOKBACK_WATCHDOG) { if (lane == 0) *error_flag = 1; break; } continue; }
-        excl += __reduce_add_sync(0xffffffffu, (int)lane <= first ? (uint32_t)d : 0u);
-        if (pref) break;
-        base -= 32;
-      }
-    }
-    if (lane == 0) {
-      st_volatile64(&desc[tile], (2ull << 32) | (excl + total));       // inclusive prefix available
-      *s_excl = excl;
-    }
-  }
-  __syncthreads();
-  *incl_total = *s_excl + total;
-  return *s_excl + wbase + (incl - tsum);
-}
+constexpr int BIN_THREADS = 256;
+constexpr int BIN_IPT = 8;
+constexpr int BIN_CHUNK = BIN_THREADS * BIN_IPT;      // tests per work item
 
-// ================================================================== A5a: compaction
-// Gaussians with tiles_touched > 0, in ascending index order: ckeys = bits(depth), cvals = index.
-__global__ void __launch_bounds__(SCAN_THREADS) k_compact(uint32_t n, const uint32_t* __restrict__ tiles_touched,
-                                                          const float4* __restrict__ rec_uvdo, unsigned long long* __restrict__ desc,
-                                                          uint32_t* __restrict__ ckeys, uint32_t* __restrict__ cvals,
-                                                          Counters* __restrict__ counters) {
+// ================================================================== A5a: flat test space
+// area_prefix[i] = number of tests of the Gaussians before position i of the sorted visible list (area_prefix[n] =
+// all tests); chunk_first[k] = position of the Gaussian that contains test k * BIN_CHUNK.
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const uint32_t* __restrict__ sorted_g,
+                                                            const uint2* __restrict__ rec_rect, unsigned long long* __restrict__ desc,
+                                                            uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
+                                                            unsigned long long* __restrict__ bin_desc, Counters* __restrict__ counters,
+                                                            unsigned long long max_tests) {
   __shared__ uint32_t s_tile, s_warp[SCAN_THREADS / 32], s_excl;
-  const uint32_t num_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  while (true) {
-    __syncthreads();
-    if (threadIdx.x == 0) s_tile = atomicAdd(&counters->ticket_compact, 1u);
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    if (tile >= num_tiles) break;
-    const uint32_t g0 = tile * SCAN_TILE + threadIdx.x * SCAN_IPT;
-    uint32_t c[SCAN_IPT];
-    if (g0 + SCAN_IPT <= n) {
-      const uint4 v = *reinterpret_cast<const uint4*>(tiles_touched + g0);
-      c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
-    } else {
-#pragma unroll
-      for (int i = 0; i < SCAN_IPT; ++i) c[i] = (g0 + i < n) ? tiles_touched[g0 + i] : 0u;
-    }
-    const uint32_t tsum = (c[0] != 0) + (c[1] != 0) + (c[2] != 0) + (c[3] != 0);
-    uint32_t incl_total;
-    uint32_t off = tile_scan(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total);
-    if (tile == num_tiles - 1 && threadIdx.x == 0) counters->n_emit = incl_total;
-#pragma unroll
-    for (int i = 0; i < SCAN_IPT; ++i)
-      if (c[i]) { ckeys[off] = __float_as_uint(rec_uvdo[g0 + i].z); cvals[off] = g0 + i; ++off; }
+  const uint32_t n = counters->n_visible;
+  if (n == 0 || counters->area_sum > max_tests) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters->n_tests = 0; counters->n_pairs = 0; if (n) counters->overflow = 1; }
+    return;
   }
-}
-
-// ================================================================== A5b: offsets + pair emission in depth order
-// items = the emitting Gaussians in depth order (sorted_g); the pair lists of consecutive items are
-// consecutive, so after the stable sort by tile every tile's list is in (depth, index) order.
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_offsets(FrameConst fc, const uint32_t* __restrict__ sorted_g,
-                                                               const uint32_t* __restrict__ tiles_touched,
-                                                               unsigned long long* __restrict__ desc, uint32_t* __restrict__ offsets,
-                                                               Counters* __restrict__ counters) {
-  __shared__ uint32_t s_tile, s_warp[SCAN_THREADS / 32], s_excl;
-  const uint32_t n = counters->n_emit;
   const uint32_t num_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  if (n == 0) { if (blockIdx.x == 0 && threadIdx.x == 0) counters->n_pairs = 0; return; }
   while (true) {
     __syncthreads();
     if (threadIdx.x == 0) s_tile = atomicAdd(&counters->ticket_scan, 1u);
@@ -118,55 +51,176 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_offsets(FrameConst fc, co
     const uint32_t tile = s_tile;
     if (tile >= num_tiles) break;
     const uint32_t i0 = tile * SCAN_TILE + threadIdx.x * SCAN_IPT;
-    uint32_t c[SCAN_IPT];
+    uint32_t a[SCAN_IPT];
 #pragma unroll
-    for (int i = 0; i < SCAN_IPT; ++i) c[i] = (i0 + i < n) ? tiles_touched[sorted_g[i0 + i]] : 0u;
-    const uint32_t tsum = c[0] + c[1] + c[2] + c[3];
-    uint32_t incl_total;
-    uint32_t off = tile_scan(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total);
-    if (tile == num_tiles - 1 && threadIdx.x == 0) {
-      if (incl_total > fc.max_pairs) { counters->overflow = 1; counters->n_pairs = 0; }
-      else counters->n_pairs = incl_total;
+    for (int j = 0; j < SCAN_IPT; ++j) {
+      a[j] = 0;
+      if (i0 + j < n) { const uint2 r = rec_rect[sorted_g[i0 + j]]; a[j] = ((r.x >> 16) - (r.x & 0xffffu)) * ((r.y >> 16) - (r.y & 0xffffu)); }
     }
+    const uint32_t tsum = a[0] + a[1] + a[2] + a[3];
+    uint32_t incl_total;
+    uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total);
+    if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
 #pragma unroll
-    for (int i = 0; i < SCAN_IPT; ++i) { if (i0 + i < n) offsets[i0 + i] = off; off += c[i]; }
+    for (int j = 0; j < SCAN_IPT; ++j) {
+      if (i0 + j >= n) break;
+      area_prefix[i0 + j] = off;
+      const unsigned long long end = (unsigned long long)off + a[j];
+      for (unsigned long long kb = ((unsigned long long)off + BIN_CHUNK - 1) / BIN_CHUNK; kb * BIN_CHUNK < end; ++kb) {
+        chunk_first[kb] = i0 + j;
+        bin_desc[kb] = 0ull;
+      }
+      off += a[j];
+    }
   }
 }
 
-// One warp per emitting Gaussian, items dealt round-robin to the warps of the grid: in depth order the nearest
-// Gaussians -- the ones covering hundreds or thousands of tiles -- are neighbours, and this spreads them over all SMs.
-// Pairs are written in the oracle's order (ty ascending, then tx) at offsets[i].
-__global__ void __launch_bounds__(256) k_emit(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ offsets,
-                                              const uint2* __restrict__ rec_rect, const float4* __restrict__ rec_uvdo,
-                                              const float4* __restrict__ rec_conic, const uint32_t* __restrict__ sel_bits,
-                                              uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                              const Counters* __restrict__ counters) {
-  if (counters->overflow) return;
-  const uint32_t n = counters->n_emit;
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t nwarps = gridDim.x * (blockDim.x >> 5);
-  for (uint32_t i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); i < n; i += nwarps) {
-    const uint32_t g = sorted_g[i];
-    uint32_t off = offsets[i];
-    const uint2 r = rec_rect[g];
-    const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
-    const uint32_t w = x_hi - x_lo, area = w * (y_hi - y_lo);
-    float4 uv, cn;
-    if (fc.exact_tiles) { uv = rec_uvdo[g]; cn = rec_conic[g]; }
-    for (uint32_t base = 0; base < area; base += 32) {
-      const uint32_t idx = base + lane;
-      const uint32_t ry = idx / w, ty = y_lo + ry, tx = x_lo + (idx - ry * w);
-      const uint32_t t = ty * fc.cam.TX + tx;
-      bool sel = idx < area && (fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u));
-      if (sel && fc.exact_tiles) sel = tile_alpha_reach(uv.x, uv.y, cn.x, cn.y, cn.z, cn.w, tx, ty, fc.cam.W, fc.cam.H);   // R39
-      const uint32_t bal = __ballot_sync(0xffffffffu, sel);
-      if (sel) {
-        const uint32_t p = off + __popc(bal & ((1u << lane) - 1u));
-        keys[p] = t;
-        vals[p] = g;
-      }
-      off += __popc(bal);
+__device__ __forceinline__ void sh_basis(int deg, float x, float y, float z, float* Y) {   // R5
+  Y[0] = 0.28209479177387814f;
+  if (deg < 1) return;
+  Y[1] = -0.4886025119029199f * y; Y[2] = 0.4886025119029199f * z; Y[3] = -0.4886025119029199f * x;
+  if (deg < 2) return;
+  const float xx = x * x, yy = y * y, zz = z * z, xy = x * y, yz = y * z, xz = x * z;
+  Y[4] = 1.0925484305920792f * xy; Y[5] = -1.0925484305920792f * yz;
+  Y[6] = 0.31539156525252005f * (2.0f * zz - xx - yy);
+  Y[7] = -1.0925484305920792f * xz; Y[8] = 0.5462742152960396f * (xx - yy);
+  if (deg < 3) return;
+  Y[9] = -0.5900435899266435f * y * (3.0f * xx - yy);
+  Y[10] = 2.890611442640554f * xy * z;
+  Y[11] = -0.4570457994644658f * y * (4.0f * zz - xx - yy);
+  Y[12] = 0.3731763325901154f * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
+  Y[13] = -0.4570457994644658f * x * (4.0f * zz - xx - yy);
+  Y[14] = 1.445305721320277f * z * (xx - yy);
+  Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
+}
+
+template <int DEG>
+__device__ __forceinline__ void sh_colour(const FrameConst& fc, uint32_t g, const float4* __restrict__ cull4, const float* __restrict__ sh,
+                                          float4* __restrict__ rec_rgb) {
+  constexpr int K = (DEG + 1) * (DEG + 1);
+  const float4 c4 = cull4[g];
+  float dx = c4.x - fc.cam.campos[0], dy = c4.y - fc.cam.campos[1], dz = c4.z - fc.cam.campos[2];
+  const float inv = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
+  dx *= inv; dy *= inv; dz *= inv;
+  float Y[K];
+  sh_basis(DEG, dx, dy, dz, Y);
+  float cr = 0.5f, cg = 0.5f, cb = 0.5f;
+  const float* p = sh + (size_t)g * K * 3;
+  if constexpr (K % 4 == 0) {            // K*3 floats = 3K/4 float4, 16 B aligned
+    const float4* p4 = reinterpret_cast<const float4*>(p);
+    float buf[K * 3];
+#pragma unroll
+    for (int i = 0; i < K * 3 / 4; ++i) {
+      const float4 t = __ldg(p4 + i);
+      buf[4 * i] = t.x; buf[4 * i + 1] = t.y; buf[4 * i + 2] = t.z; buf[4 * i + 3] = t.w;
     }
+#pragma unroll
+    for (int kk = 0; kk < K; ++kk) { cr += Y[kk] * buf[3 * kk]; cg += Y[kk] * buf[3 * kk + 1]; cb += Y[kk] * buf[3 * kk + 2]; }
+  } else {
+#pragma unroll
+    for (int kk = 0; kk < K; ++kk) { cr += Y[kk] * p[3 * kk]; cg += Y[kk] * p[3 * kk + 1]; cb += Y[kk] * p[3 * kk + 2]; }
+  }
+  rec_rgb[g] = make_float4(fmaxf(cr, 0.0f), fmaxf(cg, 0.0f), fmaxf(cb, 0.0f), 0.0f);
+}
+
+// ================================================================== A5b: tests -> pairs, counts, colours
+struct BinSmem {
+  uint32_t prefix[BIN_CHUNK + 2];   // area_prefix of the Gaussians of this chunk (+ sentinel)
+  uint32_t st_tile[BIN_CHUNK];      // passing tests of the chunk, in order: tile id
+  uint32_t st_g[BIN_CHUNK];         //                                        Gaussian
+  uint8_t has[BIN_CHUNK + 8];       // Gaussian (chunk-local) emitted at least one pair here
+  uint32_t warp[BIN_THREADS / 32];
+  uint32_t excl, chunk;
+};
+
+struct BinGauss {                   // the Gaussian a thread is currently testing
+  uint32_t g, start, end, x_lo, y_lo, w;
+  float u, v, A, B, C, tau;
+};
+
+template <int DEG>
+__global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
+                                                     const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
+                                                     const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                     const uint32_t* __restrict__ sel_bits, const float4* __restrict__ cull4,
+                                                     const float* __restrict__ sh, unsigned long long* __restrict__ desc,
+                                                     uint32_t* __restrict__ tiles_touched, float4* __restrict__ rec_rgb,
+                                                     uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, Counters* __restrict__ counters) {
+  __shared__ BinSmem sm;
+  const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
+  const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
+  const uint32_t tid = threadIdx.x;
+  const int TX = fc.cam.TX;
+  while (true) {
+    __syncthreads();
+    if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin, 1u);
+    __syncthreads();
+    const uint32_t chunk = sm.chunk;
+    if (chunk >= num_chunks) break;
+    const uint32_t cbase = chunk * BIN_CHUNK;
+    const uint32_t tend = (total_tests - cbase < (uint32_t)BIN_CHUNK) ? total_tests : cbase + BIN_CHUNK;
+    const uint32_t i_first = chunk_first[chunk];
+    const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
+    const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
+    for (uint32_t i = tid; i <= m; i += BIN_THREADS) { sm.prefix[i] = area_prefix[i_first + i]; sm.has[i] = 0; }
+    __syncthreads();
+    // ---------------------------------------------------------------- tests
+    const uint32_t t0 = cbase + tid * BIN_IPT;
+    uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
+    if (t0 < tend) {
+      uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
+      while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
+      uint32_t li = lo, segcnt = 0;
+      BinGauss G;
+      auto load = [&](uint32_t l) {
+        G.g = sorted_g[i_first + l];
+        G.start = sm.prefix[l]; G.end = sm.prefix[l + 1];
+        const uint2 r = rec_rect[G.g];
+        G.x_lo = r.x & 0xffffu; G.y_lo = r.y & 0xffffu; G.w = (r.x >> 16) - G.x_lo;
+        if (fc.exact_tiles) {
+          const float4 a = rec_uvdo[G.g], b = rec_conic[G.g];
+          G.u = a.x; G.v = a.y; G.A = b.x; G.B = b.y; G.C = b.z; G.tau = b.w;
+        }
+      };
+      auto flush = [&]() {
+        if (segcnt) { atomicAdd(&tiles_touched[G.g], segcnt); sm.has[li] = 1; }
+        segcnt = 0;
+      };
+      load(li);
+#pragma unroll
+      for (int k = 0; k < BIN_IPT; ++k) {
+        const uint32_t t = t0 + k;
+        if (t < tend) {
+          if (t >= G.end) { flush(); do { ++li; } while (sm.prefix[li + 1] <= t); load(li); }
+          const uint32_t local = t - G.start, ry = local / G.w;
+          const uint32_t tx = G.x_lo + (local - ry * G.w), ty = G.y_lo + ry, tile = ty * TX + tx;
+          bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
+          if (pass && fc.exact_tiles) pass = tile_alpha_reach(G.u, G.v, G.A, G.B, G.C, G.tau, tx, ty, fc.cam.W, fc.cam.H);   // R39
+          if (pass) { mask |= 1u << k; ++segcnt; }
+          tl[k] = tile; gg[k] = G.g;
+        }
+      }
+      flush();
+    }
+    // ---------------------------------------------------------------- rank the passing tests (chunk-local + global)
+    uint32_t incl_total;
+    const uint32_t goff = tgs_scan::chunk_scan<BIN_THREADS>(__popc(mask), chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total);
+    const uint32_t cexcl = sm.excl, ctotal = incl_total - cexcl;
+    const bool overflow = incl_total > fc.max_pairs;
+    if (chunk == num_chunks - 1 && tid == 0) {
+      if (overflow) { counters->overflow = 1; counters->n_pairs = 0; }
+      else counters->n_pairs = incl_total;
+    }
+    uint32_t lpos = goff - cexcl;
+#pragma unroll
+    for (int k = 0; k < BIN_IPT; ++k)
+      if ((mask >> k) & 1u) { sm.st_tile[lpos] = tl[k]; sm.st_g[lpos] = gg[k]; ++lpos; }
+    __syncthreads();
+    if (!overflow)
+      for (uint32_t p = tid; p < ctotal; p += BIN_THREADS) { keys[cexcl + p] = sm.st_tile[p]; vals[cexcl + p] = sm.st_g[p]; }
+    // ---------------------------------------------------------------- colours of the Gaussians that emitted here
+    for (uint32_t l = tid; l < m; l += BIN_THREADS)
+      if (sm.has[l]) sh_colour<DEG>(fc, sorted_g[i_first + l], cull4, sh, rec_rgb);
   }
 }
 
@@ -196,22 +250,27 @@ __global__ void __launch_bounds__(256) k_keys64(const uint32_t* __restrict__ key
 }  // namespace
 
 uint32_t scan_tile_items() { return SCAN_TILE; }
+uint32_t bin_chunk_items() { return BIN_CHUNK; }
 
-void launch_compact(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-  const uint32_t num_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;
-  cudaMemsetAsync(b.scan_desc, 0, (size_t)(num_tiles + 1) * sizeof(uint64_t), s);
-  const uint32_t grid = num_tiles < (uint32_t)(num_sms * 4) ? num_tiles : (uint32_t)(num_sms * 4);
-  k_compact<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc.n, b.tiles_touched, b.rec_uvdo, (unsigned long long*)b.scan_desc, b.ckeys[0],
-                                                    b.cvals[0], b.counters);
-}
-
-void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms) {
-  const uint32_t num_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_emit <= N)
-  cudaMemsetAsync(b.scan_desc, 0, (size_t)(num_tiles + 1) * sizeof(uint64_t), s);
-  const uint32_t grid = num_tiles < (uint32_t)(num_sms * 4) ? num_tiles : (uint32_t)(num_sms * 4);
-  k_scan_offsets<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, b.cvals[sorted_g_idx], b.tiles_touched, (unsigned long long*)b.scan_desc,
-                                                         b.offsets, b.counters);
-  k_emit<<<num_sms * 8, 256, 0, s>>>(fc, b.cvals[sorted_g_idx], b.offsets, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, b.keys[0], b.vals[0], b.counters);
+// sorted_g_idx: which of cvals[] holds the visible Gaussians in (depth, index) order
+void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms) {
+  const uint32_t scan_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_visible <= N)
+  const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
+  const uint32_t* sorted_g = b.cvals[sorted_g_idx];
+  uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
+  k_scan_area<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, sorted_g, b.rec_rect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
+                                                      (unsigned long long*)b.bin_desc, b.counters, max_tests);
+  grid = (uint32_t)(num_sms * 4);
+#define LAUNCH(D)                                                                                                                     \
+  k_bin<D><<<grid, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, \
+                                        b.cull4, b.sh, (unsigned long long*)b.bin_desc, b.tiles_touched, b.rec_rgb, b.keys[0], b.vals[0], b.counters)
+  switch (fc.sh_degree) {
+    case 0: LAUNCH(0); break;
+    case 1: LAUNCH(1); break;
+    case 2: LAUNCH(2); break;
+    default: LAUNCH(3); break;
+  }
+#undef LAUNCH
 }
 
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms) {

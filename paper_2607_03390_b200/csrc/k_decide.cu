@@ -8,6 +8,7 @@
 // A5a count + SH colour, F reduction (L109).
 #include "tgs_internal.cuh"
 #include "decide_math.cuh"
+#include "scan.cuh"
 
 namespace {
 
@@ -26,11 +27,13 @@ __device__ __forceinline__ float key2f(uint32_t k) {
 // Sigma = R S S^T R^T, quaternion (w,x,y,z) normalised; tau = 2 ln(255 o) (L119, R18).
 __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restrict__ means, const float* __restrict__ scales,
                                                 const float* __restrict__ quats, const float* __restrict__ opacity,
-                                                float4* __restrict__ cull4, float* __restrict__ cov3d, float* __restrict__ tau) {
+                                                float4* __restrict__ cull4, float4* __restrict__ g2) {
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
   const float o = opacity[g];
-  cull4[g] = make_float4(means[3 * g], means[3 * g + 1], means[3 * g + 2], o);
+  // cull record: mean + the largest scale (bounds the screen extent without the covariance, see k_preprocess)
+  cull4[g] = make_float4(means[3 * g], means[3 * g + 1], means[3 * g + 2],
+                         fmaxf(fabsf(scales[3 * g]), fmaxf(fabsf(scales[3 * g + 1]), fabsf(scales[3 * g + 2]))));
   float w = quats[4 * g], x = quats[4 * g + 1], y = quats[4 * g + 2], z = quats[4 * g + 3];
   const float nrm = sqrtf(((w * w + x * x) + y * y) + z * z);
   w /= nrm; x /= nrm; y /= nrm; z /= nrm;
@@ -43,22 +46,26 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 #pragma unroll
     for (int k = 0; k < 3; ++k) Mx[i * 3 + k] = R[i * 3 + k] * scales[3 * g + k];
 #define SIG(i, j) ((Mx[(i) * 3] * Mx[(j) * 3] + Mx[(i) * 3 + 1] * Mx[(j) * 3 + 1]) + Mx[(i) * 3 + 2] * Mx[(j) * 3 + 2])
-  float* c = cov3d + 6 * (size_t)g;
-  c[0] = SIG(0, 0); c[1] = SIG(0, 1); c[2] = SIG(0, 2); c[3] = SIG(1, 1); c[4] = SIG(1, 2); c[5] = SIG(2, 2);
+  // second-stage record, 32 B: Sigma (xx,xy,xz,yy,yz,zz), opacity, tau
+  g2[2 * (size_t)g] = make_float4(SIG(0, 0), SIG(0, 1), SIG(0, 2), SIG(1, 1));
+  g2[2 * (size_t)g + 1] = make_float4(SIG(1, 2), SIG(2, 2), o, (float)(2.0 * log(255.0 * (double)o)));
 #undef SIG
-  tau[g] = (float)(2.0 * log(255.0 * (double)o));
 }
 
 // ------------------------------------------------------------------ per-frame init
-// counters <- 0; tile_flags <- 0; S frames: D^min <- INVALID bits, sigma^max <- 0;
-// R / P frames: rendered_next <- 0; R frames: F <- (+inf, +inf, -inf, -inf).
+// counters <- 0; tile_flags <- 0; tiles_touched <- 0; look-back descriptors of the preprocess chunks <- 0;
+// S frames: D^min <- INVALID bits, sigma^max <- 0; R / P frames: rendered_next <- 0;
+// R frames: F <- (+inf, +inf, -inf, -inf).
 __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint32_t* warp_depth,
                                                     uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
+                                                    uint4* tiles_touched4, uint32_t n_tt4, uint2* pre_desc, uint32_t n_desc,
                                                     uint32_t* F_key, int reset_F) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
   if (tid < sizeof(Counters) / 4) ((uint32_t*)counters)[tid] = 0;
   if (reset_F && tid < 4) F_key[tid] = (tid < 2) ? 0xff800000u /* key(+inf) */ : 0x007fffffu /* key(-inf) */;
   for (uint32_t i = tid; i < (uint32_t)fc.n_tiles; i += nth) tile_flags[i] = 0;
+  for (uint32_t i = tid; i < n_tt4; i += nth) tiles_touched4[i] = make_uint4(0u, 0u, 0u, 0u);
+  for (uint32_t i = tid; i < n_desc; i += nth) pre_desc[i] = make_uint2(0u, 0u);
   if (fc.do_tgb) {
     const uint32_t px = (uint32_t)(fc.cam.W * fc.cam.H);
     for (uint32_t i = tid; i < px; i += nth) { warp_depth[i] = TGS_INVALID_BITS; warp_sigma[i] = 0; }
@@ -152,73 +159,156 @@ __device__ __forceinline__ void mark_oc_tile(const CamConst& k, float u, float v
     if (!(atomicOr(&tile_flags[t], 1u) & 1u)) atomicAdd(&counters->n_oc_marked, 1u);
 }
 
-// Newly visible Gaussians with large rects (queued by k_preprocess): one warp per Gaussian, lanes over the tiles
-// of the rect.  Stops as soon as every tile of the frame carries the T^oc mark.
-__global__ void __launch_bounds__(256) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_uvdo,
+// Newly visible Gaussians with rects of more than 4 tiles (queued by k_preprocess): one CTA per Gaussian, threads
+// over the tiles of the rect (a near Gaussian covers thousands).  Stops as soon as every tile carries the mark.
+__global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_uvdo,
                                                  const float4* __restrict__ rec_conic, const uint2* __restrict__ rec_rect,
                                                  uint32_t* __restrict__ tile_flags, Counters* __restrict__ counters) {
   const CamConst& k = fc.cam;
-  const uint32_t lane = threadIdx.x & 31;
   const uint32_t nq = counters->n_nv_queue;
-  while (true) {
-    uint32_t j = 0;
-    if (lane == 0) j = atomicAdd(&counters->ticket_mark, 1u);
-    j = __shfl_sync(0xffffffffu, j, 0);
-    if (j >= nq) break;
+  for (uint32_t j = blockIdx.x; j < nq; j += gridDim.x) {
     if (*reinterpret_cast<volatile uint32_t*>(&counters->n_oc_marked) >= (uint32_t)fc.n_tiles) break;
     const uint32_t g = nv_queue[j];
     const float4 r0 = rec_uvdo[g], r1 = rec_conic[g];
     const uint2 r = rec_rect[g];
     const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
     const uint32_t w = x_hi - x_lo, area = w * (y_hi - y_lo);
-    for (uint32_t i = lane; i < area; i += 32) mark_oc_tile(k, r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, x_lo + i % w, y_lo + i / w, tile_flags, counters);
+    for (uint32_t i = threadIdx.x; i < area; i += blockDim.x) {
+      const uint32_t ry = i / w;
+      mark_oc_tile(k, r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, x_lo + (i - ry * w), y_lo + ry, tile_flags, counters);
+    }
   }
 }
 
 // ------------------------------------------------------------------ A3 preprocess (+AFC +TOC +newly-visible +T^oc)
-// One thread per Gaussian.  The 16 B cull record {mean, opacity} is read for all N; the 24 B covariance only
-// for Gaussians that survive near / AFC / TOC; SH (the bulk of the bytes) is not touched here at all.
-// Order of the tests and of every fp32 operation: DESIGN.md §2 (O3), identical to what the oracle states.
-__global__ void __launch_bounds__(256) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float* __restrict__ cov3d,
-                                                    const float* __restrict__ tau_arr, const uint8_t* __restrict__ rendered,
-                                                    const float* __restrict__ warp_depth, const float* __restrict__ warp_sigma,
-                                                    const uint32_t* __restrict__ F_key, float4* __restrict__ rec_uvdo,
-                                                    float4* __restrict__ rec_conic, uint2* __restrict__ rec_rect,
-                                                    uint32_t* __restrict__ rec_flags, float4* __restrict__ rec_b0,
-                                                    float4* __restrict__ rec_b1, uint32_t* __restrict__ tile_flags,
-                                                    uint32_t* __restrict__ nv_queue, Counters* __restrict__ counters) {
-  const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+// Persistent grid; a work item is a chunk of 1024 consecutive Gaussians (ticket order), 4 per thread.
+//  phase A (all Gaussians, 16 B each): near cull, projection of the mean, AFC, TOC + newly-visible lookups in the
+//          warped TGB, and a conservative off-screen test; the survivors are compacted in shared memory;
+//  phase B (survivors only, +32 B each): EWA covariance, conic, radius, rect, records, T^oc marks of small rects;
+//  phase C: the visible Gaussians of the chunk are appended, in ascending index order, to the list the depth sort
+//          works on (single-pass scan with decoupled look-back over the chunks).
+// SH (the bulk of the scene bytes) is not touched here at all.  Order of the tests and of every fp32 operation of a
+// decision: DESIGN.md §2 (O3), identical to what the oracle states.
+//
+// Off-screen test (an early-out, never a different decision): with s = the largest scale, lambda_max(Sigma') <=
+// |J|_F^2 s^2 + 0.3 and |J row|^2 <= (f/z)^2 (1 + lim^2) because the Jacobian's x/z, y/z are clamped to +-lim (R3), so
+// r <= 3 sqrt(lambda_b + 0.32) + 1.  A Gaussian whose centre is further outside the tile grid than this bound has an
+// empty rect.  It is only applied when lambda_b <= 1e4: then det(Sigma') >= 0.3 (a + c) - rounding(1e-6 a c) > 0, so
+// the Gaussian cannot be one the full computation would have flagged DEGENERATE instead of EMPTY.
+constexpr int PRE_THREADS = 256;
+constexpr int PRE_IPT = 4;
+constexpr int PRE_CHUNK = PRE_THREADS * PRE_IPT;
+
+struct PreSmem {
+  uint16_t list[PRE_CHUNK];     // survivors of phase A: local index | newly-visible << 15 | visible << 14
+  uint32_t depth[PRE_CHUNK];    // bits(d) of the visible survivors (indexed like list)
+  uint32_t warp[PRE_THREADS / 32];
+  uint32_t excl, chunk, nsurv;
+  uint32_t stat[8];
+  unsigned long long area;
+};
+
+__global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
+                                                               const uint8_t* __restrict__ rendered, const float* __restrict__ warp_depth,
+                                                               const float* __restrict__ warp_sigma, const uint32_t* __restrict__ F_key,
+                                                               float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
+                                                               uint2* __restrict__ rec_rect, uint32_t* __restrict__ rec_flags,
+                                                               float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
+                                                               uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
+                                                               unsigned long long* __restrict__ desc, uint32_t* __restrict__ vis_keys,
+                                                               uint32_t* __restrict__ vis_vals, Counters* __restrict__ counters) {
+  __shared__ PreSmem sm;
   const CamConst& k = fc.cam;
   const float* V = k.V;
-  uint32_t flags = 0;
-  if (g < fc.n) {
-    const float4 c4 = cull4[g];
-    const float x = c4.x, y = c4.y, z = c4.z;
-    const float tx = ((V[0] * x + V[1] * y) + V[2] * z) + V[3];
-    const float ty = ((V[4] * x + V[5] * y) + V[6] * z) + V[7];
-    const float tz = ((V[8] * x + V[9] * y) + V[10] * z) + V[11];
-    do {
-      if (!(tz > k.znear)) { flags = TGS_CULL_NEAR; break; }                       // L61, R4
+  const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const uint32_t num_chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
+  float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f;
+  if (fc.do_afc) { F0 = key2f(F_key[0]); F1 = key2f(F_key[1]); F2 = key2f(F_key[2]); F3 = key2f(F_key[3]); }
+  const float offx = 1.0f + k.limx * k.limx, offy = 1.0f + k.limy * k.limy;
+  const float xmax = (float)(k.TX * TGS_TILE) + 2.0f, ymax = (float)(k.TY * TGS_TILE) + 2.0f;
+  uint32_t st_near = 0, st_afc = 0, st_toc = 0, st_deg = 0, st_empty = 0, st_nv = 0;
+  unsigned long long st_area = 0;
+  if (tid < 8) sm.stat[tid] = 0;
+  if (tid == 0) sm.area = 0;
+  while (true) {
+    __syncthreads();
+    if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_pre, 1u);
+    __syncthreads();
+    const uint32_t chunk = sm.chunk;
+    if (chunk >= num_chunks) break;
+    const uint32_t base = chunk * PRE_CHUNK;
+    // ---------------------------------------------------------------- phase A
+    const uint32_t g0 = base + tid * PRE_IPT;
+    float4 c4[PRE_IPT];
+#pragma unroll
+    for (int j = 0; j < PRE_IPT; ++j) c4[j] = (g0 + j < fc.n) ? cull4[g0 + j] : make_float4(0.f, 0.f, 0.f, 0.f);
+    uint32_t rend4 = 0;
+    if (fc.do_tgb && g0 < fc.n) rend4 = *reinterpret_cast<const uint32_t*>(rendered + g0);   // g0 % 4 == 0; padded allocation
+    uint32_t surv = 0;      // 4 x {bit0 survivor, bit1 newly visible}
+    uint32_t cf[PRE_IPT] = {0u, 0u, 0u, 0u};   // flags of the Gaussians culled in phase A (survivors: written in phase B)
+#pragma unroll
+    for (int j = 0; j < PRE_IPT; ++j) {
+      const uint32_t g = g0 + j;
+      if (g >= fc.n) continue;
+      const float x = c4[j].x, y = c4[j].y, z = c4[j].z;
+      const float tx = ((V[0] * x + V[1] * y) + V[2] * z) + V[3];
+      const float ty = ((V[4] * x + V[5] * y) + V[6] * z) + V[7];
+      const float tz = ((V[8] * x + V[9] * y) + V[10] * z) + V[11];
+      if (!(tz > k.znear)) { cf[j] = TGS_CULL_NEAR; ++st_near; continue; }                 // L61, R4
       const float u = (k.fx * tx) / tz + k.cx, v = (k.fy * ty) / tz + k.cy;
-      if (fc.do_afc) {                                                             // L109-111
-        const float F0 = key2f(F_key[0]), F1 = key2f(F_key[1]), F2 = key2f(F_key[2]), F3 = key2f(F_key[3]);
+      if (fc.do_afc) {                                                                            // L109-111
         const float nx = (2.0f * u + 1.0f) / k.Wf - 1.0f, ny = (2.0f * v + 1.0f) / k.Hf - 1.0f;
-        if (!(F0 <= nx && nx <= F2 && F1 <= ny && ny <= F3)) { flags = TGS_CULL_AFC; break; }
+        if (!(F0 <= nx && nx <= F2 && F1 <= ny && ny <= F3)) { cf[j] = TGS_CULL_AFC; ++st_afc; continue; }
       }
       uint32_t fl = 0;
-      if (fc.do_tgb && !rendered[g]) {                                             // L113, L119
-        const float fu = floorf(u + 0.5f), fv = floorf(v + 0.5f);
-        if (fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf) {
-          const size_t q = (size_t)(int)fv * k.W + (int)fu;
-          const float D = warp_depth[q], s = warp_sigma[q];
-          if (fc.do_toc && tz > D + fc.lambda2 * s) { flags = TGS_CULL_TOC; break; }
-          if (tz <= D - fc.lambda1 * s) fl = TGS_NEWLY_VISIBLE;
+      const float fu = floorf(u + 0.5f), fv = floorf(v + 0.5f);
+      const bool centre_in = fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf;
+      if (fc.do_tgb && !((rend4 >> (8 * j)) & 0xffu) && centre_in) {                              // L113, L119
+        const size_t q = (size_t)(int)fv * k.W + (int)fu;
+        const float D = warp_depth[q], s = warp_sigma[q];
+        if (fc.do_toc && tz > D + fc.lambda2 * s) { cf[j] = TGS_CULL_TOC; ++st_toc; continue; }
+        if (tz <= D - fc.lambda1 * s) fl = 2u;
+      }
+      if (!centre_in) {                                                                           // provably empty rect
+        const float kx = k.fx / tz, ky = k.fy / tz;
+        const float lam_b = (((kx * kx) * offx + (ky * ky) * offy) * (c4[j].w * c4[j].w)) * 1.02f + 0.7f;
+        if (lam_b <= 1.0e4f) {
+          const float rb = 3.03f * sqrtf(lam_b) + 3.0f;
+          if (u + rb < -17.0f || v + rb < -17.0f || u - rb > xmax || v - rb > ymax) { cf[j] = TGS_CULL_EMPTY; ++st_empty; continue; }
         }
       }
-      const float2 s01 = *reinterpret_cast<const float2*>(cov3d + 6 * (size_t)g);
-      const float2 s23 = *reinterpret_cast<const float2*>(cov3d + 6 * (size_t)g + 2);
-      const float2 s45 = *reinterpret_cast<const float2*>(cov3d + 6 * (size_t)g + 4);
-      const float S0 = s01.x, S1 = s01.y, S2 = s23.x, S3 = s23.y, S4 = s45.x, S5 = s45.y;
+      surv |= (1u | fl) << (2 * j);
+    }
+    if (g0 + PRE_IPT <= fc.n) *reinterpret_cast<uint4*>(rec_flags + g0) = make_uint4(cf[0], cf[1], cf[2], cf[3]);
+    else
+      for (int j = 0; j < PRE_IPT; ++j) if (g0 + j < fc.n) rec_flags[g0 + j] = cf[j];
+    // survivors -> sm.list, in ascending index order
+    const uint32_t ns_t = (surv & 1u) + ((surv >> 2) & 1u) + ((surv >> 4) & 1u) + ((surv >> 6) & 1u);
+    uint32_t incl = ns_t;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
+    if (lane == 31) sm.warp[wid] = incl;
+    __syncthreads();
+    uint32_t pos = incl - ns_t, total = 0;
+#pragma unroll
+    for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < wid) pos += t; total += t; }
+#pragma unroll
+    for (int j = 0; j < PRE_IPT; ++j)
+      if ((surv >> (2 * j)) & 1u) sm.list[pos++] = (uint16_t)((tid * PRE_IPT + j) | (((surv >> (2 * j + 1)) & 1u) << 15));
+    __syncthreads();
+    // ---------------------------------------------------------------- phase B
+    for (uint32_t i = tid; i < total; i += PRE_THREADS) {
+      const uint32_t e = sm.list[i];
+      const uint32_t g = base + (e & 0x3ffu);
+      const uint32_t fl = (e >> 15) ? TGS_NEWLY_VISIBLE : 0u;
+      const float4 c = cull4[g];
+      const float4 ga = g2[2 * (size_t)g], gb = g2[2 * (size_t)g + 1];
+      const float x = c.x, y = c.y, z = c.z;
+      const float tx = ((V[0] * x + V[1] * y) + V[2] * z) + V[3];
+      const float ty = ((V[4] * x + V[5] * y) + V[6] * z) + V[7];
+      const float tz = ((V[8] * x + V[9] * y) + V[10] * z) + V[11];
+      const float u = (k.fx * tx) / tz + k.cx, v = (k.fy * ty) / tz + k.cy;
+      const float S0 = ga.x, S1 = ga.y, S2 = ga.z, S3 = ga.w, S4 = gb.x, S5 = gb.y, opac = gb.z, tau = gb.w;
       const float rxz = tx / tz, ryz = ty / tz;
       const float jx = fminf(k.limx, fmaxf(-k.limx, rxz)) * tz;
       const float jy = fminf(k.limy, fmaxf(-k.limy, ryz)) * tz;
@@ -234,11 +324,11 @@ __global__ void __launch_bounds__(256) k_preprocess(FrameConst fc, const float4*
       const float q2 = (S2 * T10 + S4 * T11) + S5 * T12;
       const float a = ((T00 * a0 + T01 * a1) + T02 * a2) + 0.3f;
       const float b = (T10 * a0 + T11 * a1) + T12 * a2;
-      const float c = ((T10 * q0 + T11 * q1) + T12 * q2) + 0.3f;
-      const float det = a * c - b * b;
-      if (!(det > 0.0f)) { flags = TGS_CULL_DEGENERATE; break; }
-      const float A = c / det, B = -b / det, C = a / det;
-      const float mid = 0.5f * (a + c);
+      const float cc = ((T10 * q0 + T11 * q1) + T12 * q2) + 0.3f;
+      const float det = a * cc - b * b;
+      if (!(det > 0.0f)) { rec_flags[g] = TGS_CULL_DEGENERATE; ++st_deg; continue; }
+      const float A = cc / det, B = -b / det, C = a / det;
+      const float mid = 0.5f * (a + cc);
       const float lam = mid + sqrtf(fmaxf(0.1f, mid * mid - det));
       const float rad = ceilf(3.0f * sqrtf(lam));
       const float TXf = (float)k.TX, TYf = (float)k.TY;
@@ -246,215 +336,120 @@ __global__ void __launch_bounds__(256) k_preprocess(FrameConst fc, const float4*
       const uint32_t x_hi = (uint32_t)fminf(fmaxf(floorf((u + rad + 15.0f) / 16.0f), 0.0f), TXf);
       const uint32_t y_lo = (uint32_t)fminf(fmaxf(floorf((v - rad) / 16.0f), 0.0f), TYf);
       const uint32_t y_hi = (uint32_t)fminf(fmaxf(floorf((v + rad + 15.0f) / 16.0f), 0.0f), TYf);
-      if (!(x_hi > x_lo && y_hi > y_lo)) { flags = TGS_CULL_EMPTY; break; }
-      flags = fl | TGS_VISIBLE;
-      const float tau = tau_arr[g];
-      rec_uvdo[g] = make_float4(u, v, tz, c4.w);
+      if (!(x_hi > x_lo && y_hi > y_lo)) { rec_flags[g] = TGS_CULL_EMPTY; ++st_empty; continue; }
+      rec_flags[g] = fl | TGS_VISIBLE;
+      if (fl) ++st_nv;
+      const uint32_t area = (x_hi - x_lo) * (y_hi - y_lo);
+      st_area += area;
+      rec_uvdo[g] = make_float4(u, v, tz, opac);
       rec_conic[g] = make_float4(A, B, C, tau);
       rec_rect[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
       // blend-side parameters: the quadratic form as a sum of two squares (no cancellation between its terms)
-      rec_b0[g] = make_float4(u, v, -0.72134752f * A, -b / c);
-      rec_b1[g] = make_float4(-0.72134752f / c, log2f(c4.w), tz, 0.0f);
+      rec_b0[g] = make_float4(u, v, -0.72134752f * A, -b / cc);
+      rec_b1[g] = make_float4(-0.72134752f / cc, log2f(opac), tz, 0.0f);
+      sm.list[i] = (uint16_t)(e | 0x4000u);
+      sm.depth[i] = __float_as_uint(tz);
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)
-        if ((x_hi - x_lo) * (y_hi - y_lo) > 16u) nv_queue[atomicAdd(&counters->n_nv_queue, 1u)] = g;   // large rect: k_mark_oc
+        if (area > 4u) nv_queue[atomicAdd(&counters->n_nv_queue, 1u)] = g;         // larger rects: k_mark_oc
         else
           for (uint32_t tyy = y_lo; tyy < y_hi; ++tyy)
             for (uint32_t txx = x_lo; txx < x_hi; ++txx) mark_oc_tile(k, u, v, A, B, C, tau, txx, tyy, tile_flags, counters);
       }
-    } while (false);
-    rec_flags[g] = flags;
+    }
+    __syncthreads();
+    // ---------------------------------------------------------------- phase C: visible list, ascending index
+    uint32_t nv_t = 0;
+#pragma unroll
+    for (int j = 0; j < PRE_IPT; ++j) { const uint32_t i = tid * PRE_IPT + j; if (i < total && (sm.list[i] & 0x4000u)) ++nv_t; }
+    uint32_t incl_total;
+    uint32_t off = tgs_scan::chunk_scan<PRE_THREADS>(nv_t, chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total);
+    if (chunk == num_chunks - 1 && tid == 0) counters->n_visible = incl_total;
+#pragma unroll
+    for (int j = 0; j < PRE_IPT; ++j) {
+      const uint32_t i = tid * PRE_IPT + j;
+      if (i < total && (sm.list[i] & 0x4000u)) { vis_keys[off] = sm.depth[i]; vis_vals[off] = base + (sm.list[i] & 0x3ffu); ++off; }
+    }
   }
-  // statistics: one atomic per warp and non-zero class
-  const uint32_t lane = threadIdx.x & 31;
-#define COUNT(bit, field)                                              \
-  {                                                                    \
-    const uint32_t m = __ballot_sync(0xffffffffu, (flags & (bit)) != 0); \
-    if (m && lane == 0) atomicAdd(&counters->field, __popc(m));        \
+  // statistics: one atomic per CTA and class
+  st_near = warp_sum(st_near); st_afc = warp_sum(st_afc); st_toc = warp_sum(st_toc); st_deg = warp_sum(st_deg);
+  st_empty = warp_sum(st_empty); st_nv = warp_sum(st_nv);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) st_area += __shfl_xor_sync(0xffffffffu, st_area, d);
+  if (lane == 0) {
+    if (st_near) atomicAdd(&sm.stat[0], st_near);
+    if (st_afc) atomicAdd(&sm.stat[1], st_afc);
+    if (st_toc) atomicAdd(&sm.stat[2], st_toc);
+    if (st_deg) atomicAdd(&sm.stat[3], st_deg);
+    if (st_empty) atomicAdd(&sm.stat[4], st_empty);
+    if (st_nv) atomicAdd(&sm.stat[6], st_nv);
+    if (st_area) atomicAdd(&sm.area, st_area);
   }
-  COUNT(TGS_CULL_NEAR, n_near) COUNT(TGS_CULL_AFC, n_afc) COUNT(TGS_CULL_TOC, n_toc) COUNT(TGS_CULL_DEGENERATE, n_degenerate)
-  COUNT(TGS_CULL_EMPTY, n_empty) COUNT(TGS_VISIBLE, n_visible)
-  {
-    const uint32_t m = __ballot_sync(0xffffffffu, (flags & (TGS_VISIBLE | TGS_NEWLY_VISIBLE)) == (TGS_VISIBLE | TGS_NEWLY_VISIBLE));
-    if (m && lane == 0) atomicAdd(&counters->n_newly_visible, __popc(m));
+  __syncthreads();
+  if (tid == 0) {
+    if (sm.stat[0]) atomicAdd(&counters->n_near, sm.stat[0]);
+    if (sm.stat[1]) atomicAdd(&counters->n_afc, sm.stat[1]);
+    if (sm.stat[2]) atomicAdd(&counters->n_toc, sm.stat[2]);
+    if (sm.stat[3]) atomicAdd(&counters->n_degenerate, sm.stat[3]);
+    if (sm.stat[4]) atomicAdd(&counters->n_empty, sm.stat[4]);
+    if (sm.stat[6]) atomicAdd(&counters->n_newly_visible, sm.stat[6]);
+    if (sm.area) atomicAdd(&counters->area_sum, sm.area);
   }
-#undef COUNT
 }
 
 // ------------------------------------------------------------------ A4 tile selection: T_sel = T^oc U T^um (L123)
-// One CTA.  Builds the tile mask, the bit set used by the pair counting, and the work order of the blend
+// One CTA of 1024 threads, each owning a run of consecutive tiles (a multiple of 32, so a thread writes whole words
+// of the bit set).  Builds the tile mask, the bit set used by the pair binning, and the work order of the blend
 // kernel: selected tiles first (ascending id), then the tiles that are only stitched.
 __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* __restrict__ tile_flags, uint8_t* __restrict__ tile_mask,
                                                  uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tile_order,
                                                  Counters* __restrict__ counters) {
-  __shared__ uint32_t s_warp[32];
-  __shared__ uint32_t s_base, s_noc, s_num;
+  __shared__ uint32_t s_sel[32], s_oc[32], s_um[32];
   const int T = fc.n_tiles;
   const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  if (threadIdx.x == 0) { s_base = 0; s_noc = 0; s_num = 0; }
-  __syncthreads();
-  // pass 1: masks, bits, selected list
-  for (int base = 0; base < T; base += 1024) {
-    const int t = base + threadIdx.x;
-    uint32_t f = 0; bool sel = false;
-    if (t < T) {
-      f = tile_flags[t] & 3u;
-      sel = fc.all_tiles || f != 0;
-      tile_mask[t] = (uint8_t)(f | (sel ? 4u : 0u));
+  const int words = (T + 31) / 32, wpt = (words + 1023) / 1024;      // bit-set words per thread
+  const int t0 = threadIdx.x * wpt * 32, t1 = min(T, t0 + wpt * 32);
+  uint32_t nsel = 0, noc = 0, num = 0;
+  for (int t = t0; t < t1; t += 32) {
+    uint32_t word = 0;
+    for (int i = 0; i < 32 && t + i < T; ++i) {
+      const uint32_t f = tile_flags[t + i] & 3u;
+      const bool sel = fc.all_tiles || f != 0;
+      tile_mask[t + i] = (uint8_t)(f | (sel ? 4u : 0u));
+      word |= (sel ? 1u : 0u) << i;
+      noc += f & 1u; num += (f >> 1) & 1u;
     }
-    const uint32_t bal = __ballot_sync(0xffffffffu, sel);
-    if (lane == 0 && base + (int)(wid * 32) < T) sel_bits[(base >> 5) + wid] = bal;
-    const uint32_t boc = __ballot_sync(0xffffffffu, (f & 1u) != 0), bum = __ballot_sync(0xffffffffu, (f & 2u) != 0);
-    if (lane == 0) { s_warp[wid] = __popc(bal); if (boc) atomicAdd(&s_noc, __popc(boc)); if (bum) atomicAdd(&s_num, __popc(bum)); }
-    __syncthreads();
-    uint32_t before = s_base;
-    for (uint32_t w = 0; w < wid; ++w) before += s_warp[w];
-    if (sel) tile_order[before + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)t;
-    __syncthreads();
-    if (threadIdx.x == 0) { uint32_t tot = 0; for (int w = 0; w < 32; ++w) tot += s_warp[w]; s_base += tot; }
-    __syncthreads();
+    sel_bits[t >> 5] = word;
+    nsel += __popc(word);
   }
-  const uint32_t nsel = s_base;
-  __syncthreads();
-  if (threadIdx.x == 0) { counters->n_sel = nsel; counters->n_sel_oc = s_noc; counters->n_sel_um = s_num; s_base = nsel; }
-  __syncthreads();
-  // pass 2: the non-selected tiles follow
-  for (int base = 0; base < T; base += 1024) {
-    const int t = base + threadIdx.x;
-    const bool ns = t < T && !(fc.all_tiles || (tile_flags[t] & 3u) != 0);
-    const uint32_t bal = __ballot_sync(0xffffffffu, ns);
-    if (lane == 0) s_warp[wid] = __popc(bal);
-    __syncthreads();
-    uint32_t before = s_base;
-    for (uint32_t w = 0; w < wid; ++w) before += s_warp[w];
-    if (ns) tile_order[before + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)t;
-    __syncthreads();
-    if (threadIdx.x == 0) { uint32_t tot = 0; for (int w = 0; w < 32; ++w) tot += s_warp[w]; s_base += tot; }
-    __syncthreads();
-  }
-}
-
-// number of set bits of `bits` with index in [lo, hi)
-__device__ __forceinline__ uint32_t popc_range(const uint32_t* __restrict__ bits, uint32_t lo, uint32_t hi) {
-  uint32_t cnt = 0;
-  uint32_t w = lo >> 5;
-  const uint32_t wend = (hi - 1) >> 5;
-  uint32_t m = 0xffffffffu << (lo & 31);
-  for (; w < wend; ++w) { cnt += __popc(bits[w] & m); m = 0xffffffffu; }
-  m &= 0xffffffffu >> (31 - ((hi - 1) & 31));
-  return cnt + __popc(bits[w] & m);
-}
-
-__device__ __forceinline__ void sh_basis(int deg, float x, float y, float z, float* Y) {   // R5
-  Y[0] = 0.28209479177387814f;
-  if (deg < 1) return;
-  Y[1] = -0.4886025119029199f * y; Y[2] = 0.4886025119029199f * z; Y[3] = -0.4886025119029199f * x;
-  if (deg < 2) return;
-  const float xx = x * x, yy = y * y, zz = z * z, xy = x * y, yz = y * z, xz = x * z;
-  Y[4] = 1.0925484305920792f * xy; Y[5] = -1.0925484305920792f * yz;
-  Y[6] = 0.31539156525252005f * (2.0f * zz - xx - yy);
-  Y[7] = -1.0925484305920792f * xz; Y[8] = 0.5462742152960396f * (xx - yy);
-  if (deg < 3) return;
-  Y[9] = -0.5900435899266435f * y * (3.0f * xx - yy);
-  Y[10] = 2.890611442640554f * xy * z;
-  Y[11] = -0.4570457994644658f * y * (4.0f * zz - xx - yy);
-  Y[12] = 0.3731763325901154f * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
-  Y[13] = -0.4570457994644658f * x * (4.0f * zz - xx - yy);
-  Y[14] = 1.445305721320277f * z * (xx - yy);
-  Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
-}
-
-// ------------------------------------------------------------------ A5a pair count + SH colour
-// tiles_touched[g] = number of pairs this Gaussian emits (0 if invisible): the SELECTED tiles of its rect (L123)
-// that it intersects (L61) -- with exact_tiles (R39) those where max alpha over the tile's pixel box >= 1/255,
-// else every tile of the 3-sigma rect.  Rects of more than 4 tiles are counted by the whole warp (lanes over
-// tiles): near Gaussians cover hundreds of tiles and would otherwise serialise one thread.
-// SH -> RGB (L61 "color c_i"; R5) only for Gaussians that emit at least one pair: on S frames the 12K bytes
-// of SH are read only for Gaussians that reach a selected tile.
-template <int DEG>
-__global__ void __launch_bounds__(256) k_count_color(FrameConst fc, const float4* __restrict__ cull4, const float* __restrict__ sh,
-                                                     const uint32_t* __restrict__ rec_flags, const uint2* __restrict__ rec_rect,
-                                                     const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
-                                                     const uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tiles_touched,
-                                                     float4* __restrict__ rec_rgb) {
-  const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
-  const uint32_t lane = threadIdx.x & 31;
-  const int TX = fc.cam.TX;
-  uint32_t cnt = 0;
-  const bool vis = g < fc.n && (rec_flags[g] & TGS_VISIBLE);
-  uint32_t x_lo = 0, y_lo = 0, w = 0, area = 0;
-  if (vis) {
-    const uint2 r = rec_rect[g];
-    x_lo = r.x & 0xffffu; y_lo = r.y & 0xffffu;
-    w = (r.x >> 16) - x_lo; area = w * ((r.y >> 16) - y_lo);
-  }
-  if (!fc.exact_tiles) {
-    if (vis) {
-      if (fc.all_tiles) cnt = area;
-      else
-        for (uint32_t ty = y_lo; ty < y_lo + area / w; ++ty) cnt += popc_range(sel_bits, ty * TX + x_lo, ty * TX + x_lo + w);
-    }
-  } else {
-    float4 uv = make_float4(0.f, 0.f, 0.f, 0.f), cn = make_float4(0.f, 0.f, 0.f, -1.f);
-    if (vis) { uv = rec_uvdo[g]; cn = rec_conic[g]; }
-    const bool big = area > 4u;
-    if (vis && !big)
-      for (uint32_t i = 0; i < area; ++i) {
-        const uint32_t ty = y_lo + i / w, tx = x_lo + i % w, t = ty * TX + tx;
-        if ((fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u)) && tile_alpha_reach(uv.x, uv.y, cn.x, cn.y, cn.z, cn.w, tx, ty, fc.cam.W, fc.cam.H)) ++cnt;
-      }
-    uint32_t m = __ballot_sync(0xffffffffu, vis && big);
-    while (m) {
-      const int src = __ffs(m) - 1;
-      m &= m - 1;
-      const float su = __shfl_sync(0xffffffffu, uv.x, src), sv = __shfl_sync(0xffffffffu, uv.y, src);
-      const float sA = __shfl_sync(0xffffffffu, cn.x, src), sB = __shfl_sync(0xffffffffu, cn.y, src);
-      const float sC = __shfl_sync(0xffffffffu, cn.z, src), st = __shfl_sync(0xffffffffu, cn.w, src);
-      const uint32_t sx = __shfl_sync(0xffffffffu, x_lo, src), sy = __shfl_sync(0xffffffffu, y_lo, src);
-      const uint32_t sw = __shfl_sync(0xffffffffu, w, src), sa = __shfl_sync(0xffffffffu, area, src);
-      uint32_t c = 0;
-      if (st >= 0.0f)
-        for (uint32_t i = lane; i < sa; i += 32) {
-          const uint32_t ry = i / sw, ty = sy + ry, tx = sx + (i - ry * sw), t = ty * TX + tx;
-          if ((fc.all_tiles || ((sel_bits[t >> 5] >> (t & 31)) & 1u)) && tile_alpha_reach(su, sv, sA, sB, sC, st, tx, ty, fc.cam.W, fc.cam.H)) ++c;
-        }
-      c = warp_sum(c);
-      if ((int)lane == src) cnt = c;
-    }
-  }
-  if (g >= fc.n) return;
-  tiles_touched[g] = cnt;
-  if (!cnt) return;
-  constexpr int K = (DEG + 1) * (DEG + 1);
-  const float4 c4 = cull4[g];
-  float dx = c4.x - fc.cam.campos[0], dy = c4.y - fc.cam.campos[1], dz = c4.z - fc.cam.campos[2];
-  const float inv = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
-  dx *= inv; dy *= inv; dz *= inv;
-  float Y[K];
-  sh_basis(DEG, dx, dy, dz, Y);
-  float cr = 0.5f, cg = 0.5f, cb = 0.5f;
-  const float* p = sh + (size_t)g * K * 3;
-  if constexpr (K % 4 == 0) {            // K*3 floats = 3K/4 float4, 16 B aligned
-    const float4* p4 = reinterpret_cast<const float4*>(p);
-    float buf[K * 3];
+  // block-wide exclusive scan of nsel; totals of noc, num
+  uint32_t incl = nsel;
 #pragma unroll
-    for (int i = 0; i < K * 3 / 4; ++i) {
-      const float4 t = __ldg(p4 + i);
-      buf[4 * i] = t.x; buf[4 * i + 1] = t.y; buf[4 * i + 2] = t.z; buf[4 * i + 3] = t.w;
-    }
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
+  noc = warp_sum(noc); num = warp_sum(num);
+  if (lane == 31) s_sel[wid] = incl;
+  if (lane == 0) { s_oc[wid] = noc; s_um[wid] = num; }
+  __syncthreads();
+  uint32_t before = incl - nsel, total = 0, toc = 0, tum = 0;
 #pragma unroll
-    for (int kk = 0; kk < K; ++kk) { cr += Y[kk] * buf[3 * kk]; cg += Y[kk] * buf[3 * kk + 1]; cb += Y[kk] * buf[3 * kk + 2]; }
-  } else {
-#pragma unroll
-    for (int kk = 0; kk < K; ++kk) { cr += Y[kk] * p[3 * kk]; cg += Y[kk] * p[3 * kk + 1]; cb += Y[kk] * p[3 * kk + 2]; }
+  for (int w = 0; w < 32; ++w) { const uint32_t v = s_sel[w]; if ((uint32_t)w < wid) before += v; total += v; toc += s_oc[w]; tum += s_um[w]; }
+  if (threadIdx.x == 0) { counters->n_sel = total; counters->n_sel_oc = toc; counters->n_sel_um = tum; }
+  // selected tiles of this thread's run at [before, ...), the others at total + (t0 - before) ...
+  uint32_t ps = before, pn = total + ((uint32_t)min(t0, T) - before);
+  for (int t = t0; t < t1; ++t) {
+    const bool sel = fc.all_tiles || (tile_flags[t] & 3u) != 0;
+    if (sel) tile_order[ps++] = (uint32_t)t; else tile_order[pn++] = (uint32_t)t;
   }
-  rec_rgb[g] = make_float4(fmaxf(cr, 0.0f), fmaxf(cg, 0.0f), fmaxf(cb, 0.0f), 0.0f);
 }
 
 // ------------------------------------------------------------------ F_min / F_max over G_rendered (L109) + |G_rendered|
-__global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint8_t* __restrict__ rendered_now, const float4* __restrict__ rec_uvdo,
-                                                 uint32_t* __restrict__ F_key, Counters* __restrict__ counters, int update_F) {
+// Only visible Gaussians can have been blended: the reduction runs over the visible list, not over all N.
+__global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint32_t* __restrict__ vis_vals, const uint8_t* __restrict__ rendered_now,
+                                                 const float4* __restrict__ rec_uvdo, uint32_t* __restrict__ F_key,
+                                                 Counters* __restrict__ counters, int update_F) {
   uint32_t kmin_x = 0xffffffffu, kmin_y = 0xffffffffu, kmax_x = 0, kmax_y = 0, cnt = 0;
-  for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < fc.n; g += gridDim.x * blockDim.x) {
+  const uint32_t nv = counters->n_visible;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += gridDim.x * blockDim.x) {
+    const uint32_t g = vis_vals[i];
     if (!rendered_now[g]) continue;
     ++cnt;
     if (update_F) {
@@ -464,31 +459,40 @@ __global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint8_t* _
       kmin_x = min(kmin_x, kx); kmax_x = max(kmax_x, kx); kmin_y = min(kmin_y, ky); kmax_y = max(kmax_y, ky);
     }
   }
+  __shared__ uint32_t s_red[5];
+  if (threadIdx.x == 0) { s_red[0] = 0; s_red[1] = 0xffffffffu; s_red[2] = 0xffffffffu; s_red[3] = 0; s_red[4] = 0; }
+  __syncthreads();
   cnt = warp_sum(cnt);
   kmin_x = __reduce_min_sync(0xffffffffu, kmin_x); kmin_y = __reduce_min_sync(0xffffffffu, kmin_y);
   kmax_x = __reduce_max_sync(0xffffffffu, kmax_x); kmax_y = __reduce_max_sync(0xffffffffu, kmax_y);
-  if ((threadIdx.x & 31) == 0) {
-    if (cnt) atomicAdd(&counters->n_rendered, cnt);
-    if (update_F && cnt) {
-      atomicMin(&F_key[0], kmin_x); atomicMin(&F_key[1], kmin_y); atomicMax(&F_key[2], kmax_x); atomicMax(&F_key[3], kmax_y);
-    }
+  if ((threadIdx.x & 31) == 0 && cnt) {
+    atomicAdd(&s_red[0], cnt); atomicMin(&s_red[1], kmin_x); atomicMin(&s_red[2], kmin_y); atomicMax(&s_red[3], kmax_x); atomicMax(&s_red[4], kmax_y);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0 && s_red[0]) {
+    atomicAdd(&counters->n_rendered, s_red[0]);
+    if (update_F) { atomicMin(&F_key[0], s_red[1]); atomicMin(&F_key[1], s_red[2]); atomicMax(&F_key[2], s_red[3]); atomicMax(&F_key[3], s_red[4]); }
   }
 }
 
 }  // namespace
 
 // ====================================================================== launchers
+uint32_t preprocess_chunk_items() { return PRE_CHUNK; }
+
 void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const float* scales, const float* quats,
                    const float* opacity, const float* sh, DevBuffers& b) {
   if (!n) return;
-  k_repack<<<(n + 255) / 256, 256, 0, s>>>(n, means, scales, quats, opacity, b.cull4, b.cov3d, b.tau);
+  k_repack<<<(n + 255) / 256, 256, 0, s>>>(n, means, scales, quats, opacity, b.cull4, b.g2);
   cudaMemcpyAsync(b.sh, sh, (size_t)n * K * 3 * sizeof(float), cudaMemcpyDeviceToDevice, s);
 }
 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
+  const uint32_t n_desc = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK + 1;
   k_frame_init<<<592, 256, 0, s>>>(fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
-                                   (uint32_t*)rendered_next, n_words, b.F_key, reset_F ? 1 : 0);
+                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, (uint2*)b.pre_desc, n_desc,
+                                   b.F_key, reset_F ? 1 : 0);
 }
 
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma) {
@@ -501,31 +505,22 @@ void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   k_fill_corr<<<grid, 256, 0, s>>>(fc, b.warp_depth, b.fill_depth, b.tile_flags);
 }
 
-void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
-  k_preprocess<<<(fc.n + 255) / 256, 256, 0, s>>>(fc, b.cull4, b.cov3d, b.tau, b.rendered, b.warp_depth, b.warp_sigma, b.F_key,
-                                                  b.rec_uvdo, b.rec_conic, b.rec_rect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue, b.counters);
+void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
+  const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
+  const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
+  k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
+                                                       b.rec_rect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
+                                                       (unsigned long long*)b.pre_desc, b.ckeys[0], b.cvals[0], b.counters);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-  k_mark_oc<<<num_sms * 4, 256, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_rect, b.tile_flags, b.counters);
+  k_mark_oc<<<num_sms * 8, 128, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_rect, b.tile_flags, b.counters);
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   k_select<<<1, 1024, 0, s>>>(fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters);
 }
 
-void launch_count_color(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
-  const dim3 grid((fc.n + 255) / 256);
-#define LAUNCH(D) k_count_color<D><<<grid, 256, 0, s>>>(fc, b.cull4, b.sh, b.rec_flags, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, b.tiles_touched, b.rec_rgb)
-  switch (fc.sh_degree) {
-    case 0: LAUNCH(0); break;
-    case 1: LAUNCH(1); break;
-    case 2: LAUNCH(2); break;
-    default: LAUNCH(3); break;
-  }
-#undef LAUNCH
-}
-
-void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint8_t* rendered_now, bool update_F) {
-  k_frustum<<<592, 256, 0, s>>>(fc, rendered_now, b.rec_uvdo, b.F_key, b.counters, update_F ? 1 : 0);
+void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F) {
+  k_frustum<<<296, 256, 0, s>>>(fc, vis_vals, rendered_now, b.rec_uvdo, b.F_key, b.counters, update_F ? 1 : 0);
 }

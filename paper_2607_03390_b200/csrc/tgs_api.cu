@@ -43,7 +43,7 @@ struct tgs_ctx {
   Sched sched;
   int force_all = 0;
   // capacities
-  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; uint32_t bin_chunks_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
   uint64_t* keys64 = nullptr;  // test-only scratch of tgs_debug_get("keys")
   uint64_t device_bytes = 0;
   DevBuffers b;
@@ -137,6 +137,12 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs) {
   const uint32_t tiles = (max_pairs + sort_tile_items() - 1) / sort_tile_items() + 1;
   if (int r = dev_alloc(c, &b.sort_desc, (size_t)4 * tiles * 256, c->allocs_pairs)) return r;
   c->sort_tiles_cap = tiles;
+  // flat (Gaussian, tile) test space of k_bin: up to 8 tests per pair of capacity (and below 2^32)
+  unsigned long long max_tests = (unsigned long long)max_pairs * 8ull;
+  if (max_tests > 0xfff00000ull) max_tests = 0xfff00000ull;
+  c->bin_chunks_cap = (uint32_t)(max_tests / bin_chunk_items()) + 2;
+  if (int r = dev_alloc(c, &b.chunk_first, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
+  if (int r = dev_alloc(c, &b.bin_desc, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
   c->max_pairs = max_pairs;
   return TGS_OK;
 }
@@ -241,10 +247,10 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   DevBuffers& b = c->b;
   c->n = 0;
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
-  A(b.cull4, n) A(b.cov3d, 6 * (size_t)n) A(b.tau, n) A(b.sh, (size_t)n * K * 3)
-  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, n) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
-  A(b.tiles_touched, (size_t)n + 4) A(b.offsets, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
-  A(b.scan_desc, (size_t)n / scan_tile_items() + 3)
+  A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
+  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
+  A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
+  A(b.pre_desc, (size_t)n / preprocess_chunk_items() + 3) A(b.scan_desc, (size_t)n / scan_tile_items() + 3)
   A(b.ckeys[0], n) A(b.ckeys[1], n) A(b.cvals[0], n) A(b.cvals[1], n) A(b.nv_queue, n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
   A(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
@@ -372,8 +378,8 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 1
   if (ftype == TGS_FRAME_S) launch_fill_corr(s, fc, b);                                                    // A2
   mark();                                                                      // 2
-  launch_preprocess(s, fc, b);                                                                             // A3 (+ small-rect T^oc)
-  if (ftype == TGS_FRAME_S) launch_mark_oc(s, fc, b, c->num_sms);                                          // A4: T^oc of large rects
+  launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
+  if (ftype == TGS_FRAME_S) launch_mark_oc(s, fc, b, c->num_sms);                                          // A4: T^oc of larger rects
   mark();                                                                      // 3
   launch_select(s, fc, b);                                                                                 // A4: T_sel
   if (ftype == TGS_FRAME_S) {
@@ -381,11 +387,10 @@ int tgs_render(tgs_ctx* c, int mode) {
     CK(cudaEventRecord(c->ev_sel, s));
     c->sel_pending = true;
   }
-  launch_count_color(s, fc, b);                                                                            // A5: counts, colour
-  launch_compact(s, fc, b, c->num_sms);
-  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_emit, 4, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, c->num_sms);            // A6 level 1: by depth
-  launch_scan_emit(s, fc, b, dsorted, c->num_sms);                                                         // A5: offsets + pairs
+  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 4, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
+                                  &b.counters->ticket_sort[0], &b.counters->error, c->num_sms);            // A6 level 1: visible Gaussians by depth
+  CK(cudaMemsetAsync(b.scan_desc, 0, ((size_t)c->n / scan_tile_items() + 3) * sizeof(uint64_t), s));
+  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // A5: tests -> pairs, counts, colours
   mark();                                                                      // 4
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_sort_passes(fc.n_tiles), b.sort_hist + 4 * 256,
                                  b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, c->num_sms);   // A6 level 2: by tile
@@ -394,7 +399,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 6
   launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);                         // A8 + A9
   mark();                                                                      // 7
-  if (builds_priors) launch_frustum(s, fc, b, rendered_next, ftype == TGS_FRAME_R);                        // F_min/F_max (L109)
+  if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);                        // F_min/F_max (L109)
   CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
   mark();                                                                      // 8
   CK(cudaEventRecord(c->ev_done, s));
@@ -491,7 +496,6 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
   else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }
   else if (name == "tiles_touched") { src = b.tiles_touched; have = N * 4; }
-  else if (name == "offsets") { src = b.offsets; have = N * 4; }
   else if (name == "ranges") { src = b.ranges; have = T * 8; }
   else if (name == "tile_order") { src = b.tile_order; have = T * 4; }
   else if (name == "warp_depth") { src = b.warp_depth; have = px * 4; }
@@ -501,8 +505,7 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   else if (name == "prior_depth") { src = b.depth[c->prior_idx]; have = px * 4; }
   else if (name == "prior_sigma") { src = b.sigma[c->prior_idx]; have = px * 4; }
   else if (name == "prior_image") { src = b.image[c->prior_idx]; have = px * 12; }
-  else if (name == "cov3d") { src = b.cov3d; have = N * 24; }
-  else if (name == "tau") { src = b.tau; have = N * 4; }
+  else if (name == "g2") { src = b.g2; have = N * 32; }
   else return TGS_E_INVALID_ARG;
   if (!src) return TGS_E_INVALID_ARG;
   if (dst && bytes && have) { if (int r = copy_out(c, dst, src, bytes < have ? bytes : have, mem)) return r; }

@@ -44,13 +44,14 @@ struct Counters {
   uint32_t n_rendered;
   uint32_t overflow;
   uint32_t error;           // look-back watchdog etc.
-  uint32_t n_emit;          // Gaussians that emit at least one pair
+  uint32_t n_tests;         // sum of the rect areas of the visible Gaussians: the flat (Gaussian, tile) test space
   uint32_t n_nv_queue;      // newly visible Gaussians queued for the cooperative T^oc marking
   uint32_t n_oc_marked;     // tiles whose T^oc bit is set
   // work tickets of the persistent kernels
-  uint32_t ticket_scan, ticket_blend, ticket_compact, ticket_mark;
+  uint32_t ticket_pre, ticket_scan, ticket_bin, ticket_blend;
   uint32_t ticket_sort[8];  // [0..3] depth sort, [4..7] tile sort
-  uint32_t pad[3];
+  uint32_t pad[1];
+  unsigned long long area_sum;         // same as n_tests, accumulated in 64 bits by k_preprocess (overflow check)
   unsigned long long n_interactions;   // L (only when interaction counting is on)
 };
 static_assert(sizeof(Counters) == 136, "Counters layout");
@@ -58,9 +59,8 @@ static_assert(sizeof(Counters) == 136, "Counters layout");
 // ------------------------------------------------------------------ device buffers of a context
 struct DevBuffers {
   // scene (repacked at load)
-  float4* cull4 = nullptr;       // [N] {x,y,z,opacity}
-  float* cov3d = nullptr;        // [N][6] xx,xy,xz,yy,yz,zz
-  float* tau = nullptr;          // [N] 2 ln(255 o)
+  float4* cull4 = nullptr;       // [N] {x,y,z, largest scale}: the only record read for every Gaussian every frame
+  float4* g2 = nullptr;          // [N][2] {Sxx,Sxy,Sxz,Syy},{Syz,Szz,opacity,tau = 2 ln(255 o)}: read by survivors of the culls
   float* sh = nullptr;           // [N][K][3]
   // per-Gaussian records of the current frame
   float4* rec_uvdo = nullptr;    // [N] {u,v,d,o}
@@ -72,20 +72,24 @@ struct DevBuffers {
   // -1/2 delta^T Sigma'^-1 delta completed to a sum of two squares: A' = -log2e/2 * c/det, k = -b/c, D' = -log2e/2 / c
   float4* rec_b0 = nullptr;      // [N] {u, v, A', k}
   float4* rec_b1 = nullptr;      // [N] {D', log2 o, d, -}
-  uint32_t* tiles_touched = nullptr;  // [N]
-  uint32_t* offsets = nullptr;        // [N] exclusive scan
+  uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
+  // visible Gaussians: ckeys = bits(depth), cvals = index; [0] in index order (k_preprocess), sorted by the depth sort
+  uint32_t* ckeys[2] = {nullptr, nullptr};   // [N]
+  uint32_t* cvals[2] = {nullptr, nullptr};   // [N]
+  uint32_t* area_prefix = nullptr;           // [N+1] tests before each sorted visible Gaussian
+  uint32_t* chunk_first = nullptr;           // [bin_chunks_cap] sorted position of the Gaussian holding a chunk's first test
+  uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with rects of more than 4 tiles
   // pairs
   uint32_t* keys[2] = {nullptr, nullptr};    // [max_pairs] tile id of a pair
   uint32_t* vals[2] = {nullptr, nullptr};    // [max_pairs] Gaussian index of a pair
-  uint32_t* ckeys[2] = {nullptr, nullptr};   // [N] bits(depth) of the emitting Gaussians
-  uint32_t* cvals[2] = {nullptr, nullptr};   // [N] their indices
-  uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with large rects
   uint32_t* sort_hist = nullptr;      // [2][4][256]: depth sort, tile sort
   uint32_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors
   uint32_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
-  uint64_t* scan_desc = nullptr;      // look-back descriptors of the offsets scan
+  uint64_t* pre_desc = nullptr;       // look-back descriptors: visible-list compaction of k_preprocess
+  uint64_t* scan_desc = nullptr;      //                        k_scan_area
+  uint64_t* bin_desc = nullptr;       //                        k_bin [bin_chunks_cap]
   // tiles
   uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
   uint8_t* tile_mask = nullptr;       // [T] bit0 oc, bit1 um, bit2 selected
@@ -109,13 +113,11 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next);
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma);
 void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
-void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
-void launch_count_color(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
-void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint8_t* rendered_now, bool update_F);
+void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
-void launch_compact(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
-void launch_scan_emit(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms);
+void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
 // Sorts *n_ptr items on digits [0, passes) of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int passes,
                 uint32_t* hist, uint32_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, int num_sms);
@@ -125,4 +127,6 @@ void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorte
                   const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions);
 uint32_t sort_tile_items();
 uint32_t scan_tile_items();
+uint32_t bin_chunk_items();
+uint32_t preprocess_chunk_items();
 int tile_sort_passes(int n_tiles);
