@@ -198,7 +198,9 @@ def run_ours(args):
                 "ms_stage": {n: float(v) for n, v in zip(stage_names, ms)},
                 "n_pairs": float(np.mean([s["n_pairs"] for s in lst])), "n_visible": float(np.mean([s["n_visible"] for s in lst])),
                 "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
-                "n_interactions": float(np.mean([s["n_interactions"] for s in lst]))}
+                "n_interactions": float(np.mean([s["n_interactions"] for s in lst])),
+                "n_blended": float(np.mean([s["n_blended"] for s in lst])),
+                "n_pixel_slots": float(np.mean([s["n_pixel_slots"] for s in lst]))}
 
     stages = {"R": summarise(per_type[0]), "P": summarise(per_type[1]), "S": summarise(per_type[2])}
     # dominant kernel = the stage with the largest share of the profiled frames' time

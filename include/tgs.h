@@ -83,6 +83,8 @@ typedef struct {
   uint32_t overflow;   /* 1: n_pairs exceeded the capacity, frame invalid */
   uint64_t n_interactions; /* L: (pixel, Gaussian) pairs evaluated by the blend; 0 unless counting is on
                               (tgs_debug_run_stage("count_interactions_on")) */
+  uint64_t n_blended;      /* of those, the ones with alpha >= 1/255 that were composited (counting on) */
+  uint64_t n_pixel_slots;  /* pixel slots issued by the blend loop, dead lanes included (counting on) */
   float ms_stage[8];   /* per-stage device time when timing is on (tgs_debug_run_stage("timing_on")):
                           0 warp, 1 fill+corr, 2 preprocess, 3 select+count+scan+keys, 4 sort, 5 ranges,
                           6 blend+stitch, 7 post (F reduction, stats) */

@@ -39,7 +39,7 @@ class TgsStats(C.Structure):
                 ("n_newly_visible", C.c_uint32),
                 ("n_pairs", C.c_uint64),
                 ("n_tiles", C.c_uint32), ("n_sel_oc", C.c_uint32), ("n_sel_um", C.c_uint32), ("n_sel", C.c_uint32),
-                ("n_rendered", C.c_uint32), ("overflow", C.c_uint32), ("n_interactions", C.c_uint64),
+                ("n_rendered", C.c_uint32), ("overflow", C.c_uint32), ("n_interactions", C.c_uint64), ("n_blended", C.c_uint64), ("n_pixel_slots", C.c_uint64),
                 ("ms_stage", C.c_float * 8), ("ms_total", C.c_float),
                 ("device_bytes", C.c_uint64)]
 

@@ -4,13 +4,18 @@
 // L101 + L125-128 (bilinear TAB, Eq.4).  Constants of R2: alpha <= 0.99, skip alpha < 1/255, stop when
 // T(1-alpha) < 1e-4.
 //
-// One persistent grid; a work item is a tile of `tile_order` (selected tiles first).  A CTA is 64 threads
-// = one 16x16 tile, each thread owning a run of 4 horizontally adjacent pixels, so that everything that depends
-// only on the Gaussian and the row (two shared-memory loads, dy, D' dy^2 + log2 o, t at the first pixel) is paid once
-// per 4 interactions: alpha_i = exp2(A' t_i^2 + D' dy^2 + log2 o), t_i = t_0 - i, is 3 FMA-pipe instructions per
-// pixel + 5 per run.  The form is -1/2 delta^T Sigma'^-1 delta completed to two squares, which has no cancellation
-// between terms (screen-filling anisotropic splats lose 1e-4 of alpha in the 3-term conic form).  The tile's
-// sorted Gaussians are staged through shared memory in batches of 128 records.
+// One persistent grid; a work item is a tile of `tile_order` (selected tiles first).  A CTA is 64 threads = one
+// 16x16 tile.  The tile's sorted Gaussians stream through shared memory in batches of 128 records, double
+// buffered with cp.async (the gather of batch b+1 overlaps the arithmetic of batch b).
+//
+// DENSE mode (all pixels of the tile): each thread owns a run of 4 horizontally adjacent pixels, so that what
+// depends only on the Gaussian and the row (two shared-memory loads, dy, D' dy^2 + log2 o, t at the first pixel) is
+// paid once per 4 interactions: alpha_i = exp2(A' t_i^2 + D' dy^2 + log2 o), t_i = t_0 - i.  The form is
+// -1/2 delta^T Sigma'^-1 delta completed to two squares, which has no cancellation between terms (R36).
+// SPARSE mode: a tile is finished only when its LAST pixel is saturated or the list ends, and in a cloud with gaps
+// a few pixels per tile never saturate while most are done after a small part of the list.  When at most 64 pixels
+// are still alive at a batch boundary, their states are compacted through shared memory to one pixel per thread
+// (again at <= 32: one warp), so the rest of the list costs work in proportion to the pixels that still need it.
 // This kernel is FP32-pipe / issue bound, not HBM bound.
 #include "tgs_internal.cuh"
 
@@ -18,7 +23,7 @@ namespace {
 
 constexpr int BLEND_THREADS = 64;      // 16 rows x 4 runs of 4 pixels
 constexpr int BLEND_BATCH = 128;
-constexpr int PPT = 4;                 // pixels per thread
+constexpr int PPT = 4;                 // pixels per thread (dense mode)
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
 // log2(1/255) = -7.99435...; anything below this bound (with a safety gap far above the rounding of e and of
 // ex2.approx) has alpha < 1/255 for sure, so the exact test on alpha is only evaluated near or above the threshold
@@ -29,19 +34,65 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-struct BlendSmem {
+struct Batch {
   float4 a[BLEND_BATCH];     // u, v, A', k
-  float4 b[BLEND_BATCH];     // D', log2(o), d, r
-  float2 c[BLEND_BATCH];     // g, b
+  float4 b[BLEND_BATCH];     // D', log2(o), d, -
+  float4 c[BLEND_BATCH];     // r, g, b, -
   uint32_t id[BLEND_BATCH];  // Gaussian index (for the G_rendered marks)
   uint8_t contrib[BLEND_BATCH];   // G_rendered marks of the batch (benign same-value races)
+};
+
+struct Pixel {               // per-pixel state of the front-to-back loop; sum of the weights = 1 - T (telescoping)
+  float T, Cr, Cg, Cb, S1, S2, d0;
+};
+
+struct BlendSmem {
+  Batch bt[2];
+  float st[BLEND_THREADS][7];      // pixel states in transit during a compaction
+  uint16_t st_px[BLEND_THREADS];   // their pixel index inside the tile (ly * 16 + lx)
+  uint32_t alive_cnt[2][2];        // [parity][warp] alive pixels
   uint32_t work;
 };
 
-struct Pixel {               // per-pixel state of the front-to-back loop
-  float T, Cr, Cg, Cb, Sw, S1, S2, d0;
-};
+// one (pixel, Gaussian) interaction (sparse mode); returns false when the pixel is finished
+__device__ __forceinline__ bool blend_one(Pixel& p, float e, float r, float g, float b, float d, bool& marked, uint32_t& nhit) {
+  const float alpha = fminf(0.99f, ex2_approx(e));
+  if (alpha < ALPHA_MIN) return true;
+  const float Tn = p.T * (1.0f - alpha);
+  if (Tn < 1.0e-4f) return false;
+  const float wgt = alpha * p.T;
+  p.Cr = fmaf(wgt, r, p.Cr); p.Cg = fmaf(wgt, g, p.Cg); p.Cb = fmaf(wgt, b, p.Cb);
+  if (p.T == 1.0f) p.d0 = d;              // first contribution: the depth moments are taken about it (R30)
+  const float dd = d - p.d0;
+  p.S1 = fmaf(wgt, dd, p.S1); p.S2 = fmaf(wgt * dd, dd, p.S2);
+  p.T = Tn;
+  marked = true;
+  ++nhit;
+  return true;
+}
+
+__device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p, size_t pix, float* __restrict__ image,
+                                            float* __restrict__ depth, float* __restrict__ sigma) {
+  image[pix * 3 + 0] = p.Cr + p.T * fc.bg[0];
+  image[pix * 3 + 1] = p.Cg + p.T * fc.bg[1];
+  image[pix * 3 + 2] = p.Cb + p.T * fc.bg[2];
+  if (p.T < 1.0f) {
+    const float Sw = 1.0f - p.T;
+    const float m1 = p.S1 / Sw;
+    depth[pix] = p.d0 + m1;
+    sigma[pix] = sqrtf(fmaxf(0.0f, p.S2 / Sw - m1 * m1));
+  } else {
+    depth[pix] = TGS_DEPTH_INVALID;
+    sigma[pix] = 0.0f;
+  }
+}
 
 template <bool MARK, bool COUNT>
 __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
@@ -53,17 +104,18 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
                                                          uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters) {
   __shared__ BlendSmem sm;
   const CamConst& k = fc.cam;
-  const uint32_t lane = threadIdx.x & 31;
-  const int lx = (threadIdx.x & 3) * PPT, ly = threadIdx.x >> 2;
+  const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int lx = (tid & 3) * PPT, ly = tid >> 2;
   const uint32_t n_sel = counters->n_sel;
   while (true) {
     __syncthreads();
-    if (threadIdx.x == 0) sm.work = atomicAdd(&counters->ticket_blend, 1u);
+    if (tid == 0) sm.work = atomicAdd(&counters->ticket_blend, 1u);
     __syncthreads();
     const uint32_t w = sm.work;
     if (w >= (uint32_t)fc.n_tiles) break;
     const uint32_t tile = tile_order[w];
-    const int px0 = (int)(tile % k.TX) * TGS_TILE + lx, py = (int)(tile / k.TX) * TGS_TILE + ly;
+    const int tile_x0 = (int)(tile % k.TX) * TGS_TILE, tile_y0 = (int)(tile / k.TX) * TGS_TILE;
+    const int px0 = tile_x0 + lx, py = tile_y0 + ly;
     const bool row_in = py < k.H;
     if (w >= n_sel) {
       // ------------------------------------------------ A9 stitch (Eq.4, second case)
@@ -100,94 +152,195 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     }
     // -------------------------------------------------- A8 blend
     const uint2 range = ranges[tile];
-    const float fpx = (float)px0, fpy = (float)py;
-    Pixel p[PPT];
-    bool alive[PPT];
+    const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
+    float fpx = (float)px0, fpy = (float)py;
+    // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
+    float2 T2[2], Cr2[2], Cg2[2], Cb2[2], S12[2], S22[2], D02[2];
+    Pixel sp;
+    bool alive[PPT], valid[PPT];
 #pragma unroll
-    for (int i = 0; i < PPT; ++i) {
-      p[i].T = 1.0f; p[i].Cr = p[i].Cg = p[i].Cb = 0.0f; p[i].Sw = p[i].S1 = p[i].S2 = p[i].d0 = 0.0f;
-      alive[i] = row_in && px0 + i < k.W;
+    for (int q = 0; q < 2; ++q) {
+      T2[q] = make_float2(1.0f, 1.0f);
+      Cr2[q] = Cg2[q] = Cb2[q] = S12[q] = S22[q] = D02[q] = make_float2(0.0f, 0.0f);
     }
-    uint32_t nint = 0;
-    for (uint32_t start = range.x; start < range.y; start += BLEND_BATCH) {
-      const bool any_alive = alive[0] || alive[1] || alive[2] || alive[3];
-      if (__syncthreads_count(any_alive) == 0) break;
-      const uint32_t nb = min((uint32_t)BLEND_BATCH, range.y - start);
-      for (uint32_t j = threadIdx.x; j < nb; j += BLEND_THREADS) {
-        const uint32_t g = vals[start + j];
-        const float4 r0 = rec_b0[g], r1 = rec_b1[g], r2 = rec_rgb[g];
-        sm.a[j] = r0;
-        sm.b[j] = make_float4(r1.x, r1.y, r1.z, r2.x);
-        sm.c[j] = make_float2(r2.y, r2.z);
-        sm.id[j] = g;
-        if (MARK) sm.contrib[j] = 0;
+#pragma unroll
+    for (int i = 0; i < PPT; ++i) { valid[i] = row_in && px0 + i < k.W; alive[i] = valid[i]; }
+    auto get_px = [&](int i) {
+      Pixel r;
+      const int q = i >> 1;
+      if (i & 1) { r.T = T2[q].y; r.Cr = Cr2[q].y; r.Cg = Cg2[q].y; r.Cb = Cb2[q].y; r.S1 = S12[q].y; r.S2 = S22[q].y; r.d0 = D02[q].y; }
+      else { r.T = T2[q].x; r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = D02[q].x; }
+      return r;
+    };
+    bool sparse = false, have = false;      // sparse mode: this thread owns pixel `spx` of the tile in p[0]
+    uint32_t spx = 0, slots = TGS_TILE * TGS_TILE;
+    uint32_t gid[2];
+    auto load_ids = [&](uint32_t b) {
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        const uint32_t idx = range.x + b * BLEND_BATCH + tid + s * BLEND_THREADS;
+        gid[s] = (b < nb && idx < range.y) ? vals[idx] : 0xffffffffu;
       }
-      __syncthreads();
-      if (any_alive) {
-#pragma unroll 2
-        for (uint32_t j = 0; j < nb; ++j) {
-          const float4 ga = sm.a[j];
-          const float4 gb = sm.b[j];
-          const float dy = ga.y - fpy;
-          const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
-          float t = fmaf(ga.w, dy, ga.x - fpx);                       // t at the first pixel of the run
-          if (COUNT) nint += (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3];
-          bool hit[PPT];
-          float e[PPT];
+    };
+    auto issue = [&](uint32_t b) {
+      Batch& B = sm.bt[b & 1];
 #pragma unroll
-          for (int i = 0; i < PPT; ++i) {
-            e[i] = fmaf(ga.z * t, t, e1);                             // log2(o) + log2 of the falloff
-            hit[i] = alive[i] && e[i] >= LOG2_ALPHA_MIN_LO;           // else surely alpha < 1/255: no MUFU
-            t -= 1.0f;
-          }
-          if (!(hit[0] || hit[1] || hit[2] || hit[3])) continue;
-          const float2 gc = sm.c[j];
-          bool marked = false;
-#pragma unroll
-          for (int i = 0; i < PPT; ++i) {
-            if (!hit[i]) continue;
-            const float alpha = fminf(0.99f, ex2_approx(e[i]));
-            if (alpha < ALPHA_MIN) continue;
-            const float Tn = p[i].T * (1.0f - alpha);
-            if (Tn < 1.0e-4f) { alive[i] = false; continue; }
-            const float wgt = alpha * p[i].T;
-            p[i].Cr = fmaf(wgt, gb.w, p[i].Cr); p[i].Cg = fmaf(wgt, gc.x, p[i].Cg); p[i].Cb = fmaf(wgt, gc.y, p[i].Cb);
-            if (p[i].Sw == 0.0f) p[i].d0 = gb.z;
-            const float dd = gb.z - p[i].d0;
-            p[i].Sw += wgt; p[i].S1 = fmaf(wgt, dd, p[i].S1); p[i].S2 = fmaf(wgt * dd, dd, p[i].S2);
-            p[i].T = Tn;
-            marked = true;
-          }
-          if (MARK && marked) sm.contrib[j] = 1;
-          if (!(alive[0] || alive[1] || alive[2] || alive[3])) break;
+      for (int s = 0; s < 2; ++s) {
+        const uint32_t j = tid + s * BLEND_THREADS;
+        if (gid[s] != 0xffffffffu) {
+          cp_async16(&B.a[j], rec_b0 + gid[s]); cp_async16(&B.b[j], rec_b1 + gid[s]); cp_async16(&B.c[j], rec_rgb + gid[s]);
+          B.id[j] = gid[s];
+          if (MARK) B.contrib[j] = 0;
         }
       }
-      if (MARK) {
-        __syncthreads();
-        for (uint32_t j = threadIdx.x; j < nb; j += BLEND_THREADS)
-          if (sm.contrib[j]) rendered_next[sm.id[j]] = 1;
-      }
-    }
+      cp_async_commit();
+    };
+    auto writeback_marks = [&](uint32_t b) {       // own slots of batch b
+      const Batch& B = sm.bt[b & 1];
+      const uint32_t cnt = min((uint32_t)BLEND_BATCH, len - b * BLEND_BATCH);
 #pragma unroll
-    for (int i = 0; i < PPT; ++i) {
-      const int px = px0 + i;
-      if (!row_in || px >= k.W) continue;
-      const size_t pix = (size_t)py * k.W + px;
-      image[pix * 3 + 0] = p[i].Cr + p[i].T * fc.bg[0];
-      image[pix * 3 + 1] = p[i].Cg + p[i].T * fc.bg[1];
-      image[pix * 3 + 2] = p[i].Cb + p[i].T * fc.bg[2];
-      if (p[i].Sw > 0.0f) {
-        const float m1 = p[i].S1 / p[i].Sw;
-        depth[pix] = p[i].d0 + m1;
-        sigma[pix] = sqrtf(fmaxf(0.0f, p[i].S2 / p[i].Sw - m1 * m1));
-      } else {
-        depth[pix] = TGS_DEPTH_INVALID;
-        sigma[pix] = 0.0f;
+      for (int s = 0; s < 2; ++s) {
+        const uint32_t j = tid + s * BLEND_THREADS;
+        if (j < cnt && B.contrib[j]) rendered_next[B.id[j]] = 1;
       }
+    };
+    load_ids(0); issue(0); load_ids(1);
+    uint32_t nint = 0, nhit = 0, nslot = 0;
+    int computed = -1;
+    for (uint32_t b = 0; b < nb; ++b) {
+      const uint32_t na_t = sparse ? (uint32_t)(have && alive[0]) : (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3];
+      const uint32_t na_w = __reduce_add_sync(0xffffffffu, na_t);
+      if (lane == 0) sm.alive_cnt[b & 1][wid] = na_w;
+      cp_async_wait_all();
+      __syncthreads();
+      const uint32_t alive0 = sm.alive_cnt[b & 1][0], total_alive = alive0 + sm.alive_cnt[b & 1][1];
+      if (MARK && b > 0) writeback_marks(b - 1);
+      computed = -1;
+      if (total_alive == 0) break;
+      if (b + 1 < nb) issue(b + 1);
+      load_ids(b + 2);
+      // ---- compaction of the alive pixels to one per thread
+      if ((total_alive <= BLEND_THREADS && slots > BLEND_THREADS) || (total_alive <= 32 && slots > 32)) {
+        uint32_t incl = na_t;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
+        uint32_t pos = (wid ? alive0 : 0u) + incl - na_t;
+        if (!sparse) {
+#pragma unroll
+          for (int i = 0; i < PPT; ++i) {
+            if (!valid[i]) continue;
+            const Pixel pi = get_px(i);
+            if (alive[i]) {
+              float* s = sm.st[pos];
+              s[0] = pi.T; s[1] = pi.Cr; s[2] = pi.Cg; s[3] = pi.Cb; s[4] = pi.S1; s[5] = pi.S2; s[6] = pi.d0;
+              sm.st_px[pos] = (uint16_t)(ly * TGS_TILE + lx + i);
+              ++pos;
+            } else write_pixel(fc, pi, (size_t)py * k.W + px0 + i, image, depth, sigma);
+          }
+        } else if (have) {
+          if (alive[0]) {
+            float* s = sm.st[pos];
+            s[0] = sp.T; s[1] = sp.Cr; s[2] = sp.Cg; s[3] = sp.Cb; s[4] = sp.S1; s[5] = sp.S2; s[6] = sp.d0;
+            sm.st_px[pos] = (uint16_t)spx;
+          } else write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
+        }
+        __syncthreads();
+        sparse = true;
+        have = tid < total_alive;
+        alive[0] = have; alive[1] = alive[2] = alive[3] = false;
+        if (have) {
+          const float* s = sm.st[tid];
+          sp.T = s[0]; sp.Cr = s[1]; sp.Cg = s[2]; sp.Cb = s[3]; sp.S1 = s[4]; sp.S2 = s[5]; sp.d0 = s[6];
+          spx = sm.st_px[tid];
+          fpx = (float)(tile_x0 + (int)(spx & 15u)); fpy = (float)(tile_y0 + (int)(spx >> 4));
+        }
+        slots = total_alive <= 32 ? 32u : (uint32_t)BLEND_THREADS;
+      }
+      // ---- the batch
+      const Batch& B = sm.bt[b & 1];
+      Batch& Bw = sm.bt[b & 1];
+      const uint32_t cnt = min((uint32_t)BLEND_BATCH, len - b * BLEND_BATCH);
+      if (!sparse) {
+        if (na_t) {
+          // branch-free: 85 % of the interactions of an alive pixel composite, so every pixel runs the whole update with
+          // alpha forced to 0 where it is skipped (alpha < 1/255), stops (T (1 - alpha) < 1e-4) or is finished
+          const float2 one2 = make_float2(1.0f, 1.0f), neg2 = make_float2(-1.0f, -1.0f);
+#pragma unroll 2
+          for (uint32_t j = 0; j < cnt; ++j) {
+            const float4 ga = B.a[j];
+            const float4 gb = B.b[j];
+            const float4 gc = B.c[j];
+            if (COUNT) { nslot += PPT; nint += (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3]; }
+            const float dy = ga.y - fpy;
+            const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
+            const float t0 = fmaf(ga.w, dy, ga.x - fpx);                // t at the first pixel of the run
+            const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z), d2 = make_float2(gb.z, gb.z);
+            const float2 tt[2] = {__fadd2_rn(make_float2(t0, t0), make_float2(0.0f, -1.0f)),
+                                  __fadd2_rn(make_float2(t0, t0), make_float2(-2.0f, -3.0f))};
+            bool any_bl = false;
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
+              float2 al = make_float2(fminf(0.99f, ex2_approx(e.x)), fminf(0.99f, ex2_approx(e.y)));
+              const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha)
+              const bool ok0 = alive[2 * q] && al.x >= ALPHA_MIN, ok1 = alive[2 * q + 1] && al.y >= ALPHA_MIN;
+              const bool bl0 = ok0 && Tn.x >= 1.0e-4f, bl1 = ok1 && Tn.y >= 1.0e-4f;
+              alive[2 * q] = alive[2 * q] && (bl0 || !ok0);
+              alive[2 * q + 1] = alive[2 * q + 1] && (bl1 || !ok1);
+              al.x = bl0 ? al.x : 0.0f; al.y = bl1 ? al.y : 0.0f;
+              if (COUNT) nhit += (uint32_t)bl0 + (uint32_t)bl1;
+              any_bl = any_bl || bl0 || bl1;
+              if (bl0 && T2[q].x == 1.0f) D02[q].x = gb.z;            // first contribution: moments are taken about it (R30)
+              if (bl1 && T2[q].y == 1.0f) D02[q].y = gb.z;
+              const float2 wgt = __fmul2_rn(al, T2[q]);
+              T2[q] = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));            // unchanged where alpha was forced to 0
+              Cr2[q] = __ffma2_rn(wgt, make_float2(gc.x, gc.x), Cr2[q]);
+              Cg2[q] = __ffma2_rn(wgt, make_float2(gc.y, gc.y), Cg2[q]);
+              Cb2[q] = __ffma2_rn(wgt, make_float2(gc.z, gc.z), Cb2[q]);
+              const float2 dd = __ffma2_rn(D02[q], neg2, d2);                    // d - d0
+              S12[q] = __ffma2_rn(wgt, dd, S12[q]);
+              S22[q] = __ffma2_rn(__fmul2_rn(wgt, dd), dd, S22[q]);
+            }
+            if (MARK && any_bl) Bw.contrib[j] = 1;
+            if (!(alive[0] || alive[1] || alive[2] || alive[3])) break;
+          }
+        }
+      } else if (__any_sync(0xffffffffu, alive[0])) {
+        for (uint32_t j = 0; j < cnt; ++j) {
+          if ((j & 15u) == 0u && !__any_sync(0xffffffffu, alive[0])) break;
+          const float4 ga = B.a[j];
+          const float4 gb = B.b[j];
+          if (COUNT) nslot += 1;
+          const float dx = ga.x - fpx, dy = ga.y - fpy;
+          const float t = fmaf(ga.w, dy, dx);
+          const float e1 = fmaf(gb.x * dy, dy, gb.y);
+          const float e = fmaf(ga.z * t, t, e1);
+          if (COUNT) nint += (uint32_t)alive[0];
+          if (alive[0] && e >= LOG2_ALPHA_MIN_LO) {
+            const float4 gc = B.c[j];
+            bool marked = false;
+            alive[0] = blend_one(sp, e, gc.x, gc.y, gc.z, gb.z, marked, nhit);
+            if (MARK && marked) Bw.contrib[j] = 1;
+          }
+        }
+      }
+      computed = (int)b;
+    }
+    if (MARK && computed >= 0) { __syncthreads(); writeback_marks((uint32_t)computed); }
+    // -------------------------------------------------- outputs
+    if (!sparse) {
+#pragma unroll
+      for (int i = 0; i < PPT; ++i)
+        if (valid[i]) write_pixel(fc, get_px(i), (size_t)py * k.W + px0 + i, image, depth, sigma);
+    } else if (have) {
+      write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
     }
     if (COUNT) {
       nint = __reduce_add_sync(0xffffffffu, nint);
       if (lane == 0 && nint) atomicAdd(&counters->n_interactions, (unsigned long long)nint);
+      nhit = __reduce_add_sync(0xffffffffu, nhit);
+      nslot = __reduce_max_sync(0xffffffffu, nslot) * 32u;     // lanes that left the loop early still occupy the warp
+      if (lane == 0) { atomicAdd(&counters->n_blended, (unsigned long long)nhit); atomicAdd(&counters->n_slots, (unsigned long long)nslot); }
     }
   }
 }
@@ -196,7 +349,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
 
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
                   uint8_t* rendered_next, int num_sms, bool count_interactions) {
-  const int grid = num_sms * 16;
+  const int grid = num_sms * 12;
 #define LAUNCH(M, C)                                                                                                          \
   k_blend<M, C><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \

@@ -446,7 +446,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_total = c->n; out->n_near = h.n_near; out->n_afc = h.n_afc; out->n_toc = h.n_toc; out->n_degenerate = h.n_degenerate;
   out->n_empty = h.n_empty; out->n_visible = h.n_visible; out->n_newly_visible = h.n_newly_visible;
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
-  out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions;
+  out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions; out->n_blended = h.n_blended; out->n_pixel_slots = h.n_slots;
   out->device_bytes = c->device_bytes;
   if (c->timing) {
     for (int i = 0; i < 8; ++i) cudaEventElapsedTime(&out->ms_stage[i], c->ev_stage[i], c->ev_stage[i + 1]);

@@ -53,8 +53,10 @@ struct Counters {
   uint32_t pad[1];
   unsigned long long area_sum;         // same as n_tests, accumulated in 64 bits by k_preprocess (overflow check)
   unsigned long long n_interactions;   // L (only when interaction counting is on)
+  unsigned long long n_blended;        // interactions that passed alpha >= 1/255 and were composited (counting on)
+  unsigned long long n_slots;          // pixel slots the blend loop issued: warp iterations x pixels per warp (counting on)
 };
-static_assert(sizeof(Counters) == 136, "Counters layout");
+static_assert(sizeof(Counters) == 152, "Counters layout");
 
 // ------------------------------------------------------------------ device buffers of a context
 struct DevBuffers {
