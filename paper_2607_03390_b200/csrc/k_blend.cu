@@ -157,14 +157,17 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
     float2 T2[2], Cr2[2], Cg2[2], Cb2[2], S12[2], S22[2], D02[2];
     Pixel sp;
-    bool alive[PPT], valid[PPT];
+    // dense mode keeps no alive flags: a finished pixel carries T < 0 (its |T| is the final transmittance), so that
+    // T (1 - alpha) >= 1e-4 fails for it by itself; pixels outside the image start finished
+    bool valid[PPT], salive = false;
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
-      T2[q] = make_float2(1.0f, 1.0f);
       Cr2[q] = Cg2[q] = Cb2[q] = S12[q] = S22[q] = D02[q] = make_float2(0.0f, 0.0f);
     }
 #pragma unroll
-    for (int i = 0; i < PPT; ++i) { valid[i] = row_in && px0 + i < k.W; alive[i] = valid[i]; }
+    for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
+    T2[0] = make_float2(valid[0] ? 1.0f : -1.0f, valid[1] ? 1.0f : -1.0f);
+    T2[1] = make_float2(valid[2] ? 1.0f : -1.0f, valid[3] ? 1.0f : -1.0f);
     auto get_px = [&](int i) {
       Pixel r;
       const int q = i >> 1;
@@ -208,7 +211,8 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     uint32_t nint = 0, nhit = 0, nslot = 0;
     int computed = -1;
     for (uint32_t b = 0; b < nb; ++b) {
-      const uint32_t na_t = sparse ? (uint32_t)(have && alive[0]) : (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3];
+      const uint32_t na_t = sparse ? (uint32_t)(have && salive)
+                                   : (uint32_t)(T2[0].x > 0.0f) + (uint32_t)(T2[0].y > 0.0f) + (uint32_t)(T2[1].x > 0.0f) + (uint32_t)(T2[1].y > 0.0f);
       const uint32_t na_w = __reduce_add_sync(0xffffffffu, na_t);
       if (lane == 0) sm.alive_cnt[b & 1][wid] = na_w;
       cp_async_wait_all();
@@ -229,8 +233,10 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
 #pragma unroll
           for (int i = 0; i < PPT; ++i) {
             if (!valid[i]) continue;
-            const Pixel pi = get_px(i);
-            if (alive[i]) {
+            Pixel pi = get_px(i);
+            const bool alive_i = pi.T > 0.0f;
+            pi.T = fabsf(pi.T);
+            if (alive_i) {
               float* s = sm.st[pos];
               s[0] = pi.T; s[1] = pi.Cr; s[2] = pi.Cg; s[3] = pi.Cb; s[4] = pi.S1; s[5] = pi.S2; s[6] = pi.d0;
               sm.st_px[pos] = (uint16_t)(ly * TGS_TILE + lx + i);
@@ -238,7 +244,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
             } else write_pixel(fc, pi, (size_t)py * k.W + px0 + i, image, depth, sigma);
           }
         } else if (have) {
-          if (alive[0]) {
+          if (salive) {
             float* s = sm.st[pos];
             s[0] = sp.T; s[1] = sp.Cr; s[2] = sp.Cg; s[3] = sp.Cb; s[4] = sp.S1; s[5] = sp.S2; s[6] = sp.d0;
             sm.st_px[pos] = (uint16_t)spx;
@@ -247,7 +253,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
         __syncthreads();
         sparse = true;
         have = tid < total_alive;
-        alive[0] = have; alive[1] = alive[2] = alive[3] = false;
+        salive = have;
         if (have) {
           const float* s = sm.st[tid];
           sp.T = s[0]; sp.Cr = s[1]; sp.Cg = s[2]; sp.Cb = s[3]; sp.S1 = s[4]; sp.S2 = s[5]; sp.d0 = s[6];
@@ -261,7 +267,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
       Batch& Bw = sm.bt[b & 1];
       const uint32_t cnt = min((uint32_t)BLEND_BATCH, len - b * BLEND_BATCH);
       if (!sparse) {
-        if (na_t) {
+        if (__any_sync(0xffffffffu, na_t != 0u)) {
           // branch-free: 85 % of the interactions of an alive pixel composite, so every pixel runs the whole update with
           // alpha forced to 0 where it is skipped (alpha < 1/255), stops (T (1 - alpha) < 1e-4) or is finished
           const float2 one2 = make_float2(1.0f, 1.0f), neg2 = make_float2(-1.0f, -1.0f);
@@ -270,30 +276,33 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
             const float4 ga = B.a[j];
             const float4 gb = B.b[j];
             const float4 gc = B.c[j];
-            if (COUNT) { nslot += PPT; nint += (uint32_t)alive[0] + (uint32_t)alive[1] + (uint32_t)alive[2] + (uint32_t)alive[3]; }
+            if (COUNT) {
+              nslot += PPT;
+              nint += (uint32_t)(T2[0].x > 0.0f) + (uint32_t)(T2[0].y > 0.0f) + (uint32_t)(T2[1].x > 0.0f) + (uint32_t)(T2[1].y > 0.0f);
+            }
             const float dy = ga.y - fpy;
             const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
             const float t0 = fmaf(ga.w, dy, ga.x - fpx);                // t at the first pixel of the run
             const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z), d2 = make_float2(gb.z, gb.z);
             const float2 tt[2] = {__fadd2_rn(make_float2(t0, t0), make_float2(0.0f, -1.0f)),
                                   __fadd2_rn(make_float2(t0, t0), make_float2(-2.0f, -3.0f))};
-            bool any_bl = false;
+            float2 wsum = make_float2(0.0f, 0.0f);
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
               const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
               float2 al = make_float2(fminf(0.99f, ex2_approx(e.x)), fminf(0.99f, ex2_approx(e.y)));
-              const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha)
-              const bool ok0 = alive[2 * q] && al.x >= ALPHA_MIN, ok1 = alive[2 * q + 1] && al.y >= ALPHA_MIN;
-              const bool bl0 = ok0 && Tn.x >= 1.0e-4f, bl1 = ok1 && Tn.y >= 1.0e-4f;
-              alive[2 * q] = alive[2 * q] && (bl0 || !ok0);
-              alive[2 * q + 1] = alive[2 * q + 1] && (bl1 || !ok1);
+              al.x = al.x >= ALPHA_MIN ? al.x : 0.0f;                             // skip (R2)
+              al.y = al.y >= ALPHA_MIN ? al.y : 0.0f;
+              const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha); < 0 for a finished pixel
+              const bool bl0 = Tn.x >= 1.0e-4f, bl1 = Tn.y >= 1.0e-4f;            // else: stop (R2) or already finished
               al.x = bl0 ? al.x : 0.0f; al.y = bl1 ? al.y : 0.0f;
-              if (COUNT) nhit += (uint32_t)bl0 + (uint32_t)bl1;
-              any_bl = any_bl || bl0 || bl1;
+              if (COUNT) nhit += (uint32_t)(al.x > 0.0f) + (uint32_t)(al.y > 0.0f);
               if (bl0 && T2[q].x == 1.0f) D02[q].x = gb.z;            // first contribution: moments are taken about it (R30)
               if (bl1 && T2[q].y == 1.0f) D02[q].y = gb.z;
-              const float2 wgt = __fmul2_rn(al, T2[q]);
-              T2[q] = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));            // unchanged where alpha was forced to 0
+              const float2 wgt = __fmul2_rn(al, T2[q]);               // 0 (or -0) where nothing is composited
+              T2[q].x = bl0 ? Tn.x : -fabsf(T2[q].x);                 // Tn = T where alpha was skipped
+              T2[q].y = bl1 ? Tn.y : -fabsf(T2[q].y);
+              wsum = __fadd2_rn(wsum, wgt);
               Cr2[q] = __ffma2_rn(wgt, make_float2(gc.x, gc.x), Cr2[q]);
               Cg2[q] = __ffma2_rn(wgt, make_float2(gc.y, gc.y), Cg2[q]);
               Cb2[q] = __ffma2_rn(wgt, make_float2(gc.z, gc.z), Cb2[q]);
@@ -301,13 +310,13 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
               S12[q] = __ffma2_rn(wgt, dd, S12[q]);
               S22[q] = __ffma2_rn(__fmul2_rn(wgt, dd), dd, S22[q]);
             }
-            if (MARK && any_bl) Bw.contrib[j] = 1;
-            if (!(alive[0] || alive[1] || alive[2] || alive[3])) break;
+            if (MARK && wsum.x + wsum.y > 0.0f) Bw.contrib[j] = 1;
+            if ((j & 7u) == 7u && __all_sync(0xffffffffu, fmaxf(fmaxf(T2[0].x, T2[0].y), fmaxf(T2[1].x, T2[1].y)) < 0.0f)) break;
           }
         }
-      } else if (__any_sync(0xffffffffu, alive[0])) {
+      } else if (__any_sync(0xffffffffu, salive)) {
         for (uint32_t j = 0; j < cnt; ++j) {
-          if ((j & 15u) == 0u && !__any_sync(0xffffffffu, alive[0])) break;
+          if ((j & 15u) == 0u && !__any_sync(0xffffffffu, salive)) break;
           const float4 ga = B.a[j];
           const float4 gb = B.b[j];
           if (COUNT) nslot += 1;
@@ -315,11 +324,11 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
           const float t = fmaf(ga.w, dy, dx);
           const float e1 = fmaf(gb.x * dy, dy, gb.y);
           const float e = fmaf(ga.z * t, t, e1);
-          if (COUNT) nint += (uint32_t)alive[0];
-          if (alive[0] && e >= LOG2_ALPHA_MIN_LO) {
+          if (COUNT) nint += (uint32_t)salive;
+          if (salive && e >= LOG2_ALPHA_MIN_LO) {
             const float4 gc = B.c[j];
             bool marked = false;
-            alive[0] = blend_one(sp, e, gc.x, gc.y, gc.z, gb.z, marked, nhit);
+            salive = blend_one(sp, e, gc.x, gc.y, gc.z, gb.z, marked, nhit);
             if (MARK && marked) Bw.contrib[j] = 1;
           }
         }
@@ -331,7 +340,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
     if (!sparse) {
 #pragma unroll
       for (int i = 0; i < PPT; ++i)
-        if (valid[i]) write_pixel(fc, get_px(i), (size_t)py * k.W + px0 + i, image, depth, sigma);
+        if (valid[i]) { Pixel pi = get_px(i); pi.T = fabsf(pi.T); write_pixel(fc, pi, (size_t)py * k.W + px0 + i, image, depth, sigma); }
     } else if (have) {
       write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
     }

@@ -15,8 +15,10 @@ namespace {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_IPT = 16;
-constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;   // 4096 pairs per tile
+constexpr int SORT_IPT = 8;
+constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;   // 2048 pairs per tile
+constexpr int SORT_CTAS_PER_SM = 5;
+constexpr int LOOKBACK_BATCH = 4;                    // predecessor descriptors fetched per look-back step
 constexpr int RADIX = 256;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, FLAG_MASK = 3u << 30, VALUE_MASK = ~FLAG_MASK;
 constexpr uint32_t LOOKBACK_WATCHDOG = 1u << 26;
@@ -76,7 +78,7 @@ struct SortSmem {
   uint32_t tile;
 };
 
-__global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+__global__ void __launch_bounds__(SORT_THREADS, SORT_CTAS_PER_SM) k_onesweep(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                                                            uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
                                                            const uint32_t* __restrict__ n_ptr, uint32_t* __restrict__ ticket,
                                                            uint32_t* __restrict__ error_flag, const uint32_t* __restrict__ hist_scan,
@@ -134,12 +136,20 @@ __global__ void __launch_bounds__(SORT_THREADS) k_onesweep(const uint32_t* __res
     if (tile > 0) {
       st_volatile(my, FLAG_AGG | cnt);
       uint32_t polls = 0;
-      for (int t = (int)tile - 1; t >= 0;) {
-        const uint32_t v = ld_volatile(desc + (size_t)t * RADIX + d);
-        if ((v & FLAG_MASK) == 0) { if (++polls > LOOKBACK_WATCHDOG) { *error_flag = 2; break; } continue; }
-        excl += v & VALUE_MASK;
-        if ((v & FLAG_MASK) == FLAG_PREFIX) break;
-        --t;
+      int t = (int)tile - 1;
+      bool done = false;
+      while (!done) {                       // LOOKBACK_BATCH independent loads in flight per step instead of one
+        uint32_t v[LOOKBACK_BATCH];
+#pragma unroll
+        for (int i = 0; i < LOOKBACK_BATCH; ++i) v[i] = (t - i >= 0) ? ld_volatile(desc + (size_t)(t - i) * RADIX + d) : FLAG_PREFIX;
+#pragma unroll
+        for (int i = 0; i < LOOKBACK_BATCH; ++i) {
+          if (done) break;
+          if ((v[i] & FLAG_MASK) == 0) { if (++polls > LOOKBACK_WATCHDOG) { *error_flag = 2; done = true; } break; }   // not ready: poll again from here
+          excl += v[i] & VALUE_MASK;
+          --t;
+          if ((v[i] & FLAG_MASK) == FLAG_PREFIX) done = true;
+        }
       }
     }
     st_volatile(my, FLAG_PREFIX | (excl + cnt));
@@ -200,7 +210,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
   k_sort_scan_hist<<<1, 256, 0, s>>>(hist, passes);
   int cur = 0;
   for (int p = 0; p < passes; ++p) {
-    k_onesweep<<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
+    k_onesweep<<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
                                                                    error_flag, hist + p * RADIX, desc + (size_t)p * tiles_cap * RADIX, p);
     cur ^= 1;
   }
