@@ -35,8 +35,7 @@ constexpr int BIN_CHUNK = BIN_THREADS * BIN_IPT;      // tests per work item
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const uint32_t* __restrict__ sorted_g,
                                                             const uint2* __restrict__ rec_rect, unsigned long long* __restrict__ desc,
                                                             uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
-                                                            unsigned long long* __restrict__ bin_desc, Counters* __restrict__ counters,
-                                                            unsigned long long max_tests) {
+                                                            Counters* __restrict__ counters, unsigned long long max_tests) {
   __shared__ uint32_t s_tile, s_warp[SCAN_THREADS / 32], s_excl;
   const uint32_t n = counters->n_visible;
   if (n == 0 || counters->area_sum > max_tests) {
@@ -59,17 +58,14 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
     }
     const uint32_t tsum = a[0] + a[1] + a[2] + a[3];
     uint32_t incl_total;
-    uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total);
+    uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total, fc.epoch);
     if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
 #pragma unroll
     for (int j = 0; j < SCAN_IPT; ++j) {
       if (i0 + j >= n) break;
       area_prefix[i0 + j] = off;
       const unsigned long long end = (unsigned long long)off + a[j];
-      for (unsigned long long kb = ((unsigned long long)off + BIN_CHUNK - 1) / BIN_CHUNK; kb * BIN_CHUNK < end; ++kb) {
-        chunk_first[kb] = i0 + j;
-        bin_desc[kb] = 0ull;
-      }
+      for (unsigned long long kb = ((unsigned long long)off + BIN_CHUNK - 1) / BIN_CHUNK; kb * BIN_CHUNK < end; ++kb) chunk_first[kb] = i0 + j;
       off += a[j];
     }
   }
@@ -131,6 +127,7 @@ struct BinSmem {
   uint8_t has[BIN_CHUNK + 8];       // Gaussian (chunk-local) emitted at least one pair here
   uint32_t warp[BIN_THREADS / 32];
   uint32_t excl, chunk;
+  uint32_t hist[2][256];            // digit histograms of the tile ids of the emitted pairs (for the tile sort)
 };
 
 struct BinGauss {                   // the Gaussian a thread is currently testing
@@ -145,12 +142,14 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
                                                      const uint32_t* __restrict__ sel_bits, const float4* __restrict__ cull4,
                                                      const float* __restrict__ sh, unsigned long long* __restrict__ desc,
                                                      uint32_t* __restrict__ tiles_touched, float4* __restrict__ rec_rgb,
-                                                     uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, Counters* __restrict__ counters) {
+                                                     uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
+                                                     Counters* __restrict__ counters) {
   __shared__ BinSmem sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
   const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
-  const uint32_t tid = threadIdx.x;
+  const uint32_t tid = threadIdx.x, lane = tid & 31;
   const int TX = fc.cam.TX;
+  for (int i = tid; i < 2 * 256; i += BIN_THREADS) (&sm.hist[0][0])[i] = 0;
   while (true) {
     __syncthreads();
     if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin, 1u);
@@ -204,7 +203,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
     }
     // ---------------------------------------------------------------- rank the passing tests (chunk-local + global)
     uint32_t incl_total;
-    const uint32_t goff = tgs_scan::chunk_scan<BIN_THREADS>(__popc(mask), chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total);
+    const uint32_t goff = tgs_scan::chunk_scan<BIN_THREADS>(__popc(mask), chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total, fc.epoch);
     const uint32_t cexcl = sm.excl, ctotal = incl_total - cexcl;
     const bool overflow = incl_total > fc.max_pairs;
     if (chunk == num_chunks - 1 && tid == 0) {
@@ -217,11 +216,26 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
       if ((mask >> k) & 1u) { sm.st_tile[lpos] = tl[k]; sm.st_g[lpos] = gg[k]; ++lpos; }
     __syncthreads();
     if (!overflow)
-      for (uint32_t p = tid; p < ctotal; p += BIN_THREADS) { keys[cexcl + p] = sm.st_tile[p]; vals[cexcl + p] = sm.st_g[p]; }
+      for (uint32_t p0 = 0; p0 < ctotal; p0 += BIN_THREADS) {
+        const uint32_t p = p0 + tid;
+        const bool in = p < ctotal;
+        const uint32_t tile = in ? sm.st_tile[p] : 0xffffffffu;
+        if (in) { keys[cexcl + p] = tile; vals[cexcl + p] = sm.st_g[p]; atomicAdd(&sm.hist[0][tile & 255u], 1u); }
+        // upper digit: consecutive pairs are consecutive tiles of one Gaussian, so it comes in runs: one atomic per run
+        const uint32_t hi = tile >> 8, prev = __shfl_up_sync(0xffffffffu, hi, 1);
+        const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || hi != prev);
+        if (in && ((heads >> lane) & 1u)) {
+          const uint32_t above = heads & ~((2u << lane) - 1u);               // heads of later runs
+          const uint32_t run = (above ? (uint32_t)__ffs(above) - 1u : 32u) - lane;
+          atomicAdd(&sm.hist[1][hi & 255u], run);
+        }
+      }
     // ---------------------------------------------------------------- colours of the Gaussians that emitted here
     for (uint32_t l = tid; l < m; l += BIN_THREADS)
       if (sm.has[l]) sh_colour<DEG>(fc, sorted_g[i_first + l], cull4, sh, rec_rgb);
   }
+  __syncthreads();
+  for (int i = tid; i < 2 * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
 }
 
 // ================================================================== A7: per-tile ranges
@@ -259,11 +273,11 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   const uint32_t* sorted_g = b.cvals[sorted_g_idx];
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
   k_scan_area<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, sorted_g, b.rec_rect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
-                                                      (unsigned long long*)b.bin_desc, b.counters, max_tests);
+                                                      b.counters, max_tests);
   grid = (uint32_t)(num_sms * 4);
 #define LAUNCH(D)                                                                                                                     \
   k_bin<D><<<grid, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_rect, b.rec_uvdo, b.rec_conic, b.sel_bits, \
-                                        b.cull4, b.sh, (unsigned long long*)b.bin_desc, b.tiles_touched, b.rec_rgb, b.keys[0], b.vals[0], b.counters)
+                                        b.cull4, b.sh, (unsigned long long*)b.bin_desc, b.tiles_touched, b.rec_rgb, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters)
   switch (fc.sh_degree) {
     case 0: LAUNCH(0); break;
     case 1: LAUNCH(1); break;

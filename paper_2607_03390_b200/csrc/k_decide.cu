@@ -53,19 +53,19 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 }
 
 // ------------------------------------------------------------------ per-frame init
-// counters <- 0; tile_flags <- 0; tiles_touched <- 0; look-back descriptors of the preprocess chunks <- 0;
+// counters <- 0; sort histograms <- 0; tile_flags <- 0; tiles_touched <- 0;
 // S frames: D^min <- INVALID bits, sigma^max <- 0; R / P frames: rendered_next <- 0;
 // R frames: F <- (+inf, +inf, -inf, -inf).
 __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint32_t* warp_depth,
                                                     uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
-                                                    uint4* tiles_touched4, uint32_t n_tt4, uint2* pre_desc, uint32_t n_desc,
+                                                    uint4* tiles_touched4, uint32_t n_tt4, uint32_t* sort_hist,
                                                     uint32_t* F_key, int reset_F) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
   if (tid < sizeof(Counters) / 4) ((uint32_t*)counters)[tid] = 0;
   if (reset_F && tid < 4) F_key[tid] = (tid < 2) ? 0xff800000u /* key(+inf) */ : 0x007fffffu /* key(-inf) */;
   for (uint32_t i = tid; i < (uint32_t)fc.n_tiles; i += nth) tile_flags[i] = 0;
   for (uint32_t i = tid; i < n_tt4; i += nth) tiles_touched4[i] = make_uint4(0u, 0u, 0u, 0u);
-  for (uint32_t i = tid; i < n_desc; i += nth) pre_desc[i] = make_uint2(0u, 0u);
+  if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
     const uint32_t px = (uint32_t)(fc.cam.W * fc.cam.H);
     for (uint32_t i = tid; i < px; i += nth) { warp_depth[i] = TGS_INVALID_BITS; warp_sigma[i] = 0; }
@@ -206,6 +206,7 @@ struct PreSmem {
   uint32_t excl, chunk, nsurv;
   uint32_t stat[8];
   unsigned long long area;
+  uint32_t hist[4][256];        // digit histograms of the depth keys of the visible Gaussians (for the depth sort)
 };
 
 __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
@@ -216,7 +217,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
                                                                unsigned long long* __restrict__ desc, uint32_t* __restrict__ vis_keys,
-                                                               uint32_t* __restrict__ vis_vals, Counters* __restrict__ counters) {
+                                                               uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ depth_hist,
+                                                               Counters* __restrict__ counters) {
   __shared__ PreSmem sm;
   const CamConst& k = fc.cam;
   const float* V = k.V;
@@ -230,6 +232,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
   unsigned long long st_area = 0;
   if (tid < 8) sm.stat[tid] = 0;
   if (tid == 0) sm.area = 0;
+  for (int i = tid; i < 4 * 256; i += PRE_THREADS) (&sm.hist[0][0])[i] = 0;
   while (true) {
     __syncthreads();
     if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_pre, 1u);
@@ -362,12 +365,17 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) { const uint32_t i = tid * PRE_IPT + j; if (i < total && (sm.list[i] & 0x4000u)) ++nv_t; }
     uint32_t incl_total;
-    uint32_t off = tgs_scan::chunk_scan<PRE_THREADS>(nv_t, chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total);
+    uint32_t off = tgs_scan::chunk_scan<PRE_THREADS>(nv_t, chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total, fc.epoch);
     if (chunk == num_chunks - 1 && tid == 0) counters->n_visible = incl_total;
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) {
       const uint32_t i = tid * PRE_IPT + j;
-      if (i < total && (sm.list[i] & 0x4000u)) { vis_keys[off] = sm.depth[i]; vis_vals[off] = base + (sm.list[i] & 0x3ffu); ++off; }
+      if (i < total && (sm.list[i] & 0x4000u)) {
+        const uint32_t key = sm.depth[i];
+        vis_keys[off] = key; vis_vals[off] = base + (sm.list[i] & 0x3ffu); ++off;
+        atomicAdd(&sm.hist[0][key & 255u], 1u); atomicAdd(&sm.hist[1][(key >> 8) & 255u], 1u);
+        atomicAdd(&sm.hist[2][(key >> 16) & 255u], 1u); atomicAdd(&sm.hist[3][key >> 24], 1u);
+      }
     }
   }
   // statistics: one atomic per CTA and class
@@ -385,6 +393,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
     if (st_area) atomicAdd(&sm.area, st_area);
   }
   __syncthreads();
+  for (int i = tid; i < 4 * 256; i += PRE_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&depth_hist[i], h); }
   if (tid == 0) {
     if (sm.stat[0]) atomicAdd(&counters->n_near, sm.stat[0]);
     if (sm.stat[1]) atomicAdd(&counters->n_afc, sm.stat[1]);
@@ -489,9 +498,8 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
-  const uint32_t n_desc = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK + 1;
   k_frame_init<<<592, 256, 0, s>>>(fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
-                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, (uint2*)b.pre_desc, n_desc,
+                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, b.sort_hist,
                                    b.F_key, reset_F ? 1 : 0);
 }
 
@@ -510,7 +518,7 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
   k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
-                                                       (unsigned long long*)b.pre_desc, b.ckeys[0], b.cvals[0], b.counters);
+                                                       (unsigned long long*)b.pre_desc, b.ckeys[0], b.cvals[0], b.sort_hist, b.counters);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

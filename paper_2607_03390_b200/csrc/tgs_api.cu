@@ -43,7 +43,8 @@ struct tgs_ctx {
   Sched sched;
   int force_all = 0;
   // capacities
-  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; uint32_t bin_chunks_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; uint32_t bin_chunks_cap = 0; int sort_passes_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
+  uint32_t epoch = 0;          // frame number, tag of the look-back descriptors
   uint64_t* keys64 = nullptr;  // test-only scratch of tgs_debug_get("keys")
   uint64_t device_bytes = 0;
   DevBuffers b;
@@ -63,10 +64,11 @@ struct tgs_ctx {
 namespace {
 
 template <typename T>
-int dev_alloc(tgs_ctx* c, T** p, size_t count, std::vector<void*>& list) {
+int dev_alloc(tgs_ctx* c, T** p, size_t count, std::vector<void*>& list, bool zero = false) {
   *p = nullptr;
   if (!count) count = 1;
   CK(cudaMalloc((void**)p, count * sizeof(T)));
+  if (zero) CK(cudaMemsetAsync(*p, 0, count * sizeof(T), c->stream));   // look-back descriptors: epoch 0 = never valid
   list.push_back(*p);
   c->device_bytes += count * sizeof(T);
   return TGS_OK;
@@ -123,8 +125,11 @@ int alloc_frame_buffers(tgs_ctx* c) {
   return TGS_OK;
 }
 
-int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs) {
-  if (max_pairs <= c->max_pairs) return TGS_OK;
+int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs, int passes) {
+  if (max_pairs <= c->max_pairs && passes <= c->sort_passes_cap) return TGS_OK;
+  if (max_pairs < c->max_pairs) max_pairs = c->max_pairs;
+  if (passes < c->sort_passes_cap) passes = c->sort_passes_cap;
+  c->max_pairs = 0;
   cudaStreamSynchronize(c->stream);
   for (void* p : c->allocs_pairs) cudaFree(p);
   c->allocs_pairs.clear();
@@ -135,16 +140,22 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs) {
     if (int r = dev_alloc(c, &b.vals[i], (size_t)max_pairs, c->allocs_pairs)) return r;
   }
   const uint32_t tiles = (max_pairs + sort_tile_items() - 1) / sort_tile_items() + 1;
-  if (int r = dev_alloc(c, &b.sort_desc, (size_t)4 * tiles * 256, c->allocs_pairs)) return r;
-  c->sort_tiles_cap = tiles;
+  if (int r = dev_alloc(c, &b.sort_desc, (size_t)passes * tiles * 256, c->allocs_pairs, true)) return r;
+  c->sort_tiles_cap = tiles; c->sort_passes_cap = passes;
   // flat (Gaussian, tile) test space of k_bin: up to 8 tests per pair of capacity (and below 2^32)
   unsigned long long max_tests = (unsigned long long)max_pairs * 8ull;
   if (max_tests > 0xfff00000ull) max_tests = 0xfff00000ull;
   c->bin_chunks_cap = (uint32_t)(max_tests / bin_chunk_items()) + 2;
   if (int r = dev_alloc(c, &b.chunk_first, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
-  if (int r = dev_alloc(c, &b.bin_desc, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
+  if (int r = dev_alloc(c, &b.bin_desc, (size_t)c->bin_chunks_cap, c->allocs_pairs, true)) return r;
   c->max_pairs = max_pairs;
   return TGS_OK;
+}
+
+int tile_key_bits(int n_tiles) {
+  int bits = 1;
+  while ((1ll << bits) < n_tiles) ++bits;
+  return bits;
 }
 
 uint32_t auto_max_pairs(const tgs_ctx* c) {
@@ -247,14 +258,16 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   DevBuffers& b = c->b;
   c->n = 0;
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
+#define AZ(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene, true)) return r;
   A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
   A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
-  A(b.pre_desc, (size_t)n / preprocess_chunk_items() + 3) A(b.scan_desc, (size_t)n / scan_tile_items() + 3)
+  AZ(b.pre_desc, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
   A(b.ckeys[0], n) A(b.ckeys[1], n) A(b.cvals[0], n) A(b.cvals[1], n) A(b.nv_queue, n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
-  A(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
+  AZ(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
 #undef A
+#undef AZ
   const float *d_means = means, *d_scales = scales, *d_quats = quats, *d_opacity = opacity, *d_sh = sh;
   std::vector<void*> tmp;
   if (mem == TGS_HOST) {
@@ -332,13 +345,14 @@ int tgs_render(tgs_ctx* c, int mode) {
   if (ftype != TGS_FRAME_R && !c->priors_valid) return TGS_E_NO_PRIORS;
 
   if (int r = alloc_frame_buffers(c)) return r;
-  if (int r = alloc_pair_buffers(c, c->prm.max_pairs ? c->prm.max_pairs : auto_max_pairs(c))) return r;
+  const int tile_bits = tile_key_bits(c->TX * c->TY), tile_passes = (tile_bits + 7) / 8;
+  if (int r = alloc_pair_buffers(c, c->prm.max_pairs ? c->prm.max_pairs : auto_max_pairs(c), tile_passes)) return r;
   // grow the pair buffers when the previous frame came close to (or over) the capacity
   if (!c->prm.max_pairs && c->have_frame) {
     if (cudaEventQuery(c->ev_done) == cudaSuccess && (c->h_counters->overflow || c->h_counters->n_pairs > c->max_pairs / 2)) {
       unsigned long long want = (unsigned long long)c->max_pairs * 2ull;
       if (want > (1ull << 30) - 1) want = (1ull << 30) - 1;
-      if (int r = alloc_pair_buffers(c, (uint32_t)want)) return r;
+      if (int r = alloc_pair_buffers(c, (uint32_t)want, tile_passes)) return r;
     }
   }
 
@@ -363,6 +377,14 @@ int tgs_render(tgs_ctx* c, int mode) {
   fc.all_tiles = !(ftype == TGS_FRAME_S && c->prm.enable_sr && !c->force_all);
   fc.exact_tiles = c->prm.exact_tiles ? 1 : 0;
   fc.n_tiles = c->TX * c->TY;
+  if (++c->epoch >= (1u << 30)) {   // tag wrap-around: forget every descriptor (once per 2^30 frames)
+    for (void* p : {(void*)c->b.pre_desc, (void*)c->b.scan_desc}) CK(cudaMemsetAsync(p, 0, ((size_t)c->n / 1024 + 3) * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.dsort_desc, 0, (size_t)4 * c->dsort_tiles_cap * 256 * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.sort_desc, 0, (size_t)c->sort_passes_cap * c->sort_tiles_cap * 256 * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.bin_desc, 0, (size_t)c->bin_chunks_cap * 8, c->stream));
+    c->epoch = 1;
+  }
+  fc.epoch = c->epoch;
 
   DevBuffers& b = c->b;
   cudaStream_t s = c->stream;
@@ -387,13 +409,12 @@ int tgs_render(tgs_ctx* c, int mode) {
     CK(cudaEventRecord(c->ev_sel, s));
     c->sel_pending = true;
   }
-  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 4, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, c->num_sms);            // A6 level 1: visible Gaussians by depth
-  CK(cudaMemsetAsync(b.scan_desc, 0, ((size_t)c->n / scan_tile_items() + 3) * sizeof(uint64_t), s));
+  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
+                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms);            // A6 level 1: visible Gaussians by depth
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // A5: tests -> pairs, counts, colours
   mark();                                                                      // 4
-  const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_sort_passes(fc.n_tiles), b.sort_hist + 4 * 256,
-                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, c->num_sms);   // A6 level 2: by tile
+  const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
+                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms);   // A6 level 2: by tile
   mark();                                                                      // 5
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
   mark();                                                                      // 6

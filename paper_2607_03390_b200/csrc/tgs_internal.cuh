@@ -34,6 +34,7 @@ struct FrameConst {
   int do_afc, do_toc, do_tgb, all_tiles;
   int exact_tiles;          // R39
   int n_tiles;
+  uint32_t epoch;           // frame number (1 .. 2^30 - 1): tag of the look-back descriptors
 };
 
 // ------------------------------------------------------------------ device counters (one block, zeroed per frame)
@@ -87,8 +88,8 @@ struct DevBuffers {
   uint32_t* keys[2] = {nullptr, nullptr};    // [max_pairs] tile id of a pair
   uint32_t* vals[2] = {nullptr, nullptr};    // [max_pairs] Gaussian index of a pair
   uint32_t* sort_hist = nullptr;      // [2][4][256]: depth sort, tile sort
-  uint32_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors
-  uint32_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
+  uint64_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors (epoch-tagged)
+  uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
   uint64_t* pre_desc = nullptr;       // look-back descriptors: visible-list compaction of k_preprocess
   uint64_t* scan_desc = nullptr;      //                        k_scan_area
   uint64_t* bin_desc = nullptr;       //                        k_bin [bin_chunks_cap]
@@ -120,9 +121,10 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
-// Sorts *n_ptr items on digits [0, passes) of the uint32 key; returns the index (0/1) of the result buffers.
-int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int passes,
-                uint32_t* hist, uint32_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, int num_sms);
+// Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
+int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
+                const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
+                int num_sms);
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
