@@ -213,7 +213,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
                                                                const uint8_t* __restrict__ rendered, const float* __restrict__ warp_depth,
                                                                const float* __restrict__ warp_sigma, const uint32_t* __restrict__ F_key,
                                                                float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
-                                                               uint2* __restrict__ rec_rect, uint32_t* __restrict__ rec_flags,
+                                                               uint2* __restrict__ rec_rect, uint2* __restrict__ rec_trect,
+                                                               uint32_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
                                                                unsigned long long* __restrict__ desc, uint32_t* __restrict__ vis_keys,
@@ -342,7 +343,24 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
       if (!(x_hi > x_lo && y_hi > y_lo)) { rec_flags[g] = TGS_CULL_EMPTY; ++st_empty; continue; }
       rec_flags[g] = fl | TGS_VISIBLE;
       if (fl) ++st_nv;
-      const uint32_t area = (x_hi - x_lo) * (y_hi - y_lo);
+      // Test rect (never a different decision): the tiles of the 3-sigma rect that can reach alpha >= 1/255 lie inside the
+      // bounding box of the ellipse q <= tau, |dx| <= sqrt(tau a), |dy| <= sqrt(tau c) (min over dy of q = dx^2 / a).  A tile
+      // wholly outside that box, enlarged by 1 %, has q_min >= 1.02 tau in exact arithmetic, and the fp32 evaluation of the
+      // oracle differs from it by at most ~1e-6 (18 kappa + 1700) -- below 0.02 tau when cond(Sigma') <= 400 and tau >= 0.5
+      // (DESIGN.md §7).  Otherwise, and when the box would be empty, the whole rect is kept (or one tile of it).
+      uint32_t tx_lo = x_lo, tx_hi = x_hi, ty_lo = y_lo, ty_hi = y_hi;
+      if (!(tau >= 0.0f)) { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }              // o < 1/255: reaches nothing; one (failing) test
+      else if (tau >= 0.5f && lam * lam <= 400.0f * det) {
+        const float ex = sqrtf(tau * a) * 1.01f + 0.01f, ey = sqrtf(tau * cc) * 1.01f + 0.01f;
+        const float fx_lo = ceilf((u - ex - 15.0f) / 16.0f), fx_hi = floorf((u + ex) / 16.0f) + 1.0f;
+        const float fy_lo = ceilf((v - ey - 15.0f) / 16.0f), fy_hi = floorf((v + ey) / 16.0f) + 1.0f;
+        const uint32_t nx_lo = (uint32_t)fminf(fmaxf(fx_lo, (float)x_lo), (float)x_hi), nx_hi = (uint32_t)fminf(fmaxf(fx_hi, (float)x_lo), (float)x_hi);
+        const uint32_t ny_lo = (uint32_t)fminf(fmaxf(fy_lo, (float)y_lo), (float)y_hi), ny_hi = (uint32_t)fminf(fmaxf(fy_hi, (float)y_lo), (float)y_hi);
+        if (nx_hi > nx_lo && ny_hi > ny_lo) { tx_lo = nx_lo; tx_hi = nx_hi; ty_lo = ny_lo; ty_hi = ny_hi; }
+        else { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }
+      }
+      rec_trect[g] = make_uint2(tx_lo | (tx_hi << 16), ty_lo | (ty_hi << 16));
+      const uint32_t area = (tx_hi - tx_lo) * (ty_hi - ty_lo);
       st_area += area;
       rec_uvdo[g] = make_float4(u, v, tz, opac);
       rec_conic[g] = make_float4(A, B, C, tau);
@@ -355,8 +373,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)
         if (area > 4u) nv_queue[atomicAdd(&counters->n_nv_queue, 1u)] = g;         // larger rects: k_mark_oc
         else
-          for (uint32_t tyy = y_lo; tyy < y_hi; ++tyy)
-            for (uint32_t txx = x_lo; txx < x_hi; ++txx) mark_oc_tile(k, u, v, A, B, C, tau, txx, tyy, tile_flags, counters);
+          for (uint32_t tyy = ty_lo; tyy < ty_hi; ++tyy)
+            for (uint32_t txx = tx_lo; txx < tx_hi; ++txx) mark_oc_tile(k, u, v, A, B, C, tau, txx, tyy, tile_flags, counters);
       }
     }
     __syncthreads();
@@ -517,12 +535,12 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
   k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
-                                                       b.rec_rect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
+                                                       b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        (unsigned long long*)b.pre_desc, b.ckeys[0], b.cvals[0], b.sort_hist, b.counters);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-  k_mark_oc<<<num_sms * 8, 128, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_rect, b.tile_flags, b.counters);
+  k_mark_oc<<<num_sms * 8, 128, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_trect, b.tile_flags, b.counters);
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {

@@ -142,12 +142,13 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs, int passes) {
   const uint32_t tiles = (max_pairs + sort_tile_items() - 1) / sort_tile_items() + 1;
   if (int r = dev_alloc(c, &b.sort_desc, (size_t)passes * tiles * 256, c->allocs_pairs, true)) return r;
   c->sort_tiles_cap = tiles; c->sort_passes_cap = passes;
-  // flat (Gaussian, tile) test space of k_bin: up to 8 tests per pair of capacity (and below 2^32)
-  unsigned long long max_tests = (unsigned long long)max_pairs * 8ull;
+  // flat (Gaussian, tile) test space of k_bin: up to 4 tests per pair of capacity (and below 2^32)
+  unsigned long long max_tests = (unsigned long long)max_pairs * 4ull;
   if (max_tests > 0xfff00000ull) max_tests = 0xfff00000ull;
   c->bin_chunks_cap = (uint32_t)(max_tests / bin_chunk_items()) + 2;
   if (int r = dev_alloc(c, &b.chunk_first, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
   if (int r = dev_alloc(c, &b.bin_desc, (size_t)c->bin_chunks_cap, c->allocs_pairs, true)) return r;
+  if (int r = dev_alloc(c, &b.chunk_mask, (size_t)c->bin_chunks_cap * (bin_chunk_items() / 8), c->allocs_pairs)) return r;
   c->max_pairs = max_pairs;
   return TGS_OK;
 }
@@ -260,7 +261,7 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
 #define AZ(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene, true)) return r;
   A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
-  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
+  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_trect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
   AZ(b.pre_desc, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
   A(b.ckeys[0], n) A(b.ckeys[1], n) A(b.cvals[0], n) A(b.cvals[1], n) A(b.nv_queue, n)
@@ -412,6 +413,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms);            // A6 level 1: visible Gaussians by depth
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // A5: tests -> pairs, counts, colours
+  launch_colour(s, fc, b, dsorted, c->num_sms);                                                            // A5: SH -> RGB of the emitting Gaussians
   mark();                                                                      // 4
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
                                  b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms);   // A6 level 2: by tile

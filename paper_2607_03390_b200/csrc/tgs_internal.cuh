@@ -68,7 +68,8 @@ struct DevBuffers {
   // per-Gaussian records of the current frame
   float4* rec_uvdo = nullptr;    // [N] {u,v,d,o}
   float4* rec_conic = nullptr;   // [N] {A,B,C,tau}
-  uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16
+  uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16: tiles of the 3-sigma extent (R3)
+  uint2* rec_trect = nullptr;    // [N] same layout: the sub-rect whose tiles are tested / can hold pairs (k_preprocess)
   uint32_t* rec_flags = nullptr; // [N]
   float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
   // blend-side parameters (values, not decisions): alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, which is
@@ -92,7 +93,8 @@ struct DevBuffers {
   uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
   uint64_t* pre_desc = nullptr;       // look-back descriptors: visible-list compaction of k_preprocess
   uint64_t* scan_desc = nullptr;      //                        k_scan_area
-  uint64_t* bin_desc = nullptr;       //                        k_bin [bin_chunks_cap]
+  uint64_t* bin_desc = nullptr;       // k_bin: [bin_chunks_cap] {pairs of the chunk, pairs before it}
+  uint8_t* chunk_mask = nullptr;      // k_bin: [bin_chunks_cap][128] outcome of 8 tests per byte
   // tiles
   uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
   uint8_t* tile_mask = nullptr;       // [T] bit0 oc, bit1 um, bit2 selected
@@ -121,6 +123,7 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
+void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms);
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
