@@ -8,7 +8,6 @@
 // A5a count + SH colour, F reduction (L109).
 #include "tgs_internal.cuh"
 #include "decide_math.cuh"
-#include "scan.cuh"
 
 namespace {
 
@@ -185,8 +184,9 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
 //  phase A (all Gaussians, 16 B each): near cull, projection of the mean, AFC, TOC + newly-visible lookups in the
 //          warped TGB, and a conservative off-screen test; the survivors are compacted in shared memory;
 //  phase B (survivors only, +32 B each): EWA covariance, conic, radius, rect, records, T^oc marks of small rects;
-//  phase C: the visible Gaussians of the chunk are appended, in ascending index order, to the list the depth sort
-//          works on (single-pass scan with decoupled look-back over the chunks).
+//  phase C: the visible Gaussians of the chunk are appended to the list the depth sort works on (one atomic per chunk:
+//          chunks land in arrival order, ascending index inside a chunk; k_fix_ties restores the index order of
+//          equal depths after the sort, so the final order does not depend on it).
 // SH (the bulk of the scene bytes) is not touched here at all.  Order of the tests and of every fp32 operation of a
 // decision: DESIGN.md §2 (O3), identical to what the oracle states.
 //
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
                                                                uint32_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
-                                                               unsigned long long* __restrict__ desc, uint32_t* __restrict__ vis_keys,
+                                                               uint32_t* __restrict__ vis_keys,
                                                                uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ depth_hist,
                                                                Counters* __restrict__ counters) {
   __shared__ PreSmem sm;
@@ -382,9 +382,17 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
     uint32_t nv_t = 0;
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) { const uint32_t i = tid * PRE_IPT + j; if (i < total && (sm.list[i] & 0x4000u)) ++nv_t; }
-    uint32_t incl_total;
-    uint32_t off = tgs_scan::chunk_scan<PRE_THREADS>(nv_t, chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total, fc.epoch);
-    if (chunk == num_chunks - 1 && tid == 0) counters->n_visible = incl_total;
+    uint32_t vincl = nv_t;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, vincl, d); if (lane >= (uint32_t)d) vincl += o; }
+    if (lane == 31) sm.warp[wid] = vincl;
+    __syncthreads();
+    uint32_t off = vincl - nv_t, vtotal = 0;
+#pragma unroll
+    for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < wid) off += t; vtotal += t; }
+    if (tid == 0) sm.excl = vtotal ? atomicAdd(&counters->n_visible, vtotal) : 0u;
+    __syncthreads();
+    off += sm.excl;
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) {
       const uint32_t i = tid * PRE_IPT + j;
@@ -536,7 +544,7 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
   k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
-                                                       (unsigned long long*)b.pre_desc, b.ckeys[0], b.cvals[0], b.sort_hist, b.counters);
+                                                       b.ckeys[0], b.cvals[0], b.sort_hist, b.counters);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

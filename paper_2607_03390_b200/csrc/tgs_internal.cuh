@@ -91,8 +91,7 @@ struct DevBuffers {
   uint32_t* sort_hist = nullptr;      // [2][4][256]: depth sort, tile sort
   uint64_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors (epoch-tagged)
   uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
-  uint64_t* pre_desc = nullptr;       // look-back descriptors: visible-list compaction of k_preprocess
-  uint64_t* scan_desc = nullptr;      //                        k_scan_area
+  uint64_t* scan_desc = nullptr;      // look-back descriptors of k_scan_area
   uint64_t* bin_desc = nullptr;       // k_bin: [bin_chunks_cap] {pairs of the chunk, pairs before it}
   uint8_t* chunk_mask = nullptr;      // k_bin: [bin_chunks_cap][128] outcome of 8 tests per byte
   // tiles
@@ -128,6 +127,7 @@ void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sort
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms);
+void launch_fix_ties(cudaStream_t s, const uint32_t* keys, uint32_t* vals, const uint32_t* n_ptr, int num_sms);
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
