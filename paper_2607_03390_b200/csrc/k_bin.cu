@@ -418,7 +418,6 @@ void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sort
 }
 
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms) {
-  cudaMemsetAsync(b.ranges, 0, (size_t)fc.n_tiles * sizeof(uint2), s);
   k_ranges<<<num_sms * 8, 256, 0, s>>>(b.keys[sorted_idx], b.counters, b.ranges, fc.n_tiles);
 }
 

@@ -6,6 +6,8 @@
 // A1 forward warp (Eq.3), A2 depth fill + correspondence + T^um (L121),
 // A3 preprocess + AFC + TOC + newly-visible + T^oc (L61, L109-113, L119), A4 tile selection (L117-123),
 // A5a count + SH colour, F reduction (L109).
+#include <cstddef>
+
 #include "tgs_internal.cuh"
 #include "decide_math.cuh"
 
@@ -57,12 +59,17 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 // R frames: F <- (+inf, +inf, -inf, -inf).
 __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint32_t* warp_depth,
                                                     uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
-                                                    uint4* tiles_touched4, uint32_t n_tt4, uint32_t* sort_hist,
+                                                    uint4* tiles_touched4, uint32_t n_tt4, uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
                                                     uint32_t* F_key, int reset_F) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-  if (tid < sizeof(Counters) / 4) ((uint32_t*)counters)[tid] = 0;
+  // R / P frames select every tile and carry no T^oc / T^um flags: the outputs of k_select are written here
+  const bool trivial_sel = fc.ftype != TGS_FRAME_S;
+  if (tid < sizeof(Counters) / 4) ((uint32_t*)counters)[tid] = (trivial_sel && tid == offsetof(Counters, n_sel) / 4) ? (uint32_t)fc.n_tiles : 0u;
   if (reset_F && tid < 4) F_key[tid] = (tid < 2) ? 0xff800000u /* key(+inf) */ : 0x007fffffu /* key(-inf) */;
-  for (uint32_t i = tid; i < (uint32_t)fc.n_tiles; i += nth) tile_flags[i] = 0;
+  for (uint32_t i = tid; i < (uint32_t)fc.n_tiles; i += nth) {
+    tile_flags[i] = 0; ranges[i] = make_uint2(0u, 0u);
+    if (trivial_sel) { tile_mask[i] = 4; tile_order[i] = i; if ((i & 31u) == 0u) sel_bits[i >> 5] = 0xffffffffu; }
+  }
   for (uint32_t i = tid; i < n_tt4; i += nth) tiles_touched4[i] = make_uint4(0u, 0u, 0u, 0u);
   if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
@@ -525,7 +532,7 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
   k_frame_init<<<592, 256, 0, s>>>(fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
-                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, b.sort_hist,
+                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
                                    b.F_key, reset_F ? 1 : 0);
 }
 

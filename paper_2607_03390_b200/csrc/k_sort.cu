@@ -43,7 +43,8 @@ struct SortSmem {
 };
 
 // one digit: rank within the tile (warp match + per-warp counters), look-back, scatter through smem
-__global__ void __launch_bounds__(SORT_THREADS, SORT_CTAS_PER_SM) k_onesweep(
+template <int LB_BATCH, int CTAS_PER_SM>
+__global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ n_ptr, uint32_t* __restrict__ ticket, uint32_t* __restrict__ error_flag,
     const uint32_t* __restrict__ hist, unsigned long long* __restrict__ desc, int shift, int nbits, uint32_t epoch) {
@@ -130,7 +131,8 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_CTAS_PER_SM) k_onesweep(
 #pragma unroll
     for (int w = 0; w < SORT_WARPS; ++w) if ((uint32_t)w < wid) loff += sm.scan_tmp[w];
     // decoupled look-back, one digit per thread (descriptor rows are 2 KB, read coalesced); 4 predecessors per step
-    // at first, 8 per step when the chain is long (a small input starts all its tiles at once: nobody has a prefix yet)
+    // at first, LB_BATCH per step when the chain is long (a small input starts all its tiles at once: nobody has a
+    // prefix yet, so the instance used for the few visible Gaussians walks 32 at a time)
     unsigned long long* my = desc + (size_t)tile * RADIX + d;
     uint32_t excl = 0;
     if (tile > 0) {
@@ -140,12 +142,12 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_CTAS_PER_SM) k_onesweep(
       bool done = false;
       int batch = 4;
       while (!done) {
-        unsigned long long v[8];
+        unsigned long long v[LB_BATCH];
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < LB_BATCH; ++i)
           if (i < batch) v[i] = (t - i >= 0) ? ld_volatile64(desc + (size_t)(t - i) * RADIX + d) : (tag | FLAG_PREFIX);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < LB_BATCH; ++i) {
           if (done || i >= batch) break;
           const bool mine = (v[i] >> 34) == (unsigned long long)epoch;
           const uint32_t fl = mine ? (uint32_t)(v[i] >> 32) & 3u : 0u;
@@ -154,7 +156,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_CTAS_PER_SM) k_onesweep(
           --t;
           if (fl == 2) done = true;
         }
-        batch = 8;
+        batch = LB_BATCH;
       }
     }
     st_volatile64(my, tag | FLAG_PREFIX | (excl + cnt));
@@ -223,19 +225,24 @@ int tile_sort_passes(int n_tiles) {
 // (filled by the producer of the keys), `tickets` = one zeroed counter per pass, `desc` = [passes][tiles_cap][256].
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
-                int num_sms) {
+                int num_sms, bool small_input) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(k_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    cudaFuncSetAttribute(k_onesweep<8, SORT_CTAS_PER_SM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    cudaFuncSetAttribute(k_onesweep<32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
     attr_set = true;
   }
   const int passes = (key_bits + 7) / 8;
   int cur = 0;
   for (int p = 0; p < passes; ++p) {
     const int nbits = key_bits - 8 * p < 8 ? key_bits - 8 * p : 8;
-    k_onesweep<<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(
-        keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX,
-        (unsigned long long*)desc + (size_t)p * tiles_cap * RADIX, 8 * p, nbits, epoch);
+    unsigned long long* d = (unsigned long long*)desc + (size_t)p * tiles_cap * RADIX;
+    if (small_input)
+      k_onesweep<32, 2><<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
+                                                                           error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
+    else
+      k_onesweep<8, SORT_CTAS_PER_SM><<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(
+          keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
     cur ^= 1;
   }
   return cur;

@@ -404,20 +404,20 @@ int tgs_render(tgs_ctx* c, int mode) {
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
   if (ftype == TGS_FRAME_S) launch_mark_oc(s, fc, b, c->num_sms);                                          // A4: T^oc of larger rects
   mark();                                                                      // 3
-  launch_select(s, fc, b);                                                                                 // A4: T_sel
+  if (ftype == TGS_FRAME_S) launch_select(s, fc, b);                                                       // A4: T_sel (R / P: all tiles, k_frame_init)
   if (ftype == TGS_FRAME_S) {
     CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     CK(cudaEventRecord(c->ev_sel, s));
     c->sel_pending = true;
   }
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms);            // A6 level 1: visible Gaussians by depth
+                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // A6 level 1: visible Gaussians by depth
   launch_fix_ties(s, b.ckeys[dsorted], b.cvals[dsorted], &b.counters->n_visible, c->num_sms);             // R28: equal depths by index
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // A5: tests -> pairs, counts, colours
   launch_colour(s, fc, b, dsorted, c->num_sms);                                                            // A5: SH -> RGB of the emitting Gaussians
   mark();                                                                      // 4
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
-                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms);   // A6 level 2: by tile
+                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // A6 level 2: by tile
   mark();                                                                      // 5
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
   mark();                                                                      // 6

@@ -126,7 +126,7 @@ void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sort
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
-                int num_sms);
+                int num_sms, bool small_input);
 void launch_fix_ties(cudaStream_t s, const uint32_t* keys, uint32_t* vals, const uint32_t* n_ptr, int num_sms);
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
