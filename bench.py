@@ -27,10 +27,13 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full render"
-# FP32-pipe cost of one (pixel, Gaussian) interaction of the blend inner loop, in warp-lane instructions on
-# the FMA pipe, counted from the SASS of k_blend: 2 FADD (dx, dy) + 5 FMUL/FFMA (exponent)
-# + 1 FADD (log2 o) = 8 up to the alpha test, which most interactions do not pass.
-BLEND_FMA_LANE_INSTR = 8.0
+# Lane-instructions one alive (pixel, Gaussian) interaction of the blend needs: 12 on the FMA pipe
+# (exponent 2, 1 - alpha, T (1 - alpha), alpha T, 3 colour FMAs, d - d0, w dd, 2 moment FMAs; a packed FFMA2 half
+# counts as 1) + 1 MUFU.EX2 + 8 on the ALU pipe (clamp, 2 threshold tests, first-contribution test, 4 selects).
+BLEND_LANE_INSTR = 21.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_blend<1,0> launch on config 3, from the ncu --set full capture
+# summarised in profiles/ (the file names the command); per launch, like `achieved`.
+BLEND_DRAM_TRAFFIC_BYTES = 45.7e6
 
 
 def _peaks():
@@ -188,7 +191,7 @@ def run_ours(args):
         return None
 
     hbm_gbs, sm_mhz_max, peak_kind = _peaks()
-    stage_names = ["warp", "fill_corr", "preprocess_markoc", "select_count_compact_depthsort_emit", "tile_sort", "ranges", "blend_stitch", "post"]
+    stage_names = ["init_warp_fill", "preprocess_select", "depth_sort", "bin_pairs", "sh_colour", "tile_sort_ranges", "blend_stitch", "post"]
 
     def summarise(lst):
         if not lst:
@@ -211,34 +214,43 @@ def run_ours(args):
     dom = int(np.argmax(tot))
     all_stats = [s for lst in per_type.values() for s in lst]
     roof = None
+    sm_clk = (clocks or {}).get("sm_mhz") or sm_mhz_max
+    T_ = ((sc.camera.W + 15) // 16) * ((sc.camera.H + 15) // 16)
+    tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
+    mean = lambda key: float(np.mean([s[key] for s in all_stats]))
+    # per-stage achieved fraction of the roofline that bounds it; algorithmic bytes / work from the
+    # per-frame counters, time from the stage events (kernel boundaries and launch gaps included)
+    t_stage = np.mean([s["ms_stage"] for s in all_stats], axis=0) * 1e-3
+    P, Nv, L = mean("n_pairs"), mean("n_visible"), mean("n_interactions")
+    alu_peak = 148 * 128 * sm_clk * 1e6 / 1e12          # T lane-instr/s at the clock seen under load
+    stage_roof = {
+        "preprocess_select": {"bound": "hbm", "achieved": (sc.n * (16 + 4) + Nv * (32 + 16 + 100)) / t_stage[1] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
+        "depth_sort": {"bound": "hbm", "achieved": Nv * 16 * 4 / t_stage[2] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
+        "sh_colour": {"bound": "hbm", "achieved": Nv * (8 + 16 + 12 * (sc.sh_degree + 1) ** 2 + 16) / t_stage[4] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
+        "tile_sort_ranges": {"bound": "hbm", "achieved": P * (16 * tile_passes + 4) / t_stage[5] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
+        "blend_stitch": {"bound": "alu", "achieved": L * BLEND_LANE_INSTR / t_stage[6] / 1e12, "peak": alu_peak, "unit": "T lane-instr/s"},
+    }
+    for v in stage_roof.values():
+        v["frac"] = v["achieved"] / v["peak"]
     if stage_names[dom] == "blend_stitch":
-        # FP32 (FMA-pipe) bound: lane-instructions/s = interactions * instr per interaction / time
-        L = np.mean([s["n_interactions"] for s in all_stats])
-        t = np.mean([s["ms_stage"][6] for s in all_stats]) * 1e-3
-        sm_clk = (clocks or {}).get("sm_mhz") or sm_mhz_max
-        peak = 148 * 128 * sm_clk * 1e6 / 1e12          # T lane-instr/s at the clock seen under load
-        ach = L * BLEND_FMA_LANE_INSTR / t / 1e12
-        roof = {"kernel": "k_blend", "bound": "alu", "achieved": ach, "peak": peak, "unit": "T lane-instr/s (FP32 pipe)",
-                "frac": ach / peak, "traffic": None, "interactions_per_launch": float(L), "ms_per_launch": t * 1e3,
-                "peak_note": f"148 SM x 128 FP32 lanes x {sm_clk:.0f} MHz (median SM clock during the run)"}
+        # instruction-issue bound ("alu"): lane-instructions/s = alive interactions * instr per interaction / time
+        t = t_stage[6]
+        ach = L * BLEND_LANE_INSTR / t / 1e12
+        roof = {"kernel": "k_blend", "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-instr/s",
+                "frac": ach / alu_peak, "traffic": BLEND_DRAM_TRAFFIC_BYTES, "interactions_per_launch": float(L),
+                "blended_per_launch": mean("n_blended"), "pixel_slots_per_launch": mean("n_pixel_slots"),
+                "ms_per_launch": t * 1e3,
+                "peak_note": f"148 SM x 4 schedulers x 32 lanes x {sm_clk:.0f} MHz (median SM clock during the run): one warp "
+                             f"instruction per scheduler and clock; the FMA pipe (128 lanes/clk/SM) and the ALU pipe (64) are not tighter "
+                             f"for this mix (DESIGN.md 7.2)"}
     else:
-        # HBM bound stages: algorithmic bytes per launch / duration
-        P = np.mean([s["n_pairs"] for s in all_stats])
-        t = np.mean([s["ms_stage"][dom] for s in all_stats]) * 1e-3
-        T_ = ((sc.camera.W + 15) // 16) * ((sc.camera.H + 15) // 16)
-        tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
-        if stage_names[dom] == "tile_sort":
-            by = P * (4 + tile_passes * 16)        # histogram read + per digit 8 B read + 8 B written
-            kname = "k_onesweep (tile sort, + k_sort_hist)"
-        elif stage_names[dom] == "preprocess_markoc":
-            by = sc.n * 16 + np.mean([s["n_visible"] for s in all_stats]) * (24 + 44)
-            kname = "k_preprocess"
-        else:
-            by = P * 8 + sc.n * 8
-            kname = stage_names[dom]
-        ach = by / t / 1e9
-        roof = {"kernel": kname, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
-                "traffic": None, "ms_per_launch": t * 1e3, "peak_note": f"{peak_kind} copy bandwidth"}
+        key = stage_names[dom]
+        r = stage_roof.get(key)
+        if r is None:
+            by = P * 8 + Nv * 64
+            r = {"bound": "hbm", "achieved": by / t_stage[dom] / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+            r["frac"] = r["achieved"] / r["peak"]
+        roof = {"kernel": key, **r, "traffic": None, "ms_per_launch": float(t_stage[dom] * 1e3), "peak_note": f"{peak_kind} copy bandwidth"}
 
     fps_tgs = world * K / (ms_tgs * 1e-3)
     fps_full = world * K / (ms_full * 1e-3)
@@ -255,17 +267,16 @@ def run_ours(args):
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 16 * 4 + 8 * 4, "d2h_bytes_per_step": cam.W * cam.H * 3 * 4,
                 "note": "camera by value through tgs_set_camera; image read into pinned host memory every frame"},
         "gpu_launches": None,
-        "stages": stages, "roofline": roof, "clocks": clocks,
+        "stages": stages, "roofline": roof, "stage_rooflines": stage_roof, "clocks": clocks,
     }
-    # launches per frame: init, [warp, fill], preprocess, select, count, scan_emit, hist, scan_hist, passes x onesweep,
-    # ranges, blend, [frustum]
+    # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), fix_ties, scan_area, bin_test, bin_emit,
+    # colour, tile sort (digits), ranges, blend = 13 + tile digits; + frustum on R / P; + warp, fill_corr, mark_oc,
+    # select on S
     T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
     tpasses = (max(1, int(np.ceil(np.log2(T)))) + 7) // 8
     nR = sum(1 for s in all_stats if s["frame_type"] != 2)
-    # init, preprocess, select, count, compact, depth sort (hist, scan, 4 digits), scan_emit, tile sort (hist, scan, digits),
-    # ranges, blend, + frustum (R/P) or + warp, fill, mark_oc (S)
-    base = 1 + 1 + 1 + 1 + 1 + 6 + 1 + (2 + tpasses) + 1 + 1
-    per_ref, per_s = base + 1, base + 3
+    base = 13 + tpasses
+    per_ref, per_s = base + 1, base + 4
     frac_ref = nR / max(1, len(all_stats))
     out["gpu_launches"] = int(round(K * (frac_ref * per_ref + (1 - frac_ref) * per_s)))
     if world > 1:

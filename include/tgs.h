@@ -86,8 +86,9 @@ typedef struct {
   uint64_t n_blended;      /* of those, the ones with alpha >= 1/255 that were composited (counting on) */
   uint64_t n_pixel_slots;  /* pixel slots issued by the blend loop, dead lanes included (counting on) */
   float ms_stage[8];   /* per-stage device time when timing is on (tgs_debug_run_stage("timing_on")):
-                          0 warp, 1 fill+corr, 2 preprocess, 3 select+count+scan+keys, 4 sort, 5 ranges,
-                          6 blend+stitch, 7 post (F reduction, stats) */
+                          0 init + warp + fill/correspondence, 1 preprocess + tile selection, 2 depth sort of the visible
+                          Gaussians, 3 pair binning (tile tests, emission), 4 SH colours, 5 tile sort + ranges,
+                          6 blend + stitch, 7 post (F reduction, stats) */
   float ms_total;
   uint64_t device_bytes; /* device memory held by the context */
 } tgs_stats;

@@ -395,35 +395,35 @@ int tgs_render(tgs_ctx* c, int mode) {
   uint8_t* rendered_next = builds_priors ? b.rendered_next : nullptr;
   int ev = 0;
   auto mark = [&]() { if (c->timing) cudaEventRecord(c->ev_stage[ev], s); ++ev; };
-  mark();                                                                      // 0
+  mark();                                                                      // 0: init, A1 warp, A2 fill + correspondence
   launch_frame_init(s, fc, b, ftype == TGS_FRAME_R, rendered_next);
   if (ftype == TGS_FRAME_S) launch_warp(s, fc, b, b.depth[c->prior_idx], b.sigma[c->prior_idx]);          // A1
-  mark();                                                                      // 1
   if (ftype == TGS_FRAME_S) launch_fill_corr(s, fc, b);                                                    // A2
-  mark();                                                                      // 2
+  mark();                                                                      // 1: A3 preprocess, A4 selection
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
-  if (ftype == TGS_FRAME_S) launch_mark_oc(s, fc, b, c->num_sms);                                          // A4: T^oc of larger rects
-  mark();                                                                      // 3
-  if (ftype == TGS_FRAME_S) launch_select(s, fc, b);                                                       // A4: T_sel (R / P: all tiles, k_frame_init)
   if (ftype == TGS_FRAME_S) {
+    launch_mark_oc(s, fc, b, c->num_sms);                                                                  // A4: T^oc of larger rects
+    launch_select(s, fc, b);                                                                               // A4: T_sel (R / P: all tiles, k_frame_init)
     CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     CK(cudaEventRecord(c->ev_sel, s));
     c->sel_pending = true;
   }
+  mark();                                                                      // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // A6 level 1: visible Gaussians by depth
+                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // visible Gaussians by depth
   launch_fix_ties(s, b.ckeys[dsorted], b.cvals[dsorted], &b.counters->n_visible, c->num_sms);             // R28: equal depths by index
-  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // A5: tests -> pairs, counts, colours
-  launch_colour(s, fc, b, dsorted, c->num_sms);                                                            // A5: SH -> RGB of the emitting Gaussians
-  mark();                                                                      // 4
+  mark();                                                                      // 3: A5 pairs
+  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
+  mark();                                                                      // 4: A5 colours
+  launch_colour(s, fc, b, dsorted, c->num_sms);                                                            // SH -> RGB of the emitting Gaussians
+  mark();                                                                      // 5: A6 level 2 + A7
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
-                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // A6 level 2: by tile
-  mark();                                                                      // 5
+                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // pairs by tile
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
-  mark();                                                                      // 6
-  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);                         // A8 + A9
-  mark();                                                                      // 7
-  if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);                        // F_min/F_max (L109)
+  mark();                                                                      // 6: A8 + A9
+  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);
+  mark();                                                                      // 7: post
+  if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
   CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
   mark();                                                                      // 8
   CK(cudaEventRecord(c->ev_done, s));
