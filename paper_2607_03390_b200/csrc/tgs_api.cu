@@ -53,6 +53,8 @@ struct tgs_ctx {
   Counters* h_counters = nullptr;      // pinned
   uint32_t* h_sel = nullptr;           // pinned: n_sel of the last S frame (for the eta rule)
   cudaEvent_t ev_sel = nullptr, ev_done = nullptr;
+  cudaStream_t side = nullptr;          // second stream: work that is off the critical path of a frame (SH colours, A2)
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr;
   bool sel_pending = false;
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
@@ -228,6 +230,8 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   if (cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
+  cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
+  for (cudaEvent_t* e : {&c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2}) cudaEventCreateWithFlags(e, cudaEventDisableTiming);
   for (auto& e : c->ev_stage) cudaEventCreate(&e);
   *out = c;
   return TGS_OK;
@@ -241,6 +245,8 @@ void tgs_destroy(tgs_ctx* c) {
   cudaFree(c->b.counters); cudaFree(c->b.F_key); cudaFree(c->b.sort_hist);
   cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
   cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
+  cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
+  for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_fork2, c->ev_join2}) cudaEventDestroy(e);
   for (auto& e : c->ev_stage) cudaEventDestroy(e);
   delete c;
 }
@@ -398,11 +404,19 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 0: init, A1 warp, A2 fill + correspondence
   launch_frame_init(s, fc, b, ftype == TGS_FRAME_R, rendered_next);
   if (ftype == TGS_FRAME_S) launch_warp(s, fc, b, b.depth[c->prior_idx], b.sigma[c->prior_idx]);          // A1
-  if (ftype == TGS_FRAME_S) launch_fill_corr(s, fc, b);                                                    // A2
+  // A2 (depth fill, correspondence, T^um) is only needed by the tile selection: it runs beside the preprocess.
+  // With stage timing on, everything stays on one stream so that the stage events bracket what they name.
+  const bool fork = !c->timing;
+  if (ftype == TGS_FRAME_S) {
+    if (fork) { CK(cudaEventRecord(c->ev_fork2, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork2, 0)); }
+    launch_fill_corr(fork ? c->side : s, fc, b);                                                           // A2
+    if (fork) CK(cudaEventRecord(c->ev_join2, c->side));
+  }
   mark();                                                                      // 1: A3 preprocess, A4 selection
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
   if (ftype == TGS_FRAME_S) {
     launch_mark_oc(s, fc, b, c->num_sms);                                                                  // A4: T^oc of larger rects
+    if (fork) CK(cudaStreamWaitEvent(s, c->ev_join2, 0));
     launch_select(s, fc, b);                                                                               // A4: T_sel (R / P: all tiles, k_frame_init)
     CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     CK(cudaEventRecord(c->ev_sel, s));
@@ -414,13 +428,16 @@ int tgs_render(tgs_ctx* c, int mode) {
   launch_fix_ties(s, b.ckeys[dsorted], b.cvals[dsorted], &b.counters->n_visible, c->num_sms);             // R28: equal depths by index
   mark();                                                                      // 3: A5 pairs
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
-  mark();                                                                      // 4: A5 colours
-  launch_colour(s, fc, b, dsorted, c->num_sms);                                                            // SH -> RGB of the emitting Gaussians
+  mark();                                                                      // 4: A5 colours (beside the tile sort: only the blend needs them)
+  if (fork) { CK(cudaEventRecord(c->ev_fork, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0)); }
+  launch_colour(fork ? c->side : s, fc, b, dsorted, c->num_sms);                                           // SH -> RGB of the emitting Gaussians
+  if (fork) CK(cudaEventRecord(c->ev_join, c->side));
   mark();                                                                      // 5: A6 level 2 + A7
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
                                  b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // pairs by tile
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
   mark();                                                                      // 6: A8 + A9
+  if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
   launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);
   mark();                                                                      // 7: post
   if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
