@@ -3,18 +3,20 @@
 // Gaussians by depth from front to back"), L123 (only Gaussians intersecting T_selected are sorted).
 //
 // The visible Gaussians arrive sorted by (depth, index).  Every (Gaussian, tile of its test rect) combination -- the
-// test rect is the part of the 3-sigma rect that k_preprocess could not rule out -- is one TEST; the tests of all Gaussians, in that order and row-major inside a rect, form one flat index space
-// (k_scan_area: prefix sums of the rect areas).  k_bin cuts that space into equal chunks -- so a screen-filling
-// Gaussian is spread over many CTAs instead of stalling one warp -- evaluates each test once (tile selected, L123,
-// and reached with alpha >= 1/255, R39), ranks the passing tests with a single-pass scan (decoupled look-back) and
-// writes the pairs (tile id, Gaussian) in exactly the oracle's emission order; the stable sort by tile id that
-// follows (k_sort.cu) then leaves every tile's list in (depth, index) order.  The same kernel counts the pairs per
-// Gaussian; k_colour then evaluates SH -> RGB (L61 "color c_i"; R5) for the Gaussians that emitted at least one pair,
-// so on S frames the SH bytes are read only for Gaussians that reach a selected tile.
+// test rect is the part of the 3-sigma rect that k_preprocess could not rule out -- is one TEST; the tests of all
+// Gaussians, in that order and row-major inside a rect, form one flat index space (k_scan_area: prefix sums of the
+// rect areas).  The space is cut into equal chunks -- so a screen-filling Gaussian is spread over many CTAs instead
+// of stalling one warp.  k_bin_test evaluates each test once (tile selected, L123, and reached with alpha >= 1/255,
+// R39), with no dependency between chunks, and leaves one mask byte per 8 tests plus the pair count of every chunk;
+// its last CTA scans the counts.  k_bin_emit walks the chunks again (no tests) and writes the pairs (tile id,
+// Gaussian) in exactly the oracle's emission order; the stable sort by tile id that follows (k_sort.cu) then leaves
+// every tile's list in (depth, index) order.  k_bin_test also counts the pairs per Gaussian; k_colour evaluates
+// SH -> RGB (L61 "color c_i"; R5) for the Gaussians that emitted at least one pair, so on S frames the SH bytes are
+// read only for Gaussians that reach a selected tile.
 //
 // Compiled with -fmad=false: the tile test is decision arithmetic (decide_math.cuh).
-// Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory; the
-// kernels are persistent grids pulling work tickets, so a frame needs no host round trip.
+// Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory, so a
+// frame needs no host round trip.
 #include "tgs_internal.cuh"
 #include "decide_math.cuh"
 #include "scan.cuh"
