@@ -5,14 +5,13 @@
 // The visible Gaussians arrive sorted by (depth, index).  Every (Gaussian, tile of its test rect) combination -- the
 // test rect is the part of the 3-sigma rect that k_preprocess could not rule out -- is one TEST; the tests of all
 // Gaussians, in that order and row-major inside a rect, form one flat index space (k_scan_area: prefix sums of the
-// rect areas).  The space is cut into equal chunks -- so a screen-filling Gaussian is spread over many CTAs instead
-// of stalling one warp.  k_bin_test evaluates each test once (tile selected, L123, and reached with alpha >= 1/255,
-// R39), with no dependency between chunks, and leaves one mask byte per 8 tests plus the pair count of every chunk;
-// its last CTA scans the counts.  k_bin_emit walks the chunks again (no tests) and writes the pairs (tile id,
-// Gaussian) in exactly the oracle's emission order; the stable sort by tile id that follows (k_sort.cu) then leaves
-// every tile's list in (depth, index) order.  k_bin_test also counts the pairs per Gaussian; k_colour evaluates
-// SH -> RGB (L61 "color c_i"; R5) for the Gaussians that emitted at least one pair, so on S frames the SH bytes are
-// read only for Gaussians that reach a selected tile.
+// rect areas).  k_bin cuts that space into equal chunks -- so a screen-filling Gaussian is spread over many CTAs
+// instead of stalling one warp -- evaluates each test once (tile selected, L123, and reached with alpha >= 1/255,
+// R39), ranks the passing tests with a single-pass scan (decoupled look-back over the chunks) and writes the pairs
+// (tile id, Gaussian) in exactly the oracle's emission order; the stable sort by tile id that follows (k_sort.cu)
+// then leaves every tile's list in (depth, index) order.  The same kernel counts the pairs per Gaussian and the
+// digit histograms of the tile sort; k_colour evaluates SH -> RGB (L61 "color c_i"; R5) for the Gaussians that
+// emitted at least one pair, so on S frames the SH bytes are read only for Gaussians that reach a selected tile.
 //
 // Compiled with -fmad=false: the tile test is decision arithmetic (decide_math.cuh).
 // Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory, so a
@@ -174,178 +173,110 @@ __device__ __forceinline__ bool tile_reach(const GaussParams& P, uint32_t tx, ui
   return box_qmin(P.u, P.v, P.A, P.B, P.C, x0, x1, y0, y1) <= P.tau;       // the oracle's sequence decides
 }
 
-// ---- k_bin_test: every test of the flat space, once.  A chunk = 1024 consecutive tests, 8 per thread; the outcome
-// is one mask byte per thread (chunk_mask) and the number of passing tests of the chunk (chunk_cnt).  No chunk
-// depends on another one.  The CTA that finishes last turns the counts into exclusive offsets (and P).
-__global__ void __launch_bounds__(BIN_THREADS) k_bin_test(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
-                                                          const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
-                                                          const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
-                                                          const uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tiles_touched,
-                                                          uint8_t* __restrict__ chunk_mask, uint2* __restrict__ chunk_cnt,
-                                                          Counters* __restrict__ counters) {
-  __shared__ uint32_t s_prefix[BIN_CHUNK + 2];
-  __shared__ GaussParams s_gp[BIN_PCAP];
-  __shared__ uint32_t s_warp[BIN_THREADS / 32];
-  __shared__ uint32_t s_last;
+// ---- k_bin: tests, ranks (single-pass scan with decoupled look-back over the chunks) and pairs of one chunk
+struct BinSmem {
+  uint32_t prefix[BIN_CHUNK + 2];       // area_prefix of the Gaussians of this chunk (+ sentinel)
+  uint32_t st_tile[BIN_CHUNK];          // passing tests of the chunk, in order: tile id
+  uint32_t st_g[BIN_CHUNK];             //                                        Gaussian
+  GaussParams gp[BIN_PCAP];
+  uint32_t warp[BIN_THREADS / 32];
+  uint32_t excl, chunk;
+  uint32_t hist[2][256];                // digit histograms of the tile ids of the emitted pairs (for the tile sort)
+};
+
+__global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
+                                                     const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
+                                                     const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                     const uint32_t* __restrict__ sel_bits, unsigned long long* __restrict__ desc,
+                                                     uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ keys,
+                                                     uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
+                                                     Counters* __restrict__ counters) {
+  __shared__ BinSmem sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
   const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
-  const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const uint32_t tid = threadIdx.x, lane = tid & 31;
   const int TX = fc.cam.TX;
   const bool exact = fc.exact_tiles != 0;
-  for (uint32_t chunk = blockIdx.x; chunk < num_chunks; chunk += gridDim.x) {
+  for (int i = tid; i < 2 * 256; i += BIN_THREADS) (&sm.hist[0][0])[i] = 0;
+  while (true) {
+    __syncthreads();
+    if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin, 1u);
+    __syncthreads();
+    const uint32_t chunk = sm.chunk;
+    if (chunk >= num_chunks) break;
     const uint32_t cbase = chunk * BIN_CHUNK;
     const uint32_t tend = (total_tests - cbase < (uint32_t)BIN_CHUNK) ? total_tests : cbase + BIN_CHUNK;
     const uint32_t i_first = chunk_first[chunk];
     const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
     const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
-    __syncthreads();
-    for (uint32_t i = tid; i <= m; i += BIN_THREADS) s_prefix[i] = area_prefix[i_first + i];
+    for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
     for (uint32_t i = tid; i < m && i < (uint32_t)BIN_PCAP; i += BIN_THREADS)
-      s_gp[i] = load_params(sorted_g[i_first + i], exact, rec_rect, rec_uvdo, rec_conic);
+      sm.gp[i] = load_params(sorted_g[i_first + i], exact, rec_rect, rec_uvdo, rec_conic);
     __syncthreads();
+    // ---------------------------------------------------------------- tests
     const uint32_t t0 = cbase + tid * BIN_IPT;
-    uint32_t mask = 0;
+    uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
     if (t0 < tend) {
       uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
-      while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (s_prefix[mid] <= t0) lo = mid; else hi = mid; }
+      while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
       uint32_t li = lo, segcnt = 0, end, rx, ry, x_lo, y_lo;
       GaussParams G;
       auto load = [&](uint32_t l, uint32_t t) {
-        G = l < (uint32_t)BIN_PCAP ? s_gp[l] : load_params(sorted_g[i_first + l], exact, rec_rect, rec_uvdo, rec_conic);
-        end = s_prefix[l + 1];
-        const uint32_t local = t - s_prefix[l];
+        G = l < (uint32_t)BIN_PCAP ? sm.gp[l] : load_params(sorted_g[i_first + l], exact, rec_rect, rec_uvdo, rec_conic);
+        end = sm.prefix[l + 1];
+        const uint32_t local = t - sm.prefix[l];
         ry = local / G.w; rx = local - ry * G.w;
         x_lo = G.lo & 0xffffu; y_lo = G.lo >> 16;
+      };
+      auto flush = [&]() {
+        if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
+        segcnt = 0;
       };
       load(li, t0);
 #pragma unroll
       for (int k = 0; k < BIN_IPT; ++k) {
         const uint32_t t = t0 + k;
         if (t < tend) {
-          if (t >= end) {
-            if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
-            segcnt = 0;
-            do { ++li; } while (s_prefix[li + 1] <= t);
-            load(li, t);
-          }
+          if (t >= end) { flush(); do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
           const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
           bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
           if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
           if (pass) { mask |= 1u << k; ++segcnt; }
+          tl[k] = tile; gg[k] = G.g;
           if (++rx == G.w) { rx = 0; ++ry; }
         }
       }
-      if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
+      flush();
     }
-    chunk_mask[(size_t)chunk * BIN_THREADS + tid] = (uint8_t)mask;
-    const uint32_t wsum = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(mask));
-    if (lane == 0) s_warp[wid] = wsum;
-    __syncthreads();
-    if (tid == 0) { uint32_t c = 0; for (int w = 0; w < BIN_THREADS / 32; ++w) c += s_warp[w]; chunk_cnt[chunk].x = c; }
-  }
-  // ---- the last CTA to arrive: exclusive scan of the chunk counts
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(&counters->ticket_bin, 1u) == gridDim.x - 1u) ? 1u : 0u;
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  const uint32_t per = (num_chunks + BIN_THREADS - 1) / BIN_THREADS;
-  const uint32_t c0 = tid * per, c1 = min(num_chunks, c0 + per);
-  uint32_t sum = 0;
-  for (uint32_t c = c0; c < c1; ++c) sum += *reinterpret_cast<volatile uint32_t*>(&chunk_cnt[c].x);
-  uint32_t incl = sum;
+    // ---------------------------------------------------------------- rank the passing tests (chunk-local + global)
+    uint32_t incl_total;
+    const uint32_t goff = tgs_scan::chunk_scan<BIN_THREADS>(__popc(mask), chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total, fc.epoch);
+    const uint32_t cexcl = sm.excl, ctotal = incl_total - cexcl;
+    const bool overflow = incl_total > fc.max_pairs;
+    if (chunk == num_chunks - 1 && tid == 0) {
+      if (overflow) { counters->overflow = 1; counters->n_pairs = 0; }
+      else counters->n_pairs = incl_total;
+    }
+    uint32_t lpos = goff - cexcl;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
-  if (lane == 31) s_warp[wid] = incl;
-  __syncthreads();
-  uint32_t off = incl - sum, total = 0;
-  for (int w = 0; w < BIN_THREADS / 32; ++w) { if ((uint32_t)w < wid) off += s_warp[w]; total += s_warp[w]; }
-  for (uint32_t c = c0; c < c1; ++c) { const uint32_t v = *reinterpret_cast<volatile uint32_t*>(&chunk_cnt[c].x); chunk_cnt[c].y = off; off += v; }
-  if (tid == 0) {
-    if (total > fc.max_pairs) { counters->overflow = 1; counters->n_pairs = 0; }
-    else counters->n_pairs = total;
-  }
-}
-
-// ---- k_bin_emit: the passing tests of a chunk become pairs (tile id, Gaussian) at the chunk's offset, in test order
-struct EmitSmem {
-  uint32_t prefix[BIN_CHUNK + 2];
-  uint32_t st_tile[BIN_CHUNK];
-  uint32_t st_g[BIN_CHUNK];
-  uint32_t warp[BIN_THREADS / 32];
-  uint32_t hist[2][256];                // digit histograms of the tile ids of the emitted pairs (for the tile sort)
-};
-
-__global__ void __launch_bounds__(BIN_THREADS) k_bin_emit(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
-                                                          const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
-                                                          const uint8_t* __restrict__ chunk_mask, const uint2* __restrict__ chunk_cnt,
-                                                          uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                                          uint32_t* __restrict__ tile_hist, const Counters* __restrict__ counters) {
-  __shared__ EmitSmem sm;
-  if (counters->overflow) return;
-  const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
-  const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
-  const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int TX = fc.cam.TX;
-  for (int i = tid; i < 2 * 256; i += BIN_THREADS) (&sm.hist[0][0])[i] = 0;
-  for (uint32_t chunk = blockIdx.x; chunk < num_chunks; chunk += gridDim.x) {
-    const uint2 cc = chunk_cnt[chunk];                           // {pairs of the chunk, pairs before it}
-    if (cc.x == 0) continue;
-    const uint32_t cbase = chunk * BIN_CHUNK;
-    const uint32_t i_first = chunk_first[chunk];
-    const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
-    const uint32_t m = i_last - i_first + 1;
-    const uint32_t mask = chunk_mask[(size_t)chunk * BIN_THREADS + tid];
+    for (int k = 0; k < BIN_IPT; ++k)
+      if ((mask >> k) & 1u) { sm.st_tile[lpos] = tl[k]; sm.st_g[lpos] = gg[k]; ++lpos; }
     __syncthreads();
-    for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
-    // chunk-local rank of this thread's first pass
-    const uint32_t cnt = __popc(mask);
-    uint32_t incl = cnt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
-    if (lane == 31) sm.warp[wid] = incl;
-    __syncthreads();
-    uint32_t lpos = incl - cnt;
-    for (int w = 0; w < BIN_THREADS / 32; ++w) if ((uint32_t)w < wid) lpos += sm.warp[w];
-    if (mask) {
-      const uint32_t t0 = cbase + tid * BIN_IPT;
-      uint32_t lo = 0, hi = m;
-      while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
-      uint32_t li = lo, end, rx, ry, x_lo, y_lo, w, g;
-      auto load = [&](uint32_t l, uint32_t t) {
-        g = sorted_g[i_first + l];
-        const uint2 r = rec_rect[g];
-        x_lo = r.x & 0xffffu; y_lo = r.y & 0xffffu; w = (r.x >> 16) - x_lo;
-        end = sm.prefix[l + 1];
-        const uint32_t local = t - sm.prefix[l];
-        ry = local / w; rx = local - ry * w;
-      };
-      load(li, t0);
-#pragma unroll
-      for (int k = 0; k < BIN_IPT; ++k) {
-        if ((mask >> k) == 0u) break;                            // no further pass of this thread
-        const uint32_t t = t0 + k;
-        if (t >= end) { do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
-        if ((mask >> k) & 1u) { sm.st_tile[lpos] = (y_lo + ry) * TX + x_lo + rx; sm.st_g[lpos] = g; ++lpos; }
-        if (++rx == w) { rx = 0; ++ry; }
+    if (!overflow)
+      for (uint32_t p0 = 0; p0 < ctotal; p0 += BIN_THREADS) {
+        const uint32_t p = p0 + tid;
+        const bool in = p < ctotal;
+        const uint32_t tile = in ? sm.st_tile[p] : 0xffffffffu;
+        if (in) { keys[cexcl + p] = tile; vals[cexcl + p] = sm.st_g[p]; atomicAdd(&sm.hist[0][tile & 255u], 1u); }
+        // upper digit: consecutive pairs are consecutive tiles of one Gaussian, so it comes in runs: one atomic per run
+        const uint32_t hi = tile >> 8, prev = __shfl_up_sync(0xffffffffu, hi, 1);
+        const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || hi != prev);
+        if (in && ((heads >> lane) & 1u)) {
+          const uint32_t above = heads & ~((2u << lane) - 1u);               // heads of later runs
+          const uint32_t run = (above ? (uint32_t)__ffs(above) - 1u : 32u) - lane;
+          atomicAdd(&sm.hist[1][hi & 255u], run);
+        }
       }
-    }
-    __syncthreads();
-    for (uint32_t p0 = 0; p0 < cc.x; p0 += BIN_THREADS) {
-      const uint32_t p = p0 + tid;
-      const bool in = p < cc.x;
-      const uint32_t tile = in ? sm.st_tile[p] : 0xffffffffu;
-      if (in) { keys[cc.y + p] = tile; vals[cc.y + p] = sm.st_g[p]; atomicAdd(&sm.hist[0][tile & 255u], 1u); }
-      // upper digit: consecutive pairs are consecutive tiles of one Gaussian, so it comes in runs: one atomic per run
-      const uint32_t hi8 = tile >> 8, prev = __shfl_up_sync(0xffffffffu, hi8, 1);
-      const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || hi8 != prev);
-      if (in && ((heads >> lane) & 1u)) {
-        const uint32_t above = heads & ~((2u << lane) - 1u);               // heads of later runs
-        const uint32_t run = (above ? (uint32_t)__ffs(above) - 1u : 32u) - lane;
-        atomicAdd(&sm.hist[1][hi8 & 255u], run);
-      }
-    }
   }
   __syncthreads();
   for (int i = tid; i < 2 * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
@@ -401,10 +332,8 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
   k_scan_area<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
                                                       b.counters, max_tests);
-  k_bin_test<<<num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic,
-                                                               b.sel_bits, b.tiles_touched, b.chunk_mask, (uint2*)b.bin_desc, b.counters);
-  k_bin_emit<<<num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.chunk_mask,
-                                                               (const uint2*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+  k_bin<<<num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
+                                                          (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
 }
 
 void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms) {

@@ -150,7 +150,6 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs, int passes) {
   c->bin_chunks_cap = (uint32_t)(max_tests / bin_chunk_items()) + 2;
   if (int r = dev_alloc(c, &b.chunk_first, (size_t)c->bin_chunks_cap, c->allocs_pairs)) return r;
   if (int r = dev_alloc(c, &b.bin_desc, (size_t)c->bin_chunks_cap, c->allocs_pairs, true)) return r;
-  if (int r = dev_alloc(c, &b.chunk_mask, (size_t)c->bin_chunks_cap * (bin_chunk_items() / 8), c->allocs_pairs)) return r;
   c->max_pairs = max_pairs;
   return TGS_OK;
 }

@@ -92,8 +92,7 @@ struct DevBuffers {
   uint64_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors (epoch-tagged)
   uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
   uint64_t* scan_desc = nullptr;      // look-back descriptors of k_scan_area
-  uint64_t* bin_desc = nullptr;       // k_bin: [bin_chunks_cap] {pairs of the chunk, pairs before it}
-  uint8_t* chunk_mask = nullptr;      // k_bin: [bin_chunks_cap][128] outcome of 8 tests per byte
+  uint64_t* bin_desc = nullptr;       //                        k_bin [bin_chunks_cap]
   // tiles
   uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
   uint8_t* tile_mask = nullptr;       // [T] bit0 oc, bit1 um, bit2 selected
