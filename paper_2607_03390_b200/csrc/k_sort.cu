@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
     const uint32_t tile = sm.tile;
     if (tile >= num_tiles) break;
     for (int i = threadIdx.x; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&sm.warp_hist[0][0])[i] = 0;
+    sm.gbase[threadIdx.x] = 0;                            // doubles as the tile's digit histogram until the look-back
     const uint32_t base = tile * SORT_TILE + wid * (32 * SORT_IPT);
     uint32_t key[SORT_IPT], val[SORT_IPT];
 #pragma unroll
@@ -88,6 +89,17 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
       val[i] = idx < n ? vals_in[idx] : 0u;
     }
     __syncthreads();
+    // The tile's digit counts are published as its look-back AGGREGATE before the (long) ranking: by the time a
+    // successor looks back, its predecessors' aggregates are there and nobody spins.
+#pragma unroll
+    for (int i = 0; i < SORT_IPT; ++i) atomicAdd(&sm.gbase[(uint32_t)(key[i] >> shift) & 255u], 1u);
+    __syncthreads();
+    unsigned long long* my = desc + (size_t)tile * RADIX + threadIdx.x;
+    {
+      uint32_t c = sm.gbase[threadIdx.x];
+      if (threadIdx.x == 255u) c -= SORT_TILE - min((uint32_t)SORT_TILE, n - tile * SORT_TILE);   // padding keys all have digit 255
+      if (tile > 0) st_volatile64(my, tag | FLAG_AGG | c);
+    }
     uint32_t rank[SORT_IPT], mt[SORT_IPT];
 #pragma unroll
     for (int i = 0; i < SORT_IPT; ++i) {      // lanes of the warp with the same digit, from one ballot per bit: match.any
@@ -133,10 +145,8 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
     // decoupled look-back, one digit per thread (descriptor rows are 2 KB, read coalesced); 4 predecessors per step
     // at first, LB_BATCH per step when the chain is long (a small input starts all its tiles at once: nobody has a
     // prefix yet, so the instance used for the few visible Gaussians walks 32 at a time)
-    unsigned long long* my = desc + (size_t)tile * RADIX + d;
     uint32_t excl = 0;
     if (tile > 0) {
-      st_volatile64(my, tag | FLAG_AGG | cnt);
       uint32_t polls = 0;
       int t = (int)tile - 1;
       bool done = false;
@@ -151,7 +161,7 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
           if (done || i >= batch) break;
           const bool mine = (v[i] >> 34) == (unsigned long long)epoch;
           const uint32_t fl = mine ? (uint32_t)(v[i] >> 32) & 3u : 0u;
-          if (fl == 0) { if (++polls > LOOKBACK_WATCHDOG) { *error_flag = 2; done = true; } break; }   // not ready: poll again from here
+          if (fl == 0) { __nanosleep(64); if (++polls > LOOKBACK_WATCHDOG) { *error_flag = 2; done = true; } break; }   // not ready: poll again from here
           excl += (uint32_t)v[i];
           --t;
           if (fl == 2) done = true;
