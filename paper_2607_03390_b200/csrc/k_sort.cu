@@ -238,7 +238,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
                 int num_sms, bool small_input) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(k_onesweep<8, SORT_CTAS_PER_SM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    cudaFuncSetAttribute(k_onesweep<4, SORT_CTAS_PER_SM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
     cudaFuncSetAttribute(k_onesweep<32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
     attr_set = true;
   }
@@ -251,7 +251,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
       k_onesweep<32, 2><<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
                                                                            error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
     else
-      k_onesweep<8, SORT_CTAS_PER_SM><<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(
+      k_onesweep<4, SORT_CTAS_PER_SM><<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(
           keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
     cur ^= 1;
   }
