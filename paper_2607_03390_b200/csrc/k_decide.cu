@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* _
     }
   }
   const int any = __syncthreads_or(unmatched ? 1 : 0);
-  if (threadIdx.x == 0 && any) tile_flags[blockIdx.y * k.TX + blockIdx.x] = 2u;   // bit1 = T^um (first writer of this word)
+  if (threadIdx.x == 0 && any) atomicOr(&tile_flags[blockIdx.y * k.TX + blockIdx.x], 2u);   // bit1 = T^um (k_preprocess ORs bit0 concurrently)
 }
 
 }  // namespace

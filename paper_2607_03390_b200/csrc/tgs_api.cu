@@ -409,22 +409,24 @@ int tgs_render(tgs_ctx* c, int mode) {
   if (ftype == TGS_FRAME_S) {
     if (fork) { CK(cudaEventRecord(c->ev_fork2, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork2, 0)); }
     launch_fill_corr(fork ? c->side : s, fc, b);                                                           // A2
-    if (fork) CK(cudaEventRecord(c->ev_join2, c->side));
   }
   mark();                                                                      // 1: A3 preprocess, A4 selection
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
   if (ftype == TGS_FRAME_S) {
-    launch_mark_oc(s, fc, b, c->num_sms);                                                                  // A4: T^oc of larger rects
-    if (fork) CK(cudaStreamWaitEvent(s, c->ev_join2, 0));
-    launch_select(s, fc, b);                                                                               // A4: T_sel (R / P: all tiles, k_frame_init)
-    CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    CK(cudaEventRecord(c->ev_sel, s));
+    // A4 (T^oc of larger rects, T_sel) is only needed by the pair binning: it runs beside the depth sort
+    cudaStream_t s4 = fork ? c->side : s;
+    if (fork) { CK(cudaEventRecord(c->ev_fork, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0)); }
+    launch_mark_oc(s4, fc, b, c->num_sms);                                                                 // A4: T^oc of larger rects
+    launch_select(s4, fc, b);                                                                              // A4: T_sel (R / P: all tiles, k_frame_init)
+    CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s4));
+    CK(cudaEventRecord(c->ev_sel, s4));
     c->sel_pending = true;
   }
   mark();                                                                      // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // visible Gaussians by depth
   launch_fix_ties(s, b.ckeys[dsorted], b.cvals[dsorted], &b.counters->n_visible, c->num_sms);             // R28: equal depths by index
+  if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   mark();                                                                      // 3: A5 pairs
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
   mark();                                                                      // 4: A5 colours (beside the tile sort: only the blend needs them)
