@@ -191,9 +191,10 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
 //  phase A (all Gaussians, 16 B each): near cull, projection of the mean, AFC, TOC + newly-visible lookups in the
 //          warped TGB, and a conservative off-screen test; the survivors are compacted in shared memory;
 //  phase B (survivors only, +32 B each): EWA covariance, conic, radius, rect, records, T^oc marks of small rects;
-//  phase C: the visible Gaussians of the chunk are appended to the list the depth sort works on (one atomic per chunk:
-//          chunks land in arrival order, ascending index inside a chunk; k_fix_ties restores the index order of
-//          equal depths after the sort, so the final order does not depend on it).
+//  phase C: the visible Gaussians of the chunk go, compacted, to the chunk's own 1024 slots of a staging list, and the
+//          chunk's count to pre_cnt; the CTA that finishes last scans the counts; k_compact_vis then closes the gaps.
+//          The list the depth sort works on is thus in ascending index order (equal depths stay in index order
+//          through the stable sort, R28) and no chunk waits for another one.
 // SH (the bulk of the scene bytes) is not touched here at all.  Order of the tests and of every fp32 operation of a
 // decision: DESIGN.md §2 (O3), identical to what the oracle states.
 //
@@ -225,8 +226,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
                                                                uint32_t* __restrict__ vis_keys,
-                                                               uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ depth_hist,
-                                                               Counters* __restrict__ counters) {
+                                                               uint32_t* __restrict__ vis_vals, uint2* __restrict__ pre_cnt,
+                                                               uint32_t* __restrict__ depth_hist, Counters* __restrict__ counters) {
   __shared__ PreSmem sm;
   const CamConst& k = fc.cam;
   const float* V = k.V;
@@ -397,9 +398,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
     uint32_t off = vincl - nv_t, vtotal = 0;
 #pragma unroll
     for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < wid) off += t; vtotal += t; }
-    if (tid == 0) sm.excl = vtotal ? atomicAdd(&counters->n_visible, vtotal) : 0u;
-    __syncthreads();
-    off += sm.excl;
+    if (tid == 0) pre_cnt[chunk].x = vtotal;
+    off += base;                                             // staging slots of this chunk
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) {
       const uint32_t i = tid * PRE_IPT + j;
@@ -410,6 +410,28 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
         atomicAdd(&sm.hist[2][(key >> 16) & 255u], 1u); atomicAdd(&sm.hist[3][key >> 24], 1u);
       }
     }
+  }
+  // ---- the last CTA to arrive: exclusive scan of the chunks' visible counts (pre_cnt = {count, offset}), N_v
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) sm.excl = (atomicAdd(&counters->pre_done, 1u) == gridDim.x - 1u) ? 1u : 0u;
+  __syncthreads();
+  if (sm.excl) {
+    __threadfence();
+    const uint32_t per = (num_chunks + PRE_THREADS - 1) / PRE_THREADS;
+    const uint32_t c0 = tid * per, c1 = min(num_chunks, c0 + per);
+    uint32_t sum = 0;
+    for (uint32_t c = c0; c < c1; ++c) sum += *reinterpret_cast<volatile uint32_t*>(&pre_cnt[c].x);
+    uint32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
+    if (lane == 31) sm.warp[wid] = incl;
+    __syncthreads();
+    uint32_t off = incl - sum, tot = 0;
+    for (int w = 0; w < PRE_THREADS / 32; ++w) { if ((uint32_t)w < wid) off += sm.warp[w]; tot += sm.warp[w]; }
+    for (uint32_t c = c0; c < c1; ++c) { const uint32_t v = *reinterpret_cast<volatile uint32_t*>(&pre_cnt[c].x); pre_cnt[c].y = off; off += v; }
+    if (tid == 0) counters->n_visible = tot;
+    __syncthreads();
   }
   // statistics: one atomic per CTA and class
   st_near = warp_sum(st_near); st_afc = warp_sum(st_afc); st_toc = warp_sum(st_toc); st_deg = warp_sum(st_deg);
@@ -435,6 +457,20 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
     if (sm.stat[4]) atomicAdd(&counters->n_empty, sm.stat[4]);
     if (sm.stat[6]) atomicAdd(&counters->n_newly_visible, sm.stat[6]);
     if (sm.area) atomicAdd(&counters->area_sum, sm.area);
+  }
+}
+
+// Visible list: the chunks' runs from the staging list (1024 slots per chunk) to their offsets (ascending index order).
+__global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __restrict__ pre_cnt, const uint32_t* __restrict__ st_keys,
+                                                     const uint32_t* __restrict__ st_vals, uint32_t* __restrict__ vis_keys,
+                                                     uint32_t* __restrict__ vis_vals) {
+  const uint32_t num_chunks = (n + PRE_CHUNK - 1) / PRE_CHUNK;
+  for (uint32_t c = blockIdx.x; c < num_chunks; c += gridDim.x) {
+    const uint2 cc = pre_cnt[c];
+    for (uint32_t i = threadIdx.x; i < cc.x; i += blockDim.x) {
+      vis_keys[cc.y + i] = st_keys[(size_t)c * PRE_CHUNK + i];
+      vis_vals[cc.y + i] = st_vals[(size_t)c * PRE_CHUNK + i];
+    }
   }
 }
 
@@ -551,7 +587,8 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
   k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
-                                                       b.ckeys[0], b.cvals[0], b.sort_hist, b.counters);
+                                                       b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
+  k_compact_vis<<<num_sms * 8, 128, 0, s>>>(fc.n, b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0]);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

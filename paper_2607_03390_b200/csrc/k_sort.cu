@@ -198,29 +198,7 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
   }
 }
 
-// After a stable sort by key: items with equal keys in ascending value order (R28: equal depths by Gaussian index),
-// whatever order they had in the input.  Runs of equal depth bits are rare and short; one thread sorts a run.
-__global__ void __launch_bounds__(256) k_fix_ties(const uint32_t* __restrict__ keys, uint32_t* __restrict__ vals, const uint32_t* __restrict__ n_ptr) {
-  const uint32_t n = *n_ptr;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i + 1 < n; i += gridDim.x * blockDim.x) {
-    const uint32_t k = keys[i];
-    if (keys[i + 1] != k || (i > 0 && keys[i - 1] == k)) continue;       // not the first item of a run of >= 2
-    uint32_t e = i + 2;
-    while (e < n && keys[e] == k) ++e;
-    for (uint32_t a = i + 1; a < e; ++a) {                               // insertion sort of vals[i, e)
-      const uint32_t v = vals[a];
-      uint32_t b = a;
-      while (b > i && vals[b - 1] > v) { vals[b] = vals[b - 1]; --b; }
-      vals[b] = v;
-    }
-  }
-}
-
 }  // namespace
-
-void launch_fix_ties(cudaStream_t s, const uint32_t* keys, uint32_t* vals, const uint32_t* n_ptr, int num_sms) {
-  k_fix_ties<<<num_sms * 4, 256, 0, s>>>(keys, vals, n_ptr);
-}
 
 uint32_t sort_tile_items() { return SORT_TILE; }
 

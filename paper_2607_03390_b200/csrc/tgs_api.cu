@@ -268,8 +268,8 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
   A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_trect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
-  AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
-  A(b.ckeys[0], n) A(b.ckeys[1], n) A(b.cvals[0], n) A(b.cvals[1], n) A(b.nv_queue, n)
+  A(b.pre_cnt, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
+  A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
   AZ(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
 #undef A
@@ -425,7 +425,6 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // visible Gaussians by depth
-  launch_fix_ties(s, b.ckeys[dsorted], b.cvals[dsorted], &b.counters->n_visible, c->num_sms);             // R28: equal depths by index
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   mark();                                                                      // 3: A5 pairs
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts

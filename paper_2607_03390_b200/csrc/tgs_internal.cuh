@@ -51,7 +51,7 @@ struct Counters {
   // work tickets of the persistent kernels
   uint32_t ticket_pre, ticket_scan, ticket_bin, ticket_blend;
   uint32_t ticket_sort[8];  // [0..3] depth sort, [4..7] tile sort
-  uint32_t pad[1];
+  uint32_t pre_done;        // CTAs of k_preprocess that have finished
   unsigned long long area_sum;         // same as n_tests, accumulated in 64 bits by k_preprocess (overflow check)
   unsigned long long n_interactions;   // L (only when interaction counting is on)
   unsigned long long n_blended;        // interactions that passed alpha >= 1/255 and were composited (counting on)
@@ -79,9 +79,11 @@ struct DevBuffers {
   uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
-  // visible Gaussians: ckeys = bits(depth), cvals = index; [0] in index order (k_preprocess), sorted by the depth sort
+  // visible Gaussians: ckeys = bits(depth), cvals = index; [1] staging (1024 slots per chunk), [0] in index order
+  // (k_compact_vis), then ping-pong of the depth sort
   uint32_t* ckeys[2] = {nullptr, nullptr};   // [N]
   uint32_t* cvals[2] = {nullptr, nullptr};   // [N]
+  uint2* pre_cnt = nullptr;                  // [ceil(N/1024)] {visible Gaussians of a preprocess chunk, of the chunks before it}
   uint32_t* area_prefix = nullptr;           // [N+1] tests before each sorted visible Gaussian
   uint32_t* chunk_first = nullptr;           // [bin_chunks_cap] sorted position of the Gaussian holding a chunk's first test
   uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with rects of more than 4 tiles
@@ -126,7 +128,6 @@ void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sort
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms, bool small_input);
-void launch_fix_ties(cudaStream_t s, const uint32_t* keys, uint32_t* vals, const uint32_t* n_ptr, int num_sms);
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
