@@ -214,6 +214,32 @@ def test_edge_whole_screen_splats():
     P.compare_frame(g, o, sc.n, ora.FRAME_S)
 
 
+def test_edge_needles_faint_and_equal_depths():
+    """Paths that decide without the oracle's full sequence must never change a decision (R40): needle-like
+    splats (cond(Sigma') >> 400: no test-rect shrink), opacities around 1/255 (tau < 0.5 and tau < 0), off-screen
+    Gaussians of every size, and a slab of Gaussians at exactly the same depth (equal sort keys: order by index)."""
+    P = _p()
+    tgs = _tgs()
+    rng = np.random.default_rng(77)
+    sc = make_config(1, n=30_000, frames=2, width=333, height=207)
+    n = sc.n
+    sc.scales[: n // 3] = np.exp(rng.uniform(np.log(2e-4), np.log(0.8), size=(n // 3, 3))).astype(np.float32)   # needles / discs
+    sc.opacity[n // 3: n // 2] = rng.uniform(0.002, 0.012, size=n // 2 - n // 3).astype(np.float32)              # around 1/255
+    sc.means[n // 2: n // 2 + 4000, 2] = np.float32(0.25)                                                        # one depth for 4000
+    sc.means[-3000:] *= 4.0                                                                                      # far off screen
+    g, o = P.make_pair(sc)
+    V = look_at((0.0, 0.0, -6.0), (0, 0, 0), (0, 1, 0))                                                          # axis-aligned: equal z -> equal depth
+    g.set_camera(V, sc.camera); o.set_camera(V, sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, _ = P.compare_frame(g, o, n, ora.FRAME_R)
+    keys = o.get("keys")
+    assert (np.diff(keys) == 0).sum() > 1000            # equal (tile, depth) keys do occur: their order is by index
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[1], sc.camera); o.set_camera(sc.poses[1], sc.camera)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    P.compare_frame(g, o, n, ora.FRAME_S)
+
+
 def test_edge_capacity_overflow_and_errors():
     P = _p()
     tgs = _tgs()
