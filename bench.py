@@ -88,6 +88,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(ms, world, device=None):
+    """Replicas only: the job's time for K frames per rank is the slowest rank's device time."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_fps(world, steps, ms):
+    """Whole-job frames per second of `world` replicas that each rendered `steps` frames in `ms` (max over ranks)."""
+    return world * steps / (ms * 1e-3)
+
+
 def trajectory_pose(sc, f):
     """Frame f of an endless smooth trajectory: the config's poses played forward, then backward, ..."""
     F = len(sc.poses)
@@ -141,12 +157,7 @@ def run_ours(args):
                     ctx.read_image(readback)        # device -> pinned host, blocks until the frame is there
             e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
     sampler = ClockSampler(local)
     if rank == 0:
@@ -252,9 +263,7 @@ def run_ours(args):
             r["frac"] = r["achieved"] / r["peak"]
         roof = {"kernel": key, **r, "traffic": None, "ms_per_launch": float(t_stage[dom] * 1e3), "peak_note": f"{peak_kind} copy bandwidth"}
 
-    fps_tgs = world * K / (ms_tgs * 1e-3)
-    fps_full = world * K / (ms_full * 1e-3)
-    fps_e2e = world * K / (ms_e2e * 1e-3)
+    fps_tgs, fps_full, fps_e2e = aggregate_fps(world, K, ms_tgs), aggregate_fps(world, K, ms_full), aggregate_fps(world, K, ms_e2e)
     out = {
         "metric": METRIC, "value": fps_tgs, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_tgs / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
