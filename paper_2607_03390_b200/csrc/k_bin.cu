@@ -38,6 +38,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
                                                             const uint2* __restrict__ rec_rect, unsigned long long* __restrict__ desc,
                                                             uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
                                                             Counters* __restrict__ counters, unsigned long long max_tests) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   __shared__ uint32_t s_tile, s_warp[SCAN_THREADS / 32], s_excl;
   const uint32_t n = counters->n_visible;
   if (n == 0 || counters->area_sum > max_tests) {
@@ -191,6 +193,8 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
                                                      uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ keys,
                                                      uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
                                                      Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   __shared__ BinSmem sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
   const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
@@ -289,6 +293,8 @@ template <int DEG>
 __global__ void __launch_bounds__(128) k_colour(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ tiles_touched,
                                                 const float4* __restrict__ cull4, const float* __restrict__ sh,
                                                 float4* __restrict__ rec_rgb, const Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   const uint32_t n = counters->n_visible;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const uint32_t g = sorted_g[i];
@@ -299,6 +305,8 @@ __global__ void __launch_bounds__(128) k_colour(FrameConst fc, const uint32_t* _
 // ================================================================== A7: per-tile ranges
 __global__ void __launch_bounds__(256) k_ranges(const uint32_t* __restrict__ keys, const Counters* __restrict__ counters,
                                                 uint2* __restrict__ ranges, int n_tiles) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   const uint32_t n = counters->n_pairs;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const uint32_t t = keys[i];
@@ -330,15 +338,15 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
   const uint32_t* sorted_g = b.cvals[sorted_g_idx];
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
-  k_scan_area<<<grid ? grid : 1, SCAN_THREADS, 0, s>>>(fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
+  TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
                                                       b.counters, max_tests);
-  k_bin<<<num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s>>>(fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
+  TGS_LAUNCH((k_bin), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
                                                           (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
 }
 
 void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms) {
   const uint32_t* sorted_g = b.cvals[sorted_g_idx];
-#define LAUNCH(D) k_colour<D><<<num_sms * 16, 128, 0, s>>>(fc, sorted_g, b.tiles_touched, b.cull4, b.sh, b.rec_rgb, b.counters)
+#define LAUNCH(D) TGS_LAUNCH((k_colour<D>), num_sms * 16, 128, 0, s, fc, sorted_g, b.tiles_touched, b.cull4, b.sh, b.rec_rgb, b.counters)
   switch (fc.sh_degree) {
     case 0: LAUNCH(0); break;
     case 1: LAUNCH(1); break;
@@ -349,7 +357,7 @@ void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sort
 }
 
 void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms) {
-  k_ranges<<<num_sms * 8, 256, 0, s>>>(b.keys[sorted_idx], b.counters, b.ranges, fc.n_tiles);
+  TGS_LAUNCH((k_ranges), num_sms * 8, 256, 0, s, b.keys[sorted_idx], b.counters, b.ranges, fc.n_tiles);
 }
 
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out) {

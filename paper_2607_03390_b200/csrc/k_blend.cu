@@ -102,6 +102,8 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
                                                          const float* __restrict__ fill_depth, const float* __restrict__ warp_sigma,
                                                          float* __restrict__ image, float* __restrict__ depth, float* __restrict__ sigma,
                                                          uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   __shared__ BlendSmem sm;
   const CamConst& k = fc.cam;
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -360,7 +362,7 @@ void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorte
                   uint8_t* rendered_next, int num_sms, bool count_interactions) {
   const int grid = num_sms * 12;
 #define LAUNCH(M, C)                                                                                                          \
-  k_blend<M, C><<<grid, BLEND_THREADS, 0, s>>>(fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
+  TGS_LAUNCH((k_blend<M, C>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \
                                                b.sigma[out_idx], rendered_next, b.counters)
   if (rendered_next) { if (count_interactions) LAUNCH(true, true); else LAUNCH(true, false); }

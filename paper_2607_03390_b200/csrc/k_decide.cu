@@ -61,6 +61,8 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
                                                     uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
                                                     uint4* tiles_touched4, uint32_t n_tt4, uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
                                                     uint32_t* F_key, int reset_F) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
   // R / P frames select every tile and carry no T^oc / T^um flags: the outputs of k_select are written here
   const bool trivial_sel = fc.ftype != TGS_FRAME_S;
@@ -87,6 +89,7 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
 __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __restrict__ prior_depth,
                                               const float* __restrict__ prior_sigma, uint32_t* __restrict__ warp_depth,
                                               uint32_t* __restrict__ warp_sigma) {
+  TGS_PDL_WAIT();
   const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
   const CamConst& k = fc.cam;
   if (x >= k.W || y >= k.H) return;
@@ -114,6 +117,7 @@ __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __rest
 // is inside the image (R20).  Tile in T^um <=> any in-image pixel unmatched (R22).
 __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* __restrict__ warp_depth, float* __restrict__ fill_depth,
                                                    uint32_t* __restrict__ tile_flags) {
+  TGS_PDL_WAIT();
   const CamConst& k = fc.cam;
   const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
   const int x = blockIdx.x * TGS_TILE + lx, y = blockIdx.y * TGS_TILE + ly;
@@ -170,6 +174,8 @@ __device__ __forceinline__ void mark_oc_tile(const CamConst& k, float u, float v
 __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_uvdo,
                                                  const float4* __restrict__ rec_conic, const uint2* __restrict__ rec_rect,
                                                  uint32_t* __restrict__ tile_flags, Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   const CamConst& k = fc.cam;
   const uint32_t nq = counters->n_nv_queue;
   for (uint32_t j = blockIdx.x; j < nq; j += gridDim.x) {
@@ -228,6 +234,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
                                                                uint32_t* __restrict__ vis_keys,
                                                                uint32_t* __restrict__ vis_vals, uint2* __restrict__ pre_cnt,
                                                                uint32_t* __restrict__ depth_hist, Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   __shared__ PreSmem sm;
   const CamConst& k = fc.cam;
   const float* V = k.V;
@@ -464,6 +472,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
 __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __restrict__ pre_cnt, const uint32_t* __restrict__ st_keys,
                                                      const uint32_t* __restrict__ st_vals, uint32_t* __restrict__ vis_keys,
                                                      uint32_t* __restrict__ vis_vals) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   const uint32_t num_chunks = (n + PRE_CHUNK - 1) / PRE_CHUNK;
   for (uint32_t c = blockIdx.x; c < num_chunks; c += gridDim.x) {
     const uint2 cc = pre_cnt[c];
@@ -481,6 +491,8 @@ __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __
 __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* __restrict__ tile_flags, uint8_t* __restrict__ tile_mask,
                                                  uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tile_order,
                                                  Counters* __restrict__ counters) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   __shared__ uint32_t s_sel[32], s_oc[32], s_um[32];
   const int T = fc.n_tiles;
   const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -524,6 +536,8 @@ __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* 
 __global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint32_t* __restrict__ vis_vals, const uint8_t* __restrict__ rendered_now,
                                                  const float4* __restrict__ rec_uvdo, uint32_t* __restrict__ F_key,
                                                  Counters* __restrict__ counters, int update_F) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   uint32_t kmin_x = 0xffffffffu, kmin_y = 0xffffffffu, kmax_x = 0, kmax_y = 0, cnt = 0;
   const uint32_t nv = counters->n_visible;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += gridDim.x * blockDim.x) {
@@ -567,38 +581,38 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
-  k_frame_init<<<592, 256, 0, s>>>(fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
+  TGS_LAUNCH((k_frame_init), 592, 256, 0, s, fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
                                    (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
                                    b.F_key, reset_F ? 1 : 0);
 }
 
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma) {
   dim3 grid((fc.cam.W + 31) / 32, (fc.cam.H + 7) / 8);
-  k_warp<<<grid, 256, 0, s>>>(fc, prior_depth, prior_sigma, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma);
+  TGS_LAUNCH((k_warp), grid, 256, 0, s, fc, prior_depth, prior_sigma, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma);
 }
 
 void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   dim3 grid(fc.cam.TX, fc.cam.TY);
-  k_fill_corr<<<grid, 256, 0, s>>>(fc, b.warp_depth, b.fill_depth, b.tile_flags);
+  TGS_LAUNCH((k_fill_corr), grid, 256, 0, s, fc, b.warp_depth, b.fill_depth, b.tile_flags);
 }
 
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
-  k_preprocess<<<grid ? grid : 1, PRE_THREADS, 0, s>>>(fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
+  TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
-  k_compact_vis<<<num_sms * 8, 128, 0, s>>>(fc.n, b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0]);
+  TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0]);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-  k_mark_oc<<<num_sms * 8, 128, 0, s>>>(fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_trect, b.tile_flags, b.counters);
+  TGS_LAUNCH((k_mark_oc), num_sms * 8, 128, 0, s, fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_trect, b.tile_flags, b.counters);
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
-  k_select<<<1, 1024, 0, s>>>(fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters);
+  TGS_LAUNCH((k_select), 1, 1024, 0, s, fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters);
 }
 
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F) {
-  k_frustum<<<296, 256, 0, s>>>(fc, vis_vals, rendered_now, b.rec_uvdo, b.F_key, b.counters, update_F ? 1 : 0);
+  TGS_LAUNCH((k_frustum), 296, 256, 0, s, fc, vis_vals, rendered_now, b.rec_uvdo, b.F_key, b.counters, update_F ? 1 : 0);
 }

@@ -48,6 +48,8 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ n_ptr, uint32_t* __restrict__ ticket, uint32_t* __restrict__ error_flag,
     const uint32_t* __restrict__ hist, unsigned long long* __restrict__ desc, int shift, int nbits, uint32_t epoch) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& sm = *reinterpret_cast<SortSmem*>(smem_raw);
   const uint32_t n = *n_ptr;
@@ -226,10 +228,10 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
     const int nbits = key_bits - 8 * p < 8 ? key_bits - 8 * p : 8;
     unsigned long long* d = (unsigned long long*)desc + (size_t)p * tiles_cap * RADIX;
     if (small_input)
-      k_onesweep<32, 2><<<num_sms * 2, SORT_THREADS, sizeof(SortSmem), s>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
+      TGS_LAUNCH((k_onesweep<32, 2>), num_sms * 2, SORT_THREADS, sizeof(SortSmem), s, keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
                                                                            error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
     else
-      k_onesweep<4, SORT_CTAS_PER_SM><<<num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s>>>(
+      TGS_LAUNCH((k_onesweep<4, SORT_CTAS_PER_SM>), num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem), s, 
           keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
     cur ^= 1;
   }

@@ -112,6 +112,30 @@ struct DevBuffers {
   Counters* counters = nullptr;
 };
 
+// ------------------------------------------------------------------ programmatic dependent launch (sm_90+)
+// Every kernel of a frame is launched with programmatic stream serialization: its CTAs may be scheduled while the
+// previous kernel of the stream drains, and wait in TGS_PDL_WAIT() (griddepcontrol.wait: the previous grid has completed
+// and its writes are visible) before they touch anything a predecessor produced.  Persistent kernels, whose grid is
+// resident from the start, call TGS_PDL_TRIGGER() at once so that the next grid is launched as their CTAs retire.
+#define TGS_PDL_WAIT() asm volatile("griddepcontrol.wait;" ::: "memory")
+#define TGS_PDL_TRIGGER() asm volatile("griddepcontrol.launch_dependents;" ::: "memory")
+struct PdlLaunch {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute at;
+  PdlLaunch(dim3 grid, dim3 block, size_t smem, cudaStream_t s) {
+    cfg = cudaLaunchConfig_t();
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at; cfg.numAttrs = 1;
+  }
+};
+#define TGS_LAUNCH(kernel, grid, block, smem, stream, ...)   \
+  do {                                                       \
+    PdlLaunch L_(grid, block, smem, stream);                 \
+    cudaLaunchKernelEx(&L_.cfg, kernel, __VA_ARGS__);        \
+  } while (0)
+
 // ------------------------------------------------------------------ launchers (definitions in k_*.cu)
 void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const float* scales, const float* quats,
                    const float* opacity, const float* sh, DevBuffers& b);
