@@ -293,6 +293,70 @@ def run_ours(args):
     return out
 
 
+# ---------------------------------------------------------------------------------------------- ablation
+def run_ablation(args):
+    """Leave-one-out / one-at-a-time ablation of AFC, TOC and SR (the shape of the paper's Table IV) and the
+    eta / lambda_SR sensitivity (Table VI) on the synthetic trajectory: FPS over `steps` frames of the AUTO
+    schedule and PSNR of the S frames against the full render of the same pose.  Single GPU; prints one JSON line."""
+    import torch
+    from paper_2607_03390_b200 import build as tgs_build
+    from synth import make_config
+    tgs_build.build()
+    from paper_2607_03390_b200 import tgs
+    torch.cuda.set_device(0)
+    sc = make_config(args.config, n=args.n, frames=None)
+    stream = torch.cuda.Stream()
+    ctx, ref = tgs.Context(0, stream.cuda_stream), tgs.Context(0, stream.cuda_stream)
+    ctx.load_scene(sc); ref.load_scene(sc)
+    cam, K, W = sc.camera, args.steps, max(args.warmup, 3)
+
+    def variant(**kw):
+        prm = ctx.default_params()
+        for k, v in kw.items():
+            setattr(prm, k, v)
+        ctx.set_params(prm)
+        ctx.reset_priors()
+        for f in range(W):
+            ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+        ctx.reset_priors()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for f in range(K):
+                ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        fps = K / (e0.elapsed_time(e1) * 1e-3)
+        ctx.reset_priors()
+        psnr, types, sel = [], [], []
+        for f in range(min(K, 40)):
+            ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+            st = ctx.get_stats()
+            types.append("RPS"[st["frame_type"]])
+            if st["frame_type"] == tgs.FRAME_S:
+                sel.append(st["n_sel"] / st["n_tiles"])
+                ref.set_camera(trajectory_pose(sc, f), cam); ref.render(tgs.FULL)
+                mse = float(((ctx.read_image() - ref.read_image()) ** 2).mean())
+                psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
+        return {"fps": fps, "psnr_S_vs_full_dB": float(np.mean(psnr)) if psnr else None, "tgsf": types.count("S") / len(types),
+                "mean_selected_fraction": float(np.mean(sel)) if sel else None}
+
+    rows = {
+        "full_render (lambda_sr=1)": variant(lambda_sr=1, lambda_tdc=1),
+        "AFC only": variant(enable_afc=1, enable_toc=0, enable_sr=0),
+        "TOC only": variant(enable_afc=0, enable_toc=1, enable_sr=0),
+        "SR only": variant(enable_afc=0, enable_toc=0, enable_sr=1),
+        "AFC+TOC (TDC)": variant(enable_sr=0),
+        "TemporalGS (all)": variant(),
+        "eta=0.2": variant(eta=0.2), "eta=0.6": variant(eta=0.6),
+        "lambda_sr=2": variant(lambda_sr=2), "lambda_sr=10": variant(lambda_sr=10),
+        "lambda_tdc=25": variant(lambda_tdc=25), "lambda_tdc=75": variant(lambda_tdc=75),
+    }
+    return {"metric": "ablation: FPS / PSNR(S vs full) / share of S frames per variant", "config": {"workload": f"config {args.config} ({sc.name})"},
+            "steps": K, "warmup": W, "data": "synthetic", "ablation": rows}
+
+
 # ---------------------------------------------------------------------------------------------- CPU oracle legs
 def oracle_sample(config, n, frames_modes, budget_s=None):
     """Time the oracle, as it stands, on the given (frame index, mode) list of the config's trajectory."""
@@ -373,12 +437,16 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the number of Gaussians (debug only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ablation", action="store_true", help="module ablation and sensitivity table instead of the bench line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         out = run_reference(args)
         if out is not None:
             print(json.dumps(out))
+        return
+    if args.ablation:
+        print(json.dumps(run_ablation(args)))
         return
     out = run_ours(args)
     if out is None:
