@@ -633,7 +633,9 @@ int ora_render(ora_ctx* c, int mode) {
   if (ftype != ORA_FRAME_S) commit_priors(c, ftype);
   const double t4 = now_ms();
   c->st.ms_temporal = t1 - t0; c->st.ms_preprocess = t2 - t1; c->st.ms_sort = t3 - t2; c->st.ms_blend = t4 - t3; c->st.ms_total = t4 - t0;
-  ora_schedule_feedback(&c->sched, ftype, c->st.n_sel, c->st.n_tiles, c->prm.eta);
+  // R41: the eta rule is part of selective rendering (section III-E); with SR switched off no tile is
+  // "selected" by the method, so an S frame never forces a pseudo-reference frame.
+  ora_schedule_feedback(&c->sched, ftype, c->prm.enable_sr ? c->st.n_sel : 0u, c->st.n_tiles, c->prm.eta);
   return ftype;
 }
 

@@ -336,7 +336,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   // ---- A0: frame type (R9, R23)
   if (c->sel_pending) {   // eta rule needs the selected-tile count of the previous S frame
     CK(cudaEventSynchronize(c->ev_sel));
-    c->sched.force_P = ((float)c->h_sel[0] > c->prm.eta * (float)c->last_n_tiles) ? 1 : 0;
+    c->sched.force_P = (c->prm.enable_sr && (float)c->h_sel[0] > c->prm.eta * (float)c->last_n_tiles) ? 1 : 0;   // L128; R41: only with SR on
     c->sel_pending = false;
   }
   int ftype;

@@ -163,6 +163,24 @@ def test_auto_schedule_matches_oracle():
     assert ora.FRAME_P in types_g and ora.FRAME_S in types_g and types_g[0] == ora.FRAME_R and types_g[9] == ora.FRAME_R
 
 
+def test_auto_schedule_without_selective_rendering():
+    """R41: with SR off an S frame renders every tile but never forces a P frame (the eta rule belongs to SR)."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=4000, frames=8)
+    g, o = P.make_pair(sc, {"lambda_tdc": 10, "lambda_sr": 5, "enable_sr": 0})
+    types_g, types_o = [], []
+    for f in range(10):
+        V = sc.poses[f % len(sc.poses)]
+        g.set_camera(V, sc.camera); o.set_camera(V, sc.camera)
+        g.render(tgs.AUTO); types_o.append(o.render(ora.AUTO))
+        sg = g.get_stats()
+        types_g.append(sg["frame_type"])
+        assert sg["n_sel"] == sg["n_tiles"]
+    R, Pf, S = ora.FRAME_R, ora.FRAME_P, ora.FRAME_S
+    assert types_g == types_o == [R, S, S, S, S, Pf, S, S, S, S]
+
+
 # ------------------------------------------------------------------------------------------------ edge cases
 def test_edge_empty_frame_and_single_gaussian():
     P = _p()

@@ -673,3 +673,24 @@ def test_p11_eta_forces_pseudo_reference():
         L.ora_schedule_feedback(s, t, sel.get(f, 5), 100, 0.40)
     R, P, S = ora.FRAME_R, ora.FRAME_P, ora.FRAME_S
     assert seq == [R, S, S, P, S, S, S, S]                          # since_ref restarts at the forced P (R23)
+
+
+def test_r41_eta_rule_only_with_selective_rendering():
+    """With SR switched off every tile is rendered on an S frame (n_sel = T > eta T), yet no P frame is forced: the
+    eta rule is part of selective rendering.  The share of S frames is then (lambda_SR - 1)/lambda_SR,
+    the value Table VI prints for lambda_SR = 5 (80.00 %, L268)."""
+    sc = make_config(1, n=2000, frames=8, width=64, height=48)
+    types = {}
+    for sr in (0, 1):
+        o = Oracle()
+        o.load_scene(sc)
+        p = o.default_params(); p.enable_sr = sr; p.lambda_tdc = 10; p.lambda_sr = 5
+        o.set_params(p)
+        seq = []
+        for f in range(10):
+            o.set_camera(sc.poses[f % len(sc.poses)], sc.camera)
+            seq.append(o.render(ora.AUTO))
+        types[sr] = seq
+    R, P, S = ora.FRAME_R, ora.FRAME_P, ora.FRAME_S
+    assert types[0] == [R, S, S, S, S, P, S, S, S, S]               # 80 % S frames
+    assert types[1][:4] == [R, S, P, S]                             # sparse cloud: every tile unmatched -> forced P (DESIGN.md §4)
