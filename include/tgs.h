@@ -121,6 +121,13 @@ int tgs_render(tgs_ctx*, int mode);
 /* Current frame.  rgb [H][W][3] in [0,1] (+bg); depth [H][W] (Eq.1; stitched on S frames, R31);
  * sigma [H][W] (Eq.2), nullable; sel [TY][TX]: bit0 = T^oc (L119), bit1 = T^um (L121), bit2 = selected. */
 int tgs_read_image(tgs_ctx*, float* rgb, int mem);
+/* Streaming read-back for frame loops: enqueues the copy of the current frame's image to `rgb_host` (page-locked
+ * host memory, [H][W][3]) on a copy stream of the context and returns at once, so the transfer overlaps the rendering
+ * of the following frames (a later frame that would overwrite the device buffer waits for the copy by itself).  The
+ * data are valid only after tgs_wait_reads, which blocks until every enqueued read has finished; the other blocking
+ * calls do not imply it.  The caller keeps `rgb_host` alive and untouched until then. */
+int tgs_read_image_async(tgs_ctx*, float* rgb_host);
+int tgs_wait_reads(tgs_ctx*);
 int tgs_read_depth(tgs_ctx*, float* depth, float* sigma, int mem);
 int tgs_read_tile_mask(tgs_ctx*, uint8_t* sel, int mem);
 int tgs_get_stats(tgs_ctx*, tgs_stats* out);

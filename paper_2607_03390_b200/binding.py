@@ -21,7 +21,7 @@ CULL_NEAR, CULL_AFC, CULL_TOC, CULL_DEGENERATE, CULL_EMPTY, VISIBLE, NEWLY_VISIB
 DEPTH_INVALID = np.float32(3.0e38)
 
 EXPORTS = ["tgs_create", "tgs_destroy", "tgs_load_gaussians", "tgs_set_camera", "tgs_default_params", "tgs_set_params",
-           "tgs_render", "tgs_read_image", "tgs_read_depth", "tgs_read_tile_mask", "tgs_get_stats", "tgs_reset_priors",
+           "tgs_render", "tgs_read_image", "tgs_read_image_async", "tgs_wait_reads", "tgs_read_depth", "tgs_read_tile_mask", "tgs_get_stats", "tgs_reset_priors",
            "tgs_strerror", "tgs_last_error", "tgs_debug_get", "tgs_debug_put", "tgs_debug_run_stage"]
 
 
@@ -77,6 +77,8 @@ def lib():
         L.tgs_set_params.argtypes = [vp, C.POINTER(TgsParams)]
         L.tgs_render.argtypes = [vp, C.c_int]
         L.tgs_read_image.argtypes = [vp, vp, C.c_int]
+        L.tgs_read_image_async.argtypes = [vp, vp]
+        L.tgs_wait_reads.argtypes = [vp]
         L.tgs_read_depth.argtypes = [vp, vp, vp, C.c_int]
         L.tgs_read_tile_mask.argtypes = [vp, vp, C.c_int]
         L.tgs_get_stats.argtypes = [vp, C.POINTER(TgsStats)]
@@ -188,6 +190,14 @@ class Context:
         p, m = _ptr_mem(out)
         self._chk(self.L.tgs_read_image(self.h, C.c_void_p(p), m), "tgs_read_image")
         return out
+
+    def read_image_async(self, out):
+        """`out`: page-locked host array [H][W][3] float32; valid after wait_reads()."""
+        assert out.dtype == np.float32 and out.flags["C_CONTIGUOUS"] and out.size == self.H * self.W * 3
+        self._chk(self.L.tgs_read_image_async(self.h, C.c_void_p(out.ctypes.data)), "tgs_read_image_async")
+
+    def wait_reads(self):
+        self._chk(self.L.tgs_wait_reads(self.h), "tgs_wait_reads")
 
     def read_depth(self, depth=None, sigma=None):
         if depth is None:

@@ -53,6 +53,9 @@ struct tgs_ctx {
   Counters* h_counters = nullptr;      // pinned
   uint32_t* h_sel = nullptr;           // pinned: n_sel of the last S frame (for the eta rule)
   cudaEvent_t ev_sel = nullptr, ev_done = nullptr;
+  cudaStream_t copy = nullptr;          // read-back stream of tgs_read_image_async
+  cudaEvent_t ev_copy[2] = {nullptr, nullptr};   // last asynchronous read of image[i] has finished
+  bool copy_pending[2] = {false, false};
   cudaStream_t side = nullptr;          // second stream: work that is off the critical path of a frame (SH colours, A2)
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr;
   bool sel_pending = false;
@@ -230,6 +233,8 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
   cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
+  cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking);
+  for (auto& e : c->ev_copy) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
   for (cudaEvent_t* e : {&c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2}) cudaEventCreateWithFlags(e, cudaEventDisableTiming);
   for (auto& e : c->ev_stage) cudaEventCreate(&e);
   *out = c;
@@ -245,6 +250,8 @@ void tgs_destroy(tgs_ctx* c) {
   cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
   cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
   cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
+  cudaStreamSynchronize(c->copy); cudaStreamDestroy(c->copy);
+  for (auto& e : c->ev_copy) cudaEventDestroy(e);
   for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_fork2, c->ev_join2}) cudaEventDestroy(e);
   for (auto& e : c->ev_stage) cudaEventDestroy(e);
   delete c;
@@ -438,6 +445,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
   mark();                                                                      // 6: A8 + A9
   if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
+  if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
   launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);
   mark();                                                                      // 7: post
   if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
@@ -465,6 +473,24 @@ int tgs_render(tgs_ctx* c, int mode) {
 int tgs_read_image(tgs_ctx* c, float* rgb, int mem) {
   if (!c || !rgb || !c->have_frame) return TGS_E_INVALID_ARG;
   return copy_out(c, rgb, c->b.image[c->cur_idx], (size_t)c->W * c->H * 3 * sizeof(float), mem);
+}
+
+int tgs_read_image_async(tgs_ctx* c, float* rgb_host) {
+  if (!c || !rgb_host || !c->have_frame) return TGS_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamWaitEvent(c->copy, c->ev_done, 0));                     // the frame is complete
+  CK(cudaMemcpyAsync(rgb_host, c->b.image[c->cur_idx], (size_t)c->W * c->H * 3 * sizeof(float), cudaMemcpyDeviceToHost, c->copy));
+  CK(cudaEventRecord(c->ev_copy[c->cur_idx], c->copy));
+  c->copy_pending[c->cur_idx] = true;
+  return TGS_OK;
+}
+
+int tgs_wait_reads(tgs_ctx* c) {
+  if (!c) return TGS_E_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->copy));
+  c->copy_pending[0] = c->copy_pending[1] = false;
+  return TGS_OK;
 }
 
 int tgs_read_depth(tgs_ctx* c, float* depth, float* sigma, int mem) {

@@ -303,6 +303,29 @@ def test_device_pointers_and_torch_stream():
     assert np.abs(img.cpu().numpy() - o.read_image()).max() < 1.2e-2
 
 
+def test_async_readback_matches_blocking_read():
+    """tgs_read_image_async over a run of R / S / P frames (S frames reuse one device buffer: the next frame must wait
+    for the pending copy) returns the same images as the blocking read."""
+    import torch
+    tgs = _tgs()
+    sc = make_config(1, n=6000, frames=8)
+    a, b = tgs.Context(0), tgs.Context(0)
+    for c in (a, b):
+        c.load_scene(sc)
+        p = c.default_params(); p.lambda_sr = 3; p.eta = 2.0      # R S S P S S P ...
+        c.set_params(p)
+    bufs = [torch.empty((sc.camera.H, sc.camera.W, 3), dtype=torch.float32).pin_memory() for _ in range(len(sc.poses))]
+    ref = []
+    for f, V in enumerate(sc.poses):
+        a.set_camera(V, sc.camera); a.render(tgs.AUTO); a.read_image_async(bufs[f].numpy())
+        b.set_camera(V, sc.camera); b.render(tgs.AUTO); ref.append(b.read_image().copy())
+    a.wait_reads()
+    types = []
+    for f in range(len(sc.poses)):
+        assert np.array_equal(bufs[f].numpy(), ref[f]), f
+    assert b.get_stats()["frame_type"] in (tgs.FRAME_S, tgs.FRAME_P)
+
+
 # ------------------------------------------------------------------------------------------------ full size
 def test_full_size_config3_reference_and_temporal():
     """BASELINE.json config 3 (3 M Gaussians, SH 3, 1920x1080) in the launch configuration bench.py times: one
