@@ -24,6 +24,8 @@ namespace {
 constexpr int BLEND_THREADS = 64;      // 16 rows x 4 runs of 4 pixels
 constexpr int BLEND_BATCH = 128;
 constexpr int PPT = 4;                 // pixels per thread (dense mode)
+constexpr int DENSE_GROUP = 8;         // records between two "whole warp finished" tests of the dense loop (divides BLEND_BATCH)
+constexpr int DENSE_UNROLL = 8;
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
 // log2(1/255) = -7.99435...; anything below this bound (with a safety gap far above the rounding of e and of
 // ex2.approx) has alpha < 1/255 for sure, so the exact test on alpha is only evaluated near or above the threshold
@@ -196,6 +198,11 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
           cp_async16(&B.a[j], rec_b0 + gid[s]); cp_async16(&B.b[j], rec_b1 + gid[s]); cp_async16(&B.c[j], rec_rgb + gid[s]);
           B.id[j] = gid[s];
           if (MARK) B.contrib[j] = 0;
+        } else {
+          // padding behind the end of the list: log2 o = -inf gives alpha = 0 at every pixel, so the dense loop can run
+          // in whole groups of DENSE_GROUP records without a bound check per record
+          B.a[j] = make_float4(0.0f, 0.0f, 0.0f, 0.0f); B.b[j] = make_float4(0.0f, -INFINITY, 0.0f, 0.0f);
+          B.c[j] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         }
       }
       cp_async_commit();
@@ -273,12 +280,14 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
           // branch-free: 85 % of the interactions of an alive pixel composite, so every pixel runs the whole update with
           // alpha forced to 0 where it is skipped (alpha < 1/255), stops (T (1 - alpha) < 1e-4) or is finished
           const float2 one2 = make_float2(1.0f, 1.0f), neg2 = make_float2(-1.0f, -1.0f);
-#pragma unroll 2
-          for (uint32_t j = 0; j < cnt; ++j) {
+          for (uint32_t j0 = 0; j0 < cnt; j0 += DENSE_GROUP) {
+#pragma unroll(DENSE_UNROLL)
+           for (uint32_t jj = 0; jj < DENSE_GROUP; ++jj) {
+            const uint32_t j = j0 + jj;
             const float4 ga = B.a[j];
             const float4 gb = B.b[j];
             const float4 gc = B.c[j];
-            if (COUNT) {
+            if (COUNT && j < cnt) {
               nslot += PPT;
               nint += (uint32_t)(T2[0].x > 0.0f) + (uint32_t)(T2[0].y > 0.0f) + (uint32_t)(T2[1].x > 0.0f) + (uint32_t)(T2[1].y > 0.0f);
             }
@@ -313,7 +322,8 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
               S22[q] = __ffma2_rn(__fmul2_rn(wgt, dd), dd, S22[q]);
             }
             if (MARK && wsum.x + wsum.y > 0.0f) Bw.contrib[j] = 1;
-            if ((j & 7u) == 7u && __all_sync(0xffffffffu, fmaxf(fmaxf(T2[0].x, T2[0].y), fmaxf(T2[1].x, T2[1].y)) < 0.0f)) break;
+           }
+           if (__all_sync(0xffffffffu, fmaxf(fmaxf(T2[0].x, T2[0].y), fmaxf(T2[1].x, T2[1].y)) < 0.0f)) break;
           }
         }
       } else if (__any_sync(0xffffffffu, salive)) {
