@@ -72,7 +72,13 @@ typedef struct {
   int exact_tiles;        /* 1 (default, R39): a Gaussian "intersects" a tile (L61) iff its max alpha over the tile's pixel
                              box is >= 1/255 -- the test L119 uses for tile contributions; 0: every tile of the 3-sigma
                              rect.  Images, TGB and G_rendered do not depend on it, only the pair lists get shorter. */
+  int prior_policy;       /* TGS_PRIORS_ANCHORED (default; the paper, L86: S frames always warp from the last R / P frame) or
+                             TGS_PRIORS_CHAINED (R42): the stitched {I, D, sigma} of every S frame replace the priors and
+                             G_rendered grows by the Gaussians that frame blended */
+  int tgb_downscale;      /* 1 (default) or 2: the TGB is warped, repaired and looked up on a ceil(W/2) x ceil(H/2) grid,
+                             the paper's setting for large scenes (L142); downscale = min depth / max sigma of 2x2 (R43) */
 } tgs_params;
+enum { TGS_PRIORS_ANCHORED = 0, TGS_PRIORS_CHAINED = 1 };
 
 typedef struct {
   int frame_type; /* TGS_FRAME_R / P / S */

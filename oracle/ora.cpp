@@ -507,6 +507,16 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
   (void)ftype;
 }
 
+// R42, prior_policy = CHAINED (north_star: "the new frame ... becomes the next frame's TGB/TAB"): after an S frame
+// its stitched image, depth and sigma (Eq.4, R31) replace TAB and TGB, W_t becomes this frame's pose, and
+// G_rendered (L103) grows by the Gaussians blended in the selected tiles -- the un-rendered tiles show the same
+// surfaces as before, so their contributors stay members.  F (L109) stays the reference frame's.
+void commit_chained(ora_ctx* c) {
+  c->prior_image = c->image; c->prior_depth = c->depth; c->prior_sigma = c->sigma;
+  for (uint32_t g = 0; g < c->n; ++g) c->rendered[g] = c->rendered[g] | c->rendered_now[g];
+  std::memcpy(c->prior_view, c->cam.V, sizeof(c->prior_view));
+}
+
 // after an R / P frame the outputs become the priors (O2, A10); R also stores F (L109, R8)
 void commit_priors(ora_ctx* c, int ftype) {
   c->prior_image = c->image; c->prior_depth = c->depth; c->prior_sigma = c->sigma;
@@ -534,6 +544,7 @@ extern "C" {
 void ora_default_params(ora_params* p) {
   p->lambda1 = 3.0f; p->lambda2 = 0.0f; p->lambda_tdc = 50; p->lambda_sr = 5; p->eta = 0.40f;
   p->bg[0] = p->bg[1] = p->bg[2] = 0.0f; p->enable_afc = p->enable_toc = p->enable_sr = 1; p->exact_tiles = 1;
+  p->prior_policy = 0; p->tgb_downscale = 1;
 }
 
 ora_ctx* ora_create(void) { ora_ctx* c = new ora_ctx(); ora_default_params(&c->prm); return c; }
@@ -631,6 +642,7 @@ int ora_render(ora_ctx* c, int mode) {
   const double t3 = now_ms();
   blend_and_stitch(c, ftype);
   if (ftype != ORA_FRAME_S) commit_priors(c, ftype);
+  else if (c->prm.prior_policy == 1) commit_chained(c);
   const double t4 = now_ms();
   c->st.ms_temporal = t1 - t0; c->st.ms_preprocess = t2 - t1; c->st.ms_sort = t3 - t2; c->st.ms_blend = t4 - t3; c->st.ms_total = t4 - t0;
   // R41: the eta rule is part of selective rendering (section III-E); with SR switched off no tile is
@@ -668,7 +680,7 @@ long long ora_get(ora_ctx* c, const char* nm, void* dst, size_t bytes) {
   const std::string name(nm);
   ORA_GET("records", c->rec) ORA_GET("keys", c->keys) ORA_GET("vals", c->vals) ORA_GET("ranges", c->ranges)
   ORA_GET("warp_depth", c->warp_depth) ORA_GET("warp_sigma", c->warp_sigma) ORA_GET("fill_depth", c->fill_depth)
-  ORA_GET("corr_xy", c->corr_xy) ORA_GET("matched", c->matched) ORA_GET("rendered", c->rendered)
+  ORA_GET("corr_xy", c->corr_xy) ORA_GET("matched", c->matched) ORA_GET("rendered", c->rendered) ORA_GET("rendered_now", c->rendered_now)
   ORA_GET("rendered_sure", c->rendered_sure) ORA_GET("rendered_maybe", c->rendered_maybe) ORA_GET("borderline", c->borderline)
   ORA_GET("prior_depth", c->prior_depth) ORA_GET("prior_sigma", c->prior_sigma) ORA_GET("prior_image", c->prior_image)
   ORA_GET("cov3d", c->cov3d) ORA_GET("tau", c->tau)

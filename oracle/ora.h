@@ -45,6 +45,9 @@ typedef struct {
   int enable_afc, enable_toc, enable_sr; /* Table IV toggles */
   int exact_tiles;        /* 1: a Gaussian "intersects" a tile iff max alpha over the tile's pixel box >= 1/255
                              (R39, same box test as L119); 0: every tile of the 3-sigma rect (vanilla 3DGS) */
+  int prior_policy;       /* 0 ANCHORED (paper, L86: priors always come from the last R / P frame); 1 CHAINED (R42): the
+                             stitched outputs of every S frame replace the priors, G_rendered grows by what it blended */
+  int tgb_downscale;      /* 1 (default) or 2: TGB warped, repaired and looked up on a (W/2) x (H/2) grid (L142, R43) */
 } ora_params;
 
 typedef struct {        /* 80 bytes */

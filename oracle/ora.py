@@ -30,7 +30,8 @@ assert RECORD_DTYPE.itemsize == 80
 class OraParams(C.Structure):
     _fields_ = [("lambda1", C.c_float), ("lambda2", C.c_float), ("lambda_tdc", C.c_int), ("lambda_sr", C.c_int),
                 ("eta", C.c_float), ("bg", C.c_float * 3),
-                ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int), ("exact_tiles", C.c_int)]
+                ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int), ("exact_tiles", C.c_int),
+                ("prior_policy", C.c_int), ("tgb_downscale", C.c_int)]
 
 
 class OraStats(C.Structure):
@@ -110,7 +111,7 @@ def _fp(a):
 _GET_DTYPES = {
     "records": RECORD_DTYPE, "keys": np.uint64, "vals": np.uint32, "ranges": np.uint32,
     "warp_depth": np.float32, "warp_sigma": np.float32, "fill_depth": np.float32, "corr_xy": np.float32,
-    "matched": np.uint8, "rendered": np.uint8, "rendered_sure": np.uint8, "rendered_maybe": np.uint8,
+    "matched": np.uint8, "rendered": np.uint8, "rendered_now": np.uint8, "rendered_sure": np.uint8, "rendered_maybe": np.uint8,
     "borderline": np.uint8, "F": np.float32, "prior_depth": np.float32, "prior_sigma": np.float32,
     "prior_image": np.float32, "prior_view": np.float32, "M": np.float32, "Minv": np.float32,
     "cov3d": np.float32, "tau": np.float32,

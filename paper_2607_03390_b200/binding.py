@@ -29,7 +29,7 @@ class TgsParams(C.Structure):
     _fields_ = [("lambda1", C.c_float), ("lambda2", C.c_float), ("lambda_tdc", C.c_int), ("lambda_sr", C.c_int),
                 ("eta", C.c_float), ("bg", C.c_float * 3),
                 ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int), ("max_pairs", C.c_uint32),
-                ("exact_tiles", C.c_int)]
+                ("exact_tiles", C.c_int), ("prior_policy", C.c_int), ("tgb_downscale", C.c_int)]
 
 
 class TgsStats(C.Structure):

@@ -209,6 +209,8 @@ void tgs_default_params(tgs_params* p) {
   p->enable_afc = p->enable_toc = p->enable_sr = 1;
   p->max_pairs = 0;
   p->exact_tiles = 1;
+  p->prior_policy = TGS_PRIORS_ANCHORED;
+  p->tgb_downscale = 1;
 }
 
 int tgs_create(tgs_ctx** out, int device, void* stream) {
@@ -324,7 +326,8 @@ int tgs_set_camera(tgs_ctx* c, const float view[16], float fx, float fy, float c
 
 int tgs_set_params(tgs_ctx* c, const tgs_params* p) {
   if (!c || !p || p->lambda_tdc < 1 || p->lambda_sr < 1 || !std::isfinite(p->lambda1) || !std::isfinite(p->lambda2) ||
-      !std::isfinite(p->eta) || !finite_all(p->bg, 3)) return TGS_E_INVALID_ARG;
+      !std::isfinite(p->eta) || !finite_all(p->bg, 3) || (p->prior_policy != TGS_PRIORS_ANCHORED && p->prior_policy != TGS_PRIORS_CHAINED) ||
+      (p->tgb_downscale != 1 && p->tgb_downscale != 2)) return TGS_E_INVALID_ARG;
   c->prm = *p;
   return TGS_OK;
 }
@@ -402,9 +405,13 @@ int tgs_render(tgs_ctx* c, int mode) {
   DevBuffers& b = c->b;
   cudaStream_t s = c->stream;
   const bool builds_priors = ftype != TGS_FRAME_S;
+  // R42 (prior_policy = CHAINED): an S frame's stitched outputs become the priors too; its G_rendered marks are OR-ed
+  // into the current set in place (k_preprocess has read the set before the blend writes it: stream order)
+  const bool chains = ftype == TGS_FRAME_S && c->prm.prior_policy == TGS_PRIORS_CHAINED;
   const int out_idx = c->prior_idx ^ 1;   // never overwrite the priors while they are being read
   const float* prior_image = c->priors_valid ? b.image[c->prior_idx] : nullptr;
   uint8_t* rendered_next = builds_priors ? b.rendered_next : nullptr;
+  uint8_t* rendered_marks = chains ? b.rendered : rendered_next;
   int ev = 0;
   auto mark = [&]() { if (c->timing) cudaEventRecord(c->ev_stage[ev], s); ++ev; };
   mark();                                                                      // 0: init, A1 warp, A2 fill + correspondence
@@ -446,7 +453,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   mark();                                                                      // 6: A8 + A9
   if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
   if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
-  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_next, c->num_sms, c->count_interactions);
+  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_marks, c->num_sms, c->count_interactions);
   mark();                                                                      // 7: post
   if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
   CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
@@ -462,6 +469,7 @@ int tgs_render(tgs_ctx* c, int mode) {
     c->priors_valid = true;
     if (ftype == TGS_FRAME_R) c->F_valid = true;
   }
+  if (chains) { c->prior_idx = out_idx; memcpy(c->prior_view, c->view, sizeof(c->prior_view)); }
   if (ftype == TGS_FRAME_R) { c->sched.since_R = 0; c->sched.since_ref = 0; c->sched.force_P = 0; }
   else if (ftype == TGS_FRAME_P) { c->sched.since_ref = 0; c->sched.force_P = 0; }
   ++c->sched.since_R; ++c->sched.since_ref;

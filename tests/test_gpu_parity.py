@@ -142,6 +142,49 @@ def test_layered_scene_config5_reduced():
     assert sg["n_toc"] > 0.2 * sc.n
 
 
+def test_chained_priors_policy():
+    """prior_policy = CHAINED (R42): every S frame starts from the oracle's current priors (injected), is compared in
+    full, and must then have committed its own outputs: priors = the frame's stitched image / depth / sigma, pose of
+    this frame, G_rendered = previous set OR what this frame blended (between the oracle's sure / maybe sets)."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(5, n=60_000, frames=12, width=320, height=180)
+    sc.scales[:, :2] *= 6.0
+    g, o = P.make_pair(sc, {"prior_policy": 1})
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    partial = 0
+    for f in (1, 2, 3, 4):
+        P.inject_priors(g, o)
+        before = o.get("rendered").astype(bool)
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G["temporal"]); assert o.render(ora.TEMPORAL) == ora.FRAME_S
+        sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+        partial += 0 < sg["n_sel"] < sg["n_tiles"]
+        d, sgm = g.read_depth()
+        assert np.array_equal(P.bits(g.debug_get("prior_image")), P.bits(g.read_image().ravel()))
+        assert np.array_equal(P.bits(g.debug_get("prior_depth")), P.bits(d.ravel()))
+        assert np.array_equal(P.bits(g.debug_get("prior_sigma")), P.bits(sgm.ravel()))
+        assert np.array_equal(o.get("prior_view"), np.asarray(sc.poses[f], np.float32).ravel())
+        r_g = g.debug_get("rendered").astype(bool)
+        sure, maybe = o.get("rendered_sure").astype(bool), o.get("rendered_maybe").astype(bool)
+        assert not np.any((before | sure) & ~r_g) and not np.any(r_g & ~(before | maybe))
+        assert np.array_equal(o.get("rendered").astype(bool), before | o.get("rendered_now").astype(bool))
+    assert partial >= 2          # the chain ran on frames that stitch a part of the image
+    # the chained GPU context on its own (no injection): the second S frame warps from the first one's pose
+    g2 = tgs.Context(0); g2.load_scene(sc)
+    p = g2.default_params(); p.prior_policy = 1; g2.set_params(p)
+    a = tgs.Context(0); a.load_scene(sc)
+    for f in range(4):
+        for c in (g2, a):
+            c.set_camera(sc.poses[f], sc.camera); c.render(tgs.FULL if f == 0 else tgs.TEMPORAL)
+        if f == 1:
+            assert np.array_equal(g2.read_image(), a.read_image())        # same priors for the first S frame
+    assert not np.array_equal(g2.debug_get("prior_image"), a.debug_get("prior_image"))
+    assert np.abs(g2.read_image() - a.read_image()).mean() < 2e-2
+
+
 # ------------------------------------------------------------------------------------------------ scheduler through the ABI
 def test_auto_schedule_matches_oracle():
     P = _p()

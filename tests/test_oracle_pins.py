@@ -595,6 +595,52 @@ def test_p9_moved_camera_selects_tiles_and_stitches():
     assert mse < 1e-2
 
 
+def test_r42_chained_priors():
+    """prior_policy = CHAINED (R42; north_star: the new frame becomes the next frame's TGB / TAB).  Pins that do not
+    re-type the commit: (a) the first S frame after a reference frame is the same under both policies (same priors);
+    (b) at an unchanged pose nothing is selected and a chain of S frames keeps reproducing the reference image;
+    (c) the second S frame of a chain equals an ANCHORED S frame of a second oracle whose priors were set, through the
+    public put interface, to the first S frame's read-back outputs and pose; (d) G_rendered only grows."""
+    sc = _tiny_scene()
+    poses = [look_at((0.4 + 0.05 * i, 0.2, -4.0), (0, 0, 0), (0, 1, 0)) for i in range(3)]
+
+    def ctx(policy):
+        o = Oracle(); o.load_scene(sc)
+        p = o.default_params(); p.prior_policy = policy; o.set_params(p)
+        o.set_camera(poses[0], sc.camera); assert o.render(ora.FULL) == ora.FRAME_R
+        return o
+    a, c = ctx(0), ctx(1)
+    r0 = c.get("rendered").copy()
+    for o in (a, c):
+        o.set_camera(poses[1], sc.camera); assert o.render(ora.TEMPORAL) == ora.FRAME_S
+    img1 = c.read_image(); d1, s1 = c.read_depth()
+    assert np.array_equal(a.read_image().view(np.uint32), img1.view(np.uint32))                       # (a)
+    assert np.array_equal(a.get("keys"), c.get("keys")) and a.stats()["n_sel"] == c.stats()["n_sel"]
+    # the anchored context still holds the reference frame's priors, the chained one this frame's outputs
+    assert np.array_equal(a.get("prior_view"), np.asarray(poses[0], np.float32).ravel())
+    assert np.array_equal(c.get("prior_view"), np.asarray(poses[1], np.float32).ravel())
+    assert np.array_equal(c.get("prior_image").view(np.uint32), img1.ravel().view(np.uint32))
+    assert np.array_equal(c.get("prior_depth").view(np.uint32), d1.ravel().view(np.uint32))
+    r1 = c.get("rendered").copy()
+    assert np.all(r1 >= r0) and np.array_equal(r1, r0 | c.get("rendered_now"))                          # (d)
+    assert np.array_equal(a.get("rendered"), r0)
+    # (c) second S frame of the chain vs an anchored frame from hand-set priors
+    c.set_camera(poses[2], sc.camera); assert c.render(ora.TEMPORAL) == ora.FRAME_S
+    b = Oracle(); b.load_scene(sc); b.set_camera(poses[0], sc.camera); b.render(ora.FULL)   # F of the reference frame
+    b.put("prior_depth", d1.ravel()); b.put("prior_sigma", s1.ravel()); b.put("prior_image", img1.ravel())
+    b.put("rendered", r1); b.put("prior_view", np.asarray(poses[1], np.float32).ravel())
+    b.set_camera(poses[2], sc.camera); assert b.render(ora.TEMPORAL) == ora.FRAME_S
+    assert np.array_equal(b.read_image().view(np.uint32), c.read_image().view(np.uint32))
+    assert np.array_equal(b.read_tile_mask(), c.read_tile_mask()) and np.array_equal(b.get("keys"), c.get("keys"))
+    # (b) unchanged pose: a chain of S frames selects nothing and keeps the image
+    e = ctx(1)
+    ref = e.read_image()
+    for _ in range(3):
+        assert e.render(ora.TEMPORAL) == ora.FRAME_S
+        assert e.stats()["n_sel"] == 0
+        np.testing.assert_allclose(e.read_image(), ref, atol=1e-5)
+
+
 def test_p9_priors_required():
     sc = _tiny_scene()
     o = Oracle()
