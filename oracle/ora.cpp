@@ -144,6 +144,10 @@ struct ora_ctx {
   float prior_view[16];
   // per-frame
   float M[12], Minv[12];
+  // TGB grid of this frame (R43): ds = 1: the image grid; ds = 2: ceil(W/2) x ceil(H/2), grid pixel (i, j) sits at the
+  // image position (2i + 0.5, 2j + 0.5), i.e. a pinhole camera with fx/2, fy/2, (cx - 0.5)/2, (cy - 0.5)/2
+  int ds = 1, Wt = 0, Ht = 0;
+  float tfx = 0, tfy = 0, tcx = 0, tcy = 0;
   std::vector<float> warp_depth, warp_sigma, fill_depth, corr_xy;
   std::vector<uint8_t> matched;
   std::vector<ora_record> rec;
@@ -165,25 +169,53 @@ bool finite_all(const float* p, size_t n) {
 // ---------------------------------------------------------------- O9 forward warp (A1)
 // PAPER.md:L86-97 Eq.3.  Nearest-pixel splat (R14), min depth / max sigma kept independently (R15),
 // initialised to z_far+eps / 0 (L97, R12); sigma' = sigma |M_R[row 3] . ray| (R13).
+void tgb_grid(ora_ctx* c) {
+  const Cam& k = c->cam;
+  c->ds = c->prm.tgb_downscale == 2 ? 2 : 1;
+  if (c->ds == 1) { c->Wt = k.W; c->Ht = k.H; c->tfx = k.fx; c->tfy = k.fy; c->tcx = k.cx; c->tcy = k.cy; }
+  else {
+    c->Wt = (k.W + 1) / 2; c->Ht = (k.H + 1) / 2;
+    c->tfx = k.fx * 0.5f; c->tfy = k.fy * 0.5f; c->tcx = (k.cx - 0.5f) * 0.5f; c->tcy = (k.cy - 0.5f) * 0.5f;
+  }
+}
+
+// TGB source value of grid pixel (x, y).  ds = 2 (L142 "downscale the TGB by 2", operator unspecified -> R43): nearest
+// valid depth of the 2x2 block and the largest sigma of its valid pixels -- the same "closer geometry, maximum
+// deviation, for high recall" rule the paper states for colliding warped pixels (L91).
+void tgb_source(const ora_ctx* c, int x, int y, float* D, float* sg) {
+  const int W = c->cam.W, H = c->cam.H;
+  if (c->ds == 1) { *D = c->prior_depth[(size_t)y * W + x]; *sg = c->prior_sigma[(size_t)y * W + x]; return; }
+  float d = ORA_DEPTH_INVALID, s = 0.0f;
+  for (int yy = 2 * y; yy < std::min(H, 2 * y + 2); ++yy)
+    for (int xx = 2 * x; xx < std::min(W, 2 * x + 2); ++xx) {
+      const float v = c->prior_depth[(size_t)yy * W + xx];
+      if (!(v < 1.0e38f)) continue;
+      d = std::fmin(d, v); s = std::fmax(s, c->prior_sigma[(size_t)yy * W + xx]);
+    }
+  *D = d; *sg = s;
+}
+
 void forward_warp(ora_ctx* c) {
-  const Cam& k = c->cam; const int W = k.W, H = k.H; const float* M = c->M;
+  const Cam& k = c->cam; const int W = c->Wt, H = c->Ht; const float* M = c->M;
+  const float fx = c->tfx, fy = c->tfy, cx = c->tcx, cy = c->tcy;
   c->warp_depth.assign((size_t)W * H, ORA_DEPTH_INVALID);
   c->warp_sigma.assign((size_t)W * H, 0.0f);
   for (int y = 0; y < H; ++y)
     for (int x = 0; x < W; ++x) {
-      const float D = c->prior_depth[(size_t)y * W + x];
+      float D, sg;
+      tgb_source(c, x, y, &D, &sg);
       if (!(D < 1.0e38f)) continue;                       // R11: no geometry -> not warped
-      const float rx = ((float)x - k.cx) / k.fx, ry = ((float)y - k.cy) / k.fy;
+      const float rx = ((float)x - cx) / fx, ry = ((float)y - cy) / fy;
       const float Px = D * rx, Py = D * ry, Pz = D;
       const float X = ((M[0] * Px + M[1] * Py) + M[2] * Pz) + M[3];
       const float Y = ((M[4] * Px + M[5] * Py) + M[6] * Pz) + M[7];
       const float Z = ((M[8] * Px + M[9] * Py) + M[10] * Pz) + M[11];
       if (!(Z > k.znear)) continue;
-      const float u = (k.fx * X) / Z + k.cx, v = (k.fy * Y) / Z + k.cy;
+      const float u = (fx * X) / Z + cx, v = (fy * Y) / Z + cy;
       const float fu = std::floor(u + 0.5f), fv = std::floor(v + 0.5f);
       if (!(fu >= 0.0f && fu < (float)W && fv >= 0.0f && fv < (float)H)) continue;
       const size_t q = (size_t)(int)fv * W + (int)fu;
-      const float s = c->prior_sigma[(size_t)y * W + x] * std::fabs((M[8] * rx + M[9] * ry) + M[10]);
+      const float s = sg * std::fabs((M[8] * rx + M[9] * ry) + M[10]);
       c->warp_depth[q] = std::fmin(c->warp_depth[q], Z);
       c->warp_sigma[q] = std::fmax(c->warp_sigma[q], s);
     }
@@ -193,7 +225,8 @@ void forward_warp(ora_ctx* c) {
 // PAPER.md:L121.  R19: 8 neighbours, single pass from the unrepaired buffer, border never filled.
 // R20: matched <=> D' valid, back-projected z > z_near, nearest pixel of (x,y) inside the image.  R22: in-image pixels.
 void fill_and_correspond(ora_ctx* c) {
-  const Cam& k = c->cam; const int W = k.W, H = k.H; const float* M = c->Minv;
+  const int W = c->Wt, H = c->Ht; const float* M = c->Minv;
+  struct { float fx, fy, cx, cy, znear; } k = {c->tfx, c->tfy, c->tcx, c->tcy, c->cam.znear};
   c->fill_depth = c->warp_depth;
   for (int y = 1; y < H - 1; ++y)
     for (int x = 1; x < W - 1; ++x) {
@@ -262,7 +295,7 @@ void preprocess(ora_ctx* c, int ftype) {
     if (do_tgb && !c->rendered[g]) {                                                   // L113, L119, R16, R17
       const float fu = std::floor(u + 0.5f), fv = std::floor(v + 0.5f);
       if (fu >= 0.0f && fu < (float)W && fv >= 0.0f && fv < (float)H) {
-        const size_t q = (size_t)(int)fv * W + (int)fu;
+        const size_t q = (size_t)((int)fv / c->ds) * c->Wt + (size_t)((int)fu / c->ds);   // R43: the block of the nearest pixel
         const float D = c->warp_depth[q], s = c->warp_sigma[q];
         if (c->prm.enable_toc && tz > D + c->prm.lambda2 * s) { r.flags = ORA_CULL_TOC; ++st.n_toc; continue; }
         if (tz <= D - c->prm.lambda1 * s) fl |= ORA_NEWLY_VISIBLE;
@@ -326,9 +359,10 @@ void select_tiles(ora_ctx* c, int ftype) {
     for (int ty = 0; ty < TY; ++ty)
       for (int tx = 0; tx < TX; ++tx) {
         bool um = false;
-        for (int y = ty * TILE; y < std::min(H, ty * TILE + TILE) && !um; ++y)
-          for (int x = tx * TILE; x < std::min(W, tx * TILE + TILE); ++x)
-            if (!c->matched[(size_t)y * W + x]) { um = true; break; }
+        const int tg = TILE / c->ds;                       // tile edge in TGB grid pixels
+        for (int y = ty * tg; y < std::min(c->Ht, ty * tg + tg) && !um; ++y)
+          for (int x = tx * tg; x < std::min(c->Wt, tx * tg + tg); ++x)
+            if (!c->matched[(size_t)y * c->Wt + x]) { um = true; break; }
         if (um) c->tile_mask[(size_t)ty * TX + tx] |= 2;
       }
     // T^oc: newly visible Gaussians whose max alpha over the tile's pixel box >= 1/255 (L119, R18)
@@ -416,7 +450,18 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
         for (int px = tx * TILE; px < std::min(W, tx * TILE + TILE); ++px) {
           const size_t pix = (size_t)py * W + px;
           if (!sel) {   // Eq.4 second case: warped TAB
-            const double xs = c->corr_xy[pix * 2], ys = c->corr_xy[pix * 2 + 1];
+            double xs, ys;
+            const size_t tq = (size_t)(py / c->ds) * c->Wt + (size_t)(px / c->ds);
+            if (c->ds == 1) { xs = c->corr_xy[pix * 2]; ys = c->corr_xy[pix * 2 + 1]; }
+            else {   // R43: the pixel's own ray with the repaired depth of its TGB block, backward Eq.3 (L121, L101)
+              const float D = c->fill_depth[tq]; const float* Mi = c->Minv;
+              const float rx = ((float)px - k.cx) / k.fx, ry = ((float)py - k.cy) / k.fy;
+              const float Px = D * rx, Py = D * ry, Pz = D;
+              const float X = ((Mi[0] * Px + Mi[1] * Py) + Mi[2] * Pz) + Mi[3];
+              const float Y = ((Mi[4] * Px + Mi[5] * Py) + Mi[6] * Pz) + Mi[7];
+              const float Z = ((Mi[8] * Px + Mi[9] * Py) + Mi[10] * Pz) + Mi[11];
+              xs = (k.fx * X) / Z + k.cx; ys = (k.fy * Y) / Z + k.cy;
+            }
             const double x0 = std::floor(xs), y0 = std::floor(ys);
             const double wx = xs - x0, wy = ys - y0;
             const int ix0 = std::min(std::max((int)x0, 0), W - 1), ix1 = std::min(std::max((int)x0 + 1, 0), W - 1);
@@ -426,8 +471,8 @@ void blend_and_stitch(ora_ctx* c, int ftype) {
               const double v01 = c->prior_image[((size_t)iy1 * W + ix0) * 3 + ch], v11 = c->prior_image[((size_t)iy1 * W + ix1) * 3 + ch];
               c->image[pix * 3 + ch] = (float)((v00 * (1 - wx) + v10 * wx) * (1 - wy) + (v01 * (1 - wx) + v11 * wx) * wy);
             }
-            c->depth[pix] = c->fill_depth[pix];
-            c->sigma[pix] = c->warp_sigma[pix];
+            c->depth[pix] = c->fill_depth[tq];
+            c->sigma[pix] = c->warp_sigma[tq];
             continue;
           }
           double T = 1.0, C[3] = {0, 0, 0}, Sw = 0, Sd = 0, Sdd = 0;
@@ -631,6 +676,7 @@ int ora_render(ora_ctx* c, int mode) {
   if (ftype == ORA_FRAME_S) {
     relative_pose(c->prior_view, c->cam.V, c->M);       // reference -> current (forward, Eq.3)
     relative_pose(c->cam.V, c->prior_view, c->Minv);    // current -> reference (backward, L121)
+    tgb_grid(c);
     forward_warp(c);
     fill_and_correspond(c);
   }
@@ -719,6 +765,7 @@ int ora_stage(ora_ctx* c, const char* stage) {
   if (s == "warp") {
     relative_pose(c->prior_view, c->cam.V, c->M);
     relative_pose(c->cam.V, c->prior_view, c->Minv);
+    tgb_grid(c);
     forward_warp(c); return ORA_OK;
   }
   if (s == "fill") { fill_and_correspond(c); return ORA_OK; }

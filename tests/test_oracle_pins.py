@@ -595,6 +595,92 @@ def test_p9_moved_camera_selects_tiles_and_stitches():
     assert mse < 1e-2
 
 
+def _block_reduce(D, S):
+    """R43 written out with numpy: nearest valid depth of each 2x2 block, largest sigma of its valid pixels."""
+    H, W = D.shape
+    Hh, Wh = (H + 1) // 2, (W + 1) // 2
+    Dp = np.full((2 * Hh, 2 * Wh), np.float32(ora.DEPTH_INVALID)); Dp[:H, :W] = D
+    Sp = np.zeros((2 * Hh, 2 * Wh), np.float32); Sp[:H, :W] = np.where(D < 1e38, S, 0)
+    Db = Dp.reshape(Hh, 2, Wh, 2).min(axis=(1, 3))
+    Sb = Sp.reshape(Hh, 2, Wh, 2).max(axis=(1, 3))
+    return Db, Sb
+
+
+def test_r43_half_resolution_tgb_is_the_pipeline_of_a_half_resolution_camera():
+    """tgb_downscale = 2 (L142; R43).  (a) identity pose: the warped TGB is the 2x2 block reduction of the priors;
+    (b) general pose, odd image size: warp, repaired depth and matched flags equal, bit for bit, those of a second
+    oracle run at downscale 1 with the camera (fx/2, fy/2, (cx-0.5)/2, (cy-0.5)/2) on ceil(W/2) x ceil(H/2) whose
+    priors are the block-reduced buffers -- the downscale-1 pipeline is pinned by P7 / P8."""
+    rng = np.random.default_rng(5)
+    cam = Camera(W=97, H=63, fx=91.0, fy=87.0, cx=48.0, cy=31.0)
+    D = rng.uniform(2.0, 6.0, size=(cam.H, cam.W)).astype(np.float32)
+    D[20:40, 30:60] = 2.5                                            # a smooth patch: filled holes and matched pixels
+    S = rng.uniform(0.0, 0.3, size=D.shape).astype(np.float32)
+    D[rng.random(D.shape) < 0.3] = ora.DEPTH_INVALID
+    Db, Sb = _block_reduce(D, S)
+    Vref = look_at((0, 0, -1), (0, 0, 3), (0, 1, 0))
+    o = _prior_ctx(cam, Vref, D, S)
+    p = o.default_params(); p.tgb_downscale = 2; o.set_params(p)
+    o.stage("warp")                                                  # (a): M = identity
+    assert np.array_equal(o.get("warp_depth").reshape(Db.shape), Db)
+    assert np.array_equal(o.get("warp_sigma").reshape(Db.shape), Sb)
+    Vnew = look_at((0.12, -0.05, -1.2), (0.05, 0, 3), (0, 1, 0))
+    o.set_camera(Vnew, cam); o.stage("warp"); o.stage("fill")
+    camh = Camera(W=Db.shape[1], H=Db.shape[0], fx=float(np.float32(cam.fx) * np.float32(0.5)), fy=float(np.float32(cam.fy) * np.float32(0.5)),
+                  cx=float((np.float32(cam.cx) - np.float32(0.5)) * np.float32(0.5)), cy=float((np.float32(cam.cy) - np.float32(0.5)) * np.float32(0.5)))
+    h = _prior_ctx(camh, Vref, Db, Sb)
+    h.set_camera(Vnew, camh); h.stage("warp"); h.stage("fill")
+    for name in ("warp_depth", "warp_sigma", "fill_depth", "matched", "corr_xy"):
+        a, b = o.get(name), h.get(name)
+        assert a.shape == b.shape and np.array_equal(a.view(np.uint8), b.view(np.uint8)), name
+    assert 0.05 < h.get("matched").mean() < 1.0 and (h.get("fill_depth") < 1e38).sum() > (h.get("warp_depth") < 1e38).sum()
+
+
+def test_r43_half_resolution_tgb_frame():
+    """A whole S frame with tgb_downscale = 2: same pose => nothing selected, the image is the TAB, depth / sigma of a
+    pixel are those of its block; moved camera => T^um is decided on the 8x8 grid pixels of a tile, TOC looks up the
+    block of the Gaussian's nearest pixel (checked against the read-back warped TGB), stitched pixels stay inside
+    the TAB's range and close to the downscale-1 frame."""
+    sc = _tiny_scene()
+    W, H = sc.camera.W, sc.camera.H
+    V0, V1 = look_at((0.4, 0.2, -4.0), (0, 0, 0), (0, 1, 0)), look_at((0.5, 0.2, -4.0), (0, 0, 0), (0, 1, 0))
+    o = Oracle(); o.load_scene(sc)
+    p = o.default_params(); p.tgb_downscale = 2; o.set_params(p)
+    o.set_camera(V0, sc.camera); o.render(ora.FULL)
+    tab = o.read_image(); d0, s0 = o.read_depth()
+    Db, Sb = _block_reduce(d0, s0)
+    assert o.render(ora.TEMPORAL) == ora.FRAME_S
+    assert o.stats()["n_sel"] == 0
+    np.testing.assert_allclose(o.read_image(), tab, atol=1e-5)
+    d, sg = o.read_depth()
+    up = lambda a: np.kron(a, np.ones((2, 2), a.dtype))[:H, :W]
+    assert np.array_equal(d, up(Db))
+    np.testing.assert_allclose(sg, up(Sb), rtol=1e-6)      # sigma' = sigma |M_R[row 3] . ray| with M = I up to rounding
+    # moved camera
+    o.set_camera(V1, sc.camera); assert o.render(ora.TEMPORAL) == ora.FRAME_S
+    st, mask = o.stats(), o.read_tile_mask()
+    assert 0 < st["n_sel"] < st["n_tiles"]
+    m = o.get("matched").reshape(Db.shape)
+    TY, TX = mask.shape
+    um = np.array([[not m[8 * ty:8 * ty + 8, 8 * tx:8 * tx + 8].all() for tx in range(TX)] for ty in range(TY)])
+    assert np.array_equal((mask & 2) != 0, um)
+    rec = o.get("records"); wd = o.get("warp_depth").reshape(Db.shape); rendered = o.get("rendered").astype(bool)
+    toc = (rec["flags"] & ora.CULL_TOC) != 0
+    assert toc.sum() > 0
+    fu, fv = np.floor(rec["u"] + np.float32(0.5)).astype(int), np.floor(rec["v"] + np.float32(0.5)).astype(int)
+    inside = (fu >= 0) & (fu < W) & (fv >= 0) & (fv < H)
+    assert inside[toc].all() and not rendered[toc].any()
+    assert np.all(rec["d"][toc] > wd[fv[toc] // 2, fu[toc] // 2])                    # lambda2 = 0
+    cand = inside & ~rendered & ((rec["flags"] & (ora.CULL_NEAR | ora.CULL_AFC)) == 0)
+    assert np.array_equal(toc[cand], rec["d"][cand] > wd[fv[cand] // 2, fu[cand] // 2])
+    img2 = o.read_image()
+    sel_px = np.kron((mask & 4) != 0, np.ones((16, 16), bool))[:H, :W]
+    assert img2[~sel_px].max() <= tab.max() + 1e-6 and img2[~sel_px].min() >= tab.min() - 1e-6
+    o1 = Oracle(); o1.load_scene(sc); o1.set_camera(V0, sc.camera); o1.render(ora.FULL)
+    o1.set_camera(V1, sc.camera); o1.render(ora.TEMPORAL)
+    assert float(((img2 - o1.read_image()) ** 2).mean()) < 1e-3
+
+
 def test_r42_chained_priors():
     """prior_policy = CHAINED (R42; north_star: the new frame becomes the next frame's TGB / TAB).  Pins that do not
     re-type the commit: (a) the first S frame after a reference frame is the same under both policies (same priors);
