@@ -128,7 +128,8 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
         const int px = px0 + i;
         if (!row_in || px >= k.W) continue;
         const size_t pix = (size_t)py * k.W + px;
-        const float D = fill_depth[pix];
+        const size_t tq = (size_t)(py / fc.tg.ds) * fc.tg.W + (size_t)(px / fc.tg.ds);   // TGB grid pixel (R43)
+        const float D = fill_depth[tq];
         const float* M = fc.Minv;
         const float rx = ((float)px - k.cx) / k.fx, ry = ((float)py - k.cy) / k.fy;
         const float Px = D * rx, Py = D * ry;
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const ui
           image[pix * 3 + ch] = top * (1.0f - wy) + bot * wy;
         }
         depth[pix] = D;
-        sigma[pix] = warp_sigma[pix];
+        sigma[pix] = warp_sigma[tq];
       }
       continue;
     }

@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
   for (uint32_t i = tid; i < n_tt4; i += nth) tiles_touched4[i] = make_uint4(0u, 0u, 0u, 0u);
   if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
-    const uint32_t px = (uint32_t)(fc.cam.W * fc.cam.H);
+    const uint32_t px = (uint32_t)(fc.tg.W * fc.tg.H);
     for (uint32_t i = tid; i < px; i += nth) { warp_depth[i] = TGS_INVALID_BITS; warp_sigma[i] = 0; }
   }
   if (rendered_next_words)
@@ -91,9 +91,24 @@ __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __rest
                                               uint32_t* __restrict__ warp_sigma) {
   TGS_PDL_WAIT();
   const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
-  const CamConst& k = fc.cam;
+  const CamConst& kc = fc.cam;
+  const TgbGrid& k = fc.tg;
   if (x >= k.W || y >= k.H) return;
-  const float D = prior_depth[(size_t)y * k.W + x];
+  float D, sg;
+  if (k.ds == 1) { D = prior_depth[(size_t)y * kc.W + x]; sg = prior_sigma[(size_t)y * kc.W + x]; }
+  else {                                                          // R43: 2x2 block, nearest valid depth / largest sigma
+    D = TGS_DEPTH_INVALID; sg = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int xx = 2 * x + i, yy = 2 * y + j;
+        if (xx >= kc.W || yy >= kc.H) continue;
+        const float v = prior_depth[(size_t)yy * kc.W + xx];
+        if (!(v < 1.0e38f)) continue;
+        D = fminf(D, v); sg = fmaxf(sg, prior_sigma[(size_t)yy * kc.W + xx]);
+      }
+  }
   if (!(D < 1.0e38f)) return;                                   // R11
   const float* M = fc.M;
   const float rx = ((float)x - k.cx) / k.fx, ry = ((float)y - k.cy) / k.fy;
@@ -101,12 +116,12 @@ __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __rest
   const float X = ((M[0] * Px + M[1] * Py) + M[2] * Pz) + M[3];
   const float Y = ((M[4] * Px + M[5] * Py) + M[6] * Pz) + M[7];
   const float Z = ((M[8] * Px + M[9] * Py) + M[10] * Pz) + M[11];
-  if (!(Z > k.znear)) return;
+  if (!(Z > kc.znear)) return;
   const float u = (k.fx * X) / Z + k.cx, v = (k.fy * Y) / Z + k.cy;
   const float fu = floorf(u + 0.5f), fv = floorf(v + 0.5f);
   if (!(fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf)) return;
   const size_t q = (size_t)(int)fv * k.W + (int)fu;
-  const float s = prior_sigma[(size_t)y * k.W + x] * fabsf((M[8] * rx + M[9] * ry) + M[10]);   // R13
+  const float s = sg * fabsf((M[8] * rx + M[9] * ry) + M[10]);   // R13
   atomicMin(&warp_depth[q], __float_as_uint(Z));
   if (s > 0.0f) atomicMax(&warp_sigma[q], __float_as_uint(s));
 }
@@ -118,10 +133,12 @@ __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __rest
 __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* __restrict__ warp_depth, float* __restrict__ fill_depth,
                                                    uint32_t* __restrict__ tile_flags) {
   TGS_PDL_WAIT();
-  const CamConst& k = fc.cam;
-  const int lx = threadIdx.x & 15, ly = threadIdx.x >> 4;
-  const int x = blockIdx.x * TGS_TILE + lx, y = blockIdx.y * TGS_TILE + ly;
-  const bool inside = x < k.W && y < k.H;
+  const TgbGrid& k = fc.tg;
+  const float znear = fc.cam.znear;
+  const int edge = TGS_TILE / k.ds;                              // a tile is edge x edge grid pixels (R43)
+  const int lx = threadIdx.x % edge, ly = threadIdx.x / edge;
+  const int x = blockIdx.x * edge + lx, y = blockIdx.y * edge + ly;
+  const bool inside = ly < edge && x < k.W && y < k.H;
   bool unmatched = false;
   if (inside) {
     const float* wd = warp_depth;
@@ -142,7 +159,7 @@ __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* _
       const float X = ((M[0] * Px + M[1] * Py) + M[2] * Pz) + M[3];
       const float Y = ((M[4] * Px + M[5] * Py) + M[6] * Pz) + M[7];
       const float Z = ((M[8] * Px + M[9] * Py) + M[10] * Pz) + M[11];
-      if (Z > k.znear) {
+      if (Z > znear) {
         const float xs = (k.fx * X) / Z + k.cx, ys = (k.fy * Y) / Z + k.cy;
         const float fu = floorf(xs + 0.5f), fv = floorf(ys + 0.5f);
         if (fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf) unmatched = false;
@@ -150,7 +167,7 @@ __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* _
     }
   }
   const int any = __syncthreads_or(unmatched ? 1 : 0);
-  if (threadIdx.x == 0 && any) atomicOr(&tile_flags[blockIdx.y * k.TX + blockIdx.x], 2u);   // bit1 = T^um (k_preprocess ORs bit0 concurrently)
+  if (threadIdx.x == 0 && any) atomicOr(&tile_flags[blockIdx.y * fc.cam.TX + blockIdx.x], 2u);   // bit1 = T^um (k_preprocess ORs bit0 concurrently)
 }
 
 }  // namespace
@@ -284,7 +301,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, co
       const float fu = floorf(u + 0.5f), fv = floorf(v + 0.5f);
       const bool centre_in = fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf;
       if (fc.do_tgb && !((rend4 >> (8 * j)) & 0xffu) && centre_in) {                              // L113, L119
-        const size_t q = (size_t)(int)fv * k.W + (int)fu;
+        const size_t q = (size_t)((int)fv / fc.tg.ds) * fc.tg.W + (size_t)((int)fu / fc.tg.ds);   // R43: block of the nearest pixel
         const float D = warp_depth[q], s = warp_sigma[q];
         if (fc.do_toc && tz > D + fc.lambda2 * s) { cf[j] = TGS_CULL_TOC; ++st_toc; continue; }
         if (tz <= D - fc.lambda1 * s) fl = 2u;
@@ -587,7 +604,7 @@ void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool
 }
 
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma) {
-  dim3 grid((fc.cam.W + 31) / 32, (fc.cam.H + 7) / 8);
+  dim3 grid((fc.tg.W + 31) / 32, (fc.tg.H + 7) / 8);
   TGS_LAUNCH((k_warp), grid, 256, 0, s, fc, prior_depth, prior_sigma, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma);
 }
 

@@ -384,6 +384,14 @@ int tgs_render(tgs_ctx* c, int mode) {
   k.W = c->W; k.H = c->H; k.TX = c->TX; k.TY = c->TY;
   if (ftype == TGS_FRAME_S) { relative_pose(c->prior_view, c->view, fc.M); relative_pose(c->view, c->prior_view, fc.Minv); }
   else { memset(fc.M, 0, sizeof(fc.M)); memset(fc.Minv, 0, sizeof(fc.Minv)); }
+  TgbGrid& tg = fc.tg;
+  tg.ds = c->prm.tgb_downscale == 2 ? 2 : 1;
+  if (tg.ds == 1) { tg.W = c->W; tg.H = c->H; tg.fx = c->fx; tg.fy = c->fy; tg.cx = c->cx; tg.cy = c->cy; }
+  else {
+    tg.W = (c->W + 1) / 2; tg.H = (c->H + 1) / 2;
+    tg.fx = c->fx * 0.5f; tg.fy = c->fy * 0.5f; tg.cx = (c->cx - 0.5f) * 0.5f; tg.cy = (c->cy - 0.5f) * 0.5f;
+  }
+  tg.Wf = (float)tg.W; tg.Hf = (float)tg.H;
   fc.lambda1 = c->prm.lambda1; fc.lambda2 = c->prm.lambda2;
   for (int j = 0; j < 3; ++j) fc.bg[j] = c->prm.bg[j];
   fc.n = c->n; fc.max_pairs = c->max_pairs; fc.sh_degree = c->deg; fc.ftype = ftype;
@@ -543,6 +551,7 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   const std::string name(nm);
   const DevBuffers& b = c->b;
   const size_t N = c->n, px = (size_t)c->W * c->H, T = (size_t)c->TX * c->TY;
+  const size_t tpx = c->fc.tg.W > 0 ? (size_t)c->fc.tg.W * c->fc.tg.H : px;   // TGB grid of the last frame (R43)
   const void* src = nullptr; size_t have = 0;
   if (name == "keys" || name == "vals") {
     if (!c->have_frame) return TGS_E_INVALID_ARG;
@@ -573,9 +582,9 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   else if (name == "tiles_touched") { src = b.tiles_touched; have = N * 4; }
   else if (name == "ranges") { src = b.ranges; have = T * 8; }
   else if (name == "tile_order") { src = b.tile_order; have = T * 4; }
-  else if (name == "warp_depth") { src = b.warp_depth; have = px * 4; }
-  else if (name == "warp_sigma") { src = b.warp_sigma; have = px * 4; }
-  else if (name == "fill_depth") { src = b.fill_depth; have = px * 4; }
+  else if (name == "warp_depth") { src = b.warp_depth; have = tpx * 4; }
+  else if (name == "warp_sigma") { src = b.warp_sigma; have = tpx * 4; }
+  else if (name == "fill_depth") { src = b.fill_depth; have = tpx * 4; }
   else if (name == "rendered") { src = b.rendered; have = N; }
   else if (name == "prior_depth") { src = b.depth[c->prior_idx]; have = px * 4; }
   else if (name == "prior_sigma") { src = b.sigma[c->prior_idx]; have = px * 4; }

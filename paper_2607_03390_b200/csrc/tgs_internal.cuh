@@ -21,8 +21,17 @@ struct CamConst {
   int W, H, TX, TY;
 };
 
+// TGB grid of an S frame (R43): ds = 1: the image grid and the camera's intrinsics; ds = 2: ceil(W/2) x
+// ceil(H/2), grid pixel (i, j) at the image position (2i + 0.5, 2j + 0.5) = a pinhole camera with fx/2, fy/2,
+// (cx - 0.5)/2, (cy - 0.5)/2.  Source value of a grid pixel: nearest valid depth / largest sigma of its 2x2 block.
+struct TgbGrid {
+  int ds, W, H;
+  float Wf, Hf, fx, fy, cx, cy;
+};
+
 struct FrameConst {
   CamConst cam;
+  TgbGrid tg;
   float M[12];              // reference -> current (Eq.3)
   float Minv[12];           // current -> reference (backward query, L121)
   float lambda1, lambda2;   // L99

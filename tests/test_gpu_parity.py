@@ -142,6 +142,28 @@ def test_layered_scene_config5_reduced():
     assert sg["n_toc"] > 0.2 * sc.n
 
 
+@pytest.mark.parametrize("size", [(320, 180), (333, 187)])
+def test_half_resolution_tgb(size):
+    """tgb_downscale = 2 (R43): warped / repaired TGB on the half grid bit-exact, T^um from 8x8 grid
+    pixels per tile, TOC lookups in 2x2 blocks, stitch with the block depth; even and odd image sizes."""
+    P = _p()
+    sc = make_config(5, n=60_000, frames=12, width=size[0], height=size[1])
+    sc.scales[:, :2] *= 6.0
+    g, o = P.make_pair(sc, {"tgb_downscale": 2})
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(P.MODE_G["full"]); o.render(ora.FULL)
+    P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    P.inject_priors(g, o)
+    partial = 0
+    for f in (1, 2, 3):
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G["temporal"]); assert o.render(ora.TEMPORAL) == ora.FRAME_S
+        sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+        assert g.debug_get("warp_depth").size == ((size[0] + 1) // 2) * ((size[1] + 1) // 2)
+        partial += 0 < sg["n_sel"] < sg["n_tiles"]
+    assert partial >= 1 and sg["n_toc"] > 0.1 * sc.n
+
+
 def test_chained_priors_policy():
     """prior_policy = CHAINED (R42): every S frame starts from the oracle's current priors (injected), is compared in
     full, and must then have committed its own outputs: priors = the frame's stitched image / depth / sigma, pose of
