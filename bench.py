@@ -367,6 +367,11 @@ def run_ablation(args):
         "eta=0.2": variant(eta=0.2), "eta=0.6": variant(eta=0.6),
         "lambda_sr=2": variant(lambda_sr=2), "lambda_sr=10": variant(lambda_sr=10),
         "lambda_tdc=25": variant(lambda_tdc=25), "lambda_tdc=75": variant(lambda_tdc=75),
+        # the paper's large-scene setting (L142) and the chained prior policy (R42, drift vs ANCHORED)
+        "tgb_downscale=2": variant(tgb_downscale=2),
+        "prior_policy=CHAINED": variant(prior_policy=1),
+        "CHAINED, lambda_sr=10": variant(prior_policy=1, lambda_sr=10),
+        "CHAINED + tgb_downscale=2": variant(prior_policy=1, tgb_downscale=2),
     }
     return {"metric": "ablation: FPS / PSNR(S vs full) / share of S frames per variant", "config": {"workload": f"config {args.config} ({sc.name})"},
             "steps": K, "warmup": W, "data": "synthetic", "ablation": rows}

@@ -114,6 +114,13 @@ void tgs_destroy(tgs_ctx*);
 int tgs_load_gaussians(tgs_ctx*, uint32_t n, int sh_degree, const float* means, const float* scales,
                        const float* quats, const float* opacity, const float* sh, int mem);
 
+/* load a trained 3DGS checkpoint in the public `point_cloud.ply` layout (binary_little_endian, float32
+ * vertex properties x y z, f_dc_0..2, f_rest_* (channel-major, 3 ((deg+1)^2 - 1) of them, consecutive), opacity (logit),
+ * scale_0..2 (log), rot_0..3 (w x y z); other properties are ignored).  `path` is a host file name.  The rows are
+ * uploaded as they are and activated on the device (exp, sigmoid, SH re-interleaved), then loaded exactly like
+ * tgs_load_gaussians.  TGS_E_INVALID_ARG: unreadable / malformed file or a non-finite value; tgs_last_error says which. */
+int tgs_load_ply(tgs_ctx*, const char* path);
+
 /* Camera of the NEXT frame (W, K).  Changing W, H or the intrinsics invalidates the priors. */
 int tgs_set_camera(tgs_ctx*, const float view[16], float fx, float fy, float cx, float cy, int W, int H,
                    float znear, float zfar);

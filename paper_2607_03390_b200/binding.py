@@ -20,7 +20,7 @@ OK, E_INVALID_ARG, E_NO_SCENE, E_NO_CAMERA, E_NO_PRIORS, E_CAPACITY, E_CUDA = 0,
 CULL_NEAR, CULL_AFC, CULL_TOC, CULL_DEGENERATE, CULL_EMPTY, VISIBLE, NEWLY_VISIBLE = 1, 2, 4, 8, 16, 32, 64
 DEPTH_INVALID = np.float32(3.0e38)
 
-EXPORTS = ["tgs_create", "tgs_destroy", "tgs_load_gaussians", "tgs_set_camera", "tgs_default_params", "tgs_set_params",
+EXPORTS = ["tgs_create", "tgs_destroy", "tgs_load_gaussians", "tgs_load_ply", "tgs_set_camera", "tgs_default_params", "tgs_set_params",
            "tgs_render", "tgs_read_image", "tgs_read_image_async", "tgs_wait_reads", "tgs_read_depth", "tgs_read_tile_mask", "tgs_get_stats", "tgs_reset_priors",
            "tgs_strerror", "tgs_last_error", "tgs_debug_get", "tgs_debug_put", "tgs_debug_run_stage"]
 
@@ -75,6 +75,7 @@ def lib():
         L.tgs_default_params.argtypes = [C.POINTER(TgsParams)]
         L.tgs_default_params.restype = None
         L.tgs_set_params.argtypes = [vp, C.POINTER(TgsParams)]
+        L.tgs_load_ply.argtypes = [vp, C.c_char_p]
         L.tgs_render.argtypes = [vp, C.c_int]
         L.tgs_read_image.argtypes = [vp, vp, C.c_int]
         L.tgs_read_image_async.argtypes = [vp, vp]
@@ -155,6 +156,10 @@ class Context:
         self.n = int(arrs[0][0].shape[0])
         rc = self.L.tgs_load_gaussians(self.h, self.n, sh_degree, *[C.c_void_p(p) for _, p in arrs], mems.pop())
         return self._chk(rc, "tgs_load_gaussians")
+
+    def load_ply(self, path):
+        """Trained 3DGS checkpoint (`point_cloud.ply`); returns (n, sh_degree) is not needed: stats carry n_total."""
+        return self._chk(self.L.tgs_load_ply(self.h, str(path).encode()), "tgs_load_ply")
 
     def load_scene(self, sc):
         return self.load_gaussians(sc.means, sc.scales, sc.quats, sc.opacity, sc.sh, sc.sh_degree)

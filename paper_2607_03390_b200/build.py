@@ -26,6 +26,7 @@ SOURCES = {
     "k_bin.cu": ["-fmad=false"],       # the tile test is decision arithmetic (decide_math.cuh)       # k_emit repeats the tile test of k_count_color (decide_math.cuh)
     "k_sort.cu": [],
     "k_blend.cu": [],
+    "tgs_ply.cu": [],
 }
 
 

@@ -332,6 +332,11 @@ int tgs_set_params(tgs_ctx* c, const tgs_params* p) {
   return TGS_OK;
 }
 
+// accessors for tgs_ply.cu (the context is defined in this file only)
+int tgs_ply_report(tgs_ctx* c, const char* msg) { snprintf(c->err, sizeof(c->err), "%s", msg); return 0; }
+cudaStream_t tgs_ply_stream(tgs_ctx* c) { return c->stream; }
+int tgs_ply_device(tgs_ctx* c) { return c->device; }
+
 int tgs_reset_priors(tgs_ctx* c) {
   if (!c) return TGS_E_INVALID_ARG;
   invalidate_priors(c);

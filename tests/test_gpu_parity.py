@@ -9,6 +9,7 @@ import numpy as np
 import pytest
 
 from oracle import ora
+from oracle.ora import Oracle
 from synth import Camera, make_config, look_at
 
 pytestmark = pytest.mark.gpu
@@ -389,6 +390,45 @@ def test_async_readback_matches_blocking_read():
     for f in range(len(sc.poses)):
         assert np.array_equal(bufs[f].numpy(), ref[f]), f
     assert b.get_stats()["frame_type"] in (tgs.FRAME_S, tgs.FRAME_P)
+
+
+def test_load_ply_checkpoint(tmp_path):
+    """f4: tgs_load_ply (device-side activations) against the oracle's reader of the same file; the rendered frame must
+    agree like any other frame; malformed files are rejected."""
+    from oracle.ply import read_ply
+    from ply_fixture import write_ply
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(2, n=20_000, frames=3, width=320, height=180)
+    path = tmp_path / "point_cloud.ply"
+    write_ply(path, sc.means, sc.scales, sc.quats, sc.opacity, sc.sh)
+    d = read_ply(path)
+    g, o = tgs.Context(0), Oracle()
+    g.load_ply(path)
+    o.load_gaussians(d["means"], d["scales"], d["quats"], d["opacity"], d["sh"], d["sh_degree"])
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so = g.get_stats(), o.stats()
+    assert sg["n_total"] == sc.n == so["n_total"]
+    # expf on the device vs exp in double: scales / opacities differ by an ulp, so a handful of decisions may flip
+    assert abs(int(sg["n_visible"]) - int(so["n_visible"])) <= 3 and abs(int(sg["n_pairs"]) - int(so["n_pairs"])) <= 1e-3 * so["n_pairs"] + 5
+    err = np.abs(g.read_image() - o.read_image()).max(-1)
+    assert np.quantile(err, 0.999) <= 2e-3 and err.max() <= 1.2e-2
+    # same scene through tgs_load_gaussians with the oracle-activated arrays
+    g2 = tgs.Context(0)
+    g2.load_gaussians(d["means"], d["scales"], d["quats"], d["opacity"], d["sh"], d["sh_degree"])
+    g2.set_camera(sc.poses[0], sc.camera); g2.render(tgs.FULL)
+    assert np.abs(g2.read_image() - g.read_image()).max() <= 2e-3
+    # error behaviour
+    assert g.L.tgs_load_ply(g.h, str(tmp_path / "missing.ply").encode()) == -1
+    raw = open(path, "rb").read()
+    open(tmp_path / "short.ply", "wb").write(raw[:-100])
+    assert g.L.tgs_load_ply(g.h, str(tmp_path / "short.ply").encode()) == -1
+    open(tmp_path / "ascii.ply", "wb").write(raw.replace(b"binary_little_endian", b"ascii"))
+    assert g.L.tgs_load_ply(g.h, str(tmp_path / "ascii.ply").encode()) == -1
+    bad = bytearray(raw); bad[-4:] = np.float32(np.nan).tobytes()
+    open(tmp_path / "nan.ply", "wb").write(bytes(bad))
+    assert g.L.tgs_load_ply(g.h, str(tmp_path / "nan.ply").encode()) == -1
 
 
 # ------------------------------------------------------------------------------------------------ full size

@@ -826,3 +826,46 @@ def test_r41_eta_rule_only_with_selective_rendering():
     R, P, S = ora.FRAME_R, ora.FRAME_P, ora.FRAME_S
     assert types[0] == [R, S, S, S, S, P, S, S, S, S]               # 80 % S frames
     assert types[1][:4] == [R, S, P, S]                             # sparse cloud: every tile unmatched -> forced P
+
+
+# ----------------------------------------------------------------------------------------- f4: checkpoint loader
+def test_f4_read_ply_hand_written_file(tmp_path):
+    """Closed forms of the activations and the channel-major f_rest order, on a file written byte by byte here."""
+    import struct
+    from oracle.ply import read_ply
+    K = 4
+    names = ["x", "y", "z", "f_dc_0", "f_dc_1", "f_dc_2"] + [f"f_rest_{i}" for i in range(9)] + ["opacity", "scale_0", "scale_1", "scale_2",
+                                                                                                 "rot_0", "rot_1", "rot_2", "rot_3", "extra"]
+    ln3 = math.log(3.0)
+    v0 = [1.0, 2.0, 3.0, 0.1, 0.2, 0.3] + [100.0 + i for i in range(9)] + [0.0, 0.0, ln3, math.log(0.5), 1.0, 0.0, 0.0, 0.0, 7.0]
+    v1 = [-1.0, 0.5, 9.0, 0.4, 0.5, 0.6] + [200.0 + i for i in range(9)] + [ln3, -ln3, 0.0, ln3, 0.0, 2.0, 0.0, 0.0, 7.0]
+    path = tmp_path / "hand.ply"
+    with open(path, "wb") as f:
+        f.write(b"ply\nformat binary_little_endian 1.0\ncomment hand written\nelement vertex 2\n")
+        for nm in names:
+            f.write(f"property float {nm}\n".encode())
+        f.write(b"end_header\n")
+        f.write(struct.pack("<%df" % len(v0), *v0) + struct.pack("<%df" % len(v1), *v1))
+    d = read_ply(path)
+    assert d["sh_degree"] == 1 and d["sh"].shape == (2, K, 3)
+    np.testing.assert_allclose(d["means"], [[1, 2, 3], [-1, 0.5, 9]])
+    np.testing.assert_allclose(d["scales"], [[1.0, 3.0, 0.5], [1 / 3.0, 1.0, 3.0]], rtol=1e-6)
+    np.testing.assert_allclose(d["opacity"], [0.5, 0.75], rtol=1e-6)
+    np.testing.assert_allclose(d["quats"], [[1, 0, 0, 0], [0, 2, 0, 0]])          # not normalised here
+    np.testing.assert_allclose(d["sh"][0, 0], [0.1, 0.2, 0.3], rtol=1e-6)
+    for ch in range(3):
+        for k in range(1, K):
+            assert d["sh"][0, k, ch] == 100.0 + ch * 3 + (k - 1) and d["sh"][1, k, ch] == 200.0 + ch * 3 + (k - 1)
+
+
+def test_f4_ply_round_trip_of_a_synthetic_scene(tmp_path):
+    from oracle.ply import read_ply
+    from ply_fixture import write_ply
+    sc = make_config(2, n=3000, frames=2)
+    path = tmp_path / "scene.ply"
+    write_ply(path, sc.means, sc.scales, sc.quats, sc.opacity, sc.sh)
+    d = read_ply(path)
+    assert d["sh_degree"] == sc.sh_degree
+    np.testing.assert_array_equal(d["means"], sc.means); np.testing.assert_array_equal(d["sh"], sc.sh)
+    np.testing.assert_array_equal(d["quats"], sc.quats)
+    np.testing.assert_allclose(d["scales"], sc.scales, rtol=1e-6); np.testing.assert_allclose(d["opacity"], sc.opacity, rtol=1e-5, atol=1e-7)
