@@ -32,8 +32,8 @@ METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full r
 # counts as 1) + 1 MUFU.EX2 + 8 on the ALU pipe (clamp, 2 threshold tests, first-contribution test, 4 selects).
 BLEND_LANE_INSTR = 21.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_blend<1,0> launch on config 3, from the ncu --set full capture
-# summarised in profiles/ (the file names the command); per launch, like `achieved`.
-BLEND_DRAM_TRAFFIC_BYTES = 45.7e6
+# summarised in profiles/r1c_top_kernels.md (the file names the command); per launch, like `achieved`.
+BLEND_DRAM_TRAFFIC_BYTES = 46.0e6
 
 
 def _peaks():
@@ -109,6 +109,18 @@ def trajectory_pose(sc, f):
     F = len(sc.poses)
     k = f % (2 * F - 2) if F > 1 else 0
     return sc.poses[k if k < F else 2 * F - 2 - k]
+
+
+def _ssim(a, b):
+    """Mean SSIM of two [H][W][3] images in [0,1] (the paper's second quality metric, L138): Gaussian window sigma 1.5,
+    C1 = 0.01^2, C2 = 0.03^2, per channel, on the host with scipy.  Reported only (quality is unpinned)."""
+    from scipy.ndimage import gaussian_filter
+    a, b = a.astype(np.float64), b.astype(np.float64)
+    f = lambda x: gaussian_filter(x, sigma=(1.5, 1.5, 0), truncate=3.5)
+    ma, mb = f(a), f(b)
+    va, vb, cab = f(a * a) - ma * ma, f(b * b) - mb * mb, f(a * b) - ma * mb
+    c1, c2 = 0.01 ** 2, 0.03 ** 2
+    return float((((2 * ma * mb + c1) * (2 * cab + c2)) / ((ma * ma + mb * mb + c1) * (va + vb + c2))).mean())
 
 
 def run_ours(args):
@@ -197,7 +209,7 @@ def run_ours(args):
         per_type[st["frame_type"]].append(st)
     ctx.debug_run_stage("count_interactions_off")
     # PSNR of S frames against the full render of the same pose (reported; unpinned by the paper)
-    psnr = []
+    psnr, ssim = [], []
     ctx.reset_priors()
     ref_ctx = tgs.Context(local, stream.cuda_stream)
     ref_ctx.load_scene(sc)
@@ -207,8 +219,10 @@ def run_ours(args):
         if ctx.get_stats()["frame_type"] == tgs.FRAME_S:
             ref_ctx.set_camera(trajectory_pose(sc, f), cam)
             ref_ctx.render(tgs.FULL)
-            mse = float(((ctx.read_image() - ref_ctx.read_image()) ** 2).mean())
+            a, b = ctx.read_image(), ref_ctx.read_image()
+            mse = float(((a - b) ** 2).mean())
             psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
+            ssim.append(_ssim(a, b))
     ref_ctx.destroy()
 
     if rank != 0:
@@ -288,12 +302,13 @@ def run_ours(args):
                    "l2": "scene arrays (>= 700 MB) exceed the 126 MB L2; no explicit flush", "parallelism": "replicas only"},
         "fps_full_render": fps_full, "ms_per_step_full_render": ms_full / K, "speedup_vs_full_render": fps_tgs / fps_full,
         "psnr_S_vs_full_dB": float(np.mean(psnr)) if psnr else None,
+        "ssim_S_vs_full": float(np.mean(ssim)) if ssim else None,
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 16 * 4 + 8 * 4, "d2h_bytes_per_step": cam.W * cam.H * 3 * 4,
                 "note": "camera by value through tgs_set_camera; every frame's image copied to pinned host memory (tgs_read_image_async: the copy of frame f overlaps the rendering of frame f+1), all copies complete inside the timed region"},
         "gpu_launches": None,
         "stages": stages, "roofline": roof, "stage_rooflines": stage_roof, "clocks": clocks,
     }
-    # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), fix_ties, scan_area, bin,
+    # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), compact_vis, scan_area, bin,
     # colour, tile sort (digits), ranges, blend = 12 + tile digits; + frustum on R / P; + warp, fill_corr, mark_oc,
     # select on S
     T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
