@@ -176,16 +176,19 @@ __device__ __forceinline__ bool tile_reach(const GaussParams& P, uint32_t tx, ui
 }
 
 // ---- k_bin: tests, ranks (single-pass scan with decoupled look-back over the chunks) and pairs of one chunk
+// TileT: uint16_t when every tile id fits (T <= 65536: up to 4K images), which lets 8 CTAs share an SM; else uint32_t, 7
+template <typename TileT>
 struct BinSmem {
   uint32_t prefix[BIN_CHUNK + 2];       // area_prefix of the Gaussians of this chunk (+ sentinel)
-  uint32_t st_tile[BIN_CHUNK];          // passing tests of the chunk, in order: tile id
-  uint32_t st_g[BIN_CHUNK];             //                                        Gaussian
+  TileT st_tile[2][BIN_CHUNK];          // passing tests of a chunk, in order: tile id (double buffered: pipeline)
+  uint32_t st_g[2][BIN_CHUNK];          //                                      Gaussian
   GaussParams gp[BIN_PCAP];
   uint32_t warp[BIN_THREADS / 32];
   uint32_t excl, chunk;
-  uint32_t hist[2][256];                // digit histograms of the tile ids of the emitted pairs (for the tile sort)
+  uint32_t hist[sizeof(TileT) == 2 ? 2 : 3][256];   // digit histograms of the tile ids of the emitted pairs (for the tile sort)
 };
 
+template <typename TileT>
 __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
                                                      const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
                                                      const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
@@ -195,95 +198,122 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
                                                      Counters* __restrict__ counters) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
-  __shared__ BinSmem sm;
+  __shared__ BinSmem<TileT> sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
   const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
   const uint32_t tid = threadIdx.x, lane = tid & 31;
   const int TX = fc.cam.TX;
   const bool exact = fc.exact_tiles != 0;
-  for (int i = tid; i < 2 * 256; i += BIN_THREADS) (&sm.hist[0][0])[i] = 0;
+  constexpr int NH = sizeof(TileT) == 2 ? 2 : 3;      // digits of a tile id (ids up to 2^24 with 32-bit staging)
+  for (int i = tid; i < NH * 256; i += BIN_THREADS) (&sm.hist[0][0])[i] = 0;
+  // Software pipeline over the chunks of this CTA: the tests of chunk k+1 run BEFORE the look-back of chunk k.  A chunk
+  // publishes its aggregate right after its tests; by the time its CTA has tested another chunk, the predecessors'
+  // aggregates are there, so the look-back does not spin on stragglers (profiles/r1c: 41 % of the warp samples of the
+  // unpipelined kernel sat at the barrier behind a polling warp 0).  Passing tests wait in a double-buffered stage.
+  uint32_t pend = 0xffffffffu, pend_total = 0, it = 0;
   while (true) {
     __syncthreads();
     if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin, 1u);
     __syncthreads();
     const uint32_t chunk = sm.chunk;
-    if (chunk >= num_chunks) break;
-    const uint32_t cbase = chunk * BIN_CHUNK;
-    const uint32_t tend = (total_tests - cbase < (uint32_t)BIN_CHUNK) ? total_tests : cbase + BIN_CHUNK;
-    const uint32_t i_first = chunk_first[chunk];
-    const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
-    const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
-    for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
-    for (uint32_t i = tid; i < m && i < (uint32_t)BIN_PCAP; i += BIN_THREADS)
-      sm.gp[i] = load_params(sorted_g[i_first + i], exact, rec_rect, rec_uvdo, rec_conic);
-    __syncthreads();
-    // ---------------------------------------------------------------- tests
-    const uint32_t t0 = cbase + tid * BIN_IPT;
-    uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
-    if (t0 < tend) {
-      uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
-      while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
-      uint32_t li = lo, segcnt = 0, end, rx, ry, x_lo, y_lo;
-      GaussParams G;
-      auto load = [&](uint32_t l, uint32_t t) {
-        G = l < (uint32_t)BIN_PCAP ? sm.gp[l] : load_params(sorted_g[i_first + l], exact, rec_rect, rec_uvdo, rec_conic);
-        end = sm.prefix[l + 1];
-        const uint32_t local = t - sm.prefix[l];
-        ry = local / G.w; rx = local - ry * G.w;
-        x_lo = G.lo & 0xffffu; y_lo = G.lo >> 16;
-      };
-      auto flush = [&]() {
-        if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
-        segcnt = 0;
-      };
-      load(li, t0);
+    const bool have = chunk < num_chunks;
+    const uint32_t buf = it & 1u;
+    uint32_t total = 0;
+    if (have) {
+      const uint32_t cbase = chunk * BIN_CHUNK;
+      const uint32_t tend = (total_tests - cbase < (uint32_t)BIN_CHUNK) ? total_tests : cbase + BIN_CHUNK;
+      const uint32_t i_first = chunk_first[chunk];
+      const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
+      const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
+      for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
+      for (uint32_t i = tid; i < m && i < (uint32_t)BIN_PCAP; i += BIN_THREADS)
+        sm.gp[i] = load_params(sorted_g[i_first + i], exact, rec_rect, rec_uvdo, rec_conic);
+      __syncthreads();
+      // -------------------------------------------------------------- tests
+      const uint32_t t0 = cbase + tid * BIN_IPT;
+      uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
+      if (t0 < tend) {
+        uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
+        while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
+        uint32_t li = lo, segcnt = 0, end, rx, ry, x_lo, y_lo;
+        GaussParams G;
+        auto load = [&](uint32_t l, uint32_t t) {
+          G = l < (uint32_t)BIN_PCAP ? sm.gp[l] : load_params(sorted_g[i_first + l], exact, rec_rect, rec_uvdo, rec_conic);
+          end = sm.prefix[l + 1];
+          const uint32_t local = t - sm.prefix[l];
+          ry = local / G.w; rx = local - ry * G.w;
+          x_lo = G.lo & 0xffffu; y_lo = G.lo >> 16;
+        };
+        auto flush = [&]() {
+          if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
+          segcnt = 0;
+        };
+        load(li, t0);
 #pragma unroll
-      for (int k = 0; k < BIN_IPT; ++k) {
-        const uint32_t t = t0 + k;
-        if (t < tend) {
-          if (t >= end) { flush(); do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
-          const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
-          bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
-          if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
-          if (pass) { mask |= 1u << k; ++segcnt; }
-          tl[k] = tile; gg[k] = G.g;
-          if (++rx == G.w) { rx = 0; ++ry; }
+        for (int k = 0; k < BIN_IPT; ++k) {
+          const uint32_t t = t0 + k;
+          if (t < tend) {
+            if (t >= end) { flush(); do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
+            const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
+            bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
+            if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
+            if (pass) { mask |= 1u << k; ++segcnt; }
+            tl[k] = tile; gg[k] = G.g;
+            if (++rx == G.w) { rx = 0; ++ry; }
+          }
         }
+        flush();
       }
-      flush();
-    }
-    // ---------------------------------------------------------------- rank the passing tests (chunk-local + global)
-    uint32_t incl_total;
-    const uint32_t goff = tgs_scan::chunk_scan<BIN_THREADS>(__popc(mask), chunk, desc, sm.warp, &sm.excl, &counters->error, &incl_total, fc.epoch);
-    const uint32_t cexcl = sm.excl, ctotal = incl_total - cexcl;
-    const bool overflow = incl_total > fc.max_pairs;
-    if (chunk == num_chunks - 1 && tid == 0) {
-      if (overflow) { counters->overflow = 1; counters->n_pairs = 0; }
-      else counters->n_pairs = incl_total;
-    }
-    uint32_t lpos = goff - cexcl;
+      // -------------------------------------------------------------- chunk-local ranks, stage, publish the aggregate
+      const uint32_t cnt = __popc(mask);
+      uint32_t incl = cnt;
 #pragma unroll
-    for (int k = 0; k < BIN_IPT; ++k)
-      if ((mask >> k) & 1u) { sm.st_tile[lpos] = tl[k]; sm.st_g[lpos] = gg[k]; ++lpos; }
-    __syncthreads();
-    if (!overflow)
-      for (uint32_t p0 = 0; p0 < ctotal; p0 += BIN_THREADS) {
-        const uint32_t p = p0 + tid;
-        const bool in = p < ctotal;
-        const uint32_t tile = in ? sm.st_tile[p] : 0xffffffffu;
-        if (in) { keys[cexcl + p] = tile; vals[cexcl + p] = sm.st_g[p]; atomicAdd(&sm.hist[0][tile & 255u], 1u); }
-        // upper digit: consecutive pairs are consecutive tiles of one Gaussian, so it comes in runs: one atomic per run
-        const uint32_t hi = tile >> 8, prev = __shfl_up_sync(0xffffffffu, hi, 1);
-        const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || hi != prev);
-        if (in && ((heads >> lane) & 1u)) {
-          const uint32_t above = heads & ~((2u << lane) - 1u);               // heads of later runs
-          const uint32_t run = (above ? (uint32_t)__ffs(above) - 1u : 32u) - lane;
-          atomicAdd(&sm.hist[1][hi & 255u], run);
-        }
+      for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
+      if (lane == 31) sm.warp[tid >> 5] = incl;
+      __syncthreads();
+      uint32_t lpos = incl - cnt;
+#pragma unroll
+      for (int w = 0; w < BIN_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < (tid >> 5)) lpos += t; total += t; }
+      if (tid == 0) tgs_scan::publish_aggregate(total, chunk, desc, fc.epoch);
+#pragma unroll
+      for (int k = 0; k < BIN_IPT; ++k)
+        if ((mask >> k) & 1u) { sm.st_tile[buf][lpos] = (TileT)tl[k]; sm.st_g[buf][lpos] = gg[k]; ++lpos; }
+    }
+    // ---------------------------------------------------------------- finish the chunk tested one round ago
+    if (pend != 0xffffffffu) {
+      if (tid < 32) {
+        const uint32_t e = tgs_scan::lookback_warp(pend_total, pend, desc, &counters->error, fc.epoch, false);
+        if (lane == 0) sm.excl = e;
       }
+      __syncthreads();
+      const uint32_t cexcl = sm.excl, ctotal = pend_total, incl_total = cexcl + ctotal, pbuf = buf ^ 1u;
+      const bool overflow = incl_total > fc.max_pairs;
+      if (pend == num_chunks - 1 && tid == 0) {
+        if (overflow) { counters->overflow = 1; counters->n_pairs = 0; }
+        else counters->n_pairs = incl_total;
+      }
+      if (!overflow)
+        for (uint32_t p0 = 0; p0 < ctotal; p0 += BIN_THREADS) {
+          const uint32_t p = p0 + tid;
+          const bool in = p < ctotal;
+          const uint32_t tile = in ? (uint32_t)sm.st_tile[pbuf][p] : 0xffffffffu;
+          if (in) { keys[cexcl + p] = tile; vals[cexcl + p] = sm.st_g[pbuf][p]; atomicAdd(&sm.hist[0][tile & 255u], 1u); }
+          // upper digit: consecutive pairs are consecutive tiles of one Gaussian, so it comes in runs: one atomic per run
+          const uint32_t hi = tile >> 8, prev = __shfl_up_sync(0xffffffffu, hi, 1);
+          const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || hi != prev);
+          if (in && ((heads >> lane) & 1u)) {
+            const uint32_t above = heads & ~((2u << lane) - 1u);               // heads of later runs
+            const uint32_t run = (above ? (uint32_t)__ffs(above) - 1u : 32u) - lane;
+            atomicAdd(&sm.hist[1][hi & 255u], run);
+          }
+          if (NH == 3 && in) atomicAdd(&sm.hist[NH - 1][(tile >> 16) & 255u], 1u);
+        }
+    }
+    if (!have) break;
+    pend = chunk; pend_total = total; ++it;
   }
   __syncthreads();
-  for (int i = tid; i < 2 * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
+  for (int i = tid; i < NH * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
 }
 
 // ================================================================== A5c: SH -> RGB of the Gaussians that emitted pairs
@@ -340,7 +370,11 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
                                                       b.counters, max_tests);
-  TGS_LAUNCH((k_bin), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
+  if (fc.n_tiles <= 65536)
+    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
+                                                          (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+  else
+    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
                                                           (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
 }
 

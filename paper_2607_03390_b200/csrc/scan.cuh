@@ -20,13 +20,19 @@ __device__ __forceinline__ void st_volatile64(unsigned long long* p, unsigned lo
 
 // Exclusive prefix over all earlier chunks of this chunk's `total` (call from warp 0, all 32 lanes).
 // desc[chunk] is published as "aggregate" first and "inclusive prefix" at the end.
+// publish = false: the caller has already published the aggregate with publish_aggregate (deferred look-back).
+__device__ __forceinline__ void publish_aggregate(uint32_t total, uint32_t chunk, unsigned long long* __restrict__ desc, uint32_t epoch) {
+  const unsigned long long tag = (unsigned long long)epoch << 34;
+  st_volatile64(&desc[chunk], tag | ((chunk > 0 ? 1ull : 2ull) << 32) | total);      // chunk 0: its aggregate is its prefix
+}
+
 __device__ __forceinline__ uint32_t lookback_warp(uint32_t total, uint32_t chunk, unsigned long long* __restrict__ desc,
-                                                  uint32_t* error_flag, uint32_t epoch) {
+                                                  uint32_t* error_flag, uint32_t epoch, bool publish = true) {
   const unsigned long long tag = (unsigned long long)epoch << 34;
   const uint32_t lane = threadIdx.x & 31;
   uint32_t excl = 0;
   if (chunk > 0) {
-    if (lane == 0) st_volatile64(&desc[chunk], tag | (1ull << 32) | total);   // aggregate available
+    if (publish && lane == 0) st_volatile64(&desc[chunk], tag | (1ull << 32) | total);   // aggregate available
     int base = (int)chunk - 1;
     uint32_t polls = 0;
     while (true) {

@@ -298,6 +298,21 @@ def test_edge_whole_screen_splats():
     P.compare_frame(g, o, sc.n, ora.FRAME_S)
 
 
+def test_edge_more_than_65536_tiles():
+    """Maximum sizes: a 4112 x 4112 image has 257^2 = 66049 tiles, so tile ids need 17 bits: three digits in the tile
+    sort and the 32-bit staging instance of k_bin."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(1, n=3000, frames=1, width=4112, height=4112)
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, _ = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    assert sg["n_tiles"] == 257 * 257 and sg["n_pairs"] > 10_000
+    keys = o.get("keys")
+    assert (keys >> 32).max() > 65536              # pairs beyond the 16-bit tile ids exist
+
+
 def test_edge_needles_faint_and_equal_depths():
     """Paths that decide without the oracle's full sequence must never change a decision (R40): needle-like
     splats (cond(Sigma') >> 400: no test-rect shrink), opacities around 1/255 (tau < 0.5 and tau < 0), off-screen
