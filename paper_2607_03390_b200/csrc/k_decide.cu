@@ -240,7 +240,7 @@ struct PreSmem {
   uint32_t hist[4][256];        // digit histograms of the depth keys of the visible Gaussians (for the depth sort)
 };
 
-__global__ void __launch_bounds__(PRE_THREADS, 3) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
+__global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
                                                                const uint8_t* __restrict__ rendered, const float* __restrict__ warp_depth,
                                                                const float* __restrict__ warp_sigma, const uint32_t* __restrict__ F_key,
                                                                float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
@@ -513,38 +513,38 @@ __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* 
   __shared__ uint32_t s_sel[32], s_oc[32], s_um[32];
   const int T = fc.n_tiles;
   const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int words = (T + 31) / 32, wpt = (words + 1023) / 1024;      // bit-set words per thread
-  const int t0 = threadIdx.x * wpt * 32, t1 = min(T, t0 + wpt * 32);
-  uint32_t nsel = 0, noc = 0, num = 0;
-  for (int t = t0; t < t1; t += 32) {
-    uint32_t word = 0;
-    for (int i = 0; i < 32 && t + i < T; ++i) {
-      const uint32_t f = tile_flags[t + i] & 3u;
-      const bool sel = fc.all_tiles || f != 0;
-      tile_mask[t + i] = (uint8_t)(f | (sel ? 4u : 0u));
-      word |= (sel ? 1u : 0u) << i;
-      noc += f & 1u; num += (f >> 1) & 1u;
-    }
-    sel_bits[t >> 5] = word;
+  // a warp owns a run of consecutive 32-tile words; a lane owns one tile of a word (coalesced loads, ballots)
+  const int words = (T + 31) / 32, wpw = (words + 31) / 32;
+  const int w0 = min(words, (int)wid * wpw), w1 = min(words, w0 + wpw);
+  uint32_t nsel = 0, noc = 0, num = 0;                     // warp-uniform
+  for (int w = w0; w < w1; ++w) {
+    const int t = w * 32 + (int)lane;
+    const uint32_t f = t < T ? tile_flags[t] & 3u : 0u;
+    const bool sel = t < T && (fc.all_tiles || f != 0);
+    if (t < T) tile_mask[t] = (uint8_t)(f | (sel ? 4u : 0u));
+    const uint32_t word = __ballot_sync(0xffffffffu, sel);
+    if (lane == 0) sel_bits[w] = word;
     nsel += __popc(word);
+    noc += __popc(__ballot_sync(0xffffffffu, (f & 1u) != 0)); num += __popc(__ballot_sync(0xffffffffu, (f & 2u) != 0));
   }
-  // block-wide exclusive scan of nsel; totals of noc, num
-  uint32_t incl = nsel;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
-  noc = warp_sum(noc); num = warp_sum(num);
-  if (lane == 31) s_sel[wid] = incl;
-  if (lane == 0) { s_oc[wid] = noc; s_um[wid] = num; }
+  if (lane == 0) { s_sel[wid] = nsel; s_oc[wid] = noc; s_um[wid] = num; }
   __syncthreads();
-  uint32_t before = incl - nsel, total = 0, toc = 0, tum = 0;
+  uint32_t before = 0, total = 0, toc = 0, tum = 0;
 #pragma unroll
   for (int w = 0; w < 32; ++w) { const uint32_t v = s_sel[w]; if ((uint32_t)w < wid) before += v; total += v; toc += s_oc[w]; tum += s_um[w]; }
   if (threadIdx.x == 0) { counters->n_sel = total; counters->n_sel_oc = toc; counters->n_sel_um = tum; }
-  // selected tiles of this thread's run at [before, ...), the others at total + (t0 - before) ...
-  uint32_t ps = before, pn = total + ((uint32_t)min(t0, T) - before);
-  for (int t = t0; t < t1; ++t) {
-    const bool sel = fc.all_tiles || (tile_flags[t] & 3u) != 0;
-    if (sel) tile_order[ps++] = (uint32_t)t; else tile_order[pn++] = (uint32_t)t;
+  // work order of the blend: the selected tiles in ascending id at [0, total), the others behind them in ascending id
+  uint32_t ps = before;
+  for (int w = w0; w < w1; ++w) {
+    const int t = w * 32 + (int)lane;
+    const bool sel = t < T && (fc.all_tiles || (tile_flags[t] & 3u) != 0);
+    const uint32_t word = __ballot_sync(0xffffffffu, sel);
+    const uint32_t rank = __popc(word & ((1u << lane) - 1u));
+    if (t < T) {
+      if (sel) tile_order[ps + rank] = (uint32_t)t;
+      else tile_order[total + ((uint32_t)(w * 32) - ps) + (lane - rank)] = (uint32_t)t;     // unselected tiles before t: t - selected before t
+    }
+    ps += __popc(word);
   }
 }
 
@@ -615,7 +615,7 @@ void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
 
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
-  const uint32_t grid = chunks < (uint32_t)(num_sms * 3) ? chunks : (uint32_t)(num_sms * 3);
+  const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
