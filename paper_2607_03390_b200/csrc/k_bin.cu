@@ -10,8 +10,7 @@
 // R39), ranks the passing tests with a single-pass scan (decoupled look-back over the chunks) and writes the pairs
 // (tile id, Gaussian) in exactly the oracle's emission order; the stable sort by tile id that follows (k_sort.cu)
 // then leaves every tile's list in (depth, index) order.  The same kernel counts the pairs per Gaussian and the
-// digit histograms of the tile sort; k_colour evaluates SH -> RGB (L61 "color c_i"; R5) for the Gaussians that
-// emitted at least one pair, so on S frames the SH bytes are read only for Gaussians that reach a selected tile.
+// digit histograms of the tile sort; k_colour_all evaluates SH -> RGB (L61 "color c_i"; R5) of the visible Gaussians.
 //
 // Compiled with -fmad=false: the tile test is decision arithmetic (decide_math.cuh).
 // Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory, so a
@@ -316,19 +315,25 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
   for (int i = tid; i < NH * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
 }
 
-// ================================================================== A5c: SH -> RGB of the Gaussians that emitted pairs
-// L61 "color c_i"; R5.  One thread per visible Gaussian; the 12 K bytes of SH are read only if it emitted a pair, so
-// on S frames only for Gaussians that reach a selected tile.
+// ================================================================== A5c: SH -> RGB (L61 "color c_i"; R5)
+// For every visible Gaussian, straight from the flags k_preprocess wrote: needs neither the sorted list nor the pair
+// counts, so it runs on its own stream beside the depth sort, which leaves most SMs idle.  (A variant that waited for
+// k_bin and skipped Gaussians without pairs read fewer SH bytes on S frames but could only run beside the tile sort,
+// whose CTAs fill the register file: no overlap, 20-47 us on the critical path.)
 template <int DEG>
-__global__ void __launch_bounds__(128) k_colour(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ tiles_touched,
-                                                const float4* __restrict__ cull4, const float* __restrict__ sh,
-                                                float4* __restrict__ rec_rgb, const Counters* __restrict__ counters) {
+__global__ void __launch_bounds__(128) k_colour_all(FrameConst fc, const uint32_t* __restrict__ rec_flags, const float4* __restrict__ cull4,
+                                                    const float* __restrict__ sh, float4* __restrict__ rec_rgb) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
-  const uint32_t n = counters->n_visible;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    const uint32_t g = sorted_g[i];
-    if (tiles_touched[g]) sh_colour<DEG>(fc, g, cull4, sh, rec_rgb);
+  const uint32_t n4 = (fc.n + 3) / 4;                        // rec_flags is padded to a multiple of 4
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
+    const uint4 f = reinterpret_cast<const uint4*>(rec_flags)[i];
+    const uint32_t fl[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t g = 4 * i + j;
+      if (g < fc.n && (fl[j] & TGS_VISIBLE)) sh_colour<DEG>(fc, g, cull4, sh, rec_rgb);
+    }
   }
 }
 
@@ -378,9 +383,8 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
                                                           (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
 }
 
-void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms) {
-  const uint32_t* sorted_g = b.cvals[sorted_g_idx];
-#define LAUNCH(D) TGS_LAUNCH((k_colour<D>), num_sms * 16, 128, 0, s, fc, sorted_g, b.tiles_touched, b.cull4, b.sh, b.rec_rgb, b.counters)
+void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
+#define LAUNCH(D) TGS_LAUNCH((k_colour_all<D>), num_sms * 16, 128, 0, s, fc, b.rec_flags, b.cull4, b.sh, b.rec_rgb)
   switch (fc.sh_degree) {
     case 0: LAUNCH(0); break;
     case 1: LAUNCH(1); break;

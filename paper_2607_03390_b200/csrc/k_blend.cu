@@ -97,7 +97,7 @@ __device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p
 }
 
 template <bool MARK, bool COUNT>
-__global__ void __launch_bounds__(BLEND_THREADS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
+__global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
                                                          const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,

@@ -56,8 +56,9 @@ struct tgs_ctx {
   cudaStream_t copy = nullptr;          // read-back stream of tgs_read_image_async
   cudaEvent_t ev_copy[2] = {nullptr, nullptr};   // last asynchronous read of image[i] has finished
   bool copy_pending[2] = {false, false};
-  cudaStream_t side = nullptr;          // second stream: work that is off the critical path of a frame (SH colours, A2)
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr;
+  cudaStream_t side = nullptr;          // second stream: work that is off the critical path of a frame (A2, A4)
+  cudaStream_t side2 = nullptr;         // third stream: SH colours beside the depth sort
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr, ev_fork3 = nullptr;
   bool sel_pending = false;
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
@@ -235,9 +236,10 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
   cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
+  cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking);
   cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking);
   for (auto& e : c->ev_copy) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-  for (cudaEvent_t* e : {&c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2}) cudaEventCreateWithFlags(e, cudaEventDisableTiming);
+  for (cudaEvent_t* e : {&c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2, &c->ev_fork3}) cudaEventCreateWithFlags(e, cudaEventDisableTiming);
   for (auto& e : c->ev_stage) cudaEventCreate(&e);
   *out = c;
   return TGS_OK;
@@ -252,9 +254,10 @@ void tgs_destroy(tgs_ctx* c) {
   cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
   cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
   cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
+  cudaStreamSynchronize(c->side2); cudaStreamDestroy(c->side2);
   cudaStreamSynchronize(c->copy); cudaStreamDestroy(c->copy);
   for (auto& e : c->ev_copy) cudaEventDestroy(e);
-  for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_fork2, c->ev_join2}) cudaEventDestroy(e);
+  for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_fork2, c->ev_join2, c->ev_fork3}) cudaEventDestroy(e);
   for (auto& e : c->ev_stage) cudaEventDestroy(e);
   delete c;
 }
@@ -449,16 +452,22 @@ int tgs_render(tgs_ctx* c, int mode) {
     CK(cudaEventRecord(c->ev_sel, s4));
     c->sel_pending = true;
   }
+  // SH colours of every visible Gaussian on a third stream beside the depth sort (few CTAs, most SMs idle).  Behind k_bin
+  // a colour kernel only queues up behind the tile sort, whose CTAs fill the register file (measured: no overlap).
+  const bool early_colour = fork;
+  if (early_colour) {
+    CK(cudaEventRecord(c->ev_fork3, s)); CK(cudaStreamWaitEvent(c->side2, c->ev_fork3, 0));
+    launch_colour_all(c->side2, fc, b, c->num_sms);
+    CK(cudaEventRecord(c->ev_join, c->side2));
+  }
   mark();                                                                      // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // visible Gaussians by depth
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   mark();                                                                      // 3: A5 pairs
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
-  mark();                                                                      // 4: A5 colours (beside the tile sort: only the blend needs them)
-  if (fork) { CK(cudaEventRecord(c->ev_fork, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0)); }
-  launch_colour(fork ? c->side : s, fc, b, dsorted, c->num_sms);                                           // SH -> RGB of the emitting Gaussians
-  if (fork) CK(cudaEventRecord(c->ev_join, c->side));
+  mark();                                                                      // 4: A5 colours (production: third stream, beside the depth sort)
+  if (!early_colour) launch_colour_all(s, fc, b, c->num_sms);                                             // stage timing: the production kernel, in line
   mark();                                                                      // 5: A6 level 2 + A7
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
                                  b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // pairs by tile

@@ -156,7 +156,7 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
-void launch_colour(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, int num_sms);
+void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
