@@ -446,6 +446,34 @@ def test_load_ply_checkpoint(tmp_path):
     assert g.L.tgs_load_ply(g.h, str(tmp_path / "nan.ply").encode()) == -1
 
 
+def test_repeatability_of_a_frame_stream():
+    """The path has no order-dependent arithmetic (integer atomics, fixed per-tile blend order, look-back scans): the
+    same stream rendered again must reproduce pair lists, masks and images bit for bit -- a cheap detector of races in
+    the chained scans and the software-pipelined binning."""
+    tgs = _tgs()
+    sc = make_config(3, n=400_000, frames=6, width=960, height=540)
+    g = tgs.Context(0); g.load_scene(sc)
+    p = g.default_params(); p.lambda_sr = 3; g.set_params(p)
+
+    def stream():
+        g.reset_priors()
+        out = []
+        for f in range(6):
+            g.set_camera(sc.poses[f], sc.camera); g.render(tgs.AUTO)
+            d, s_ = g.read_depth()
+            out.append((g.get_stats()["frame_type"], g.debug_get("keys").copy(), g.debug_get("vals").copy(), g.read_tile_mask().copy(),
+                        g.read_image().copy(), d.copy(), s_.copy(), g.debug_get("rendered").copy()))
+        return out
+    ref = stream()
+    assert {r[0] for r in ref} == {tgs.FRAME_R, tgs.FRAME_P, tgs.FRAME_S} or {r[0] for r in ref} >= {tgs.FRAME_R, tgs.FRAME_S}
+    for rep in range(4):
+        cur = stream()
+        for f, (a, b) in enumerate(zip(ref, cur)):
+            assert a[0] == b[0]
+            for i in range(1, 8):
+                assert np.array_equal(a[i], b[i]), (rep, f, i)
+
+
 # ------------------------------------------------------------------------------------------------ full size
 def test_full_size_config3_reference_and_temporal():
     """BASELINE.json config 3 (3 M Gaussians, SH 3, 1920x1080) in the launch configuration bench.py times: one
