@@ -267,7 +267,7 @@ def run_ours(args):
         "preprocess_select": {"bound": "hbm", "achieved": (sc.n * (16 + 4) + Nv * (32 + 16 + 100)) / t_stage[1] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
         "depth_sort": {"bound": "hbm", "achieved": Nv * 16 * 4 / t_stage[2] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
         "sh_colour": {"bound": "hbm", "achieved": Nv * (8 + 16 + 12 * (sc.sh_degree + 1) ** 2 + 16) / t_stage[4] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
-        "tile_sort_ranges": {"bound": "hbm", "achieved": P * (16 * tile_passes + 4) / t_stage[5] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
+        "tile_sort_ranges": {"bound": "hbm", "achieved": P * 16 * tile_passes / t_stage[5] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
         "blend_stitch": {"bound": "alu", "achieved": L * BLEND_LANE_INSTR / t_stage[6] / 1e12, "peak": alu_peak, "unit": "T lane-instr/s"},
     }
     for v in stage_roof.values():
@@ -309,12 +309,12 @@ def run_ours(args):
         "stages": stages, "roofline": roof, "stage_rooflines": stage_roof, "clocks": clocks,
     }
     # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), compact_vis, scan_area, bin,
-    # colour, tile sort (digits), ranges, blend = 12 + tile digits; + frustum on R / P; + warp, fill_corr, mark_oc,
-    # select on S
+    # colour, tile sort (digits, the last one writes the ranges), blend = 11 + tile digits; + frustum on R / P; + warp,
+    # fill_corr, mark_oc, select on S
     T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
     tpasses = (max(1, int(np.ceil(np.log2(T)))) + 7) // 8
     nR = sum(1 for s in all_stats if s["frame_type"] != 2)
-    base = 12 + tpasses
+    base = 11 + tpasses
     per_ref, per_s = base + 1, base + 4
     frac_ref = nR / max(1, len(all_stats))
     out["gpu_launches"] = int(round(K * (frac_ref * per_ref + (1 - frac_ref) * per_s)))

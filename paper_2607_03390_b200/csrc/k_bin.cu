@@ -338,21 +338,11 @@ __global__ void __launch_bounds__(128) k_colour_all(FrameConst fc, const uint32_
 }
 
 // ================================================================== A7: per-tile ranges
-__global__ void __launch_bounds__(256) k_ranges(const uint32_t* __restrict__ keys, const Counters* __restrict__ counters,
-                                                uint2* __restrict__ ranges, int n_tiles) {
-  TGS_PDL_WAIT();
-  TGS_PDL_TRIGGER();
-  const uint32_t n = counters->n_pairs;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    const uint32_t t = keys[i];
-    if (t >= (uint32_t)n_tiles) continue;
-    if (i == 0) ranges[t].x = 0;
-    else {
-      const uint32_t p = keys[i - 1];
-      if (p != t) { ranges[t].x = i; if (p < (uint32_t)n_tiles) ranges[p].y = i; }
-    }
-    if (i == n - 1) ranges[t].y = n;
-  }
+// Written by the last pass of the tile sort (k_sort.cu) as {~start, end}, all zero for a tile without pairs.
+// test-only: the plain {start, end} form the oracle reports ({0, 0} for an empty tile)
+__global__ void __launch_bounds__(256) k_ranges_decode(const uint2* __restrict__ ranges, int n_tiles, uint2* __restrict__ out) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < n_tiles) { const uint2 r = ranges[t]; out[t] = r.y ? make_uint2(~r.x, r.y) : make_uint2(0u, 0u); }
 }
 
 // test-only: the 64-bit sort keys tile << 32 | bits(depth) of the sorted pair list
@@ -394,8 +384,8 @@ void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
 #undef LAUNCH
 }
 
-void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms) {
-  TGS_LAUNCH((k_ranges), num_sms * 8, 256, 0, s, b.keys[sorted_idx], b.counters, b.ranges, fc.n_tiles);
+void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out) {
+  k_ranges_decode<<<(n_tiles + 255) / 256, 256, 0, s>>>(b.ranges, n_tiles, out);
 }
 
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out) {

@@ -156,7 +156,8 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
       continue;
     }
     // -------------------------------------------------- A8 blend
-    const uint2 range = ranges[tile];
+    uint2 range = ranges[tile];                      // {~start, end}, zero for a tile without pairs (k_sort.cu, A7)
+    range.x = range.y ? ~range.x : 0u;
     const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
     float fpx = (float)px0, fpy = (float)py;
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp

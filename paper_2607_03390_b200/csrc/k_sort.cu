@@ -48,7 +48,8 @@ template <int LB_BATCH, int CTAS_PER_SM, int SORT_IPT>
 __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ n_ptr, uint32_t* __restrict__ ticket, uint32_t* __restrict__ error_flag,
-    const uint32_t* __restrict__ hist, unsigned long long* __restrict__ desc, int shift, int nbits, uint32_t epoch) {
+    const uint32_t* __restrict__ hist, unsigned long long* __restrict__ desc, int shift, int nbits, uint32_t epoch,
+    uint2* __restrict__ ranges) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
@@ -197,6 +198,20 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
         const uint32_t o = sm.gbase[(uint32_t)(k >> shift) & 255u] + p;
         keys_out[o] = k;
         vals_out[o] = sm.vals[p];
+        if (ranges) {
+          // A7 in the last pass (the keys are the tile ids, now fully sorted): ranges[t] = {~start, end}, zero = empty.
+          // Inside a digit segment of this tile the neighbours in shared memory are the neighbours of the final list,
+          // so a change of tile id is a boundary written with plain stores; at the ends of a segment the neighbour
+          // belongs to another tile of the sort, so start / end go through atomicMax (max of ~o = min of o).
+          const uint32_t dg = (uint32_t)(k >> shift) & 255u;
+          const uint32_t kp = p > 0 ? sm.keys[p - 1] : 0xffffffffu;
+          const bool seg_first = p == 0 || ((uint32_t)(kp >> shift) & 255u) != dg;
+          bool seg_last = p + 1 >= valid;
+          if (!seg_last) seg_last = ((uint32_t)(sm.keys[p + 1] >> shift) & 255u) != dg;
+          if (seg_first) atomicMax(&ranges[k].x, ~o);
+          else if (kp != k) { ranges[k].x = ~o; ranges[kp].y = o; }
+          if (seg_last) atomicMax(&ranges[k].y, o + 1u);
+        }
       }
     }
   }
@@ -217,7 +232,7 @@ int tile_sort_passes(int n_tiles) {
 // (filled by the producer of the keys), `tickets` = one zeroed counter per pass, `desc` = [passes][tiles_cap][256].
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
-                int num_sms, bool small_input) {
+                int num_sms, bool small_input, uint2* ranges) {
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_BIG>));
@@ -231,10 +246,10 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
     unsigned long long* d = (unsigned long long*)desc + (size_t)p * tiles_cap * RADIX;
     if (small_input)
       TGS_LAUNCH((k_onesweep<32, 2, SORT_IPT_SMALL>), num_sms * 2, SORT_THREADS, sizeof(SortSmem<SORT_IPT_SMALL>), s, keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p,
-                                                                           error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
+                                                                           error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch, p == passes - 1 ? ranges : (uint2*)nullptr);
     else
       TGS_LAUNCH((k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG>), num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem<SORT_IPT_BIG>), s, 
-          keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch);
+          keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n_ptr, tickets + p, error_flag, hist + p * RADIX, d, 8 * p, nbits, epoch, p == passes - 1 ? ranges : (uint2*)nullptr);
     cur ^= 1;
   }
   return cur;

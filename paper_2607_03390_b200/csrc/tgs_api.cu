@@ -46,6 +46,7 @@ struct tgs_ctx {
   uint32_t max_pairs = 0; uint32_t sort_tiles_cap = 0; uint32_t dsort_tiles_cap = 0; uint32_t bin_chunks_cap = 0; int sort_passes_cap = 0; size_t px_cap = 0; int tiles_cap = 0;
   uint32_t epoch = 0;          // frame number, tag of the look-back descriptors
   uint64_t* keys64 = nullptr;  // test-only scratch of tgs_debug_get("keys")
+  uint2* ranges_dec = nullptr; // test-only scratch of tgs_debug_get("ranges")
   uint64_t device_bytes = 0;
   DevBuffers b;
   std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
@@ -113,6 +114,7 @@ int alloc_frame_buffers(tgs_ctx* c) {
   cudaStreamSynchronize(c->stream);
   for (void* p : c->allocs_frame) cudaFree(p);
   c->allocs_frame.clear();
+  c->ranges_dec = nullptr;
   DevBuffers& b = c->b;
   for (int i = 0; i < 2; ++i) {
     if (int r = dev_alloc(c, &b.image[i], px * 3, c->allocs_frame)) return r;
@@ -470,8 +472,8 @@ int tgs_render(tgs_ctx* c, int mode) {
   if (!early_colour) launch_colour_all(s, fc, b, c->num_sms);                                             // stage timing: the production kernel, in line
   mark();                                                                      // 5: A6 level 2 + A7
   const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
-                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false);   // pairs by tile
-  launch_ranges(s, fc, b, sorted, c->num_sms);                                                             // A7
+                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false,
+                                 b.ranges);                                                                // pairs by tile + A7 in the last pass
   mark();                                                                      // 6: A8 + A9
   if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
   if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
@@ -594,7 +596,11 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
   else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }
   else if (name == "tiles_touched") { src = b.tiles_touched; have = N * 4; }
-  else if (name == "ranges") { src = b.ranges; have = T * 8; }
+  else if (name == "ranges") {
+    if (!c->ranges_dec) { if (int r = dev_alloc(c, &c->ranges_dec, T, c->allocs_frame)) return r; }
+    launch_ranges_decode(c->stream, b, (int)T, c->ranges_dec);
+    src = c->ranges_dec; have = T * 8;
+  }
   else if (name == "tile_order") { src = b.tile_order; have = T * 4; }
   else if (name == "warp_depth") { src = b.warp_depth; have = tpx * 4; }
   else if (name == "warp_sigma") { src = b.warp_sigma; have = tpx * 4; }

@@ -160,9 +160,9 @@ void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
-                int num_sms, bool small_input);
+                int num_sms, bool small_input, uint2* ranges = nullptr);   // ranges: A7 fused into the last pass ({~start, end} per key)
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
-void launch_ranges(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int num_sms);
+void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out);   // test-only: {~start, end} -> {start, end}
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
                   const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions);
 uint32_t sort_tile_items();
