@@ -30,12 +30,49 @@ constexpr int BIN_IPT = 8;
 constexpr int BIN_CTAS_PER_SM = 8;
 constexpr int BIN_CHUNK = BIN_THREADS * BIN_IPT;      // tests per work item
 
+// Tile-test parameters of one visible Gaussian; 48 B, written in SORTED order by k_scan_area so that a k_bin chunk
+// reads the parameters of its Gaussians as one contiguous, coalesced block instead of gathering three records each
+// (scenes of many small Gaussians -- config 4: ~500 Gaussians per 1024-test chunk -- were bound by those gathers).
+struct alignas(16) GaussParams {
+  float u, v, A, B;
+  float C, tau, kC, kA;                 // kC ~ -B/C, kA ~ -B/A
+  uint32_t g, lo, w, pad;               // lo = x_lo | y_lo << 16
+};
+static_assert(sizeof(GaussParams) == 48, "three uint4 per Gaussian");
+
+constexpr int BIN_PCAP = 192;           // Gaussians of a chunk staged in shared memory (the rest is read from global)
+
+__device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exact, const float4* __restrict__ rec_uvdo,
+                                                   const float4* __restrict__ rec_conic) {
+  GaussParams P;
+  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
+  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
+  if (exact) {
+    const float4 a = rec_uvdo[g], b = rec_conic[g];
+    P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
+    P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
+  }
+  return P;
+}
+__device__ __forceinline__ void store_params(uint4* __restrict__ dst, const GaussParams& P) {
+  const uint4* s = reinterpret_cast<const uint4*>(&P);
+  dst[0] = s[0]; dst[1] = s[1]; dst[2] = s[2];
+}
+__device__ __forceinline__ GaussParams load_params(const uint4* __restrict__ src) {
+  GaussParams P;
+  uint4* d = reinterpret_cast<uint4*>(&P);
+  d[0] = src[0]; d[1] = src[1]; d[2] = src[2];
+  return P;
+}
+
 // ================================================================== A5a: flat test space
 // area_prefix[i] = number of tests of the Gaussians before position i of the sorted visible list (area_prefix[n] =
 // all tests); chunk_first[k] = position of the Gaussian that contains test k * BIN_CHUNK.
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const uint32_t* __restrict__ sorted_g,
                                                             const uint2* __restrict__ rec_rect, unsigned long long* __restrict__ desc,
                                                             uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
+                                                            const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                            uint4* __restrict__ bin_params,
                                                             Counters* __restrict__ counters, unsigned long long max_tests) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
@@ -57,7 +94,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
 #pragma unroll
     for (int j = 0; j < SCAN_IPT; ++j) {
       a[j] = 0;
-      if (i0 + j < n) { const uint2 r = rec_rect[sorted_g[i0 + j]]; a[j] = ((r.x >> 16) - (r.x & 0xffffu)) * ((r.y >> 16) - (r.y & 0xffffu)); }
+      if (i0 + j < n) {
+        const uint32_t g = sorted_g[i0 + j];
+        const uint2 r = rec_rect[g];
+        a[j] = ((r.x >> 16) - (r.x & 0xffffu)) * ((r.y >> 16) - (r.y & 0xffffu));
+        store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g, r, fc.exact_tiles != 0, rec_uvdo, rec_conic));
+      }
     }
     const uint32_t tsum = a[0] + a[1] + a[2] + a[3];
     uint32_t incl_total;
@@ -128,27 +170,6 @@ __device__ __forceinline__ void sh_colour(const FrameConst& fc, uint32_t g, cons
 // with M = A dx^2 + C t^2 (>= |2B dx t|, the form is positive semi-definite) every edge value of either evaluation is
 // within a few 2^-24 * 2M of the exact one, hence the two agree unless |best - tau| <= 1e-5 * max M; only in that band
 // (a fraction of a percent of the tests) the exact sequence is run.  The decision is always the oracle's.
-struct GaussParams {
-  float u, v, A, B, C, tau, kC, kA;     // kC ~ -B/C, kA ~ -B/A
-  uint32_t g, lo, w;                    // lo = x_lo | y_lo << 16
-};
-
-constexpr int BIN_PCAP = 192;           // Gaussians of a chunk staged in shared memory (the rest is read from global)
-
-__device__ __forceinline__ GaussParams load_params(uint32_t g, bool exact, const uint2* __restrict__ rec_rect,
-                                                   const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic) {
-  GaussParams P;
-  const uint2 r = rec_rect[g];
-  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu);
-  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
-  if (exact) {
-    const float4 a = rec_uvdo[g], b = rec_conic[g];
-    P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
-    P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
-  }
-  return P;
-}
-
 // fast evaluation of one box edge: dx fixed, t free in [lo, hi]; q = A dx^2 + 2B dx t + C t^2 at the clamped optimum
 __device__ __forceinline__ void edge_fast(float A, float B2, float C, float k, float dx, float lo, float hi, float& best, float& Mmax) {
   const float t = fminf(fmaxf(k * dx, lo), hi);
@@ -188,11 +209,10 @@ struct BinSmem {
 };
 
 template <typename TileT>
-__global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32_t* __restrict__ sorted_g, const uint32_t* __restrict__ area_prefix,
-                                                     const uint32_t* __restrict__ chunk_first, const uint2* __restrict__ rec_rect,
-                                                     const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+__global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4* __restrict__ bin_params, const uint32_t* __restrict__ area_prefix,
+                                                     const uint32_t* __restrict__ chunk_first,
                                                      const uint32_t* __restrict__ sel_bits, unsigned long long* __restrict__ desc,
-                                                     uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ keys,
+                                                     uint32_t* __restrict__ keys,
                                                      uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
                                                      Counters* __restrict__ counters) {
   TGS_PDL_WAIT();
@@ -225,8 +245,12 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
       const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
       const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
       for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
-      for (uint32_t i = tid; i < m && i < (uint32_t)BIN_PCAP; i += BIN_THREADS)
-        sm.gp[i] = load_params(sorted_g[i_first + i], exact, rec_rect, rec_uvdo, rec_conic);
+      {   // the chunk's parameters are one contiguous block of the sorted array: coalesced 16 B copies
+        const uint32_t nq = 3u * (m < (uint32_t)BIN_PCAP ? m : (uint32_t)BIN_PCAP);
+        const uint4* src = bin_params + 3 * (size_t)i_first;
+        uint4* dst = reinterpret_cast<uint4*>(sm.gp);
+        for (uint32_t i = tid; i < nq; i += BIN_THREADS) dst[i] = src[i];
+      }
       __syncthreads();
       // -------------------------------------------------------------- tests
       const uint32_t t0 = cbase + tid * BIN_IPT;
@@ -234,34 +258,29 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint32
       if (t0 < tend) {
         uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
         while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
-        uint32_t li = lo, segcnt = 0, end, rx, ry, x_lo, y_lo;
+        uint32_t li = lo, end, rx, ry, x_lo, y_lo;
         GaussParams G;
         auto load = [&](uint32_t l, uint32_t t) {
-          G = l < (uint32_t)BIN_PCAP ? sm.gp[l] : load_params(sorted_g[i_first + l], exact, rec_rect, rec_uvdo, rec_conic);
+          G = l < (uint32_t)BIN_PCAP ? sm.gp[l] : load_params(bin_params + 3 * (size_t)(i_first + l));
           end = sm.prefix[l + 1];
           const uint32_t local = t - sm.prefix[l];
           ry = local / G.w; rx = local - ry * G.w;
           x_lo = G.lo & 0xffffu; y_lo = G.lo >> 16;
-        };
-        auto flush = [&]() {
-          if (segcnt) atomicAdd(&tiles_touched[G.g], segcnt);
-          segcnt = 0;
         };
         load(li, t0);
 #pragma unroll
         for (int k = 0; k < BIN_IPT; ++k) {
           const uint32_t t = t0 + k;
           if (t < tend) {
-            if (t >= end) { flush(); do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
+            if (t >= end) { do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
             const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
             bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
             if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
-            if (pass) { mask |= 1u << k; ++segcnt; }
+            if (pass) mask |= 1u << k;
             tl[k] = tile; gg[k] = G.g;
             if (++rx == G.w) { rx = 0; ++ry; }
           }
         }
-        flush();
       }
       // -------------------------------------------------------------- chunk-local ranks, stage, publish the aggregate
       const uint32_t cnt = __popc(mask);
@@ -345,6 +364,12 @@ __global__ void __launch_bounds__(256) k_ranges_decode(const uint2* __restrict__
   if (t < n_tiles) { const uint2 r = ranges[t]; out[t] = r.y ? make_uint2(~r.x, r.y) : make_uint2(0u, 0u); }
 }
 
+// test-only: pairs per Gaussian (the oracle's record.tiles_touched), counted from the pair list
+__global__ void __launch_bounds__(256) k_count_pairs(const uint32_t* __restrict__ vals, uint32_t n, uint32_t* __restrict__ out) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) atomicAdd(&out[vals[i]], 1u);
+}
+
 // test-only: the 64-bit sort keys tile << 32 | bits(depth) of the sorted pair list
 __global__ void __launch_bounds__(256) k_keys64(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
                                                 const float4* __restrict__ rec_uvdo, uint32_t n, uint64_t* __restrict__ out) {
@@ -364,13 +389,13 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   const uint32_t* sorted_g = b.cvals[sorted_g_idx];
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
-                                                      b.counters, max_tests);
+                                                      b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests);
   if (fc.n_tiles <= 65536)
-    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
   else
-    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, sorted_g, b.area_prefix, b.chunk_first, b.rec_trect, b.rec_uvdo, b.rec_conic, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.tiles_touched, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
 }
 
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
@@ -386,6 +411,11 @@ void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
 
 void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out) {
   k_ranges_decode<<<(n_tiles + 255) / 256, 256, 0, s>>>(b.ranges, n_tiles, out);
+}
+
+void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n_pairs, uint32_t n) {
+  cudaMemsetAsync(b.tiles_touched, 0, (size_t)n * 4, s);
+  if (n_pairs) k_count_pairs<<<(n_pairs + 255) / 256, 256, 0, s>>>(b.vals[sorted_idx], n_pairs, b.tiles_touched);
 }
 
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out) {

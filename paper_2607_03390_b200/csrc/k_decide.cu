@@ -54,12 +54,12 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 }
 
 // ------------------------------------------------------------------ per-frame init
-// counters <- 0; sort histograms <- 0; tile_flags <- 0; tiles_touched <- 0;
+// counters <- 0; sort histograms <- 0; tile_flags <- 0;
 // S frames: D^min <- INVALID bits, sigma^max <- 0; R / P frames: rendered_next <- 0;
 // R frames: F <- (+inf, +inf, -inf, -inf).
 __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint32_t* warp_depth,
                                                     uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
-                                                    uint4* tiles_touched4, uint32_t n_tt4, uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
+                                                    uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
                                                     uint32_t* F_key, int reset_F) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
@@ -72,7 +72,6 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
     tile_flags[i] = 0; ranges[i] = make_uint2(0u, 0u);
     if (trivial_sel) { tile_mask[i] = 4; tile_order[i] = i; if ((i & 31u) == 0u) sel_bits[i >> 5] = 0xffffffffu; }
   }
-  for (uint32_t i = tid; i < n_tt4; i += nth) tiles_touched4[i] = make_uint4(0u, 0u, 0u, 0u);
   if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
     const uint32_t px = (uint32_t)(fc.tg.W * fc.tg.H);
@@ -599,7 +598,7 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
   TGS_LAUNCH((k_frame_init), 592, 256, 0, s, fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
-                                   (uint32_t*)rendered_next, n_words, (uint4*)b.tiles_touched, (fc.n + 3) / 4, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
+                                   (uint32_t*)rendered_next, n_words, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
                                    b.F_key, reset_F ? 1 : 0);
 }
 

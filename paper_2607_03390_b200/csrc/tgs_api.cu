@@ -283,7 +283,7 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_trect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
   A(b.pre_cnt, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
-  A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n)
+  A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n) A(b.bin_params, 3 * (size_t)n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
   AZ(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
 #undef A
@@ -595,7 +595,13 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   else if (name == "rec_rect") { src = b.rec_rect; have = N * 8; }
   else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
   else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }
-  else if (name == "tiles_touched") { src = b.tiles_touched; have = N * 4; }
+  else if (name == "tiles_touched") {
+    if (!c->have_frame) return TGS_E_INVALID_ARG;
+    CK(cudaEventSynchronize(c->ev_done));
+    if (c->h_counters->overflow) return TGS_E_CAPACITY;
+    launch_count_pairs(c->stream, c->b, c->sorted_idx, (uint32_t)c->h_counters->n_pairs, (uint32_t)N);
+    src = b.tiles_touched; have = N * 4;
+  }
   else if (name == "ranges") {
     if (!c->ranges_dec) { if (int r = dev_alloc(c, &c->ranges_dec, T, c->allocs_frame)) return r; }
     launch_ranges_decode(c->stream, b, (int)T, c->ranges_dec);

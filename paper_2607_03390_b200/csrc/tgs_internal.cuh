@@ -85,7 +85,7 @@ struct DevBuffers {
   // -1/2 delta^T Sigma'^-1 delta completed to a sum of two squares: A' = -log2e/2 * c/det, k = -b/c, D' = -log2e/2 / c
   float4* rec_b0 = nullptr;      // [N] {u, v, A', k}
   float4* rec_b1 = nullptr;      // [N] {D', log2 o, d, -}
-  uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian
+  uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian (test-only: filled by tgs_debug_get)
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
   // visible Gaussians: ckeys = bits(depth), cvals = index; [1] staging (1024 slots per chunk), [0] in index order
@@ -96,6 +96,7 @@ struct DevBuffers {
   uint32_t* area_prefix = nullptr;           // [N+1] tests before each sorted visible Gaussian
   uint32_t* chunk_first = nullptr;           // [bin_chunks_cap] sorted position of the Gaussian holding a chunk's first test
   uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with rects of more than 4 tiles
+  uint4* bin_params = nullptr;               // [N][3] tile-test parameters of the visible Gaussians in SORTED order (k_scan_area -> k_bin)
   // pairs
   uint32_t* keys[2] = {nullptr, nullptr};    // [max_pairs] tile id of a pair
   uint32_t* vals[2] = {nullptr, nullptr};    // [max_pairs] Gaussian index of a pair
@@ -162,6 +163,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms, bool small_input, uint2* ranges = nullptr);   // ranges: A7 fused into the last pass ({~start, end} per key)
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
+void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n_pairs, uint32_t n);   // test-only
 void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out);   // test-only: {~start, end} -> {start, end}
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
                   const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions);
