@@ -61,6 +61,7 @@ struct tgs_ctx {
   cudaStream_t side2 = nullptr;         // third stream: SH colours beside the depth sort
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr, ev_fork3 = nullptr;
   bool sel_pending = false;
+  uint32_t nv_hint = 0;                 // visible Gaussians of a recent frame (selects the depth-sort instance)
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
   bool count_interactions = false;
@@ -312,6 +313,7 @@ int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, cons
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) { snprintf(c->err, sizeof(c->err), "load: %s", cudaGetErrorString(e)); return TGS_E_CUDA; }
   c->n = n; c->deg = deg; c->K = K;
+  c->nv_hint = n / 4;
   invalidate_priors(c);
   c->have_frame = false;
   return TGS_OK;
@@ -374,6 +376,9 @@ int tgs_render(tgs_ctx* c, int mode) {
   const int tile_bits = tile_key_bits(c->TX * c->TY), tile_passes = (tile_bits + 7) / 8;
   if (int r = alloc_pair_buffers(c, c->prm.max_pairs ? c->prm.max_pairs : auto_max_pairs(c), tile_passes)) return r;
   // grow the pair buffers when the previous frame came close to (or over) the capacity
+  // which instance of the depth sort: the small-input one (many tiles in flight, long look-back steps) or the one of the
+  // tile sort; decided from the visible count of the last frame whose counters have arrived (a hint, never waited for)
+  if (c->have_frame && cudaEventQuery(c->ev_done) == cudaSuccess) c->nv_hint = c->h_counters->n_visible;
   if (!c->prm.max_pairs && c->have_frame) {
     if (cudaEventQuery(c->ev_done) == cudaSuccess && (c->h_counters->overflow || c->h_counters->n_pairs > c->max_pairs / 2)) {
       unsigned long long want = (unsigned long long)c->max_pairs * 2ull;
@@ -464,7 +469,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   }
   mark();                                                                      // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, true);            // visible Gaussians by depth
+                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, c->nv_hint < 1000000u);   // visible Gaussians by depth
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   mark();                                                                      // 3: A5 pairs
   launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
