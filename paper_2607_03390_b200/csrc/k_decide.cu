@@ -227,7 +227,10 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
 // the Gaussian cannot be one the full computation would have flagged DEGENERATE instead of EMPTY.
 constexpr int PRE_THREADS = 256;
 constexpr int PRE_IPT = 4;
-constexpr int PRE_CHUNK = PRE_THREADS * PRE_IPT;
+constexpr int PRE_SUB = 2;                 // phase A passes per work item: phases B / C then run on the survivors of all of them
+constexpr int PRE_EPT = PRE_IPT * PRE_SUB; // list entries per thread in phase C
+constexpr int PRE_CHUNK = PRE_THREADS * PRE_IPT * PRE_SUB;
+static_assert(PRE_CHUNK <= 4096, "12-bit local index in PreSmem::list");
 
 struct PreSmem {
   uint16_t list[PRE_CHUNK];     // survivors of phase A: local index | newly-visible << 15 | visible << 14
@@ -274,7 +277,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
     if (chunk >= num_chunks) break;
     const uint32_t base = chunk * PRE_CHUNK;
     // ---------------------------------------------------------------- phase A
-    const uint32_t g0 = base + tid * PRE_IPT;
+    uint32_t total = 0;
+   for (int sub = 0; sub < PRE_SUB; ++sub) {
+    const uint32_t g0 = base + (uint32_t)sub * (PRE_THREADS * PRE_IPT) + tid * PRE_IPT;
     float4 c4[PRE_IPT];
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j) c4[j] = (g0 + j < fc.n) ? cull4[g0 + j] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -325,17 +330,19 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
     for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
     if (lane == 31) sm.warp[wid] = incl;
     __syncthreads();
-    uint32_t pos = incl - ns_t, total = 0;
+    uint32_t pos = total + incl - ns_t, sub_total = 0;
 #pragma unroll
-    for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < wid) pos += t; total += t; }
+    for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t t = sm.warp[w]; if ((uint32_t)w < wid) pos += t; sub_total += t; }
 #pragma unroll
     for (int j = 0; j < PRE_IPT; ++j)
-      if ((surv >> (2 * j)) & 1u) sm.list[pos++] = (uint16_t)((tid * PRE_IPT + j) | (((surv >> (2 * j + 1)) & 1u) << 15));
+      if ((surv >> (2 * j)) & 1u) sm.list[pos++] = (uint16_t)((sub * (PRE_THREADS * PRE_IPT) + tid * PRE_IPT + j) | (((surv >> (2 * j + 1)) & 1u) << 15));
+    total += sub_total;
     __syncthreads();
+   }
     // ---------------------------------------------------------------- phase B
     for (uint32_t i = tid; i < total; i += PRE_THREADS) {
       const uint32_t e = sm.list[i];
-      const uint32_t g = base + (e & 0x3ffu);
+      const uint32_t g = base + (e & 0xfffu);
       const uint32_t fl = (e >> 15) ? TGS_NEWLY_VISIBLE : 0u;
       const float4 c = cull4[g];
       const float4 ga = g2[2 * (size_t)g], gb = g2[2 * (size_t)g + 1];
@@ -413,7 +420,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
     // ---------------------------------------------------------------- phase C: visible list, ascending index
     uint32_t nv_t = 0;
 #pragma unroll
-    for (int j = 0; j < PRE_IPT; ++j) { const uint32_t i = tid * PRE_IPT + j; if (i < total && (sm.list[i] & 0x4000u)) ++nv_t; }
+    for (int j = 0; j < PRE_EPT; ++j) { const uint32_t i = tid * PRE_EPT + j; if (i < total && (sm.list[i] & 0x4000u)) ++nv_t; }
     uint32_t vincl = nv_t;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, vincl, d); if (lane >= (uint32_t)d) vincl += o; }
@@ -425,11 +432,11 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
     if (tid == 0) pre_cnt[chunk].x = vtotal;
     off += base;                                             // staging slots of this chunk
 #pragma unroll
-    for (int j = 0; j < PRE_IPT; ++j) {
-      const uint32_t i = tid * PRE_IPT + j;
+    for (int j = 0; j < PRE_EPT; ++j) {
+      const uint32_t i = tid * PRE_EPT + j;
       if (i < total && (sm.list[i] & 0x4000u)) {
         const uint32_t key = sm.depth[i];
-        vis_keys[off] = key; vis_vals[off] = base + (sm.list[i] & 0x3ffu); ++off;
+        vis_keys[off] = key; vis_vals[off] = base + (sm.list[i] & 0xfffu); ++off;
         atomicAdd(&sm.hist[0][key & 255u], 1u); atomicAdd(&sm.hist[1][(key >> 8) & 255u], 1u);
         atomicAdd(&sm.hist[2][(key >> 16) & 255u], 1u); atomicAdd(&sm.hist[3][key >> 24], 1u);
       }
