@@ -319,6 +319,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
         }
       }
       surv |= (1u | fl) << (2 * j);
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(g2 + 2 * (size_t)g));   // phase B reads the covariance of this survivor
     }
     if (g0 + PRE_IPT <= fc.n) *reinterpret_cast<uint4*>(rec_flags + g0) = make_uint4(cf[0], cf[1], cf[2], cf[3]);
     else
