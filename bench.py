@@ -340,33 +340,35 @@ def run_ablation(args):
     ctx.load_scene(sc); ref.load_scene(sc)
     cam, K, W = sc.camera, args.steps, max(args.warmup, 3)
 
-    def variant(**kw):
+    def variant(stride=1, **kw):
+        """`stride`: every stride-th pose of the trajectory, i.e. the camera moves `stride` times faster per frame (the
+        camera-speed axis of the paper's Table V)."""
         prm = ctx.default_params()
         for k, v in kw.items():
             setattr(prm, k, v)
         ctx.set_params(prm)
         ctx.reset_priors()
         for f in range(W):
-            ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+            ctx.set_camera(trajectory_pose(sc, f * stride), cam); ctx.render(tgs.AUTO)
         ctx.reset_priors()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with torch.cuda.stream(stream):
             e0.record(stream)
             for f in range(K):
-                ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+                ctx.set_camera(trajectory_pose(sc, f * stride), cam); ctx.render(tgs.AUTO)
             e1.record(stream)
         torch.cuda.synchronize()
         fps = K / (e0.elapsed_time(e1) * 1e-3)
         ctx.reset_priors()
         psnr, types, sel = [], [], []
         for f in range(min(K, 40)):
-            ctx.set_camera(trajectory_pose(sc, f), cam); ctx.render(tgs.AUTO)
+            ctx.set_camera(trajectory_pose(sc, f * stride), cam); ctx.render(tgs.AUTO)
             st = ctx.get_stats()
             types.append("RPS"[st["frame_type"]])
             if st["frame_type"] == tgs.FRAME_S:
                 sel.append(st["n_sel"] / st["n_tiles"])
-                ref.set_camera(trajectory_pose(sc, f), cam); ref.render(tgs.FULL)
+                ref.set_camera(trajectory_pose(sc, f * stride), cam); ref.render(tgs.FULL)
                 mse = float(((ctx.read_image() - ref.read_image()) ** 2).mean())
                 psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
         return {"fps": fps, "psnr_S_vs_full_dB": float(np.mean(psnr)) if psnr else None, "tgsf": types.count("S") / len(types),
@@ -387,6 +389,9 @@ def run_ablation(args):
         "prior_policy=CHAINED": variant(prior_policy=1),
         "CHAINED, lambda_sr=10": variant(prior_policy=1, lambda_sr=10),
         "CHAINED + tgb_downscale=2": variant(prior_policy=1, tgb_downscale=2),
+        # camera speed (Table V): every 2nd / 4th / 8th pose of the trajectory per frame
+        "camera speed x2": variant(stride=2), "camera speed x4": variant(stride=4), "camera speed x8": variant(stride=8),
+        "full render, camera speed x8": variant(stride=8, lambda_sr=1, lambda_tdc=1),
     }
     return {"metric": "ablation: FPS / PSNR(S vs full) / share of S frames per variant", "config": {"workload": f"config {args.config} ({sc.name})"},
             "steps": K, "warmup": W, "data": "synthetic", "ablation": rows}
