@@ -54,6 +54,11 @@ struct tgs_ctx {
   Counters* h_counters = nullptr;      // pinned
   uint32_t* h_sel = nullptr;           // pinned: n_sel of the last S frame (for the eta rule)
   cudaEvent_t ev_sel = nullptr, ev_done = nullptr;
+  // the device counters are double-buffered by frame parity: their (latency-bound) copy to the host runs on the third
+  // stream while the next frame, which uses the other block, has already started
+  Counters* counters2[2] = {nullptr, nullptr};
+  cudaEvent_t ev_cnt[2] = {nullptr, nullptr}, ev_post = nullptr;
+  bool cnt_pending[2] = {false, false};
   cudaStream_t copy = nullptr;          // read-back stream of tgs_read_image_async
   cudaEvent_t ev_copy[2] = {nullptr, nullptr};   // last asynchronous read of image[i] has finished
   bool copy_pending[2] = {false, false};
@@ -233,7 +238,10 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   if (cudaMallocHost((void**)&c->h_counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
   if (cudaMallocHost((void**)&c->h_sel, 2 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   memset(c->h_counters, 0, sizeof(Counters));
-  if (cudaMalloc((void**)&c->b.counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
+  for (auto& p : c->counters2) if (cudaMalloc((void**)&p, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
+  c->b.counters = c->counters2[0];
+  for (auto& e : c->ev_cnt) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&c->ev_post, cudaEventDisableTiming);
   if (cudaMalloc((void**)&c->b.F_key, 4 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   if (cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
@@ -253,7 +261,10 @@ void tgs_destroy(tgs_ctx* c) {
   cudaSetDevice(c->device);
   cudaStreamSynchronize(c->stream);
   free_list(c, c->allocs_scene); free_list(c, c->allocs_frame); free_list(c, c->allocs_pairs);
-  cudaFree(c->b.counters); cudaFree(c->b.F_key); cudaFree(c->b.sort_hist);
+  for (auto p : c->counters2) cudaFree(p);
+  for (auto e : c->ev_cnt) cudaEventDestroy(e);
+  cudaEventDestroy(c->ev_post);
+  cudaFree(c->b.F_key); cudaFree(c->b.sort_hist);
   cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
   cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
   cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
@@ -424,6 +435,9 @@ int tgs_render(tgs_ctx* c, int mode) {
     c->epoch = 1;
   }
   fc.epoch = c->epoch;
+  const int ci = (int)(c->epoch & 1u);
+  c->b.counters = c->counters2[ci];
+  if (c->cnt_pending[ci]) { CK(cudaStreamWaitEvent(c->stream, c->ev_cnt[ci], 0)); c->cnt_pending[ci] = false; }   // its last copy to the host
 
   DevBuffers& b = c->b;
   cudaStream_t s = c->stream;
@@ -485,9 +499,17 @@ int tgs_render(tgs_ctx* c, int mode) {
   launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_marks, c->num_sms, c->count_interactions);
   mark();                                                                      // 7: post
   if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
-  CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
-  mark();                                                                      // 8
-  CK(cudaEventRecord(c->ev_done, s));
+  if (fork) {
+    CK(cudaEventRecord(c->ev_post, s)); CK(cudaStreamWaitEvent(c->side2, c->ev_post, 0));
+    CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, c->side2));
+    CK(cudaEventRecord(c->ev_done, c->side2));
+    CK(cudaEventRecord(c->ev_cnt[ci], c->side2));
+    c->cnt_pending[ci] = true;
+  } else {
+    CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
+    mark();                                                                    // 8
+    CK(cudaEventRecord(c->ev_done, s));
+  }
   CK(cudaGetLastError());
   // ---- A10: prior commit (pointer swap) and scheduler counters
   c->cur_idx = out_idx; c->sorted_idx = sorted;
