@@ -57,7 +57,10 @@ struct tgs_ctx {
   // the device counters are double-buffered by frame parity: their (latency-bound) copy to the host runs on the third
   // stream while the next frame, which uses the other block, has already started
   Counters* counters2[2] = {nullptr, nullptr};
-  cudaEvent_t ev_cnt[2] = {nullptr, nullptr}, ev_post = nullptr;
+  cudaEvent_t ev_cnt[2] = {nullptr, nullptr}, ev_post = nullptr, ev_post2 = nullptr;
+  bool post2_pending = false;
+  uint32_t* F_base = nullptr;          // F_key of the last R frame = F_base + 4 * F_idx; an R frame builds the other one
+  int F_idx = 0;
   bool cnt_pending[2] = {false, false};
   cudaStream_t copy = nullptr;          // read-back stream of tgs_read_image_async
   cudaEvent_t ev_copy[2] = {nullptr, nullptr};   // last asynchronous read of image[i] has finished
@@ -242,7 +245,9 @@ int tgs_create(tgs_ctx** out, int device, void* stream) {
   c->b.counters = c->counters2[0];
   for (auto& e : c->ev_cnt) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_post, cudaEventDisableTiming);
-  if (cudaMalloc((void**)&c->b.F_key, 4 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
+  cudaEventCreateWithFlags(&c->ev_post2, cudaEventDisableTiming);
+  if (cudaMalloc((void**)&c->F_base, 8 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);   // two F's, by frame parity
+  c->b.F_key = c->F_base;
   if (cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
   cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
   cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
@@ -263,8 +268,8 @@ void tgs_destroy(tgs_ctx* c) {
   free_list(c, c->allocs_scene); free_list(c, c->allocs_frame); free_list(c, c->allocs_pairs);
   for (auto p : c->counters2) cudaFree(p);
   for (auto e : c->ev_cnt) cudaEventDestroy(e);
-  cudaEventDestroy(c->ev_post);
-  cudaFree(c->b.F_key); cudaFree(c->b.sort_hist);
+  cudaEventDestroy(c->ev_post); cudaEventDestroy(c->ev_post2);
+  cudaFree(c->F_base); cudaFree(c->b.sort_hist);
   cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
   cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
   cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
@@ -437,6 +442,7 @@ int tgs_render(tgs_ctx* c, int mode) {
   fc.epoch = c->epoch;
   const int ci = (int)(c->epoch & 1u);
   c->b.counters = c->counters2[ci];
+  c->b.F_key = c->F_base + 4 * (ftype == TGS_FRAME_R ? ci : c->F_idx);   // R: reset + built here (k_frustum, third stream); P / S: read
   if (c->cnt_pending[ci]) { CK(cudaStreamWaitEvent(c->stream, c->ev_cnt[ci], 0)); c->cnt_pending[ci] = false; }   // its last copy to the host
 
   DevBuffers& b = c->b;
@@ -462,6 +468,7 @@ int tgs_render(tgs_ctx* c, int mode) {
     launch_fill_corr(fork ? c->side : s, fc, b);                                                           // A2
   }
   mark();                                                                      // 1: A3 preprocess, A4 selection
+  if (c->post2_pending) { CK(cudaStreamWaitEvent(s, c->ev_post2, 0)); c->post2_pending = false; }          // k_frustum of the previous frame
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
   if (ftype == TGS_FRAME_S) {
     // A4 (T^oc of larger rects, T_sel) is only needed by the pair binning: it runs beside the depth sort
@@ -498,9 +505,16 @@ int tgs_render(tgs_ctx* c, int mode) {
   if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
   launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_marks, c->num_sms, c->count_interactions);
   mark();                                                                      // 7: post
-  if (builds_priors) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
+  if (builds_priors && !fork) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
   if (fork) {
+    // post-processing on the third stream, beside the start of the next frame: F / |G_rendered| over the visible list
+    // (the next frame waits for ev_post2 before it overwrites that list or reads F) and the counters' copy to the host
     CK(cudaEventRecord(c->ev_post, s)); CK(cudaStreamWaitEvent(c->side2, c->ev_post, 0));
+    if (builds_priors) {
+      launch_frustum(c->side2, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);
+      CK(cudaEventRecord(c->ev_post2, c->side2));
+      c->post2_pending = true;
+    }
     CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, c->side2));
     CK(cudaEventRecord(c->ev_done, c->side2));
     CK(cudaEventRecord(c->ev_cnt[ci], c->side2));
@@ -518,7 +532,7 @@ int tgs_render(tgs_ctx* c, int mode) {
     std::swap(b.rendered, b.rendered_next);
     memcpy(c->prior_view, c->view, sizeof(c->prior_view));
     c->priors_valid = true;
-    if (ftype == TGS_FRAME_R) c->F_valid = true;
+    if (ftype == TGS_FRAME_R) { c->F_valid = true; c->F_idx = ci; }
   }
   if (chains) { c->prior_idx = out_idx; memcpy(c->prior_view, c->view, sizeof(c->prior_view)); }
   if (ftype == TGS_FRAME_R) { c->sched.since_R = 0; c->sched.since_ref = 0; c->sched.force_P = 0; }
@@ -592,6 +606,7 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   if (!c || !nm || (mem != TGS_HOST && mem != TGS_DEVICE)) return TGS_E_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   const std::string name(nm);
+  if (c->post2_pending) CK(cudaStreamWaitEvent(c->stream, c->ev_post2, 0));   // k_frustum of the last frame (third stream)
   const DevBuffers& b = c->b;
   const size_t N = c->n, px = (size_t)c->W * c->H, T = (size_t)c->TX * c->TY;
   const size_t tpx = c->fc.tg.W > 0 ? (size_t)c->fc.tg.W * c->fc.tg.H : px;   // TGB grid of the last frame (R43)
