@@ -21,9 +21,14 @@
 
 namespace {
 
-constexpr int BLEND_THREADS = 64;      // 16 rows x 4 runs of 4 pixels
+constexpr int PPT = 4;                 // pixels per thread (dense mode): a run of PPT horizontally adjacent pixels
+constexpr int NQ = PPT / 2;            // packed pairs per thread
+constexpr int RUNS = 16 / PPT;         // runs per tile row
+constexpr int BLEND_THREADS = 256 / PPT;   // 16 rows x RUNS runs
+constexpr int BLEND_WARPS = BLEND_THREADS / 32;
+constexpr int BLEND_MIN_CTAS = PPT == 4 ? 10 : 16;
 constexpr int BLEND_BATCH = 128;
-constexpr int PPT = 4;                 // pixels per thread (dense mode)
+constexpr int IDS_PER_THREAD = BLEND_BATCH / BLEND_THREADS;
 constexpr int DENSE_GROUP = 8;         // records between two "whole warp finished" tests of the dense loop (divides BLEND_BATCH)
 constexpr int DENSE_UNROLL = 8;
 constexpr float ALPHA_MIN = 1.0f / 255.0f;
@@ -59,7 +64,7 @@ struct BlendSmem {
   Batch bt[2];
   float st[BLEND_THREADS][7];      // pixel states in transit during a compaction
   uint16_t st_px[BLEND_THREADS];   // their pixel index inside the tile (ly * 16 + lx)
-  uint32_t alive_cnt[2][2];        // [parity][warp] alive pixels
+  uint32_t alive_cnt[2][BLEND_WARPS];   // [parity][warp] alive pixels
   uint32_t work;
 };
 
@@ -97,7 +102,7 @@ __device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p
 }
 
 template <bool MARK, bool COUNT>
-__global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
+__global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
                                                          const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,
@@ -109,7 +114,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
   __shared__ BlendSmem sm;
   const CamConst& k = fc.cam;
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int lx = (tid & 3) * PPT, ly = tid >> 2;
+  const int lx = (int)(tid % RUNS) * PPT, ly = (int)(tid / RUNS);
   const uint32_t n_sel = counters->n_sel;
   while (true) {
     __syncthreads();
@@ -161,19 +166,19 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
     const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
     float fpx = (float)px0, fpy = (float)py;
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
-    float2 T2[2], Cr2[2], Cg2[2], Cb2[2], S12[2], S22[2], D02[2];
+    float2 T2[NQ], Cr2[NQ], Cg2[NQ], Cb2[NQ], S12[NQ], S22[NQ], D02[NQ];
     Pixel sp;
     // dense mode keeps no alive flags: a finished pixel carries T < 0 (its |T| is the final transmittance), so that
     // T (1 - alpha) >= 1e-4 fails for it by itself; pixels outside the image start finished
     bool valid[PPT], salive = false;
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < NQ; ++q) {
       Cr2[q] = Cg2[q] = Cb2[q] = S12[q] = S22[q] = D02[q] = make_float2(0.0f, 0.0f);
     }
 #pragma unroll
     for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
-    T2[0] = make_float2(valid[0] ? 1.0f : -1.0f, valid[1] ? 1.0f : -1.0f);
-    T2[1] = make_float2(valid[2] ? 1.0f : -1.0f, valid[3] ? 1.0f : -1.0f);
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) T2[q] = make_float2(valid[2 * q] ? 1.0f : -1.0f, valid[2 * q + 1] ? 1.0f : -1.0f);
     auto get_px = [&](int i) {
       Pixel r;
       const int q = i >> 1;
@@ -181,12 +186,18 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
       else { r.T = T2[q].x; r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = D02[q].x; }
       return r;
     };
+    auto count_alive = [&]() {
+      uint32_t c = 0;
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) c += (uint32_t)(T2[q].x > 0.0f) + (uint32_t)(T2[q].y > 0.0f);
+      return c;
+    };
     bool sparse = false, have = false;      // sparse mode: this thread owns pixel `spx` of the tile in p[0]
     uint32_t spx = 0, slots = TGS_TILE * TGS_TILE;
-    uint32_t gid[2];
+    uint32_t gid[IDS_PER_THREAD];
     auto load_ids = [&](uint32_t b) {
 #pragma unroll
-      for (int s = 0; s < 2; ++s) {
+      for (int s = 0; s < IDS_PER_THREAD; ++s) {
         const uint32_t idx = range.x + b * BLEND_BATCH + tid + s * BLEND_THREADS;
         gid[s] = (b < nb && idx < range.y) ? vals[idx] : 0xffffffffu;
       }
@@ -194,7 +205,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
     auto issue = [&](uint32_t b) {
       Batch& B = sm.bt[b & 1];
 #pragma unroll
-      for (int s = 0; s < 2; ++s) {
+      for (int s = 0; s < IDS_PER_THREAD; ++s) {
         const uint32_t j = tid + s * BLEND_THREADS;
         if (gid[s] != 0xffffffffu) {
           cp_async16(&B.a[j], rec_b0 + gid[s]); cp_async16(&B.b[j], rec_b1 + gid[s]); cp_async16(&B.c[j], rec_rgb + gid[s]);
@@ -213,7 +224,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
       const Batch& B = sm.bt[b & 1];
       const uint32_t cnt = min((uint32_t)BLEND_BATCH, len - b * BLEND_BATCH);
 #pragma unroll
-      for (int s = 0; s < 2; ++s) {
+      for (int s = 0; s < IDS_PER_THREAD; ++s) {
         const uint32_t j = tid + s * BLEND_THREADS;
         if (j < cnt && B.contrib[j]) rendered_next[B.id[j]] = 1;
       }
@@ -223,23 +234,25 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
     int computed = -1;
     for (uint32_t b = 0; b < nb; ++b) {
       const uint32_t na_t = sparse ? (uint32_t)(have && salive)
-                                   : (uint32_t)(T2[0].x > 0.0f) + (uint32_t)(T2[0].y > 0.0f) + (uint32_t)(T2[1].x > 0.0f) + (uint32_t)(T2[1].y > 0.0f);
+                                   : count_alive();
       const uint32_t na_w = __reduce_add_sync(0xffffffffu, na_t);
       if (lane == 0) sm.alive_cnt[b & 1][wid] = na_w;
       cp_async_wait_all();
       __syncthreads();
-      const uint32_t alive0 = sm.alive_cnt[b & 1][0], total_alive = alive0 + sm.alive_cnt[b & 1][1];
+      uint32_t alive_before = 0, total_alive = 0;        // alive pixels in the warps before this one, in the tile
+#pragma unroll
+      for (int w_ = 0; w_ < BLEND_WARPS; ++w_) { const uint32_t a_ = sm.alive_cnt[b & 1][w_]; if ((uint32_t)w_ < wid) alive_before += a_; total_alive += a_; }
       if (MARK && b > 0) writeback_marks(b - 1);
       computed = -1;
       if (total_alive == 0) break;
       if (b + 1 < nb) issue(b + 1);
       load_ids(b + 2);
       // ---- compaction of the alive pixels to one per thread
-      if ((total_alive <= BLEND_THREADS && slots > BLEND_THREADS) || (total_alive <= 32 && slots > 32)) {
+      if ((total_alive <= BLEND_THREADS && slots > BLEND_THREADS) || (BLEND_THREADS > 32 && total_alive <= 32 && slots > 32)) {
         uint32_t incl = na_t;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= (uint32_t)d) incl += o; }
-        uint32_t pos = (wid ? alive0 : 0u) + incl - na_t;
+        uint32_t pos = alive_before + incl - na_t;
         if (!sparse) {
 #pragma unroll
           for (int i = 0; i < PPT; ++i) {
@@ -291,17 +304,18 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
             const float4 gc = B.c[j];
             if (COUNT && j < cnt) {
               nslot += PPT;
-              nint += (uint32_t)(T2[0].x > 0.0f) + (uint32_t)(T2[0].y > 0.0f) + (uint32_t)(T2[1].x > 0.0f) + (uint32_t)(T2[1].y > 0.0f);
+              nint += count_alive();
             }
             const float dy = ga.y - fpy;
             const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
             const float t0 = fmaf(ga.w, dy, ga.x - fpx);                // t at the first pixel of the run
             const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z), d2 = make_float2(gb.z, gb.z);
-            const float2 tt[2] = {__fadd2_rn(make_float2(t0, t0), make_float2(0.0f, -1.0f)),
-                                  __fadd2_rn(make_float2(t0, t0), make_float2(-2.0f, -3.0f))};
+            float2 tt[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) tt[q] = __fadd2_rn(make_float2(t0, t0), make_float2(-(float)(2 * q), -(float)(2 * q + 1)));
             float2 wsum = make_float2(0.0f, 0.0f);
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
+            for (int q = 0; q < NQ; ++q) {
               const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
               float2 al = make_float2(fminf(0.99f, ex2_approx(e.x)), fminf(0.99f, ex2_approx(e.y)));
               al.x = al.x >= ALPHA_MIN ? al.x : 0.0f;                             // skip (R2)
@@ -325,7 +339,10 @@ __global__ void __launch_bounds__(BLEND_THREADS, 10) k_blend(FrameConst fc, cons
             }
             if (MARK && wsum.x + wsum.y > 0.0f) Bw.contrib[j] = 1;
            }
-           if (__all_sync(0xffffffffu, fmaxf(fmaxf(T2[0].x, T2[0].y), fmaxf(T2[1].x, T2[1].y)) < 0.0f)) break;
+           float tmax = fmaxf(T2[0].x, T2[0].y);
+#pragma unroll
+           for (int q = 1; q < NQ; ++q) tmax = fmaxf(tmax, fmaxf(T2[q].x, T2[q].y));
+           if (__all_sync(0xffffffffu, tmax < 0.0f)) break;
           }
         }
       } else if (__any_sync(0xffffffffu, salive)) {
