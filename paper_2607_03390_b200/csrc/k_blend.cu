@@ -26,8 +26,8 @@ constexpr int NQ = PPT / 2;            // packed pairs per thread
 constexpr int RUNS = 16 / PPT;         // runs per tile row
 constexpr int BLEND_THREADS = 256 / PPT;   // 16 rows x RUNS runs
 constexpr int BLEND_WARPS = BLEND_THREADS / 32;
-constexpr int BLEND_MIN_CTAS = PPT == 4 ? 10 : 16;
-constexpr int BLEND_BATCH = PPT == 4 ? 128 : 64;   // records per batch (two batches in flight per CTA)
+constexpr int BLEND_MIN_CTAS = PPT == 4 ? 10 : PPT == 8 ? 16 : 8;
+constexpr int BLEND_BATCH = PPT == 8 ? 64 : 128;   // records per batch (two batches in flight per CTA)
 constexpr int IDS_PER_THREAD = BLEND_BATCH / BLEND_THREADS;
 constexpr int DENSE_GROUP = 8;         // records between two "whole warp finished" tests of the dense loop (divides BLEND_BATCH)
 constexpr int DENSE_UNROLL = 8;
@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
 
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
                   uint8_t* rendered_next, int num_sms, bool count_interactions) {
-  const int grid = num_sms * (PPT == 4 ? 12 : 16);
+  const int grid = num_sms * (PPT == 4 ? 12 : PPT == 8 ? 16 : 8);
 #define LAUNCH(M, C)                                                                                                          \
   TGS_LAUNCH((k_blend<M, C>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \
