@@ -55,6 +55,8 @@ def test_defaults_are_the_papers(lib):
     # PAPER.md:L99 lambda1 = 3, lambda2 = 0; L142 lambda_TDC = 50, lambda_SR = 5; L128 eta = 40 %
     assert (p.lambda1, p.lambda2, p.lambda_tdc, p.lambda_sr) == (3.0, 0.0, 50, 5) and abs(p.eta - 0.4) < 1e-7
     assert (p.enable_afc, p.enable_toc, p.enable_sr) == (1, 1, 1)
+    # R39 exact tile intersection on; R42 ANCHORED priors (the paper, L86); R43 / L142 TGB at full resolution unless asked
+    assert (p.exact_tiles, p.prior_policy, p.tgb_downscale) == (1, 0, 1)
     assert lib.tgs_strerror(tgs.E_NO_PRIORS).decode().startswith("no valid temporal priors")
 
 
