@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __
 // kernel: selected tiles first (ascending id), then the tiles that are only stitched.
 __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* __restrict__ tile_flags, uint8_t* __restrict__ tile_mask,
                                                  uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tile_order,
-                                                 Counters* __restrict__ counters) {
+                                                 Counters* __restrict__ counters, volatile uint32_t* __restrict__ host_n_sel) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   __shared__ uint32_t s_sel[32], s_oc[32], s_um[32];
@@ -539,7 +539,12 @@ __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* 
   uint32_t before = 0, total = 0, toc = 0, tum = 0;
 #pragma unroll
   for (int w = 0; w < 32; ++w) { const uint32_t v = s_sel[w]; if ((uint32_t)w < wid) before += v; total += v; toc += s_oc[w]; tum += s_um[w]; }
-  if (threadIdx.x == 0) { counters->n_sel = total; counters->n_sel_oc = toc; counters->n_sel_um = tum; }
+  if (threadIdx.x == 0) {
+    counters->n_sel = total; counters->n_sel_oc = toc; counters->n_sel_um = tum;
+    // the eta rule needs this count on the host (A0): a zero-copy store into pinned host memory -- a D2H memcpy would
+    // queue behind an image read-back in flight on the copy engine
+    if (host_n_sel) { *host_n_sel = total; __threadfence_system(); }
+  }
   // work order of the blend: the selected tiles in ascending id at [0, total), the others behind them in ascending id
   uint32_t ps = before;
   for (int w = w0; w < w1; ++w) {
@@ -633,8 +638,18 @@ void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num
   TGS_LAUNCH((k_mark_oc), num_sms * 8, 128, 0, s, fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_trect, b.tile_flags, b.counters);
 }
 
-void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
-  TGS_LAUNCH((k_select), 1, 1024, 0, s, fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters);
+void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t* host_n_sel) {
+  TGS_LAUNCH((k_select), 1, 1024, 0, s, fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters, (volatile uint32_t*)host_n_sel);
+}
+
+// The frame's counters to pinned host memory by zero-copy stores (no copy engine: see k_select).
+__global__ void __launch_bounds__(64) k_export_counters(const Counters* __restrict__ counters, volatile uint32_t* __restrict__ host) {
+  TGS_PDL_WAIT();
+  if (threadIdx.x < sizeof(Counters) / 4) host[threadIdx.x] = reinterpret_cast<const uint32_t*>(counters)[threadIdx.x];
+  __threadfence_system();
+}
+void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host) {
+  TGS_LAUNCH((k_export_counters), 1, 64, 0, s, (const Counters*)b.counters, (volatile uint32_t*)host);
 }
 
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F) {

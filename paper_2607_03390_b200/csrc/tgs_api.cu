@@ -475,8 +475,7 @@ int tgs_render(tgs_ctx* c, int mode) {
     cudaStream_t s4 = fork ? c->side : s;
     if (fork) { CK(cudaEventRecord(c->ev_fork, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork, 0)); }
     launch_mark_oc(s4, fc, b, c->num_sms);                                                                 // A4: T^oc of larger rects
-    launch_select(s4, fc, b);                                                                              // A4: T_sel (R / P: all tiles, k_frame_init)
-    CK(cudaMemcpyAsync(c->h_sel, &b.counters->n_sel, sizeof(uint32_t), cudaMemcpyDeviceToHost, s4));
+    launch_select(s4, fc, b, c->h_sel);                                                                    // A4: T_sel (R / P: all tiles, k_frame_init); n_sel -> host
     CK(cudaEventRecord(c->ev_sel, s4));
     c->sel_pending = true;
   }
@@ -515,12 +514,12 @@ int tgs_render(tgs_ctx* c, int mode) {
       CK(cudaEventRecord(c->ev_post2, c->side2));
       c->post2_pending = true;
     }
-    CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, c->side2));
+    launch_export_counters(c->side2, b, c->h_counters);
     CK(cudaEventRecord(c->ev_done, c->side2));
     CK(cudaEventRecord(c->ev_cnt[ci], c->side2));
     c->cnt_pending[ci] = true;
   } else {
-    CK(cudaMemcpyAsync(c->h_counters, b.counters, sizeof(Counters), cudaMemcpyDeviceToHost, s));
+    launch_export_counters(s, b, c->h_counters);
     mark();                                                                    // 8
     CK(cudaEventRecord(c->ev_done, s));
   }

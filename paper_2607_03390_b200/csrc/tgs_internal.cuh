@@ -153,7 +153,8 @@ void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma);
 void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
-void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b);
+void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t* host_n_sel);
+void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
