@@ -63,8 +63,8 @@ struct tgs_ctx {
   int F_idx = 0;
   bool cnt_pending[2] = {false, false};
   cudaStream_t copy = nullptr;          // read-back stream of tgs_read_image_async
-  cudaEvent_t ev_copy[2] = {nullptr, nullptr};   // last asynchronous read of image[i] has finished
-  bool copy_pending[2] = {false, false};
+  cudaEvent_t ev_copy[3] = {nullptr, nullptr, nullptr};   // last asynchronous read of image[i] has finished
+  bool copy_pending[3] = {false, false, false};
   cudaStream_t side = nullptr;          // second stream: work that is off the critical path of a frame (A2, A4)
   cudaStream_t side2 = nullptr;         // third stream: SH colours beside the depth sort
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr, ev_fork3 = nullptr;
@@ -125,7 +125,7 @@ int alloc_frame_buffers(tgs_ctx* c) {
   c->allocs_frame.clear();
   c->ranges_dec = nullptr;
   DevBuffers& b = c->b;
-  for (int i = 0; i < 2; ++i) {
+  for (int i = 0; i < 3; ++i) {
     if (int r = dev_alloc(c, &b.image[i], px * 3, c->allocs_frame)) return r;
     if (int r = dev_alloc(c, &b.depth[i], px, c->allocs_frame)) return r;
     if (int r = dev_alloc(c, &b.sigma[i], px, c->allocs_frame)) return r;
@@ -451,7 +451,10 @@ int tgs_render(tgs_ctx* c, int mode) {
   // R42 (prior_policy = CHAINED): an S frame's stitched outputs become the priors too; its G_rendered marks are OR-ed
   // into the current set in place (k_preprocess has read the set before the blend writes it: stream order)
   const bool chains = ftype == TGS_FRAME_S && c->prm.prior_policy == TGS_PRIORS_CHAINED;
-  const int out_idx = c->prior_idx ^ 1;   // never overwrite the priors while they are being read
+  // never the priors (they are being read), and not the previous frame's buffers either when there is a third choice:
+  // an asynchronous read-back of that image may still be running (tgs_read_image_async)
+  int out_idx = (c->prior_idx + 1) % 3;
+  if (out_idx == c->cur_idx) out_idx = (out_idx + 1) % 3 == c->prior_idx ? out_idx : (out_idx + 1) % 3;
   const float* prior_image = c->priors_valid ? b.image[c->prior_idx] : nullptr;
   uint8_t* rendered_next = builds_priors ? b.rendered_next : nullptr;
   uint8_t* rendered_marks = chains ? b.rendered : rendered_next;
@@ -561,7 +564,7 @@ int tgs_wait_reads(tgs_ctx* c) {
   if (!c) return TGS_E_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->copy));
-  c->copy_pending[0] = c->copy_pending[1] = false;
+  c->copy_pending[0] = c->copy_pending[1] = c->copy_pending[2] = false;
   return TGS_OK;
 }
 

@@ -112,9 +112,10 @@ struct DevBuffers {
   uint32_t* tile_order = nullptr;     // [T] selected tiles first, then the others
   uint2* ranges = nullptr;            // [T] {start,end}
   // images
-  float* image[2] = {nullptr, nullptr};   // [H][W][3]
-  float* depth[2] = {nullptr, nullptr};   // [H][W]
-  float* sigma[2] = {nullptr, nullptr};   // [H][W]
+  // three sets: the priors, the frame being rendered, and the previous frame, whose image may still be on its way to the host
+  float* image[3] = {nullptr, nullptr, nullptr};   // [H][W][3]
+  float* depth[3] = {nullptr, nullptr, nullptr};   // [H][W]
+  float* sigma[3] = {nullptr, nullptr, nullptr};   // [H][W]
   float* warp_depth = nullptr;  // D^min (uint bits during the splat)
   float* warp_sigma = nullptr;  // sigma^max
   float* fill_depth = nullptr;  // D'
