@@ -309,13 +309,13 @@ def run_ours(args):
         "stages": stages, "roofline": roof, "stage_rooflines": stage_roof, "clocks": clocks,
     }
     # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), compact_vis, scan_area, bin,
-    # colour, tile sort (digits, the last one writes the ranges), blend = 11 + tile digits; + frustum on R / P; + warp,
-    # fill_corr, mark_oc, select on S
+    # colour, tile sort (digits, the last one writes the ranges), blend = 11 + tile digits; + export_counters; + frustum
+    # on R / P; + warp, fill_corr, mark_oc, select on S
     T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
     tpasses = (max(1, int(np.ceil(np.log2(T)))) + 7) // 8
     nR = sum(1 for s in all_stats if s["frame_type"] != 2)
     base = 11 + tpasses
-    per_ref, per_s = base + 1, base + 4
+    per_ref, per_s = base + 2, base + 5        # + k_export_counters on every frame
     frac_ref = nR / max(1, len(all_stats))
     out["gpu_launches"] = int(round(K * (frac_ref * per_ref + (1 - frac_ref) * per_s)))
     if world > 1:
