@@ -165,6 +165,28 @@ def test_half_resolution_tgb(size):
     assert partial >= 1 and sg["n_toc"] > 0.1 * sc.n
 
 
+def test_parameters_switched_between_frames():
+    """tgb_downscale and prior_policy changed from frame to frame (tgs_set_params between renders): each frame starts from
+    the oracle's priors and must match it in full."""
+    P = _p()
+    sc = make_config(5, n=50_000, frames=8, width=352, height=200)
+    sc.scales[:, :2] *= 6.0
+    g, o = P.make_pair(sc)
+    plan = [("full", 1, 0), ("temporal", 1, 0), ("temporal", 2, 0), ("pseudo", 1, 0), ("temporal", 2, 1), ("temporal", 1, 1), ("temporal", 2, 0)]
+    for f, (mode, ds, pol) in enumerate(plan):
+        pg, po = g.default_params(), o.default_params()
+        for prm in (pg, po):
+            prm.tgb_downscale = ds; prm.prior_policy = pol
+        g.set_params(pg); o.set_params(po)
+        if f:
+            P.inject_priors(g, o)
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G[mode]); ft = o.render(P.MODE_O[mode])
+        P.compare_frame(g, o, sc.n, ft)
+        if mode == "temporal":
+            assert g.debug_get("warp_depth").size == (((352 + ds - 1) // ds) * ((200 + ds - 1) // ds))
+
+
 def test_chained_priors_policy():
     """prior_policy = CHAINED (R42): every S frame starts from the oracle's current priors (injected), is compared in
     full, and must then have committed its own outputs: priors = the frame's stitched image / depth / sigma, pose of
