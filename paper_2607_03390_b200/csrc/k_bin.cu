@@ -22,7 +22,7 @@
 namespace {
 
 constexpr int SCAN_THREADS = 256;
-constexpr int SCAN_IPT = 4;
+constexpr int SCAN_IPT = 2;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 
 constexpr int BIN_THREADS = 128;
@@ -101,7 +101,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
         store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g, r, fc.exact_tiles != 0, rec_uvdo, rec_conic));
       }
     }
-    const uint32_t tsum = a[0] + a[1] + a[2] + a[3];
+    uint32_t tsum = 0;
+#pragma unroll
+    for (int j = 0; j < SCAN_IPT; ++j) tsum += a[j];
     uint32_t incl_total;
     uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total, fc.epoch);
     if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
