@@ -514,3 +514,32 @@ def test_full_size_config3_reference_and_temporal():
     sg, so, out = P.compare_frame(g, o, sc.n, ora.FRAME_S)
     # this cloud has no closed surfaces: forward-warped pixels scatter, so nearly every tile is unmatched
     assert sg["n_sel"] <= sg["n_tiles"] and sg["n_afc"] > 0 and sg["n_toc"] > 0
+
+
+@pytest.mark.parametrize("cfg", [2, 4, 5])
+def test_full_size_other_configs(cfg):
+    """BASELINE.json configs 2 (500 k, 1280x720), 4 (8 M aerial, 1080p; more than 1 M visible Gaussians: the depth
+    sort runs in its large-input instance once the hint has arrived) and 5 (3 M stacked sheets, SH 1, 1080p: a strict
+    subset of the tiles is selected, TOC culls most of the cloud) at full size: one reference frame and one
+    TemporalGS frame on injected priors, every output compared with the oracle."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(cfg, frames=4)
+    g, o = P.make_pair(sc)
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, out = P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    assert sg["n_pairs"] > 500_000
+    if cfg == 4:
+        # a second full render at the same pose: by now the visible count of the first frame has reached the host, so
+        # the depth sort switches to the instance of the tile sort; the frame must not change
+        assert sg["n_visible"] > 1_000_000
+        g.render(tgs.FULL)
+        P.compare_frame(g, o, sc.n, ora.FRAME_R)
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[2], sc.camera); o.set_camera(sc.poses[2], sc.camera)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    sg, so, out = P.compare_frame(g, o, sc.n, ora.FRAME_S)
+    assert sg["n_sel"] <= sg["n_tiles"]
+    if cfg == 5:
+        assert 0 < sg["n_sel"] < sg["n_tiles"] and sg["n_toc"] > 0
