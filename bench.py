@@ -27,10 +27,11 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full render"
-# Lane-instructions one alive (pixel, Gaussian) interaction of the blend needs: 12 on the FMA pipe
-# (exponent 2, 1 - alpha, T (1 - alpha), alpha T, 3 colour FMAs, d - d0, w dd, 2 moment FMAs; a packed FFMA2 half
-# counts as 1) + 1 MUFU.EX2 + 8 on the ALU pipe (clamp, 2 threshold tests, first-contribution test, 4 selects).
-BLEND_LANE_INSTR = 21.0
+# Lane-instructions one alive (pixel, Gaussian) interaction of the blend needs: 11.5 on the FMA pipe
+# (exponent 2, 1 - alpha, T (1 - alpha), alpha T, 3 colour FMAs, w dd, 2 moment FMAs; per run of 4 pixels d - d_ref and the
+# sum of the weights, 1/4 each; a packed FFMA2 half counts as 1) + 1 MUFU.EX2 + 6.5 on the ALU pipe (clamp, 2 threshold
+# tests, 3 selects; per run the any-pixel-composited test and the select of d_ref).
+BLEND_LANE_INSTR = 19.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_blend<1,0> launch on config 3, from the ncu --set full capture
 # summarised in profiles/r1h_top_kernels.md (the file names the command); per launch, like `achieved`.
 BLEND_DRAM_TRAFFIC_BYTES = 47.3e6

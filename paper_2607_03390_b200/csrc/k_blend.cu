@@ -166,14 +166,19 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
     const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
     float fpx = (float)px0, fpy = (float)py;
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
-    float2 T2[NQ], Cr2[NQ], Cg2[NQ], Cb2[NQ], S12[NQ], S22[NQ], D02[NQ];
+    float2 T2[NQ], Cr2[NQ], Cg2[NQ], Cb2[NQ], S12[NQ], S22[NQ];
+    // reference depth of the run's Eq.1-2 moments (R30): the depth of the first record that any of its PPT pixels
+    // composites (`open` until then).  Per run, not per pixel: two compares / selects per record instead of two per pixel;
+    // a pixel whose own first contribution comes later only has its moments taken about a slightly nearer depth
+    float dref = 0.0f;
+    bool open = true;
     Pixel sp;
     // dense mode keeps no alive flags: a finished pixel carries T < 0 (its |T| is the final transmittance), so that
     // T (1 - alpha) >= 1e-4 fails for it by itself; pixels outside the image start finished
     bool valid[PPT], salive = false;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
-      Cr2[q] = Cg2[q] = Cb2[q] = S12[q] = S22[q] = D02[q] = make_float2(0.0f, 0.0f);
+      Cr2[q] = Cg2[q] = Cb2[q] = S12[q] = S22[q] = make_float2(0.0f, 0.0f);
     }
 #pragma unroll
     for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
@@ -182,8 +187,8 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
     auto get_px = [&](int i) {
       Pixel r;
       const int q = i >> 1;
-      if (i & 1) { r.T = T2[q].y; r.Cr = Cr2[q].y; r.Cg = Cg2[q].y; r.Cb = Cb2[q].y; r.S1 = S12[q].y; r.S2 = S22[q].y; r.d0 = D02[q].y; }
-      else { r.T = T2[q].x; r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = D02[q].x; }
+      if (i & 1) { r.T = T2[q].y; r.Cr = Cr2[q].y; r.Cg = Cg2[q].y; r.Cb = Cb2[q].y; r.S1 = S12[q].y; r.S2 = S22[q].y; r.d0 = dref; }
+      else { r.T = T2[q].x; r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = dref; }
       return r;
     };
     auto count_alive = [&]() {
@@ -309,7 +314,10 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
             const float dy = ga.y - fpy;
             const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
             const float t0 = fmaf(ga.w, dy, ga.x - fpx);                // t at the first pixel of the run
-            const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z), d2 = make_float2(gb.z, gb.z);
+            const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z);
+            dref = open ? gb.z : dref;                                  // follows the list until the run's first contribution
+            const float ddf = gb.z - dref;
+            const float2 dd = make_float2(ddf, ddf);                    // d - d_ref
             float2 tt[NQ];
 #pragma unroll
             for (int q = 0; q < NQ; ++q) tt[q] = __fadd2_rn(make_float2(t0, t0), make_float2(-(float)(2 * q), -(float)(2 * q + 1)));
@@ -324,8 +332,6 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
               const bool bl0 = Tn.x >= 1.0e-4f, bl1 = Tn.y >= 1.0e-4f;            // else: stop (R2) or already finished
               al.x = bl0 ? al.x : 0.0f; al.y = bl1 ? al.y : 0.0f;
               if (COUNT) nhit += (uint32_t)(al.x > 0.0f) + (uint32_t)(al.y > 0.0f);
-              if (bl0 && T2[q].x == 1.0f) D02[q].x = gb.z;            // first contribution: moments are taken about it (R30)
-              if (bl1 && T2[q].y == 1.0f) D02[q].y = gb.z;
               const float2 wgt = __fmul2_rn(al, T2[q]);               // 0 (or -0) where nothing is composited
               T2[q].x = bl0 ? Tn.x : -fabsf(T2[q].x);                 // Tn = T where alpha was skipped
               T2[q].y = bl1 ? Tn.y : -fabsf(T2[q].y);
@@ -333,11 +339,12 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
               Cr2[q] = __ffma2_rn(wgt, make_float2(gc.x, gc.x), Cr2[q]);
               Cg2[q] = __ffma2_rn(wgt, make_float2(gc.y, gc.y), Cg2[q]);
               Cb2[q] = __ffma2_rn(wgt, make_float2(gc.z, gc.z), Cb2[q]);
-              const float2 dd = __ffma2_rn(D02[q], neg2, d2);                    // d - d0
               S12[q] = __ffma2_rn(wgt, dd, S12[q]);
               S22[q] = __ffma2_rn(__fmul2_rn(wgt, dd), dd, S22[q]);
             }
-            if (MARK && wsum.x + wsum.y > 0.0f) Bw.contrib[j] = 1;
+            const bool hit = wsum.x + wsum.y > 0.0f;                    // some pixel of the run composited this record
+            if (MARK && hit) Bw.contrib[j] = 1;
+            open = open && !hit;
            }
            float tmax = fmaxf(T2[0].x, T2[0].y);
 #pragma unroll
