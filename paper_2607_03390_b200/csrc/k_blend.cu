@@ -18,6 +18,7 @@
 // (again at <= 32: one warp), so the rest of the list costs work in proportion to the pixels that still need it.
 // This kernel is FP32-pipe / issue bound, not HBM bound.
 #include "tgs_internal.cuh"
+#include <type_traits>
 
 namespace {
 
@@ -35,6 +36,9 @@ constexpr float ALPHA_MIN = 1.0f / 255.0f;
 // log2(1/255) = -7.99435...; anything below this bound (with a safety gap far above the rounding of e and of
 // ex2.approx) has alpha < 1/255 for sure, so the exact test on alpha is only evaluated near or above the threshold
 constexpr float LOG2_ALPHA_MIN_LO = -7.9950f;
+// log2(0.99) = -0.01449957...; a Gaussian with log2 o below this bound (1e-6 relative under 0.99, four times the error of
+// ex2.approx) has alpha = o exp(q) < 0.99 at every pixel (q <= 0), so min(0.99, .) is the identity for it
+constexpr float LOG2_O_NEVER_CLAMPED = -0.014501f;
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -300,7 +304,9 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
           // branch-free: 85 % of the interactions of an alive pixel composite, so every pixel runs the whole update with
           // alpha forced to 0 where it is skipped (alpha < 1/255), stops (T (1 - alpha) < 1e-4) or is finished
           const float2 one2 = make_float2(1.0f, 1.0f), neg2 = make_float2(-1.0f, -1.0f);
-          for (uint32_t j0 = 0; j0 < cnt; j0 += DENSE_GROUP) {
+          // a group of DENSE_GROUP records; CLAMP = false: none of them can reach alpha = 0.99 (one FMNMX less per pixel)
+          auto dense_group = [&](const uint32_t j0, auto clamp_tag) {
+           constexpr bool CLAMP = decltype(clamp_tag)::value;
 #pragma unroll(DENSE_UNROLL)
            for (uint32_t jj = 0; jj < DENSE_GROUP; ++jj) {
             const uint32_t j = j0 + jj;
@@ -317,7 +323,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
             const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z);
             dref = open ? gb.z : dref;                                  // follows the list until the run's first contribution
             const float ddf = gb.z - dref;
-            const float2 dd = make_float2(ddf, ddf);                    // d - d_ref
+            const float2 dd = make_float2(ddf, ddf), dd2 = make_float2(ddf * ddf, ddf * ddf);   // d - d_ref and its square
             float2 tt[NQ];
 #pragma unroll
             for (int q = 0; q < NQ; ++q) tt[q] = __fadd2_rn(make_float2(t0, t0), make_float2(-(float)(2 * q), -(float)(2 * q + 1)));
@@ -325,7 +331,8 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
               const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
-              float2 al = make_float2(fminf(0.99f, ex2_approx(e.x)), fminf(0.99f, ex2_approx(e.y)));
+              float2 al = make_float2(ex2_approx(e.x), ex2_approx(e.y));
+              if (CLAMP) { al.x = fminf(0.99f, al.x); al.y = fminf(0.99f, al.y); }
               al.x = al.x >= ALPHA_MIN ? al.x : 0.0f;                             // skip (R2)
               al.y = al.y >= ALPHA_MIN ? al.y : 0.0f;
               const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha); < 0 for a finished pixel
@@ -340,12 +347,18 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
               Cg2[q] = __ffma2_rn(wgt, make_float2(gc.y, gc.y), Cg2[q]);
               Cb2[q] = __ffma2_rn(wgt, make_float2(gc.z, gc.z), Cb2[q]);
               S12[q] = __ffma2_rn(wgt, dd, S12[q]);
-              S22[q] = __ffma2_rn(__fmul2_rn(wgt, dd), dd, S22[q]);
+              S22[q] = __ffma2_rn(wgt, dd2, S22[q]);
             }
             const bool hit = wsum.x + wsum.y > 0.0f;                    // some pixel of the run composited this record
             if (MARK && hit) Bw.contrib[j] = 1;
             open = open && !hit;
            }
+          };
+          for (uint32_t j0 = 0; j0 < cnt; j0 += DENSE_GROUP) {
+           float lmax = B.b[j0].y;
+#pragma unroll
+           for (uint32_t jj = 1; jj < DENSE_GROUP; ++jj) lmax = fmaxf(lmax, B.b[j0 + jj].y);
+           if (lmax > LOG2_O_NEVER_CLAMPED) dense_group(j0, std::true_type()); else dense_group(j0, std::false_type());
            float tmax = fmaxf(T2[0].x, T2[0].y);
 #pragma unroll
            for (int q = 1; q < NQ; ++q) tmax = fmaxf(tmax, fmaxf(T2[q].x, T2[q].y));
