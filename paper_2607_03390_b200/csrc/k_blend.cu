@@ -39,6 +39,13 @@ constexpr float LOG2_ALPHA_MIN_LO = -7.9950f;
 // log2(0.99) = -0.01449957...; a Gaussian with log2 o below this bound (1e-6 relative under 0.99, four times the error of
 // ex2.approx) has alpha = o exp(q) < 0.99 at every pixel (q <= 0), so min(0.99, .) is the identity for it
 constexpr float LOG2_O_NEVER_CLAMPED = -0.014501f;
+// The skip test alpha >= 1/255 of the dense loop costs nothing: the exponent is biased by EX2_BIAS so that alpha = 1/255
+// falls on 2^-126, the smallest normal number -- ex2.approx.ftz flushes every result below it to zero -- and the result is
+// scaled back by EX2_SCALE = 2^-EX2_BIAS (the bias as rounded to fp32, so the scale is exact to 6e-8; the threshold sits at
+// (1 - 5e-7) / 255).  Price: the biased exponent (~ -120) is rounded to 7.6e-6, alpha is good to 5e-6 relative instead of
+// 3e-7 -- far inside the RGB tolerance and the margins the oracle attaches to the skip / stop decisions.
+constexpr float EX2_BIAS = -118.00564575195312f;
+constexpr float EX2_SCALE = 3.3360998530693856e+35f;
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -318,7 +325,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
               nint += count_alive();
             }
             const float dy = ga.y - fpy;
-            const float e1 = fmaf(gb.x * dy, dy, gb.y);                 // D' dy^2 + log2 o
+            const float e1 = fmaf(gb.x * dy, dy, gb.y) + EX2_BIAS;      // D' dy^2 + log2 o (+ the bias of the free skip test)
             const float t0 = fmaf(ga.w, dy, ga.x - fpx);                // t at the first pixel of the run
             const float2 e12 = make_float2(e1, e1), A2 = make_float2(ga.z, ga.z);
             dref = open ? gb.z : dref;                                  // follows the list until the run's first contribution
@@ -331,10 +338,8 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
               const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
-              float2 al = make_float2(ex2_approx(e.x), ex2_approx(e.y));
+              float2 al = __fmul2_rn(make_float2(ex2_approx(e.x), ex2_approx(e.y)), make_float2(EX2_SCALE, EX2_SCALE));   // 0 below 1/255: skip (R2)
               if (CLAMP) { al.x = fminf(0.99f, al.x); al.y = fminf(0.99f, al.y); }
-              al.x = al.x >= ALPHA_MIN ? al.x : 0.0f;                             // skip (R2)
-              al.y = al.y >= ALPHA_MIN ? al.y : 0.0f;
               const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha); < 0 for a finished pixel
               const bool bl0 = Tn.x >= 1.0e-4f, bl1 = Tn.y >= 1.0e-4f;            // else: stop (R2) or already finished
               al.x = bl0 ? al.x : 0.0f; al.y = bl1 ? al.y : 0.0f;
