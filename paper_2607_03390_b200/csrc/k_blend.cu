@@ -46,6 +46,13 @@ constexpr float LOG2_O_NEVER_CLAMPED = -0.014501f;
 // 3e-7 -- far inside the RGB tolerance and the margins the oracle attaches to the skip / stop decisions.
 constexpr float EX2_BIAS = -118.00564575195312f;
 constexpr float EX2_SCALE = 3.3360998530693856e+35f;
+// The dense loop keeps the transmittance scaled, T' = EX2_SCALE T, so that the unscaled ex2 result beta = alpha / EX2_SCALE
+// gives the weight alpha T = beta T' and the update T'(1 - alpha) = T' - EX2_SCALE (beta T') in two packed instructions
+// (instead of scale, 1 - alpha, T (1 - alpha), alpha T); the stop test compares with 1e-4 EX2_SCALE.  Groups that hold a
+// Gaussian with o > 0.99 take alpha = min(0.99, beta EX2_SCALE) and T' (1 - alpha) as written: next to the clamp 1 - alpha
+// must be exact (two clamped Gaussians give T = 0.01^2 against the threshold 1e-4, R33).
+constexpr float EX2_SCALE_INV = 2.997512208892664e-36f;    // 1 / EX2_SCALE
+constexpr float T_STOP_SCALED = 3.3360997079982872e+31f;   // 1e-4f * EX2_SCALE
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -58,6 +65,9 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// T' -> T, sign kept (a finished pixel carries T' < 0); an untouched pixel is exactly 1 (write_pixel and the sparse mode test T == 1)
+__device__ __forceinline__ float unscale_T(float t) { return fabsf(t) == EX2_SCALE ? copysignf(1.0f, t) : t * EX2_SCALE_INV; }
 
 struct Batch {
   float4 a[BLEND_BATCH];     // u, v, A', k
@@ -194,12 +204,12 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
 #pragma unroll
     for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) T2[q] = make_float2(valid[2 * q] ? 1.0f : -1.0f, valid[2 * q + 1] ? 1.0f : -1.0f);
+    for (int q = 0; q < NQ; ++q) T2[q] = make_float2(valid[2 * q] ? EX2_SCALE : -EX2_SCALE, valid[2 * q + 1] ? EX2_SCALE : -EX2_SCALE);   // T' = EX2_SCALE T
     auto get_px = [&](int i) {
       Pixel r;
       const int q = i >> 1;
-      if (i & 1) { r.T = T2[q].y; r.Cr = Cr2[q].y; r.Cg = Cg2[q].y; r.Cb = Cb2[q].y; r.S1 = S12[q].y; r.S2 = S22[q].y; r.d0 = dref; }
-      else { r.T = T2[q].x; r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = dref; }
+      if (i & 1) { r.T = unscale_T(T2[q].y); r.Cr = Cr2[q].y; r.Cg = Cg2[q].y; r.Cb = Cb2[q].y; r.S1 = S12[q].y; r.S2 = S22[q].y; r.d0 = dref; }
+      else { r.T = unscale_T(T2[q].x); r.Cr = Cr2[q].x; r.Cg = Cg2[q].x; r.Cb = Cb2[q].x; r.S1 = S12[q].x; r.S2 = S22[q].x; r.d0 = dref; }
       return r;
     };
     auto count_alive = [&]() {
@@ -311,6 +321,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
           // branch-free: 85 % of the interactions of an alive pixel composite, so every pixel runs the whole update with
           // alpha forced to 0 where it is skipped (alpha < 1/255), stops (T (1 - alpha) < 1e-4) or is finished
           const float2 one2 = make_float2(1.0f, 1.0f), neg2 = make_float2(-1.0f, -1.0f);
+          const float2 scale2 = make_float2(EX2_SCALE, EX2_SCALE), nscale2 = make_float2(-EX2_SCALE, -EX2_SCALE);
           // a group of DENSE_GROUP records; CLAMP = false: none of them can reach alpha = 0.99 (one FMNMX less per pixel)
           auto dense_group = [&](const uint32_t j0, auto clamp_tag) {
            constexpr bool CLAMP = decltype(clamp_tag)::value;
@@ -338,14 +349,21 @@ __global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameCo
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
               const float2 e = __ffma2_rn(__fmul2_rn(A2, tt[q]), tt[q], e12);     // log2(o) + log2 of the falloff
-              float2 al = __fmul2_rn(make_float2(ex2_approx(e.x), ex2_approx(e.y)), make_float2(EX2_SCALE, EX2_SCALE));   // 0 below 1/255: skip (R2)
-              if (CLAMP) { al.x = fminf(0.99f, al.x); al.y = fminf(0.99f, al.y); }
-              const float2 Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));    // T (1 - alpha); < 0 for a finished pixel
-              const bool bl0 = Tn.x >= 1.0e-4f, bl1 = Tn.y >= 1.0e-4f;            // else: stop (R2) or already finished
-              al.x = bl0 ? al.x : 0.0f; al.y = bl1 ? al.y : 0.0f;
-              if (COUNT) nhit += (uint32_t)(al.x > 0.0f) + (uint32_t)(al.y > 0.0f);
-              const float2 wgt = __fmul2_rn(al, T2[q]);               // 0 (or -0) where nothing is composited
-              T2[q].x = bl0 ? Tn.x : -fabsf(T2[q].x);                 // Tn = T where alpha was skipped
+              const float2 be = make_float2(ex2_approx(e.x), ex2_approx(e.y));   // alpha / EX2_SCALE; 0 below 1/255: skip (R2)
+              float2 wgt, Tn;                                                      // alpha T and T' (1 - alpha); Tn < 0 for a finished pixel
+              if (CLAMP) {
+                float2 al = __fmul2_rn(be, scale2);
+                al.x = fminf(0.99f, al.x); al.y = fminf(0.99f, al.y);
+                Tn = __fmul2_rn(T2[q], __ffma2_rn(al, neg2, one2));
+                wgt = __fmul2_rn(al, __fmul2_rn(T2[q], make_float2(EX2_SCALE_INV, EX2_SCALE_INV)));
+              } else {
+                wgt = __fmul2_rn(be, T2[q]);
+                Tn = __ffma2_rn(wgt, nscale2, T2[q]);
+              }
+              const bool bl0 = Tn.x >= T_STOP_SCALED, bl1 = Tn.y >= T_STOP_SCALED;   // else: stop (R2) or already finished
+              wgt.x = bl0 ? wgt.x : 0.0f; wgt.y = bl1 ? wgt.y : 0.0f;                // 0 where nothing is composited
+              if (COUNT) nhit += (uint32_t)(wgt.x > 0.0f) + (uint32_t)(wgt.y > 0.0f);
+              T2[q].x = bl0 ? Tn.x : -fabsf(T2[q].x);                 // Tn = T' where alpha was skipped
               T2[q].y = bl1 ? Tn.y : -fabsf(T2[q].y);
               wsum = __fadd2_rn(wsum, wgt);
               Cr2[q] = __ffma2_rn(wgt, make_float2(gc.x, gc.x), Cr2[q]);
