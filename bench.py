@@ -27,14 +27,14 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full render"
-# Lane-instructions one alive (pixel, Gaussian) interaction of the blend needs: 11.5 on the FMA pipe
-# (exponent 2, 1 - alpha, T (1 - alpha), alpha T, 3 colour FMAs, w dd, 2 moment FMAs; per run of 4 pixels d - d_ref and the
-# sum of the weights, 1/4 each; a packed FFMA2 half counts as 1) + 1 MUFU.EX2 + 6.5 on the ALU pipe (clamp, 2 threshold
-# tests, 3 selects; per run the any-pixel-composited test and the select of d_ref).
-BLEND_LANE_INSTR = 19.0
+# Lane-instructions one alive (pixel, Gaussian) interaction of the blend needs: 9.5 on the FMA pipe
+# (exponent 2, weight, update of T', 3 colour FMAs, 2 moment FMAs; per run of 4 pixels d - d_ref, its square and the sum of
+# the weights, 1/4 each; a packed FFMA2 half counts as 1) + 1 MUFU.EX2 + 3.5 on the ALU pipe (stop test, 2 selects; per run
+# the any-pixel-composited test and the select of d_ref).
+BLEND_LANE_INSTR = 14.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_blend<1,0> launch on config 3, from the ncu --set full capture
-# summarised in profiles/r1h_top_kernels.md (the file names the command); per launch, like `achieved`.
-BLEND_DRAM_TRAFFIC_BYTES = 47.3e6
+# summarised in profiles/r1i_top_kernels.md (the file names the command); per launch, like `achieved`.
+BLEND_DRAM_TRAFFIC_BYTES = 48.6e6
 
 
 def _peaks():
@@ -280,7 +280,7 @@ def run_ours(args):
         roof = {"kernel": "k_blend", "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-instr/s",
                 "frac": ach / alu_peak, "traffic": BLEND_DRAM_TRAFFIC_BYTES, "interactions_per_launch": float(L),
                 "blended_per_launch": mean("n_blended"), "pixel_slots_per_launch": mean("n_pixel_slots"),
-                "ms_per_launch": t * 1e3,
+                "ms_per_launch": t * 1e3, "lane_instr_per_interaction": BLEND_LANE_INSTR,
                 "peak_note": f"148 SM x 4 schedulers x 32 lanes x {sm_clk:.0f} MHz (median SM clock during the run): one warp "
                              f"instruction per scheduler and clock; the FMA pipe (128 lanes/clk/SM) and the ALU pipe (64) are not tighter "
                              f"for this mix (DESIGN.md 7.2)"}
