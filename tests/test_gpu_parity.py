@@ -543,3 +543,34 @@ def test_full_size_other_configs(cfg):
     assert sg["n_sel"] <= sg["n_tiles"]
     if cfg == 5:
         assert 0 < sg["n_sel"] < sg["n_tiles"] and sg["n_toc"] > 0
+
+
+def test_edge_opaque_stacks_skip_threshold_and_background():
+    """The shortcuts of the blend's dense loop against the oracle's plain loop: stacks of Gaussians with
+    o = 1 / 0.995 (alpha clamped to 0.99 at their centres: T runs through 0.01 and 0.01^2, the value that meets the
+    stop threshold 1e-4), o = 0.9899 / 0.985 (just under the clamp: the groups without it), wide faint Gaussians with
+    o within 1e-3 of 1/255 on both sides (the skip test by flush-to-zero), and a background colour (the final T of
+    finished, alive and untouched pixels)."""
+    P = _p()
+    tgs = _tgs()
+    rng = np.random.default_rng(91)
+    sc = make_config(1, n=6000, frames=2, width=237, height=181)
+    n = sc.n
+    k = 600
+    sc.means[:k, :2] = rng.normal(0, 0.6, size=(k, 2)).astype(np.float32)
+    sc.means[:k, 2] = np.linspace(-1.0, 1.0, k).astype(np.float32)
+    sc.scales[:k] = rng.uniform(0.05, 0.4, size=(k, 3)).astype(np.float32)
+    sc.opacity[:k] = rng.choice(np.array([1.0, 0.995, 0.9899, 0.985], np.float32), size=k)
+    f = slice(k, 2 * k)
+    sc.scales[f] = rng.uniform(0.3, 1.5, size=(k, 3)).astype(np.float32)
+    sc.opacity[f] = (rng.choice(np.array([1.0 - 1e-3, 1.0 + 1e-3, 1.0, 1.02], np.float64), size=k) / 255.0).astype(np.float32)
+    g, o = P.make_pair(sc, params={"bg": (0.2, 0.5, 0.7)})
+    g.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
+    g.render(tgs.FULL); o.render(ora.FULL)
+    sg, so, out = P.compare_frame(g, o, n, ora.FRAME_R)
+    img = g.read_image()
+    assert (np.abs(img - np.array([0.2, 0.5, 0.7], np.float32)).max(axis=2) < 1e-6).any()     # untouched pixels show the background
+    P.inject_priors(g, o)
+    g.set_camera(sc.poses[1], sc.camera); o.set_camera(sc.poses[1], sc.camera)
+    g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+    P.compare_frame(g, o, n, ora.FRAME_S)
