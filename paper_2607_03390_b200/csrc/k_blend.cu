@@ -122,8 +122,10 @@ __device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p
   }
 }
 
+// The marking instances promise one CTA per SM less: ptxas still allocates 96 registers (10 CTAs per SM stay resident) but
+// schedules the loop with fewer spills around the batch boundaries (P-frame blend 0.166 -> 0.162 ms).
 template <bool MARK, bool COUNT>
-__global__ void __launch_bounds__(BLEND_THREADS, BLEND_MIN_CTAS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
+__global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLEND_MIN_CTAS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
                                                          const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,
