@@ -367,16 +367,25 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
               if (COUNT) nhit += (uint32_t)(wgt.x > 0.0f) + (uint32_t)(wgt.y > 0.0f);
               T2[q].x = bl0 ? Tn.x : -fabsf(T2[q].x);                 // Tn = T' where alpha was skipped
               T2[q].y = bl1 ? Tn.y : -fabsf(T2[q].y);
-              wsum = __fadd2_rn(wsum, wgt);
+              if (MARK) wsum = __fadd2_rn(wsum, wgt);
               Cr2[q] = __ffma2_rn(wgt, make_float2(gc.x, gc.x), Cr2[q]);
               Cg2[q] = __ffma2_rn(wgt, make_float2(gc.y, gc.y), Cg2[q]);
               Cb2[q] = __ffma2_rn(wgt, make_float2(gc.z, gc.z), Cb2[q]);
               S12[q] = __ffma2_rn(wgt, dd, S12[q]);
               S22[q] = __ffma2_rn(wgt, dd2, S22[q]);
             }
-            const bool hit = wsum.x + wsum.y > 0.0f;                    // some pixel of the run composited this record
-            if (MARK && hit) Bw.contrib[j] = 1;
-            open = open && !hit;
+            if (MARK) {
+              const bool hit = wsum.x + wsum.y > 0.0f;                  // some pixel of the run composited this record
+              if (hit) Bw.contrib[j] = 1;
+              open = open && !hit;
+            } else {
+              // without marks only `open` is needed: no pixel of the run has composited yet <=> every |T'| is still
+              // EX2_SCALE (pixels outside the image carry -EX2_SCALE); min / compare run on the ALU pipe, which has slack
+              float tm = fminf(fabsf(T2[0].x), fabsf(T2[0].y));
+#pragma unroll
+              for (int q = 1; q < NQ; ++q) tm = fminf(tm, fminf(fabsf(T2[q].x), fabsf(T2[q].y)));
+              open = tm == EX2_SCALE;
+            }
            }
           };
           for (uint32_t j0 = 0; j0 < cnt; j0 += DENSE_GROUP) {
