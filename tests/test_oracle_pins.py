@@ -869,3 +869,148 @@ def test_f4_ply_round_trip_of_a_synthetic_scene(tmp_path):
     np.testing.assert_array_equal(d["means"], sc.means); np.testing.assert_array_equal(d["sh"], sc.sh)
     np.testing.assert_array_equal(d["quats"], sc.quats)
     np.testing.assert_allclose(d["scales"], sc.scales, rtol=1e-6); np.testing.assert_allclose(d["opacity"], sc.opacity, rtol=1e-5, atol=1e-7)
+
+
+# ----------------------------------------------------------------------------------------- stitch: the bilinear tap
+def _stitch_ctx(cam, Z0, tab, Vnew):
+    """Priors = a fronto-parallel plane at Z0 seen from the identity pose, TAB = `tab`; no Gaussian is visible (the only
+    one sits behind the camera), so T^oc is empty and T_sel = T^um: the interior tiles are stitched (Eq.4)."""
+    D = np.full((cam.H, cam.W), Z0, np.float32)
+    o = _prior_ctx(cam, np.eye(4), D, np.zeros_like(D), image=tab)
+    o.set_camera(Vnew, cam)
+    assert o.render(ora.TEMPORAL) == ora.FRAME_S
+    st = o.stats()
+    assert st["n_pairs"] == 0 and st["n_sel_oc"] == 0
+    mask = o.read_tile_mask()
+    stitched = np.kron((mask & 4) == 0, np.ones((16, 16), bool))[: cam.H, : cam.W]
+    return o, stitched
+
+
+def test_stitch_bilinear_tap_reproduces_linear_and_xy_ramps_at_fractional_offsets():
+    """PAPER.md:L101 ("Here we use bilinear interpolation"), Eq.4 L125.  A camera translation with f b / Z0 = 3 + 1/4 px
+    in x and 2 + 1/3 px in y maps every stitched pixel (px, py) to the TAB position (px - 3.25, py - 2.333...).  Bilinear
+    interpolation reproduces a + b x + c y + d x y exactly, so the stitched image is that polynomial at the shifted
+    position in closed form.  Swapping wx / wy, or the taps v10 / v01, changes the result by (b - c)(wy - wx) != 0."""
+    cam = Camera(W=80, H=64, fx=100.0, fy=100.0, cx=39.5, cy=31.5)
+    Z0, sx, sy = 5.0, 3.25, 2.0 + 1.0 / 3.0
+    ys, xs = np.meshgrid(np.arange(cam.H, dtype=np.float64), np.arange(cam.W, dtype=np.float64), indexing="ij")
+    coef = [(0.10, 0.004, 0.0010, 0.0), (0.70, -0.003, 0.0050, 0.0), (0.05, 0.002, 0.0030, 0.00008)]   # a, b, c, d per channel
+    poly = lambda x, y: np.stack([a + b * x + c * y + d * x * y for (a, b, c, d) in coef], -1)
+    tab = poly(xs, ys)
+    Vnew = np.eye(4)
+    Vnew[0, 3], Vnew[1, 3] = sx * Z0 / cam.fx, sy * Z0 / cam.fy
+    o, stitched = _stitch_ctx(cam, Z0, tab, Vnew)
+    assert stitched[16:, 16:].all() and stitched.sum() >= 64 * 48            # every interior tile is stitched
+    img = o.read_image()
+    exp = poly(xs - sx, ys - sy)
+    np.testing.assert_allclose(img[stitched], exp[stitched], atol=3e-6)
+    # the check has teeth: the transposed weights would be off by |b - c| |wy - wx| = 0.001 / 12 ... 0.008 / 12
+    wrong = poly(np.floor(xs - sx) + (sy - 2.0), np.floor(ys - sy) + (sx - 3.0))
+    assert np.abs(wrong - exp)[stitched].min(axis=0).max() > 5e-5
+    d, s = o.read_depth()
+    assert np.all(d[stitched] == np.float32(Z0)) and np.all(s[stitched] == 0)       # R31: repaired depth, warped sigma
+
+
+def test_stitch_bilinear_tap_matches_library_interpolation_on_a_random_tab():
+    """Same stitch on a random (non-linear) TAB and a general pose: every stitched pixel equals
+    scipy.ndimage.map_coordinates(order=1) at the oracle's own backward correspondence (x, y) (L121), and four pixels
+    are written out by hand from their four taps."""
+    from scipy.ndimage import map_coordinates
+    rng = np.random.default_rng(11)
+    cam = Camera(W=96, H=80, fx=110.0, fy=105.0, cx=47.5, cy=39.5)
+    tab = rng.uniform(0, 1, size=(cam.H, cam.W, 3))
+    a = math.radians(0.8)
+    Vnew = np.eye(4)
+    Vnew[:3, :3] = [[math.cos(a), 0, -math.sin(a)], [0, 1, 0], [math.sin(a), 0, math.cos(a)]]
+    Vnew[:3, 3] = [0.07, -0.05, 0.1]
+    o, stitched = _stitch_ctx(cam, 4.0, tab, Vnew)
+    assert stitched.sum() > 2000
+    xy = o.get("corr_xy").reshape(cam.H, cam.W, 2).astype(np.float64)
+    img = o.read_image()
+    tab32 = tab.astype(np.float32).astype(np.float64)
+    frac = xy - np.floor(xy)
+    assert (np.abs(frac[stitched] - 0.5) < 0.45).mean() > 0.5               # genuinely fractional positions
+    for ch in range(3):
+        ref = map_coordinates(tab32[..., ch], [xy[..., 1][stitched], xy[..., 0][stitched]], order=1, mode="nearest")
+        np.testing.assert_allclose(img[..., ch][stitched], ref, atol=2e-6)
+    pts = np.argwhere(stitched)[[5, 400, 1100, 1900]]
+    for (py, px) in pts:
+        x, y = xy[py, px]
+        i, j = int(math.floor(x)), int(math.floor(y))
+        fx_, fy_ = x - i, y - j
+        assert 0 <= i < cam.W - 1 and 0 <= j < cam.H - 1
+        top = tab32[j, i] * (1 - fx_) + tab32[j, i + 1] * fx_              # row j: left tap (i), right tap (i + 1)
+        bot = tab32[j + 1, i] * (1 - fx_) + tab32[j + 1, i + 1] * fx_      # row j + 1
+        np.testing.assert_allclose(img[py, px], top * (1 - fy_) + bot * fy_, atol=2e-6)
+
+
+# ----------------------------------------------------------------------------------------- P6b: SH bands 2, 3 at generic directions
+def test_p6_sh_all_16_functions_at_generic_directions_vs_complex_harmonics():
+    """R5: real SH that keep the Condon-Shortley phase, order m = -l..l:  Y_l^0;  sqrt2 Re Y_l^m (m > 0);
+    sqrt2 Im Y_l^|m| (m < 0), with Y_l^m the complex harmonics of scipy.special (Condon-Shortley phase included).  At a
+    generic direction every one of the 16 functions is non-zero, so an exchange or a sign flip inside a band fails."""
+    from scipy.special import sph_harm_y
+    rng = np.random.default_rng(12)
+    dirs = [np.array([1.0, 2.0, 3.0]) / math.sqrt(14.0)] + [v / np.linalg.norm(v) for v in rng.normal(size=(5, 3))]
+    for d in dirs:
+        theta, phi = math.acos(d[2]), math.atan2(d[1], d[0])
+        exp = np.zeros(16)
+        for l in range(4):
+            for m in range(-l, l + 1):
+                Yc = sph_harm_y(l, abs(m), theta, phi)
+                exp[l * l + l + m] = Yc.real if m == 0 else math.sqrt(2.0) * (Yc.real if m > 0 else Yc.imag)
+        Y = ora.sh_basis(3, d)
+        np.testing.assert_allclose(Y, exp, atol=1e-12)
+    # the values at (1, 2, 3)/sqrt(14), from the closed forms R5 lists, signs included
+    x, y, z = dirs[0]
+    assert np.abs(ora.sh_basis(3, dirs[0])).min() > 0.02                     # all 16 functions are away from zero there
+    hand = {4: 1.0925484305920792 * x * y, 5: -1.0925484305920792 * y * z, 7: -1.0925484305920792 * x * z,
+            8: 0.5462742152960396 * (x * x - y * y), 10: 2.890611442640554 * x * y * z, 15: -0.5900435899266435 * x * (x * x - 3 * y * y)}
+    Y = ora.sh_basis(3, dirs[0])
+    for k, v in hand.items():
+        assert abs(Y[k] - v) < 1e-12
+    assert Y[4] > 0 and Y[5] < 0 and Y[7] < 0 and Y[8] < 0 and Y[10] > 0 and Y[15] > 0
+
+
+# ----------------------------------------------------------------------------------------- P3c: decisions ON the thresholds
+def _stack_1px(opacities):
+    """Coincident Gaussians on the optical axis of a 1 x 1 image: q = 0, so alpha = o exactly at the only pixel."""
+    cam = Camera(W=1, H=1, fx=50.0, fy=50.0, cx=0.0, cy=0.0)
+    K = len(opacities)
+    z = 2.0 + 0.01 * np.arange(K)
+    o = Oracle()
+    _one(o, np.stack([np.zeros(K), np.zeros(K), z], 1), np.full((K, 3), 0.5), np.tile([1, 0, 0, 0], (K, 1)), opacities,
+         np.full((K, 3), 1.0), cam)
+    o.render(ora.FULL)
+    return o.get("rendered").astype(int).tolist(), float(o.read_image()[0, 0, 0])
+
+
+def test_p3_stop_decision_on_the_threshold_is_the_fp32_sequence():
+    """R2 / R33: "stop when T (1 - alpha) < 1e-4", decided in fp32 in the written order.  (a) Two alpha-clamped Gaussians:
+    (1 - 0.99f)^2 = 9.99998e-5 < 1e-4f in fp32 (in fp64 (1 - 0.99)^2 > 1e-4): the second one stops the loop and is not in
+    G_rendered.  (b) Three opacities chosen so that the fp32 product lands EXACTLY on 1e-4f: "<" is strict, so the third is
+    blended and the fourth stops.  The expected decisions are evaluated here in numpy float32."""
+    f = np.float32
+    c = Y00 * 1.0 + 0.5
+    T1 = f(1) - f(0.99)
+    assert f(T1 * T1) < f(1e-4) and (1.0 - 0.99) * (1.0 - 0.99) > 1e-4
+    ren, v = _stack_1px([1.0, 1.0, 0.5])
+    assert ren == [1, 0, 0]
+    assert abs(v - 0.99 * c) < 1e-6
+    o1, o2, o3 = f(0.9161449670791626), f(0.9036414623260498), f(0.9876239895820618)
+    T = f(f(f(1) - o1) * (f(1) - o2))
+    assert f(T * (f(1) - o3)) == f(1e-4) and o3 < f(0.99)                    # exactly on the threshold, below the clamp
+    ren, v = _stack_1px([o1, o2, o3, 0.5])
+    assert ren == [1, 1, 1, 0]                                               # not "<" -> blended; the next one stops
+    w3 = float(o3) * (1 - float(o1)) * (1 - float(o2))
+    assert abs(v - c * (float(o1) + float(o2) * (1 - float(o1)) + w3)) < 1e-6
+
+
+def test_p3_skip_decision_on_the_threshold():
+    """R2: "skip alpha < 1/255": alpha = 1/255f exactly is kept, the next float below is skipped."""
+    f = np.float32
+    a = f(1.0) / f(255.0)
+    ren, v = _stack_1px([a])
+    assert ren == [1] and abs(v - float(a) * (Y00 + 0.5)) < 1e-9
+    ren, v = _stack_1px([np.nextafter(a, f(0))])
+    assert ren == [0] and v == 0.0
