@@ -6,7 +6,7 @@ and full render every frame, on the CUDA path through the C-ABI (BASELINE.json: 
 
 A step = one frame of the trajectory = one pass of the whole hot path (A0-A10 of DESIGN.md §1).  With N > 1
 (torchrun) every rank renders the same trajectory on its own GPU: the path does not shard ("replicas only",
-DESIGN.md §9), so `value` is the sum of the ranks' frames over the slowest rank's time ("weak").
+DESIGN.md §8), so `value` is the sum of the ranks' frames over the slowest rank's time ("weak").
 `--impl reference` times the CPU oracle as it stands on the host cores (rank 0 only).
 Prints ONE JSON line (rank 0).
 """

@@ -55,14 +55,19 @@ class OraSched(C.Structure):
 
 
 def build(force: bool = False) -> str:
-    """Compile oracle/ora.cpp -> oracle/libora.so (g++ -O2, no contraction, no fast-math)."""
-    if (not force and os.path.exists(_SO)
-            and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
-        return _SO
-    cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-shared", "-fPIC",
-           "-o", _SO, _SRC]
-    subprocess.run(cmd, check=True)
-    return _SO
+    """Compile oracle/ora.cpp -> oracle/libora.so (g++ -O2, no contraction, no fast-math).
+    ORA_SANITIZE=1 builds oracle/libora_san.so with -fsanitize=address,undefined instead (run the pins under
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so); profiles/r2_sanitizers.md has the command and its result)."""
+    san = os.environ.get("ORA_SANITIZE") == "1"
+    so = os.path.join(_HERE, "libora_san.so") if san else _SO
+    if (not force and os.path.exists(so)
+            and os.path.getmtime(so) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
+        return so
+    cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-shared", "-fPIC"]
+    if san:
+        cmd += ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+    subprocess.run(cmd + ["-o", so, _SRC], check=True)
+    return so
 
 
 _lib = None

@@ -23,7 +23,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE
 SOURCES = {
     "tgs_api.cu": [],
     "k_decide.cu": ["-fmad=false"],
-    "k_bin.cu": ["-fmad=false"],       # the tile test is decision arithmetic (decide_math.cuh)       # k_emit repeats the tile test of k_count_color (decide_math.cuh)
+    "k_bin.cu": ["-fmad=false"],       # the tile test is decision arithmetic (decide_math.cuh)
     "k_sort.cu": [],
     "k_blend.cu": [],
     "tgs_ply.cu": [],

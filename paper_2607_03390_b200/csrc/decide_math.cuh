@@ -1,5 +1,5 @@
-// decide_math.cuh -- fp32 decision arithmetic shared by the kernels that must take the SAME decision twice
-// (pair counting in k_decide.cu, pair emission in k_bin.cu).  Only translation units compiled with
+// decide_math.cuh -- fp32 decision arithmetic shared by the kernels that take the tile test box-min q <= tau
+// (T^oc marks in k_decide.cu, pair emission in k_bin.cu).  Only translation units compiled with
 // -fmad=false may include it: every +,-,*,/ is one IEEE rounding in the order written (DESIGN.md §2 R33).
 // NOT shared with oracle/.
 #pragma once

@@ -73,13 +73,17 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
                                                             uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
                                                             const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
                                                             uint4* __restrict__ bin_params,
-                                                            Counters* __restrict__ counters, unsigned long long max_tests) {
+                                                            Counters* __restrict__ counters, unsigned long long max_tests,
+                                                            volatile uint32_t* __restrict__ host_overflow) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   __shared__ uint32_t s_tile, s_warp[SCAN_THREADS / 32], s_excl;
   const uint32_t n = counters->n_visible;
   if (n == 0 || counters->area_sum > max_tests) {
-    if (blockIdx.x == 0 && threadIdx.x == 0) { counters->n_tests = 0; counters->n_pairs = 0; if (n) counters->overflow = 1; }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+      counters->n_tests = 0; counters->n_pairs = 0;
+      if (n) { counters->overflow = 1; *host_overflow = 1u; __threadfence_system(); }
+    }
     return;
   }
   const uint32_t num_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
@@ -216,7 +220,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
                                                      const uint32_t* __restrict__ sel_bits, unsigned long long* __restrict__ desc,
                                                      uint32_t* __restrict__ keys,
                                                      uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
-                                                     Counters* __restrict__ counters) {
+                                                     Counters* __restrict__ counters, volatile uint32_t* __restrict__ host_overflow) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   __shared__ BinSmem<TileT> sm;
@@ -309,7 +313,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
       const uint32_t cexcl = sm.excl, ctotal = pend_total, incl_total = cexcl + ctotal, pbuf = buf ^ 1u;
       const bool overflow = incl_total > fc.max_pairs;
       if (pend == num_chunks - 1 && tid == 0) {
-        if (overflow) { counters->overflow = 1; counters->n_pairs = 0; }
+        if (overflow) { counters->overflow = 1; counters->n_pairs = 0; *host_overflow = 1u; __threadfence_system(); }   // the host reads it after ev_bin
         else counters->n_pairs = incl_total;
       }
       if (!overflow)
@@ -385,19 +389,20 @@ uint32_t scan_tile_items() { return SCAN_TILE; }
 uint32_t bin_chunk_items() { return BIN_CHUNK; }
 
 // sorted_g_idx: which of cvals[] holds the visible Gaussians in (depth, index) order
-void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms) {
+void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms,
+                uint32_t* host_overflow) {
   const uint32_t scan_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_visible <= N)
   const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
   const uint32_t* sorted_g = b.cvals[sorted_g_idx];
   uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
-                                                      b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests);
+                                                      b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
   if (fc.n_tiles <= 65536)
     TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters, (volatile uint32_t*)host_overflow);
   else
     TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters);
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters, (volatile uint32_t*)host_overflow);
 }
 
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
 }
 
 // ------------------------------------------------------------------ A3 preprocess (+AFC +TOC +newly-visible +T^oc)
-// Persistent grid; a work item is a chunk of 1024 consecutive Gaussians (ticket order), 4 per thread.
+// Persistent grid; a work item is a chunk of 2048 consecutive Gaussians (ticket order): two phase-A passes of 1024, 4 per thread.
 //  phase A (all Gaussians, 16 B each): near cull, projection of the mean, AFC, TOC + newly-visible lookups in the
 //          warped TGB, and a conservative off-screen test; the survivors are compacted in shared memory;
 //  phase B (survivors only, +32 B each): EWA covariance, conic, radius, rect, records, T^oc marks of small rects;
@@ -388,8 +388,10 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       // wholly outside that box, enlarged by 1 %, has q_min >= 1.02 tau in exact arithmetic, and the fp32 evaluation of the
       // oracle differs from it by at most ~1e-6 (18 kappa + 1700) -- below 0.02 tau when cond(Sigma') <= 400 and tau >= 0.5
       // (DESIGN.md §7).  Otherwise, and when the box would be empty, the whole rect is kept (or one tile of it).
+      // exact_tiles = 0 (tgs.h): "intersect" = every tile of the 3-sigma rect, so the test rect IS the rect.
       uint32_t tx_lo = x_lo, tx_hi = x_hi, ty_lo = y_lo, ty_hi = y_hi;
-      if (!(tau >= 0.0f)) { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }              // o < 1/255: reaches nothing; one (failing) test
+      if (!fc.exact_tiles) {}
+      else if (!(tau >= 0.0f)) { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }         // o < 1/255: reaches nothing; one (failing) test
       else if (tau >= 0.5f && lam * lam <= 400.0f * det) {
         const float ex = sqrtf(tau * a) * 1.01f + 0.01f, ey = sqrtf(tau * cc) * 1.01f + 0.01f;
         const float fx_lo = ceilf((u - ex - 15.0f) / 16.0f), fx_hi = floorf((u + ex) / 16.0f) + 1.0f;

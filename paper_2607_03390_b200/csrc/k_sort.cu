@@ -201,15 +201,17 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
         if (ranges) {
           // A7 in the last pass (the keys are the tile ids, now fully sorted): ranges[t] = {~start, end}, zero = empty.
           // Inside a digit segment of this tile the neighbours in shared memory are the neighbours of the final list,
-          // so a change of tile id is a boundary written with plain stores; at the ends of a segment the neighbour
-          // belongs to another tile of the sort, so start / end go through atomicMax (max of ~o = min of o).
+          // so a change of tile id is a boundary; at the ends of a segment the neighbour belongs to another tile of the
+          // sort, so start / end are candidates combined by atomicMax (max of ~o = min of o).
           const uint32_t dg = (uint32_t)(k >> shift) & 255u;
           const uint32_t kp = p > 0 ? sm.keys[p - 1] : 0xffffffffu;
           const bool seg_first = p == 0 || ((uint32_t)(kp >> shift) & 255u) != dg;
           bool seg_last = p + 1 >= valid;
           if (!seg_last) seg_last = ((uint32_t)(sm.keys[p + 1] >> shift) & 255u) != dg;
+          // every update is an atomicMax (a tile's range may be touched by several CTAs: no plain store ever meets an
+          // atomic on the same word)
           if (seg_first) atomicMax(&ranges[k].x, ~o);
-          else if (kp != k) { ranges[k].x = ~o; ranges[kp].y = o; }
+          else if (kp != k) { atomicMax(&ranges[k].x, ~o); atomicMax(&ranges[kp].y, o); }
           if (seg_last) atomicMax(&ranges[k].y, o + 1u);
         }
       }
@@ -220,6 +222,12 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_onesweep(
 }  // namespace
 
 uint32_t sort_tile_items() { return SORT_THREADS * SORT_IPT_SMALL; }   // capacity of the descriptor arrays: the smaller tile
+
+// Per-device function attributes (dynamic shared memory above 48 KB); tgs_create calls this for the context's device.
+void sort_prepare_device() {
+  cudaFuncSetAttribute(k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_BIG>));
+  cudaFuncSetAttribute(k_onesweep<32, 2, SORT_IPT_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_SMALL>));
+}
 
 int tile_sort_passes(int n_tiles) {
   int tile_bits = 1;
@@ -233,12 +241,6 @@ int tile_sort_passes(int n_tiles) {
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms, bool small_input, uint2* ranges) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_BIG>));
-    cudaFuncSetAttribute(k_onesweep<32, 2, SORT_IPT_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_SMALL>));
-    attr_set = true;
-  }
   const int passes = (key_bits + 7) / 8;
   int cur = 0;
   for (int p = 0; p < passes; ++p) {

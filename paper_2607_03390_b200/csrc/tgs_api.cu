@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <exception>
 #include <string>
 #include <vector>
 
@@ -69,6 +70,12 @@ struct tgs_ctx {
   cudaStream_t side2 = nullptr;         // third stream: SH colours beside the depth sort
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr, ev_fork3 = nullptr;
   bool sel_pending = false;
+  // pair-buffer overflow of the previous frame: k_bin stores the flag into pinned memory (zero-copy) and ev_bin marks the
+  // end of that kernel; the next tgs_render waits for it (mid-frame: tile sort and blend are still running) before it
+  // decides the frame type, so that priors committed by an overflowed frame are never used
+  uint32_t* h_ovf = nullptr;            // pinned, [2] by frame parity
+  cudaEvent_t ev_bin = nullptr;
+  bool bin_pending = false; int bin_slot = 0;
   uint32_t nv_hint = 0;                 // visible Gaussians of a recent frame (selects the depth-sort instance)
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
@@ -225,63 +232,73 @@ void tgs_default_params(tgs_params* p) {
   p->tgb_downscale = 1;
 }
 
-int tgs_create(tgs_ctx** out, int device, void* stream) {
-  if (!out) return TGS_E_INVALID_ARG;
-  *out = nullptr;
+static void destroy_ctx(tgs_ctx* c) {   // tolerates a partially constructed context (tgs_create's failure paths)
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  for (cudaStream_t* st : {&c->side, &c->side2, &c->copy}) if (*st) { cudaStreamSynchronize(*st); cudaStreamDestroy(*st); *st = nullptr; }
+  free_list(c, c->allocs_scene); free_list(c, c->allocs_frame); free_list(c, c->allocs_pairs);
+  for (auto& p : c->counters2) if (p) cudaFree(p);
+  if (c->F_base) cudaFree(c->F_base);
+  if (c->b.sort_hist) cudaFree(c->b.sort_hist);
+  if (c->h_counters) cudaFreeHost(c->h_counters);
+  if (c->h_sel) cudaFreeHost(c->h_sel);
+  if (c->h_ovf) cudaFreeHost(c->h_ovf);
+  for (auto& e : c->ev_cnt) if (e) cudaEventDestroy(e);
+  for (auto& e : c->ev_copy) if (e) cudaEventDestroy(e);
+  for (auto& e : c->ev_stage) if (e) cudaEventDestroy(e);
+  for (cudaEvent_t* e : {&c->ev_post, &c->ev_post2, &c->ev_sel, &c->ev_done, &c->ev_bin, &c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2, &c->ev_fork3})
+    if (*e) cudaEventDestroy(*e);
+  delete c;
+}
+
+static int create_impl(tgs_ctx** out, int device, void* stream) {
   int count = 0;
   if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return TGS_E_CUDA;
   tgs_ctx* c = new tgs_ctx();
   c->device = device; c->stream = (cudaStream_t)stream;
+  for (auto& e : c->ev_stage) e = nullptr;
   tgs_default_params(&c->prm);
-  auto fail = [&](int code) { delete c; return code; };
-  if (cudaSetDevice(device) != cudaSuccess) return fail(TGS_E_CUDA);
+  bool ok = cudaSetDevice(device) == cudaSuccess;
   cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(TGS_E_CUDA);
-  c->num_sms = prop.multiProcessorCount;
-  if (cudaMallocHost((void**)&c->h_counters, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
-  if (cudaMallocHost((void**)&c->h_sel, 2 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
-  memset(c->h_counters, 0, sizeof(Counters));
-  for (auto& p : c->counters2) if (cudaMalloc((void**)&p, sizeof(Counters)) != cudaSuccess) return fail(TGS_E_CUDA);
+  ok = ok && cudaGetDeviceProperties(&prop, device) == cudaSuccess;
+  if (ok) c->num_sms = prop.multiProcessorCount;
+  ok = ok && cudaMallocHost((void**)&c->h_counters, sizeof(Counters)) == cudaSuccess;
+  ok = ok && cudaMallocHost((void**)&c->h_sel, 2 * sizeof(uint32_t)) == cudaSuccess;
+  ok = ok && cudaMallocHost((void**)&c->h_ovf, 2 * sizeof(uint32_t)) == cudaSuccess;
+  if (ok) { memset(c->h_counters, 0, sizeof(Counters)); c->h_ovf[0] = c->h_ovf[1] = 0; c->h_sel[0] = c->h_sel[1] = 0; }
+  for (auto& p : c->counters2) ok = ok && cudaMalloc((void**)&p, sizeof(Counters)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->F_base, 8 * sizeof(uint32_t)) == cudaSuccess;   // two F's, by frame parity
+  ok = ok && cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) == cudaSuccess;
+  for (auto& e : c->ev_cnt) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+  for (auto& e : c->ev_copy) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+  for (cudaEvent_t* e : {&c->ev_post, &c->ev_post2, &c->ev_sel, &c->ev_done, &c->ev_bin, &c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2, &c->ev_fork3})
+    ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+  for (cudaStream_t* st : {&c->side, &c->side2, &c->copy}) ok = ok && cudaStreamCreateWithFlags(st, cudaStreamNonBlocking) == cudaSuccess;
+  for (auto& e : c->ev_stage) ok = ok && cudaEventCreate(&e) == cudaSuccess;
+  if (!ok) { cudaGetLastError(); destroy_ctx(c); return TGS_E_CUDA; }
   c->b.counters = c->counters2[0];
-  for (auto& e : c->ev_cnt) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-  cudaEventCreateWithFlags(&c->ev_post, cudaEventDisableTiming);
-  cudaEventCreateWithFlags(&c->ev_post2, cudaEventDisableTiming);
-  if (cudaMalloc((void**)&c->F_base, 8 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);   // two F's, by frame parity
   c->b.F_key = c->F_base;
-  if (cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) != cudaSuccess) return fail(TGS_E_CUDA);
-  cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming);
-  cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming);
-  cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
-  cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking);
-  cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking);
-  for (auto& e : c->ev_copy) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-  for (cudaEvent_t* e : {&c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2, &c->ev_fork3}) cudaEventCreateWithFlags(e, cudaEventDisableTiming);
-  for (auto& e : c->ev_stage) cudaEventCreate(&e);
+  sort_prepare_device();
   *out = c;
   return TGS_OK;
 }
 
-void tgs_destroy(tgs_ctx* c) {
-  if (!c) return;
-  cudaSetDevice(c->device);
-  cudaStreamSynchronize(c->stream);
-  free_list(c, c->allocs_scene); free_list(c, c->allocs_frame); free_list(c, c->allocs_pairs);
-  for (auto p : c->counters2) cudaFree(p);
-  for (auto e : c->ev_cnt) cudaEventDestroy(e);
-  cudaEventDestroy(c->ev_post); cudaEventDestroy(c->ev_post2);
-  cudaFree(c->F_base); cudaFree(c->b.sort_hist);
-  cudaFreeHost(c->h_counters); cudaFreeHost(c->h_sel);
-  cudaEventDestroy(c->ev_sel); cudaEventDestroy(c->ev_done);
-  cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side);
-  cudaStreamSynchronize(c->side2); cudaStreamDestroy(c->side2);
-  cudaStreamSynchronize(c->copy); cudaStreamDestroy(c->copy);
-  for (auto& e : c->ev_copy) cudaEventDestroy(e);
-  for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_fork2, c->ev_join2, c->ev_fork3}) cudaEventDestroy(e);
-  for (auto& e : c->ev_stage) cudaEventDestroy(e);
-  delete c;
+// No exception crosses the C-ABI (tgs.h): the host-side containers (std::vector, std::string) may throw std::bad_alloc.
+#define TGS_NOEXCEPT_BODY(ctx, expr)                                                                        \
+  try { return (expr); }                                                                                     \
+  catch (const std::exception& e_) { if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), "host exception: %s", e_.what()); return TGS_E_INVALID_ARG; } \
+  catch (...) { return TGS_E_INVALID_ARG; }
+
+int tgs_create(tgs_ctx** out, int device, void* stream) {
+  if (!out) return TGS_E_INVALID_ARG;
+  *out = nullptr;
+  TGS_NOEXCEPT_BODY((tgs_ctx*)nullptr, create_impl(out, device, stream))
 }
 
-int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, const float* scales, const float* quats,
+void tgs_destroy(tgs_ctx* c) { destroy_ctx(c); }
+
+static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* means, const float* scales, const float* quats,
                        const float* opacity, const float* sh, int mem) {
   if (!c) return TGS_E_INVALID_ARG;
   if (deg < 0 || deg > 3 || n == 0 || !means || !scales || !quats || !opacity || !sh || (mem != TGS_HOST && mem != TGS_DEVICE)) return TGS_E_INVALID_ARG;
@@ -366,11 +383,29 @@ int tgs_reset_priors(tgs_ctx* c) {
   return TGS_OK;
 }
 
-int tgs_render(tgs_ctx* c, int mode) {
+static int render_impl(tgs_ctx* c, int mode) {
   if (!c) return TGS_E_INVALID_ARG;
   if (!c->n) return TGS_E_NO_SCENE;
   if (!c->cam_set) return TGS_E_NO_CAMERA;
   CK(cudaSetDevice(c->device));
+  // ---- what the previous frame left for the host mid-frame: the overflow flag of its pair binning ...
+  if (c->bin_pending) {
+    CK(cudaEventSynchronize(c->ev_bin));          // k_bin of the previous frame has finished (its tile sort / blend may still run)
+    c->bin_pending = false;
+    if (c->h_ovf[c->bin_slot]) {
+      // That frame is background only (TGS_E_CAPACITY from tgs_get_stats) and whatever it committed -- TAB, TGB, G_rendered,
+      // an F of (+inf, -inf) that would make AFC cull everything -- must never be used: drop the priors, so the next AUTO
+      // frame is a reference frame, and grow the automatic capacity before it.
+      c->h_ovf[c->bin_slot] = 0;
+      invalidate_priors(c);
+      c->sel_pending = false;
+      if (!c->prm.max_pairs) {
+        unsigned long long want = (unsigned long long)c->max_pairs * 2ull;
+        if (want > (1ull << 30) - 1) want = (1ull << 30) - 1;
+        if (int r = alloc_pair_buffers(c, (uint32_t)want, c->sort_passes_cap)) return r;
+      }
+    }
+  }
   // ---- A0: frame type (R9, R23)
   if (c->sel_pending) {   // eta rule needs the selected-tile count of the previous S frame
     CK(cudaEventSynchronize(c->ev_sel));
@@ -495,7 +530,10 @@ int tgs_render(tgs_ctx* c, int mode) {
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, c->nv_hint < 1000000u);   // visible Gaussians by depth
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   mark();                                                                      // 3: A5 pairs
-  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms);                                            // tests -> pairs, counts
+  c->h_ovf[ci] = 0;
+  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms, c->h_ovf + ci);                             // tests -> pairs, counts
+  CK(cudaEventRecord(c->ev_bin, s));
+  c->bin_pending = true; c->bin_slot = ci;
   mark();                                                                      // 4: A5 colours (production: third stream, beside the depth sort)
   if (!early_colour) launch_colour_all(s, fc, b, c->num_sms);                                             // stage timing: the production kernel, in line
   mark();                                                                      // 5: A6 level 2 + A7
@@ -604,7 +642,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
 static uint32_t f2key_host(float f) { uint32_t b; memcpy(&b, &f, 4); return (b & 0x80000000u) ? ~b : (b | 0x80000000u); }
 static float key2f_host(uint32_t k) { const uint32_t b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k; float f; memcpy(&f, &b, 4); return f; }
 
-long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int mem) {
+static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int mem) {
   if (!c || !nm || (mem != TGS_HOST && mem != TGS_DEVICE)) return TGS_E_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   const std::string name(nm);
@@ -666,7 +704,7 @@ long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int
   return (long long)have;
 }
 
-int tgs_debug_put(tgs_ctx* c, const char* nm, const void* src, size_t bytes, int mem) {
+static int debug_put_impl(tgs_ctx* c, const char* nm, const void* src, size_t bytes, int mem) {
   if (!c || !nm || !src || (mem != TGS_HOST && mem != TGS_DEVICE) || !c->cam_set || !c->n) return TGS_E_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   if (int r = alloc_frame_buffers(c)) return r;
@@ -706,7 +744,7 @@ int tgs_debug_put(tgs_ctx* c, const char* nm, const void* src, size_t bytes, int
   return TGS_E_INVALID_ARG;
 }
 
-int tgs_debug_run_stage(tgs_ctx* c, const char* st) {
+static int debug_run_stage_impl(tgs_ctx* c, const char* st) {
   if (!c || !st) return TGS_E_INVALID_ARG;
   const std::string s(st);
   if (s == "timing_on") { c->timing = true; return TGS_OK; }
@@ -717,5 +755,14 @@ int tgs_debug_run_stage(tgs_ctx* c, const char* st) {
   if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
   return TGS_E_INVALID_ARG;
 }
+
+int tgs_load_gaussians(tgs_ctx* c, uint32_t n, int deg, const float* means, const float* scales, const float* quats,
+                       const float* opacity, const float* sh, int mem) {
+  TGS_NOEXCEPT_BODY(c, load_gaussians_impl(c, n, deg, means, scales, quats, opacity, sh, mem))
+}
+int tgs_render(tgs_ctx* c, int mode) { TGS_NOEXCEPT_BODY(c, render_impl(c, mode)) }
+long long tgs_debug_get(tgs_ctx* c, const char* nm, void* dst, size_t bytes, int mem) { TGS_NOEXCEPT_BODY(c, debug_get_impl(c, nm, dst, bytes, mem)) }
+int tgs_debug_put(tgs_ctx* c, const char* nm, const void* src, size_t bytes, int mem) { TGS_NOEXCEPT_BODY(c, debug_put_impl(c, nm, src, bytes, mem)) }
+int tgs_debug_run_stage(tgs_ctx* c, const char* st) { TGS_NOEXCEPT_BODY(c, debug_run_stage_impl(c, st)) }
 
 }  // extern "C"

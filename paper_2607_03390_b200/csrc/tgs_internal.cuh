@@ -158,7 +158,8 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t
 void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
-void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms);
+void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms,
+                uint32_t* host_overflow);   // pinned host word: set to 1 (zero-copy store) when the pair buffers overflow
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
@@ -174,3 +175,4 @@ uint32_t scan_tile_items();
 uint32_t bin_chunk_items();
 uint32_t preprocess_chunk_items();
 int tile_sort_passes(int n_tiles);
+void sort_prepare_device();   // function attributes of the sort kernels on the current device (once per context)

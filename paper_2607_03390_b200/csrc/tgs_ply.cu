@@ -57,11 +57,24 @@ cudaStream_t tgs_ply_stream(tgs_ctx* c);
 int tgs_ply_device(tgs_ctx* c);
 }
 
+static int load_ply_impl(tgs_ctx* c, const char* path);
+
+// No exception crosses the C-ABI: std::bad_alloc / std::length_error from the host-side containers become an error code.
 extern "C" int tgs_load_ply(tgs_ctx* c, const char* path) {
   if (!c || !path) return TGS_E_INVALID_ARG;
+  try {
+    return load_ply_impl(c, path);
+  } catch (...) {
+    tgs_ply_report(c, "tgs_load_ply: out of host memory or malformed header");
+    return TGS_E_INVALID_ARG;
+  }
+}
+
+static int load_ply_impl(tgs_ctx* c, const char* path) {
   FILE* f = fopen(path, "rb");
   if (!f) { tgs_ply_report(c, "tgs_load_ply: cannot open file"); return TGS_E_INVALID_ARG; }
-  auto bail = [&](const char* msg) { fclose(f); tgs_ply_report(c, msg); return (int)TGS_E_INVALID_ARG; };
+  struct FileGuard { FILE*& f; ~FileGuard() { if (f) fclose(f); } } guard{f};     // also on an exception
+  auto bail = [&](const char* msg) { tgs_ply_report(c, msg); return (int)TGS_E_INVALID_ARG; };
   // ---- header
   char line[512];
   if (!fgets(line, sizeof(line), f) || strncmp(line, "ply", 3) != 0) return bail("tgs_load_ply: not a ply file");
@@ -102,9 +115,16 @@ extern "C" int tgs_load_ply(tgs_ctx* c, const char* path) {
   L.K = (deg + 1) * (deg + 1);
   // ---- rows
   const size_t row_floats = (size_t)L.stride, total = row_floats * (size_t)n;
+  {   // the header's vertex count is untrusted: compare it with what the file really holds before allocating anything
+    const long data_at = ftell(f);
+    if (data_at < 0 || fseek(f, 0, SEEK_END) != 0) return bail("tgs_load_ply: cannot seek");
+    const long file_end = ftell(f);
+    if (file_end < data_at || fseek(f, data_at, SEEK_SET) != 0) return bail("tgs_load_ply: cannot seek");
+    if ((unsigned long long)(file_end - data_at) / sizeof(float) < (unsigned long long)total) return bail("tgs_load_ply: file shorter than the header says");
+  }
   std::vector<float> rows(total);
   if (fread(rows.data(), sizeof(float), total, f) != total) return bail("tgs_load_ply: file shorter than the header says");
-  fclose(f);
+  fclose(f); f = nullptr;
   if (cudaSetDevice(tgs_ply_device(c)) != cudaSuccess) return TGS_E_CUDA;
   cudaStream_t s = tgs_ply_stream(c);
   float *d_rows = nullptr, *d_means = nullptr, *d_scales = nullptr, *d_quats = nullptr, *d_op = nullptr, *d_sh = nullptr;

@@ -8,6 +8,9 @@ Tolerances (BASELINE.json north_star; derivation in DESIGN.md §5):
   pixels the oracle marks `borderline` (an alpha or transmittance test within its rounding margin) may take
   the other branch: there RGB <= 1.2e-2 and they must be rare.
 """
+import json
+import os
+
 import numpy as np
 
 from oracle import ora
@@ -97,26 +100,35 @@ def compare_temporal_buffers(g, o):
     assert np.array_equal(bits(g.debug_get("fill_depth")), bits(fd_o))
 
 
-def compare_outputs(g, o, ftype):
+def compare_outputs(g, o, ftype, border_max=5e-2, border_rgb_tol=BORDERLINE_RGB_TOL):
+    """Float outputs.  north_star's tolerance (RGB <= 2e-3, depth <= 1e-4 relative) holds on every pixel the oracle does
+    not flag `borderline`; flagged pixels (a skip / stop decision within its rounding margin, R38) may take the
+    other branch: there RGB <= `border_rgb_tol`, and their share must stay below `border_max`.  Returns what was
+    measured, so that the tests can print it and assert per-config bounds (DESIGN.md §5 has the table)."""
     img_g, img_o = g.read_image(), o.read_image()
     d_g, s_g = g.read_depth()
     d_o, s_o = o.read_depth()
     border = o.get("borderline").reshape(d_o.shape).astype(bool)
     err = np.abs(img_g - img_o).max(-1)
-    assert border.mean() < 5e-2, border.mean()   # T parks just above 1e-4 behind two near-opaque Gaussians
-    assert err[~border].max() <= RGB_TOL, err[~border].max()
-    assert err.max() <= BORDERLINE_RGB_TOL, err.max()
+    m = {"border_share": float(border.mean()), "rgb_max_off_border": float(err[~border].max()) if (~border).any() else 0.0,
+         "rgb_max_on_border": float(err[border].max()) if border.any() else 0.0,
+         "border_over_2e-3_share": float((err[border] > RGB_TOL).mean()) if border.any() else 0.0,
+         "depth_rel_max": 0.0, "sigma_err_max_rel_depth": 0.0}
+    assert m["border_share"] <= border_max, m   # T parks just above 1e-4 behind two near-opaque Gaussians (DESIGN.md §5)
+    assert m["rgb_max_off_border"] <= RGB_TOL, m
+    assert m["rgb_max_on_border"] <= border_rgb_tol, m
     ok = ~border
     vg, vo = d_g < 1e38, d_o < 1e38
     assert np.array_equal(vg[ok], vo[ok])
     both = vg & vo & ok
-    if not both.any():
-        return float(err.max()), 0.0
-    rel = np.abs(d_g[both] - d_o[both]) / d_o[both]
-    assert rel.max() <= DEPTH_RTOL, rel.max()
-    serr = np.abs(s_g[both] - s_o[both]) / d_o[both]
-    assert serr.max() <= SIGMA_TOL_REL_DEPTH, serr.max()
-    return float(err.max()), float(rel.max())
+    if both.any():
+        rel = np.abs(d_g[both] - d_o[both]) / d_o[both]
+        m["depth_rel_max"] = float(rel.max())
+        assert rel.max() <= DEPTH_RTOL, m
+        serr = np.abs(s_g[both] - s_o[both]) / d_o[both]
+        m["sigma_err_max_rel_depth"] = float(serr.max())
+        assert serr.max() <= SIGMA_TOL_REL_DEPTH, m
+    return m
 
 
 def compare_rendered(g, o):
@@ -139,7 +151,10 @@ def compare_stats(g, o):
     return sg, so
 
 
-def compare_frame(g, o, n, ftype, check_rendered=True):
+REPORT = []          # one dict per compared frame (printed by the tests; `pytest -rP` or -s shows it)
+
+
+def compare_frame(g, o, n, ftype, check_rendered=True, label=None, **tol):
     """Everything of one frame, both sides already rendered."""
     sg, so = compare_stats(g, o)
     if ftype == ora.FRAME_S:
@@ -147,7 +162,15 @@ def compare_frame(g, o, n, ftype, check_rendered=True):
     assert np.array_equal(g.read_tile_mask(), o.read_tile_mask())
     compare_records(g, o, n)
     compare_binning(g, o)
-    out = compare_outputs(g, o, ftype)
+    out = compare_outputs(g, o, ftype, **tol)
     if ftype != ora.FRAME_S and check_rendered:
-        compare_rendered(g, o)
+        out["rendered_diff"] = compare_rendered(g, o)
+        out["rendered"] = int(so["n_rendered"])
+    out.update(frame="RPS"[ftype], label=label, n_pairs=int(sg["n_pairs"]), n_sel=int(sg["n_sel"]), n_tiles=int(sg["n_tiles"]))
+    REPORT.append(out)
+    print("[parity] " + " ".join(f"{k}={v:.3g}" if isinstance(v, float) else f"{k}={v}" for k, v in out.items()))
+    path = os.environ.get("TGS_PARITY_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps(out) + "\n")
     return sg, so, out
