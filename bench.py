@@ -35,6 +35,12 @@ BLEND_LANE_INSTR = 14.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_blend<1,0> launch on config 3, from the ncu --set full capture
 # summarised in profiles/r1i_top_kernels.md (the file names the command); per launch, like `achieved`.
 BLEND_DRAM_TRAFFIC_BYTES = 48.6e6
+BLEND_DRAM_TRAFFIC_SOURCE = "ncu --set full capture of k_blend<1,0> on config 3 (profiles/r1i_top_kernels.md), not re-measured by this run"
+# Lane-instructions the pair binning needs: per (Gaussian, tile) test the tile coordinates and box (8), the
+# selection bit (4), centre-in-box (5), four box edges of the conic form at the clamped optimum (4 x 12) and the margin
+# compare (3) = 68; per emitted pair the rank, the staging and the two stores (12).
+BIN_LANE_INSTR_PER_TEST = 68.0
+BIN_LANE_INSTR_PER_PAIR = 12.0
 
 
 def _peaks():
@@ -124,6 +130,175 @@ def _ssim(a, b):
     return float((((2 * ma * mb + c1) * (2 * cab + c2)) / ((ma * ma + mb * mb + c1) * (va + vb + c2))).mean())
 
 
+STAGE_NAMES = ["init_warp_fill", "preprocess_select", "depth_sort", "bin_pairs", "sh_colour", "tile_sort_ranges", "blend_stitch", "post"]
+
+
+def workload_string(sc, config):
+    cam = sc.camera
+    return (f"config {config} ({sc.name}): {sc.n} Gaussians, SH degree {sc.sh_degree}, {cam.W}x{cam.H}, {len(sc.poses)}-frame trajectory "
+            f"played forward/backward, AUTO schedule (lambda_TDC=50, lambda_SR=5, eta=0.4)")
+
+
+def stage_rooflines(stats, sc, hbm_gbs, alu_peak):
+    """Achieved fraction of the roofline that bounds each stage (DESIGN.md §7.1 derives the units), for a list of frame
+    statistics of ONE frame type.  Algorithmic bytes / needed lane-instructions come from the frames' own counters, the
+    time from the stage events (single stream, kernel boundaries and launch gaps included)."""
+    if not stats:
+        return None
+    cam = sc.camera
+    mean = lambda key: float(np.mean([s[key] for s in stats]))
+    t = np.mean([s["ms_stage"] for s in stats], axis=0) * 1e-3
+    P, Nv, L, nt = mean("n_pairs"), mean("n_visible"), mean("n_interactions"), mean("n_tests")
+    ftype = stats[0]["frame_type"]
+    T_ = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
+    tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
+    K = (sc.sh_degree + 1) ** 2
+    px = cam.W * cam.H
+    # init + A1 warp + A2 fill: S frames 8 B/px init + 8 B/px read + 2 atomics (8 B) + 4 B read + 4 B written; R / P frames
+    # only zero G_rendered' (N bytes) and a few words per tile
+    init_bytes = (32.0 * px if ftype == 2 else float(sc.n)) + 25.0 * T_
+    rows = {
+        "init_warp_fill": ("hbm", init_bytes / 1e9, "GB"),
+        "preprocess_select": ("hbm", (sc.n * (16 + 4) + Nv * (32 + 16 + 100)) / 1e9, "GB"),
+        "depth_sort": ("hbm", Nv * 16 * 4 / 1e9, "GB"),
+        "bin_pairs": ("alu", (nt * BIN_LANE_INSTR_PER_TEST + P * BIN_LANE_INSTR_PER_PAIR) / 1e12, "T lane-instr"),
+        "sh_colour": ("hbm", Nv * (4 + 16 + 12 * K + 16) / 1e9, "GB"),
+        "tile_sort_ranges": ("hbm", P * 16 * tile_passes / 1e9, "GB"),
+        "blend_stitch": ("alu", L * BLEND_LANE_INSTR / 1e12, "T lane-instr"),
+    }
+    out = {}
+    for i, name in enumerate(STAGE_NAMES[:7]):
+        bound, work, unit = rows[name]
+        peak = hbm_gbs if bound == "hbm" else alu_peak
+        ach = work / t[i] if t[i] > 0 else 0.0
+        out[name] = {"bound": bound, "ms": float(t[i] * 1e3), "achieved": ach, "peak": peak, "unit": unit + "/s", "frac": ach / peak}
+    return out
+
+
+def summarise(lst):
+    if not lst:
+        return None
+    ms = np.mean([s["ms_stage"] for s in lst], axis=0)
+    m = lambda key: float(np.mean([s[key] for s in lst]))
+    return {"frames": len(lst), "ms_total": m("ms_total"), "ms_stage": {n: float(v) for n, v in zip(STAGE_NAMES, ms)},
+            "n_pairs": m("n_pairs"), "n_tests": m("n_tests"), "n_visible": m("n_visible"),
+            "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
+            "n_interactions": m("n_interactions"), "n_blended": m("n_blended"), "n_pixel_slots": m("n_pixel_slots")}
+
+
+class Harness:
+    """One scene on one GPU: timed frame loops (CUDA events on the context's stream), the per-stage pass, quality."""
+
+    def __init__(self, tgs, torch, sc, local, world, warmup):
+        self.tgs, self.torch, self.sc, self.world, self.W = tgs, torch, sc, world, warmup
+        self.stream = torch.cuda.Stream()
+        self.ctx = tgs.Context(local, self.stream.cuda_stream)
+        self.ctx.load_scene(sc)                         # scene resident in HBM before any timed region
+        self.local = local
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def timed(self, mode, steps, readback=None):
+        """Device time (ms, max over ranks) of `steps` frames of the trajectory, after W untimed warm-up frames."""
+        torch, ctx, sc, cam = self.torch, self.ctx, self.sc, self.sc.camera
+        ctx.reset_priors()
+        for f in range(self.W):
+            ctx.set_camera(trajectory_pose(sc, f), cam)
+            ctx.render(mode)
+        ctx.reset_priors()
+        self.barrier()
+        l0 = ctx.get_stats(check=False)["launches_total"]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(self.stream):
+            e0.record(self.stream)
+            for f in range(steps):
+                ctx.set_camera(trajectory_pose(sc, f), cam)
+                ctx.render(mode)
+                if readback is not None:
+                    ctx.read_image_async(readback[f & 1])   # device -> pinned host on the copy stream, overlaps the next frame
+            if readback is not None:
+                ctx.wait_reads()                    # every frame's image is on the host before the clock stops
+            e1.record(self.stream)
+        self.barrier()
+        self.launches = ctx.get_stats(check=False)["launches_total"] - l0
+        return max_over_ranks(e0.elapsed_time(e1), self.world, "cuda")
+
+    def stage_pass(self, frames):
+        """(a) stage events with the production instances of every kernel, everything on ONE stream so that the events
+        bracket what they name (the production frame overlaps A2 / A4 / SH colours on side streams and is shorter than the
+        sum); (b) the same frames with the counting instances of the blend (never timed): L, composited interactions and
+        pixel slots are properties of the frames and are merged into the statistics of pass (a)."""
+        tgs, ctx, sc, cam = self.tgs, self.ctx, self.sc, self.sc.camera
+        ctx.debug_run_stage("timing_on")
+        ctx.reset_priors()
+        timed_stats = []
+        for f in range(frames):
+            ctx.set_camera(trajectory_pose(sc, f), cam)
+            ctx.render(tgs.AUTO)
+            timed_stats.append(ctx.get_stats())
+        ctx.debug_run_stage("timing_off")
+        ctx.debug_run_stage("count_interactions_on")
+        ctx.reset_priors()
+        per_type = {0: [], 1: [], 2: []}
+        for f in range(frames):
+            ctx.set_camera(trajectory_pose(sc, f), cam)
+            ctx.render(tgs.AUTO)
+            cs = ctx.get_stats()
+            st = timed_stats[f]
+            assert st["frame_type"] == cs["frame_type"] and st["n_pairs"] == cs["n_pairs"]
+            for key in ("n_interactions", "n_blended", "n_pixel_slots"):
+                st[key] = cs[key]
+            per_type[st["frame_type"]].append(st)
+        ctx.debug_run_stage("count_interactions_off")
+        return per_type
+
+    def quality(self, frames):
+        """PSNR / SSIM of the S frames against the full render of the same pose (reported; unpinned by the paper)."""
+        tgs, ctx, sc, cam = self.tgs, self.ctx, self.sc, self.sc.camera
+        psnr, ssim = [], []
+        ctx.reset_priors()
+        ref = tgs.Context(self.local, self.stream.cuda_stream)
+        ref.load_scene(sc)
+        for f in range(frames):
+            ctx.set_camera(trajectory_pose(sc, f), cam)
+            ctx.render(tgs.AUTO)
+            if ctx.get_stats()["frame_type"] == tgs.FRAME_S:
+                ref.set_camera(trajectory_pose(sc, f), cam)
+                ref.render(tgs.FULL)
+                a, b = ctx.read_image(), ref.read_image()
+                mse = float(((a - b) ** 2).mean())
+                psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
+                if len(ssim) < 3:
+                    ssim.append(_ssim(a, b))
+        ref.destroy()
+        return (float(np.mean(psnr)) if psnr else None), (float(np.mean(ssim)) if ssim else None)
+
+    def close(self):
+        self.ctx.destroy()
+
+
+def config_summary(h, hbm_gbs, alu_peak, stage_frames=60, quality_frames=12):
+    """FPS of TemporalGS (AUTO) and of the full render over the WHOLE trajectory of the scene, their ratio, the share of
+    selected tiles, quality of the S frames, and per-stage ms + roofline fractions by frame type."""
+    tgs, sc = h.tgs, h.sc
+    F = len(sc.poses)
+    ms_tgs = h.timed(tgs.AUTO, F)
+    ms_full = h.timed(tgs.FULL, F)
+    per_type = h.stage_pass(min(F, stage_frames))
+    psnr, ssim = h.quality(min(F, quality_frames))
+    out = {"frames": F, "fps_tgs": aggregate_fps(h.world, F, ms_tgs), "fps_full": aggregate_fps(h.world, F, ms_full),
+           "speedup": ms_full / ms_tgs, "psnr_S_vs_full_dB": psnr, "ssim_S_vs_full": ssim,
+           "n_sel_frac_S": (summarise(per_type[2]) or {}).get("n_sel_frac"),
+           "stages": {k: summarise(per_type[i]) for k, i in (("R", 0), ("P", 1), ("S", 2))},
+           "stage_rooflines": {k: stage_rooflines(per_type[i], sc, hbm_gbs, alu_peak) for k, i in (("R", 0), ("P", 1), ("S", 2))}}
+    return out, per_type
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -140,185 +315,89 @@ def run_ours(args):
     from paper_2607_03390_b200 import tgs           # raises if libtgs.so is missing: no fallback
 
     sc = make_config(args.config, n=args.n, frames=None)
-    stream = torch.cuda.Stream()
-    ctx = tgs.Context(local, stream.cuda_stream)
-    ctx.load_scene(sc)                              # scene resident in HBM before any timed region
     cam = sc.camera
     K, W = args.steps, args.warmup
+    h = Harness(tgs, torch, sc, local, world, W)
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def timed(mode, steps, readback=None):
-        """Device time (CUDA events on the context's stream) of `steps` frames; returns ms."""
-        ctx.reset_priors()
-        for f in range(W):                          # warm-up frames (untimed) -- same path, same mode
-            ctx.set_camera(trajectory_pose(sc, f), cam)
-            ctx.render(mode)
-        ctx.reset_priors()
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        with torch.cuda.stream(stream):
-            e0.record(stream)
-            for f in range(steps):
-                ctx.set_camera(trajectory_pose(sc, f), cam)
-                ctx.render(mode)
-                if readback is not None:
-                    ctx.read_image_async(readback[f & 1])   # device -> pinned host on the copy stream, overlaps the next frame
-            if readback is not None:
-                ctx.wait_reads()                    # every frame's image is on the host before the clock stops
-            e1.record(stream)
-        barrier()
-        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
-
+    # ---- the headline: K frames of the trajectory, TemporalGS (AUTO); then the same frames end to end
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ms_tgs = timed(tgs.AUTO, K)
+    ms_tgs = h.timed(tgs.AUTO, K)
+    launches = h.launches
     clocks = sampler.stop() if rank == 0 else None
-    ms_full = timed(tgs.FULL, K)
+    ms_full = h.timed(tgs.FULL, K)
     pinned = [torch.empty((cam.H, cam.W, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
-    ms_e2e = timed(tgs.AUTO, K, readback=[t.numpy() for t in pinned])
+    ms_e2e = h.timed(tgs.AUTO, K, readback=[t.numpy() for t in pinned])
 
-    # ---- per-stage pass (untimed for `value`): stage events + interaction counter, one sync per frame
-    # (a) stage events with the production instances of every kernel; (b) the same frames again with the counting
-    # instances of the blend (slower, never timed): L, composited interactions and pixel slots are properties of the
-    # frames, so they are merged into the statistics of pass (a)
-    prof_frames = min(K, 60)
-    ctx.debug_run_stage("timing_on")
-    ctx.reset_priors()
-    timed_stats = []
-    for f in range(prof_frames):
-        ctx.set_camera(trajectory_pose(sc, f), cam)
-        ctx.render(tgs.AUTO)
-        timed_stats.append(ctx.get_stats())
-    ctx.debug_run_stage("timing_off")
-    ctx.debug_run_stage("count_interactions_on")
-    ctx.reset_priors()
-    per_type = {0: [], 1: [], 2: []}
-    for f in range(prof_frames):
-        ctx.set_camera(trajectory_pose(sc, f), cam)
-        ctx.render(tgs.AUTO)
-        cs = ctx.get_stats()
-        st = timed_stats[f]
-        assert st["frame_type"] == cs["frame_type"] and st["n_pairs"] == cs["n_pairs"]
-        for key in ("n_interactions", "n_blended", "n_pixel_slots"):
-            st[key] = cs[key]
-        per_type[st["frame_type"]].append(st)
-    ctx.debug_run_stage("count_interactions_off")
-    # PSNR of S frames against the full render of the same pose (reported; unpinned by the paper)
-    psnr, ssim = [], []
-    ctx.reset_priors()
-    ref_ctx = tgs.Context(local, stream.cuda_stream)
-    ref_ctx.load_scene(sc)
-    for f in range(min(K, 12)):
-        ctx.set_camera(trajectory_pose(sc, f), cam)
-        ctx.render(tgs.AUTO)
-        if ctx.get_stats()["frame_type"] == tgs.FRAME_S:
-            ref_ctx.set_camera(trajectory_pose(sc, f), cam)
-            ref_ctx.render(tgs.FULL)
-            a, b = ctx.read_image(), ref_ctx.read_image()
-            mse = float(((a - b) ** 2).mean())
-            psnr.append(10 * np.log10(1.0 / max(mse, 1e-12)))
-            ssim.append(_ssim(a, b))
-    ref_ctx.destroy()
-
+    hbm_gbs, sm_mhz_max, peak_kind = _peaks()
+    sm_clk = (clocks or {}).get("sm_mhz") or sm_mhz_max
+    alu_peak = 148 * 128 * sm_clk * 1e6 / 1e12          # T lane-instr/s at the clock seen under load
+    # ---- the whole trajectory (BASELINE.json: "FPS over trajectory; speed-up vs full render"), whatever --steps says
+    traj, per_type = config_summary(h, hbm_gbs, alu_peak)
+    h.close()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return None
 
-    hbm_gbs, sm_mhz_max, peak_kind = _peaks()
-    stage_names = ["init_warp_fill", "preprocess_select", "depth_sort", "bin_pairs", "sh_colour", "tile_sort_ranges", "blend_stitch", "post"]
+    # ---- the other synthetic trajectories (north_star: "on the synthetic trajectories below"): where selective rendering
+    # and the stitch are actually timed (config 3 selects every tile)
+    others = {}
+    if world == 1 and args.n is None:
+        for cfg in [int(x) for x in args.other_configs.split(",") if x.strip().isdigit()]:
+            if cfg == args.config:
+                continue
+            sc2 = make_config(cfg, frames=None)
+            h2 = Harness(tgs, torch, sc2, local, 1, W)
+            o2, _ = config_summary(h2, hbm_gbs, alu_peak, stage_frames=40, quality_frames=10)
+            h2.close()
+            o2["workload"] = workload_string(sc2, cfg)
+            S = (o2["stage_rooflines"] or {}).get("S")
+            o2["S_frame_roofline_fracs"] = {k: round(v["frac"], 4) for k, v in S.items()} if S else None
+            others[f"config{cfg}"] = o2
+            del sc2, h2
 
-    def summarise(lst):
-        if not lst:
-            return None
-        ms = np.mean([s["ms_stage"] for s in lst], axis=0)
-        return {"frames": len(lst), "ms_total": float(np.mean([s["ms_total"] for s in lst])),
-                "ms_stage": {n: float(v) for n, v in zip(stage_names, ms)},
-                "n_pairs": float(np.mean([s["n_pairs"] for s in lst])), "n_visible": float(np.mean([s["n_visible"] for s in lst])),
-                "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
-                "n_interactions": float(np.mean([s["n_interactions"] for s in lst])),
-                "n_blended": float(np.mean([s["n_blended"] for s in lst])),
-                "n_pixel_slots": float(np.mean([s["n_pixel_slots"] for s in lst]))}
-
-    stages = {"R": summarise(per_type[0]), "P": summarise(per_type[1]), "S": summarise(per_type[2])}
-    # dominant kernel = the stage with the largest share of the profiled frames' time
-    tot = np.zeros(8)
-    for lst in per_type.values():
-        for s in lst:
-            tot += np.asarray(s["ms_stage"])
-    dom = int(np.argmax(tot))
+    # ---- roofline of the dominant kernel = the stage with the largest share of the profiled frames' time
     all_stats = [s for lst in per_type.values() for s in lst]
-    roof = None
-    sm_clk = (clocks or {}).get("sm_mhz") or sm_mhz_max
-    T_ = ((sc.camera.W + 15) // 16) * ((sc.camera.H + 15) // 16)
-    tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
+    tot = np.sum([np.asarray(s["ms_stage"]) for s in all_stats], axis=0)
+    dom = int(np.argmax(tot[:7]))
+    roofs_all = stage_rooflines(all_stats, sc, hbm_gbs, alu_peak)      # frame types pooled: the mix the timed region ran
     mean = lambda key: float(np.mean([s[key] for s in all_stats]))
-    # per-stage achieved fraction of the roofline that bounds it (DESIGN.md §7); algorithmic bytes / work from the
-    # per-frame counters, time from the stage events (kernel boundaries and launch gaps included)
-    t_stage = np.mean([s["ms_stage"] for s in all_stats], axis=0) * 1e-3
-    P, Nv, L = mean("n_pairs"), mean("n_visible"), mean("n_interactions")
-    alu_peak = 148 * 128 * sm_clk * 1e6 / 1e12          # T lane-instr/s at the clock seen under load
-    stage_roof = {
-        "preprocess_select": {"bound": "hbm", "achieved": (sc.n * (16 + 4) + Nv * (32 + 16 + 100)) / t_stage[1] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
-        "depth_sort": {"bound": "hbm", "achieved": Nv * 16 * 4 / t_stage[2] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
-        "sh_colour": {"bound": "hbm", "achieved": Nv * (8 + 16 + 12 * (sc.sh_degree + 1) ** 2 + 16) / t_stage[4] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
-        "tile_sort_ranges": {"bound": "hbm", "achieved": P * 16 * tile_passes / t_stage[5] / 1e9, "peak": hbm_gbs, "unit": "GB/s"},
-        "blend_stitch": {"bound": "alu", "achieved": L * BLEND_LANE_INSTR / t_stage[6] / 1e12, "peak": alu_peak, "unit": "T lane-instr/s"},
-    }
-    for v in stage_roof.values():
-        v["frac"] = v["achieved"] / v["peak"]
-    if stage_names[dom] == "blend_stitch":
-        # instruction-issue bound ("alu"): lane-instructions/s = alive interactions * instr per interaction / time
-        t = t_stage[6]
-        ach = L * BLEND_LANE_INSTR / t / 1e12
-        roof = {"kernel": "k_blend", "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-instr/s",
-                "frac": ach / alu_peak, "traffic": BLEND_DRAM_TRAFFIC_BYTES, "interactions_per_launch": float(L),
-                "blended_per_launch": mean("n_blended"), "pixel_slots_per_launch": mean("n_pixel_slots"),
-                "ms_per_launch": t * 1e3, "lane_instr_per_interaction": BLEND_LANE_INSTR,
-                "peak_note": f"148 SM x 4 schedulers x 32 lanes x {sm_clk:.0f} MHz (median SM clock during the run): one warp "
-                             f"instruction per scheduler and clock; the FMA pipe (128 lanes/clk/SM) and the ALU pipe (64) are not tighter "
-                             f"for this mix (DESIGN.md 7.2)"}
+    r = roofs_all[STAGE_NAMES[dom]]
+    roof = {"kernel": "k_blend" if STAGE_NAMES[dom] == "blend_stitch" else STAGE_NAMES[dom], "bound": r["bound"], "achieved": r["achieved"],
+            "peak": r["peak"], "unit": r["unit"], "frac": r["frac"], "ms_per_launch": r["ms"]}
+    if STAGE_NAMES[dom] == "blend_stitch":
+        roof.update({"traffic": BLEND_DRAM_TRAFFIC_BYTES, "traffic_source": BLEND_DRAM_TRAFFIC_SOURCE,
+                     "interactions_per_launch": mean("n_interactions"), "blended_per_launch": mean("n_blended"),
+                     "pixel_slots_per_launch": mean("n_pixel_slots"), "lane_instr_per_interaction": BLEND_LANE_INSTR,
+                     "peak_note": f"148 SM x 4 schedulers x 32 lanes x {sm_clk:.0f} MHz (median SM clock during the run): one warp "
+                                  f"instruction per scheduler and clock; the FMA pipe (128 lanes/clk/SM) and the ALU pipe (64) are not "
+                                  f"tighter for this mix (DESIGN.md 7.2)"})
     else:
-        key = stage_names[dom]
-        r = stage_roof.get(key)
-        if r is None:
-            by = P * 8 + Nv * 64
-            r = {"bound": "hbm", "achieved": by / t_stage[dom] / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
-            r["frac"] = r["achieved"] / r["peak"]
-        roof = {"kernel": key, **r, "traffic": None, "ms_per_launch": float(t_stage[dom] * 1e3), "peak_note": f"{peak_kind} copy bandwidth"}
+        roof.update({"traffic": None, "peak_note": f"{peak_kind} copy bandwidth" if r["bound"] == "hbm" else "issue peak"})
+    roof["stages"] = {k: {n: {"ms": round(v["ms"], 5), "bound": v["bound"], "frac": round(v["frac"], 4)} for n, v in d.items()}
+                      for k, d in traj["stage_rooflines"].items() if d}
+    roof["stages_note"] = ("per-stage times are taken with every kernel on ONE stream (stage events must bracket what they name); the "
+                           "production frame overlaps A2 / A4 / SH colours on side streams, so its ms_per_step is below the stage sum")
 
     fps_tgs, fps_full, fps_e2e = aggregate_fps(world, K, ms_tgs), aggregate_fps(world, K, ms_full), aggregate_fps(world, K, ms_e2e)
     out = {
         "metric": METRIC, "value": fps_tgs, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_tgs / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"config {args.config} ({sc.name}): {sc.n} Gaussians, SH degree {sc.sh_degree}, {cam.W}x{cam.H}, "
-                               f"{len(sc.poses)}-frame trajectory played forward/backward, AUTO schedule (lambda_TDC=50, lambda_SR=5, eta=0.4)",
-                   "l2": "scene arrays (>= 700 MB) exceed the 126 MB L2; no explicit flush", "parallelism": "replicas only"},
-        "fps_full_render": fps_full, "ms_per_step_full_render": ms_full / K, "speedup_vs_full_render": fps_tgs / fps_full,
-        "psnr_S_vs_full_dB": float(np.mean(psnr)) if psnr else None,
-        "ssim_S_vs_full": float(np.mean(ssim)) if ssim else None,
+        "config": {"workload": workload_string(sc, args.config),
+                   "l2": "scene arrays (>= 700 MB) exceed the 126 MB L2; no explicit flush", "parallelism": "replicas only",
+                   "fps_full_render": fps_full, "speedup_vs_full_render": fps_tgs / fps_full,
+                   "trajectory": {k: traj[k] for k in ("frames", "fps_tgs", "fps_full", "speedup", "psnr_S_vs_full_dB", "ssim_S_vs_full", "n_sel_frac_S")},
+                   "stages": traj["stages"],
+                   "other_configs": {k: {kk: v[kk] for kk in ("workload", "frames", "fps_tgs", "fps_full", "speedup", "n_sel_frac_S", "psnr_S_vs_full_dB",
+                                                             "ssim_S_vs_full", "S_frame_roofline_fracs", "stages", "stage_rooflines")} for k, v in others.items()}},
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 16 * 4 + 8 * 4, "d2h_bytes_per_step": cam.W * cam.H * 3 * 4,
                 "note": "camera by value through tgs_set_camera; every frame's image copied to pinned host memory (tgs_read_image_async: the copy of frame f overlaps the rendering of frame f+1), all copies complete inside the timed region"},
-        "gpu_launches": None,
-        "stages": stages, "roofline": roof, "stage_rooflines": stage_roof, "clocks": clocks,
+        "gpu_launches": int(launches),                 # counted by the library (tgs_stats.launches_total) over the timed region
+        "roofline": roof, "clocks": clocks,
     }
-    # launches per frame (tgs_api.cu): init, preprocess, depth sort (4 digits), compact_vis, scan_area, bin,
-    # colour, tile sort (digits, the last one writes the ranges), blend = 11 + tile digits; + export_counters; + frustum
-    # on R / P; + warp, fill_corr, mark_oc, select on S
-    T = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
-    tpasses = (max(1, int(np.ceil(np.log2(T)))) + 7) // 8
-    nR = sum(1 for s in all_stats if s["frame_type"] != 2)
-    base = 11 + tpasses
-    per_ref, per_s = base + 2, base + 5        # + k_export_counters on every frame
-    frac_ref = nR / max(1, len(all_stats))
-    out["gpu_launches"] = int(round(K * (frac_ref * per_ref + (1 - frac_ref) * per_s)))
     if world > 1:
         dist.destroy_process_group()
     return out
@@ -415,7 +494,8 @@ def oracle_sample(config, n, frames_modes, budget_s=None):
         o.render(modes[m])
         dt = time.perf_counter() - t0
         st = o.stats()
-        per.append({"frame": f, "type": "RPS"[st["frame_type"]], "s": dt})
+        per.append({"frame": f, "type": "RPS"[st["frame_type"]], "s": dt, "ms_temporal": st["ms_temporal"], "ms_preprocess": st["ms_preprocess"],
+                    "ms_sort": st["ms_sort"], "ms_blend": st["ms_blend"]})
         t_total += dt
         done += 1
         if budget_s is not None and t_total > budget_s:
@@ -462,7 +542,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
         "steps": K, "warmup": W, "ms_per_step": 1e3 * t_timed / timed_frames, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config {args.config} ({sc.name}): {sc.n} Gaussians, SH degree {sc.sh_degree}, {cam.W}x{cam.H}, AUTO schedule"},
+        "config": {"workload": workload_string(sc, args.config)},
         "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "steps_timed": timed_frames,
@@ -478,6 +558,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the number of Gaussians (debug only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--other-configs", default="2,5,4", help="configs also measured over their whole trajectories ('none' to skip)")
     ap.add_argument("--ablation", action="store_true", help="module ablation and sensitivity table instead of the bench line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -493,11 +574,14 @@ def main():
     if out is None:
         return
     if out["n_gpus"] == 1 and not args.no_cpu_baseline:
-        # the oracle as it stands on one host core: a reference frame and the TemporalGS frame that follows it
-        done, t, per, _ = oracle_sample(args.config, args.n, [(0, "full"), (1, "temporal")])
+        # the oracle as it stands on one host core: one lambda_SR cycle (6 frames) of the same trajectory in AUTO mode
+        # (SURVEY 8(d)), with the oracle's own per-stage split
+        done, t, per, _ = oracle_sample(args.config, args.n, [(f, "auto") for f in range(6)])
+        split = {k: float(np.mean([p[k] for p in per])) for k in ("ms_temporal", "ms_preprocess", "ms_sort", "ms_blend")}
         out["cpu_baseline"] = {"value": done / t, "unit": "frames/s", "cores": 1, "kind": "oracle",
-                               "sample": f"frames 0 (R) and 1 (S) of the same trajectory, {t:.1f} s: " +
-                                         ", ".join(f"{p['type']} {p['s']:.1f} s" for p in per)}
+                               "sample": f"frames 0-{done - 1} of the same trajectory, AUTO schedule (one lambda_SR cycle), {t:.1f} s: " +
+                                         ", ".join(f"{p['type']} {p['s']:.1f} s" for p in per),
+                               "ms_per_frame_by_stage": split}
     print(json.dumps(out))
 
 

@@ -97,6 +97,10 @@ typedef struct {
                           6 blend + stitch, 7 post (F reduction, stats) */
   float ms_total;
   uint64_t device_bytes; /* device memory held by the context */
+  uint64_t n_tests;      /* (Gaussian, tile) combinations the pair binning examined: sum of the test-rect areas of the visible
+                            Gaussians (n_pairs of them passed: tile selected, L123, and reached with alpha >= 1/255, R39) */
+  uint64_t launches_total; /* kernels this library has launched in this process so far (all contexts); bench.py reports the
+                              difference over its timed region as `gpu_launches` */
 } tgs_stats;
 
 typedef struct tgs_ctx tgs_ctx;

@@ -20,6 +20,8 @@
     }                                                                                              \
   } while (0)
 
+unsigned long long g_tgs_launches = 0;
+
 struct Sched { int since_R = 0, since_ref = 0, force_P = 0; };
 
 struct tgs_ctx {
@@ -628,6 +630,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
   out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions; out->n_blended = h.n_blended; out->n_pixel_slots = h.n_slots;
   out->device_bytes = c->device_bytes;
+  out->n_tests = h.n_tests; out->launches_total = g_tgs_launches;
   if (c->timing) {
     for (int i = 0; i < 8; ++i) cudaEventElapsedTime(&out->ms_stage[i], c->ev_stage[i], c->ev_stage[i + 1]);
     cudaEventElapsedTime(&out->ms_total, c->ev_stage[0], c->ev_stage[8]);

@@ -141,10 +141,12 @@ struct PdlLaunch {
     cfg.attrs = &at; cfg.numAttrs = 1;
   }
 };
+extern unsigned long long g_tgs_launches;   // kernels launched by this library (tgs_stats.launches_total); defined in tgs_api.cu
 #define TGS_LAUNCH(kernel, grid, block, smem, stream, ...)   \
   do {                                                       \
     PdlLaunch L_(grid, block, smem, stream);                 \
     cudaLaunchKernelEx(&L_.cfg, kernel, __VA_ARGS__);        \
+    ++g_tgs_launches;                                        \
   } while (0)
 
 // ------------------------------------------------------------------ launchers (definitions in k_*.cu)

@@ -6,7 +6,7 @@ Tolerances (BASELINE.json north_star; derivation in DESIGN.md §5):
   decision floats (u, v, d, conic, warped depth/sigma, repaired depth): bit-exact (same fp32 operation order);
   RGB: max abs error <= 2e-3; depth: <= 1e-4 relative; sigma: <= 2e-3 * depth (sqrt of an fp32 cancellation);
   pixels the oracle marks `borderline` (an alpha or transmittance test within its rounding margin) may take
-  the other branch: there RGB <= 1.2e-2 and they must be rare.
+  the other branch: there RGB <= 6e-3 (measured <= 3.8e-3) and their share is bounded per test (measured <= 1.42 %).
 """
 import json
 import os
@@ -17,10 +17,12 @@ from oracle import ora
 from oracle.ora import Oracle
 from paper_2607_03390_b200 import tgs
 
-RGB_TOL = 2e-3
-DEPTH_RTOL = 1e-4
-SIGMA_TOL_REL_DEPTH = 2e-3
-BORDERLINE_RGB_TOL = 1.2e-2
+RGB_TOL = 2e-3                 # north_star: max abs error per RGB channel
+RGB_GUARD_OFF_BORDER = 2e-4    # regression guard, 10x the worst value measured on any test frame (1.9e-5)
+DEPTH_RTOL = 1e-4              # north_star: relative depth
+SIGMA_TOL_REL_DEPTH = 2e-3     # the builder's own (north_star states none): sigma is the square root of an fp32 cancellation
+BORDERLINE_RGB_TOL = 6e-3      # pixels whose skip / stop decision is within its rounding margin (worst measured: 3.8e-3)
+BORDER_MAX_DEFAULT = 2.5e-2    # share of such pixels (worst measured on any test frame: 1.42 %)
 
 MODE_G = {"full": tgs.FULL, "pseudo": tgs.PSEUDO_REF, "temporal": tgs.TEMPORAL, "auto": tgs.AUTO}
 MODE_O = {"full": ora.FULL, "pseudo": ora.PSEUDO_REF, "temporal": ora.TEMPORAL, "auto": ora.AUTO}
@@ -100,7 +102,7 @@ def compare_temporal_buffers(g, o):
     assert np.array_equal(bits(g.debug_get("fill_depth")), bits(fd_o))
 
 
-def compare_outputs(g, o, ftype, border_max=5e-2, border_rgb_tol=BORDERLINE_RGB_TOL):
+def compare_outputs(g, o, ftype, border_max=BORDER_MAX_DEFAULT, border_rgb_tol=BORDERLINE_RGB_TOL):
     """Float outputs.  north_star's tolerance (RGB <= 2e-3, depth <= 1e-4 relative) holds on every pixel the oracle does
     not flag `borderline`; flagged pixels (a skip / stop decision within its rounding margin, R38) may take the
     other branch: there RGB <= `border_rgb_tol`, and their share must stay below `border_max`.  Returns what was
@@ -116,6 +118,7 @@ def compare_outputs(g, o, ftype, border_max=5e-2, border_rgb_tol=BORDERLINE_RGB_
          "depth_rel_max": 0.0, "sigma_err_max_rel_depth": 0.0}
     assert m["border_share"] <= border_max, m   # T parks just above 1e-4 behind two near-opaque Gaussians
     assert m["rgb_max_off_border"] <= RGB_TOL, m
+    assert m["rgb_max_off_border"] <= RGB_GUARD_OFF_BORDER, m
     assert m["rgb_max_on_border"] <= border_rgb_tol, m
     ok = ~border
     vg, vo = d_g < 1e38, d_o < 1e38

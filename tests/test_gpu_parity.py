@@ -403,7 +403,7 @@ def test_device_pointers_and_torch_stream():
     h.set_camera(sc.poses[0], sc.camera); o.set_camera(sc.poses[0], sc.camera)
     h.render(tgs.FULL); o.render(ora.FULL)
     assert np.array_equal(img.cpu().numpy(), h.read_image())
-    assert np.abs(img.cpu().numpy() - o.read_image()).max() < 1.2e-2
+    assert np.abs(img.cpu().numpy() - o.read_image()).max() < 6e-3
 
 
 def test_async_readback_matches_blocking_read():
@@ -450,7 +450,7 @@ def test_load_ply_checkpoint(tmp_path):
     # expf on the device vs exp in double: scales / opacities differ by an ulp, so a handful of decisions may flip
     assert abs(int(sg["n_visible"]) - int(so["n_visible"])) <= 3 and abs(int(sg["n_pairs"]) - int(so["n_pairs"])) <= 1e-3 * so["n_pairs"] + 5
     err = np.abs(g.read_image() - o.read_image()).max(-1)
-    assert np.quantile(err, 0.999) <= 2e-3 and err.max() <= 1.2e-2
+    assert np.quantile(err, 0.999) <= 2e-3 and err.max() <= 6e-3
     # same scene through tgs_load_gaussians with the oracle-activated arrays
     g2 = tgs.Context(0)
     g2.load_gaussians(d["means"], d["scales"], d["quats"], d["opacity"], d["sh"], d["sh_degree"])
@@ -499,7 +499,9 @@ def test_repeatability_of_a_frame_stream():
 # ------------------------------------------------------------------------------------------------ full size
 # Per-config bounds on the share of `borderline` pixels (DESIGN.md §5 has the measured table they come from) and on the
 # RGB error on them; everywhere else north_star's 2e-3 applies unchanged.
-FULL_SIZE_BOUNDS = {2: dict(border_max=5e-2), 3: dict(border_max=5e-2), 4: dict(border_max=5e-2), 5: dict(border_max=5e-2)}
+# measured (r2a): config 2 0.98 %, 3 1.42 %, 4 0.52 %, 5 0.79 %; worst RGB error on such a pixel 2.0e-3, 2.8e-3, 3.8e-3, 1.4e-3
+FULL_SIZE_BOUNDS = {2: dict(border_max=1.5e-2, border_rgb_tol=4e-3), 3: dict(border_max=2e-2, border_rgb_tol=5e-3),
+                    4: dict(border_max=1e-2, border_rgb_tol=6e-3), 5: dict(border_max=1.2e-2, border_rgb_tol=3e-3)}
 
 
 def test_full_size_config3_reference_and_temporal():
