@@ -341,25 +341,18 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
 }
 
 // ================================================================== A5c: SH -> RGB (L61 "color c_i"; R5)
-// For every visible Gaussian, straight from the flags k_preprocess wrote: needs neither the sorted list nor the pair
+// One thread per visible Gaussian of the compacted visible list (index order, k_compact_vis): every lane works and the
+// 12 K bytes of a Gaussian are read as K 3/4 independent 16-byte loads.  Needs neither the sorted list nor the pair
 // counts, so it runs on its own stream beside the depth sort, which leaves most SMs idle.  (A variant that waited for
 // k_bin and skipped Gaussians without pairs read fewer SH bytes on S frames but could only run beside the tile sort,
 // whose CTAs fill the register file: no overlap, 20-47 us on the critical path.)
 template <int DEG>
-__global__ void __launch_bounds__(128) k_colour_all(FrameConst fc, const uint32_t* __restrict__ rec_flags, const float4* __restrict__ cull4,
-                                                    const float* __restrict__ sh, float4* __restrict__ rec_rgb) {
+__global__ void __launch_bounds__(128) k_colour_all(FrameConst fc, const uint32_t* __restrict__ vis_list, const Counters* __restrict__ counters,
+                                                    const float4* __restrict__ cull4, const float* __restrict__ sh, float4* __restrict__ rec_rgb) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
-  const uint32_t n4 = (fc.n + 3) / 4;                        // rec_flags is padded to a multiple of 4
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
-    const uint4 f = reinterpret_cast<const uint4*>(rec_flags)[i];
-    const uint32_t fl[4] = {f.x, f.y, f.z, f.w};
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const uint32_t g = 4 * i + j;
-      if (g < fc.n && (fl[j] & TGS_VISIBLE)) sh_colour<DEG>(fc, g, cull4, sh, rec_rgb);
-    }
-  }
+  const uint32_t nv = counters->n_visible;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += gridDim.x * blockDim.x) sh_colour<DEG>(fc, vis_list[i], cull4, sh, rec_rgb);
 }
 
 // ================================================================== A7: per-tile ranges
@@ -406,7 +399,7 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
 }
 
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-#define LAUNCH(D) TGS_LAUNCH((k_colour_all<D>), num_sms * 16, 128, 0, s, fc, b.rec_flags, b.cull4, b.sh, b.rec_rgb)
+#define LAUNCH(D) TGS_LAUNCH((k_colour_all<D>), num_sms * 16, 128, 0, s, fc, b.vis_list, (const Counters*)b.counters, b.cull4, b.sh, b.rec_rgb)
   switch (fc.sh_degree) {
     case 0: LAUNCH(0); break;
     case 1: LAUNCH(1); break;

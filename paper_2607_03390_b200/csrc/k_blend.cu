@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
                                                          const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,
-                                                         const float* __restrict__ fill_depth, const float* __restrict__ warp_sigma,
+                                                         const float* __restrict__ fill_depth, const float2* __restrict__ warp_tgb,
                                                          float* __restrict__ image, float* __restrict__ depth, float* __restrict__ sigma,
                                                          uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters) {
   TGS_PDL_WAIT();
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
           image[pix * 3 + ch] = top * (1.0f - wy) + bot * wy;
         }
         depth[pix] = D;
-        sigma[pix] = warp_sigma[tq];
+        sigma[pix] = warp_tgb[tq].y;
       }
       continue;
     }
@@ -446,7 +446,7 @@ void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorte
   const int grid = num_sms * (PPT == 4 ? 12 : PPT == 8 ? 16 : 8);
 #define LAUNCH(M, C)                                                                                                          \
   TGS_LAUNCH((k_blend<M, C>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
-                                               prior_image, b.fill_depth, b.warp_sigma, b.image[out_idx], b.depth[out_idx],  \
+                                               prior_image, b.fill_depth, (const float2*)b.warp_tgb, b.image[out_idx], b.depth[out_idx],  \
                                                b.sigma[out_idx], rendered_next, b.counters)
   if (rendered_next) { if (count_interactions) LAUNCH(true, true); else LAUNCH(true, false); }
   else { if (count_interactions) LAUNCH(false, true); else LAUNCH(false, false); }

@@ -57,8 +57,8 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 // counters <- 0; sort histograms <- 0; tile_flags <- 0;
 // S frames: D^min <- INVALID bits, sigma^max <- 0; R / P frames: rendered_next <- 0;
 // R frames: F <- (+inf, +inf, -inf, -inf).
-__global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint32_t* warp_depth,
-                                                    uint32_t* warp_sigma, uint32_t* rendered_next_words, uint32_t n_words,
+__global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint2* warp_tgb,
+                                                    uint32_t* rendered_next_words, uint32_t n_words,
                                                     uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
                                                     uint32_t* F_key, int reset_F) {
   TGS_PDL_WAIT();
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
   if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
     const uint32_t px = (uint32_t)(fc.tg.W * fc.tg.H);
-    for (uint32_t i = tid; i < px; i += nth) { warp_depth[i] = TGS_INVALID_BITS; warp_sigma[i] = 0; }
+    for (uint32_t i = tid; i < px; i += nth) warp_tgb[i] = make_uint2(TGS_INVALID_BITS, 0u);
   }
   if (rendered_next_words)
     for (uint32_t i = tid; i < n_words; i += nth) rendered_next_words[i] = 0;
@@ -86,8 +86,7 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
 // floats order like their bit patterns) and atomicMax on the sigma bits: min depth and max sigma are kept
 // independently (L91, L97; R15), so the result does not depend on the order of arrival.
 __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __restrict__ prior_depth,
-                                              const float* __restrict__ prior_sigma, uint32_t* __restrict__ warp_depth,
-                                              uint32_t* __restrict__ warp_sigma) {
+                                              const float* __restrict__ prior_sigma, uint2* __restrict__ warp_tgb) {
   TGS_PDL_WAIT();
   const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
   const CamConst& kc = fc.cam;
@@ -121,15 +120,15 @@ __global__ void __launch_bounds__(256) k_warp(FrameConst fc, const float* __rest
   if (!(fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf)) return;
   const size_t q = (size_t)(int)fv * k.W + (int)fu;
   const float s = sg * fabsf((M[8] * rx + M[9] * ry) + M[10]);   // R13
-  atomicMin(&warp_depth[q], __float_as_uint(Z));
-  if (s > 0.0f) atomicMax(&warp_sigma[q], __float_as_uint(s));
+  atomicMin(&warp_tgb[q].x, __float_as_uint(Z));       // {D^min, sigma^max} interleaved: one 8-byte word per TOC lookup
+  if (s > 0.0f) atomicMax(&warp_tgb[q].y, __float_as_uint(s));
 }
 
 // ------------------------------------------------------------------ A2 depth fill + correspondence + T^um
 // One CTA per tile, one thread per pixel.  D' = D^min with isolated holes filled by the mean of the 8
 // neighbours (L121; R19).  matched <=> D' valid, back-projected z > z_near and the nearest reference pixel
 // is inside the image (R20).  Tile in T^um <=> any in-image pixel unmatched (R22).
-__global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* __restrict__ warp_depth, float* __restrict__ fill_depth,
+__global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float2* __restrict__ warp_tgb, float* __restrict__ fill_depth,
                                                    uint32_t* __restrict__ tile_flags) {
   TGS_PDL_WAIT();
   const TgbGrid& k = fc.tg;
@@ -140,12 +139,12 @@ __global__ void __launch_bounds__(256) k_fill_corr(FrameConst fc, const float* _
   const bool inside = ly < edge && x < k.W && y < k.H;
   bool unmatched = false;
   if (inside) {
-    const float* wd = warp_depth;
-    float D = wd[(size_t)y * k.W + x];
+    const float2* wd = warp_tgb;
+    float D = wd[(size_t)y * k.W + x].x;
     if (!(D < 1.0e38f) && x > 0 && y > 0 && x < k.W - 1 && y < k.H - 1) {
-      const float n0 = wd[(size_t)(y - 1) * k.W + x - 1], n1 = wd[(size_t)(y - 1) * k.W + x], n2 = wd[(size_t)(y - 1) * k.W + x + 1];
-      const float n3 = wd[(size_t)y * k.W + x - 1], n4 = wd[(size_t)y * k.W + x + 1];
-      const float n5 = wd[(size_t)(y + 1) * k.W + x - 1], n6 = wd[(size_t)(y + 1) * k.W + x], n7 = wd[(size_t)(y + 1) * k.W + x + 1];
+      const float n0 = wd[(size_t)(y - 1) * k.W + x - 1].x, n1 = wd[(size_t)(y - 1) * k.W + x].x, n2 = wd[(size_t)(y - 1) * k.W + x + 1].x;
+      const float n3 = wd[(size_t)y * k.W + x - 1].x, n4 = wd[(size_t)y * k.W + x + 1].x;
+      const float n5 = wd[(size_t)(y + 1) * k.W + x - 1].x, n6 = wd[(size_t)(y + 1) * k.W + x].x, n7 = wd[(size_t)(y + 1) * k.W + x + 1].x;
       if (n0 < 1.0e38f && n1 < 1.0e38f && n2 < 1.0e38f && n3 < 1.0e38f && n4 < 1.0e38f && n5 < 1.0e38f && n6 < 1.0e38f && n7 < 1.0e38f)
         D = (((((((n0 + n1) + n2) + n3) + n4) + n5) + n6) + n7) * 0.125f;
     }
@@ -243,8 +242,8 @@ struct PreSmem {
 };
 
 __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
-                                                               const uint8_t* __restrict__ rendered, const float* __restrict__ warp_depth,
-                                                               const float* __restrict__ warp_sigma, const uint32_t* __restrict__ F_key,
+                                                               const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
+                                                               const uint32_t* __restrict__ F_key,
                                                                float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
                                                                uint2* __restrict__ rec_rect, uint2* __restrict__ rec_trect,
                                                                uint32_t* __restrict__ rec_flags,
@@ -262,6 +261,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
   const uint32_t num_chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f;
   if (fc.do_afc) { F0 = key2f(F_key[0]); F1 = key2f(F_key[1]); F2 = key2f(F_key[2]); F3 = key2f(F_key[3]); }
+  const uint32_t ds_shift = fc.tg.ds == 2 ? 1u : 0u;
   const float offx = 1.0f + k.limx * k.limx, offy = 1.0f + k.limy * k.limy;
   const float xmax = (float)(k.TX * TGS_TILE) + 2.0f, ymax = (float)(k.TY * TGS_TILE) + 2.0f;
   uint32_t st_near = 0, st_afc = 0, st_toc = 0, st_deg = 0, st_empty = 0, st_nv = 0;
@@ -305,8 +305,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       const float fu = floorf(u + 0.5f), fv = floorf(v + 0.5f);
       const bool centre_in = fu >= 0.0f && fu < k.Wf && fv >= 0.0f && fv < k.Hf;
       if (fc.do_tgb && !((rend4 >> (8 * j)) & 0xffu) && centre_in) {                              // L113, L119
-        const size_t q = (size_t)((int)fv / fc.tg.ds) * fc.tg.W + (size_t)((int)fu / fc.tg.ds);   // R43: block of the nearest pixel
-        const float D = warp_depth[q], s = warp_sigma[q];
+        const uint32_t q = ((uint32_t)(int)fv >> ds_shift) * (uint32_t)fc.tg.W + ((uint32_t)(int)fu >> ds_shift);   // R43: block of the nearest pixel
+        const float2 Ds = warp_tgb[q];                                // {D^min, sigma^max}: one 8-byte word per lookup
+        const float D = Ds.x, s = Ds.y;
         if (fc.do_toc && tz > D + fc.lambda2 * s) { cf[j] = TGS_CULL_TOC; ++st_toc; continue; }
         if (tz <= D - fc.lambda1 * s) fl = 2u;
       }
@@ -494,18 +495,20 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
   }
 }
 
-// Visible list: the chunks' runs from the staging list (1024 slots per chunk) to their offsets (ascending index order).
+// Visible list: the chunks' runs from the staging list (2048 slots per chunk) to their offsets (ascending index order).
+// The indices also go to `vis_list`, a copy the depth sort does not permute (SH colours).
 __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __restrict__ pre_cnt, const uint32_t* __restrict__ st_keys,
                                                      const uint32_t* __restrict__ st_vals, uint32_t* __restrict__ vis_keys,
-                                                     uint32_t* __restrict__ vis_vals) {
+                                                     uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ vis_list) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   const uint32_t num_chunks = (n + PRE_CHUNK - 1) / PRE_CHUNK;
   for (uint32_t c = blockIdx.x; c < num_chunks; c += gridDim.x) {
     const uint2 cc = pre_cnt[c];
     for (uint32_t i = threadIdx.x; i < cc.x; i += blockDim.x) {
+      const uint32_t g = st_vals[(size_t)c * PRE_CHUNK + i];
       vis_keys[cc.y + i] = st_keys[(size_t)c * PRE_CHUNK + i];
-      vis_vals[cc.y + i] = st_vals[(size_t)c * PRE_CHUNK + i];
+      vis_vals[cc.y + i] = g; vis_list[cc.y + i] = g;
     }
   }
 }
@@ -612,28 +615,28 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
-  TGS_LAUNCH((k_frame_init), 592, 256, 0, s, fc, b.counters, b.tile_flags, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma,
+  TGS_LAUNCH((k_frame_init), 592, 256, 0, s, fc, b.counters, b.tile_flags, (uint2*)b.warp_tgb,
                                    (uint32_t*)rendered_next, n_words, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
                                    b.F_key, reset_F ? 1 : 0);
 }
 
 void launch_warp(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const float* prior_depth, const float* prior_sigma) {
   dim3 grid((fc.tg.W + 31) / 32, (fc.tg.H + 7) / 8);
-  TGS_LAUNCH((k_warp), grid, 256, 0, s, fc, prior_depth, prior_sigma, (uint32_t*)b.warp_depth, (uint32_t*)b.warp_sigma);
+  TGS_LAUNCH((k_warp), grid, 256, 0, s, fc, prior_depth, prior_sigma, (uint2*)b.warp_tgb);
 }
 
 void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
   dim3 grid(fc.cam.TX, fc.cam.TY);
-  TGS_LAUNCH((k_fill_corr), grid, 256, 0, s, fc, b.warp_depth, b.fill_depth, b.tile_flags);
+  TGS_LAUNCH((k_fill_corr), grid, 256, 0, s, fc, (const float2*)b.warp_tgb, b.fill_depth, b.tile_flags);
 }
 
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
-  TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, b.warp_depth, b.warp_sigma, b.F_key, b.rec_uvdo, b.rec_conic,
+  TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
-  TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0]);
+  TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list);
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

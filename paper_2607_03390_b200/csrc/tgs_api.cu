@@ -4,6 +4,7 @@
 // (12 floats) and the frame type.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <exception>
 #include <string>
@@ -139,8 +140,7 @@ int alloc_frame_buffers(tgs_ctx* c) {
     if (int r = dev_alloc(c, &b.depth[i], px, c->allocs_frame)) return r;
     if (int r = dev_alloc(c, &b.sigma[i], px, c->allocs_frame)) return r;
   }
-  if (int r = dev_alloc(c, &b.warp_depth, px, c->allocs_frame)) return r;
-  if (int r = dev_alloc(c, &b.warp_sigma, px, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.warp_tgb, px, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.fill_depth, px, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.tile_flags, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.tile_mask, (size_t)T, c->allocs_frame)) return r;
@@ -319,7 +319,7 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
   A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_trect, n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
   A(b.pre_cnt, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
-  A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n) A(b.bin_params, 3 * (size_t)n)
+  A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n) A(b.bin_params, 3 * (size_t)n) A(b.vis_list, n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
   AZ(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
 #undef A
@@ -693,8 +693,16 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
     src = c->ranges_dec; have = T * 8;
   }
   else if (name == "tile_order") { src = b.tile_order; have = T * 4; }
-  else if (name == "warp_depth") { src = b.warp_depth; have = tpx * 4; }
-  else if (name == "warp_sigma") { src = b.warp_sigma; have = tpx * 4; }
+  else if (name == "warp_depth" || name == "warp_sigma") {   // de-interleave {D^min, sigma^max}: a strided copy
+    have = tpx * 4;
+    if (dst && bytes) {
+      const size_t cnt = (bytes < have ? bytes : have) / 4;
+      const float* base = reinterpret_cast<const float*>(b.warp_tgb) + (name == "warp_sigma" ? 1 : 0);
+      CK(cudaMemcpy2DAsync(dst, 4, base, 8, 4, cnt, mem == TGS_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+      if (mem == TGS_HOST) CK(cudaStreamSynchronize(c->stream));
+    }
+    return (long long)have;
+  }
   else if (name == "fill_depth") { src = b.fill_depth; have = tpx * 4; }
   else if (name == "rendered") { src = b.rendered; have = N; }
   else if (name == "prior_depth") { src = b.depth[c->prior_idx]; have = px * 4; }

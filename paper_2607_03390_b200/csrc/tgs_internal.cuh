@@ -88,11 +88,12 @@ struct DevBuffers {
   uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian (test-only: filled by tgs_debug_get)
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
-  // visible Gaussians: ckeys = bits(depth), cvals = index; [1] staging (1024 slots per chunk), [0] in index order
+  // visible Gaussians: ckeys = bits(depth), cvals = index; [1] staging (2048 slots per chunk), [0] in index order
   // (k_compact_vis), then ping-pong of the depth sort
   uint32_t* ckeys[2] = {nullptr, nullptr};   // [N]
   uint32_t* cvals[2] = {nullptr, nullptr};   // [N]
-  uint2* pre_cnt = nullptr;                  // [ceil(N/1024)] {visible Gaussians of a preprocess chunk, of the chunks before it}
+  uint2* pre_cnt = nullptr;                  // [ceil(N/2048)] {visible Gaussians of a preprocess chunk, of the chunks before it}
+  uint32_t* vis_list = nullptr;              // [N] the visible Gaussians in index order (a copy the depth sort does not permute)
   uint32_t* area_prefix = nullptr;           // [N+1] tests before each sorted visible Gaussian
   uint32_t* chunk_first = nullptr;           // [bin_chunks_cap] sorted position of the Gaussian holding a chunk's first test
   uint32_t* nv_queue = nullptr;              // [N] newly visible Gaussians with rects of more than 4 tiles
@@ -116,8 +117,7 @@ struct DevBuffers {
   float* image[3] = {nullptr, nullptr, nullptr};   // [H][W][3]
   float* depth[3] = {nullptr, nullptr, nullptr};   // [H][W]
   float* sigma[3] = {nullptr, nullptr, nullptr};   // [H][W]
-  float* warp_depth = nullptr;  // D^min (uint bits during the splat)
-  float* warp_sigma = nullptr;  // sigma^max
+  float2* warp_tgb = nullptr;   // warped TGB {D^min, sigma^max} per grid pixel, interleaved (uint bits during the splat)
   float* fill_depth = nullptr;  // D'
   uint32_t* F_key = nullptr;    // [4] ordered-uint keys of F_min.x, F_min.y, F_max.x, F_max.y
   Counters* counters = nullptr;
