@@ -183,7 +183,7 @@ def summarise(lst):
     return {"frames": len(lst), "ms_total": m("ms_total"), "ms_stage": {n: float(v) for n, v in zip(STAGE_NAMES, ms)},
             "n_pairs": m("n_pairs"), "n_tests": m("n_tests"), "n_visible": m("n_visible"),
             "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
-            "n_interactions": m("n_interactions"), "n_blended": m("n_blended"), "n_pixel_slots": m("n_pixel_slots")}
+            "n_interactions": m("n_interactions"), "n_blended": m("n_blended"), "n_pixel_slots": m("n_pixel_slots"), "n_pairs_consumed": m("n_pairs_consumed")}
 
 
 class Harness:
@@ -250,8 +250,8 @@ class Harness:
             ctx.render(tgs.AUTO)
             cs = ctx.get_stats()
             st = timed_stats[f]
-            assert st["frame_type"] == cs["frame_type"] and st["n_pairs"] == cs["n_pairs"]
-            for key in ("n_interactions", "n_blended", "n_pixel_slots"):
+            assert st["frame_type"] == cs["frame_type"] and st["n_visible"] == cs["n_visible"]
+            for key in ("n_interactions", "n_blended", "n_pixel_slots", "n_pairs_consumed"):
                 st[key] = cs[key]
             per_type[st["frame_type"]].append(st)
         ctx.debug_run_stage("count_interactions_off")

@@ -77,13 +77,19 @@ typedef struct {
                              G_rendered grows by the Gaussians that frame blended */
   int tgb_downscale;      /* 1 (default) or 2: the TGB is warped, repaired and looked up on a ceil(W/2) x ceil(H/2) grid,
                              the paper's setting for large scenes (L142); downscale = min depth / max sigma of 2x2 (R43) */
+  int depth_slabs;        /* front-to-back slabs: the depth-ordered (Gaussian, tile) tests are binned, sorted and
+                             blended in this many consecutive pieces, and tiles whose pixels have all stopped (T < 1e-4) receive no
+                             pairs in the later pieces.  Image, TGB and G_rendered do not depend on it; the pair lists of the later
+                             pieces lack the pairs of finished tiles (records the blend would never have read).  1: one piece,
+                             the complete lists of L61; 2..4; 0 (default): automatic from the size of a recent frame */
+  uint32_t slab_split[3]; /* boundaries between the pieces in 1/1024 of the test space, ascending; 0 = built-in default */
 } tgs_params;
 enum { TGS_PRIORS_ANCHORED = 0, TGS_PRIORS_CHAINED = 1 };
 
 typedef struct {
   int frame_type; /* TGS_FRAME_R / P / S */
   uint32_t n_total, n_near, n_afc, n_toc, n_degenerate, n_empty, n_visible, n_newly_visible;
-  uint64_t n_pairs; /* P: sort length */
+  uint64_t n_pairs; /* P: pairs emitted = total sort length */
   uint32_t n_tiles, n_sel_oc, n_sel_um, n_sel;
   uint32_t n_rendered; /* |G_rendered| (R / P frames) */
   uint32_t overflow;   /* 1: n_pairs exceeded the capacity, frame invalid */
@@ -99,6 +105,11 @@ typedef struct {
   uint64_t device_bytes; /* device memory held by the context */
   uint64_t n_tests;      /* (Gaussian, tile) combinations the pair binning examined: sum of the test-rect areas of the visible
                             Gaussians (n_pairs of them passed: tile selected, L123, and reached with alpha >= 1/255, R39) */
+  uint64_t n_pairs_consumed; /* pairs the blend reached before their tile was finished (whole batches of 128; counting on): the
+                                rest of each tile's list lies behind saturated pixels and is never read */
+  uint32_t n_slabs;          /* pieces this frame was binned / sorted / blended in (tgs_params.depth_slabs) */
+  uint32_t n_pairs_slab[4];  /* pairs of each piece; n_pairs is their sum */
+  uint32_t n_finished_slab[4]; /* selected tiles finished by each piece before the last one (they get no pairs afterwards) */
   uint64_t launches_total; /* kernels this library has launched in this process so far (all contexts); bench.py reports the
                               difference over its timed region as `gpu_launches` */
 } tgs_stats;
@@ -158,7 +169,8 @@ const char* tgs_last_error(tgs_ctx*);
 /* ---- test-only: named intermediate buffers, so that a stage can be fed the oracle's inputs ----
  * tgs_debug_get copies min(bytes, size) bytes and returns the buffer's size in bytes (>= 0) or an error.
  * Readable: rec_uvdo rec_conic (float4 [N]) rec_rect (uint16x4 [N]) rec_flags (uint32 [N]) rec_rgb
- *   (float4 [N]) tiles_touched (uint32 [N]) keys (uint64 [P]) vals (uint32 [P]) ranges (uint32 [T][2])
+ *   (float4 [N]) tiles_touched (uint32 [N]) keys (uint64 [P]) vals (uint32 [P]) ranges (uint32 [T][2]) -- with more than one
+ *   slab (tgs_params.depth_slabs) these four describe the LAST slab only; the parity tests of the lists use depth_slabs = 1 --
  *   warp_depth warp_sigma fill_depth (float [H][W]) rendered (uint8 [N]) F (float[4]) prior_depth
  *   prior_sigma (float [H][W]) prior_image (float [H][W][3]) g2 (float [N][8]: Sigma xx xy xz yy yz zz, opacity, tau).
  * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):

@@ -29,7 +29,8 @@ class TgsParams(C.Structure):
     _fields_ = [("lambda1", C.c_float), ("lambda2", C.c_float), ("lambda_tdc", C.c_int), ("lambda_sr", C.c_int),
                 ("eta", C.c_float), ("bg", C.c_float * 3),
                 ("enable_afc", C.c_int), ("enable_toc", C.c_int), ("enable_sr", C.c_int), ("max_pairs", C.c_uint32),
-                ("exact_tiles", C.c_int), ("prior_policy", C.c_int), ("tgb_downscale", C.c_int)]
+                ("exact_tiles", C.c_int), ("prior_policy", C.c_int), ("tgb_downscale", C.c_int),
+                ("depth_slabs", C.c_int), ("slab_split", C.c_uint32 * 3)]
 
 
 class TgsStats(C.Structure):
@@ -41,11 +42,14 @@ class TgsStats(C.Structure):
                 ("n_tiles", C.c_uint32), ("n_sel_oc", C.c_uint32), ("n_sel_um", C.c_uint32), ("n_sel", C.c_uint32),
                 ("n_rendered", C.c_uint32), ("overflow", C.c_uint32), ("n_interactions", C.c_uint64), ("n_blended", C.c_uint64), ("n_pixel_slots", C.c_uint64),
                 ("ms_stage", C.c_float * 8), ("ms_total", C.c_float),
-                ("device_bytes", C.c_uint64), ("n_tests", C.c_uint64), ("launches_total", C.c_uint64)]
+                ("device_bytes", C.c_uint64), ("n_tests", C.c_uint64), ("n_pairs_consumed", C.c_uint64), ("n_slabs", C.c_uint32), ("n_pairs_slab", C.c_uint32 * 4), ("n_finished_slab", C.c_uint32 * 4),
+                ("launches_total", C.c_uint64)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_}
         d["ms_stage"] = list(self.ms_stage)
+        d["n_pairs_slab"] = list(self.n_pairs_slab)
+        d["n_finished_slab"] = list(self.n_finished_slab)
         return d
 
 

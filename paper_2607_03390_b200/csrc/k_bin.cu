@@ -110,7 +110,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
     for (int j = 0; j < SCAN_IPT; ++j) tsum += a[j];
     uint32_t incl_total;
     uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total, fc.epoch);
-    if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
+    if (tile == num_tiles - 1 && threadIdx.x == 0) {
+      counters->n_tests = incl_total; area_prefix[n] = incl_total;
+      // pairs <= tests: with the tests inside the capacity no slab can overflow, and the host need not wait for the end of
+      // the frame to know it (2 = cannot be ruled out yet)
+      if (incl_total > fc.max_pairs) { *host_overflow = 2u; __threadfence_system(); }
+    }
 #pragma unroll
     for (int j = 0; j < SCAN_IPT; ++j) {
       if (i0 + j >= n) break;
@@ -217,15 +222,26 @@ struct BinSmem {
 template <typename TileT>
 __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4* __restrict__ bin_params, const uint32_t* __restrict__ area_prefix,
                                                      const uint32_t* __restrict__ chunk_first,
-                                                     const uint32_t* __restrict__ sel_bits, unsigned long long* __restrict__ desc,
+                                                     const uint32_t* __restrict__ live_bits, unsigned long long* __restrict__ desc_all,
                                                      uint32_t* __restrict__ keys,
                                                      uint32_t* __restrict__ vals, uint32_t* __restrict__ tile_hist,
-                                                     Counters* __restrict__ counters, volatile uint32_t* __restrict__ host_overflow) {
+                                                     Counters* __restrict__ counters, volatile uint32_t* __restrict__ host_overflow, int slab,
+                                                     const uint32_t* __restrict__ live_sat) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   __shared__ BinSmem<TileT> sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
-  const uint32_t num_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
+  const uint32_t all_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
+  // this slab's range of chunks; inside the slab the chunks are numbered from 0 for the look-back
+  const uint32_t c_lo = (uint32_t)(((unsigned long long)all_chunks * fc.slab_bound[slab]) >> 10);
+  const uint32_t c_hi = (uint32_t)(((unsigned long long)all_chunks * fc.slab_bound[slab + 1]) >> 10);
+  uint32_t num_chunks = c_hi - c_lo;
+  unsigned long long* desc = desc_all + c_lo;
+  if (slab > 0) {   // every selected tile has finished in the earlier slabs: nothing left to bin (n_pairs_slab stays 0)
+    uint32_t fin = 0;
+    for (int j = 0; j < slab; ++j) fin += counters->n_finished[j];
+    if (fin >= counters->n_sel) num_chunks = 0;
+  }
   const uint32_t tid = threadIdx.x, lane = tid & 31;
   const int TX = fc.cam.TX;
   const bool exact = fc.exact_tiles != 0;
@@ -238,17 +254,18 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
   uint32_t pend = 0xffffffffu, pend_total = 0, it = 0;
   while (true) {
     __syncthreads();
-    if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin, 1u);
+    if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin[slab], 1u);
     __syncthreads();
-    const uint32_t chunk = sm.chunk;
+    const uint32_t chunk = sm.chunk;                                 // within the slab
     const bool have = chunk < num_chunks;
     const uint32_t buf = it & 1u;
     uint32_t total = 0;
     if (have) {
-      const uint32_t cbase = chunk * BIN_CHUNK;
+      const uint32_t gchunk = c_lo + chunk;                          // in the flat test space
+      const uint32_t cbase = gchunk * BIN_CHUNK;
       const uint32_t tend = (total_tests - cbase < (uint32_t)BIN_CHUNK) ? total_tests : cbase + BIN_CHUNK;
-      const uint32_t i_first = chunk_first[chunk];
-      const uint32_t i_last = (chunk + 1 < num_chunks) ? chunk_first[chunk + 1] : n - 1;
+      const uint32_t i_first = chunk_first[gchunk];
+      const uint32_t i_last = (gchunk + 1 < all_chunks) ? chunk_first[gchunk + 1] : n - 1;
       const uint32_t m = i_last - i_first + 1;                     // <= BIN_CHUNK + 1
       for (uint32_t i = tid; i <= m; i += BIN_THREADS) sm.prefix[i] = area_prefix[i_first + i];
       {   // the chunk's parameters are one contiguous block of the sorted array: coalesced 16 B copies
@@ -258,6 +275,19 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
         for (uint32_t i = tid; i < nq; i += BIN_THREADS) dst[i] = src[i];
       }
       __syncthreads();
+      if (slab > 0) {
+        // Later slabs: most tiles have finished.  A Gaussian whose test rect holds no live tile -- four look-ups in the
+        // summed-area table of the live tiles (k_live_sat) -- has all its tests skipped without looking at them.
+        const uint32_t mm = m < (uint32_t)BIN_PCAP ? m : (uint32_t)BIN_PCAP;
+        const uint32_t SW = (uint32_t)TX + 1u;
+        for (uint32_t l = tid; l < mm; l += BIN_THREADS) {
+          GaussParams& Gp = sm.gp[l];
+          const uint32_t x0 = Gp.lo & 0xffffu, y0 = Gp.lo >> 16, w = Gp.w, h = (sm.prefix[l + 1] - sm.prefix[l]) / (w ? w : 1u);
+          const uint32_t cnt = (live_sat[(y0 + h) * SW + x0 + w] - live_sat[y0 * SW + x0 + w]) - (live_sat[(y0 + h) * SW + x0] - live_sat[y0 * SW + x0]);
+          Gp.pad = cnt ? 0u : 1u;                                  // pad = 1: dead
+        }
+        __syncthreads();
+      }
       // -------------------------------------------------------------- tests
       const uint32_t t0 = cbase + tid * BIN_IPT;
       uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
@@ -279,8 +309,9 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
           const uint32_t t = t0 + k;
           if (t < tend) {
             if (t >= end) { do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
+            if (G.pad) continue;                                           // no live tile in this Gaussian's rect (later slabs)
             const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
-            bool pass = fc.all_tiles || ((sel_bits[tile >> 5] >> (tile & 31)) & 1u);                       // L123
+            bool pass = (live_bits[tile >> 5] >> (tile & 31)) & 1u;        // selected (L123) and not yet finished (slabs)
             if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
             if (pass) mask |= 1u << k;
             tl[k] = tile; gg[k] = G.g;
@@ -313,8 +344,8 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
       const uint32_t cexcl = sm.excl, ctotal = pend_total, incl_total = cexcl + ctotal, pbuf = buf ^ 1u;
       const bool overflow = incl_total > fc.max_pairs;
       if (pend == num_chunks - 1 && tid == 0) {
-        if (overflow) { counters->overflow = 1; counters->n_pairs = 0; *host_overflow = 1u; __threadfence_system(); }   // the host reads it after ev_bin
-        else counters->n_pairs = incl_total;
+        if (overflow) { counters->overflow = 1; counters->n_pairs_slab[slab] = 0; *host_overflow = 1u; __threadfence_system(); }
+        else { counters->n_pairs_slab[slab] = incl_total; counters->n_pairs += incl_total; }   // slabs run one after the other
       }
       if (!overflow)
         for (uint32_t p0 = 0; p0 < ctotal; p0 += BIN_THREADS) {
@@ -381,21 +412,48 @@ __global__ void __launch_bounds__(256) k_keys64(const uint32_t* __restrict__ key
 uint32_t scan_tile_items() { return SCAN_TILE; }
 uint32_t bin_chunk_items() { return BIN_CHUNK; }
 
+// Summed-area table of the live tiles, (TY + 1) x (TX + 1) with a zero border: sat[y][x] = live tiles with ty < y, tx < x.
+// One CTA: a thread per tile row (prefix along x), then a thread per column (prefix along y); 8 K entries at 1080p.
+__global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_t* __restrict__ live_bits, uint32_t* __restrict__ sat) {
+  TGS_PDL_WAIT();
+  TGS_PDL_TRIGGER();
+  const int SW = TX + 1;
+  for (int x = threadIdx.x; x <= TX; x += blockDim.x) sat[x] = 0;
+  for (int y = threadIdx.x; y < TY; y += blockDim.x) {
+    uint32_t run = 0;
+    sat[(y + 1) * SW] = 0;
+    for (int x = 0; x < TX; ++x) {
+      const int t = y * TX + x;
+      run += (live_bits[t >> 5] >> (t & 31)) & 1u;
+      sat[(y + 1) * SW + x + 1] = run;
+    }
+  }
+  __syncthreads();
+  for (int x = threadIdx.x + 1; x <= TX; x += blockDim.x) {
+    uint32_t run = 0;
+    for (int y = 1; y <= TY; ++y) { run += sat[y * SW + x]; sat[y * SW + x] = run; }
+  }
+}
+
 // sorted_g_idx: which of cvals[] holds the visible Gaussians in (depth, index) order
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms,
-                uint32_t* host_overflow) {
-  const uint32_t scan_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_visible <= N)
-  const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
-  const uint32_t* sorted_g = b.cvals[sorted_g_idx];
-  uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
-  TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
-                                                      b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
+                uint32_t* host_overflow, int slab) {
+  if (slab == 0) {
+    const uint32_t scan_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_visible <= N)
+    const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
+    const uint32_t* sorted_g = b.cvals[sorted_g_idx];
+    uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
+    TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
+                                                        b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
+  }
+  if (slab > 0) TGS_LAUNCH((k_live_sat), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
+  uint32_t* hist = b.sort_hist + (1 + slab) * 4 * 256;
   if (fc.n_tiles <= 65536)
-    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters, (volatile uint32_t*)host_overflow);
+    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], hist, b.counters, (volatile uint32_t*)host_overflow, slab, (const uint32_t*)b.live_sat);
   else
-    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.sel_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], b.sort_hist + 4 * 256, b.counters, (volatile uint32_t*)host_overflow);
+    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,
+                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], hist, b.counters, (volatile uint32_t*)host_overflow, slab, (const uint32_t*)b.live_sat);
 }
 
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

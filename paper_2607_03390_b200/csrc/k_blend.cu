@@ -126,12 +126,14 @@ __device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p
 // schedules the loop with fewer spills around the batch boundaries (P-frame blend 0.166 -> 0.162 ms).
 template <bool MARK, bool COUNT>
 __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLEND_MIN_CTAS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
-                                                         const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
+                                                         uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
                                                          const float4* __restrict__ rec_rgb, const float* __restrict__ prior_image,
                                                          const float* __restrict__ fill_depth, const float2* __restrict__ warp_tgb,
                                                          float* __restrict__ image, float* __restrict__ depth, float* __restrict__ sigma,
-                                                         uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters) {
+                                                         uint8_t* __restrict__ rendered_next, Counters* __restrict__ counters,
+                                                         uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ live_bits,
+                                                         float* __restrict__ pix_state, int slab) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   __shared__ BlendSmem sm;
@@ -139,12 +141,21 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int lx = (int)(tid % RUNS) * PPT, ly = (int)(tid / RUNS);
   const uint32_t n_sel = counters->n_sel;
+  // Front-to-back slabs: this launch blends the pairs of slab `slab`.  A tile whose pixels have all
+  // stopped is written out and leaves `live_bits` (the later slabs bin no pairs for it); a tile that is still alive at the
+  // end of its list parks its pixel states in `pix_state` and goes on in the next slab; the last slab writes every tile.
+  const bool last = slab == fc.n_slabs - 1;
+  const uint32_t n_work = slab == 0 ? (uint32_t)fc.n_tiles : n_sel;      // the stitched tiles are done with slab 0
+  uint32_t zero_tile = 0xffffffffu;                                       // (thread 0) tile whose range is to be cleared for the next slab
   while (true) {
     __syncthreads();
-    if (tid == 0) sm.work = atomicAdd(&counters->ticket_blend, 1u);
+    if (tid == 0) {
+      if (zero_tile != 0xffffffffu) { ranges[zero_tile] = make_uint2(0u, 0u); zero_tile = 0xffffffffu; }
+      sm.work = atomicAdd(&counters->ticket_blend[slab], 1u);
+    }
     __syncthreads();
     const uint32_t w = sm.work;
-    if (w >= (uint32_t)fc.n_tiles) break;
+    if (w >= n_work) break;
     const uint32_t tile = tile_order[w];
     const int tile_x0 = (int)(tile % k.TX) * TGS_TILE, tile_y0 = (int)(tile / k.TX) * TGS_TILE;
     const int px0 = tile_x0 + lx, py = tile_y0 + ly;
@@ -184,9 +195,14 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
       continue;
     }
     // -------------------------------------------------- A8 blend
+    if (slab > 0 && !((live_bits[tile >> 5] >> (tile & 31u)) & 1u)) continue;      // finished (and written) in an earlier slab
     uint2 range = ranges[tile];                      // {~start, end}, zero for a tile without pairs (k_sort.cu, A7)
     range.x = range.y ? ~range.x : 0u;
     const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
+    if (len == 0u && !last) continue;                // nothing of this slab reaches the tile: its state, if any, stays parked
+    if (!last && tid == 0) zero_tile = tile;
+    const bool restore = slab > 0 && (tile_flags[tile] & 8u) != 0u;
+    float* const st_base = pix_state + (size_t)tile * (7 * TGS_TILE * TGS_TILE);
     float fpx = (float)px0, fpy = (float)py;
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
     float2 T2[NQ], Cr2[NQ], Cg2[NQ], Cb2[NQ], S12[NQ], S22[NQ];
@@ -207,6 +223,39 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
     for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) T2[q] = make_float2(valid[2 * q] ? EX2_SCALE : -EX2_SCALE, valid[2 * q + 1] ? EX2_SCALE : -EX2_SCALE);   // T' = EX2_SCALE T
+    if (restore) {
+      // parked states, [field][pixel]: T' (scaled, negative = stopped, 0 = already written), Cr, Cg, Cb, S1, S2, d0
+      static_assert(PPT == 4, "state layout: one float4 per thread and field");
+      float f[7][PPT];
+#pragma unroll
+      for (int j = 0; j < 7; ++j) {
+        const float4 t4 = reinterpret_cast<const float4*>(st_base + j * (TGS_TILE * TGS_TILE))[tid];
+        f[j][0] = t4.x; f[j][1] = t4.y; f[j][2] = t4.z; f[j][3] = t4.w;
+      }
+      // common reference depth of the run's Eq.1-2 moments: that of its first pixel with a contribution; the moments of
+      // pixels parked with another reference (sparse mode keeps one per pixel) are re-referenced (values, not decisions)
+      bool have_ref = false;
+#pragma unroll
+      for (int i = 0; i < PPT; ++i) {
+        if (f[0][i] == 0.0f) { valid[i] = false; f[0][i] = -EX2_SCALE; }
+        else if (!have_ref && fabsf(f[0][i]) != EX2_SCALE) { have_ref = true; dref = f[6][i]; }
+      }
+      open = !have_ref;
+#pragma unroll
+      for (int i = 0; i < PPT; ++i) {
+        if (valid[i] && fabsf(f[0][i]) != EX2_SCALE && f[6][i] != dref) {
+          const float Sw = 1.0f - fabsf(f[0][i]) * EX2_SCALE_INV, dl = f[6][i] - dref;
+          f[5][i] = fmaf(dl, fmaf(Sw, dl, 2.0f * f[4][i]), f[5][i]);
+          f[4][i] = fmaf(Sw, dl, f[4][i]);
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) {
+        T2[q] = make_float2(f[0][2 * q], f[0][2 * q + 1]); Cr2[q] = make_float2(f[1][2 * q], f[1][2 * q + 1]);
+        Cg2[q] = make_float2(f[2][2 * q], f[2][2 * q + 1]); Cb2[q] = make_float2(f[3][2 * q], f[3][2 * q + 1]);
+        S12[q] = make_float2(f[4][2 * q], f[4][2 * q + 1]); S22[q] = make_float2(f[5][2 * q], f[5][2 * q + 1]);
+      }
+    }
     auto get_px = [&](int i) {
       Pixel r;
       const int q = i >> 1;
@@ -260,6 +309,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
     load_ids(0); issue(0); load_ids(1);
     uint32_t nint = 0, nhit = 0, nslot = 0;
     int computed = -1;
+    uint32_t nb_done = 0;                   // batches this tile went through (COUNT)
     for (uint32_t b = 0; b < nb; ++b) {
       const uint32_t na_t = sparse ? (uint32_t)(have && salive)
                                    : count_alive();
@@ -419,15 +469,49 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
         }
       }
       computed = (int)b;
+      if (COUNT) nb_done = b + 1u;
     }
     if (MARK && computed >= 0) { __syncthreads(); writeback_marks((uint32_t)computed); }
-    // -------------------------------------------------- outputs
-    if (!sparse) {
+    // -------------------------------------------------- outputs, or the states parked for the next slab
+    bool park = false;
+    if (!last) {
+      const bool alive_t = sparse ? (have && salive) : (count_alive() != 0u);
+      park = __syncthreads_or(alive_t ? 1 : 0) != 0;
+    }
+    if (park) {
+      float4* const st4 = reinterpret_cast<float4*>(st_base);
+      constexpr int FS = TGS_TILE * TGS_TILE / 4;                     // float4 per field
+      if (!sparse) {
+        // a pixel outside the image is parked as "written" (it never is): T' = 0
+        st4[0 * FS + tid] = make_float4(valid[0] ? T2[0].x : 0.0f, valid[1] ? T2[0].y : 0.0f, valid[2] ? T2[1].x : 0.0f, valid[3] ? T2[1].y : 0.0f);
+        st4[1 * FS + tid] = make_float4(Cr2[0].x, Cr2[0].y, Cr2[1].x, Cr2[1].y);
+        st4[2 * FS + tid] = make_float4(Cg2[0].x, Cg2[0].y, Cg2[1].x, Cg2[1].y);
+        st4[3 * FS + tid] = make_float4(Cb2[0].x, Cb2[0].y, Cb2[1].x, Cb2[1].y);
+        st4[4 * FS + tid] = make_float4(S12[0].x, S12[0].y, S12[1].x, S12[1].y);
+        st4[5 * FS + tid] = make_float4(S22[0].x, S22[0].y, S22[1].x, S22[1].y);
+        st4[6 * FS + tid] = make_float4(dref, dref, dref, dref);
+      } else {
+        // sparse mode: the pixels that were dropped at a compaction have been written; the others sit one per thread
+        st4[tid] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        __syncthreads();
+        if (have) {
+          float* const sf = st_base;
+          const float Ts = sp.T == 1.0f ? EX2_SCALE : sp.T * EX2_SCALE;
+          sf[0 * 256 + spx] = salive ? Ts : -Ts;
+          sf[1 * 256 + spx] = sp.Cr; sf[2 * 256 + spx] = sp.Cg; sf[3 * 256 + spx] = sp.Cb;
+          sf[4 * 256 + spx] = sp.S1; sf[5 * 256 + spx] = sp.S2; sf[6 * 256 + spx] = sp.d0;
+        }
+      }
+      if (tid == 0) { tile_flags[tile] |= 8u; atomicAdd(&counters->n_live_after[slab], 1u); }   // only this CTA touches the flag word while the blend runs
+    } else {
+      if (!sparse) {
 #pragma unroll
-      for (int i = 0; i < PPT; ++i)
-        if (valid[i]) { Pixel pi = get_px(i); pi.T = fabsf(pi.T); write_pixel(fc, pi, (size_t)py * k.W + px0 + i, image, depth, sigma); }
-    } else if (have) {
-      write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
+        for (int i = 0; i < PPT; ++i)
+          if (valid[i]) { Pixel pi = get_px(i); pi.T = fabsf(pi.T); write_pixel(fc, pi, (size_t)py * k.W + px0 + i, image, depth, sigma); }
+      } else if (have) {
+        write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
+      }
+      if (!last && tid == 0) { atomicAnd(&live_bits[tile >> 5], ~(1u << (tile & 31u))); atomicAdd(&counters->n_finished[slab], 1u); }   // finished: no pairs in the later slabs
     }
     if (COUNT) {
       nint = __reduce_add_sync(0xffffffffu, nint);
@@ -435,6 +519,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
       nhit = __reduce_add_sync(0xffffffffu, nhit);
       nslot = __reduce_max_sync(0xffffffffu, nslot) * 32u;     // lanes that left the loop early still occupy the warp
       if (lane == 0) { atomicAdd(&counters->n_blended, (unsigned long long)nhit); atomicAdd(&counters->n_slots, (unsigned long long)nslot); }
+      if (tid == 0 && nb_done) atomicAdd(&counters->n_consumed, (unsigned long long)min(len, nb_done * BLEND_BATCH));
     }
   }
 }
@@ -442,12 +527,12 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
 }  // namespace
 
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
-                  uint8_t* rendered_next, int num_sms, bool count_interactions) {
+                  uint8_t* rendered_next, int num_sms, bool count_interactions, int slab) {
   const int grid = num_sms * (PPT == 4 ? 12 : PPT == 8 ? 16 : 8);
 #define LAUNCH(M, C)                                                                                                          \
   TGS_LAUNCH((k_blend<M, C>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, (const float2*)b.warp_tgb, b.image[out_idx], b.depth[out_idx],  \
-                                               b.sigma[out_idx], rendered_next, b.counters)
+                                               b.sigma[out_idx], rendered_next, b.counters, b.tile_flags, b.live_bits, b.pix_state, slab)
   if (rendered_next) { if (count_interactions) LAUNCH(true, true); else LAUNCH(true, false); }
   else { if (count_interactions) LAUNCH(false, true); else LAUNCH(false, false); }
 #undef LAUNCH

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) k_repack(uint32_t n, const float* __restr
 __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* counters, uint32_t* tile_flags, uint2* warp_tgb,
                                                     uint32_t* rendered_next_words, uint32_t n_words,
                                                     uint32_t* sort_hist, uint2* ranges, uint8_t* tile_mask, uint32_t* tile_order, uint32_t* sel_bits,
-                                                    uint32_t* F_key, int reset_F) {
+                                                    uint32_t* live_bits, uint32_t* F_key, int reset_F) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
@@ -70,9 +70,9 @@ __global__ void __launch_bounds__(256) k_frame_init(FrameConst fc, Counters* cou
   if (reset_F && tid < 4) F_key[tid] = (tid < 2) ? 0xff800000u /* key(+inf) */ : 0x007fffffu /* key(-inf) */;
   for (uint32_t i = tid; i < (uint32_t)fc.n_tiles; i += nth) {
     tile_flags[i] = 0; ranges[i] = make_uint2(0u, 0u);
-    if (trivial_sel) { tile_mask[i] = 4; tile_order[i] = i; if ((i & 31u) == 0u) sel_bits[i >> 5] = 0xffffffffu; }
+    if (trivial_sel) { tile_mask[i] = 4; tile_order[i] = i; if ((i & 31u) == 0u) { sel_bits[i >> 5] = 0xffffffffu; live_bits[i >> 5] = 0xffffffffu; } }
   }
-  if (tid < 2 * 4 * 256) sort_hist[tid] = 0;
+  if (tid < (1 + TGS_MAX_SLABS) * 4 * 256) sort_hist[tid] = 0;
   if (fc.do_tgb) {
     const uint32_t px = (uint32_t)(fc.tg.W * fc.tg.H);
     for (uint32_t i = tid; i < px; i += nth) warp_tgb[i] = make_uint2(TGS_INVALID_BITS, 0u);
@@ -518,7 +518,7 @@ __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __
 // of the bit set).  Builds the tile mask, the bit set used by the pair binning, and the work order of the blend
 // kernel: selected tiles first (ascending id), then the tiles that are only stitched.
 __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* __restrict__ tile_flags, uint8_t* __restrict__ tile_mask,
-                                                 uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ tile_order,
+                                                 uint32_t* __restrict__ sel_bits, uint32_t* __restrict__ live_bits, uint32_t* __restrict__ tile_order,
                                                  Counters* __restrict__ counters, volatile uint32_t* __restrict__ host_n_sel) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
@@ -535,7 +535,7 @@ __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* 
     const bool sel = t < T && (fc.all_tiles || f != 0);
     if (t < T) tile_mask[t] = (uint8_t)(f | (sel ? 4u : 0u));
     const uint32_t word = __ballot_sync(0xffffffffu, sel);
-    if (lane == 0) sel_bits[w] = word;
+    if (lane == 0) { sel_bits[w] = word; live_bits[w] = word; }
     nsel += __popc(word);
     noc += __popc(__ballot_sync(0xffffffffu, (f & 1u) != 0)); num += __popc(__ballot_sync(0xffffffffu, (f & 2u) != 0));
   }
@@ -616,7 +616,7 @@ void launch_repack(cudaStream_t s, uint32_t n, int K, const float* means, const 
 void launch_frame_init(cudaStream_t s, const FrameConst& fc, DevBuffers& b, bool reset_F, uint8_t* rendered_next) {
   const uint32_t n_words = rendered_next ? (fc.n + 3) / 4 : 0;
   TGS_LAUNCH((k_frame_init), 592, 256, 0, s, fc, b.counters, b.tile_flags, (uint2*)b.warp_tgb,
-                                   (uint32_t*)rendered_next, n_words, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits,
+                                   (uint32_t*)rendered_next, n_words, b.sort_hist, b.ranges, b.tile_mask, b.tile_order, b.sel_bits, b.live_bits,
                                    b.F_key, reset_F ? 1 : 0);
 }
 
@@ -644,17 +644,17 @@ void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t* host_n_sel) {
-  TGS_LAUNCH((k_select), 1, 1024, 0, s, fc, b.tile_flags, b.tile_mask, b.sel_bits, b.tile_order, b.counters, (volatile uint32_t*)host_n_sel);
+  TGS_LAUNCH((k_select), 1, 1024, 0, s, fc, b.tile_flags, b.tile_mask, b.sel_bits, b.live_bits, b.tile_order, b.counters, (volatile uint32_t*)host_n_sel);
 }
 
 // The frame's counters to pinned host memory by zero-copy stores (no copy engine: see k_select).
-__global__ void __launch_bounds__(64) k_export_counters(const Counters* __restrict__ counters, volatile uint32_t* __restrict__ host) {
+__global__ void __launch_bounds__(128) k_export_counters(const Counters* __restrict__ counters, volatile uint32_t* __restrict__ host) {
   TGS_PDL_WAIT();
   if (threadIdx.x < sizeof(Counters) / 4) host[threadIdx.x] = reinterpret_cast<const uint32_t*>(counters)[threadIdx.x];
   __threadfence_system();
 }
 void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host) {
-  TGS_LAUNCH((k_export_counters), 1, 64, 0, s, (const Counters*)b.counters, (volatile uint32_t*)host);
+  TGS_LAUNCH((k_export_counters), 1, 128, 0, s, (const Counters*)b.counters, (volatile uint32_t*)host);
 }
 
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F) {

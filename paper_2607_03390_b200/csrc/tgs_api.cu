@@ -55,7 +55,8 @@ struct tgs_ctx {
   DevBuffers b;
   std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
   // stats
-  Counters* h_counters = nullptr;      // pinned
+  Counters* h_counters = nullptr;      // pinned: the block of the last rendered frame (= h_cnt2[parity])
+  Counters* h_cnt2[2] = {nullptr, nullptr};   // pinned, by frame parity: frame N - 2's statistics are complete and unchanged when frame N is set up
   uint32_t* h_sel = nullptr;           // pinned: n_sel of the last S frame (for the eta rule)
   cudaEvent_t ev_sel = nullptr, ev_done = nullptr;
   // the device counters are double-buffered by frame parity: their (latency-bound) copy to the host runs on the third
@@ -83,7 +84,15 @@ struct tgs_ctx {
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
   bool count_interactions = false;
-  cudaEvent_t ev_stage[10];
+  // stage timing: an event before every launch group, tagged with the stage (0..7) the time up to the next event goes to
+  static constexpr int MAX_EV = 48;
+  cudaEvent_t ev_stage[MAX_EV];
+  int ev_tag[MAX_EV]; int n_ev = 0;
+  int last_n_slabs = 1;
+  // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
+  // recent one-piece and two-piece frames; slabs are used where they drop more than half of the pairs
+  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0; } slab_ctl[2];
+  int hist_cls[2] = {0, 0}, hist_slabs[2] = {1, 1};   // class and number of slabs of the frame that last used each counter block
   FrameConst fc;
 };
 
@@ -145,6 +154,9 @@ int alloc_frame_buffers(tgs_ctx* c) {
   if (int r = dev_alloc(c, &b.tile_flags, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.tile_mask, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.sel_bits, (size_t)(T + 31) / 32 + 1, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.live_bits, (size_t)(T + 31) / 32 + 1, c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.live_sat, (size_t)(c->TX + 1) * (c->TY + 1), c->allocs_frame)) return r;
+  if (int r = dev_alloc(c, &b.pix_state, (size_t)T * 7 * TGS_TILE * TGS_TILE, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.tile_order, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.ranges, (size_t)T, c->allocs_frame)) return r;
   c->px_cap = px; c->tiles_cap = T;
@@ -232,6 +244,8 @@ void tgs_default_params(tgs_params* p) {
   p->exact_tiles = 1;
   p->prior_policy = TGS_PRIORS_ANCHORED;
   p->tgb_downscale = 1;
+  p->depth_slabs = 0;
+  p->slab_split[0] = p->slab_split[1] = p->slab_split[2] = 0;
 }
 
 static void destroy_ctx(tgs_ctx* c) {   // tolerates a partially constructed context (tgs_create's failure paths)
@@ -243,7 +257,7 @@ static void destroy_ctx(tgs_ctx* c) {   // tolerates a partially constructed con
   for (auto& p : c->counters2) if (p) cudaFree(p);
   if (c->F_base) cudaFree(c->F_base);
   if (c->b.sort_hist) cudaFree(c->b.sort_hist);
-  if (c->h_counters) cudaFreeHost(c->h_counters);
+  for (auto& p : c->h_cnt2) if (p) cudaFreeHost(p);
   if (c->h_sel) cudaFreeHost(c->h_sel);
   if (c->h_ovf) cudaFreeHost(c->h_ovf);
   for (auto& e : c->ev_cnt) if (e) cudaEventDestroy(e);
@@ -265,13 +279,13 @@ static int create_impl(tgs_ctx** out, int device, void* stream) {
   cudaDeviceProp prop;
   ok = ok && cudaGetDeviceProperties(&prop, device) == cudaSuccess;
   if (ok) c->num_sms = prop.multiProcessorCount;
-  ok = ok && cudaMallocHost((void**)&c->h_counters, sizeof(Counters)) == cudaSuccess;
+  for (auto& p : c->h_cnt2) ok = ok && cudaMallocHost((void**)&p, sizeof(Counters)) == cudaSuccess;
   ok = ok && cudaMallocHost((void**)&c->h_sel, 2 * sizeof(uint32_t)) == cudaSuccess;
   ok = ok && cudaMallocHost((void**)&c->h_ovf, 2 * sizeof(uint32_t)) == cudaSuccess;
-  if (ok) { memset(c->h_counters, 0, sizeof(Counters)); c->h_ovf[0] = c->h_ovf[1] = 0; c->h_sel[0] = c->h_sel[1] = 0; }
+  if (ok) { for (auto& p : c->h_cnt2) memset(p, 0, sizeof(Counters)); c->h_counters = c->h_cnt2[0]; c->h_ovf[0] = c->h_ovf[1] = 0; c->h_sel[0] = c->h_sel[1] = 0; }
   for (auto& p : c->counters2) ok = ok && cudaMalloc((void**)&p, sizeof(Counters)) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->F_base, 8 * sizeof(uint32_t)) == cudaSuccess;   // two F's, by frame parity
-  ok = ok && cudaMalloc((void**)&c->b.sort_hist, 2 * 4 * 256 * sizeof(uint32_t)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->b.sort_hist, (1 + TGS_MAX_SLABS) * 4 * 256 * sizeof(uint32_t)) == cudaSuccess;
   for (auto& e : c->ev_cnt) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
   for (auto& e : c->ev_copy) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
   for (cudaEvent_t* e : {&c->ev_post, &c->ev_post2, &c->ev_sel, &c->ev_done, &c->ev_bin, &c->ev_fork, &c->ev_join, &c->ev_fork2, &c->ev_join2, &c->ev_fork3})
@@ -349,6 +363,7 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
   if (e != cudaSuccess) { snprintf(c->err, sizeof(c->err), "load: %s", cudaGetErrorString(e)); return TGS_E_CUDA; }
   c->n = n; c->deg = deg; c->K = K;
   c->nv_hint = n / 4;
+  c->slab_ctl[0] = tgs_ctx::SlabCtl(); c->slab_ctl[1] = tgs_ctx::SlabCtl();
   invalidate_priors(c);
   c->have_frame = false;
   return TGS_OK;
@@ -369,7 +384,8 @@ int tgs_set_camera(tgs_ctx* c, const float view[16], float fx, float fy, float c
 int tgs_set_params(tgs_ctx* c, const tgs_params* p) {
   if (!c || !p || p->lambda_tdc < 1 || p->lambda_sr < 1 || !std::isfinite(p->lambda1) || !std::isfinite(p->lambda2) ||
       !std::isfinite(p->eta) || !finite_all(p->bg, 3) || (p->prior_policy != TGS_PRIORS_ANCHORED && p->prior_policy != TGS_PRIORS_CHAINED) ||
-      (p->tgb_downscale != 1 && p->tgb_downscale != 2)) return TGS_E_INVALID_ARG;
+      (p->tgb_downscale != 1 && p->tgb_downscale != 2) || p->depth_slabs < 0 || p->depth_slabs > TGS_MAX_SLABS) return TGS_E_INVALID_ARG;
+  for (int i = 0; i < 3; ++i) if (p->slab_split[i] > 1023u) return TGS_E_INVALID_ARG;
   c->prm = *p;
   return TGS_OK;
 }
@@ -392,9 +408,13 @@ static int render_impl(tgs_ctx* c, int mode) {
   CK(cudaSetDevice(c->device));
   // ---- what the previous frame left for the host mid-frame: the overflow flag of its pair binning ...
   if (c->bin_pending) {
-    CK(cudaEventSynchronize(c->ev_bin));          // k_bin of the previous frame has finished (its tile sort / blend may still run)
+    // k_scan_area / the first k_bin of the previous frame have finished (its sorts and blends may still run).  0: the tests fit
+    // the capacity, so no slab can overflow; otherwise the answer is only known when the frame has ended.
+    CK(cudaEventSynchronize(c->ev_bin));
     c->bin_pending = false;
-    if (c->h_ovf[c->bin_slot]) {
+    bool overflowed = false;
+    if (c->h_ovf[c->bin_slot]) { CK(cudaEventSynchronize(c->ev_done)); overflowed = c->h_counters->overflow != 0; }
+    if (overflowed) {
       // That frame is background only (TGS_E_CAPACITY from tgs_get_stats) and whatever it committed -- TAB, TGB, G_rendered,
       // an F of (+inf, -inf) that would make AFC cull everything -- must never be used: drop the priors, so the next AUTO
       // frame is a reference frame, and grow the automatic capacity before it.
@@ -428,12 +448,32 @@ static int render_impl(tgs_ctx* c, int mode) {
   if (int r = alloc_frame_buffers(c)) return r;
   const int tile_bits = tile_key_bits(c->TX * c->TY), tile_passes = (tile_bits + 7) / 8;
   if (int r = alloc_pair_buffers(c, c->prm.max_pairs ? c->prm.max_pairs : auto_max_pairs(c), tile_passes)) return r;
-  // grow the pair buffers when the previous frame came close to (or over) the capacity
-  // which instance of the depth sort: the small-input one (many tiles in flight, long look-back steps) or the one of the
-  // tile sort; decided from the visible count of the last frame whose counters have arrived (a hint, never waited for)
-  if (c->have_frame && cudaEventQuery(c->ev_done) == cudaSuccess) c->nv_hint = c->h_counters->n_visible;
-  if (!c->prm.max_pairs && c->have_frame) {
-    if (cudaEventQuery(c->ev_done) == cudaSuccess && (c->h_counters->overflow || c->h_counters->n_pairs > c->max_pairs / 2)) {
+  // What is known about the scene comes from the statistics of frame N - 2 (same parity: its counter block is the one this
+  // frame reuses, so its export is waited for anyway; by now it has long finished).  Deterministic, unlike "whatever has
+  // arrived": the choices below (depth-sort instance, number of slabs, capacity) do not depend on host timing.
+  if (++c->epoch >= (1u << 28)) {   // tag wrap-around: forget every descriptor (once per 2^28 frames)
+    CK(cudaMemsetAsync(c->b.scan_desc, 0, ((size_t)c->n / scan_tile_items() + 3) * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.dsort_desc, 0, (size_t)4 * c->dsort_tiles_cap * 256 * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.sort_desc, 0, (size_t)c->sort_passes_cap * c->sort_tiles_cap * 256 * 8, c->stream));
+    CK(cudaMemsetAsync(c->b.bin_desc, 0, (size_t)c->bin_chunks_cap * 8, c->stream));
+    c->epoch = 1;
+  }
+  const int ci = (int)(c->epoch & 1u);
+  if (c->cnt_pending[ci]) {
+    CK(cudaEventSynchronize(c->ev_cnt[ci])); c->cnt_pending[ci] = false;
+    const Counters& h2 = *c->h_cnt2[ci];
+    c->nv_hint = h2.n_visible;
+    if (!h2.overflow && h2.n_tests) {
+      tgs_ctx::SlabCtl& sc = c->slab_ctl[c->hist_cls[ci]];
+      sc.tests = h2.n_tests;
+      const float ratio = (float)h2.n_pairs / (float)h2.n_tests;
+      if (c->hist_slabs[ci] == 1) sc.p1 = ratio;
+      else if (c->hist_slabs[ci] == 2) {
+        sc.p2 = ratio;
+      }
+    }
+    // grow the automatic capacity when a frame came close to it (the slabs' lists are never longer than the tests)
+    if (!c->prm.max_pairs && (h2.n_pairs > c->max_pairs / 2 || h2.n_tests > c->max_pairs)) {
       unsigned long long want = (unsigned long long)c->max_pairs * 2ull;
       if (want > (1ull << 30) - 1) want = (1ull << 30) - 1;
       if (int r = alloc_pair_buffers(c, (uint32_t)want, tile_passes)) return r;
@@ -469,18 +509,38 @@ static int render_impl(tgs_ctx* c, int mode) {
   fc.all_tiles = !(ftype == TGS_FRAME_S && c->prm.enable_sr && !c->force_all);
   fc.exact_tiles = c->prm.exact_tiles ? 1 : 0;
   fc.n_tiles = c->TX * c->TY;
-  if (++c->epoch >= (1u << 30)) {   // tag wrap-around: forget every descriptor (once per 2^30 frames)
-    CK(cudaMemsetAsync(c->b.scan_desc, 0, ((size_t)c->n / scan_tile_items() + 3) * 8, c->stream));
-    CK(cudaMemsetAsync(c->b.dsort_desc, 0, (size_t)4 * c->dsort_tiles_cap * 256 * 8, c->stream));
-    CK(cudaMemsetAsync(c->b.sort_desc, 0, (size_t)c->sort_passes_cap * c->sort_tiles_cap * 256 * 8, c->stream));
-    CK(cudaMemsetAsync(c->b.bin_desc, 0, (size_t)c->bin_chunks_cap * 8, c->stream));
-    c->epoch = 1;
-  }
   fc.epoch = c->epoch;
-  const int ci = (int)(c->epoch & 1u);
-  c->b.counters = c->counters2[ci];
+  // front-to-back slabs: explicit, or automatic from the size of a recent frame's test space -- small frames
+  // are launch bound and stay in one piece
+  {
+    int ns = c->prm.depth_slabs;
+    if (ns == 0) {
+      // Two pieces pay where most tiles finish inside the first one: then the second piece bins and sorts next to nothing.
+      // Where the tiles stay alive (thin surfaces, clouds with gaps) the second piece only adds launches and the parking
+      // of the pixel states.  Measured, not guessed: pairs per test of the latest one-piece and two-piece frames of this
+      // class, the other variant re-probed every 32 frames; small frames are launch bound and stay in one piece.
+      tgs_ctx::SlabCtl& sc = c->slab_ctl[ftype == TGS_FRAME_S ? 1 : 0];
+      if (sc.tests < 2000000u || sc.p1 < 0.0f) ns = 1;
+      else if (sc.p2 < 0.0f) ns = 2;
+      else {
+        const int prefer = sc.p2 < 0.5f * sc.p1 ? 2 : 1;
+        ns = prefer;
+        if (++sc.since_probe >= 32) { ns = 3 - prefer; sc.since_probe = 0; }
+      }
+    }
+    static const uint32_t def_split[TGS_MAX_SLABS + 1][3] = {{0, 0, 0}, {0, 0, 0}, {256, 0, 0}, {160, 448, 0}, {96, 256, 512}};
+    fc.n_slabs = ns;
+    fc.slab_bound[0] = 0;
+    for (int i = 1; i < ns; ++i) {
+      uint32_t v = c->prm.slab_split[i - 1] ? c->prm.slab_split[i - 1] : def_split[ns][i - 1];
+      if (v < fc.slab_bound[i - 1]) v = fc.slab_bound[i - 1];
+      fc.slab_bound[i] = v;
+    }
+    for (int i = ns; i <= TGS_MAX_SLABS; ++i) fc.slab_bound[i] = 1024;
+  }
+  c->b.counters = c->counters2[ci];          // ci = parity of this frame's epoch (computed above)
+  c->h_counters = c->h_cnt2[ci];
   c->b.F_key = c->F_base + 4 * (ftype == TGS_FRAME_R ? ci : c->F_idx);   // R: reset + built here (k_frustum, third stream); P / S: read
-  if (c->cnt_pending[ci]) { CK(cudaStreamWaitEvent(c->stream, c->ev_cnt[ci], 0)); c->cnt_pending[ci] = false; }   // its last copy to the host
 
   DevBuffers& b = c->b;
   cudaStream_t s = c->stream;
@@ -495,9 +555,9 @@ static int render_impl(tgs_ctx* c, int mode) {
   const float* prior_image = c->priors_valid ? b.image[c->prior_idx] : nullptr;
   uint8_t* rendered_next = builds_priors ? b.rendered_next : nullptr;
   uint8_t* rendered_marks = chains ? b.rendered : rendered_next;
-  int ev = 0;
-  auto mark = [&]() { if (c->timing) cudaEventRecord(c->ev_stage[ev], s); ++ev; };
-  mark();                                                                      // 0: init, A1 warp, A2 fill + correspondence
+  c->n_ev = 0;
+  auto mark = [&](int stage) { if (c->timing && c->n_ev < tgs_ctx::MAX_EV) { cudaEventRecord(c->ev_stage[c->n_ev], s); c->ev_tag[c->n_ev++] = stage; } };
+  mark(0);                                                                     // 0: init, A1 warp, A2 fill + correspondence
   launch_frame_init(s, fc, b, ftype == TGS_FRAME_R, rendered_next);
   if (ftype == TGS_FRAME_S) launch_warp(s, fc, b, b.depth[c->prior_idx], b.sigma[c->prior_idx]);          // A1
   // A2 (depth fill, correspondence, T^um) is only needed by the tile selection: it runs beside the preprocess.
@@ -507,7 +567,7 @@ static int render_impl(tgs_ctx* c, int mode) {
     if (fork) { CK(cudaEventRecord(c->ev_fork2, s)); CK(cudaStreamWaitEvent(c->side, c->ev_fork2, 0)); }
     launch_fill_corr(fork ? c->side : s, fc, b);                                                           // A2
   }
-  mark();                                                                      // 1: A3 preprocess, A4 selection
+  mark(1);                                                                     // 1: A3 preprocess, A4 selection
   if (c->post2_pending) { CK(cudaStreamWaitEvent(s, c->ev_post2, 0)); c->post2_pending = false; }          // k_frustum of the previous frame
   launch_preprocess(s, fc, b, c->num_sms);                                                                 // A3 (+ small-rect T^oc) + visible list
   if (ftype == TGS_FRAME_S) {
@@ -527,26 +587,34 @@ static int render_impl(tgs_ctx* c, int mode) {
     launch_colour_all(c->side2, fc, b, c->num_sms);
     CK(cudaEventRecord(c->ev_join, c->side2));
   }
-  mark();                                                                      // 2: A6 level 1
+  mark(2);                                                                     // 2: A6 level 1
   const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
                                   &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, c->nv_hint < 1000000u);   // visible Gaussians by depth
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
-  mark();                                                                      // 3: A5 pairs
+  // ---- A5-A9, slab by slab (one slab: the plain pipeline)
   c->h_ovf[ci] = 0;
-  launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms, c->h_ovf + ci);                             // tests -> pairs, counts
-  CK(cudaEventRecord(c->ev_bin, s));
-  c->bin_pending = true; c->bin_slot = ci;
-  mark();                                                                      // 4: A5 colours (production: third stream, beside the depth sort)
-  if (!early_colour) launch_colour_all(s, fc, b, c->num_sms);                                             // stage timing: the production kernel, in line
-  mark();                                                                      // 5: A6 level 2 + A7
-  const int sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs, tile_bits, b.sort_hist + 4 * 256,
-                                 b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_sort[4], &b.counters->error, fc.epoch, c->num_sms, false,
-                                 b.ranges);                                                                // pairs by tile + A7 in the last pass
-  mark();                                                                      // 6: A8 + A9
-  if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
-  if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
-  launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_marks, c->num_sms, c->count_interactions);
-  mark();                                                                      // 7: post
+  int sorted = 0;
+  for (int k = 0; k < fc.n_slabs; ++k) {
+    mark(3);                                                                   // 3: A5 pairs
+    launch_bin(s, fc, b, dsorted, c->bin_chunks_cap, c->num_sms, c->h_ovf + ci, k);                        // tests -> pairs, counts
+    if (k == 0) {
+      CK(cudaEventRecord(c->ev_bin, s));
+      c->bin_pending = true; c->bin_slot = ci;
+      mark(4);                                                                 // 4: A5 colours (production: third stream, beside the depth sort)
+      if (!early_colour) launch_colour_all(s, fc, b, c->num_sms);                                         // stage timing: the production kernel, in line
+    }
+    mark(5);                                                                   // 5: A6 level 2 + A7
+    sorted = launch_sort(s, b.keys, b.vals, &b.counters->n_pairs_slab[k], tile_bits, b.sort_hist + (1 + k) * 4 * 256,
+                         b.sort_desc, c->sort_tiles_cap, &b.counters->ticket_tsort[k][0], &b.counters->error, fc.epoch * 4u + (uint32_t)k, c->num_sms, false,
+                         b.ranges);                                                                        // pairs by tile + A7 in the last pass
+    mark(6);                                                                   // 6: A8 + A9
+    if (k == 0) {
+      if (fork) CK(cudaStreamWaitEvent(s, c->ev_join, 0));
+      if (c->copy_pending[out_idx]) { CK(cudaStreamWaitEvent(s, c->ev_copy[out_idx], 0)); c->copy_pending[out_idx] = false; }   // an asynchronous read of this buffer
+    }
+    launch_blend(s, fc, b, sorted, out_idx, prior_image, rendered_marks, c->num_sms, c->count_interactions, k);
+  }
+  mark(7);                                                                     // 7: post
   if (builds_priors && !fork) launch_frustum(s, fc, b, b.cvals[dsorted], rendered_next, ftype == TGS_FRAME_R);      // F_min/F_max (L109)
   if (fork) {
     // post-processing on the third stream, beside the start of the next frame: F / |G_rendered| over the visible list
@@ -563,8 +631,10 @@ static int render_impl(tgs_ctx* c, int mode) {
     c->cnt_pending[ci] = true;
   } else {
     launch_export_counters(s, b, c->h_counters);
-    mark();                                                                    // 8
+    mark(8);                                                                   // end
     CK(cudaEventRecord(c->ev_done, s));
+    CK(cudaEventRecord(c->ev_cnt[ci], s));
+    c->cnt_pending[ci] = true;
   }
   CK(cudaGetLastError());
   // ---- A10: prior commit (pointer swap) and scheduler counters
@@ -580,7 +650,8 @@ static int render_impl(tgs_ctx* c, int mode) {
   if (ftype == TGS_FRAME_R) { c->sched.since_R = 0; c->sched.since_ref = 0; c->sched.force_P = 0; }
   else if (ftype == TGS_FRAME_P) { c->sched.since_ref = 0; c->sched.force_P = 0; }
   ++c->sched.since_R; ++c->sched.since_ref;
-  c->last_ftype = ftype; c->last_n_tiles = (uint32_t)fc.n_tiles;
+  c->last_ftype = ftype; c->last_n_tiles = (uint32_t)fc.n_tiles; c->last_n_slabs = fc.n_slabs;
+  c->hist_cls[ci] = ftype == TGS_FRAME_S ? 1 : 0; c->hist_slabs[ci] = fc.n_slabs;
   c->have_frame = true;
   return TGS_OK;
 }
@@ -630,10 +701,16 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
   out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions; out->n_blended = h.n_blended; out->n_pixel_slots = h.n_slots;
   out->device_bytes = c->device_bytes;
-  out->n_tests = h.n_tests; out->launches_total = g_tgs_launches;
+  out->n_tests = h.n_tests; out->n_pairs_consumed = h.n_consumed; out->launches_total = g_tgs_launches;
+  out->n_slabs = (uint32_t)c->last_n_slabs;
+  for (int i = 0; i < TGS_MAX_SLABS; ++i) { out->n_pairs_slab[i] = h.n_pairs_slab[i]; out->n_finished_slab[i] = h.n_finished[i]; }
   if (c->timing) {
-    for (int i = 0; i < 8; ++i) cudaEventElapsedTime(&out->ms_stage[i], c->ev_stage[i], c->ev_stage[i + 1]);
-    cudaEventElapsedTime(&out->ms_total, c->ev_stage[0], c->ev_stage[8]);
+    for (int i = 0; i + 1 < c->n_ev; ++i) {
+      float ms = 0.0f;
+      cudaEventElapsedTime(&ms, c->ev_stage[i], c->ev_stage[i + 1]);
+      if (c->ev_tag[i] >= 0 && c->ev_tag[i] < 8) out->ms_stage[c->ev_tag[i]] += ms;
+    }
+    if (c->n_ev >= 2) cudaEventElapsedTime(&out->ms_total, c->ev_stage[0], c->ev_stage[c->n_ev - 1]);
   }
   if (h.error) { snprintf(c->err, sizeof(c->err), "device watchdog: look-back stalled (code %u)", h.error); return TGS_E_CUDA; }
   if (h.overflow) return TGS_E_CAPACITY;
@@ -657,7 +734,7 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
   if (name == "keys" || name == "vals") {
     if (!c->have_frame) return TGS_E_INVALID_ARG;
     CK(cudaEventSynchronize(c->ev_done));
-    const size_t P = c->h_counters->n_pairs;
+    const size_t P = c->h_counters->n_pairs_slab[c->last_n_slabs - 1];          // the list of the last slab (one slab: the whole list)
     if (name == "keys") {
       if (!c->keys64 && P) { if (int r = dev_alloc(c, &c->keys64, (size_t)c->max_pairs, c->allocs_pairs)) return r; }
       launch_keys64(c->stream, c->b, c->sorted_idx, (uint32_t)P, c->keys64);
@@ -684,7 +761,7 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
     if (!c->have_frame) return TGS_E_INVALID_ARG;
     CK(cudaEventSynchronize(c->ev_done));
     if (c->h_counters->overflow) return TGS_E_CAPACITY;
-    launch_count_pairs(c->stream, c->b, c->sorted_idx, (uint32_t)c->h_counters->n_pairs, (uint32_t)N);
+    launch_count_pairs(c->stream, c->b, c->sorted_idx, (uint32_t)c->h_counters->n_pairs_slab[c->last_n_slabs - 1], (uint32_t)N);
     src = b.tiles_touched; have = N * 4;
   }
   else if (name == "ranges") {

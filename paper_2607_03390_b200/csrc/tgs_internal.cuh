@@ -8,6 +8,7 @@
 #include "../../include/tgs.h"
 
 #define TGS_TILE 16
+#define TGS_MAX_SLABS 4
 #define TGS_INVALID_BITS 0x7f61b1e6u /* bits of 3.0e38f */
 
 // ------------------------------------------------------------------ per-frame constants (kernel argument)
@@ -43,7 +44,12 @@ struct FrameConst {
   int do_afc, do_toc, do_tgb, all_tiles;
   int exact_tiles;          // R39
   int n_tiles;
-  uint32_t epoch;           // frame number (1 .. 2^30 - 1): tag of the look-back descriptors
+  uint32_t epoch;           // frame number (1 .. 2^28 - 1): tag of the look-back descriptors (x 4 + slab for pairs)
+  // Front-to-back slabs: the flat test space of the depth-sorted visible Gaussians is cut into n_slabs
+  // consecutive ranges of chunks; slab k is binned, sorted and blended before slab k + 1 is binned, and tiles whose pixels
+  // have all stopped are dropped from the binning of the later slabs.  slab_bound[k] / 1024 = share of the chunks before slab k.
+  int n_slabs;              // 1 .. TGS_MAX_SLABS
+  uint32_t slab_bound[TGS_MAX_SLABS + 1];
 };
 
 // ------------------------------------------------------------------ device counters (one block, zeroed per frame)
@@ -58,15 +64,22 @@ struct Counters {
   uint32_t n_nv_queue;      // newly visible Gaussians queued for the cooperative T^oc marking
   uint32_t n_oc_marked;     // tiles whose T^oc bit is set
   // work tickets of the persistent kernels
-  uint32_t ticket_pre, ticket_scan, ticket_bin, ticket_blend;
-  uint32_t ticket_sort[8];  // [0..3] depth sort, [4..7] tile sort
+  uint32_t ticket_pre, ticket_scan;
+  uint32_t ticket_sort[4];  // depth sort, one per digit
+  // per slab
+  uint32_t ticket_bin[TGS_MAX_SLABS], ticket_blend[TGS_MAX_SLABS];
+  uint32_t ticket_tsort[TGS_MAX_SLABS][4];   // tile sort, one per slab and digit
+  uint32_t n_pairs_slab[TGS_MAX_SLABS];      // pairs of a slab = length of its sort
+  uint32_t n_live_after[TGS_MAX_SLABS];      // tiles that parked their pixel states at the end of a slab's blend
+  uint32_t n_finished[TGS_MAX_SLABS];        // selected tiles finished (written) by a slab's blend before the last slab
   uint32_t pre_done;        // CTAs of k_preprocess that have finished
   unsigned long long area_sum;         // same as n_tests, accumulated in 64 bits by k_preprocess (overflow check)
   unsigned long long n_interactions;   // L (only when interaction counting is on)
   unsigned long long n_blended;        // interactions that passed alpha >= 1/255 and were composited (counting on)
   unsigned long long n_slots;          // pixel slots the blend loop issued: warp iterations x pixels per warp (counting on)
+  unsigned long long n_consumed;       // pairs the blend reached before their tile was finished, in whole batches (counting on)
 };
-static_assert(sizeof(Counters) == 152, "Counters layout");
+static_assert(sizeof(Counters) % 8 == 0 && sizeof(Counters) <= 512, "Counters layout (k_export_counters copies it with 128 threads)");
 
 // ------------------------------------------------------------------ device buffers of a context
 struct DevBuffers {
@@ -101,7 +114,7 @@ struct DevBuffers {
   // pairs
   uint32_t* keys[2] = {nullptr, nullptr};    // [max_pairs] tile id of a pair
   uint32_t* vals[2] = {nullptr, nullptr};    // [max_pairs] Gaussian index of a pair
-  uint32_t* sort_hist = nullptr;      // [2][4][256]: depth sort, tile sort
+  uint32_t* sort_hist = nullptr;      // [1 + TGS_MAX_SLABS][4][256]: depth sort, tile sort of each slab
   uint64_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors (epoch-tagged)
   uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
   uint64_t* scan_desc = nullptr;      // look-back descriptors of k_scan_area
@@ -109,7 +122,10 @@ struct DevBuffers {
   // tiles
   uint32_t* tile_flags = nullptr;     // [T] bit0 oc, bit1 um
   uint8_t* tile_mask = nullptr;       // [T] bit0 oc, bit1 um, bit2 selected
-  uint32_t* sel_bits = nullptr;       // [ceil(T/32)]
+  uint32_t* sel_bits = nullptr;       // [ceil(T/32)] T_sel
+  uint32_t* live_bits = nullptr;      // [ceil(T/32)] selected tiles whose pixels have not all stopped yet (slabs)
+  uint32_t* live_sat = nullptr;       // [(TY + 1)(TX + 1)] summed-area table of live_bits (k_live_sat, before the binning of a later slab)
+  float* pix_state = nullptr;         // [T][7][256] pixel states of the tiles that stay live from one slab to the next
   uint32_t* tile_order = nullptr;     // [T] selected tiles first, then the others
   uint2* ranges = nullptr;            // [T] {start,end}
   // images
@@ -160,8 +176,10 @@ void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t
 void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host);
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F);
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
+// k_scan_area (slab 0 only) + k_bin of one slab.  host_overflow: pinned host word, zero-copy stores: 1 = the pair buffers
+// overflowed, 2 (from k_scan_area) = the tests exceed the capacity, so an overflow cannot be ruled out before the frame ends
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms,
-                uint32_t* host_overflow);   // pinned host word: set to 1 (zero-copy store) when the pair buffers overflow
+                uint32_t* host_overflow, int slab);
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms);
 // Sorts *n_ptr items on the low key_bits bits of the uint32 key; returns the index (0/1) of the result buffers.
 int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2], const uint32_t* n_ptr, int key_bits,
@@ -171,7 +189,7 @@ void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, ui
 void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n_pairs, uint32_t n);   // test-only
 void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out);   // test-only: {~start, end} -> {start, end}
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
-                  const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions);
+                  const float* prior_image, uint8_t* rendered_next, int num_sms, bool count_interactions, int slab);
 uint32_t sort_tile_items();
 uint32_t scan_tile_items();
 uint32_t bin_chunk_items();

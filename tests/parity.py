@@ -28,24 +28,33 @@ MODE_G = {"full": tgs.FULL, "pseudo": tgs.PSEUDO_REF, "temporal": tgs.TEMPORAL, 
 MODE_O = {"full": ora.FULL, "pseudo": ora.PSEUDO_REF, "temporal": ora.TEMPORAL, "auto": ora.AUTO}
 
 
+GPU_ONLY_PARAMS = ("max_pairs", "depth_slabs", "slab_split")     # how the CUDA path organises its work, not what it computes
+
+
 def make_pair(sc, params=None):
+    """A CUDA context and an oracle on the same scene and parameters.  depth_slabs defaults to 1 here (one piece: the pair
+    lists are the complete lists of L61 and are compared bit for bit); the slab tests set it explicitly."""
     g = tgs.Context(0)
     o = Oracle()
     g.load_scene(sc)
     o.load_scene(sc)
-    if params:
-        pg, po = g.default_params(), o.default_params()
-        for k, v in params.items():
-            if k == "bg":
-                for i in range(3):
-                    pg.bg[i] = v[i]
-                    po.bg[i] = v[i]
-            else:
-                setattr(pg, k, v)
-                if k != "max_pairs":
-                    setattr(po, k, v)
-        g.set_params(pg)
-        o.set_params(po)
+    params = dict(params or {})
+    params.setdefault("depth_slabs", 1)
+    pg, po = g.default_params(), o.default_params()
+    for k, v in params.items():
+        if k == "bg":
+            for i in range(3):
+                pg.bg[i] = v[i]
+                po.bg[i] = v[i]
+        elif k == "slab_split":
+            for i, x in enumerate(v):
+                pg.slab_split[i] = x
+        else:
+            setattr(pg, k, v)
+            if k not in GPU_ONLY_PARAMS:
+                setattr(po, k, v)
+    g.set_params(pg)
+    o.set_params(po)
     return g, o
 
 
@@ -63,7 +72,7 @@ def bits(a):
     return np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
 
 
-def compare_records(g, o, n):
+def compare_records(g, o, n, pairs=True):
     rec = o.get("records")
     fl_g = g.debug_get("rec_flags")
     assert np.array_equal(fl_g, rec["flags"]), f"flags differ at {np.nonzero(fl_g != rec['flags'])[0][:10]}"
@@ -77,9 +86,10 @@ def compare_records(g, o, n):
         assert np.array_equal(bits(conic[vis, j]), bits(rec[name][vis])), name
     for j, name in enumerate(("x_lo", "x_hi", "y_lo", "y_hi")):
         assert np.array_equal(rect[vis, j], rec[name][vis]), name
-    tt = g.debug_get("tiles_touched")
-    assert np.array_equal(tt, rec["tiles_touched"])
-    col = tt > 0
+    if pairs:
+        tt = g.debug_get("tiles_touched")
+        assert np.array_equal(tt, rec["tiles_touched"])
+    col = rec["tiles_touched"] > 0
     rgb = g.debug_get("rec_rgb").reshape(n, 4)[:, :3]
     ref = np.stack([rec["r"], rec["g"], rec["b"]], 1)
     np.testing.assert_allclose(rgb[col], ref[col], atol=2e-5)
@@ -147,9 +157,11 @@ STAT_KEYS = ("frame_type", "n_total", "n_near", "n_afc", "n_toc", "n_degenerate"
              "n_pairs", "n_tiles", "n_sel_oc", "n_sel_um", "n_sel")
 
 
-def compare_stats(g, o):
+def compare_stats(g, o, pairs=True):
     sg, so = g.get_stats(), o.stats()
     for k in STAT_KEYS:
+        if k == "n_pairs" and not pairs:
+            continue
         assert sg[k] == so[k], (k, sg[k], so[k])
     return sg, so
 
@@ -170,6 +182,30 @@ def compare_frame(g, o, n, ftype, check_rendered=True, label=None, **tol):
         out["rendered_diff"] = compare_rendered(g, o)
         out["rendered"] = int(so["n_rendered"])
     out.update(frame="RPS"[ftype], label=label, n_pairs=int(sg["n_pairs"]), n_sel=int(sg["n_sel"]), n_tiles=int(sg["n_tiles"]))
+    REPORT.append(out)
+    print("[parity] " + " ".join(f"{k}={v:.3g}" if isinstance(v, float) else f"{k}={v}" for k, v in out.items()))
+    path = os.environ.get("TGS_PARITY_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps(out) + "\n")
+    return sg, so, out
+
+
+def compare_frame_slabs(g, o, n, ftype, label=None, **tol):
+    """A frame rendered in several front-to-back slabs (tgs_params.depth_slabs > 1): everything of compare_frame except the
+    pair lists, which lack the pairs of tiles that had finished in an earlier slab.  That no NEEDED pair is missing is
+    what the image, depth, sigma and G_rendered comparisons check; the counts must add up."""
+    sg, so = compare_stats(g, o, pairs=False)
+    assert sg["n_slabs"] > 1 and sum(sg["n_pairs_slab"][: sg["n_slabs"]]) == sg["n_pairs"] <= so["n_pairs"]
+    if ftype == ora.FRAME_S:
+        compare_temporal_buffers(g, o)
+    assert np.array_equal(g.read_tile_mask(), o.read_tile_mask())
+    compare_records(g, o, n, pairs=False)
+    out = compare_outputs(g, o, ftype, **tol)
+    if ftype != ora.FRAME_S:
+        out["rendered_diff"] = compare_rendered(g, o)
+    out.update(frame="RPS"[ftype], label=label, n_pairs=int(sg["n_pairs"]), n_pairs_oracle=int(so["n_pairs"]), n_slabs=int(sg["n_slabs"]),
+               n_sel=int(sg["n_sel"]), n_tiles=int(sg["n_tiles"]))
     REPORT.append(out)
     print("[parity] " + " ".join(f"{k}={v:.3g}" if isinstance(v, float) else f"{k}={v}" for k, v in out.items()))
     path = os.environ.get("TGS_PARITY_REPORT")

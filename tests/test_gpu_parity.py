@@ -681,3 +681,62 @@ def test_sanitizer_stream_smoke_sized():
         assert np.quantile(err, 0.999) < 2e-3 or f > 0        # frame 0 shares nothing with earlier frames: strict
         assert np.quantile(err, 0.99) < 2e-3
     g.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ front-to-back slabs
+@pytest.mark.parametrize("slabs,split", [(2, (0, 0, 0)), (3, (0, 0, 0)), (4, (0, 0, 0)), (3, (8, 40, 0)), (2, (1000, 0, 0)), (4, (1, 2, 3))])
+def test_depth_slabs_outputs_match_oracle_and_single_pass(slabs, split):
+    """tgs_params.depth_slabs: binning, sorting and blending in front-to-back pieces, tiles that have
+    finished receive no more pairs.  R, S and P frames of two scenes (opaque sheets: most tiles finish in the first piece;
+    a sparse cloud: most tiles stay alive through every piece, many of them in the blend's sparse mode) against the oracle
+    -- every output except the pair lists -- and against the same frames rendered in one piece."""
+    P = _p()
+    for cfg, kw, scale in ((5, dict(n=60_000, frames=12, width=320, height=180), 6.0), (1, dict(n=30_000, frames=4, width=333, height=207), 2.0)):
+        sc = make_config(cfg, **kw)
+        if cfg == 5:
+            sc.scales[:, :2] *= scale
+        else:
+            sc.scales *= scale
+        g, o = P.make_pair(sc, {"depth_slabs": slabs, "slab_split": split, "bg": (0.1, 0.2, 0.3)})
+        g1, _ = P.make_pair(sc, {"bg": (0.1, 0.2, 0.3)})
+        for f, mode in ((0, "full"), (1, "temporal"), (2, "temporal"), (3, "pseudo")):
+            if f:
+                P.inject_priors(g, o); P.inject_priors(g1, o)
+            for c in (g, g1, o):
+                c.set_camera(sc.poses[f], sc.camera)
+            g.render(P.MODE_G[mode]); g1.render(P.MODE_G[mode]); ft = o.render(P.MODE_O[mode])
+            sg, so, out = P.compare_frame_slabs(g, o, sc.n, ft, label=f"slabs={slabs} split={split} cfg={cfg}")
+            s1 = g1.get_stats()
+            assert s1["n_slabs"] == 1 and s1["n_pairs"] == so["n_pairs"] and sg["n_slabs"] == slabs
+            assert np.abs(g.read_image() - g1.read_image()).max() <= 2e-5
+            d, sgm = g.read_depth(); d1, sgm1 = g1.read_depth()
+            assert np.array_equal(d < 1e38, d1 < 1e38)
+            assert np.array_equal(g.debug_get("rendered"), g1.debug_get("rendered"))
+        if cfg == 5 and split == (0, 0, 0):
+            assert sg["n_pairs"] < so["n_pairs"]          # finished tiles really dropped pairs
+
+
+def test_depth_slabs_auto_full_size_config3_and_5():
+    """The launch configuration bench.py times (depth_slabs = 0: automatic) at full size.  The library learns from its own
+    statistics (two frames late) whether two pieces drop enough pairs: two reference frames in one piece, two probing
+    two pieces, then the decision (pairs per test halved or not), which must be stable.  On the poses used here (config 3
+    from inside the dense core, config 5's sheets) two pieces are kept.  A two-piece reference frame and a two-piece
+    TemporalGS frame, every output against the oracle."""
+    P = _p()
+    tgs = _tgs()
+    for cfg, f0 in ((3, 45), (5, 0)):
+        sc = make_config(cfg, frames=f0 + 4)
+        g, o = P.make_pair(sc, {"depth_slabs": 0})
+        g.set_camera(sc.poses[f0], sc.camera); o.set_camera(sc.poses[f0], sc.camera)
+        o.render(ora.FULL)
+        used, pairs = [], []
+        for _ in range(8):
+            g.render(tgs.FULL); st = g.get_stats(); used.append(st["n_slabs"]); pairs.append(st["n_pairs"])
+        assert used[:4] == [1, 1, 2, 2] and used[4:] == [2] * 4, (used, pairs)
+        assert pairs[2] < 0.5 * pairs[0] and pairs[0] == o.stats()["n_pairs"]
+        sg, so, out = P.compare_frame_slabs(g, o, sc.n, ora.FRAME_R, label=f"config {cfg} full size, auto slabs", **FULL_SIZE_BOUNDS[cfg])
+        P.inject_priors(g, o)
+        g.set_camera(sc.poses[f0 + 2], sc.camera); o.set_camera(sc.poses[f0 + 2], sc.camera)
+        p = g.default_params(); p.depth_slabs = 2; g.set_params(p)
+        g.render(tgs.TEMPORAL); o.render(ora.TEMPORAL)
+        P.compare_frame_slabs(g, o, sc.n, ora.FRAME_S, label=f"config {cfg} full size, two slabs", **FULL_SIZE_BOUNDS[cfg])
