@@ -189,12 +189,14 @@ def summarise(lst):
 class Harness:
     """One scene on one GPU: timed frame loops (CUDA events on the context's stream), the per-stage pass, quality."""
 
-    def __init__(self, tgs, torch, sc, local, world, warmup):
+    def __init__(self, tgs, torch, sc, local, world, warmup, depth_slabs=0):
         self.tgs, self.torch, self.sc, self.world, self.W = tgs, torch, sc, world, warmup
         self.stream = torch.cuda.Stream()
         self.ctx = tgs.Context(local, self.stream.cuda_stream)
         self.ctx.load_scene(sc)                         # scene resident in HBM before any timed region
         self.local = local
+        if depth_slabs:
+            p = self.ctx.default_params(); p.depth_slabs = depth_slabs; self.ctx.set_params(p)
 
     def barrier(self):
         self.torch.cuda.synchronize()
@@ -317,7 +319,7 @@ def run_ours(args):
     sc = make_config(args.config, n=args.n, frames=None)
     cam = sc.camera
     K, W = args.steps, args.warmup
-    h = Harness(tgs, torch, sc, local, world, W)
+    h = Harness(tgs, torch, sc, local, world, W, args.depth_slabs)
 
     # ---- the headline: K frames of the trajectory, TemporalGS (AUTO); then the same frames end to end
     sampler = ClockSampler(local)
@@ -349,7 +351,7 @@ def run_ours(args):
             if cfg == args.config:
                 continue
             sc2 = make_config(cfg, frames=None)
-            h2 = Harness(tgs, torch, sc2, local, 1, W)
+            h2 = Harness(tgs, torch, sc2, local, 1, W, args.depth_slabs)
             o2, _ = config_summary(h2, hbm_gbs, alu_peak, stage_frames=40, quality_frames=10)
             h2.close()
             o2["workload"] = workload_string(sc2, cfg)
@@ -388,6 +390,7 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_string(sc, args.config),
                    "l2": "scene arrays (>= 700 MB) exceed the 126 MB L2; no explicit flush", "parallelism": "replicas only",
+                   "depth_slabs": "automatic (library default: one or two front-to-back pieces per frame, chosen from its own statistics)" if not args.depth_slabs else args.depth_slabs,
                    "fps_full_render": fps_full, "speedup_vs_full_render": fps_tgs / fps_full,
                    "trajectory": {k: traj[k] for k in ("frames", "fps_tgs", "fps_full", "speedup", "psnr_S_vs_full_dB", "ssim_S_vs_full", "n_sel_frac_S")},
                    "stages": traj["stages"],
@@ -558,6 +561,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the number of Gaussians (debug only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--depth-slabs", type=int, default=0, help="tgs_params.depth_slabs: 0 = automatic (the default of the library), 1..4 = fixed (profiling runs)")
     ap.add_argument("--other-configs", default="2,5,4", help="configs also measured over their whole trajectories ('none' to skip)")
     ap.add_argument("--ablation", action="store_true", help="module ablation and sensitivity table instead of the bench line")
     args = ap.parse_args()

@@ -176,7 +176,8 @@ const char* tgs_last_error(tgs_ctx*);
  * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):
  *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
  * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off"
- *   "count_interactions_on" "count_interactions_off". */
+ *   "count_interactions_on" "count_interactions_off" "redzones_on" (before the scene is loaded: every device buffer allocated
+ *   afterwards is framed by 256-byte guards) "check_redzones" (TGS_OK if no guard has been written to, else TGS_E_CUDA). */
 long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int mem);
 int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);
 int tgs_debug_run_stage(tgs_ctx*, const char* stage);

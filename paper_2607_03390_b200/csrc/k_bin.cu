@@ -22,7 +22,7 @@
 namespace {
 
 constexpr int SCAN_THREADS = 256;
-constexpr int SCAN_IPT = 2;
+constexpr int SCAN_IPT = 2;          // 8 (2048-Gaussian tiles, a shorter look-back) measured slower: +20 us, the gathers of a tile are serial per thread
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 
 constexpr int BIN_THREADS = 128;
@@ -413,25 +413,35 @@ uint32_t scan_tile_items() { return SCAN_TILE; }
 uint32_t bin_chunk_items() { return BIN_CHUNK; }
 
 // Summed-area table of the live tiles, (TY + 1) x (TX + 1) with a zero border: sat[y][x] = live tiles with ty < y, tx < x.
-// One CTA: a thread per tile row (prefix along x), then a thread per column (prefix along y); 8 K entries at 1080p.
+// One CTA: a thread per tile row (prefix along x), then a thread per column (prefix along y); 8 K entries at 1080p, built
+// in shared memory (SMEM = true; grids beyond 48 KB fall back to global memory) and copied out coalesced.
+template <bool SMEM>
 __global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_t* __restrict__ live_bits, uint32_t* __restrict__ sat) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
+  extern __shared__ uint32_t s_sat[];
+  uint32_t* const w = SMEM ? s_sat : sat;
   const int SW = TX + 1;
-  for (int x = threadIdx.x; x <= TX; x += blockDim.x) sat[x] = 0;
+  for (int x = threadIdx.x; x <= TX; x += blockDim.x) w[x] = 0;
   for (int y = threadIdx.x; y < TY; y += blockDim.x) {
-    uint32_t run = 0;
-    sat[(y + 1) * SW] = 0;
+    uint32_t run = 0, word = 0;
+    w[(y + 1) * SW] = 0;
     for (int x = 0; x < TX; ++x) {
       const int t = y * TX + x;
-      run += (live_bits[t >> 5] >> (t & 31)) & 1u;
-      sat[(y + 1) * SW + x + 1] = run;
+      if (x == 0 || (t & 31) == 0) word = live_bits[t >> 5];
+      run += (word >> (t & 31)) & 1u;
+      w[(y + 1) * SW + x + 1] = run;
     }
   }
   __syncthreads();
   for (int x = threadIdx.x + 1; x <= TX; x += blockDim.x) {
     uint32_t run = 0;
-    for (int y = 1; y <= TY; ++y) { run += sat[y * SW + x]; sat[y * SW + x] = run; }
+    for (int y = 1; y <= TY; ++y) { run += w[y * SW + x]; w[y * SW + x] = run; }
+  }
+  if (SMEM) {
+    __syncthreads();
+    const int n = SW * (TY + 1);
+    for (int i = threadIdx.x; i < n; i += blockDim.x) sat[i] = s_sat[i];
   }
 }
 
@@ -446,7 +456,11 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
     TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
                                                         b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
   }
-  if (slab > 0) TGS_LAUNCH((k_live_sat), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
+  if (slab > 0) {
+    const size_t sat_bytes = (size_t)(fc.cam.TX + 1) * (fc.cam.TY + 1) * sizeof(uint32_t);
+    if (sat_bytes <= 48 * 1024) TGS_LAUNCH((k_live_sat<true>), 1, 1024, sat_bytes, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
+    else TGS_LAUNCH((k_live_sat<false>), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
+  }
   uint32_t* hist = b.sort_hist + (1 + slab) * 4 * 256;
   if (fc.n_tiles <= 65536)
     TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,

@@ -147,6 +147,11 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
   const bool last = slab == fc.n_slabs - 1;
   const uint32_t n_work = slab == 0 ? (uint32_t)fc.n_tiles : n_sel;      // the stitched tiles are done with slab 0
   uint32_t zero_tile = 0xffffffffu;                                       // (thread 0) tile whose range is to be cleared for the next slab
+  if (slab > 0) {                                                         // every selected tile finished in the earlier slabs: nothing to do
+    uint32_t fin = 0;
+    for (int j = 0; j < slab; ++j) fin += counters->n_finished[j];
+    if (fin >= n_sel) return;
+  }
   while (true) {
     __syncthreads();
     if (tid == 0) {

@@ -54,6 +54,9 @@ struct tgs_ctx {
   uint64_t device_bytes = 0;
   DevBuffers b;
   std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
+  struct Guard { unsigned char* base; size_t bytes, body; };
+  std::vector<Guard> guards;           // red zones (test-only)
+  bool redzones = false;
   // stats
   Counters* h_counters = nullptr;      // pinned: the block of the last rendered frame (= h_cnt2[parity])
   Counters* h_cnt2[2] = {nullptr, nullptr};   // pinned, by frame parity: frame N - 2's statistics are complete and unchanged when frame N is set up
@@ -98,21 +101,59 @@ struct tgs_ctx {
 
 namespace {
 
+// Every device buffer of a context comes from here.  With red zones on (tgs_debug_run_stage("redzones_on") before the
+// scene is loaded; test-only) each buffer is framed by two 256-byte guards filled with a pattern, and
+// tgs_debug_run_stage("check_redzones") verifies that no kernel has written outside its buffers -- the stand-in for
+// compute-sanitizer's memcheck, which is closed on this pool (profiles/r2_sanitizers.md).
+constexpr size_t REDZONE = 256;
+constexpr unsigned char REDZONE_BYTE = 0xA5;
 template <typename T>
 int dev_alloc(tgs_ctx* c, T** p, size_t count, std::vector<void*>& list, bool zero = false) {
   *p = nullptr;
   if (!count) count = 1;
-  CK(cudaMalloc((void**)p, count * sizeof(T)));
-  if (zero) CK(cudaMemsetAsync(*p, 0, count * sizeof(T), c->stream));   // look-back descriptors: epoch 0 = never valid
-  list.push_back(*p);
-  c->device_bytes += count * sizeof(T);
+  const size_t bytes = count * sizeof(T), pad = c->redzones ? REDZONE : 0;
+  const size_t body = (bytes + 255) / 256 * 256;                        // the rear guard starts at the next 256-byte boundary
+  unsigned char* base = nullptr;
+  CK(cudaMalloc((void**)&base, pad ? body + 2 * pad : bytes));
+  if (pad) {
+    CK(cudaMemsetAsync(base, REDZONE_BYTE, pad, c->stream));
+    CK(cudaMemsetAsync(base + pad + bytes, REDZONE_BYTE, body - bytes + pad, c->stream));
+    c->guards.push_back({base, bytes, body});
+  }
+  *p = reinterpret_cast<T*>(base + pad);
+  if (zero) CK(cudaMemsetAsync(*p, 0, bytes, c->stream));   // look-back descriptors: epoch 0 = never valid
+  list.push_back(base);
+  c->device_bytes += bytes;
   return TGS_OK;
 }
 
 void free_list(tgs_ctx* c, std::vector<void*>& list) {
-  for (void* p : list) cudaFree(p);
+  for (void* p : list) {
+    cudaFree(p);
+    for (size_t i = 0; i < c->guards.size(); ++i) if (c->guards[i].base == p) { c->guards.erase(c->guards.begin() + (long)i); break; }
+  }
   list.clear();
-  (void)c;
+}
+
+// red zones intact?  0 = yes; otherwise the number of damaged guards (the first one is described in c->err)
+int check_redzones(tgs_ctx* c) {
+  cudaDeviceSynchronize();
+  int bad = 0;
+  std::vector<unsigned char> h;
+  for (const auto& g : c->guards) {
+    const size_t rear = g.body - g.bytes + REDZONE;
+    h.resize(REDZONE + rear);
+    if (cudaMemcpy(h.data(), g.base, REDZONE, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(h.data() + REDZONE, g.base + REDZONE + g.bytes, rear, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    for (size_t i = 0; i < h.size(); ++i)
+      if (h[i] != REDZONE_BYTE) {
+        if (!bad) snprintf(c->err, sizeof(c->err), "red zone of a %zu-byte buffer damaged %s it (offset %zu)", g.bytes, i < REDZONE ? "before" : "behind",
+                           i < REDZONE ? REDZONE - i : i - REDZONE);
+        ++bad;
+        break;
+      }
+  }
+  return bad;
 }
 
 bool finite_all(const float* p, size_t n) {
@@ -140,8 +181,7 @@ int alloc_frame_buffers(tgs_ctx* c) {
   const int T = c->TX * c->TY;
   if (px <= c->px_cap && T <= c->tiles_cap) return TGS_OK;
   cudaStreamSynchronize(c->stream);
-  for (void* p : c->allocs_frame) cudaFree(p);
-  c->allocs_frame.clear();
+  free_list(c, c->allocs_frame);
   c->ranges_dec = nullptr;
   DevBuffers& b = c->b;
   for (int i = 0; i < 3; ++i) {
@@ -169,8 +209,7 @@ int alloc_pair_buffers(tgs_ctx* c, uint32_t max_pairs, int passes) {
   if (passes < c->sort_passes_cap) passes = c->sort_passes_cap;
   c->max_pairs = 0;
   cudaStreamSynchronize(c->stream);
-  for (void* p : c->allocs_pairs) cudaFree(p);
-  c->allocs_pairs.clear();
+  free_list(c, c->allocs_pairs);
   c->keys64 = nullptr;
   DevBuffers& b = c->b;
   for (int i = 0; i < 2; ++i) {
@@ -323,8 +362,7 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
   if (mem == TGS_HOST && (!finite_all(means, 3 * (size_t)n) || !finite_all(scales, 3 * (size_t)n) || !finite_all(quats, 4 * (size_t)n) ||
                           !finite_all(opacity, n) || !finite_all(sh, (size_t)n * K * 3))) return TGS_E_INVALID_ARG;
   CK(cudaStreamSynchronize(c->stream));
-  for (void* p : c->allocs_scene) cudaFree(p);
-  c->allocs_scene.clear();
+  free_list(c, c->allocs_scene);
   DevBuffers& b = c->b;
   c->n = 0;
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
@@ -841,6 +879,14 @@ static int debug_run_stage_impl(tgs_ctx* c, const char* st) {
   if (s == "count_interactions_off") { c->count_interactions = false; return TGS_OK; }
   if (s == "force_all_tiles_on") { c->force_all = 1; return TGS_OK; }
   if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
+  if (s == "redzones_on") {            // takes effect for the buffers allocated from now on: call it before tgs_load_gaussians
+    if (c->n || c->px_cap) return TGS_E_INVALID_ARG;
+    c->redzones = true; return TGS_OK;
+  }
+  if (s == "check_redzones") {
+    const int bad = check_redzones(c);
+    return bad == 0 ? TGS_OK : TGS_E_CUDA;
+  }
   return TGS_E_INVALID_ARG;
 }
 
