@@ -423,14 +423,18 @@ __global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_
   uint32_t* const w = SMEM ? s_sat : sat;
   const int SW = TX + 1;
   for (int x = threadIdx.x; x <= TX; x += blockDim.x) w[x] = 0;
-  for (int y = threadIdx.x; y < TY; y += blockDim.x) {
-    uint32_t run = 0, word = 0;
-    w[(y + 1) * SW] = 0;
-    for (int x = 0; x < TX; ++x) {
-      const int t = y * TX + x;
-      if (x == 0 || (t & 31) == 0) word = live_bits[t >> 5];
-      run += (word >> (t & 31)) & 1u;
-      w[(y + 1) * SW + x + 1] = run;
+  {   // rows: one warp per tile row, 32 tiles per step, prefix by ballot + popc
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int y = wid; y < TY; y += nw) {
+      uint32_t carry = 0;
+      if (lane == 0) w[(y + 1) * SW] = 0;
+      for (int x0 = 0; x0 < TX; x0 += 32) {
+        const int x = x0 + lane, t = y * TX + x;
+        const bool live = x < TX && ((live_bits[t >> 5] >> (t & 31)) & 1u);
+        const uint32_t bal = __ballot_sync(0xffffffffu, live);
+        if (x < TX) w[(y + 1) * SW + x + 1] = carry + __popc(bal & (0xffffffffu >> (31 - lane)));
+        carry += __popc(bal);
+      }
     }
   }
   __syncthreads();
