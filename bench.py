@@ -148,7 +148,7 @@ def stage_rooflines(stats, sc, hbm_gbs, alu_peak):
     cam = sc.camera
     mean = lambda key: float(np.mean([s[key] for s in stats]))
     t = np.mean([s["ms_stage"] for s in stats], axis=0) * 1e-3
-    P, Nv, L, nt = mean("n_pairs"), mean("n_visible"), mean("n_interactions"), mean("n_tests")
+    P, Nv, L, nt = mean("n_pairs"), mean("n_visible"), mean("n_interactions"), mean("n_tests_evaluated")   # tests really evaluated (slabs skip dead tiles)
     ftype = stats[0]["frame_type"]
     T_ = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
     tile_passes = (max(1, int(np.ceil(np.log2(T_)))) + 7) // 8
@@ -181,7 +181,7 @@ def summarise(lst):
     ms = np.mean([s["ms_stage"] for s in lst], axis=0)
     m = lambda key: float(np.mean([s[key] for s in lst]))
     return {"frames": len(lst), "ms_total": m("ms_total"), "ms_stage": {n: float(v) for n, v in zip(STAGE_NAMES, ms)},
-            "n_pairs": m("n_pairs"), "n_tests": m("n_tests"), "n_visible": m("n_visible"),
+            "n_pairs": m("n_pairs"), "n_tests": m("n_tests"), "n_tests_evaluated": m("n_tests_evaluated"), "n_visible": m("n_visible"),
             "n_sel_frac": float(np.mean([s["n_sel"] / s["n_tiles"] for s in lst])),
             "n_interactions": m("n_interactions"), "n_blended": m("n_blended"), "n_pixel_slots": m("n_pixel_slots"), "n_pairs_consumed": m("n_pairs_consumed")}
 

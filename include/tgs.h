@@ -105,6 +105,7 @@ typedef struct {
   uint64_t device_bytes; /* device memory held by the context */
   uint64_t n_tests;      /* (Gaussian, tile) combinations the pair binning examined: sum of the test-rect areas of the visible
                             Gaussians (n_pairs of them passed: tile selected, L123, and reached with alpha >= 1/255, R39) */
+  uint64_t n_tests_evaluated; /* of n_tests, those whose tile was still alive when their slab was binned (= n_tests in one piece) */
   uint64_t n_pairs_consumed; /* pairs the blend reached before their tile was finished (whole batches of 128; counting on): the
                                 rest of each tile's list lies behind saturated pixels and is never read */
   uint32_t n_slabs;          /* pieces this frame was binned / sorted / blended in (tgs_params.depth_slabs) */

@@ -252,6 +252,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
   // aggregates are there, so the look-back does not spin on stragglers (profiles/r1c: 41 % of the warp samples of the
   // unpipelined kernel sat at the barrier behind a polling warp 0).  Passing tests wait in a double-buffered stage.
   uint32_t pend = 0xffffffffu, pend_total = 0, it = 0;
+  uint32_t n_eval = 0;                  // tests whose tile was alive, i.e. that were really evaluated (statistics)
   while (true) {
     __syncthreads();
     if (tid == 0) sm.chunk = atomicAdd(&counters->ticket_bin[slab], 1u);
@@ -312,6 +313,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
             if (G.pad) continue;                                           // no live tile in this Gaussian's rect (later slabs)
             const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
             bool pass = (live_bits[tile >> 5] >> (tile & 31)) & 1u;        // selected (L123) and not yet finished (slabs)
+            n_eval += pass ? 1u : 0u;
             if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
             if (pass) mask |= 1u << k;
             tl[k] = tile; gg[k] = G.g;
@@ -369,6 +371,8 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
   }
   __syncthreads();
   for (int i = tid; i < NH * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
+  n_eval = __reduce_add_sync(0xffffffffu, n_eval);
+  if (lane == 0 && n_eval) atomicAdd(&counters->n_tests_eval, (unsigned long long)n_eval);
 }
 
 // ================================================================== A5c: SH -> RGB (L61 "color c_i"; R5)

@@ -739,7 +739,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
   out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions; out->n_blended = h.n_blended; out->n_pixel_slots = h.n_slots;
   out->device_bytes = c->device_bytes;
-  out->n_tests = h.n_tests; out->n_pairs_consumed = h.n_consumed; out->launches_total = g_tgs_launches;
+  out->n_tests = h.n_tests; out->n_tests_evaluated = h.n_tests_eval; out->n_pairs_consumed = h.n_consumed; out->launches_total = g_tgs_launches;
   out->n_slabs = (uint32_t)c->last_n_slabs;
   for (int i = 0; i < TGS_MAX_SLABS; ++i) { out->n_pairs_slab[i] = h.n_pairs_slab[i]; out->n_finished_slab[i] = h.n_finished[i]; }
   if (c->timing) {

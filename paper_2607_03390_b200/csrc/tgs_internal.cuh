@@ -77,6 +77,7 @@ struct Counters {
   unsigned long long n_interactions;   // L (only when interaction counting is on)
   unsigned long long n_blended;        // interactions that passed alpha >= 1/255 and were composited (counting on)
   unsigned long long n_slots;          // pixel slots the blend loop issued: warp iterations x pixels per warp (counting on)
+  unsigned long long n_tests_eval;     // tests k_bin evaluated (tile alive): all of them in one piece, fewer with slabs
   unsigned long long n_consumed;       // pairs the blend reached before their tile was finished, in whole batches (counting on)
 };
 static_assert(sizeof(Counters) % 8 == 0 && sizeof(Counters) <= 512, "Counters layout (k_export_counters copies it with 128 threads)");

@@ -38,14 +38,16 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_header(lib, tmp_path):
     from paper_2607_03390_b200 import tgs
     src = tmp_path / "sz.c"
-    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "tgs.h"\nint main(){printf("%zu %zu %zu %zu %zu\\n",'
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "tgs.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
                    "sizeof(tgs_params),sizeof(tgs_stats),offsetof(tgs_stats,n_pairs),offsetof(tgs_stats,ms_stage),"
-                   "offsetof(tgs_stats,device_bytes));return 0;}\n")
+                   "offsetof(tgs_stats,device_bytes),offsetof(tgs_stats,n_pairs_slab),offsetof(tgs_stats,launches_total),"
+                   "offsetof(tgs_params,depth_slabs),offsetof(tgs_params,slab_split));return 0;}\n")
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
     assert [int(x) for x in out] == [C.sizeof(tgs.TgsParams), C.sizeof(tgs.TgsStats), tgs.TgsStats.n_pairs.offset,
-                                     tgs.TgsStats.ms_stage.offset, tgs.TgsStats.device_bytes.offset]
+                                     tgs.TgsStats.ms_stage.offset, tgs.TgsStats.device_bytes.offset, tgs.TgsStats.n_pairs_slab.offset,
+                                     tgs.TgsStats.launches_total.offset, tgs.TgsParams.depth_slabs.offset, tgs.TgsParams.slab_split.offset]
 
 
 def test_defaults_are_the_papers(lib):
@@ -57,6 +59,8 @@ def test_defaults_are_the_papers(lib):
     assert (p.enable_afc, p.enable_toc, p.enable_sr) == (1, 1, 1)
     # R39 exact tile intersection on; R42 ANCHORED priors (the paper, L86); R43 / L142 TGB at full resolution unless asked
     assert (p.exact_tiles, p.prior_policy, p.tgb_downscale) == (1, 0, 1)
+    # the number of front-to-back slabs is chosen by the library unless asked
+    assert p.depth_slabs == 0 and list(p.slab_split) == [0, 0, 0]
     assert lib.tgs_strerror(tgs.E_NO_PRIORS).decode().startswith("no valid temporal priors")
 
 
