@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
 //  phase A (all Gaussians, 16 B each): near cull, projection of the mean, AFC, TOC + newly-visible lookups in the
 //          warped TGB, and a conservative off-screen test; the survivors are compacted in shared memory;
 //  phase B (survivors only, +32 B each): EWA covariance, conic, radius, rect, records, T^oc marks of small rects;
-//  phase C: the visible Gaussians of the chunk go, compacted, to the chunk's own 1024 slots of a staging list, and the
+//  phase C: the visible Gaussians of the chunk go, compacted, to the chunk's own 2048 slots of a staging list, and the
 //          chunk's count to pre_cnt; the CTA that finishes last scans the counts; k_compact_vis then closes the gaps.
 //          The list the depth sort works on is thus in ascending index order (equal depths stay in index order
 //          through the stable sort, R28) and no chunk waits for another one.
