@@ -106,6 +106,8 @@ typedef struct {
   uint64_t n_tests;      /* (Gaussian, tile) combinations the pair binning examined: sum of the test-rect areas of the visible
                             Gaussians (n_pairs of them passed: tile selected, L123, and reached with alpha >= 1/255, R39) */
   uint64_t n_tests_evaluated; /* of n_tests, those whose tile was still alive when their slab was binned (= n_tests in one piece) */
+  uint64_t n_half_tile_visits, n_half_tile_visits_dead; /* (counting on) dense-mode (record, 16 x 8 half tile) visits of the blend,
+                                and those that reach none of the half's 128 pixels with alpha >= 1/255 */
   uint64_t n_pairs_consumed; /* pairs the blend reached before their tile was finished (whole batches of 128; counting on): the
                                 rest of each tile's list lies behind saturated pixels and is never read */
   uint32_t n_slabs;          /* pieces this frame was binned / sorted / blended in (tgs_params.depth_slabs) */
@@ -177,7 +179,8 @@ const char* tgs_last_error(tgs_ctx*);
  * Writable (tgs_debug_put; marks the priors valid once depth, sigma, image and view are present):
  *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
  * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off"
- *   "count_interactions_on" "count_interactions_off" "redzones_on" (before the scene is loaded: every device buffer allocated
+ *   "count_interactions_on" "count_interactions_off" "blend_half_on" "blend_half_off" "blend_half_auto" (per-warp half-tile record
+ *   lists in the blend: default automatic, on for scenes of small splats; the result does not depend on it) "redzones_on" (before the scene is loaded: every device buffer allocated
  *   afterwards is framed by 256-byte guards) "check_redzones" (TGS_OK if no guard has been written to, else TGS_E_CUDA). */
 long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int mem);
 int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);

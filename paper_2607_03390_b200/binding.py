@@ -42,7 +42,7 @@ class TgsStats(C.Structure):
                 ("n_tiles", C.c_uint32), ("n_sel_oc", C.c_uint32), ("n_sel_um", C.c_uint32), ("n_sel", C.c_uint32),
                 ("n_rendered", C.c_uint32), ("overflow", C.c_uint32), ("n_interactions", C.c_uint64), ("n_blended", C.c_uint64), ("n_pixel_slots", C.c_uint64),
                 ("ms_stage", C.c_float * 8), ("ms_total", C.c_float),
-                ("device_bytes", C.c_uint64), ("n_tests", C.c_uint64), ("n_tests_evaluated", C.c_uint64), ("n_pairs_consumed", C.c_uint64), ("n_slabs", C.c_uint32), ("n_pairs_slab", C.c_uint32 * 4), ("n_finished_slab", C.c_uint32 * 4),
+                ("device_bytes", C.c_uint64), ("n_tests", C.c_uint64), ("n_tests_evaluated", C.c_uint64), ("n_half_tile_visits", C.c_uint64), ("n_half_tile_visits_dead", C.c_uint64), ("n_pairs_consumed", C.c_uint64), ("n_slabs", C.c_uint32), ("n_pairs_slab", C.c_uint32 * 4), ("n_finished_slab", C.c_uint32 * 4),
                 ("launches_total", C.c_uint64)]
 
     def as_dict(self):

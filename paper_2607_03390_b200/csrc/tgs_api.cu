@@ -92,6 +92,8 @@ struct tgs_ctx {
   cudaEvent_t ev_stage[MAX_EV];
   int ev_tag[MAX_EV]; int n_ev = 0;
   int last_n_slabs = 1;
+  int blend_half_mode = -1;             // -1 automatic (small splats: few tests per visible Gaussian), 0 off, 1 on
+  bool half_hint = false;
   // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
   // recent one-piece and two-piece frames; slabs are used where they drop more than half of the pairs
   struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0; } slab_ctl[2];
@@ -501,6 +503,7 @@ static int render_impl(tgs_ctx* c, int mode) {
     CK(cudaEventSynchronize(c->ev_cnt[ci])); c->cnt_pending[ci] = false;
     const Counters& h2 = *c->h_cnt2[ci];
     c->nv_hint = h2.n_visible;
+    c->half_hint = h2.n_visible > 0 && h2.n_tests < 8ull * h2.n_visible;     // small splats: most records reach one half of a tile only
     if (!h2.overflow && h2.n_tests) {
       tgs_ctx::SlabCtl& sc = c->slab_ctl[c->hist_cls[ci]];
       sc.tests = h2.n_tests;
@@ -548,6 +551,7 @@ static int render_impl(tgs_ctx* c, int mode) {
   fc.exact_tiles = c->prm.exact_tiles ? 1 : 0;
   fc.n_tiles = c->TX * c->TY;
   fc.epoch = c->epoch;
+  fc.blend_half = c->blend_half_mode < 0 ? (c->half_hint ? 1 : 0) : c->blend_half_mode;
   // front-to-back slabs: explicit, or automatic from the size of a recent frame's test space -- small frames
   // are launch bound and stay in one piece
   {
@@ -739,7 +743,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
   out->n_pairs = h.n_pairs; out->n_tiles = c->last_n_tiles; out->n_sel_oc = h.n_sel_oc; out->n_sel_um = h.n_sel_um; out->n_sel = h.n_sel;
   out->n_rendered = h.n_rendered; out->overflow = h.overflow; out->n_interactions = h.n_interactions; out->n_blended = h.n_blended; out->n_pixel_slots = h.n_slots;
   out->device_bytes = c->device_bytes;
-  out->n_tests = h.n_tests; out->n_tests_evaluated = h.n_tests_eval; out->n_pairs_consumed = h.n_consumed; out->launches_total = g_tgs_launches;
+  out->n_tests = h.n_tests; out->n_tests_evaluated = h.n_tests_eval; out->n_pairs_consumed = h.n_consumed; out->n_half_tile_visits = h.n_wrec; out->n_half_tile_visits_dead = h.n_wrec_dead; out->launches_total = g_tgs_launches;
   out->n_slabs = (uint32_t)c->last_n_slabs;
   for (int i = 0; i < TGS_MAX_SLABS; ++i) { out->n_pairs_slab[i] = h.n_pairs_slab[i]; out->n_finished_slab[i] = h.n_finished[i]; }
   if (c->timing) {
@@ -879,6 +883,9 @@ static int debug_run_stage_impl(tgs_ctx* c, const char* st) {
   if (s == "count_interactions_off") { c->count_interactions = false; return TGS_OK; }
   if (s == "force_all_tiles_on") { c->force_all = 1; return TGS_OK; }
   if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
+  if (s == "blend_half_on") { c->blend_half_mode = 1; return TGS_OK; }
+  if (s == "blend_half_off") { c->blend_half_mode = 0; return TGS_OK; }
+  if (s == "blend_half_auto") { c->blend_half_mode = -1; return TGS_OK; }
   if (s == "redzones_on") {            // takes effect for the buffers allocated from now on: call it before tgs_load_gaussians
     if (c->n || c->px_cap) return TGS_E_INVALID_ARG;
     c->redzones = true; return TGS_OK;

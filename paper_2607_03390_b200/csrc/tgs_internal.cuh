@@ -48,6 +48,7 @@ struct FrameConst {
   // Front-to-back slabs: the flat test space of the depth-sorted visible Gaussians is cut into n_slabs
   // consecutive ranges of chunks; slab k is binned, sorted and blended before slab k + 1 is binned, and tiles whose pixels
   // have all stopped are dropped from the binning of the later slabs.  slab_bound[k] / 1024 = share of the chunks before slab k.
+  int blend_half;           // k_blend<.,.,HALF>: per-warp lists of the records that reach the warp's half tile (scenes of small splats)
   int n_slabs;              // 1 .. TGS_MAX_SLABS
   uint32_t slab_bound[TGS_MAX_SLABS + 1];
 };
@@ -78,6 +79,7 @@ struct Counters {
   unsigned long long n_blended;        // interactions that passed alpha >= 1/255 and were composited (counting on)
   unsigned long long n_slots;          // pixel slots the blend loop issued: warp iterations x pixels per warp (counting on)
   unsigned long long n_tests_eval;     // tests k_bin evaluated (tile alive): all of them in one piece, fewer with slabs
+  unsigned long long n_wrec, n_wrec_dead;   // dense-mode (record, half tile = warp) visits, and those with alpha < 1/255 at all 128 pixels (counting on)
   unsigned long long n_consumed;       // pairs the blend reached before their tile was finished, in whole batches (counting on)
 };
 static_assert(sizeof(Counters) % 8 == 0 && sizeof(Counters) <= 512, "Counters layout (k_export_counters copies it with 128 threads)");
