@@ -110,12 +110,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
     for (int j = 0; j < SCAN_IPT; ++j) tsum += a[j];
     uint32_t incl_total;
     uint32_t off = tgs_scan::chunk_scan<SCAN_THREADS>(tsum, tile, desc, s_warp, &s_excl, &counters->error, &incl_total, fc.epoch);
-    if (tile == num_tiles - 1 && threadIdx.x == 0) {
-      counters->n_tests = incl_total; area_prefix[n] = incl_total;
-      // pairs <= tests: with the tests inside the capacity no slab can overflow, and the host need not wait for the end of
-      // the frame to know it (2 = cannot be ruled out yet)
-      if (incl_total > fc.max_pairs) { *host_overflow = 2u; __threadfence_system(); }
-    }
+    if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
 #pragma unroll
     for (int j = 0; j < SCAN_IPT; ++j) {
       if (i0 + j >= n) break;
@@ -219,8 +214,13 @@ struct BinSmem {
   uint32_t hist[sizeof(TileT) == 2 ? 2 : 3][256];   // digit histograms of the tile ids of the emitted pairs (for the tile sort)
 };
 
-template <typename TileT>
-__global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4* __restrict__ bin_params, const uint32_t* __restrict__ area_prefix,
+// 8 CTAs per SM (7 with 32-bit tile staging) is what the persistent grid is sized for: the register cap that goes with
+// it (64) must hold, or the eighth CTA of every SM starts only when another one has run out of tickets.
+// LATER: the instance for the second and later slabs (dead-Gaussian skip through the summed-area table, early return when
+// every tile has finished); ALL: every tile is selected and alive (R / P frames, first slab), so no bit is looked up and
+// the evaluated tests need no counting.  The first-slab instances compile to round 1's kernel.
+template <typename TileT, bool LATER, bool ALL>
+__global__ void __launch_bounds__(BIN_THREADS, sizeof(TileT) == 2 ? BIN_CTAS_PER_SM : BIN_CTAS_PER_SM - 1) k_bin(FrameConst fc, const uint4* __restrict__ bin_params, const uint32_t* __restrict__ area_prefix,
                                                      const uint32_t* __restrict__ chunk_first,
                                                      const uint32_t* __restrict__ live_bits, unsigned long long* __restrict__ desc_all,
                                                      uint32_t* __restrict__ keys,
@@ -231,13 +231,17 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
   TGS_PDL_TRIGGER();
   __shared__ BinSmem<TileT> sm;
   const uint32_t n = counters->n_visible, total_tests = counters->n_tests;
+  // pairs <= tests: with the tests inside the capacity no slab can overflow, and the host need not wait for the end of the
+  // frame to know it (2 = cannot be ruled out yet).  (Here and not in k_scan_area: a system fence inside that kernel's loop
+  // cost it 4 us even when never executed.)
+  if (!LATER && blockIdx.x == 0 && threadIdx.x == 0 && total_tests > fc.max_pairs) { *host_overflow = 2u; __threadfence_system(); }
   const uint32_t all_chunks = (uint32_t)(((unsigned long long)total_tests + BIN_CHUNK - 1) / BIN_CHUNK);
   // this slab's range of chunks; inside the slab the chunks are numbered from 0 for the look-back
-  const uint32_t c_lo = (uint32_t)(((unsigned long long)all_chunks * fc.slab_bound[slab]) >> 10);
+  const uint32_t c_lo = LATER ? (uint32_t)(((unsigned long long)all_chunks * fc.slab_bound[slab]) >> 10) : 0u;
   const uint32_t c_hi = (uint32_t)(((unsigned long long)all_chunks * fc.slab_bound[slab + 1]) >> 10);
   uint32_t num_chunks = c_hi - c_lo;
   unsigned long long* desc = desc_all + c_lo;
-  if (slab > 0) {   // every selected tile has finished in the earlier slabs: nothing left to bin (n_pairs_slab stays 0)
+  if (LATER) {      // every selected tile has finished in the earlier slabs: nothing left to bin (n_pairs_slab stays 0)
     uint32_t fin = 0;
     for (int j = 0; j < slab; ++j) fin += counters->n_finished[j];
     if (fin >= counters->n_sel) num_chunks = 0;
@@ -276,7 +280,7 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
         for (uint32_t i = tid; i < nq; i += BIN_THREADS) dst[i] = src[i];
       }
       __syncthreads();
-      if (slab > 0) {
+      if (LATER) {
         // Later slabs: most tiles have finished.  A Gaussian whose test rect holds no live tile -- four look-ups in the
         // summed-area table of the live tiles (k_live_sat) -- has all its tests skipped without looking at them.
         const uint32_t mm = m < (uint32_t)BIN_PCAP ? m : (uint32_t)BIN_PCAP;
@@ -310,10 +314,10 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
           const uint32_t t = t0 + k;
           if (t < tend) {
             if (t >= end) { do { ++li; } while (sm.prefix[li + 1] <= t); load(li, t); }
-            if (G.pad) continue;                                           // no live tile in this Gaussian's rect (later slabs)
             const uint32_t tx = x_lo + rx, ty = y_lo + ry, tile = ty * TX + tx;
-            bool pass = (live_bits[tile >> 5] >> (tile & 31)) & 1u;        // selected (L123) and not yet finished (slabs)
-            n_eval += pass ? 1u : 0u;
+            // selected (L123) and not yet finished (slabs); G.pad: no live tile in this Gaussian's rect at all (later slabs)
+            bool pass = ALL || ((!LATER || !G.pad) && ((live_bits[tile >> 5] >> (tile & 31)) & 1u));
+            if (!ALL) n_eval += pass ? 1u : 0u;
             if (pass && exact) pass = tile_reach(G, tx, ty, fc.cam.W, fc.cam.H);                           // R39
             if (pass) mask |= 1u << k;
             tl[k] = tile; gg[k] = G.g;
@@ -371,8 +375,15 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin(FrameConst fc, const uint4*
   }
   __syncthreads();
   for (int i = tid; i < NH * 256; i += BIN_THREADS) { const uint32_t h = (&sm.hist[0][0])[i]; if (h) atomicAdd(&tile_hist[i], h); }
-  n_eval = __reduce_add_sync(0xffffffffu, n_eval);
-  if (lane == 0 && n_eval) atomicAdd(&counters->n_tests_eval, (unsigned long long)n_eval);
+  if (ALL) {          // every test of the slab was evaluated
+    if (blockIdx.x == 0 && tid == 0 && num_chunks) {
+      const unsigned long long t_hi = (unsigned long long)c_hi * BIN_CHUNK;
+      atomicAdd(&counters->n_tests_eval, (t_hi < total_tests ? t_hi : (unsigned long long)total_tests) - (unsigned long long)c_lo * BIN_CHUNK);
+    }
+  } else {
+    n_eval = __reduce_add_sync(0xffffffffu, n_eval);
+    if (lane == 0 && n_eval) atomicAdd(&counters->n_tests_eval, (unsigned long long)n_eval);
+  }
 }
 
 // ================================================================== A5c: SH -> RGB (L61 "color c_i"; R5)
@@ -470,12 +481,20 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
     else TGS_LAUNCH((k_live_sat<false>), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
   }
   uint32_t* hist = b.sort_hist + (1 + slab) * 4 * 256;
-  if (fc.n_tiles <= 65536)
-    TGS_LAUNCH((k_bin<uint16_t>), num_sms * BIN_CTAS_PER_SM, BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], hist, b.counters, (volatile uint32_t*)host_overflow, slab, (const uint32_t*)b.live_sat);
-  else
-    TGS_LAUNCH((k_bin<uint32_t>), num_sms * (BIN_CTAS_PER_SM - 1), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,
-                                                          (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], hist, b.counters, (volatile uint32_t*)host_overflow, slab, (const uint32_t*)b.live_sat);
+#define BIN_LAUNCH(T, CPS, LATER_, ALL_)                                                                                              \
+  TGS_LAUNCH((k_bin<T, LATER_, ALL_>), num_sms * (CPS), BIN_THREADS, 0, s, fc, b.bin_params, b.area_prefix, b.chunk_first, b.live_bits,   \
+             (unsigned long long*)b.bin_desc, b.keys[0], b.vals[0], hist, b.counters, (volatile uint32_t*)host_overflow, slab, (const uint32_t*)b.live_sat)
+  const bool all = slab == 0 && fc.all_tiles != 0;
+  if (fc.n_tiles <= 65536) {
+    if (slab > 0) BIN_LAUNCH(uint16_t, BIN_CTAS_PER_SM, true, false);
+    else if (all) BIN_LAUNCH(uint16_t, BIN_CTAS_PER_SM, false, true);
+    else BIN_LAUNCH(uint16_t, BIN_CTAS_PER_SM, false, false);
+  } else {
+    if (slab > 0) BIN_LAUNCH(uint32_t, BIN_CTAS_PER_SM - 1, true, false);
+    else if (all) BIN_LAUNCH(uint32_t, BIN_CTAS_PER_SM - 1, false, true);
+    else BIN_LAUNCH(uint32_t, BIN_CTAS_PER_SM - 1, false, false);
+  }
+#undef BIN_LAUNCH
 }
 
 void launch_colour_all(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

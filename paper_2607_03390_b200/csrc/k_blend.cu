@@ -69,25 +69,28 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // T' -> T, sign kept (a finished pixel carries T' < 0); an untouched pixel is exactly 1 (write_pixel and the sparse mode test T == 1)
 __device__ __forceinline__ float unscale_T(float t) { return fabsf(t) == EX2_SCALE ? copysignf(1.0f, t) : t * EX2_SCALE_INV; }
 
-struct Batch {               // slot BLEND_BATCH is a null record (log2 o = -inf: alpha = 0 everywhere), the padding of the half-tile lists
-  float4 a[BLEND_BATCH + 1];     // u, v, A', k
-  float4 b[BLEND_BATCH + 1];     // D', log2(o), d, -
-  float4 c[BLEND_BATCH + 1];     // r, g, b, -
-  uint32_t id[BLEND_BATCH + 1];  // Gaussian index (for the G_rendered marks)
-  uint8_t contrib[BLEND_BATCH + 4];   // G_rendered marks of the batch (benign same-value races)
+template <bool HALF>
+struct BatchT {              // HALF: slot BLEND_BATCH is a null record (log2 o = -inf: alpha = 0 everywhere), the padding of the half-tile lists
+  static constexpr int N = BLEND_BATCH + (HALF ? 1 : 0);
+  float4 a[N];     // u, v, A', k
+  float4 b[N];     // D', log2(o), d, -
+  float4 c[N];     // r, g, b, -
+  uint32_t id[N];  // Gaussian index (for the G_rendered marks)
+  uint8_t contrib[BLEND_BATCH + (HALF ? 4 : 0)];   // G_rendered marks of the batch (benign same-value races)
 };
 
 struct Pixel {               // per-pixel state of the front-to-back loop; sum of the weights = 1 - T (telescoping)
   float T, Cr, Cg, Cb, S1, S2, d0;
 };
 
-struct BlendSmem {
-  Batch bt[2];
+template <bool HALF>
+struct BlendSmemT {
+  BatchT<HALF> bt[2];
   float st[BLEND_THREADS][7];      // pixel states in transit during a compaction
   uint16_t st_px[BLEND_THREADS];   // their pixel index inside the tile (ly * 16 + lx)
   uint32_t alive_cnt[2][BLEND_WARPS];   // [parity][warp] alive pixels
   uint32_t work;
-  uint8_t wl[BLEND_WARPS][BLEND_BATCH + DENSE_GROUP];   // HALF: per warp, the records of the batch that can reach its half tile, in order
+  uint8_t wl[HALF ? BLEND_WARPS : 1][HALF ? BLEND_BATCH + DENSE_GROUP : 4];   // HALF: per warp, the records of the batch that can reach its half tile, in order
 };
 
 // one (pixel, Gaussian) interaction (sparse mode); returns false when the pixel is finished
@@ -129,7 +132,9 @@ __device__ __forceinline__ void write_pixel(const FrameConst& fc, const Pixel& p
 // alpha >= 1/255: a conservative bound on the exponent over the half's pixel box (never skips a record that could reach;
 // the result changes only by which records share a clamp group, i.e. by rounding), evaluated by the warp while the batch sits in shared memory.  Pays on scenes of small
 // splats (config 4: 36 % of the (record, half tile) visits reach nothing; config 3: 0.5-7 %, where it is left off).
-template <bool MARK, bool COUNT, bool HALF>
+// SLABS: the instance for frames rendered in several front-to-back pieces (park / restore of pixel states, live tiles);
+// one-piece frames run the instance without any of it, whose blend loop is register-allocated as in round 1.
+template <bool MARK, bool COUNT, bool HALF, bool SLABS>
 __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLEND_MIN_CTAS) k_blend(FrameConst fc, const uint32_t* __restrict__ tile_order,
                                                          uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
                                                          const float4* __restrict__ rec_b0, const float4* __restrict__ rec_b1,
@@ -141,12 +146,13 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
                                                          float* __restrict__ pix_state, int slab) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
-  __shared__ BlendSmem sm;
+  __shared__ BlendSmemT<HALF> sm;
+  using Batch = BatchT<HALF>;
   const CamConst& k = fc.cam;
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int lx = (int)(tid % RUNS) * PPT, ly = (int)(tid / RUNS);
   const uint32_t n_sel = counters->n_sel;
-  if (HALF && tid < 2) {
+  if constexpr (HALF) if (tid < 2) {
     Batch& Bn = sm.bt[tid];
     Bn.a[BLEND_BATCH] = make_float4(0.0f, 0.0f, 0.0f, 0.0f); Bn.b[BLEND_BATCH] = make_float4(0.0f, -INFINITY, 0.0f, 0.0f);
     Bn.c[BLEND_BATCH] = make_float4(0.0f, 0.0f, 0.0f, 0.0f); Bn.id[BLEND_BATCH] = 0u;
@@ -154,10 +160,10 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
   // Front-to-back slabs: this launch blends the pairs of slab `slab`.  A tile whose pixels have all
   // stopped is written out and leaves `live_bits` (the later slabs bin no pairs for it); a tile that is still alive at the
   // end of its list parks its pixel states in `pix_state` and goes on in the next slab; the last slab writes every tile.
-  const bool last = slab == fc.n_slabs - 1;
-  const uint32_t n_work = slab == 0 ? (uint32_t)fc.n_tiles : n_sel;      // the stitched tiles are done with slab 0
+  const bool last = !SLABS || slab == fc.n_slabs - 1;
+  const uint32_t n_work = (!SLABS || slab == 0) ? (uint32_t)fc.n_tiles : n_sel;      // the stitched tiles are done with slab 0
   uint32_t zero_tile = 0xffffffffu;                                       // (thread 0) tile whose range is to be cleared for the next slab
-  if (slab > 0) {                                                         // every selected tile finished in the earlier slabs: nothing to do
+  if (SLABS && slab > 0) {                                                // every selected tile finished in the earlier slabs: nothing to do
     uint32_t fin = 0;
     for (int j = 0; j < slab; ++j) fin += counters->n_finished[j];
     if (fin >= n_sel) return;
@@ -165,7 +171,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
   while (true) {
     __syncthreads();
     if (tid == 0) {
-      if (zero_tile != 0xffffffffu) { ranges[zero_tile] = make_uint2(0u, 0u); zero_tile = 0xffffffffu; }
+      if (SLABS && zero_tile != 0xffffffffu) { ranges[zero_tile] = make_uint2(0u, 0u); zero_tile = 0xffffffffu; }
       sm.work = atomicAdd(&counters->ticket_blend[slab], 1u);
     }
     __syncthreads();
@@ -210,13 +216,13 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
       continue;
     }
     // -------------------------------------------------- A8 blend
-    if (slab > 0 && !((live_bits[tile >> 5] >> (tile & 31u)) & 1u)) continue;      // finished (and written) in an earlier slab
+    if (SLABS && slab > 0 && !((live_bits[tile >> 5] >> (tile & 31u)) & 1u)) continue;      // finished (and written) in an earlier slab
     uint2 range = ranges[tile];                      // {~start, end}, zero for a tile without pairs (k_sort.cu, A7)
     range.x = range.y ? ~range.x : 0u;
     const uint32_t len = range.y - range.x, nb = (len + BLEND_BATCH - 1) / BLEND_BATCH;
-    if (len == 0u && !last) continue;                // nothing of this slab reaches the tile: its state, if any, stays parked
-    if (!last && tid == 0) zero_tile = tile;
-    const bool restore = slab > 0 && (tile_flags[tile] & 8u) != 0u;
+    if (SLABS && len == 0u && !last) continue;       // nothing of this slab reaches the tile: its state, if any, stays parked
+    if (SLABS && !last && tid == 0) zero_tile = tile;
+    const bool restore = SLABS && slab > 0 && (tile_flags[tile] & 8u) != 0u;
     float* const st_base = pix_state + (size_t)tile * (7 * TGS_TILE * TGS_TILE);
     float fpx = (float)px0, fpy = (float)py;
     // dense mode: pixels (0,1) and (2,3) of the run as two packed pairs (fma.rn.f32x2 of sm_100); sparse mode: sp
@@ -238,7 +244,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
     for (int i = 0; i < PPT; ++i) valid[i] = row_in && px0 + i < k.W;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) T2[q] = make_float2(valid[2 * q] ? EX2_SCALE : -EX2_SCALE, valid[2 * q + 1] ? EX2_SCALE : -EX2_SCALE);   // T' = EX2_SCALE T
-    if (restore) {
+    if (SLABS && restore) {
       // parked states, [field][pixel]: T' (scaled, negative = stopped, 0 = already written), Cr, Cg, Cb, S1, S2, d0
       static_assert(PPT == 4, "state layout: one float4 per thread and field");
       float f[7][PPT];
@@ -526,11 +532,11 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
     if (MARK && computed >= 0) { __syncthreads(); writeback_marks((uint32_t)computed); }
     // -------------------------------------------------- outputs, or the states parked for the next slab
     bool park = false;
-    if (!last) {
+    if (SLABS && !last) {
       const bool alive_t = sparse ? (have && salive) : (count_alive() != 0u);
       park = __syncthreads_or(alive_t ? 1 : 0) != 0;
     }
-    if (park) {
+    if (SLABS && park) {
       float4* const st4 = reinterpret_cast<float4*>(st_base);
       constexpr int FS = TGS_TILE * TGS_TILE / 4;                     // float4 per field
       if (!sparse) {
@@ -563,7 +569,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
       } else if (have) {
         write_pixel(fc, sp, (size_t)(tile_y0 + (int)(spx >> 4)) * k.W + tile_x0 + (int)(spx & 15u), image, depth, sigma);
       }
-      if (!last && tid == 0) { atomicAnd(&live_bits[tile >> 5], ~(1u << (tile & 31u))); atomicAdd(&counters->n_finished[slab], 1u); }   // finished: no pairs in the later slabs
+      if (SLABS && !last && tid == 0) { atomicAnd(&live_bits[tile >> 5], ~(1u << (tile & 31u))); atomicAdd(&counters->n_finished[slab], 1u); }   // finished: no pairs in the later slabs
     }
     if (COUNT) {
       nint = __reduce_add_sync(0xffffffffu, nint);
@@ -582,11 +588,12 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx, const float* prior_image,
                   uint8_t* rendered_next, int num_sms, bool count_interactions, int slab) {
   const int grid = num_sms * (PPT == 4 ? 12 : PPT == 8 ? 16 : 8);
-#define LAUNCH(M, C, H)                                                                                                       \
-  TGS_LAUNCH((k_blend<M, C, H>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
+#define LAUNCH(M, C, H, SL)                                                                                                     \
+  TGS_LAUNCH((k_blend<M, C, H, SL>), grid, BLEND_THREADS, 0, s, fc, b.tile_order, b.ranges, b.vals[sorted_idx], b.rec_b0, b.rec_b1, b.rec_rgb, \
                                                prior_image, b.fill_depth, (const float2*)b.warp_tgb, b.image[out_idx], b.depth[out_idx],  \
                                                b.sigma[out_idx], rendered_next, b.counters, b.tile_flags, b.live_bits, b.pix_state, slab)
-#define LAUNCH2(M, C) do { if (fc.blend_half) LAUNCH(M, C, true); else LAUNCH(M, C, false); } while (0)
+#define LAUNCH2(M, C) do { if (fc.n_slabs > 1) { if (fc.blend_half) LAUNCH(M, C, true, true); else LAUNCH(M, C, false, true); } \
+                           else { if (fc.blend_half) LAUNCH(M, C, true, false); else LAUNCH(M, C, false, false); } } while (0)
   if (rendered_next) { if (count_interactions) LAUNCH2(true, true); else LAUNCH2(true, false); }
   else { if (count_interactions) LAUNCH2(false, true); else LAUNCH2(false, false); }
 #undef LAUNCH2

@@ -96,7 +96,7 @@ struct tgs_ctx {
   bool half_hint = false;
   // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
   // recent one-piece and two-piece frames; slabs are used where they drop more than half of the pairs
-  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0; } slab_ctl[2];
+  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0; bool asked1 = false, asked2 = false; } slab_ctl[2];
   int hist_cls[2] = {0, 0}, hist_slabs[2] = {1, 1};   // class and number of slabs of the frame that last used each counter block
   FrameConst fc;
 };
@@ -197,8 +197,7 @@ int alloc_frame_buffers(tgs_ctx* c) {
   if (int r = dev_alloc(c, &b.tile_mask, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.sel_bits, (size_t)(T + 31) / 32 + 1, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.live_bits, (size_t)(T + 31) / 32 + 1, c->allocs_frame)) return r;
-  if (int r = dev_alloc(c, &b.live_sat, (size_t)(c->TX + 1) * (c->TY + 1), c->allocs_frame)) return r;
-  if (int r = dev_alloc(c, &b.pix_state, (size_t)T * 7 * TGS_TILE * TGS_TILE, c->allocs_frame)) return r;
+  b.live_sat = nullptr; b.pix_state = nullptr;      // slab buffers: allocated by the first frame that runs in several pieces
   if (int r = dev_alloc(c, &b.tile_order, (size_t)T, c->allocs_frame)) return r;
   if (int r = dev_alloc(c, &b.ranges, (size_t)T, c->allocs_frame)) return r;
   c->px_cap = px; c->tiles_cap = T;
@@ -562,8 +561,10 @@ static int render_impl(tgs_ctx* c, int mode) {
       // of the pixel states.  Measured, not guessed: pairs per test of the latest one-piece and two-piece frames of this
       // class, the other variant re-probed every 32 frames; small frames are launch bound and stay in one piece.
       tgs_ctx::SlabCtl& sc = c->slab_ctl[ftype == TGS_FRAME_S ? 1 : 0];
-      if (sc.tests < 2000000u || sc.p1 < 0.0f) ns = 1;
-      else if (sc.p2 < 0.0f) ns = 2;
+      if (!sc.asked1) { ns = 1; sc.asked1 = true; }                               // a one-piece sample ...
+      else if (sc.tests < 2000000u) ns = 1;                                       // (small, or nothing known yet)
+      else if (!sc.asked2) { ns = 2; sc.asked2 = true; }                          // ... then ONE two-piece probe ...
+      else if (sc.p1 < 0.0f || sc.p2 < 0.0f) ns = 1;                              // ... and one piece until both have been counted
       else {
         const int prefer = sc.p2 < 0.5f * sc.p1 ? 2 : 1;
         ns = prefer;
@@ -579,6 +580,10 @@ static int render_impl(tgs_ctx* c, int mode) {
       fc.slab_bound[i] = v;
     }
     for (int i = ns; i <= TGS_MAX_SLABS; ++i) fc.slab_bound[i] = 1024;
+    if (ns > 1 && !c->b.pix_state) {
+      if (int r = dev_alloc(c, &c->b.live_sat, (size_t)(c->TX + 1) * (c->TY + 1), c->allocs_frame)) return r;
+      if (int r = dev_alloc(c, &c->b.pix_state, (size_t)(c->TX * c->TY) * 7 * TGS_TILE * TGS_TILE, c->allocs_frame)) return r;
+    }
   }
   c->b.counters = c->counters2[ci];          // ci = parity of this frame's epoch (computed above)
   c->h_counters = c->h_cnt2[ci];
