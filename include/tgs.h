@@ -186,6 +186,30 @@ long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int
 int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);
 int tgs_debug_run_stage(tgs_ctx*, const char* stage);
 
+/* ---- an entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it) ----
+ * The path's stable LSD radix sort of (uint32 key, uint32 value) pairs (A6, the tile sort of PAPER.md:L61 "for each tile, sorts its
+ * intersected Gaussians by depth": pairs emitted in depth order are sorted stably by tile id) as a call of its own, with every byte
+ * of its scratch -- digit histograms, tile tickets, look-back descriptors, the ping-pong buffers of the intermediate passes -- in
+ * ONE file-scope static device array of TGS_SORT_STATIC_SCRATCH_BYTES (~8.5 MiB), which every GPU that loads libtgs.so holds until
+ * the process exits.  The call needs no tgs_ctx and calls no cudaMalloc / cudaFree / allocating library routine; it only enqueues
+ * work (one memset, one histogram kernel, key_bytes scatter kernels, at most two small copies) on `cuda_stream` of `cuda_device`.
+ *   keys_in, vals_in   [n] DEVICE, read only           keys_out, vals_out   [n] DEVICE, must not overlap the inputs
+ *   n                  items, 0 .. TGS_SORT_STATIC_MAX_ITEMS; a larger n is rejected with TGS_E_INVALID_ARG and nothing is enqueued
+ *   key_bytes          1 .. 4: the sort is stable on the low 8 * key_bytes bits of the key (higher bits are carried, not compared)
+ *   status             nullable DEVICE word, caller-owned: receives 0, or non-zero if a look-back gave up (the output is then invalid)
+ * Returns TGS_OK, TGS_E_INVALID_ARG (null pointer, n or key_bytes out of range, overlapping buffers, bad device) or TGS_E_CUDA;
+ * tgs_static_last_error() gives the reason of the calling thread's last failure ("" if none).
+ * Every call on a device shares the array, which keeps the previous call's contents: the call clears what must start at zero
+ * (histograms, tickets, status) and tags its descriptors with a per-device call number, so calls that follow one another in ONE
+ * stream are independent.  Calls that OVERLAP on the GPU (two streams, two host threads with different streams, two processes'
+ * worth of graph replays at once) race on the array and give garbage: serialise them. */
+#define TGS_SORT_STATIC_MAX_ITEMS (1u << 20)
+#define TGS_SORT_STATIC_SCRATCH_BYTES (4352u + 256u * 2048u + 2u * 4u * TGS_SORT_STATIC_MAX_ITEMS)
+int tgs_sort_pairs_static(int cuda_device, void* cuda_stream, const uint32_t* keys_in, const uint32_t* vals_in, uint32_t* keys_out,
+                          uint32_t* vals_out, uint32_t n, int key_bytes, uint32_t* status);
+const char* tgs_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,9 @@ DEPTH_INVALID = np.float32(3.0e38)
 
 EXPORTS = ["tgs_create", "tgs_destroy", "tgs_load_gaussians", "tgs_load_ply", "tgs_set_camera", "tgs_default_params", "tgs_set_params",
            "tgs_render", "tgs_read_image", "tgs_read_image_async", "tgs_wait_reads", "tgs_read_depth", "tgs_read_tile_mask", "tgs_get_stats", "tgs_reset_priors",
-           "tgs_strerror", "tgs_last_error", "tgs_debug_get", "tgs_debug_put", "tgs_debug_run_stage"]
+           "tgs_strerror", "tgs_last_error", "tgs_debug_get", "tgs_debug_put", "tgs_debug_run_stage",
+           "tgs_sort_pairs_static", "tgs_static_last_error"]
+SORT_STATIC_MAX_ITEMS = 1 << 20
 
 
 class TgsParams(C.Structure):
@@ -96,6 +98,9 @@ def lib():
         L.tgs_debug_get.restype = C.c_longlong
         L.tgs_debug_put.argtypes = [vp, C.c_char_p, vp, C.c_size_t, C.c_int]
         L.tgs_debug_run_stage.argtypes = [vp, C.c_char_p]
+        L.tgs_sort_pairs_static.argtypes = [C.c_int, vp, vp, vp, vp, vp, C.c_uint32, C.c_int, vp]
+        L.tgs_static_last_error.argtypes = []
+        L.tgs_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -117,6 +122,19 @@ _DEBUG_DTYPES = {
     "rendered": np.uint8, "F": np.float32, "prior_depth": np.float32, "prior_sigma": np.float32, "prior_image": np.float32,
     "cov3d": np.float32, "tau": np.float32,
 }
+
+
+def sort_pairs_static(keys_in, vals_in, keys_out, vals_out, n, key_bytes, device=0, stream=None, status=None):
+    """tgs_sort_pairs_static: the entry point that allocates nothing (include/tgs.h).  The buffers are CUDA tensors of 4-byte
+    elements (anything with data_ptr()) or raw device addresses; only enqueues work on `stream` (default stream if None)."""
+    def ptr(a):
+        return C.c_void_p(a if isinstance(a, int) else (a.data_ptr() if a is not None else 0))
+    L = lib()
+    rc = L.tgs_sort_pairs_static(device, C.c_void_p(stream or 0), ptr(keys_in), ptr(vals_in), ptr(keys_out), ptr(vals_out), n, key_bytes,
+                                 ptr(status))
+    if rc != OK:
+        raise TgsError(rc, "tgs_sort_pairs_static", L.tgs_strerror(rc).decode() + "; " + L.tgs_static_last_error().decode())
+    return rc
 
 
 class Context:

@@ -256,3 +256,150 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
   }
   return cur;
 }
+
+// ------------------------------------------------------------------------------------------------------------------
+// tgs_sort_pairs_static (include/tgs.h): the same scatter passes as a call that allocates nothing.  Every byte of scratch
+// lives in the file-scope array below; the kernels get its DEVICE address, which host code obtains once per device with
+// cudaGetSymbolAddress (in host code the array's name is only a stand-in for the symbol, not a pointer a kernel could use).
+// The array is shared by all calls on a device and keeps the last call's contents: histograms / tickets / the error word
+// are cleared by every call, the descriptors are tagged with (call number * 4 + pass) and never cleared, the ping-pong
+// buffers are written before they are read.  Calls that overlap on the GPU race (documented in the header).
+#include <cstddef>
+#include <cstdio>
+#include <mutex>
+
+namespace {
+
+constexpr uint32_t STATIC_MAX_ITEMS = TGS_SORT_STATIC_MAX_ITEMS;
+constexpr uint32_t STATIC_SMALL_MAX = 1u << 18;      // up to here the 2048-item instance (more tiles in flight), above it the 4096-item one
+constexpr uint32_t STATIC_MAX_TILES = 256;           // = 2^20 / 4096 >= 2^18 / 2048
+static_assert(STATIC_MAX_ITEMS / (SORT_THREADS * SORT_IPT_BIG) <= STATIC_MAX_TILES && STATIC_SMALL_MAX / (SORT_THREADS * SORT_IPT_SMALL) <= STATIC_MAX_TILES, "descriptor rows");
+
+struct StaticSortScratch {
+  uint32_t hist[4][RADIX];                                // cleared by every call, filled by k_static_hist
+  uint32_t tickets[4];                                    // cleared by every call
+  uint32_t error;                                         // cleared by every call; 2 = a look-back gave up
+  uint32_t n;                                             // written by k_static_hist (k_onesweep reads its item count from device memory)
+  uint32_t pad[58];
+  unsigned long long desc[STATIC_MAX_TILES * RADIX];      // one region for all passes: the tag tells the passes and the calls apart
+  uint32_t tmp_keys[STATIC_MAX_ITEMS];                    // destination of every other pass
+  uint32_t tmp_vals[STATIC_MAX_ITEMS];
+};
+static_assert(sizeof(StaticSortScratch) == TGS_SORT_STATIC_SCRATCH_BYTES, "tgs.h states the size");
+static_assert(offsetof(StaticSortScratch, desc) == 4352 && offsetof(StaticSortScratch, desc) % 256 == 0, "head");
+
+static __device__ __align__(256) unsigned char g_static_sort_scratch[sizeof(StaticSortScratch)];
+
+// digit histograms of the low `passes` bytes of the keys (in the path the producer of the keys counts them; here nobody has)
+__global__ void __launch_bounds__(256) k_static_hist(const uint32_t* __restrict__ keys, uint32_t n, int passes, StaticSortScratch* __restrict__ sc) {
+  __shared__ uint32_t h[4][RADIX];
+  for (int i = threadIdx.x; i < 4 * RADIX; i += 256) (&h[0][0])[i] = 0;
+  __syncthreads();
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) {
+    const uint32_t k = keys[i];
+    for (int p = 0; p < passes; ++p) atomicAdd(&h[p][(k >> (8 * p)) & 255u], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < passes * RADIX; i += 256) {
+    const uint32_t v = (&h[0][0])[i];
+    if (v) atomicAdd(&sc->hist[0][0] + i, v);
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) sc->n = n;
+}
+
+struct StaticSortDev {
+  StaticSortScratch* ptr = nullptr;   // device address of g_static_sort_scratch on this device
+  int num_sms = 0;
+  uint32_t call = 0;                  // descriptor tag = call * 4 + pass, kept below 2^30 (the tag field of a descriptor)
+};
+constexpr int STATIC_MAX_DEVICES = 64;
+StaticSortDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (e != cudaSuccess) snprintf(g_static_err, sizeof(g_static_err), "tgs_sort_pairs_static: %s: %s", what, cudaGetErrorString(e));
+  else snprintf(g_static_err, sizeof(g_static_err), "tgs_sort_pairs_static: %s", what);
+  return code;
+}
+
+bool ranges_overlap(const void* a, const void* b, size_t bytes) {
+  const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+  return x < y + bytes && y < x + bytes;
+}
+
+}  // namespace
+
+extern "C" const char* tgs_static_last_error(void) { return g_static_err; }
+
+extern "C" int tgs_sort_pairs_static(int cuda_device, void* cuda_stream, const uint32_t* keys_in, const uint32_t* vals_in, uint32_t* keys_out,
+                                     uint32_t* vals_out, uint32_t n, int key_bytes, uint32_t* status) {
+  g_static_err[0] = 0;
+  if (n > STATIC_MAX_ITEMS) {
+    snprintf(g_static_err, sizeof(g_static_err), "tgs_sort_pairs_static: n = %u exceeds the maximum of %u items (TGS_SORT_STATIC_MAX_ITEMS): the static scratch array has a fixed size",
+             n, STATIC_MAX_ITEMS);
+    return TGS_E_INVALID_ARG;
+  }
+  if (key_bytes < 1 || key_bytes > 4) return static_fail(TGS_E_INVALID_ARG, "key_bytes must be 1..4");
+  if (cuda_device < 0 || cuda_device >= STATIC_MAX_DEVICES) return static_fail(TGS_E_INVALID_ARG, "bad device index");
+  if (n > 0) {
+    if (!keys_in || !vals_in || !keys_out || !vals_out) return static_fail(TGS_E_INVALID_ARG, "null buffer");
+    const size_t bytes = (size_t)n * 4;
+    if (ranges_overlap(keys_in, keys_out, bytes) || ranges_overlap(keys_in, vals_out, bytes) || ranges_overlap(vals_in, keys_out, bytes) ||
+        ranges_overlap(vals_in, vals_out, bytes) || ranges_overlap(keys_out, vals_out, bytes))
+      return static_fail(TGS_E_INVALID_ARG, "output buffers overlap the inputs or each other");
+  }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  cudaError_t e;
+  int prev_device = -1;
+  if ((e = cudaGetDevice(&prev_device)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaGetDevice", e);
+  if ((e = cudaSetDevice(cuda_device)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaSetDevice", e);
+  struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev_device == cuda_device ? -1 : prev_device};
+
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticSortDev& d = g_static_dev[cuda_device];
+  if (!d.ptr) {   // set-up, once per device, with that device current
+    StaticSortScratch* p = nullptr;
+    if ((e = cudaGetSymbolAddress((void**)&p, g_static_sort_scratch)) != cudaSuccess || !p) return static_fail(TGS_E_CUDA, "cudaGetSymbolAddress(g_static_sort_scratch)", e);
+    int sms = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device)) != cudaSuccess || sms <= 0) return static_fail(TGS_E_CUDA, "cudaDeviceGetAttribute", e);
+    if ((e = cudaFuncSetAttribute(k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_BIG>))) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(k_onesweep<32, 2, SORT_IPT_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<SORT_IPT_SMALL>))) != cudaSuccess)
+      return static_fail(TGS_E_CUDA, "cudaFuncSetAttribute", e);
+    d.num_sms = sms;
+    d.ptr = p;      // last: a failed set-up is tried again by the next call
+  }
+  StaticSortScratch* sc = d.ptr;
+  if (status && (e = cudaMemsetAsync(status, 0, 4, s)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaMemsetAsync(status)", e);
+  if (n == 0) return TGS_OK;
+  if (++d.call >= (1u << 28)) {   // the tags wrap: forget the old ones (static device memory starts as zeros, and tag 0..3 is never used)
+    d.call = 1;
+    if ((e = cudaMemsetAsync(sc->desc, 0, sizeof(sc->desc), s)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaMemsetAsync(desc)", e);
+  }
+  if ((e = cudaMemsetAsync(sc, 0, offsetof(StaticSortScratch, desc), s)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaMemsetAsync(head)", e);
+  const int passes = key_bytes;
+  const uint32_t hist_blocks = (n + 256u * 16u - 1u) / (256u * 16u);
+  k_static_hist<<<hist_blocks < (uint32_t)d.num_sms * 4u ? hist_blocks : (uint32_t)d.num_sms * 4u, 256, 0, s>>>(keys_in, n, passes, sc);
+  ++g_tgs_launches;
+  const bool small_input = n <= STATIC_SMALL_MAX;
+  const uint32_t* src_k = keys_in;
+  const uint32_t* src_v = vals_in;
+  for (int p = 0; p < passes; ++p) {
+    const bool to_out = ((passes - 1 - p) & 1) == 0;      // the last pass writes the caller's buffers, the passes before it alternate
+    uint32_t* dst_k = to_out ? keys_out : sc->tmp_keys;
+    uint32_t* dst_v = to_out ? vals_out : sc->tmp_vals;
+    const uint32_t tag = d.call * 4u + (uint32_t)p;
+    if (small_input)
+      k_onesweep<32, 2, SORT_IPT_SMALL><<<d.num_sms * 2, SORT_THREADS, sizeof(SortSmem<SORT_IPT_SMALL>), s>>>(
+          src_k, src_v, dst_k, dst_v, &sc->n, &sc->tickets[p], &sc->error, &sc->hist[p][0], sc->desc, 8 * p, 8, tag, (uint2*)nullptr);
+    else
+      k_onesweep<4, SORT_CTAS_PER_SM, SORT_IPT_BIG><<<d.num_sms * SORT_CTAS_PER_SM, SORT_THREADS, sizeof(SortSmem<SORT_IPT_BIG>), s>>>(
+          src_k, src_v, dst_k, dst_v, &sc->n, &sc->tickets[p], &sc->error, &sc->hist[p][0], sc->desc, 8 * p, 8, tag, (uint2*)nullptr);
+    ++g_tgs_launches;
+    src_k = dst_k;
+    src_v = dst_v;
+  }
+  if (status && (e = cudaMemcpyAsync(status, &sc->error, 4, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) return static_fail(TGS_E_CUDA, "cudaMemcpyAsync(status)", e);
+  if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(TGS_E_CUDA, "kernel launch", e);
+  return TGS_OK;
+}
