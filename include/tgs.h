@@ -180,7 +180,10 @@ const char* tgs_last_error(tgs_ctx*);
  *   prior_depth prior_sigma prior_image rendered F prior_view (float[16]).
  * tgs_debug_run_stage: "timing_on" "timing_off" "force_all_tiles_on" "force_all_tiles_off"
  *   "count_interactions_on" "count_interactions_off" "blend_half_on" "blend_half_off" "blend_half_auto" (per-warp half-tile record
- *   lists in the blend: default automatic, on for scenes of small splats; the result does not depend on it) "redzones_on" (before the scene is loaded: every device buffer allocated
+ *   lists in the blend: default automatic, on for scenes of small splats; the result does not depend on it)
+ *   "depth_sort_fused_on" "depth_sort_fused_off" "depth_sort_fused_auto" (the depth sort of the visible Gaussians and the prefix sums of
+ *   their test rects as one launch instead of five: default automatic, on for short visible lists; the result does not depend on it)
+ *   "redzones_on" (before the scene is loaded: every device buffer allocated
  *   afterwards is framed by 256-byte guards) "check_redzones" (TGS_OK if no guard has been written to, else TGS_E_CUDA). */
 long long tgs_debug_get(tgs_ctx*, const char* name, void* dst, size_t bytes, int mem);
 int tgs_debug_put(tgs_ctx*, const char* name, const void* src, size_t bytes, int mem);

@@ -1,0 +1,44 @@
+// bin_params.cuh -- the record the pair binning (k_bin.cu) reads per visible Gaussian, and the flat test space's chunk size.
+// Shared by the two kernels that can write those records: k_scan_area (k_bin.cu) and the one-launch depth sort
+// (k_sort.cu), whose last stage does k_scan_area's work.  Nothing here is decision arithmetic that could be contracted:
+// kC / kA are single multiplications by a correctly rounded reciprocal.  NOT shared with oracle/.
+#pragma once
+#include "tgs_internal.cuh"
+
+constexpr int BIN_THREADS = 128;
+constexpr int BIN_IPT = 8;
+constexpr int BIN_CHUNK = BIN_THREADS * BIN_IPT;      // tests per work item of k_bin
+
+// Tile-test parameters of one visible Gaussian; 48 B, written in SORTED order by k_scan_area so that a k_bin chunk
+// reads the parameters of its Gaussians as one contiguous, coalesced block instead of gathering three records each
+// (scenes of many small Gaussians -- config 4: ~500 Gaussians per 1024-test chunk -- were bound by those gathers).
+struct alignas(16) GaussParams {
+  float u, v, A, B;
+  float C, tau, kC, kA;                 // kC ~ -B/C, kA ~ -B/A
+  uint32_t g, lo, w, pad;               // lo = x_lo | y_lo << 16
+};
+static_assert(sizeof(GaussParams) == 48, "three uint4 per Gaussian");
+
+__device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exact, const float4* __restrict__ rec_uvdo,
+                                                   const float4* __restrict__ rec_conic) {
+  GaussParams P;
+  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
+  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
+  if (exact) {
+    const float4 a = rec_uvdo[g], b = rec_conic[g];
+    P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
+    P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
+  }
+  return P;
+}
+__device__ __forceinline__ void store_params(uint4* __restrict__ dst, const GaussParams& P) {
+  const uint4* s = reinterpret_cast<const uint4*>(&P);
+  dst[0] = s[0]; dst[1] = s[1]; dst[2] = s[2];
+}
+__device__ __forceinline__ GaussParams load_params(const uint4* __restrict__ src) {
+  GaussParams P;
+  uint4* d = reinterpret_cast<uint4*>(&P);
+  d[0] = src[0]; d[1] = src[1]; d[2] = src[2];
+  return P;
+}
+

@@ -16,6 +16,7 @@
 // Problem sizes that are not known on the host (visible Gaussians, tests, pairs) are read from device memory, so a
 // frame needs no host round trip.
 #include "tgs_internal.cuh"
+#include "bin_params.cuh"
 #include "decide_math.cuh"
 #include "scan.cuh"
 
@@ -25,45 +26,9 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_IPT = 2;          // 8 (2048-Gaussian tiles, a shorter look-back) measured slower: +20 us, the gathers of a tile are serial per thread
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 
-constexpr int BIN_THREADS = 128;
-constexpr int BIN_IPT = 8;
 constexpr int BIN_CTAS_PER_SM = 8;
-constexpr int BIN_CHUNK = BIN_THREADS * BIN_IPT;      // tests per work item
-
-// Tile-test parameters of one visible Gaussian; 48 B, written in SORTED order by k_scan_area so that a k_bin chunk
-// reads the parameters of its Gaussians as one contiguous, coalesced block instead of gathering three records each
-// (scenes of many small Gaussians -- config 4: ~500 Gaussians per 1024-test chunk -- were bound by those gathers).
-struct alignas(16) GaussParams {
-  float u, v, A, B;
-  float C, tau, kC, kA;                 // kC ~ -B/C, kA ~ -B/A
-  uint32_t g, lo, w, pad;               // lo = x_lo | y_lo << 16
-};
-static_assert(sizeof(GaussParams) == 48, "three uint4 per Gaussian");
 
 constexpr int BIN_PCAP = 192;           // Gaussians of a chunk staged in shared memory (the rest is read from global)
-
-__device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exact, const float4* __restrict__ rec_uvdo,
-                                                   const float4* __restrict__ rec_conic) {
-  GaussParams P;
-  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
-  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
-  if (exact) {
-    const float4 a = rec_uvdo[g], b = rec_conic[g];
-    P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
-    P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
-  }
-  return P;
-}
-__device__ __forceinline__ void store_params(uint4* __restrict__ dst, const GaussParams& P) {
-  const uint4* s = reinterpret_cast<const uint4*>(&P);
-  dst[0] = s[0]; dst[1] = s[1]; dst[2] = s[2];
-}
-__device__ __forceinline__ GaussParams load_params(const uint4* __restrict__ src) {
-  GaussParams P;
-  uint4* d = reinterpret_cast<uint4*>(&P);
-  d[0] = src[0]; d[1] = src[1]; d[2] = src[2];
-  return P;
-}
 
 // ================================================================== A5a: flat test space
 // area_prefix[i] = number of tests of the Gaussians before position i of the sorted visible list (area_prefix[n] =
@@ -465,11 +430,13 @@ __global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_
 }
 
 // sorted_g_idx: which of cvals[] holds the visible Gaussians in (depth, index) order
+unsigned long long bin_max_tests(uint32_t bin_chunks_cap) { return (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK; }
+
 void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_g_idx, uint32_t bin_chunks_cap, int num_sms,
                 uint32_t* host_overflow, int slab) {
-  if (slab == 0) {
+  if (slab == 0 && !fc.dsort_fused) {            // fused: k_depth_sort_fused has done A5a
     const uint32_t scan_tiles = (fc.n + SCAN_TILE - 1) / SCAN_TILE;   // upper bound (n_visible <= N)
-    const unsigned long long max_tests = (unsigned long long)(bin_chunks_cap - 2) * BIN_CHUNK;
+    const unsigned long long max_tests = bin_max_tests(bin_chunks_cap);
     const uint32_t* sorted_g = b.cvals[sorted_g_idx];
     uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
     TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,

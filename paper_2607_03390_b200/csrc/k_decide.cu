@@ -499,7 +499,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
 // The indices also go to `vis_list`, a copy the depth sort does not permute (SH colours).
 __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __restrict__ pre_cnt, const uint32_t* __restrict__ st_keys,
                                                      const uint32_t* __restrict__ st_vals, uint32_t* __restrict__ vis_keys,
-                                                     uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ vis_list) {
+                                                     uint32_t* __restrict__ vis_vals, uint32_t* __restrict__ vis_list,
+                                                     uint32_t* __restrict__ dsort_H0, uint32_t dsort_tile) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
   const uint32_t num_chunks = (n + PRE_CHUNK - 1) / PRE_CHUNK;
@@ -507,8 +508,11 @@ __global__ void __launch_bounds__(128) k_compact_vis(uint32_t n, const uint2* __
     const uint2 cc = pre_cnt[c];
     for (uint32_t i = threadIdx.x; i < cc.x; i += blockDim.x) {
       const uint32_t g = st_vals[(size_t)c * PRE_CHUNK + i];
-      vis_keys[cc.y + i] = st_keys[(size_t)c * PRE_CHUNK + i];
+      const uint32_t key = st_keys[(size_t)c * PRE_CHUNK + i];
+      vis_keys[cc.y + i] = key;
       vis_vals[cc.y + i] = g; vis_list[cc.y + i] = g;
+      // one-launch depth sort (k_sort.cu): digit counts of its first pass, per sort tile
+      if (dsort_H0) atomicAdd(dsort_H0 + (size_t)((cc.y + i) / dsort_tile) * 256u + (key & 255u), 1u);
     }
   }
 }
@@ -636,7 +640,8 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key, b.rec_uvdo, b.rec_conic,
                                                        b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
-  TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list);
+  TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list,
+             fc.dsort_fused ? b.dsort_H : (uint32_t*)nullptr, depth_sort_fused_tile_items());
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {

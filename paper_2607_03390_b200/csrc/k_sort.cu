@@ -13,6 +13,8 @@
 //
 // Look-back descriptors are (epoch << 34 | flag << 32 | count): tagged with the frame number, never zeroed.
 #include "tgs_internal.cuh"
+#include "bin_params.cuh"
+#include "scan.cuh"
 
 namespace {
 
@@ -255,6 +257,243 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
     cur ^= 1;
   }
   return cur;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Depth sort of the visible Gaussians as ONE launch.  The four onesweep launches above spend 10-14 us
+// each on ~140 co-resident tiles: a launch, a prologue and a look-back chain per digit for 2 MB of data.  Here one
+// persistent grid of at most one CTA per SM keeps the four passes inside one kernel:
+//  * tile t (2048 consecutive items of the current buffer) belongs to CTA t mod gridDim.x for all passes;
+//  * the digit counts of every tile for pass p are the rows of a matrix H[p][tile][256] in global memory.  H[0] is filled
+//    by k_compact_vis (it knows position and key of every item it writes); H[p + 1] is filled by the scatter of pass p,
+//    which knows where each item lands (destination tile = position / 2048) and its next digit: one RED per item.
+//    So a pass needs no counting phase of its own, and the offset of (tile, digit) is the digit's global base (the
+//    histograms k_preprocess accumulates, as before) plus a column sum over the rows of the earlier tiles;
+//  * between two passes all CTAs meet at a grid barrier (all CTAs are resident: the grid is not larger than the number
+//    of SMs and nothing this kernel waits for comes from a later launch).  Rows of H[p] are cleared by their tile's CTA
+//    after the barrier that ends pass p, so the matrices are all zero again when the kernel ends.
+// Data written by other CTAs of this launch are read with ld.global.cg (no stale L1 lines, no non-coherent path).
+// The result (buffer index 0, stable, ties in input order) is bit-identical to launch_sort's.
+namespace {
+
+constexpr int FUSED_IPT = SORT_IPT_SMALL;
+constexpr int FUSED_TILE = SORT_THREADS * FUSED_IPT;
+constexpr int FUSED_CTAS_PER_SM = 2;            // the grid: every CTA is resident (grid barriers)
+constexpr uint32_t FUSED_MLP = 16;             // 16-byte loads in flight per thread in the column sums
+constexpr uint32_t BARRIER_WATCHDOG = 1u << 22;
+
+__device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t expect, uint32_t* error_flag) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(ctr, 1u);
+    uint32_t polls = 0;
+    while (*reinterpret_cast<volatile uint32_t*>(ctr) < expect) {
+      __nanosleep(20);
+      if (++polls > BARRIER_WATCHDOG) { *error_flag = 3; break; }
+    }
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+template <int CTAS_PER_SM>
+__global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(uint32_t* keys0, uint32_t* vals0, uint32_t* keys1, uint32_t* vals1,
+                                                                      const uint32_t* __restrict__ hist, uint32_t* H, uint32_t tiles_cap, Counters* counters,
+                                                                      int exact, uint32_t epoch, const uint2* __restrict__ rec_trect,
+                                                                      const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                                      uint4* __restrict__ bin_params, uint32_t* __restrict__ area_prefix,
+                                                                      uint32_t* __restrict__ chunk_first, unsigned long long* __restrict__ scan_desc,
+                                                                      unsigned long long max_tests, volatile uint32_t* __restrict__ host_overflow) {
+  TGS_PDL_WAIT();
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem<FUSED_IPT>& sm = *reinterpret_cast<SortSmem<FUSED_IPT>*>(smem_raw);
+  const uint32_t n = counters->n_visible;
+  uint32_t* const barrier_ctr = &counters->ticket_sort[0];
+  uint32_t* const error_flag = &counters->error;
+  if (n == 0) {                                                 // uniform over the grid
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters->n_tests = 0; counters->n_pairs = 0; }
+    return;
+  }
+  const uint32_t num_tiles = (n + FUSED_TILE - 1) / FUSED_TILE;
+  const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5, d = threadIdx.x;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = 8 * pass;
+    const uint32_t* kin = (pass & 1) ? keys1 : keys0;
+    const uint32_t* vin = (pass & 1) ? vals1 : vals0;
+    uint32_t* kout = (pass & 1) ? keys0 : keys1;
+    uint32_t* vout = (pass & 1) ? vals0 : vals1;
+    const uint32_t* Hp = H + (size_t)pass * tiles_cap * RADIX;
+    uint32_t* Hn = pass < 3 ? H + (size_t)(pass + 1) * tiles_cap * RADIX : nullptr;
+    {   // exclusive scan of this digit's global histogram (thread d = bin d)
+      const uint32_t h = hist[pass * RADIX + d];
+      uint32_t incl = h;
+#pragma unroll
+      for (int s = 1; s < 32; s <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, s); if (lane >= (uint32_t)s) incl += o; }
+      __syncthreads();
+      if (lane == 31) sm.scan_tmp[wid] = incl;
+      __syncthreads();
+      uint32_t off = incl - h;
+#pragma unroll
+      for (int w = 0; w < SORT_WARPS; ++w) if ((uint32_t)w < wid) off += sm.scan_tmp[w];
+      sm.hbase[d] = off;
+    }
+    for (uint32_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      __syncthreads();
+      for (int i = threadIdx.x; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&sm.warp_hist[0][0])[i] = 0;
+      const uint32_t base = tile * FUSED_TILE + wid * (32 * FUSED_IPT);
+      uint32_t key[FUSED_IPT], val[FUSED_IPT];
+#pragma unroll
+      for (int i = 0; i < FUSED_IPT; ++i) {
+        const uint32_t idx = base + i * 32 + lane;
+        key[i] = idx < n ? __ldcg(kin + idx) : 0xffffffffu;     // padding sorts (stably) behind every real key of the tile
+      }
+#pragma unroll
+      for (int i = 0; i < FUSED_IPT; ++i) {
+        const uint32_t idx = base + i * 32 + lane;
+        val[i] = idx < n ? __ldcg(vin + idx) : 0u;
+      }
+      // Offset of (tile, digit) inside the digit = the counts of the earlier tiles: column sums over the first `tile` rows of
+      // Hp.  64 threads cover a row with 16-byte loads, the four 64-thread groups take every fourth row, 16 loads in flight
+      // per thread; the four partial sums per column meet in shared memory (sm.keys is free until the scatter).
+      {
+        const uint32_t q = threadIdx.x & 63u, r0 = threadIdx.x >> 6;
+        uint4 acc = make_uint4(0u, 0u, 0u, 0u);
+        const uint4* Hq = reinterpret_cast<const uint4*>(Hp) + q;
+        for (uint32_t t0 = r0; t0 < tile; t0 += 4u * FUSED_MLP) {
+          uint4 v[FUSED_MLP];
+#pragma unroll
+          for (uint32_t j = 0; j < FUSED_MLP; ++j) { const uint32_t t = t0 + 4u * j; v[j] = t < tile ? __ldcg(Hq + (size_t)t * (RADIX / 4)) : make_uint4(0u, 0u, 0u, 0u); }
+#pragma unroll
+          for (uint32_t j = 0; j < FUSED_MLP; ++j) { acc.x += v[j].x; acc.y += v[j].y; acc.z += v[j].z; acc.w += v[j].w; }
+        }
+        reinterpret_cast<uint4*>(sm.keys)[r0 * 64u + q] = acc;    // [4][256] partial column sums
+      }
+      __syncthreads();
+      uint32_t rank[FUSED_IPT];
+#pragma unroll
+      for (int i = 0; i < FUSED_IPT; ++i) {
+        const uint32_t dg = (uint32_t)(key[i] >> shift) & 255u;
+        uint32_t m = 0xffffffffu;
+#pragma unroll
+        for (int bit = 0; bit < 8; ++bit) {
+          const bool on = (dg >> bit) & 1u;
+          const uint32_t bal = __ballot_sync(0xffffffffu, on);
+          m &= on ? bal : ~bal;
+        }
+        const uint32_t prev = sm.warp_hist[wid][dg];
+        __syncwarp();
+        if ((m & lt_mask) == 0) sm.warp_hist[wid][dg] = prev + __popc(m);
+        __syncwarp();
+        rank[i] = prev + __popc(m & lt_mask);
+      }
+      __syncthreads();
+      uint32_t cnt = 0;
+#pragma unroll
+      for (int w = 0; w < SORT_WARPS; ++w) { const uint32_t t = sm.warp_hist[w][d]; sm.warp_hist[w][d] = cnt; cnt += t; }
+      uint32_t incl = cnt;
+#pragma unroll
+      for (int s = 1; s < 32; s <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, s); if (lane >= (uint32_t)s) incl += o; }
+      if (lane == 31) sm.scan_tmp[wid] = incl;
+      __syncthreads();
+      uint32_t loff = incl - cnt;
+#pragma unroll
+      for (int w = 0; w < SORT_WARPS; ++w) if ((uint32_t)w < wid) loff += sm.scan_tmp[w];
+      const uint32_t col = sm.keys[d] + sm.keys[256 + d] + sm.keys[512 + d] + sm.keys[768 + d];
+      sm.gbase[d] = sm.hbase[d] + col - loff;
+#pragma unroll
+      for (int w = 0; w < SORT_WARPS; ++w) sm.warp_hist[w][d] += loff;
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < FUSED_IPT; ++i) {
+        const uint32_t dg = (uint32_t)(key[i] >> shift) & 255u;
+        const uint32_t r = rank[i] + sm.warp_hist[wid][dg];
+        sm.keys[r] = key[i];
+        sm.vals[r] = val[i];
+      }
+      __syncthreads();
+      const uint32_t valid = min((uint32_t)FUSED_TILE, n - tile * FUSED_TILE);
+#pragma unroll 4
+      for (int i = 0; i < FUSED_IPT; ++i) {
+        const uint32_t p = i * SORT_THREADS + threadIdx.x;
+        if (p < valid) {
+          const uint32_t k = sm.keys[p];
+          const uint32_t o = sm.gbase[(uint32_t)(k >> shift) & 255u] + p;
+          kout[o] = k;
+          vout[o] = sm.vals[p];
+          if (Hn) atomicAdd(Hn + (size_t)(o / FUSED_TILE) * RADIX + ((k >> (shift + 8)) & 255u), 1u);
+        }
+      }
+    }
+    // the barrier after the last pass only protects H[3] (later tiles may still be summing its columns); a consumer of the
+    // sorted list that lives in this kernel would need it anyway
+    grid_barrier(barrier_ctr, (uint32_t)(pass + 1) * gridDim.x, error_flag);
+    // nobody reads H[pass] any more: every CTA has summed its columns before it arrived
+    for (uint32_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) const_cast<uint32_t*>(Hp)[(size_t)tile * RADIX + d] = 0u;
+  }
+  // ---- A5a on the sorted list (what k_scan_area does in the multi-launch pipeline, k_bin.cu): the records k_bin reads, in
+  // sorted order; area_prefix[i] = tests of the Gaussians before position i; chunk_first[k] = position of the Gaussian that
+  // holds test k * BIN_CHUNK.  One tile = 8 consecutive positions per thread; the prefix across the tiles is a decoupled
+  // look-back over one descriptor per tile (every tile is resident or finished).
+  if (counters->area_sum > max_tests) {                         // the tests do not fit the binning's index space: frame invalid
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters->n_tests = 0; counters->n_pairs = 0; counters->overflow = 1; *host_overflow = 1u; __threadfence_system(); }
+    return;
+  }
+  // Only now may the next kernel of the stream (k_bin) be scheduled: its CTAs would otherwise sit in their
+  // griddepcontrol.wait for this whole kernel and keep the kernels of the side streams (SH colours, T^oc, selection) off the SMs.
+  TGS_PDL_TRIGGER();
+  uint32_t* s_warp = sm.scan_tmp;
+  uint32_t* s_excl = &sm.tile;
+  for (uint32_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    __syncthreads();
+    const uint32_t i0 = tile * FUSED_TILE + threadIdx.x * FUSED_IPT;
+    uint32_t g[FUSED_IPT], a[FUSED_IPT];
+    uint2 r[FUSED_IPT];
+#pragma unroll
+    for (int j = 0; j < FUSED_IPT; ++j) g[j] = i0 + j < n ? __ldcg(vals0 + i0 + j) : 0u;
+#pragma unroll
+    for (int j = 0; j < FUSED_IPT; ++j) r[j] = i0 + j < n ? rec_trect[g[j]] : make_uint2(0u, 0u);
+    uint32_t tsum = 0;
+#pragma unroll
+    for (int j = 0; j < FUSED_IPT; ++j) { a[j] = ((r[j].x >> 16) - (r[j].x & 0xffffu)) * ((r[j].y >> 16) - (r[j].y & 0xffffu)); tsum += a[j]; }
+#pragma unroll
+    for (int j = 0; j < FUSED_IPT; ++j)
+      if (i0 + j < n) store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g[j], r[j], exact != 0, rec_uvdo, rec_conic));
+    uint32_t incl_total;
+    uint32_t off = tgs_scan::chunk_scan<SORT_THREADS>(tsum, tile, scan_desc, s_warp, s_excl, error_flag, &incl_total, epoch);
+    if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
+#pragma unroll
+    for (int j = 0; j < FUSED_IPT; ++j) {
+      if (i0 + j >= n) break;
+      area_prefix[i0 + j] = off;
+      const unsigned long long end = (unsigned long long)off + a[j];
+      for (unsigned long long kb = ((unsigned long long)off + BIN_CHUNK - 1) / BIN_CHUNK; kb * BIN_CHUNK < end; ++kb) chunk_first[kb] = i0 + j;
+      off += a[j];
+    }
+  }
+}
+
+}  // namespace
+
+uint32_t depth_sort_fused_tile_items() { return FUSED_TILE; }
+uint32_t depth_sort_fused_ctas_per_sm() { return FUSED_CTAS_PER_SM; }
+size_t depth_sort_fused_words(uint32_t tiles_cap) { return (size_t)4 * RADIX * (size_t)tiles_cap; }
+
+// The depth sort (result in buffer 0, bit-identical to launch_sort(..., key_bits = 32)) and A5a (k_scan_area) as one launch.
+// b.dsort_H = [4][tiles_cap][256] zeroed counters whose first matrix the producer of the list has filled (k_compact_vis).
+void launch_depth_sort_fused(cudaStream_t s, const FrameConst& fc, DevBuffers& b, unsigned long long max_tests, uint32_t* host_overflow, int num_sms,
+                             uint32_t n_hint) {
+  // one CTA per SM while that gives every tile its own CTA: the second CTA of an SM only becomes resident when the kernels of
+  // the side streams (SH colours) leave it the registers, and every CTA has to arrive at the barriers
+  const uint32_t tiles_hint = (n_hint + FUSED_TILE - 1) / FUSED_TILE + 2;     // a few tiles more only give a few CTAs a second tile
+#define FUSED_LAUNCH(CPS)                                                                                                                                    \
+  TGS_LAUNCH((k_depth_sort_fused<CPS>), num_sms * (CPS), SORT_THREADS, sizeof(SortSmem<FUSED_IPT>), s, b.ckeys[0], b.cvals[0], b.ckeys[1], b.cvals[1],              \
+             (const uint32_t*)b.sort_hist, b.dsort_H, b.dsort_tiles_cap, b.counters, fc.exact_tiles, fc.epoch, (const uint2*)b.rec_trect, (const float4*)b.rec_uvdo, \
+             (const float4*)b.rec_conic, b.bin_params, b.area_prefix, b.chunk_first, (unsigned long long*)b.scan_desc, max_tests, (volatile uint32_t*)host_overflow)
+  if (tiles_hint <= (uint32_t)num_sms) FUSED_LAUNCH(1);      // (the instance without a register cap is also the faster one)
+  else FUSED_LAUNCH(FUSED_CTAS_PER_SM);
+#undef FUSED_LAUNCH
 }
 
 // ------------------------------------------------------------------------------------------------------------------

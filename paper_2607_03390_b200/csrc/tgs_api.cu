@@ -84,6 +84,7 @@ struct tgs_ctx {
   cudaEvent_t ev_bin = nullptr;
   bool bin_pending = false; int bin_slot = 0;
   uint32_t nv_hint = 0;                 // visible Gaussians of a recent frame (selects the depth-sort instance)
+  uint32_t nv_hint_cls[2] = {0, 0};     // the same per frame class (R / P, S): the one-launch depth sort is for lists of one tile per SM
   int last_ftype = -1; uint32_t last_n_tiles = 0;
   bool timing = false;
   bool count_interactions = false;
@@ -92,6 +93,7 @@ struct tgs_ctx {
   cudaEvent_t ev_stage[MAX_EV];
   int ev_tag[MAX_EV]; int n_ev = 0;
   int last_n_slabs = 1;
+  int dsort_mode = -1;                  // -1 automatic (short visible lists), 0 onesweep launches, 1 one-launch depth sort
   int blend_half_mode = -1;             // -1 automatic (small splats: few tests per visible Gaussian), 0 off, 1 on
   bool half_hint = false;
   // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
@@ -375,6 +377,8 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
   A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n) A(b.bin_params, 3 * (size_t)n) A(b.vis_list, n)
   c->dsort_tiles_cap = (n + sort_tile_items() - 1) / sort_tile_items() + 1;
   AZ(b.dsort_desc, (size_t)4 * c->dsort_tiles_cap * 256)
+  AZ(b.dsort_H, depth_sort_fused_words(c->dsort_tiles_cap))
+  b.dsort_tiles_cap = c->dsort_tiles_cap;
 #undef A
 #undef AZ
   const float *d_means = means, *d_scales = scales, *d_quats = quats, *d_opacity = opacity, *d_sh = sh;
@@ -401,7 +405,7 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) { snprintf(c->err, sizeof(c->err), "load: %s", cudaGetErrorString(e)); return TGS_E_CUDA; }
   c->n = n; c->deg = deg; c->K = K;
-  c->nv_hint = n / 4;
+  c->nv_hint = n / 4; c->nv_hint_cls[0] = c->nv_hint_cls[1] = n / 4;
   c->slab_ctl[0] = tgs_ctx::SlabCtl(); c->slab_ctl[1] = tgs_ctx::SlabCtl();
   invalidate_priors(c);
   c->have_frame = false;
@@ -501,7 +505,7 @@ static int render_impl(tgs_ctx* c, int mode) {
   if (c->cnt_pending[ci]) {
     CK(cudaEventSynchronize(c->ev_cnt[ci])); c->cnt_pending[ci] = false;
     const Counters& h2 = *c->h_cnt2[ci];
-    c->nv_hint = h2.n_visible;
+    c->nv_hint = h2.n_visible; c->nv_hint_cls[c->hist_cls[ci]] = h2.n_visible;
     c->half_hint = h2.n_visible > 0 && h2.n_tests < 8ull * h2.n_visible;     // small splats: most records reach one half of a tile only
     if (!h2.overflow && h2.n_tests) {
       tgs_ctx::SlabCtl& sc = c->slab_ctl[c->hist_cls[ci]];
@@ -550,6 +554,10 @@ static int render_impl(tgs_ctx* c, int mode) {
   fc.exact_tiles = c->prm.exact_tiles ? 1 : 0;
   fc.n_tiles = c->TX * c->TY;
   fc.epoch = c->epoch;
+  // the depth sort as one launch (k_sort.cu) where the visible list of this frame class has been short enough for one tile per
+  // resident CTA; longer lists keep the onesweep launches (more CTAs per SM, look-back instead of grid barriers)
+  fc.dsort_fused = c->dsort_mode >= 0 ? c->dsort_mode
+                   : (c->nv_hint_cls[ftype == TGS_FRAME_S ? 1 : 0] <= (uint32_t)c->num_sms * depth_sort_fused_ctas_per_sm() * depth_sort_fused_tile_items() ? 1 : 0);
   fc.blend_half = c->blend_half_mode < 0 ? (c->half_hint ? 1 : 0) : c->blend_half_mode;
   // front-to-back slabs: explicit, or automatic from the size of a recent frame's test space -- small frames
   // are launch bound and stay in one piece
@@ -635,11 +643,15 @@ static int render_impl(tgs_ctx* c, int mode) {
     CK(cudaEventRecord(c->ev_join, c->side2));
   }
   mark(2);                                                                     // 2: A6 level 1
-  const int dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
-                                  &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, c->nv_hint < 1000000u);   // visible Gaussians by depth
+  c->h_ovf[ci] = 0;
+  int dsorted = 0;                                                                                         // visible Gaussians by depth
+  if (fc.dsort_fused)
+    launch_depth_sort_fused(s, fc, b, bin_max_tests(c->bin_chunks_cap), c->h_ovf + ci, c->num_sms, c->nv_hint_cls[ftype == TGS_FRAME_S ? 1 : 0]);
+  else
+    dsorted = launch_sort(s, b.ckeys, b.cvals, &b.counters->n_visible, 32, b.sort_hist, b.dsort_desc, c->dsort_tiles_cap,
+                          &b.counters->ticket_sort[0], &b.counters->error, fc.epoch, c->num_sms, c->nv_hint < 1000000u);
   if (ftype == TGS_FRAME_S && fork) CK(cudaStreamWaitEvent(s, c->ev_sel, 0));                              // join A2 + A4
   // ---- A5-A9, slab by slab (one slab: the plain pipeline)
-  c->h_ovf[ci] = 0;
   int sorted = 0;
   for (int k = 0; k < fc.n_slabs; ++k) {
     mark(3);                                                                   // 3: A5 pairs
@@ -888,6 +900,9 @@ static int debug_run_stage_impl(tgs_ctx* c, const char* st) {
   if (s == "count_interactions_off") { c->count_interactions = false; return TGS_OK; }
   if (s == "force_all_tiles_on") { c->force_all = 1; return TGS_OK; }
   if (s == "force_all_tiles_off") { c->force_all = 0; return TGS_OK; }
+  if (s == "depth_sort_fused_on") { c->dsort_mode = 1; return TGS_OK; }
+  if (s == "depth_sort_fused_off") { c->dsort_mode = 0; return TGS_OK; }
+  if (s == "depth_sort_fused_auto") { c->dsort_mode = -1; return TGS_OK; }
   if (s == "blend_half_on") { c->blend_half_mode = 1; return TGS_OK; }
   if (s == "blend_half_off") { c->blend_half_mode = 0; return TGS_OK; }
   if (s == "blend_half_auto") { c->blend_half_mode = -1; return TGS_OK; }

@@ -50,6 +50,7 @@ struct FrameConst {
   // have all stopped are dropped from the binning of the later slabs.  slab_bound[k] / 1024 = share of the chunks before slab k.
   int blend_half;           // k_blend<.,.,HALF>: per-warp lists of the records that reach the warp's half tile (scenes of small splats)
   int n_slabs;              // 1 .. TGS_MAX_SLABS
+  int dsort_fused;          // the depth sort runs as one launch (k_depth_sort_fused): k_compact_vis fills its first count matrix
   uint32_t slab_bound[TGS_MAX_SLABS + 1];
 };
 
@@ -120,6 +121,8 @@ struct DevBuffers {
   uint32_t* sort_hist = nullptr;      // [1 + TGS_MAX_SLABS][4][256]: depth sort, tile sort of each slab
   uint64_t* sort_desc = nullptr;      // tile sort: [passes][tiles][256] look-back descriptors (epoch-tagged)
   uint64_t* dsort_desc = nullptr;     // depth sort: [4][tiles][256]
+  uint32_t* dsort_H = nullptr;        // one-launch depth sort: [4][tiles][256] digit counts per tile, all zero between frames
+  uint32_t dsort_tiles_cap = 0;       // rows of one of those matrices
   uint64_t* scan_desc = nullptr;      // look-back descriptors of k_scan_area
   uint64_t* bin_desc = nullptr;       //                        k_bin [bin_chunks_cap]
   // tiles
@@ -198,4 +201,11 @@ uint32_t scan_tile_items();
 uint32_t bin_chunk_items();
 uint32_t preprocess_chunk_items();
 int tile_sort_passes(int n_tiles);
+uint32_t depth_sort_fused_tile_items();
+uint32_t depth_sort_fused_ctas_per_sm();
+size_t depth_sort_fused_words(uint32_t tiles_cap);   // size of its count matrices (uint32 words): [4][tiles][256]
+// one launch: depth sort of the visible list (result in buffer 0) + A5a (what k_scan_area does); launch_bin(slab 0) then skips k_scan_area
+void launch_depth_sort_fused(cudaStream_t s, const FrameConst& fc, DevBuffers& b, unsigned long long max_tests, uint32_t* host_overflow, int num_sms,
+                             uint32_t n_hint);   // n_hint: expected length of the list (sizes the grid only)
+unsigned long long bin_max_tests(uint32_t bin_chunks_cap);
 void sort_prepare_device();   // function attributes of the sort kernels on the current device (once per context)

@@ -832,3 +832,87 @@ def test_needle_scene_at_the_conditioning_limit_of_fp32():
     rel = np.abs(dg[ok] - do[ok]) / do[ok]
     print(f"[parity] needle scene: rgb max {err[~border].max():.3g}, depth rel max {rel.max():.3g}, pixels over 1e-4: {(rel > 1e-4).sum()}")
     assert (rel > P.DEPTH_RTOL).sum() <= 3 and rel.max() <= 2e-4
+
+
+# ------------------------------------------------------------------------------------------------ one-launch depth sort
+@pytest.mark.parametrize("case", ["config1", "medium_ragged", "sheets_slabs", "equal_depths"])
+def test_depth_sort_as_one_launch_or_as_onesweep_launches_against_the_oracle(case):
+    """The depth sort of the visible Gaussians + the prefix sums of their test rects run as ONE persistent kernel with grid
+    barriers (k_depth_sort_fused) when the visible list is short -- automatic for every small scene, so the
+    other tests exercise it -- or as four onesweep launches + k_scan_area.  Both must give the oracle's lists bit for bit;
+    here each frame is rendered by two contexts, one per path, and both are compared with the oracle and with each other
+    (R, S and P frames; ragged list lengths; two front-to-back pieces; thousands of equal depth keys, whose order is the
+    Gaussian index, R28)."""
+    P = _p()
+    params = {}
+    if case == "config1":
+        sc = make_config(1, n=16_384, frames=6)
+    elif case == "medium_ragged":
+        sc = _dense_scene(200_000, 500, 281)
+        sc.scales *= 2.0
+    elif case == "sheets_slabs":
+        sc = make_config(5, n=60_000, frames=12, width=333, height=187)
+        sc.scales[:, :2] *= 6.0
+        params = {"depth_slabs": 2}
+    else:
+        sc = make_config(5, n=40_000, frames=6, width=320, height=180)     # sheets seen head-on: ten distinct depths
+        sc.poses[:] = look_at(np.array([0.0, 0.0, -8.0]), np.array([0.0, 0.0, 0.0]), np.array([0.0, -1.0, 0.0]))
+    g, o = P.make_pair(sc, params)
+    h, _ = P.make_pair(sc, params)
+    g.debug_run_stage("depth_sort_fused_on"); h.debug_run_stage("depth_sort_fused_off")
+    for f, mode in ((0, "full"), (1, "temporal"), (2, "pseudo")):
+        if f:
+            P.inject_priors(g, o); P.inject_priors(h, o)
+        for c in (g, h, o):
+            c.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G[mode]); h.render(P.MODE_G[mode]); ft = o.render(P.MODE_O[mode])
+        for c, name in ((g, "one launch"), (h, "onesweep")):
+            if params:
+                P.compare_frame_slabs(c, o, sc.n, ft, label=f"depth sort {name}, {case}")
+            else:
+                P.compare_frame(c, o, sc.n, ft, label=f"depth sort {name}, {case}")
+        for name in ("keys", "vals", "ranges", "tiles_touched"):
+            assert np.array_equal(g.debug_get(name), h.debug_get(name)), name
+        assert np.array_equal(g.read_image(), h.read_image())
+        sg, sh_ = g.get_stats(), h.get_stats()
+        assert sg["n_tests"] == sh_["n_tests"] and sg["n_pairs"] == sh_["n_pairs"]
+    if case == "equal_depths":
+        d = o.get("records")["d"][(o.get("records")["flags"] & ora.VISIBLE) != 0]
+        assert len(np.unique(d)) <= 10 < len(d)
+
+
+def test_depth_sort_as_one_launch_with_several_tiles_per_cta_full_size_config5():
+    """Config 5 at full size: its reference frame has 2 M visible Gaussians = a thousand sort tiles for the 296 resident CTAs
+    of the one-launch depth sort (forced on; the library itself would take the onesweep launches for a list this long), so
+    every CTA walks several tiles per pass and the column sums run over hundreds of rows.  Lists, counts and image must be
+    those of the onesweep path, bit for bit; an empty list (camera turned away) must pass through both."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(5, frames=3)
+    outs = []
+    for mode in ("depth_sort_fused_on", "depth_sort_fused_off"):
+        g = tgs.Context(0)
+        g.load_scene(sc)
+        p = g.default_params(); p.depth_slabs = 1
+        g.set_params(p)
+        g.debug_run_stage(mode)
+        g.set_camera(sc.poses[0], sc.camera)
+        g.render(tgs.FULL)
+        st = g.get_stats()
+        out = [st["n_visible"], st["n_tests"], st["n_pairs"], g.debug_get("keys"), g.debug_get("vals"), g.debug_get("ranges"), g.read_image()]
+        g.set_camera(sc.poses[1], sc.camera)
+        g.render(tgs.TEMPORAL)
+        st = g.get_stats()
+        out += [st["n_visible"], st["n_pairs"], g.debug_get("keys"), g.debug_get("vals"), g.read_image()]
+        away = sc.poses[0].copy(); away[2, :] *= -1.0; away[0, :] *= -1.0          # look the other way: nothing visible
+        g.set_camera(away, sc.camera)
+        g.render(tgs.FULL)
+        st = g.get_stats()
+        out += [st["n_visible"], st["n_pairs"], g.read_image()]
+        outs.append(out)
+        g.destroy()
+    a, b = outs
+    assert a[0] > 1_500_000 and a[2] > 0 and a[7] > 0
+    assert a[12] == 0 and a[13] == 0
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
