@@ -31,6 +31,14 @@ __device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exa
   }
   return P;
 }
+// the same with the two records already loaded (exact tile tests)
+__device__ __forceinline__ GaussParams make_params_loaded(uint32_t g, uint2 r, float4 a, float4 b) {
+  GaussParams P;
+  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
+  P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
+  P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
+  return P;
+}
 __device__ __forceinline__ void store_params(uint4* __restrict__ dst, const GaussParams& P) {
   const uint4* s = reinterpret_cast<const uint4*>(&P);
   dst[0] = s[0]; dst[1] = s[1]; dst[2] = s[2];

@@ -282,17 +282,18 @@ constexpr int FUSED_CTAS_PER_SM = 2;            // the grid: every CTA is reside
 constexpr uint32_t FUSED_MLP = 16;             // 16-byte loads in flight per thread in the column sums
 constexpr uint32_t BARRIER_WATCHDOG = 1u << 22;
 
+// Arrival is a release (the CTA's earlier writes, ordered before it by the bar.sync, are visible to whoever acquires the
+// count), the poll an acquire: no separate fences.
 __device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t expect, uint32_t* error_flag) {
   __syncthreads();
   if (threadIdx.x == 0) {
-    __threadfence();
-    atomicAdd(ctr, 1u);
-    uint32_t polls = 0;
-    while (*reinterpret_cast<volatile uint32_t*>(ctr) < expect) {
-      __nanosleep(20);
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+    uint32_t polls = 0, v;
+    while (true) {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+      if (v >= expect) break;
       if (++polls > BARRIER_WATCHDOG) { *error_flag = 3; break; }
     }
-    __threadfence();
   }
   __syncthreads();
 }
@@ -318,6 +319,11 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(
   const uint32_t num_tiles = (n + FUSED_TILE - 1) / FUSED_TILE;
   const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5, d = threadIdx.x;
   const uint32_t lt_mask = (1u << lane) - 1u;
+  constexpr uint32_t MLP = CTAS_PER_SM == 1 ? 20u : FUSED_MLP;   // 16-byte loads in flight per thread in the column sums (registers permitting)
+  uint32_t hv[4];                                               // the four global digit histograms (thread d = bin d): one round trip, not four
+#pragma unroll
+  for (int p = 0; p < 4; ++p) hv[p] = hist[p * RADIX + d];
+#pragma unroll 1
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 8 * pass;
     const uint32_t* kin = (pass & 1) ? keys1 : keys0;
@@ -327,7 +333,7 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(
     const uint32_t* Hp = H + (size_t)pass * tiles_cap * RADIX;
     uint32_t* Hn = pass < 3 ? H + (size_t)(pass + 1) * tiles_cap * RADIX : nullptr;
     {   // exclusive scan of this digit's global histogram (thread d = bin d)
-      const uint32_t h = hist[pass * RADIX + d];
+      const uint32_t h = pass == 0 ? hv[0] : pass == 1 ? hv[1] : pass == 2 ? hv[2] : hv[3];
       uint32_t incl = h;
 #pragma unroll
       for (int s = 1; s < 32; s <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, incl, s); if (lane >= (uint32_t)s) incl += o; }
@@ -361,12 +367,12 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(
         const uint32_t q = threadIdx.x & 63u, r0 = threadIdx.x >> 6;
         uint4 acc = make_uint4(0u, 0u, 0u, 0u);
         const uint4* Hq = reinterpret_cast<const uint4*>(Hp) + q;
-        for (uint32_t t0 = r0; t0 < tile; t0 += 4u * FUSED_MLP) {
-          uint4 v[FUSED_MLP];
+        for (uint32_t t0 = r0; t0 < tile; t0 += 4u * MLP) {
+          uint4 v[MLP];
 #pragma unroll
-          for (uint32_t j = 0; j < FUSED_MLP; ++j) { const uint32_t t = t0 + 4u * j; v[j] = t < tile ? __ldcg(Hq + (size_t)t * (RADIX / 4)) : make_uint4(0u, 0u, 0u, 0u); }
+          for (uint32_t j = 0; j < MLP; ++j) { const uint32_t t = t0 + 4u * j; v[j] = t < tile ? __ldcg(Hq + (size_t)t * (RADIX / 4)) : make_uint4(0u, 0u, 0u, 0u); }
 #pragma unroll
-          for (uint32_t j = 0; j < FUSED_MLP; ++j) { acc.x += v[j].x; acc.y += v[j].y; acc.z += v[j].z; acc.w += v[j].w; }
+          for (uint32_t j = 0; j < MLP; ++j) { acc.x += v[j].x; acc.y += v[j].y; acc.z += v[j].z; acc.w += v[j].w; }
         }
         reinterpret_cast<uint4*>(sm.keys)[r0 * 64u + q] = acc;    // [4][256] partial column sums
       }
@@ -452,14 +458,40 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(
     uint2 r[FUSED_IPT];
 #pragma unroll
     for (int j = 0; j < FUSED_IPT; ++j) g[j] = i0 + j < n ? __ldcg(vals0 + i0 + j) : 0u;
+    // Every gather depends on g only: the test rects and (exact tile tests) the two records of the first GH Gaussians are
+    // issued together, one round trip instead of three.  Positions behind the end of the list read record 0 and store nothing.
+    constexpr int GH = CTAS_PER_SM == 1 ? FUSED_IPT : FUSED_IPT / 2;      // the instance with a register cap gathers in two halves
+    float4 ua[GH], cb[GH];
 #pragma unroll
-    for (int j = 0; j < FUSED_IPT; ++j) r[j] = i0 + j < n ? rec_trect[g[j]] : make_uint2(0u, 0u);
+    for (int j = 0; j < FUSED_IPT; ++j) r[j] = rec_trect[g[j]];
+    if (exact) {
+#pragma unroll
+      for (int j = 0; j < GH; ++j) { ua[j] = rec_uvdo[g[j]]; cb[j] = rec_conic[g[j]]; }
+    }
     uint32_t tsum = 0;
 #pragma unroll
-    for (int j = 0; j < FUSED_IPT; ++j) { a[j] = ((r[j].x >> 16) - (r[j].x & 0xffffu)) * ((r[j].y >> 16) - (r[j].y & 0xffffu)); tsum += a[j]; }
+    for (int j = 0; j < FUSED_IPT; ++j) {
+      a[j] = i0 + j < n ? ((r[j].x >> 16) - (r[j].x & 0xffffu)) * ((r[j].y >> 16) - (r[j].y & 0xffffu)) : 0u;
+      tsum += a[j];
+    }
+    if (exact) {
 #pragma unroll
-    for (int j = 0; j < FUSED_IPT; ++j)
-      if (i0 + j < n) store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g[j], r[j], exact != 0, rec_uvdo, rec_conic));
+      for (int half = 0; half < FUSED_IPT / GH; ++half) {
+        if (half > 0) {
+#pragma unroll
+          for (int j = 0; j < GH; ++j) { ua[j] = rec_uvdo[g[half * GH + j]]; cb[j] = rec_conic[g[half * GH + j]]; }
+        }
+#pragma unroll
+        for (int j = 0; j < GH; ++j) {
+          const int jj = half * GH + j;
+          if (i0 + jj < n) store_params(bin_params + 3 * (size_t)(i0 + jj), make_params_loaded(g[jj], r[jj], ua[j], cb[j]));
+        }
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < FUSED_IPT; ++j)
+        if (i0 + j < n) store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g[j], r[j], false, rec_uvdo, rec_conic));
+    }
     uint32_t incl_total;
     uint32_t off = tgs_scan::chunk_scan<SORT_THREADS>(tsum, tile, scan_desc, s_warp, s_excl, error_flag, &incl_total, epoch);
     if (tile == num_tiles - 1 && threadIdx.x == 0) { counters->n_tests = incl_total; area_prefix[n] = incl_total; }
