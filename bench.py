@@ -381,7 +381,7 @@ def run_ours(args):
     roof["stages"] = {k: {n: {"ms": round(v["ms"], 5), "bound": v["bound"], "frac": round(v["frac"], 4)} for n, v in d.items()}
                       for k, d in traj["stage_rooflines"].items() if d}
     roof["stages_note"] = ("per-stage times are taken with every kernel on ONE stream (stage events must bracket what they name); the "
-                           "production frame overlaps A2 / A4 / SH colours on side streams, so its ms_per_step is below the stage sum")
+                           "production frame overlaps A2 / A4 / SH colours on side streams, so its ms_per_step is below the stage sum; where the library runs the depth sort as one launch (short visible lists) that launch also builds the flat test space (A5a), which the multi-launch pipeline does at the start of bin_pairs: depth_sort's fraction still counts the sort's bytes only")
 
     fps_tgs, fps_full, fps_e2e = aggregate_fps(world, K, ms_tgs), aggregate_fps(world, K, ms_full), aggregate_fps(world, K, ms_e2e)
     out = {
