@@ -7,7 +7,10 @@
  *
  * General rules
  *  - Every function returns 0 (TGS_OK) on success or a negative tgs_status; no exceptions cross.
- *  - A context is bound to one CUDA device and one stream; it is not thread-safe.
+ *  - A context is bound to one CUDA device and one stream; it is not thread-safe.  Contexts that render on the SAME device
+ *    at the same time (other streams, threads or processes) must switch the one-launch depth sort off
+ *    (tgs_debug_run_stage(ctx, "depth_sort_fused_off")): its grid barriers need all of its CTAs resident, and two such
+ *    kernels could each hold part of the SMs; a watchdog then fails the frame (TGS_E_CUDA) after a few seconds.
  *  - `mem` says where a caller buffer lives: TGS_HOST or TGS_DEVICE (same device as the context).
  *    Input buffers are copied during the call; the caller keeps ownership of everything it passes.
  *  - tgs_render only enqueues work; tgs_read_* / tgs_get_stats / tgs_debug_get with TGS_HOST block until
@@ -99,7 +102,7 @@ typedef struct {
   uint64_t n_pixel_slots;  /* pixel slots issued by the blend loop, dead lanes included (counting on) */
   float ms_stage[8];   /* per-stage device time when timing is on (tgs_debug_run_stage("timing_on")):
                           0 init + warp + fill/correspondence, 1 preprocess + tile selection, 2 depth sort of the visible
-                          Gaussians, 3 pair binning (tile tests, emission), 4 SH colours, 5 tile sort + ranges,
+                          Gaussians (with the prefix sums of their test rects where it runs as one launch), 3 pair binning (tile tests, emission), 4 SH colours, 5 tile sort + ranges,
                           6 blend + stitch, 7 post (F reduction, stats) */
   float ms_total;
   uint64_t device_bytes; /* device memory held by the context */

@@ -518,6 +518,11 @@ void launch_depth_sort_fused(cudaStream_t s, const FrameConst& fc, DevBuffers& b
                              uint32_t n_hint) {
   // one CTA per SM while that gives every tile its own CTA: the second CTA of an SM only becomes resident when the kernels of
   // the side streams (SH colours) leave it the registers, and every CTA has to arrive at the barriers
+  // (A cooperative launch, which would make the driver start the grid only when all of it fits, was tried: with
+  // cudaLaunchAttributeCooperative the kernel read a visible count of zero on this driver, with or without the programmatic
+  // launch attribute, so the plain launch stays.  Within a context nothing can keep these CTAs off the SMs for good; two
+  // contexts rendering on one device at the same time could each hold part of the SMs -- the barrier's watchdog then flags
+  // the frame (TGS_E_CUDA from tgs_get_stats) instead of hanging.  include/tgs.h says so.)
   const uint32_t tiles_hint = (n_hint + FUSED_TILE - 1) / FUSED_TILE + 2;     // a few tiles more only give a few CTAs a second tile
 #define FUSED_LAUNCH(CPS)                                                                                                                                    \
   TGS_LAUNCH((k_depth_sort_fused<CPS>), num_sms * (CPS), SORT_THREADS, sizeof(SortSmem<FUSED_IPT>), s, b.ckeys[0], b.cvals[0], b.ckeys[1], b.cvals[1],              \

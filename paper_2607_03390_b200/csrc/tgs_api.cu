@@ -771,7 +771,7 @@ int tgs_get_stats(tgs_ctx* c, tgs_stats* out) {
     }
     if (c->n_ev >= 2) cudaEventElapsedTime(&out->ms_total, c->ev_stage[0], c->ev_stage[c->n_ev - 1]);
   }
-  if (h.error) { snprintf(c->err, sizeof(c->err), "device watchdog: look-back stalled (code %u)", h.error); return TGS_E_CUDA; }
+  if (h.error) { snprintf(c->err, sizeof(c->err), "device watchdog: a look-back (code 1: prefix scan, 2: radix sort) or the grid barrier of the one-launch depth sort (3) stalled (code %u)", h.error); return TGS_E_CUDA; }
   if (h.overflow) return TGS_E_CAPACITY;
   return TGS_OK;
 }
