@@ -916,3 +916,26 @@ def test_depth_sort_as_one_launch_with_several_tiles_per_cta_full_size_config5()
     assert a[12] == 0 and a[13] == 0
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("n", [1, 2047, 2048, 2049, 3 * 2048, 5 * 2048 + 17])
+def test_depth_sort_as_one_launch_list_lengths_at_the_tile_boundaries(n):
+    """Every Gaussian of a compact cloud is visible, so the list the one-launch depth sort gets has exactly n entries: one short of,
+    exactly at and one over a 2048-key tile, whole tiles only, several tiles with a ragged tail, a single key."""
+    P = _p()
+    sc = make_config(1, n=max(n, 8), frames=3)
+    if n < 8:
+        for name in ("means", "scales", "quats", "opacity", "sh"):
+            setattr(sc, name, np.ascontiguousarray(getattr(sc, name)[:n]))
+    sc.means *= np.float32(0.25)
+    sc.opacity[:] = np.clip(sc.opacity, 0.2, 0.95)
+    g, o = P.make_pair(sc)
+    g.debug_run_stage("depth_sort_fused_on")
+    for f, mode in ((0, "full"), (1, "temporal")):
+        if f:
+            P.inject_priors(g, o)
+        g.set_camera(sc.poses[f], sc.camera); o.set_camera(sc.poses[f], sc.camera)
+        g.render(P.MODE_G[mode]); ft = o.render(P.MODE_O[mode])
+        sg, so, _ = P.compare_frame(g, o, sc.n, ft, label=f"one-launch depth sort, n = {n}")
+        if f == 0:
+            assert sg["n_visible"] == n
