@@ -98,7 +98,7 @@ struct tgs_ctx {
   bool half_hint = false;
   // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
   // recent one-piece and two-piece frames; slabs are used where they drop more than half of the pairs
-  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0; bool asked1 = false, asked2 = false; } slab_ctl[2];
+  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0, tests_probe = 0; bool asked1 = false, asked2 = false, two = false; } slab_ctl[2];
   int hist_cls[2] = {0, 0}, hist_slabs[2] = {1, 1};   // class and number of slabs of the frame that last used each counter block
   FrameConst fc;
 };
@@ -566,17 +566,32 @@ static int render_impl(tgs_ctx* c, int mode) {
     if (ns == 0) {
       // Two pieces pay where most tiles finish inside the first one: then the second piece bins and sorts next to nothing.
       // Where the tiles stay alive (thin surfaces, clouds with gaps) the second piece only adds launches and the parking
-      // of the pixel states.  Measured, not guessed: pairs per test of the latest one-piece and two-piece frames of this
-      // class, the other variant re-probed every 32 frames; small frames are launch bound and stay in one piece.
-      tgs_ctx::SlabCtl& sc = c->slab_ctl[ftype == TGS_FRAME_S ? 1 : 0];
+      // of the pixel states.  Measured, not guessed: p1, p2 = pairs per test of the latest one-piece and two-piece frames of
+      // this class (R / P, S); two pieces where p2 < 0.4 p1 (config 3, per 20-frame segment of the trajectory: two pieces are
+      // the faster choice up to a ratio of 0.35 and the slower one from 0.46 on); small frames are launch bound and stay in one piece.
+      //  * With two pieces p2 is fresh every frame and p1 is not needed again: it is a property of the tile test, not of the
+      //    occlusion (0.57-0.63 over the whole trajectory), so no one-piece frame is rendered just to re-measure it.
+      //  * With one piece p2 goes stale; two pieces are probed again (one frame) every 32 frames of the class -- every 8
+      //    while the other class runs two pieces far below its threshold --, or as soon as the test space has grown by a
+      //    quarter since the last probe.
+      const int cls = ftype == TGS_FRAME_S ? 1 : 0;
+      tgs_ctx::SlabCtl& sc = c->slab_ctl[cls];
+      const tgs_ctx::SlabCtl& other = c->slab_ctl[1 - cls];
       if (!sc.asked1) { ns = 1; sc.asked1 = true; }                               // a one-piece sample ...
-      else if (sc.tests < 2000000u) ns = 1;                                       // (small, or nothing known yet)
-      else if (!sc.asked2) { ns = 2; sc.asked2 = true; }                          // ... then ONE two-piece probe ...
+      else if (sc.tests < 2000000u) { ns = 1; sc.two = false; }                   // (small, or nothing known yet)
+      else if (!sc.asked2) { ns = 2; sc.asked2 = true; sc.tests_probe = sc.tests; sc.since_probe = 0; }   // ... then ONE two-piece probe ...
       else if (sc.p1 < 0.0f || sc.p2 < 0.0f) ns = 1;                              // ... and one piece until both have been counted
       else {
-        const int prefer = sc.p2 < 0.5f * sc.p1 ? 2 : 1;
-        ns = prefer;
-        if (++sc.since_probe >= 32) { ns = 3 - prefer; sc.since_probe = 0; }
+        sc.two = sc.p2 < 0.4f * sc.p1;
+        ns = sc.two ? 2 : 1;
+        ++sc.since_probe;
+        if (!sc.two) {
+          const bool hinted = other.two && other.p2 < 0.3f * other.p1;
+          const bool grown = (unsigned long long)sc.tests * 4ull > (unsigned long long)sc.tests_probe * 5ull;
+          if (sc.since_probe >= 32 || (sc.since_probe >= 8 && hinted) || (sc.since_probe >= 4 && grown)) {
+            ns = 2; sc.since_probe = 0; sc.tests_probe = sc.tests;
+          }
+        }
       }
     }
     static const uint32_t def_split[TGS_MAX_SLABS + 1][3] = {{0, 0, 0}, {0, 0, 0}, {256, 0, 0}, {160, 448, 0}, {96, 256, 512}};

@@ -738,7 +738,7 @@ def test_depth_slabs_outputs_match_oracle_and_single_pass(slabs, split):
 def test_depth_slabs_auto_full_size_config3_and_5():
     """The launch configuration bench.py times (depth_slabs = 0: automatic) at full size.  The library learns from its own
     statistics (two frames late) whether two pieces drop enough pairs: two reference frames in one piece, one probing
-    two pieces, then the decision (pairs per test halved or not), which must be stable.  On the poses used here (config 3
+    two pieces, then the decision (pairs per test below 0.4 of the one-piece figure or not), which must be stable.  On the poses used here (config 3
     from inside the dense core, config 5's sheets) two pieces are kept.  A two-piece reference frame and a two-piece
     TemporalGS frame, every output against the oracle."""
     P = _p()
@@ -752,7 +752,7 @@ def test_depth_slabs_auto_full_size_config3_and_5():
         for _ in range(8):
             g.render(tgs.FULL); st = g.get_stats(); used.append(st["n_slabs"]); pairs.append(st["n_pairs"])
         assert used == [1, 1, 2, 1, 2, 2, 2, 2], (used, pairs)       # one piece, ONE probe of two pieces, one piece until counted, decision
-        assert pairs[2] < 0.5 * pairs[0] and pairs[0] == o.stats()["n_pairs"]
+        assert pairs[2] < 0.4 * pairs[0] and pairs[0] == o.stats()["n_pairs"]
         sg, so, out = P.compare_frame_slabs(g, o, sc.n, ora.FRAME_R, label=f"config {cfg} full size, auto slabs", **FULL_SIZE_BOUNDS[cfg])
         P.inject_priors(g, o)
         g.set_camera(sc.poses[f0 + 2], sc.camera); o.set_camera(sc.poses[f0 + 2], sc.camera)
