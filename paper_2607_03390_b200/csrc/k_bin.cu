@@ -245,23 +245,27 @@ __global__ void __launch_bounds__(BIN_THREADS, sizeof(TileT) == 2 ? BIN_CTAS_PER
         for (uint32_t i = tid; i < nq; i += BIN_THREADS) dst[i] = src[i];
       }
       __syncthreads();
+      bool chunk_alive = true;
       if (LATER) {
         // Later slabs: most tiles have finished.  A Gaussian whose test rect holds no live tile -- four look-ups in the
         // summed-area table of the live tiles (k_live_sat) -- has all its tests skipped without looking at them.
         const uint32_t mm = m < (uint32_t)BIN_PCAP ? m : (uint32_t)BIN_PCAP;
         const uint32_t SW = (uint32_t)TX + 1u;
+        bool alive_here = m > (uint32_t)BIN_PCAP;                  // Gaussians beyond the staged ones are not looked up: alive
         for (uint32_t l = tid; l < mm; l += BIN_THREADS) {
           GaussParams& Gp = sm.gp[l];
           const uint32_t x0 = Gp.lo & 0xffffu, y0 = Gp.lo >> 16, w = Gp.w, h = (sm.prefix[l + 1] - sm.prefix[l]) / (w ? w : 1u);
           const uint32_t cnt = (live_sat[(y0 + h) * SW + x0 + w] - live_sat[y0 * SW + x0 + w]) - (live_sat[(y0 + h) * SW + x0] - live_sat[y0 * SW + x0]);
           Gp.pad = cnt ? 0u : 1u;                                  // pad = 1: dead
+          alive_here = alive_here || cnt != 0u;
         }
-        __syncthreads();
+        // a chunk none of whose Gaussians can reach a live tile (most chunks of a later slab) is not enumerated at all
+        chunk_alive = __syncthreads_or(alive_here ? 1 : 0) != 0;
       }
       // -------------------------------------------------------------- tests
       const uint32_t t0 = cbase + tid * BIN_IPT;
       uint32_t mask = 0, tl[BIN_IPT], gg[BIN_IPT];
-      if (t0 < tend) {
+      if (t0 < tend && (!LATER || chunk_alive)) {
         uint32_t lo = 0, hi = m;                                   // largest li with prefix[li] <= t0
         while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.prefix[mid] <= t0) lo = mid; else hi = mid; }
         uint32_t li = lo, end, rx, ry, x_lo, y_lo;
