@@ -98,7 +98,12 @@ struct tgs_ctx {
   bool half_hint = false;
   // automatic choice of the number of slabs (depth_slabs = 0), per frame class (0: R / P, 1: S): pairs per test measured on
   // recent one-piece and two-piece frames; slabs are used where they drop more than half of the pairs
-  struct SlabCtl { float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0, tests_probe = 0; bool asked1 = false, asked2 = false, two = false; } slab_ctl[2];
+  struct SlabCtl {
+    float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0, tests_probe = 0; bool asked1 = false, asked2 = false, two = false;
+    uint32_t split = 256, split_floor = 64; int hold = 0;      // first piece in 1/1024 of the test space (automatic mode), see tgs_render
+  } slab_ctl[2];
+  uint32_t cur_split = 0;               // automatic split of the frame being enqueued (0: not automatic)
+  uint32_t hist_split[2] = {0, 0};      // split of the frame that last used each counter block (0: not the automatic one)
   int hist_cls[2] = {0, 0}, hist_slabs[2] = {1, 1};   // class and number of slabs of the frame that last used each counter block
   FrameConst fc;
 };
@@ -514,6 +519,26 @@ static int render_impl(tgs_ctx* c, int mode) {
       if (c->hist_slabs[ci] == 1) sc.p1 = ratio;
       else if (c->hist_slabs[ci] == 2) {
         sc.p2 = ratio;
+        // Where the first piece ends (automatic mode only).  The fastest split is the smallest one that leaves the second
+        // piece next to nothing (config 3, per class and 40-frame segment: 128 ... 512 of 1024, always the smallest with
+        // pairs(2nd) / pairs(1st) ~ 0); below it the second piece has to enumerate the rest of the test space for the tiles
+        // that are still alive, and the frame time rises steeply.  So: shrink by 1/8 per frame of the class while the
+        // second piece stays empty, step back up by 1/4 as soon as it does not, and then leave the split alone for 24 frames
+        // of the class and never go below what just failed.  Only statistics of a frame rendered with the CURRENT split count.
+        if (c->hist_split[ci] != 0 && c->hist_split[ci] == sc.split) {
+          const float r = (float)h2.n_pairs_slab[1] / (float)(h2.n_pairs_slab[0] ? h2.n_pairs_slab[0] : 1u);
+          // (growing only helps where it makes tiles finish: stacks of thin sheets keep half of their tiles alive whatever
+          // the split -- config 5 -- and are left at the default)
+          const bool tiles_finish = (unsigned long long)h2.n_finished[0] * 10ull >= (unsigned long long)h2.n_sel * 6ull;
+          if (r > 0.03f && tiles_finish) {
+            sc.split_floor = sc.split + sc.split / 16 < 768u ? sc.split + sc.split / 16 : 768u;
+            sc.split = sc.split + sc.split / 4 < 768u ? sc.split + sc.split / 4 : 768u;
+            sc.hold = 24;
+          } else if (r < 0.005f && sc.hold == 0) {
+            const uint32_t next = sc.split - sc.split / 8;
+            sc.split = next > sc.split_floor ? next : sc.split_floor;
+          }
+        }
       }
     }
     // grow the automatic capacity when a frame came close to it (the slabs' lists are never longer than the tests)
@@ -597,8 +622,17 @@ static int render_impl(tgs_ctx* c, int mode) {
     static const uint32_t def_split[TGS_MAX_SLABS + 1][3] = {{0, 0, 0}, {0, 0, 0}, {256, 0, 0}, {160, 448, 0}, {96, 256, 512}};
     fc.n_slabs = ns;
     fc.slab_bound[0] = 0;
+    uint32_t auto_split = 0;
+    if (c->prm.depth_slabs == 0 && ns == 2 && !c->prm.slab_split[0]) {
+      tgs_ctx::SlabCtl& sc = c->slab_ctl[ftype == TGS_FRAME_S ? 1 : 0];
+      if (!sc.two) { sc.split = 256; sc.split_floor = 64; sc.hold = 0; }       // a probe from one-piece mode starts over
+      else if (sc.hold > 0) { if (--sc.hold == 0) sc.split_floor = 64; }   // (a floor that only decays was tried: the best split of config 3 falls from 256 to 128 within 80 frames, and the floor kept it from following)
+      auto_split = sc.split;
+    }
+    c->cur_split = auto_split;
     for (int i = 1; i < ns; ++i) {
       uint32_t v = c->prm.slab_split[i - 1] ? c->prm.slab_split[i - 1] : def_split[ns][i - 1];
+      if (auto_split) v = auto_split;
       if (v < fc.slab_bound[i - 1]) v = fc.slab_bound[i - 1];
       fc.slab_bound[i] = v;
     }
@@ -725,7 +759,7 @@ static int render_impl(tgs_ctx* c, int mode) {
   else if (ftype == TGS_FRAME_P) { c->sched.since_ref = 0; c->sched.force_P = 0; }
   ++c->sched.since_R; ++c->sched.since_ref;
   c->last_ftype = ftype; c->last_n_tiles = (uint32_t)fc.n_tiles; c->last_n_slabs = fc.n_slabs;
-  c->hist_cls[ci] = ftype == TGS_FRAME_S ? 1 : 0; c->hist_slabs[ci] = fc.n_slabs;
+  c->hist_cls[ci] = ftype == TGS_FRAME_S ? 1 : 0; c->hist_slabs[ci] = fc.n_slabs; c->hist_split[ci] = c->cur_split;
   c->have_frame = true;
   return TGS_OK;
 }
