@@ -939,3 +939,25 @@ def test_depth_sort_as_one_launch_list_lengths_at_the_tile_boundaries(n):
         sg, so, _ = P.compare_frame(g, o, sc.n, ft, label=f"one-launch depth sort, n = {n}")
         if f == 0:
             assert sg["n_visible"] == n
+
+
+def test_depth_slabs_auto_split_follows_the_empty_second_piece_full_size_config3():
+    """Automatic mode, config 3 at full size from the middle of its trajectory (pose 100: every tile finishes well inside the first
+    quarter of the tests).  Once two pieces are chosen the library moves the end of the first piece down while the second piece stays
+    empty: the first piece must get shorter frame after frame, the second must stay next to nothing, and the
+    frame rendered with the split it ends up with must match the oracle like any other."""
+    P = _p()
+    tgs = _tgs()
+    sc = make_config(3, frames=101)
+    g, o = P.make_pair(sc, {"depth_slabs": 0})
+    g.set_camera(sc.poses[100], sc.camera); o.set_camera(sc.poses[100], sc.camera)
+    o.render(ora.FULL)
+    used, first, second = [], [], []
+    for _ in range(14):
+        g.render(tgs.FULL); st = g.get_stats()
+        used.append(st["n_slabs"]); first.append(st["n_pairs_slab"][0]); second.append(st["n_pairs_slab"][1])
+    assert used[:4] == [1, 1, 2, 1] and all(u == 2 for u in used[4:]), used
+    assert first[-1] < 0.75 * first[4], (first, second)            # the split has come down from a quarter of the tests
+    assert all(b <= a for a, b in zip(first[4:], first[5:])), first   # and never went up on the way: the second piece stayed empty
+    assert max(second[4:]) <= 0.03 * first[-1], (first, second)
+    P.compare_frame_slabs(g, o, sc.n, ora.FRAME_R, label="config 3 full size, pose 100, automatic split", **FULL_SIZE_BOUNDS[3])
