@@ -101,6 +101,7 @@ struct tgs_ctx {
   struct SlabCtl {
     float p1 = -1.0f, p2 = -1.0f; int since_probe = 0; uint32_t tests = 0, tests_probe = 0; bool asked1 = false, asked2 = false, two = false;
     uint32_t split = 256, split_floor = 64; int hold = 0;      // first piece in 1/1024 of the test space (automatic mode), see tgs_render
+    bool empty2 = false; int probe_k = 0;                      // the second piece of the latest two-piece frame was (nearly) empty; probes cycle through 256 / 384 / 512
   } slab_ctl[2];
   uint32_t cur_split = 0;               // automatic split of the frame being enqueued (0: not automatic)
   uint32_t hist_split[2] = {0, 0};      // split of the frame that last used each counter block (0: not the automatic one)
@@ -527,6 +528,7 @@ static int render_impl(tgs_ctx* c, int mode) {
         // of the class and never go below what just failed.  Only statistics of a frame rendered with the CURRENT split count.
         if (c->hist_split[ci] != 0 && c->hist_split[ci] == sc.split) {
           const float r = (float)h2.n_pairs_slab[1] / (float)(h2.n_pairs_slab[0] ? h2.n_pairs_slab[0] : 1u);
+          sc.empty2 = r < 0.03f && sc.split <= 576u;
           // (growing only helps where it makes tiles finish: stacks of thin sheets keep half of their tiles alive whatever
           // the split -- config 5 -- and are left at the default)
           const bool tiles_finish = (unsigned long long)h2.n_finished[0] * 10ull >= (unsigned long long)h2.n_sel * 6ull;
@@ -607,7 +609,8 @@ static int render_impl(tgs_ctx* c, int mode) {
       else if (!sc.asked2) { ns = 2; sc.asked2 = true; sc.tests_probe = sc.tests; sc.since_probe = 0; }   // ... then ONE two-piece probe ...
       else if (sc.p1 < 0.0f || sc.p2 < 0.0f) ns = 1;                              // ... and one piece until both have been counted
       else {
-        sc.two = sc.p2 < 0.4f * sc.p1;
+        // two pieces where they drop 60 % of the pairs, or where a first piece of at most 9/16 of the tests leaves the second one empty
+        sc.two = sc.p2 < 0.4f * sc.p1 || sc.empty2;
         ns = sc.two ? 2 : 1;
         ++sc.since_probe;
         if (!sc.two) {
@@ -625,7 +628,10 @@ static int render_impl(tgs_ctx* c, int mode) {
     uint32_t auto_split = 0;
     if (c->prm.depth_slabs == 0 && ns == 2 && !c->prm.slab_split[0]) {
       tgs_ctx::SlabCtl& sc = c->slab_ctl[ftype == TGS_FRAME_S ? 1 : 0];
-      if (!sc.two) { sc.split = 256; sc.split_floor = 64; sc.hold = 0; }       // a probe from one-piece mode starts over
+      if (!sc.two) {                                                           // a probe from one-piece mode: a quarter, three eighths, half of the tests in turn
+        static const uint32_t probe_split[3] = {256, 384, 512};
+        sc.split = probe_split[sc.probe_k++ % 3]; sc.split_floor = 64; sc.hold = 0;
+      }
       else if (sc.hold > 0) { if (--sc.hold == 0) sc.split_floor = 64; }   // (a floor that only decays was tried: the best split of config 3 falls from 256 to 128 within 80 frames, and the floor kept it from following)
       auto_split = sc.split;
     }
