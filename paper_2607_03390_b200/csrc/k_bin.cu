@@ -400,9 +400,15 @@ uint32_t bin_chunk_items() { return BIN_CHUNK; }
 // One CTA: a thread per tile row (prefix along x), then a thread per column (prefix along y); 8 K entries at 1080p, built
 // in shared memory (SMEM = true; grids beyond 48 KB fall back to global memory) and copied out coalesced.
 template <bool SMEM>
-__global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_t* __restrict__ live_bits, uint32_t* __restrict__ sat) {
+__global__ void __launch_bounds__(1024) k_live_sat(int TX, int TY, const uint32_t* __restrict__ live_bits, uint32_t* __restrict__ sat,
+                                                   const Counters* __restrict__ counters, int slab) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
+  {   // every selected tile finished in the earlier slabs (the usual case once the split has settled): k_bin will not look at the table
+    uint32_t fin = 0;
+    for (int j = 0; j < slab; ++j) fin += counters->n_finished[j];
+    if (fin >= counters->n_sel) return;
+  }
   extern __shared__ uint32_t s_sat[];
   uint32_t* const w = SMEM ? s_sat : sat;
   const int SW = TX + 1;
@@ -448,8 +454,8 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
   }
   if (slab > 0) {
     const size_t sat_bytes = (size_t)(fc.cam.TX + 1) * (fc.cam.TY + 1) * sizeof(uint32_t);
-    if (sat_bytes <= 48 * 1024) TGS_LAUNCH((k_live_sat<true>), 1, 1024, sat_bytes, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
-    else TGS_LAUNCH((k_live_sat<false>), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat);
+    if (sat_bytes <= 48 * 1024) TGS_LAUNCH((k_live_sat<true>), 1, 1024, sat_bytes, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat, (const Counters*)b.counters, slab);
+    else TGS_LAUNCH((k_live_sat<false>), 1, 1024, 0, s, fc.cam.TX, fc.cam.TY, (const uint32_t*)b.live_bits, b.live_sat, (const Counters*)b.counters, slab);
   }
   uint32_t* hist = b.sort_hist + (1 + slab) * 4 * 256;
 #define BIN_LAUNCH(T, CPS, LATER_, ALL_)                                                                                              \
