@@ -31,6 +31,20 @@ __device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exa
   }
   return P;
 }
+// the same from the 32-byte record k_preprocess writes for A5a (rec_bin: {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)});
+// *area = tests of the Gaussian
+__device__ __forceinline__ GaussParams make_params_bin(uint32_t g, float4 r0, float4 r1, bool exact, uint32_t* area) {
+  const uint32_t rx = __float_as_uint(r1.z), ry = __float_as_uint(r1.w);
+  GaussParams P;
+  P.g = g; P.lo = (rx & 0xffffu) | ((ry & 0xffffu) << 16); P.w = (rx >> 16) - (rx & 0xffffu); P.pad = 0;
+  *area = P.w * ((ry >> 16) - (ry & 0xffffu));
+  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
+  if (exact) {
+    P.u = r0.x; P.v = r0.y; P.A = r0.z; P.B = r0.w; P.C = r1.x; P.tau = r1.y;
+    P.kC = -r0.w * __frcp_rn(r1.x); P.kA = -r0.w * __frcp_rn(r0.z);
+  }
+  return P;
+}
 // the same with the two records already loaded (exact tile tests)
 __device__ __forceinline__ GaussParams make_params_loaded(uint32_t g, uint2 r, float4 a, float4 b) {
   GaussParams P;

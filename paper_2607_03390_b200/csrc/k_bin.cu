@@ -34,9 +34,8 @@ constexpr int BIN_PCAP = 192;           // Gaussians of a chunk staged in shared
 // area_prefix[i] = number of tests of the Gaussians before position i of the sorted visible list (area_prefix[n] =
 // all tests); chunk_first[k] = position of the Gaussian that contains test k * BIN_CHUNK.
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const uint32_t* __restrict__ sorted_g,
-                                                            const uint2* __restrict__ rec_rect, unsigned long long* __restrict__ desc,
+                                                            const float4* __restrict__ rec_bin, unsigned long long* __restrict__ desc,
                                                             uint32_t* __restrict__ area_prefix, uint32_t* __restrict__ chunk_first,
-                                                            const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
                                                             uint4* __restrict__ bin_params,
                                                             Counters* __restrict__ counters, unsigned long long max_tests,
                                                             volatile uint32_t* __restrict__ host_overflow) {
@@ -65,9 +64,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_area(FrameConst fc, const
       a[j] = 0;
       if (i0 + j < n) {
         const uint32_t g = sorted_g[i0 + j];
-        const uint2 r = rec_rect[g];
-        a[j] = ((r.x >> 16) - (r.x & 0xffffu)) * ((r.y >> 16) - (r.y & 0xffffu));
-        store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g, r, fc.exact_tiles != 0, rec_uvdo, rec_conic));
+        const float4 r0 = rec_bin[2 * (size_t)g], r1 = rec_bin[2 * (size_t)g + 1];      // one 32-byte sector per Gaussian
+        store_params(bin_params + 3 * (size_t)(i0 + j), make_params_bin(g, r0, r1, fc.exact_tiles != 0, &a[j]));
       }
     }
     uint32_t tsum = 0;
@@ -449,8 +447,8 @@ void launch_bin(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_
     const unsigned long long max_tests = bin_max_tests(bin_chunks_cap);
     const uint32_t* sorted_g = b.cvals[sorted_g_idx];
     uint32_t grid = scan_tiles < (uint32_t)(num_sms * 4) ? scan_tiles : (uint32_t)(num_sms * 4);
-    TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, b.rec_trect, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
-                                                        b.rec_uvdo, b.rec_conic, b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
+    TGS_LAUNCH((k_scan_area), grid ? grid : 1, SCAN_THREADS, 0, s, fc, sorted_g, (const float4*)b.rec_bin, (unsigned long long*)b.scan_desc, b.area_prefix, b.chunk_first,
+                                                        b.bin_params, b.counters, max_tests, (volatile uint32_t*)host_overflow);
   }
   if (slab > 0) {
     const size_t sat_bytes = (size_t)(fc.cam.TX + 1) * (fc.cam.TY + 1) * sizeof(uint32_t);

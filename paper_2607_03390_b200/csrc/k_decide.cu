@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
                                                                const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
                                                                const uint32_t* __restrict__ F_key,
                                                                float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
-                                                               uint2* __restrict__ rec_rect, uint2* __restrict__ rec_trect,
+                                                               uint2* __restrict__ rec_rect, uint2* __restrict__ rec_trect, float4* __restrict__ rec_bin,
                                                                uint32_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
@@ -403,6 +403,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
         else { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }
       }
       rec_trect[g] = make_uint2(tx_lo | (tx_hi << 16), ty_lo | (ty_hi << 16));
+      rec_bin[2 * (size_t)g] = make_float4(u, v, A, B);           // what A5a gathers behind the depth sort, in one sector
+      rec_bin[2 * (size_t)g + 1] = make_float4(C, tau, __uint_as_float(tx_lo | (tx_hi << 16)), __uint_as_float(ty_lo | (ty_hi << 16)));
       const uint32_t area = (tx_hi - tx_lo) * (ty_hi - ty_lo);
       st_area += area;
       rec_uvdo[g] = make_float4(u, v, tz, opac);
@@ -638,7 +640,7 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key, b.rec_uvdo, b.rec_conic,
-                                                       b.rec_rect, b.rec_trect, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
+                                                       b.rec_rect, b.rec_trect, b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
   TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list,
              fc.dsort_fused ? b.dsort_H : (uint32_t*)nullptr, depth_sort_fused_tile_items());

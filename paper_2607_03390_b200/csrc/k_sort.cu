@@ -301,8 +301,7 @@ __device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t expect, uin
 template <int CTAS_PER_SM>
 __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(uint32_t* keys0, uint32_t* vals0, uint32_t* keys1, uint32_t* vals1,
                                                                       const uint32_t* __restrict__ hist, uint32_t* H, uint32_t tiles_cap, Counters* counters,
-                                                                      int exact, uint32_t epoch, const uint2* __restrict__ rec_trect,
-                                                                      const float4* __restrict__ rec_uvdo, const float4* __restrict__ rec_conic,
+                                                                      int exact, uint32_t epoch, const float4* __restrict__ rec_bin,
                                                                       uint4* __restrict__ bin_params, uint32_t* __restrict__ area_prefix,
                                                                       uint32_t* __restrict__ chunk_first, unsigned long long* __restrict__ scan_desc,
                                                                       unsigned long long max_tests, volatile uint32_t* __restrict__ host_overflow) {
@@ -454,43 +453,20 @@ __global__ void __launch_bounds__(SORT_THREADS, CTAS_PER_SM) k_depth_sort_fused(
   for (uint32_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
     __syncthreads();
     const uint32_t i0 = tile * FUSED_TILE + threadIdx.x * FUSED_IPT;
+    // everything A5a needs of a Gaussian is one 32-byte record (rec_bin, k_preprocess): one sector per Gaussian, all eight
+    // fetched together; positions behind the end of the list read record 0 and store nothing
     uint32_t g[FUSED_IPT], a[FUSED_IPT];
-    uint2 r[FUSED_IPT];
 #pragma unroll
     for (int j = 0; j < FUSED_IPT; ++j) g[j] = i0 + j < n ? __ldcg(vals0 + i0 + j) : 0u;
-    // Every gather depends on g only: the test rects and (exact tile tests) the two records of the first GH Gaussians are
-    // issued together, one round trip instead of three.  Positions behind the end of the list read record 0 and store nothing.
-    constexpr int GH = CTAS_PER_SM == 1 ? FUSED_IPT : FUSED_IPT / 2;      // the instance with a register cap gathers in two halves
-    float4 ua[GH], cb[GH];
+    float4 r0[FUSED_IPT], r1[FUSED_IPT];
 #pragma unroll
-    for (int j = 0; j < FUSED_IPT; ++j) r[j] = rec_trect[g[j]];
-    if (exact) {
-#pragma unroll
-      for (int j = 0; j < GH; ++j) { ua[j] = rec_uvdo[g[j]]; cb[j] = rec_conic[g[j]]; }
-    }
+    for (int j = 0; j < FUSED_IPT; ++j) { r0[j] = rec_bin[2 * (size_t)g[j]]; r1[j] = rec_bin[2 * (size_t)g[j] + 1]; }
     uint32_t tsum = 0;
 #pragma unroll
     for (int j = 0; j < FUSED_IPT; ++j) {
-      a[j] = i0 + j < n ? ((r[j].x >> 16) - (r[j].x & 0xffffu)) * ((r[j].y >> 16) - (r[j].y & 0xffffu)) : 0u;
+      const GaussParams P = make_params_bin(g[j], r0[j], r1[j], exact != 0, &a[j]);
+      if (i0 + j < n) store_params(bin_params + 3 * (size_t)(i0 + j), P); else a[j] = 0u;
       tsum += a[j];
-    }
-    if (exact) {
-#pragma unroll
-      for (int half = 0; half < FUSED_IPT / GH; ++half) {
-        if (half > 0) {
-#pragma unroll
-          for (int j = 0; j < GH; ++j) { ua[j] = rec_uvdo[g[half * GH + j]]; cb[j] = rec_conic[g[half * GH + j]]; }
-        }
-#pragma unroll
-        for (int j = 0; j < GH; ++j) {
-          const int jj = half * GH + j;
-          if (i0 + jj < n) store_params(bin_params + 3 * (size_t)(i0 + jj), make_params_loaded(g[jj], r[jj], ua[j], cb[j]));
-        }
-      }
-    } else {
-#pragma unroll
-      for (int j = 0; j < FUSED_IPT; ++j)
-        if (i0 + j < n) store_params(bin_params + 3 * (size_t)(i0 + j), make_params(g[j], r[j], false, rec_uvdo, rec_conic));
     }
     uint32_t incl_total;
     uint32_t off = tgs_scan::chunk_scan<SORT_THREADS>(tsum, tile, scan_desc, s_warp, s_excl, error_flag, &incl_total, epoch);
@@ -526,8 +502,8 @@ void launch_depth_sort_fused(cudaStream_t s, const FrameConst& fc, DevBuffers& b
   const uint32_t tiles_hint = (n_hint + FUSED_TILE - 1) / FUSED_TILE + 2;     // a few tiles more only give a few CTAs a second tile
 #define FUSED_LAUNCH(CPS)                                                                                                                                    \
   TGS_LAUNCH((k_depth_sort_fused<CPS>), num_sms * (CPS), SORT_THREADS, sizeof(SortSmem<FUSED_IPT>), s, b.ckeys[0], b.cvals[0], b.ckeys[1], b.cvals[1],              \
-             (const uint32_t*)b.sort_hist, b.dsort_H, b.dsort_tiles_cap, b.counters, fc.exact_tiles, fc.epoch, (const uint2*)b.rec_trect, (const float4*)b.rec_uvdo, \
-             (const float4*)b.rec_conic, b.bin_params, b.area_prefix, b.chunk_first, (unsigned long long*)b.scan_desc, max_tests, (volatile uint32_t*)host_overflow)
+             (const uint32_t*)b.sort_hist, b.dsort_H, b.dsort_tiles_cap, b.counters, fc.exact_tiles, fc.epoch, (const float4*)b.rec_bin,                                     \
+             b.bin_params, b.area_prefix, b.chunk_first, (unsigned long long*)b.scan_desc, max_tests, (volatile uint32_t*)host_overflow)
   if (tiles_hint <= (uint32_t)num_sms) FUSED_LAUNCH(1);      // (the instance without a register cap is also the faster one)
   else FUSED_LAUNCH(FUSED_CTAS_PER_SM);
 #undef FUSED_LAUNCH
