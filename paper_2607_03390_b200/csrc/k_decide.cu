@@ -186,8 +186,7 @@ __device__ __forceinline__ void mark_oc_tile(const CamConst& k, float u, float v
 
 // Newly visible Gaussians with rects of more than 4 tiles (queued by k_preprocess): one CTA per Gaussian, threads
 // over the tiles of the rect (a near Gaussian covers thousands).  Stops as soon as every tile carries the mark.
-__global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_uvdo,
-                                                 const float4* __restrict__ rec_conic, const uint2* __restrict__ rec_rect,
+__global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* __restrict__ nv_queue, const float4* __restrict__ rec_bin,
                                                  uint32_t* __restrict__ tile_flags, Counters* __restrict__ counters) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
@@ -196,8 +195,9 @@ __global__ void __launch_bounds__(128) k_mark_oc(FrameConst fc, const uint32_t* 
   for (uint32_t j = blockIdx.x; j < nq; j += gridDim.x) {
     if (*reinterpret_cast<volatile uint32_t*>(&counters->n_oc_marked) >= (uint32_t)fc.n_tiles) break;
     const uint32_t g = nv_queue[j];
-    const float4 r0 = rec_uvdo[g], r1 = rec_conic[g];
-    const uint2 r = rec_rect[g];
+    const float4 q0 = rec_bin[2 * (size_t)g], q1 = rec_bin[2 * (size_t)g + 1];      // {u, v, A, B}, {C, tau, test rect}: one sector
+    const float4 r0 = make_float4(q0.x, q0.y, 0.0f, 0.0f), r1 = make_float4(q0.z, q0.w, q1.x, q1.y);
+    const uint2 r = make_uint2(__float_as_uint(q1.z), __float_as_uint(q1.w));
     const uint32_t x_lo = r.x & 0xffffu, x_hi = r.x >> 16, y_lo = r.y & 0xffffu, y_hi = r.y >> 16;
     const uint32_t w = x_hi - x_lo, area = w * (y_hi - y_lo);
     for (uint32_t i = threadIdx.x; i < area; i += blockDim.x) {
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
                                                                const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
                                                                const uint32_t* __restrict__ F_key,
                                                                float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
-                                                               uint2* __restrict__ rec_rect, uint2* __restrict__ rec_trect, float4* __restrict__ rec_bin,
+                                                               uint2* __restrict__ rec_rect, float4* __restrict__ rec_bin,
                                                                uint32_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
@@ -402,7 +402,6 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
         if (nx_hi > nx_lo && ny_hi > ny_lo) { tx_lo = nx_lo; tx_hi = nx_hi; ty_lo = ny_lo; ty_hi = ny_hi; }
         else { tx_hi = x_lo + 1u; ty_hi = y_lo + 1u; }
       }
-      rec_trect[g] = make_uint2(tx_lo | (tx_hi << 16), ty_lo | (ty_hi << 16));
       rec_bin[2 * (size_t)g] = make_float4(u, v, A, B);           // what A5a gathers behind the depth sort, in one sector
       rec_bin[2 * (size_t)g + 1] = make_float4(C, tau, __uint_as_float(tx_lo | (tx_hi << 16)), __uint_as_float(ty_lo | (ty_hi << 16)));
       const uint32_t area = (tx_hi - tx_lo) * (ty_hi - ty_lo);
@@ -640,14 +639,14 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key, b.rec_uvdo, b.rec_conic,
-                                                       b.rec_rect, b.rec_trect, b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
+                                                       b.rec_rect, b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
   TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list,
              fc.dsort_fused ? b.dsort_H : (uint32_t*)nullptr, depth_sort_fused_tile_items());
 }
 
 void launch_mark_oc(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
-  TGS_LAUNCH((k_mark_oc), num_sms * 8, 128, 0, s, fc, b.nv_queue, b.rec_uvdo, b.rec_conic, b.rec_trect, b.tile_flags, b.counters);
+  TGS_LAUNCH((k_mark_oc), num_sms * 8, 128, 0, s, fc, b.nv_queue, (const float4*)b.rec_bin, b.tile_flags, b.counters);
 }
 
 void launch_select(cudaStream_t s, const FrameConst& fc, DevBuffers& b, uint32_t* host_n_sel) {

@@ -96,7 +96,6 @@ struct DevBuffers {
   float4* rec_conic = nullptr;   // [N] {A,B,C,tau}
   uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16: tiles of the 3-sigma extent (R3)
   float4* rec_bin = nullptr;     // [N][2] {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)}: everything A5a gathers per visible Gaussian, in ONE 32-byte sector
-  uint2* rec_trect = nullptr;    // [N] same layout: the sub-rect whose tiles are tested / can hold pairs (k_preprocess)
   uint32_t* rec_flags = nullptr; // [N]
   float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
   // blend-side parameters (values, not decisions): alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, which is
