@@ -19,19 +19,7 @@ struct alignas(16) GaussParams {
 };
 static_assert(sizeof(GaussParams) == 48, "three uint4 per Gaussian");
 
-__device__ __forceinline__ GaussParams make_params(uint32_t g, uint2 r, bool exact, const float4* __restrict__ rec_uvdo,
-                                                   const float4* __restrict__ rec_conic) {
-  GaussParams P;
-  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
-  P.u = P.v = P.A = P.B = P.C = P.kC = P.kA = 0.0f; P.tau = 0.0f;
-  if (exact) {
-    const float4 a = rec_uvdo[g], b = rec_conic[g];
-    P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
-    P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
-  }
-  return P;
-}
-// the same from the 32-byte record k_preprocess writes for A5a (rec_bin: {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)});
+// from the 32-byte record k_preprocess writes for A5a (rec_bin: {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)});
 // *area = tests of the Gaussian
 __device__ __forceinline__ GaussParams make_params_bin(uint32_t g, float4 r0, float4 r1, bool exact, uint32_t* area) {
   const uint32_t rx = __float_as_uint(r1.z), ry = __float_as_uint(r1.w);
@@ -43,14 +31,6 @@ __device__ __forceinline__ GaussParams make_params_bin(uint32_t g, float4 r0, fl
     P.u = r0.x; P.v = r0.y; P.A = r0.z; P.B = r0.w; P.C = r1.x; P.tau = r1.y;
     P.kC = -r0.w * __frcp_rn(r1.x); P.kA = -r0.w * __frcp_rn(r0.z);
   }
-  return P;
-}
-// the same with the two records already loaded (exact tile tests)
-__device__ __forceinline__ GaussParams make_params_loaded(uint32_t g, uint2 r, float4 a, float4 b) {
-  GaussParams P;
-  P.g = g; P.lo = (r.x & 0xffffu) | ((r.y & 0xffffu) << 16); P.w = (r.x >> 16) - (r.x & 0xffffu); P.pad = 0;
-  P.u = a.x; P.v = a.y; P.A = b.x; P.B = b.y; P.C = b.z; P.tau = b.w;
-  P.kC = -b.y * __frcp_rn(b.z); P.kA = -b.y * __frcp_rn(b.x);
   return P;
 }
 __device__ __forceinline__ void store_params(uint4* __restrict__ dst, const GaussParams& P) {

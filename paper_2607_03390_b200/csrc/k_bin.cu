@@ -384,9 +384,9 @@ __global__ void __launch_bounds__(256) k_count_pairs(const uint32_t* __restrict_
 
 // test-only: the 64-bit sort keys tile << 32 | bits(depth) of the sorted pair list
 __global__ void __launch_bounds__(256) k_keys64(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
-                                                const float4* __restrict__ rec_uvdo, uint32_t n, uint64_t* __restrict__ out) {
+                                                const float4* __restrict__ rec_b1, uint32_t n, uint64_t* __restrict__ out) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = ((uint64_t)keys[i] << 32) | __float_as_uint(rec_uvdo[vals[i]].z);
+  if (i < n) out[i] = ((uint64_t)keys[i] << 32) | __float_as_uint(rec_b1[vals[i]].z);
 }
 
 }  // namespace
@@ -492,6 +492,20 @@ void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t 
   if (n_pairs) k_count_pairs<<<(n_pairs + 255) / 256, 256, 0, s>>>(b.vals[sorted_idx], n_pairs, b.tiles_touched);
 }
 
+// test-only: the decision records the oracle reports per Gaussian, {u, v, d, o} (which = 0) or {A, B, C, tau} (which = 1), put
+// together from what the path keeps (rec_bin {u, v, A, B | C, tau, ..}, rec_b1 {.., .., d, o}); entries of Gaussians that are
+// not visible in the current frame are stale
+__global__ void __launch_bounds__(256) k_debug_record(uint32_t n, int which, const float4* __restrict__ rec_bin, const float4* __restrict__ rec_b1,
+                                                      float4* __restrict__ out) {
+  const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  const float4 q0 = rec_bin[2 * (size_t)g], q1 = rec_bin[2 * (size_t)g + 1], b1 = rec_b1[g];
+  out[g] = which == 0 ? make_float4(q0.x, q0.y, b1.z, b1.w) : make_float4(q0.z, q0.w, q1.x, q1.y);
+}
+void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int which, float4* out) {
+  if (n) k_debug_record<<<(n + 255) / 256, 256, 0, s>>>(n, which, (const float4*)b.rec_bin, (const float4*)b.rec_b1, out);
+}
+
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out) {
-  if (n) k_keys64<<<(n + 255) / 256, 256, 0, s>>>(b.keys[sorted_idx], b.vals[sorted_idx], b.rec_uvdo, n, out);
+  if (n) k_keys64<<<(n + 255) / 256, 256, 0, s>>>(b.keys[sorted_idx], b.vals[sorted_idx], b.rec_b1, n, out);
 }

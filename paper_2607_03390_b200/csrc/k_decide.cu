@@ -244,7 +244,6 @@ struct PreSmem {
 __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
                                                                const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
                                                                const uint32_t* __restrict__ F_key,
-                                                               float4* __restrict__ rec_uvdo, float4* __restrict__ rec_conic,
                                                                uint2* __restrict__ rec_rect, float4* __restrict__ rec_bin,
                                                                uint32_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
@@ -406,12 +405,10 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       rec_bin[2 * (size_t)g + 1] = make_float4(C, tau, __uint_as_float(tx_lo | (tx_hi << 16)), __uint_as_float(ty_lo | (ty_hi << 16)));
       const uint32_t area = (tx_hi - tx_lo) * (ty_hi - ty_lo);
       st_area += area;
-      rec_uvdo[g] = make_float4(u, v, tz, opac);
-      rec_conic[g] = make_float4(A, B, C, tau);
       rec_rect[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
       // blend-side parameters: the quadratic form as a sum of two squares (no cancellation between its terms)
       rec_b0[g] = make_float4(u, v, -0.72134752f * A, -b / cc);
-      rec_b1[g] = make_float4(-0.72134752f / cc, log2f(opac), tz, 0.0f);
+      rec_b1[g] = make_float4(-0.72134752f / cc, log2f(opac), tz, opac);           // (.w is not read by the blend: the decision record {u, v, d, o | A, B, C, tau} the tests ask for is rec_bin + rec_b1.zw)
       sm.list[i] = (uint16_t)(e | 0x4000u);
       sm.depth[i] = __float_as_uint(tz);
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)
@@ -573,7 +570,7 @@ __global__ void __launch_bounds__(1024) k_select(FrameConst fc, const uint32_t* 
 // ------------------------------------------------------------------ F_min / F_max over G_rendered (L109) + |G_rendered|
 // Only visible Gaussians can have been blended: the reduction runs over the visible list, not over all N.
 __global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint32_t* __restrict__ vis_vals, const uint8_t* __restrict__ rendered_now,
-                                                 const float4* __restrict__ rec_uvdo, uint32_t* __restrict__ F_key,
+                                                 const float4* __restrict__ rec_bin, uint32_t* __restrict__ F_key,
                                                  Counters* __restrict__ counters, int update_F) {
   TGS_PDL_WAIT();
   TGS_PDL_TRIGGER();
@@ -584,7 +581,7 @@ __global__ void __launch_bounds__(256) k_frustum(FrameConst fc, const uint32_t* 
     if (!rendered_now[g]) continue;
     ++cnt;
     if (update_F) {
-      const float4 r = rec_uvdo[g];
+      const float4 r = rec_bin[2 * (size_t)g];                       // {u, v, A, B}
       const float nx = (2.0f * r.x + 1.0f) / fc.cam.Wf - 1.0f, ny = (2.0f * r.y + 1.0f) / fc.cam.Hf - 1.0f;
       const uint32_t kx = f2key(nx), ky = f2key(ny);
       kmin_x = min(kmin_x, kx); kmax_x = max(kmax_x, kx); kmin_y = min(kmin_y, ky); kmax_y = max(kmax_y, ky);
@@ -638,7 +635,7 @@ void launch_fill_corr(cudaStream_t s, const FrameConst& fc, DevBuffers& b) {
 void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int num_sms) {
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
-  TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key, b.rec_uvdo, b.rec_conic,
+  TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key,
                                                        b.rec_rect, b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
   TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list,
@@ -664,5 +661,5 @@ void launch_export_counters(cudaStream_t s, const DevBuffers& b, Counters* host)
 }
 
 void launch_frustum(cudaStream_t s, const FrameConst& fc, DevBuffers& b, const uint32_t* vis_vals, const uint8_t* rendered_now, bool update_F) {
-  TGS_LAUNCH((k_frustum), 296, 256, 0, s, fc, vis_vals, rendered_now, b.rec_uvdo, b.F_key, b.counters, update_F ? 1 : 0);
+  TGS_LAUNCH((k_frustum), 296, 256, 0, s, fc, vis_vals, rendered_now, (const float4*)b.rec_bin, b.F_key, b.counters, update_F ? 1 : 0);
 }

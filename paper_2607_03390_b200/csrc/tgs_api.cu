@@ -51,6 +51,7 @@ struct tgs_ctx {
   uint32_t epoch = 0;          // frame number, tag of the look-back descriptors
   uint64_t* keys64 = nullptr;  // test-only scratch of tgs_debug_get("keys")
   uint2* ranges_dec = nullptr; // test-only scratch of tgs_debug_get("ranges")
+  float4* dbg_rec = nullptr;   // test-only scratch of tgs_debug_get("rec_uvdo" / "rec_conic")
   uint64_t device_bytes = 0;
   DevBuffers b;
   std::vector<void*> allocs_scene, allocs_frame, allocs_pairs;
@@ -372,12 +373,13 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
                           !finite_all(opacity, n) || !finite_all(sh, (size_t)n * K * 3))) return TGS_E_INVALID_ARG;
   CK(cudaStreamSynchronize(c->stream));
   free_list(c, c->allocs_scene);
+  c->dbg_rec = nullptr;
   DevBuffers& b = c->b;
   c->n = 0;
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
 #define AZ(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene, true)) return r;
   A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
-  A(b.rec_uvdo, n) A(b.rec_conic, n) A(b.rec_rect, n) A(b.rec_bin, 2 * (size_t)n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
+  A(b.rec_rect, n) A(b.rec_bin, 2 * (size_t)n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, n) A(b.rec_b1, n)
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
   A(b.pre_cnt, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
   A(b.ckeys[0], n) A(b.ckeys[1], (size_t)n + preprocess_chunk_items()) A(b.cvals[0], n) A(b.cvals[1], (size_t)n + preprocess_chunk_items()) A(b.nv_queue, n) A(b.bin_params, 3 * (size_t)n) A(b.vis_list, n)
@@ -866,8 +868,11 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
     }
     return 16;
   }
-  else if (name == "rec_uvdo") { src = b.rec_uvdo; have = N * 16; }
-  else if (name == "rec_conic") { src = b.rec_conic; have = N * 16; }
+  else if (name == "rec_uvdo" || name == "rec_conic") {      // not stored as such: put together from rec_bin / rec_b1
+    if (!c->dbg_rec && N) { if (int r = dev_alloc(c, &c->dbg_rec, N, c->allocs_scene)) return r; }
+    launch_debug_record(c->stream, b, (uint32_t)N, name == "rec_conic" ? 1 : 0, c->dbg_rec);
+    src = c->dbg_rec; have = N * 16;
+  }
   else if (name == "rec_rect") { src = b.rec_rect; have = N * 8; }
   else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
   else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }

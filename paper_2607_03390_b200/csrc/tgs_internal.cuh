@@ -92,8 +92,6 @@ struct DevBuffers {
   float4* g2 = nullptr;          // [N][2] {Sxx,Sxy,Sxz,Syy},{Syz,Szz,opacity,tau = 2 ln(255 o)}: read by survivors of the culls
   float* sh = nullptr;           // [N][K][3]
   // per-Gaussian records of the current frame
-  float4* rec_uvdo = nullptr;    // [N] {u,v,d,o}
-  float4* rec_conic = nullptr;   // [N] {A,B,C,tau}
   uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16: tiles of the 3-sigma extent (R3)
   float4* rec_bin = nullptr;     // [N][2] {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)}: everything A5a gathers per visible Gaussian, in ONE 32-byte sector
   uint32_t* rec_flags = nullptr; // [N]
@@ -192,6 +190,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms, bool small_input, uint2* ranges = nullptr);   // ranges: A7 fused into the last pass ({~start, end} per key)
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
+void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int which, float4* out);   // test-only: {u,v,d,o} / {A,B,C,tau} per Gaussian
 void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n_pairs, uint32_t n);   // test-only
 void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out);   // test-only: {~start, end} -> {start, end}
 void launch_blend(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int sorted_idx, int out_idx,
