@@ -506,6 +506,14 @@ void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int wh
   if (n) k_debug_record<<<(n + 255) / 256, 256, 0, s>>>(n, which, (const float4*)b.rec_bin, (const float4*)b.rec_b1, out);
 }
 
+__global__ void __launch_bounds__(256) k_debug_flags(uint32_t n, const uint8_t* __restrict__ flags, uint32_t* __restrict__ out) {
+  const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < n) out[g] = flags[g];
+}
+void launch_debug_flags(cudaStream_t s, const DevBuffers& b, uint32_t n, uint32_t* out) {
+  if (n) k_debug_flags<<<(n + 255) / 256, 256, 0, s>>>(n, (const uint8_t*)b.rec_flags, out);
+}
+
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out) {
   if (n) k_keys64<<<(n + 255) / 256, 256, 0, s>>>(b.keys[sorted_idx], b.vals[sorted_idx], b.rec_b1, n, out);
 }

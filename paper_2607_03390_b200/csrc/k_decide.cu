@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
                                                                const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
                                                                const uint32_t* __restrict__ F_key,
                                                                uint2* __restrict__ rec_rect, float4* __restrict__ rec_bin,
-                                                               uint32_t* __restrict__ rec_flags,
+                                                               uint8_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
                                                                uint32_t* __restrict__ vis_keys,
@@ -321,9 +321,10 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       surv |= (1u | fl) << (2 * j);
       asm volatile("prefetch.global.L2 [%0];" ::"l"(g2 + 2 * (size_t)g));   // phase B reads the covariance of this survivor
     }
-    if (g0 + PRE_IPT <= fc.n) *reinterpret_cast<uint4*>(rec_flags + g0) = make_uint4(cf[0], cf[1], cf[2], cf[3]);
+    // one byte per Gaussian (the flags fit in seven bits): 4 N bytes a frame less to write than with words
+    if (g0 + PRE_IPT <= fc.n) *reinterpret_cast<uchar4*>(rec_flags + g0) = make_uchar4((uint8_t)cf[0], (uint8_t)cf[1], (uint8_t)cf[2], (uint8_t)cf[3]);
     else
-      for (int j = 0; j < PRE_IPT; ++j) if (g0 + j < fc.n) rec_flags[g0 + j] = cf[j];
+      for (int j = 0; j < PRE_IPT; ++j) if (g0 + j < fc.n) rec_flags[g0 + j] = (uint8_t)cf[j];
     // survivors -> sm.list, in ascending index order
     const uint32_t ns_t = (surv & 1u) + ((surv >> 2) & 1u) + ((surv >> 4) & 1u) + ((surv >> 6) & 1u);
     uint32_t incl = ns_t;
@@ -370,7 +371,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       const float b = (T10 * a0 + T11 * a1) + T12 * a2;
       const float cc = ((T10 * q0 + T11 * q1) + T12 * q2) + 0.3f;
       const float det = a * cc - b * b;
-      if (!(det > 0.0f)) { rec_flags[g] = TGS_CULL_DEGENERATE; ++st_deg; continue; }
+      if (!(det > 0.0f)) { rec_flags[g] = (uint8_t)TGS_CULL_DEGENERATE; ++st_deg; continue; }
       const float A = cc / det, B = -b / det, C = a / det;
       const float mid = 0.5f * (a + cc);
       const float lam = mid + sqrtf(fmaxf(0.1f, mid * mid - det));
@@ -380,8 +381,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       const uint32_t x_hi = (uint32_t)fminf(fmaxf(floorf((u + rad + 15.0f) / 16.0f), 0.0f), TXf);
       const uint32_t y_lo = (uint32_t)fminf(fmaxf(floorf((v - rad) / 16.0f), 0.0f), TYf);
       const uint32_t y_hi = (uint32_t)fminf(fmaxf(floorf((v + rad + 15.0f) / 16.0f), 0.0f), TYf);
-      if (!(x_hi > x_lo && y_hi > y_lo)) { rec_flags[g] = TGS_CULL_EMPTY; ++st_empty; continue; }
-      rec_flags[g] = fl | TGS_VISIBLE;
+      if (!(x_hi > x_lo && y_hi > y_lo)) { rec_flags[g] = (uint8_t)TGS_CULL_EMPTY; ++st_empty; continue; }
+      rec_flags[g] = (uint8_t)(fl | TGS_VISIBLE);
       if (fl) ++st_nv;
       // Test rect (never a different decision): the tiles of the 3-sigma rect that can reach alpha >= 1/255 lie inside the
       // bounding box of the ellipse q <= tau, |dx| <= sqrt(tau a), |dy| <= sqrt(tau c) (min over dy of q = dx^2 / a).  A tile

@@ -874,7 +874,11 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
     src = c->dbg_rec; have = N * 16;
   }
   else if (name == "rec_rect") { src = b.rec_rect; have = N * 8; }
-  else if (name == "rec_flags") { src = b.rec_flags; have = N * 4; }
+  else if (name == "rec_flags") {                            // stored as bytes, reported as words
+    if (!c->dbg_rec && N) { if (int r = dev_alloc(c, &c->dbg_rec, N, c->allocs_scene)) return r; }
+    launch_debug_flags(c->stream, b, (uint32_t)N, reinterpret_cast<uint32_t*>(c->dbg_rec));
+    src = c->dbg_rec; have = N * 4;
+  }
   else if (name == "rec_rgb") { src = b.rec_rgb; have = N * 16; }
   else if (name == "tiles_touched") {
     if (!c->have_frame) return TGS_E_INVALID_ARG;
