@@ -386,7 +386,7 @@ __global__ void __launch_bounds__(256) k_count_pairs(const uint32_t* __restrict_
 __global__ void __launch_bounds__(256) k_keys64(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
                                                 const float4* __restrict__ rec_b1, uint32_t n, uint64_t* __restrict__ out) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = ((uint64_t)keys[i] << 32) | __float_as_uint(rec_b1[vals[i]].z);
+  if (i < n) out[i] = ((uint64_t)keys[i] << 32) | __float_as_uint(rec_b1[2 * (size_t)vals[i]].z);
 }
 
 }  // namespace
@@ -499,7 +499,7 @@ __global__ void __launch_bounds__(256) k_debug_record(uint32_t n, int which, con
                                                       float4* __restrict__ out) {
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
-  const float4 q0 = rec_bin[2 * (size_t)g], q1 = rec_bin[2 * (size_t)g + 1], b1 = rec_b1[g];
+  const float4 q0 = rec_bin[2 * (size_t)g], q1 = rec_bin[2 * (size_t)g + 1], b1 = rec_b1[2 * (size_t)g];
   out[g] = which == 0 ? make_float4(q0.x, q0.y, b1.z, b1.w) : make_float4(q0.z, q0.w, q1.x, q1.y);
 }
 void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int which, float4* out) {

@@ -306,7 +306,7 @@ __global__ void __launch_bounds__(BLEND_THREADS, MARK ? BLEND_MIN_CTAS - 1 : BLE
       for (int s = 0; s < IDS_PER_THREAD; ++s) {
         const uint32_t j = tid + s * BLEND_THREADS;
         if (gid[s] != 0xffffffffu) {
-          cp_async16(&B.a[j], rec_b0 + gid[s]); cp_async16(&B.b[j], rec_b1 + gid[s]); cp_async16(&B.c[j], rec_rgb + gid[s]);
+          cp_async16(&B.a[j], rec_b0 + 2 * (size_t)gid[s]); cp_async16(&B.b[j], rec_b1 + 2 * (size_t)gid[s]); cp_async16(&B.c[j], rec_rgb + gid[s]);   // b0 / b1 interleaved: one sector
           B.id[j] = gid[s];
           if (MARK) B.contrib[j] = 0;
         } else {

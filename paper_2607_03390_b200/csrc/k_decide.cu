@@ -408,8 +408,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       st_area += area;
       rec_rect[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
       // blend-side parameters: the quadratic form as a sum of two squares (no cancellation between its terms)
-      rec_b0[g] = make_float4(u, v, -0.72134752f * A, -b / cc);
-      rec_b1[g] = make_float4(-0.72134752f / cc, log2f(opac), tz, opac);           // (.w is not read by the blend: the decision record {u, v, d, o | A, B, C, tau} the tests ask for is rec_bin + rec_b1.zw)
+      rec_b0[2 * (size_t)g] = make_float4(u, v, -0.72134752f * A, -b / cc);        // b0 / b1 interleaved: one 32-byte sector per Gaussian, written whole
+      rec_b1[2 * (size_t)g] = make_float4(-0.72134752f / cc, log2f(opac), tz, opac);           // (.w is not read by the blend: the decision record {u, v, d, o | A, B, C, tau} the tests ask for is rec_bin + rec_b1.zw)
       sm.list[i] = (uint16_t)(e | 0x4000u);
       sm.depth[i] = __float_as_uint(tz);
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)

@@ -98,8 +98,8 @@ struct DevBuffers {
   float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
   // blend-side parameters (values, not decisions): alpha = exp2(A' t^2 + D' dy^2 + log2 o), t = dx + k dy, which is
   // -1/2 delta^T Sigma'^-1 delta completed to a sum of two squares: A' = -log2e/2 * c/det, k = -b/c, D' = -log2e/2 / c
-  float4* rec_b0 = nullptr;      // [N] {u, v, A', k}
-  float4* rec_b1 = nullptr;      // [N] {D', log2 o, d, -}
+  float4* rec_b0 = nullptr;      // [N][2] blend record, interleaved: rec_b0[2 g] = {u, v, A', k},
+  float4* rec_b1 = nullptr;      //        rec_b1[2 g] = rec_b0[2 g + 1] = {D', log2 o, d, o} (one 32-byte sector per Gaussian)
   uint32_t* tiles_touched = nullptr;  // [N] pairs emitted per Gaussian (test-only: filled by tgs_debug_get)
   uint8_t* rendered = nullptr;        // [N] G_rendered of the priors (L103)
   uint8_t* rendered_next = nullptr;   // [N] being built by an R / P frame
