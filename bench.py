@@ -33,9 +33,9 @@ METRIC = "rendered FPS over trajectory (3M Gaussians, 1080p); speed-up vs full r
 # the any-pixel-composited test and the select of d_ref).
 BLEND_LANE_INSTR = 14.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one one-piece k_blend<1,0,0,0> launch on config 3, from the ncu --set full capture
-# summarised in profiles/r2v_top_kernels.md (the file names the command); per launch, like `achieved`.
-BLEND_DRAM_TRAFFIC_BYTES = 47.4e6
-BLEND_DRAM_TRAFFIC_SOURCE = "ncu --set full capture of one-piece k_blend<1,0,0,0> launches on config 3 (profiles/r2v_top_kernels.md: 46.4-47.4 MB), not re-measured by this run"
+# summarised in profiles/r2z_top_kernels.md (the file names the command); per launch, like `achieved`.
+BLEND_DRAM_TRAFFIC_BYTES = 35.8e6
+BLEND_DRAM_TRAFFIC_SOURCE = "ncu --set full capture of one-piece k_blend<1,0,0,0> launches on config 3 (profiles/r2z_top_kernels.md: 35.0-35.8 MB), not re-measured by this run"
 # Lane-instructions the pair binning needs: per (Gaussian, tile) test the tile coordinates and box (8), the
 # selection bit (4), centre-in-box (5), four box edges of the conic form at the clamped optimum (4 x 12) and the margin
 # compare (3) = 68; per emitted pair the rank, the staging and the two stores (12).
