@@ -159,7 +159,7 @@ def stage_rooflines(stats, sc, hbm_gbs, alu_peak):
     init_bytes = (32.0 * px if ftype == 2 else float(sc.n)) + 25.0 * T_
     rows = {
         "init_warp_fill": ("hbm", init_bytes / 1e9, "GB"),
-        "preprocess_select": ("hbm", (sc.n * (16 + 1) + Nv * (32 + 16 + 81)) / 1e9, "GB"),   # g2 + TGB lookups; written per visible Gaussian: A5a record 32, blend record 32, rect 8, flag 1, staged key / index 8
+        "preprocess_select": ("hbm", (sc.n * (16 + 1) + Nv * (32 + 16 + 73)) / 1e9, "GB"),   # g2 + TGB lookups; written per visible Gaussian: A5a record 32, blend record 32, flag 1, staged key / index 8
         "depth_sort": ("hbm", Nv * 16 * 4 / 1e9, "GB"),
         "bin_pairs": ("alu", (nt * BIN_LANE_INSTR_PER_TEST + P * BIN_LANE_INSTR_PER_PAIR) / 1e12, "T lane-instr"),
         "sh_colour": ("hbm", Nv * (4 + 16 + 12 * K + 16) / 1e9, "GB"),

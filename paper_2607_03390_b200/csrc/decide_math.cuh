@@ -35,3 +35,13 @@ __device__ __forceinline__ bool tile_alpha_reach(float u, float v, float A, floa
   const float y0 = (float)(ty * 16u), y1 = (float)min((int)(ty * 16u + 15u), H - 1);
   return tau >= 0.0f && box_qmin(u, v, A, B, C, x0, x1, y0, y1) <= tau;
 }
+
+// Tiles [x_lo, x_hi) x [y_lo, y_hi) of the 3-sigma extent of a Gaussian at (u, v) with radius `rad` pixels (R3),
+// clipped to the TX x TY tile grid.  k_preprocess decides with it; the test-only view of the rects recomputes it from the
+// stored (u, v, rad) instead of reading a record nobody else needs.
+__device__ __forceinline__ void tile_rect(float u, float v, float rad, float TXf, float TYf, uint32_t& x_lo, uint32_t& x_hi, uint32_t& y_lo, uint32_t& y_hi) {
+  x_lo = (uint32_t)fminf(fmaxf(floorf((u - rad) / 16.0f), 0.0f), TXf);
+  x_hi = (uint32_t)fminf(fmaxf(floorf((u + rad + 15.0f) / 16.0f), 0.0f), TXf);
+  y_lo = (uint32_t)fminf(fmaxf(floorf((v - rad) / 16.0f), 0.0f), TYf);
+  y_hi = (uint32_t)fminf(fmaxf(floorf((v + rad + 15.0f) / 16.0f), 0.0f), TYf);
+}

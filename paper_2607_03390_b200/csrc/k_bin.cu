@@ -492,18 +492,26 @@ void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t 
   if (n_pairs) k_count_pairs<<<(n_pairs + 255) / 256, 256, 0, s>>>(b.vals[sorted_idx], n_pairs, b.tiles_touched);
 }
 
-// test-only: the decision records the oracle reports per Gaussian, {u, v, d, o} (which = 0) or {A, B, C, tau} (which = 1), put
-// together from what the path keeps (rec_bin {u, v, A, B | C, tau, ..}, rec_b1 {.., .., d, o}); entries of Gaussians that are
-// not visible in the current frame are stale
-__global__ void __launch_bounds__(256) k_debug_record(uint32_t n, int which, const float4* __restrict__ rec_bin, const float4* __restrict__ rec_b1,
-                                                      float4* __restrict__ out) {
+// test-only: the records the oracle reports per Gaussian, put together from what the path keeps -- rec_bin {u, v, A, B | C, tau,
+// ..}, the blend record rec_b1 {.., .., d, rad}, the scene's opacity (g2): which = 0 {u, v, d, o}, 1 {A, B, C, tau}, 2 the
+// 3-sigma rect as {x_lo | x_hi << 16, y_lo | y_hi << 16} (uint2 per Gaussian), recomputed with the function k_preprocess
+// decides with.  Entries of Gaussians that are not visible in the current frame are stale.
+__global__ void __launch_bounds__(256) k_debug_record(uint32_t n, int which, float TXf, float TYf, const float4* __restrict__ rec_bin,
+                                                      const float4* __restrict__ rec_b1, const float4* __restrict__ g2, float4* __restrict__ out) {
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
   const float4 q0 = rec_bin[2 * (size_t)g], q1 = rec_bin[2 * (size_t)g + 1], b1 = rec_b1[2 * (size_t)g];
-  out[g] = which == 0 ? make_float4(q0.x, q0.y, b1.z, b1.w) : make_float4(q0.z, q0.w, q1.x, q1.y);
+  if (which == 0) out[g] = make_float4(q0.x, q0.y, b1.z, g2[2 * (size_t)g + 1].z);
+  else if (which == 1) out[g] = make_float4(q0.z, q0.w, q1.x, q1.y);
+  else {
+    uint32_t x_lo, x_hi, y_lo, y_hi;
+    tile_rect(q0.x, q0.y, b1.w, TXf, TYf, x_lo, x_hi, y_lo, y_hi);
+    reinterpret_cast<uint2*>(out)[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
+  }
 }
-void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int which, float4* out) {
-  if (n) k_debug_record<<<(n + 255) / 256, 256, 0, s>>>(n, which, (const float4*)b.rec_bin, (const float4*)b.rec_b1, out);
+void launch_debug_record(cudaStream_t s, const FrameConst& fc, const DevBuffers& b, uint32_t n, int which, float4* out) {
+  if (n) k_debug_record<<<(n + 255) / 256, 256, 0, s>>>(n, which, (float)fc.cam.TX, (float)fc.cam.TY, (const float4*)b.rec_bin, (const float4*)b.rec_b1,
+                                                        (const float4*)b.g2, out);
 }
 
 __global__ void __launch_bounds__(256) k_debug_flags(uint32_t n, const uint8_t* __restrict__ flags, uint32_t* __restrict__ out) {

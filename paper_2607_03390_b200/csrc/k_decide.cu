@@ -244,7 +244,7 @@ struct PreSmem {
 __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, const float4* __restrict__ cull4, const float4* __restrict__ g2,
                                                                const uint8_t* __restrict__ rendered, const float2* __restrict__ warp_tgb,
                                                                const uint32_t* __restrict__ F_key,
-                                                               uint2* __restrict__ rec_rect, float4* __restrict__ rec_bin,
+                                                               float4* __restrict__ rec_bin,
                                                                uint8_t* __restrict__ rec_flags,
                                                                float4* __restrict__ rec_b0, float4* __restrict__ rec_b1,
                                                                uint32_t* __restrict__ tile_flags, uint32_t* __restrict__ nv_queue,
@@ -377,10 +377,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       const float lam = mid + sqrtf(fmaxf(0.1f, mid * mid - det));
       const float rad = ceilf(3.0f * sqrtf(lam));
       const float TXf = (float)k.TX, TYf = (float)k.TY;
-      const uint32_t x_lo = (uint32_t)fminf(fmaxf(floorf((u - rad) / 16.0f), 0.0f), TXf);
-      const uint32_t x_hi = (uint32_t)fminf(fmaxf(floorf((u + rad + 15.0f) / 16.0f), 0.0f), TXf);
-      const uint32_t y_lo = (uint32_t)fminf(fmaxf(floorf((v - rad) / 16.0f), 0.0f), TYf);
-      const uint32_t y_hi = (uint32_t)fminf(fmaxf(floorf((v + rad + 15.0f) / 16.0f), 0.0f), TYf);
+      uint32_t x_lo, x_hi, y_lo, y_hi;
+      tile_rect(u, v, rad, TXf, TYf, x_lo, x_hi, y_lo, y_hi);
       if (!(x_hi > x_lo && y_hi > y_lo)) { rec_flags[g] = (uint8_t)TGS_CULL_EMPTY; ++st_empty; continue; }
       rec_flags[g] = (uint8_t)(fl | TGS_VISIBLE);
       if (fl) ++st_nv;
@@ -406,10 +404,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_preprocess(FrameConst fc, co
       rec_bin[2 * (size_t)g + 1] = make_float4(C, tau, __uint_as_float(tx_lo | (tx_hi << 16)), __uint_as_float(ty_lo | (ty_hi << 16)));
       const uint32_t area = (tx_hi - tx_lo) * (ty_hi - ty_lo);
       st_area += area;
-      rec_rect[g] = make_uint2(x_lo | (x_hi << 16), y_lo | (y_hi << 16));
       // blend-side parameters: the quadratic form as a sum of two squares (no cancellation between its terms)
       rec_b0[2 * (size_t)g] = make_float4(u, v, -0.72134752f * A, -b / cc);        // b0 / b1 interleaved: one 32-byte sector per Gaussian, written whole
-      rec_b1[2 * (size_t)g] = make_float4(-0.72134752f / cc, log2f(opac), tz, opac);           // (.w is not read by the blend: the decision record {u, v, d, o | A, B, C, tau} the tests ask for is rec_bin + rec_b1.zw)
+      rec_b1[2 * (size_t)g] = make_float4(-0.72134752f / cc, log2f(opac), tz, rad);            // (.w is not read by the blend: it serves the test-only views -- the 3-sigma rect is tile_rect(u, v, rad), the decision record {u, v, d, o | A, B, C, tau} is rec_bin + d + the scene's opacity)
       sm.list[i] = (uint16_t)(e | 0x4000u);
       sm.depth[i] = __float_as_uint(tz);
       if (fl && tau >= 0.0f) {                                                      // A4: T^oc (L119, R18)
@@ -637,7 +634,7 @@ void launch_preprocess(cudaStream_t s, const FrameConst& fc, DevBuffers& b, int 
   const uint32_t chunks = (fc.n + PRE_CHUNK - 1) / PRE_CHUNK;
   const uint32_t grid = chunks < (uint32_t)(num_sms * 4) ? chunks : (uint32_t)(num_sms * 4);
   TGS_LAUNCH((k_preprocess), grid ? grid : 1, PRE_THREADS, 0, s, fc, b.cull4, b.g2, b.rendered, (const float2*)b.warp_tgb, b.F_key,
-                                                       b.rec_rect, b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
+                                                       b.rec_bin, b.rec_flags, b.rec_b0, b.rec_b1, b.tile_flags, b.nv_queue,
                                                        b.ckeys[1], b.cvals[1], b.pre_cnt, b.sort_hist, b.counters);
   TGS_LAUNCH((k_compact_vis), num_sms * 8, 128, 0, s, fc.n, (const uint2*)b.pre_cnt, b.ckeys[1], b.cvals[1], b.ckeys[0], b.cvals[0], b.vis_list,
              fc.dsort_fused ? b.dsort_H : (uint32_t*)nullptr, depth_sort_fused_tile_items());

@@ -379,7 +379,7 @@ static int load_gaussians_impl(tgs_ctx* c, uint32_t n, int deg, const float* mea
 #define A(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene)) return r;
 #define AZ(ptr, cnt) if (int r = dev_alloc(c, &ptr, (size_t)(cnt), c->allocs_scene, true)) return r;
   A(b.cull4, n) A(b.g2, 2 * (size_t)n) A(b.sh, (size_t)n * K * 3)
-  A(b.rec_rect, n) A(b.rec_bin, 2 * (size_t)n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, 2 * (size_t)n)
+  A(b.rec_bin, 2 * (size_t)n) A(b.rec_flags, (size_t)n + 4) A(b.rec_rgb, n) A(b.rec_b0, 2 * (size_t)n)
   b.rec_b1 = b.rec_b0 + 1;
   A(b.tiles_touched, (size_t)n + 4) A(b.area_prefix, (size_t)n + 4) A(b.rendered, (size_t)n + 4) A(b.rendered_next, (size_t)n + 4)
   A(b.pre_cnt, (size_t)n / preprocess_chunk_items() + 3) AZ(b.scan_desc, (size_t)n / scan_tile_items() + 3)
@@ -869,12 +869,11 @@ static long long debug_get_impl(tgs_ctx* c, const char* nm, void* dst, size_t by
     }
     return 16;
   }
-  else if (name == "rec_uvdo" || name == "rec_conic") {      // not stored as such: put together from rec_bin / rec_b1
+  else if (name == "rec_uvdo" || name == "rec_conic" || name == "rec_rect") {      // not stored as such: put together from rec_bin, the blend record and the scene
     if (!c->dbg_rec && N) { if (int r = dev_alloc(c, &c->dbg_rec, N, c->allocs_scene)) return r; }
-    launch_debug_record(c->stream, b, (uint32_t)N, name == "rec_conic" ? 1 : 0, c->dbg_rec);
-    src = c->dbg_rec; have = N * 16;
+    launch_debug_record(c->stream, c->fc, b, (uint32_t)N, name == "rec_uvdo" ? 0 : name == "rec_conic" ? 1 : 2, c->dbg_rec);
+    src = c->dbg_rec; have = N * (name == "rec_rect" ? 8 : 16);
   }
-  else if (name == "rec_rect") { src = b.rec_rect; have = N * 8; }
   else if (name == "rec_flags") {                            // stored as bytes, reported as words
     if (!c->dbg_rec && N) { if (int r = dev_alloc(c, &c->dbg_rec, N, c->allocs_scene)) return r; }
     launch_debug_flags(c->stream, b, (uint32_t)N, reinterpret_cast<uint32_t*>(c->dbg_rec));

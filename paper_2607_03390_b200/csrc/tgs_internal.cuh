@@ -92,7 +92,6 @@ struct DevBuffers {
   float4* g2 = nullptr;          // [N][2] {Sxx,Sxy,Sxz,Syy},{Syz,Szz,opacity,tau = 2 ln(255 o)}: read by survivors of the culls
   float* sh = nullptr;           // [N][K][3]
   // per-Gaussian records of the current frame
-  uint2* rec_rect = nullptr;     // [N] x_lo|x_hi<<16 , y_lo|y_hi<<16: tiles of the 3-sigma extent (R3)
   float4* rec_bin = nullptr;     // [N][2] {u, v, A, B}, {C, tau, bits(trect.x), bits(trect.y)}: everything A5a gathers per visible Gaussian, in ONE 32-byte sector
   uint8_t* rec_flags = nullptr;  // [N] TGS_CULL_* / TGS_VISIBLE / TGS_NEWLY_VISIBLE of the current frame (one byte; test-only reader)
   float4* rec_rgb = nullptr;     // [N] {r,g,b,-}
@@ -190,7 +189,7 @@ int launch_sort(cudaStream_t s, uint32_t* const keys[2], uint32_t* const vals[2]
                 const uint32_t* hist, uint64_t* desc, uint32_t tiles_cap, uint32_t* tickets, uint32_t* error_flag, uint32_t epoch,
                 int num_sms, bool small_input, uint2* ranges = nullptr);   // ranges: A7 fused into the last pass ({~start, end} per key)
 void launch_keys64(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n, uint64_t* out);
-void launch_debug_record(cudaStream_t s, const DevBuffers& b, uint32_t n, int which, float4* out);
+void launch_debug_record(cudaStream_t s, const FrameConst& fc, const DevBuffers& b, uint32_t n, int which, float4* out);   // test-only: {u,v,d,o} / {A,B,C,tau} / 3-sigma rect per Gaussian
 void launch_debug_flags(cudaStream_t s, const DevBuffers& b, uint32_t n, uint32_t* out);               // test-only: the flag bytes as words   // test-only: {u,v,d,o} / {A,B,C,tau} per Gaussian
 void launch_count_pairs(cudaStream_t s, DevBuffers& b, int sorted_idx, uint32_t n_pairs, uint32_t n);   // test-only
 void launch_ranges_decode(cudaStream_t s, const DevBuffers& b, int n_tiles, uint2* out);   // test-only: {~start, end} -> {start, end}
