@@ -174,7 +174,8 @@ const char* tgs_last_error(tgs_ctx*);
 
 /* ---- test-only: named intermediate buffers, so that a stage can be fed the oracle's inputs ----
  * tgs_debug_get copies min(bytes, size) bytes and returns the buffer's size in bytes (>= 0) or an error.
- * Readable: rec_uvdo rec_conic (float4 [N]) rec_rect (uint16x4 [N]) rec_flags (uint32 [N]) rec_rgb
+ * Readable (rec_uvdo, rec_conic, rec_rect and rec_flags are views assembled on request from what the path keeps per Gaussian,
+ *   not buffers it writes as such): rec_uvdo rec_conic (float4 [N]) rec_rect (uint16x4 [N]) rec_flags (uint32 [N]) rec_rgb
  *   (float4 [N]) tiles_touched (uint32 [N]) keys (uint64 [P]) vals (uint32 [P]) ranges (uint32 [T][2]) -- with more than one
  *   slab (tgs_params.depth_slabs) these four describe the LAST slab only; the parity tests of the lists use depth_slabs = 1 --
  *   warp_depth warp_sigma fill_depth (float [H][W]) rendered (uint8 [N]) F (float[4]) prior_depth
